@@ -1,0 +1,167 @@
+/*
+ * wri.h — C ABI of libwri: batched LSQR on the data-augmented Helmholtz system of
+ * 3D wavefield reconstruction inversion, hand-written CUDA for sm_100a (B200).
+ *
+ *   min_u || lambda (A(m) u - q) ||^2 + || P u - d ||^2          (eq. 4-6,
+ *                                                                 source weight fixed: q = alpha e)
+ *   A(m) = Laplacian_h + omega^2 diag(m) (1 + i gamma)            (2nd-order 7-point
+ *                                                                 stencil + gamma sponge per
+ *                                                                 BASELINE.json north_star)
+ *   M = [lambda A ; P],  M^H = [lambda A^H , P^T],  P = sampling of receiver nodes
+ *   solver: LSQR (Paige & Saunders 1982; "Algorithm 1"), batched over
+ *   sources / frequencies ("grouping", eq. 12) with per-column scalars,
+ *   tolerance and active mask.
+ *
+ * Conventions
+ *   cell index       c = (iz*ny + iy)*nx + ix          (x fastest, z = depth), n_g = nx*ny*nz
+ *   batched vectors  complex64 (float re, float im), source-interleaved: element (c, s) at
+ *                    index c*nb + s, s = batch column; "c64 [n_g][nb]" below
+ *   pointers         *_dev  = device memory on the context's GPU, 16-byte aligned;
+ *                    *_host = host memory.  Nothing is a torch type.
+ *   ownership        the caller owns every buffer it passes, including the workspace; the
+ *                    library owns only the opaque context and a few KB of device scalars.
+ *                    Inputs are never written.  Outputs must not alias inputs.
+ *   execution        all work is enqueued on the CUDA stream given at wri_create; calls return
+ *                    after enqueue (the *_host entry synchronises the stream before returning).
+ *   errors           int return, 0 = WRI_OK, negative = error (table below); no exceptions,
+ *                    no exit().  Numerical breakdown (b = 0, beta = 0, alpha = 0) is not an
+ *                    error: the column stops (reading C-7).
+ *   no CPU fallback  every entry that computes needs a CUDA device and fails with
+ *                    WRI_ERR_CUDA without one.
+ */
+#ifndef WRI_H_
+#define WRI_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define WRI_OK                    0
+#define WRI_ERR_ARG              -1   /* null pointer, non-positive size, nb > nb_max, misaligned  */
+#define WRI_ERR_RECEIVER_RANGE   -2   /* a receiver node lies outside the grid                     */
+#define WRI_ERR_RECEIVER_DUP     -3   /* two receivers on one node (P^T must be a pure scatter)    */
+#define WRI_ERR_WORKSPACE        -4   /* workspace missing or too small                            */
+#define WRI_ERR_CUDA             -5   /* CUDA runtime error; text via wri_strerror                 */
+#define WRI_ERR_STATE            -6   /* call out of order (e.g. iterate before begin)             */
+
+typedef struct wri_ctx wri_ctx;                 /* opaque, library-owned */
+
+typedef struct { int32_t nx, ny, nz; } wri_grid;
+
+/* Sponge: gamma(ix,iy,iz) = gamma_max * ( max(dx,dy,dz) / width )^power,
+ * d_axis(i) = max(width - i, i - (n_axis-1-width), 0) on the listed faces (reading C-4).   */
+typedef struct {
+    int32_t  width;       /* cells; 0 = no sponge                                   */
+    float    gamma_max;   /* 1.0 in BASELINE.json configs                            */
+    int32_t  power;       /* 2 = quadratic                                           */
+    uint32_t faces;       /* bit0..5 = x-,x+,y-,y+,z-,z+ ; 0x3F = all six            */
+} wri_sponge;
+
+/* wri_create — build a context for one grid / model / receiver set (north_star:
+ * "wri_create(grid,h,omega,m,sponge,receivers)").
+ *   omega_host   [n_omega] angular frequencies (rad/s); a batch column picks one by index
+ *   m_dev        [n_g] float32 squared slowness (s^2/m^2), BORROWED until wri_set_model/destroy
+ *   rec_ijk_host [n_rec][3] = (ix,iy,iz) receiver nodes; validated before any CUDA call:
+ *                out of range -> WRI_ERR_RECEIVER_RANGE, duplicates -> WRI_ERR_RECEIVER_DUP
+ *   nb_max       largest batch width later calls may use
+ *   cuda_stream  cudaStream_t (NULL = default stream)                                        */
+int wri_create(wri_ctx** out, wri_grid grid, double h,
+               int32_t n_omega, const double* omega_host,
+               const float* m_dev, wri_sponge sponge,
+               int32_t n_rec, const int32_t* rec_ijk_host,
+               int32_t nb_max, void* cuda_stream);
+
+/* m changes every outer iteration of the inversion (Algorithm 2). */
+int wri_set_model(wri_ctx* ctx, const float* m_dev);
+
+/* Workspace for wri_lsqr_* at batch width nb (u, v, w vectors, receiver rows, reduction
+ * partials).  host_staging != 0 adds room for the device copies wri_lsqr_batch_host needs.
+ * The caller allocates (e.g. a torch uint8 tensor) and hands it over; it must stay alive and
+ * untouched while a solve is in flight.                                                      */
+size_t wri_workspace_bytes(const wri_ctx* ctx, int32_t nb, int32_t host_staging);
+int    wri_set_workspace(wri_ctx* ctx, void* ws_dev, size_t bytes);
+
+/* y = M x: ytop = lambda * A x  (c64 [n_g][nb]),  ybot = x at the receiver
+ * nodes (c64 [n_rec][nb], exact copies).  omega_idx_host [nb] (NULL = all 0).  No workspace. */
+int wri_apply_M(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_host, float lambda,
+                const void* x_dev, void* ytop_dev, void* ybot_dev);
+
+/* x = M^H y = lambda * A^H ytop + P^T ybot  (conjugate transpose, reading C-2). */
+int wri_apply_MH(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_host, float lambda,
+                 const void* ytop_dev, const void* ybot_dev, void* x_dev);
+
+/* wri_lsqr_batch — nb independent LSQR solves in lock-step, b_s = [lambda q_s ; d_s], x0 = 0.
+ *   q_dev        c64 [n_g][nb]     d_dev  c64 [n_rec][nb]
+ *   tol_dev      float [nb] or NULL; column s stops at the first k with
+ *                ||M^H r_k|| / ||M^H b|| <= tol_s  (LSQR's running estimate, reading C-6);
+ *                tol_s <= 0 (or NULL) runs exactly maxit iterations
+ *   u_out_dev    c64 [n_g][nb]     the wavefields x_k at each column's stop iteration
+ *   resnorms_dev float [maxit+1][nb]: ||b - M x_k|| for k = 0..maxit, held at the last value
+ *                after a column stops (reading C-9)
+ *   iters_dev    int32 [nb] iterations performed per column (may be NULL)
+ * Equivalent to wri_lsqr_begin + wri_lsqr_iterate(maxit) + wri_lsqr_end.  Needs a workspace.  */
+int wri_lsqr_batch(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_host,
+                   const void* q_dev, const void* d_dev, float lambda,
+                   const float* tol_dev, int32_t maxit,
+                   void* u_out_dev, float* resnorms_dev, int32_t* iters_dev);
+
+/* Same solve with HOST buffers: copies q, d (and tol) to the device, solves, copies u_out,
+ * resnorms and iters back, then synchronises the stream.  Needs a workspace sized with
+ * host_staging = 1.  Pinned host memory makes the copies asynchronous but is not required.   */
+int wri_lsqr_batch_host(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_host,
+                        const void* q_host, const void* d_host, float lambda,
+                        const float* tol_host, int32_t maxit,
+                        void* u_out_host, float* resnorms_host, int32_t* iters_host);
+
+/* Stepping form of the same solve (outer drivers, teacher-forced parity tests).
+ *   begin   : Golub-Kahan start  beta1 u1 = b, alpha1 v1 = M^H u1, w1 = v1, x0 = 0
+ *   iterate : n_steps more iterations (total must not exceed maxit)
+ *   end     : applies the last deferred x update; u_out/resnorms/iters are final afterwards  */
+int wri_lsqr_begin(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_host,
+                   const void* q_dev, const void* d_dev, float lambda,
+                   const float* tol_dev, int32_t maxit,
+                   void* u_out_dev, float* resnorms_dev, int32_t* iters_dev);
+int wri_lsqr_iterate(wri_ctx* ctx, int32_t n_steps);
+int wri_lsqr_end(wri_ctx* ctx);
+
+/* Device-side LSQR state between wri_lsqr_iterate calls (valid after the stream is synced).
+ * The vectors are stored UN-normalised (lazy normalisation):
+ *   after k iterations: u_{k+1} = U / beta, v_{k+1} = V / alpha, W = w_k, X = x_{k-1}; the
+ *   updates x_k = X + cx * W and w_{k+1} = V/alpha - cw * W are applied by the next iteration
+ *   (x_k also by wri_lsqr_end).
+ * Pointers are into the caller's workspace / u_out buffer and the context's scalar block.    */
+typedef struct {
+    int32_t nb, k;                   /* batch width, iterations enqueued so far               */
+    const void*   U_top;             /* c64 [n_g][nb]                                          */
+    const void*   U_bot;             /* c64 [n_rec][nb]                                        */
+    const void*   V;                 /* c64 [n_g][nb]                                          */
+    const void*   W;                 /* c64 [n_g][nb]                                          */
+    const void*   X;                 /* c64 [n_g][nb] (= u_out_dev)                            */
+    const double* alpha;             /* [nb] each, device                                      */
+    const double* beta;
+    const double* rhobar;
+    const double* phibar;
+    const double* ar0;               /* alpha1 * beta1                                         */
+    const float*  cx;                /* [nb] pending x-update coefficient phi_k/rho_k          */
+    const float*  cw;                /* [nb] pending w-update coefficient theta_{k+1}/rho_k:   */
+                                     /*      w_{k+1} = V/alpha - cw * W                        */
+    const int32_t* active;           /* [nb] 1 while the column iterates                       */
+    const int32_t* iters;            /* [nb]                                                   */
+} wri_lsqr_view;
+int wri_lsqr_peek(const wri_ctx* ctx, wri_lsqr_view* view);
+
+/* Kernels launched by this context since creation (bench.py's gpu_launches). */
+int64_t wri_launch_count(const wri_ctx* ctx);
+
+int wri_destroy(wri_ctx* ctx);
+
+/* Static text for an error code; for WRI_ERR_CUDA the last CUDA error string seen. */
+const char* wri_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WRI_H_ */

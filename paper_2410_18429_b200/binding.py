@@ -1,0 +1,268 @@
+"""ctypes binding of libwri.so — same names as include/wri.h, marshalling only."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+class WriError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("libwri error %d: %s" % (code, msg))
+        self.code = code
+
+
+class wri_grid(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32)]
+
+
+class wri_sponge(C.Structure):
+    _fields_ = [("width", C.c_int32), ("gamma_max", C.c_float), ("power", C.c_int32),
+                ("faces", C.c_uint32)]
+
+
+class wri_lsqr_view(C.Structure):
+    _fields_ = [("nb", C.c_int32), ("k", C.c_int32),
+                ("U_top", C.c_void_p), ("U_bot", C.c_void_p), ("V", C.c_void_p),
+                ("W", C.c_void_p), ("X", C.c_void_p),
+                ("alpha", C.c_void_p), ("beta", C.c_void_p), ("rhobar", C.c_void_p),
+                ("phibar", C.c_void_p), ("ar0", C.c_void_p), ("cx", C.c_void_p), ("cw", C.c_void_p),
+                ("active", C.c_void_p), ("iters", C.c_void_p)]
+
+
+WRI_OK = 0
+WRI_ERR_ARG = -1
+WRI_ERR_RECEIVER_RANGE = -2
+WRI_ERR_RECEIVER_DUP = -3
+WRI_ERR_WORKSPACE = -4
+WRI_ERR_CUDA = -5
+WRI_ERR_STATE = -6
+
+_lib = None
+
+
+def lib_path() -> str:
+    return os.path.join(_HERE, "libwri.so")
+
+
+def load_library():
+    """Load libwri.so (must have been built: python -m paper_2410_18429_b200.build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = lib_path()
+    if not os.path.exists(path):
+        raise WriError(WRI_ERR_CUDA, "libwri.so is not built (run python -m paper_2410_18429_b200.build); "
+                                     "there is no CPU fallback")
+    lib = C.CDLL(path)
+    P, I32, F32, F64 = C.c_void_p, C.c_int32, C.c_float, C.c_double
+    lib.wri_create.argtypes = [C.POINTER(P), wri_grid, F64, I32, P, P, wri_sponge, I32, P, I32, P]
+    lib.wri_set_model.argtypes = [P, P]
+    lib.wri_workspace_bytes.argtypes = [P, I32, I32]
+    lib.wri_workspace_bytes.restype = C.c_size_t
+    lib.wri_set_workspace.argtypes = [P, P, C.c_size_t]
+    lib.wri_apply_M.argtypes = [P, I32, P, F32, P, P, P]
+    lib.wri_apply_MH.argtypes = [P, I32, P, F32, P, P, P]
+    solve = [P, I32, P, P, P, F32, P, I32, P, P, P]
+    lib.wri_lsqr_batch.argtypes = solve
+    lib.wri_lsqr_batch_host.argtypes = solve
+    lib.wri_lsqr_begin.argtypes = solve
+    lib.wri_lsqr_iterate.argtypes = [P, I32]
+    lib.wri_lsqr_end.argtypes = [P]
+    lib.wri_lsqr_peek.argtypes = [P, C.POINTER(wri_lsqr_view)]
+    lib.wri_launch_count.argtypes = [P]
+    lib.wri_launch_count.restype = C.c_int64
+    lib.wri_destroy.argtypes = [P]
+    lib.wri_strerror.argtypes = [C.c_int]
+    lib.wri_strerror.restype = C.c_char_p
+    _lib = lib
+    return lib
+
+
+def _ck(code):
+    if code != WRI_OK:
+        raise WriError(code, load_library().wri_strerror(code).decode())
+
+
+def _dptr(t):
+    return C.c_void_p(t.data_ptr()) if t is not None else None
+
+
+def _i32(a):
+    if a is None:
+        return None, None
+    a = np.ascontiguousarray(a, dtype=np.int32)
+    return a, a.ctypes.data_as(C.c_void_p)
+
+
+class Wri:
+    """One wri_ctx: grid + model + receivers on the current CUDA device and stream.
+
+    Tensors are torch CUDA tensors: m float32 [n_g]; batched vectors complex64 [n_g, nb]
+    (source-interleaved), receiver rows complex64 [n_rec, nb].
+    """
+
+    def __init__(self, grid, h, omegas, m, sponge_width, rec_ijk, nb_max, gamma_max=1.0, power=2,
+                 faces=0x3F, stream=None):
+        import torch
+        lib = load_library()
+        self._torch = torch
+        self.nx, self.ny, self.nz = (int(g) for g in grid)
+        self.ng = self.nx * self.ny * self.nz
+        self.nb_max = int(nb_max)
+        om = np.ascontiguousarray(omegas, dtype=np.float64)
+        rec = np.ascontiguousarray(rec_ijk, dtype=np.int32).reshape(-1, 3)
+        self.n_rec = rec.shape[0]
+        self.m = m
+        self._ws = None
+        self._keep = []
+        if stream is None and torch.cuda.is_available():
+            stream = torch.cuda.current_stream().cuda_stream
+        h_ctx = C.c_void_p()
+        _ck(lib.wri_create(C.byref(h_ctx), wri_grid(self.nx, self.ny, self.nz), float(h), om.size,
+                           om.ctypes.data_as(C.c_void_p), _dptr(m),
+                           wri_sponge(int(sponge_width), float(gamma_max), int(power), int(faces)),
+                           self.n_rec, rec.ctypes.data_as(C.c_void_p) if self.n_rec else None,
+                           self.nb_max, C.c_void_p(stream or 0)))
+        self._h = h_ctx
+        self._lib = lib
+
+    @classmethod
+    def from_workload(cls, w, device="cuda", nb_max=None):
+        import torch
+        m = torch.from_numpy(w.m).to(device)
+        return cls((w.nx, w.ny, w.nz), w.h, w.omegas, m, w.sponge_width, w.rec_ijk,
+                   nb_max or w.nb, gamma_max=w.gamma_max, power=w.power, faces=w.faces)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.wri_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- workspace
+    def workspace_bytes(self, nb, host_staging=False):
+        return int(self._lib.wri_workspace_bytes(self._h, int(nb), int(bool(host_staging))))
+
+    def ensure_workspace(self, nb, host_staging=False):
+        need = self.workspace_bytes(nb, host_staging)
+        if self._ws is None or self._ws.numel() < need:
+            self._ws = None
+            self._ws = self._torch.empty(need, dtype=self._torch.uint8, device=self.m.device)
+            _ck(self._lib.wri_set_workspace(self._h, _dptr(self._ws), self._ws.numel()))
+        return self._ws
+
+    def set_model(self, m):
+        self.m = m
+        _ck(self._lib.wri_set_model(self._h, _dptr(m)))
+
+    # ---- operator
+    def apply_M(self, x, lam, omega_idx=None):
+        t = self._torch
+        nb = x.shape[1]
+        ytop = t.empty_like(x)
+        ybot = t.empty((self.n_rec, nb), dtype=t.complex64, device=x.device)
+        keep, oi = _i32(omega_idx)
+        _ck(self._lib.wri_apply_M(self._h, nb, oi, float(lam), _dptr(x), _dptr(ytop), _dptr(ybot)))
+        return ytop, ybot
+
+    def apply_MH(self, ytop, ybot, lam, omega_idx=None):
+        t = self._torch
+        nb = ytop.shape[1]
+        x = t.empty_like(ytop)
+        keep, oi = _i32(omega_idx)
+        _ck(self._lib.wri_apply_MH(self._h, nb, oi, float(lam), _dptr(ytop), _dptr(ybot), _dptr(x)))
+        return x
+
+    # ---- solver
+    def _outputs(self, nb, maxit, device):
+        t = self._torch
+        u = t.empty((self.ng, nb), dtype=t.complex64, device=device)
+        res = t.empty((maxit + 1, nb), dtype=t.float32, device=device)
+        it = t.empty(nb, dtype=t.int32, device=device)
+        return u, res, it
+
+    def lsqr_batch(self, q, d, lam, tol=None, maxit=50, omega_idx=None, out=None):
+        nb = q.shape[1]
+        self.ensure_workspace(nb)
+        u, res, it = out if out is not None else self._outputs(nb, maxit, q.device)
+        keep, oi = _i32(omega_idx)
+        _ck(self._lib.wri_lsqr_batch(self._h, nb, oi, _dptr(q), _dptr(d), float(lam), _dptr(tol),
+                                     int(maxit), _dptr(u), _dptr(res), _dptr(it)))
+        return u, res, it
+
+    def lsqr_batch_host(self, q, d, lam, tol=None, maxit=50, omega_idx=None, out=None):
+        """Host-buffer entry: q, d, tol and the outputs are CPU tensors (pinned for speed)."""
+        t = self._torch
+        nb = q.shape[1]
+        self.ensure_workspace(nb, host_staging=True)
+        if out is None:
+            out = (t.empty((self.ng, nb), dtype=t.complex64).pin_memory(),
+                   t.empty((maxit + 1, nb), dtype=t.float32).pin_memory(),
+                   t.empty(nb, dtype=t.int32).pin_memory())
+        u, res, it = out
+        keep, oi = _i32(omega_idx)
+        _ck(self._lib.wri_lsqr_batch_host(self._h, nb, oi, _dptr(q), _dptr(d), float(lam), _dptr(tol),
+                                          int(maxit), _dptr(u), _dptr(res), _dptr(it)))
+        return u, res, it
+
+    def lsqr_begin(self, q, d, lam, tol=None, maxit=50, omega_idx=None):
+        nb = q.shape[1]
+        self.ensure_workspace(nb)
+        u, res, it = self._outputs(nb, maxit, q.device)
+        keep, oi = _i32(omega_idx)
+        self._keep = [q, d, tol, u, res, it]
+        _ck(self._lib.wri_lsqr_begin(self._h, nb, oi, _dptr(q), _dptr(d), float(lam), _dptr(tol),
+                                     int(maxit), _dptr(u), _dptr(res), _dptr(it)))
+        return u, res, it
+
+    def lsqr_iterate(self, n_steps=1):
+        _ck(self._lib.wri_lsqr_iterate(self._h, int(n_steps)))
+
+    def lsqr_end(self):
+        _ck(self._lib.wri_lsqr_end(self._h))
+
+    def lsqr_peek(self):
+        """Copies of the device LSQR state as numpy arrays (synchronises)."""
+        t = self._torch
+        v = wri_lsqr_view()
+        _ck(self._lib.wri_lsqr_peek(self._h, C.byref(v)))
+        t.cuda.synchronize()
+        nb = v.nb
+
+        def grab(ptr, shape, dtype):
+            typestr = {np.complex64: "<c8", np.float64: "<f8", np.float32: "<f4", np.int32: "<i4"}[dtype]
+            view = t.as_tensor(_DevArray(ptr, tuple(int(x) for x in shape), typestr), device=self.m.device)
+            return view.clone().cpu().numpy()
+
+        out = {"nb": nb, "k": v.k}
+        for name in ("U_top", "V", "W", "X"):
+            out[name] = grab(getattr(v, name), (self.ng, nb), np.complex64)
+        out["U_bot"] = grab(v.U_bot, (self.n_rec, nb), np.complex64) if self.n_rec else \
+            np.zeros((0, nb), np.complex64)
+        for name in ("alpha", "beta", "rhobar", "phibar", "ar0"):
+            out[name] = grab(getattr(v, name), (nb,), np.float64)
+        out["cx"] = grab(v.cx, (nb,), np.float32)
+        out["cw"] = grab(v.cw, (nb,), np.float32)
+        out["active"] = grab(v.active, (nb,), np.int32)
+        out["iters"] = grab(v.iters, (nb,), np.int32)
+        return out
+
+    def launch_count(self):
+        return int(self._lib.wri_launch_count(self._h))
+
+
+class _DevArray:
+    """Raw device pointer exposed through __cuda_array_interface__ (read-only view for torch)."""
+
+    def __init__(self, ptr, shape, typestr):
+        self.__cuda_array_interface__ = {"data": (int(ptr), False), "shape": shape,
+                                         "typestr": typestr, "version": 2}

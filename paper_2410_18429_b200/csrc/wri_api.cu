@@ -1,0 +1,493 @@
+// wri_api.cu — C ABI of libwri (include/wri.h): context, validation, launch sequencing.
+// All arithmetic of the path runs in the kernels of wri_kernels.cuh; there is no CPU fallback.
+#include "../../include/wri.h"
+#include "wri_kernels.cuh"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <vector>
+
+using namespace wri;
+
+namespace {
+
+thread_local char g_cuda_msg[256] = "no CUDA error recorded";
+
+int cuda_fail(cudaError_t e, const char* what) {
+    snprintf(g_cuda_msg, sizeof g_cuda_msg, "CUDA error in %s: %s", what, cudaGetErrorString(e));
+    return WRI_ERR_CUDA;
+}
+#define CK(call)                                                   \
+    do {                                                           \
+        cudaError_t e__ = (call);                                  \
+        if (e__ != cudaSuccess) return cuda_fail(e__, #call);      \
+    } while (0)
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+struct Tiling {
+    int vec;            // complex numbers per thread (2 = 128-bit accesses)
+    dim3 block, grid;
+    int zc;
+    size_t n_tiles;
+};
+
+}  // namespace
+
+struct wri_ctx {
+    wri_grid g{};
+    double h = 0;
+    size_t ng = 0;
+    std::vector<double> omega;
+    wri_sponge sponge{};
+    int n_rec = 0, nb_max = 0;
+    cudaStream_t stream = nullptr;
+    const float* m = nullptr;
+    // library-owned device memory
+    float* gtab = nullptr;       // gx | gy | gz
+    int* rec = nullptr;          // [n_rec] cell indices
+    float* coef = nullptr;       // [N_COEF][nb_max]
+    double* stat = nullptr;      // [N_STAT][nb_max]
+    int* active = nullptr;       // [nb_max]
+    int* iters = nullptr;        // [nb_max]
+    // caller's workspace
+    char* ws = nullptr;
+    size_t ws_bytes = 0;
+    // solve in flight
+    bool solving = false;
+    int nb = 0, k = 0, maxit = 0;
+    float lambda = 0;
+    float2 *U = nullptr, *V = nullptr, *W = nullptr, *X = nullptr, *U_bot = nullptr;
+    double* partials = nullptr;
+    const float* tol = nullptr;
+    float* resnorms = nullptr;
+    int* iters_out = nullptr;
+    Tiling tl{};
+    int64_t launches = 0;
+};
+
+namespace {
+
+// Tile shape for batch width nb: threads span the (ix, s) row first, then y; blocks march zc planes.
+Tiling make_tiling(const wri_ctx* c, int nb) {
+    Tiling t;
+    t.vec = (nb % 2 == 0) ? 2 : 1;
+    const long long items = (long long)c->g.nx * nb / t.vec;       // per x-row
+    int tx = 128;
+    while (tx > 32 && tx / 2 >= items) tx /= 2;
+    int ty = 256 / tx;
+    while (ty > 1 && ty / 2 >= c->g.ny) ty /= 2;
+    t.block = dim3(tx, ty, 1);
+    const unsigned gx = (unsigned)((items + tx - 1) / tx);
+    const unsigned gy = (unsigned)((c->g.ny + ty - 1) / ty);
+    // planes per tile: enough tiles for >= ~16 waves of 148 SMs x 4 blocks, but at least 8 planes
+    int zc = c->g.nz;
+    const long long want = 148LL * 4 * 16;
+    while (zc > 8 && (long long)gx * gy * ((c->g.nz + zc - 1) / zc) < want) zc = (zc + 1) / 2;
+    t.zc = zc;
+    const unsigned gz = (unsigned)((c->g.nz + zc - 1) / zc);
+    t.grid = dim3(gx, gy, gz);
+    t.n_tiles = (size_t)gx * gy * gz;
+    return t;
+}
+
+struct WsLayout {
+    size_t U, V, W, U_bot, partials, Xs, Ds, tols, res, its, total;
+};
+WsLayout ws_layout(const wri_ctx* c, int nb, int host_staging, int maxit_cap) {
+    WsLayout L{};
+    const size_t vec = align_up(c->ng * (size_t)nb * sizeof(float2), 256);
+    const size_t bot = align_up((size_t)std::max(c->n_rec, 1) * nb * sizeof(float2), 256);
+    const Tiling t = make_tiling(c, nb);
+    size_t o = 0;
+    L.U = o; o += vec;
+    L.V = o; o += vec;
+    L.W = o; o += vec;
+    L.U_bot = o; o += bot;
+    L.partials = o; o += align_up(t.n_tiles * nb * sizeof(double), 256);
+    if (host_staging) {
+        L.Xs = o; o += vec;
+        L.Ds = o; o += bot;
+        L.tols = o; o += align_up((size_t)nb * sizeof(float), 256);
+        L.res = o; o += align_up((size_t)(maxit_cap + 1) * nb * sizeof(float), 256);
+        L.its = o; o += align_up((size_t)nb * sizeof(int), 256);
+    }
+    L.total = o;
+    return L;
+}
+constexpr int kHostMaxitCap = 4096;   // resnorm staging rows reserved for wri_lsqr_batch_host
+
+int upload_columns(wri_ctx* c, int nb, const int32_t* omega_idx, float lambda) {
+    std::vector<float> w2(nb), one(nb, 1.f), lam(nb, lambda);
+    for (int s = 0; s < nb; ++s) {
+        const int j = omega_idx ? omega_idx[s] : 0;
+        if (j < 0 || j >= (int)c->omega.size()) return WRI_ERR_ARG;
+        w2[s] = (float)(c->omega[j] * c->omega[j]);
+    }
+    const size_t NM = c->nb_max;
+    CK(cudaMemcpyAsync(c->coef + C_W2 * NM, w2.data(), nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(c->coef + C_ONE * NM, one.data(), nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(c->coef + C_LAM * NM, lam.data(), nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    return WRI_OK;
+}
+
+PassParams base_params(const wri_ctx* c, int nb, const Tiling& t) {
+    PassParams p{};
+    p.m = c->m;
+    p.gx = c->gtab;
+    p.gy = c->gtab + c->g.nx;
+    p.gz = c->gtab + c->g.nx + c->g.ny;
+    p.w2 = c->coef + C_W2 * (size_t)c->nb_max;
+    p.nx = c->g.nx; p.ny = c->g.ny; p.nz = c->g.nz; p.nb = nb;
+    p.zc = t.zc;
+    p.ih2 = (float)(1.0 / (c->h * c->h));
+    p.m6ih2 = (float)(-6.0 / (c->h * c->h));
+    p.sgn = 1.f;
+    return p;
+}
+
+template <int MODE>
+int launch_pass(wri_ctx* c, const PassParams& p, const Tiling& t) {
+    const size_t smem = (MODE == MODE_APPLY) ? 0 : (size_t)t.block.x * t.block.y * t.vec * sizeof(double);
+    if (t.vec == 2) k_pass<2, MODE><<<t.grid, t.block, smem, c->stream>>>(p);
+    else            k_pass<1, MODE><<<t.grid, t.block, smem, c->stream>>>(p);
+    c->launches++;
+    CK(cudaGetLastError());
+    return WRI_OK;
+}
+
+template <int PHASE>
+int launch_scalars(wri_ctx* c, const float2* d) {
+    ScalParams s{};
+    s.partials = c->partials;
+    s.n_tiles = (int)c->tl.n_tiles;
+    s.nb = c->nb; s.nb_max = c->nb_max;
+    s.n_rec = c->n_rec; s.rec = c->rec;
+    s.V = c->V; s.U_bot = c->U_bot; s.d = d;
+    s.coef = c->coef; s.stat = c->stat; s.active = c->active; s.iters = c->iters;
+    s.tol = c->tol; s.resnorms = c->resnorms; s.iters_out = c->iters_out;
+    s.k = c->k; s.maxit = c->maxit; s.lambda = c->lambda;
+    const int T = 1024;
+    const size_t smem = (size_t)(T + c->nb) * sizeof(double);
+    k_scalars<PHASE><<<1, T, smem, c->stream>>>(s);
+    c->launches++;
+    CK(cudaGetLastError());
+    return WRI_OK;
+}
+
+int check_batch_args(const wri_ctx* c, int nb) {
+    if (!c) return WRI_ERR_ARG;
+    if (nb <= 0 || nb > c->nb_max) return WRI_ERR_ARG;
+    if ((long long)c->ng * nb > 0x7fffffffLL * 1LL) return WRI_ERR_ARG;   // element indices stay below 2^31
+    return WRI_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* wri_strerror(int code) {
+    switch (code) {
+        case WRI_OK: return "ok";
+        case WRI_ERR_ARG: return "invalid argument (null pointer, bad size, nb > nb_max, or misaligned buffer)";
+        case WRI_ERR_RECEIVER_RANGE: return "receiver node outside the grid";
+        case WRI_ERR_RECEIVER_DUP: return "duplicate receiver node";
+        case WRI_ERR_WORKSPACE: return "workspace missing or too small";
+        case WRI_ERR_CUDA: return g_cuda_msg;
+        case WRI_ERR_STATE: return "call out of order";
+        default: return "unknown error code";
+    }
+}
+
+int wri_create(wri_ctx** out, wri_grid grid, double h, int32_t n_omega, const double* omega_host,
+               const float* m_dev, wri_sponge sponge, int32_t n_rec, const int32_t* rec_ijk_host,
+               int32_t nb_max, void* cuda_stream) {
+    if (!out) return WRI_ERR_ARG;
+    *out = nullptr;
+    if (grid.nx <= 0 || grid.ny <= 0 || grid.nz <= 0 || !(h > 0.0) || n_omega <= 0 || !omega_host ||
+        !m_dev || n_rec < 0 || (n_rec > 0 && !rec_ijk_host) || nb_max <= 0 || sponge.width < 0 ||
+        sponge.power < 0)
+        return WRI_ERR_ARG;
+    const size_t ng = (size_t)grid.nx * grid.ny * grid.nz;
+    if (ng > 0x7fffffffULL) return WRI_ERR_ARG;
+    // receivers: validated on the host before any CUDA call (reading C-8)
+    std::vector<int> cells(n_rec);
+    for (int r = 0; r < n_rec; ++r) {
+        const int ix = rec_ijk_host[3 * r], iy = rec_ijk_host[3 * r + 1], iz = rec_ijk_host[3 * r + 2];
+        if (ix < 0 || ix >= grid.nx || iy < 0 || iy >= grid.ny || iz < 0 || iz >= grid.nz)
+            return WRI_ERR_RECEIVER_RANGE;
+        cells[r] = (iz * grid.ny + iy) * grid.nx + ix;
+    }
+    {
+        std::vector<int> sorted(cells);
+        std::sort(sorted.begin(), sorted.end());
+        if (std::adjacent_find(sorted.begin(), sorted.end()) != sorted.end()) return WRI_ERR_RECEIVER_DUP;
+    }
+    int ndev = 0;
+    CK(cudaGetDeviceCount(&ndev));
+    if (ndev <= 0) return cuda_fail(cudaErrorNoDevice, "wri_create");
+
+    wri_ctx* c = new wri_ctx();
+    c->g = grid; c->h = h; c->ng = ng;
+    c->omega.assign(omega_host, omega_host + n_omega);
+    c->sponge = sponge; c->n_rec = n_rec; c->nb_max = nb_max;
+    c->stream = (cudaStream_t)cuda_stream;
+    c->m = m_dev;
+
+    // sponge profile per axis, computed in double and rounded once; gamma = max over axes
+    const int L = sponge.width;
+    std::vector<float> gt((size_t)grid.nx + grid.ny + grid.nz, 0.f);
+    auto fill = [&](float* dst, int n, bool lo, bool hi) {
+        for (int i = 0; i < n; ++i) {
+            double d = 0.0;
+            if (L > 0) {
+                if (lo) d = std::max(d, (double)(L - i));
+                if (hi) d = std::max(d, (double)(i - (n - 1 - L)));
+                dst[i] = (float)((double)sponge.gamma_max * std::pow(d / (double)L, (double)sponge.power));
+                if (d == 0.0) dst[i] = 0.f;
+            }
+        }
+    };
+    fill(gt.data(), grid.nx, sponge.faces & 1u, sponge.faces & 2u);
+    fill(gt.data() + grid.nx, grid.ny, sponge.faces & 4u, sponge.faces & 8u);
+    fill(gt.data() + grid.nx + grid.ny, grid.nz, sponge.faces & 16u, sponge.faces & 32u);
+
+    auto fail = [&](int code) { wri_destroy(c); return code; };
+#define CKC(call)                                                          \
+    do {                                                                   \
+        cudaError_t e__ = (call);                                          \
+        if (e__ != cudaSuccess) return fail(cuda_fail(e__, #call));        \
+    } while (0)
+    CKC(cudaMalloc(&c->gtab, gt.size() * sizeof(float)));
+    CKC(cudaMemcpy(c->gtab, gt.data(), gt.size() * sizeof(float), cudaMemcpyHostToDevice));
+    CKC(cudaMalloc(&c->rec, std::max(n_rec, 1) * sizeof(int)));
+    if (n_rec) CKC(cudaMemcpy(c->rec, cells.data(), n_rec * sizeof(int), cudaMemcpyHostToDevice));
+    CKC(cudaMalloc(&c->coef, (size_t)N_COEF * nb_max * sizeof(float)));
+    CKC(cudaMemset(c->coef, 0, (size_t)N_COEF * nb_max * sizeof(float)));
+    CKC(cudaMalloc(&c->stat, (size_t)N_STAT * nb_max * sizeof(double)));
+    CKC(cudaMemset(c->stat, 0, (size_t)N_STAT * nb_max * sizeof(double)));
+    CKC(cudaMalloc(&c->active, nb_max * sizeof(int)));
+    CKC(cudaMalloc(&c->iters, nb_max * sizeof(int)));
+    CKC(cudaMemset(c->active, 0, nb_max * sizeof(int)));
+    CKC(cudaMemset(c->iters, 0, nb_max * sizeof(int)));
+#undef CKC
+    *out = c;
+    return WRI_OK;
+}
+
+int wri_destroy(wri_ctx* c) {
+    if (!c) return WRI_OK;
+    cudaFree(c->gtab); cudaFree(c->rec); cudaFree(c->coef); cudaFree(c->stat);
+    cudaFree(c->active); cudaFree(c->iters);
+    delete c;
+    return WRI_OK;
+}
+
+int wri_set_model(wri_ctx* c, const float* m_dev) {
+    if (!c || !m_dev) return WRI_ERR_ARG;
+    c->m = m_dev;
+    return WRI_OK;
+}
+
+size_t wri_workspace_bytes(const wri_ctx* c, int32_t nb, int32_t host_staging) {
+    if (!c || nb <= 0 || nb > c->nb_max) return 0;
+    return ws_layout(c, nb, host_staging, kHostMaxitCap).total;
+}
+
+int wri_set_workspace(wri_ctx* c, void* ws_dev, size_t bytes) {
+    if (!c || !ws_dev || !aligned16(ws_dev)) return WRI_ERR_ARG;
+    if (c->solving) return WRI_ERR_STATE;
+    c->ws = (char*)ws_dev;
+    c->ws_bytes = bytes;
+    return WRI_OK;
+}
+
+int64_t wri_launch_count(const wri_ctx* c) { return c ? c->launches : 0; }
+
+int wri_apply_M(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, float lambda,
+                const void* x_dev, void* ytop_dev, void* ybot_dev) {
+    int rc = check_batch_args(c, nb);
+    if (rc) return rc;
+    if (!x_dev || !ytop_dev || (c->n_rec && !ybot_dev) || !aligned16(x_dev) || !aligned16(ytop_dev))
+        return WRI_ERR_ARG;
+    if ((rc = upload_columns(c, nb, omega_idx_host, lambda))) return rc;
+    const Tiling t = make_tiling(c, nb);
+    PassParams p = base_params(c, nb, t);
+    p.in = (const float2*)x_dev; p.out = (float2*)ytop_dev;
+    p.ca = c->coef + C_LAM * (size_t)c->nb_max;
+    p.sgn = 1.f;
+    if ((rc = launch_pass<MODE_APPLY>(c, p, t))) return rc;
+    if (c->n_rec) {
+        const long long n = (long long)c->n_rec * nb;
+        k_gather<<<(unsigned)std::min<long long>((n + 255) / 256, 1184), 256, 0, c->stream>>>(
+            (const float2*)x_dev, c->rec, c->n_rec, nb, (float2*)ybot_dev);
+        c->launches++;
+        CK(cudaGetLastError());
+    }
+    return WRI_OK;
+}
+
+int wri_apply_MH(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, float lambda,
+                 const void* ytop_dev, const void* ybot_dev, void* x_dev) {
+    int rc = check_batch_args(c, nb);
+    if (rc) return rc;
+    if (!x_dev || !ytop_dev || (c->n_rec && !ybot_dev) || !aligned16(x_dev) || !aligned16(ytop_dev))
+        return WRI_ERR_ARG;
+    if ((rc = upload_columns(c, nb, omega_idx_host, lambda))) return rc;
+    const Tiling t = make_tiling(c, nb);
+    PassParams p = base_params(c, nb, t);
+    p.in = (const float2*)ytop_dev; p.out = (float2*)x_dev;
+    p.ca = c->coef + C_LAM * (size_t)c->nb_max;
+    p.sgn = -1.f;
+    if ((rc = launch_pass<MODE_APPLY>(c, p, t))) return rc;
+    if (c->n_rec) {
+        const long long n = (long long)c->n_rec * nb;
+        k_scatter_add<<<(unsigned)std::min<long long>((n + 255) / 256, 1184), 256, 0, c->stream>>>(
+            (float2*)x_dev, c->rec, c->n_rec, nb, (const float2*)ybot_dev);
+        c->launches++;
+        CK(cudaGetLastError());
+    }
+    return WRI_OK;
+}
+
+int wri_lsqr_begin(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const void* q_dev,
+                   const void* d_dev, float lambda, const float* tol_dev, int32_t maxit,
+                   void* u_out_dev, float* resnorms_dev, int32_t* iters_dev) {
+    int rc = check_batch_args(c, nb);
+    if (rc) return rc;
+    if (!q_dev || (c->n_rec && !d_dev) || !u_out_dev || !resnorms_dev || maxit < 0 ||
+        !aligned16(q_dev) || !aligned16(u_out_dev) || q_dev == u_out_dev)
+        return WRI_ERR_ARG;
+    if (!c->ws) return WRI_ERR_WORKSPACE;
+    const WsLayout L = ws_layout(c, nb, 0, 0);
+    if (c->ws_bytes < L.total) return WRI_ERR_WORKSPACE;
+    if ((rc = upload_columns(c, nb, omega_idx_host, lambda))) return rc;
+
+    c->nb = nb; c->k = 0; c->maxit = maxit; c->lambda = lambda;
+    c->U = (float2*)(c->ws + L.U); c->V = (float2*)(c->ws + L.V); c->W = (float2*)(c->ws + L.W);
+    c->U_bot = (float2*)(c->ws + L.U_bot);
+    c->partials = (double*)(c->ws + L.partials);
+    c->X = (float2*)u_out_dev;
+    c->tol = tol_dev; c->resnorms = resnorms_dev; c->iters_out = iters_dev;
+    c->tl = make_tiling(c, nb);
+    const size_t vbytes = c->ng * (size_t)nb * sizeof(float2);
+    const size_t NM = c->nb_max;
+
+    // beta1 u1 = b = [lambda q ; d]   (q is consumed before V is cleared: the host entry
+    // stages q in the V slot)
+    PassParams p = base_params(c, nb, c->tl);
+    p.partials = c->partials;
+    p.in = (const float2*)q_dev; p.out = c->U; p.ca = c->coef + C_LAM * NM;
+    if ((rc = launch_pass<MODE_INIT>(c, p, c->tl))) return rc;
+    CK(cudaMemsetAsync(c->X, 0, vbytes, c->stream));
+    CK(cudaMemsetAsync(c->W, 0, vbytes, c->stream));
+    CK(cudaMemsetAsync(c->V, 0, vbytes, c->stream));
+    if ((rc = launch_scalars<PH_INIT_B>(c, (const float2*)d_dev))) return rc;
+    // alpha1 v1 = M^H u1
+    p.in = c->U; p.out = c->V; p.sgn = -1.f;
+    p.ca = c->coef + C_CA_A * NM; p.cb = c->coef + C_CB_A * NM;
+    if ((rc = launch_pass<MODE_A>(c, p, c->tl))) return rc;
+    if ((rc = launch_scalars<PH_INIT_A>(c, nullptr))) return rc;
+    c->solving = true;
+    return WRI_OK;
+}
+
+int wri_lsqr_iterate(wri_ctx* c, int32_t n_steps) {
+    if (!c || n_steps < 0) return WRI_ERR_ARG;
+    if (!c->solving) return WRI_ERR_STATE;
+    if (c->k + n_steps > c->maxit) return WRI_ERR_ARG;
+    const size_t NM = c->nb_max;
+    int rc;
+    for (int i = 0; i < n_steps; ++i) {
+        c->k++;
+        PassParams p = base_params(c, c->nb, c->tl);
+        p.partials = c->partials;
+        // pass F: U <- (lambda/alpha) A V - (alpha/beta) U ; deferred x, w updates
+        p.in = c->V; p.out = c->U; p.W = c->W; p.X = c->X; p.sgn = 1.f;
+        p.ca = c->coef + C_CA_F * NM; p.cb = c->coef + C_CB_F * NM; p.cv = c->coef + C_CV_F * NM;
+        p.cx = c->coef + C_CX * NM; p.cw = c->coef + C_CW * NM;
+        if ((rc = launch_pass<MODE_F>(c, p, c->tl))) return rc;
+        if ((rc = launch_scalars<PH_F>(c, nullptr))) return rc;
+        // pass A: V <- (lambda/beta) A^H U - (beta/alpha) V
+        p.in = c->U; p.out = c->V; p.W = nullptr; p.X = nullptr; p.sgn = -1.f;
+        p.ca = c->coef + C_CA_A * NM; p.cb = c->coef + C_CB_A * NM;
+        if ((rc = launch_pass<MODE_A>(c, p, c->tl))) return rc;
+        if ((rc = launch_scalars<PH_A>(c, nullptr))) return rc;
+    }
+    return WRI_OK;
+}
+
+int wri_lsqr_end(wri_ctx* c) {
+    if (!c) return WRI_ERR_ARG;
+    if (!c->solving) return WRI_ERR_STATE;
+    const long long n = (long long)c->ng * c->nb;
+    const size_t NM = c->nb_max;
+    k_flush_x<<<148 * 8, 256, 0, c->stream>>>(c->X, c->W, c->coef + C_CX * NM, n, c->nb);
+    c->launches++;
+    CK(cudaGetLastError());
+    CK(cudaMemsetAsync(c->coef + C_CX * NM, 0, c->nb * sizeof(float), c->stream));
+    c->solving = false;
+    return WRI_OK;
+}
+
+int wri_lsqr_batch(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const void* q_dev,
+                   const void* d_dev, float lambda, const float* tol_dev, int32_t maxit,
+                   void* u_out_dev, float* resnorms_dev, int32_t* iters_dev) {
+    int rc = wri_lsqr_begin(c, nb, omega_idx_host, q_dev, d_dev, lambda, tol_dev, maxit, u_out_dev,
+                            resnorms_dev, iters_dev);
+    if (rc) return rc;
+    if ((rc = wri_lsqr_iterate(c, maxit))) { c->solving = false; return rc; }
+    return wri_lsqr_end(c);
+}
+
+int wri_lsqr_batch_host(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const void* q_host,
+                        const void* d_host, float lambda, const float* tol_host, int32_t maxit,
+                        void* u_out_host, float* resnorms_host, int32_t* iters_host) {
+    int rc = check_batch_args(c, nb);
+    if (rc) return rc;
+    if (!q_host || (c->n_rec && !d_host) || !u_out_host || !resnorms_host || maxit < 0 ||
+        maxit > kHostMaxitCap)
+        return WRI_ERR_ARG;
+    if (!c->ws) return WRI_ERR_WORKSPACE;
+    const WsLayout L = ws_layout(c, nb, 1, kHostMaxitCap);
+    if (c->ws_bytes < L.total) return WRI_ERR_WORKSPACE;
+    const size_t vbytes = c->ng * (size_t)nb * sizeof(float2);
+    const size_t dbytes = (size_t)c->n_rec * nb * sizeof(float2);
+    float2* Xs = (float2*)(c->ws + L.Xs);
+    float2* Ds = (float2*)(c->ws + L.Ds);
+    float* tols = (float*)(c->ws + L.tols);
+    float* res = (float*)(c->ws + L.res);
+    int* its = (int*)(c->ws + L.its);
+    // q is staged in the V slot: wri_lsqr_begin consumes q before it clears V
+    float2* Qs = (float2*)(c->ws + L.V);
+    CK(cudaMemcpyAsync(Qs, q_host, vbytes, cudaMemcpyHostToDevice, c->stream));
+    if (dbytes) CK(cudaMemcpyAsync(Ds, d_host, dbytes, cudaMemcpyHostToDevice, c->stream));
+    if (tol_host) CK(cudaMemcpyAsync(tols, tol_host, nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    rc = wri_lsqr_batch(c, nb, omega_idx_host, Qs, Ds, lambda, tol_host ? tols : nullptr, maxit, Xs, res, its);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(u_out_host, Xs, vbytes, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaMemcpyAsync(resnorms_host, res, (size_t)(maxit + 1) * nb * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+    if (iters_host) CK(cudaMemcpyAsync(iters_host, its, nb * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    return WRI_OK;
+}
+
+int wri_lsqr_peek(const wri_ctx* c, wri_lsqr_view* v) {
+    if (!c || !v) return WRI_ERR_ARG;
+    if (!c->U) return WRI_ERR_STATE;
+    const size_t NM = c->nb_max;
+    v->nb = c->nb; v->k = c->k;
+    v->U_top = c->U; v->U_bot = c->U_bot; v->V = c->V; v->W = c->W; v->X = c->X;
+    v->alpha = c->stat + S_ALPHA * NM; v->beta = c->stat + S_BETA * NM;
+    v->rhobar = c->stat + S_RHOBAR * NM; v->phibar = c->stat + S_PHIBAR * NM;
+    v->ar0 = c->stat + S_AR0 * NM;
+    v->cx = c->coef + C_CX * NM;
+    v->cw = c->coef + C_CW * NM;
+    v->active = c->active; v->iters = c->iters;
+    return WRI_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,457 @@
+// wri_kernels.cuh — sm_100a device code of libwri (see include/wri.h for the operations).
+//
+// Layout: complex64 vectors are source-interleaved, element (c, s) at c*nb + s with
+// c = (iz*ny + iy)*nx + ix.  One x-row of the grid is therefore a contiguous run of
+// RL = nx*nb complex numbers; x-neighbours are +-nb elements away, y-neighbours +-RL,
+// z-neighbours +-RL*ny.  A thread owns VEC consecutive columns of one cell (16 B when
+// VEC = 2) and marches along z with a three-plane register pipeline, so each element of
+// the stencil input is fetched from HBM once per pass; x/y neighbours are re-read through
+// L1/L2 (they are the centre loads of neighbouring threads of the same tile).
+//
+// Every LSQR vector operation is fused into the two stencil passes:
+//   pass F : U <- ca * A V  - cb * U,  ||U||^2 partials,  X += cx W,  W <- cv V - cw W
+//   pass A : V <- ca * A^H U - cb * V, ||V||^2 partials
+// with per-column coefficients (lazy normalisation: U, V stay un-normalised).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace wri {
+
+enum PassMode { MODE_APPLY = 0, MODE_A = 1, MODE_F = 2, MODE_INIT = 3 };
+
+// per-column float coefficients, one row of nb_max each
+enum Coef { C_CA_F = 0, C_CB_F, C_CV_F, C_CX, C_CW, C_CA_A, C_CB_A, C_CT_A, C_W2, C_ONE, C_LAM, N_COEF };
+// per-column double state, one row of nb_max each
+enum Stat { S_ALPHA = 0, S_BETA, S_RHOBAR, S_PHIBAR, S_AR0, N_STAT };
+
+struct PassParams {
+    const float2* in;      // stencil input [n_g][nb]
+    float2* out;           // result; also the "old" vector of the axpy (in place)
+    float2* W;             // MODE_F only
+    float2* X;             // MODE_F only
+    const float* m;        // [n_g] squared slowness
+    const float* gx;       // [nx] sponge profile per axis, gamma = max(gx,gy,gz)
+    const float* gy;
+    const float* gz;
+    const float* w2;       // [nb] omega^2 per column
+    const float* ca;       // [nb] scale of the operator term (includes lambda)
+    const float* cb;       // [nb] scale of the old vector
+    const float* cv;       // [nb] MODE_F: scale of V in the w update
+    const float* cx;       // [nb] MODE_F
+    const float* cw;       // [nb] MODE_F
+    double* partials;      // [n_tiles][nb] squared-norm partial sums
+    int nx, ny, nz, nb;
+    int zc;                // planes per tile
+    float ih2;             // 1/h^2
+    float m6ih2;           // -6/h^2
+    float sgn;             // +1: A, -1: A^H (conjugated diagonal)
+};
+
+template <int VEC> struct CV { float2 a[VEC]; };
+
+template <int VEC> __device__ __forceinline__ CV<VEC> ldg_ro(const float2* p);
+template <> __device__ __forceinline__ CV<1> ldg_ro<1>(const float2* p) {
+    CV<1> r; r.a[0] = __ldg(p); return r;
+}
+template <> __device__ __forceinline__ CV<2> ldg_ro<2>(const float2* p) {
+    float4 t = __ldg(reinterpret_cast<const float4*>(p));
+    CV<2> r; r.a[0] = make_float2(t.x, t.y); r.a[1] = make_float2(t.z, t.w); return r;
+}
+// streaming load of data that is read once and rewritten in place
+template <int VEC> __device__ __forceinline__ CV<VEC> ld_rw(const float2* p);
+template <> __device__ __forceinline__ CV<1> ld_rw<1>(const float2* p) {
+    CV<1> r; r.a[0] = __ldcs(p); return r;
+}
+template <> __device__ __forceinline__ CV<2> ld_rw<2>(const float2* p) {
+    float4 t = __ldcs(reinterpret_cast<const float4*>(p));
+    CV<2> r; r.a[0] = make_float2(t.x, t.y); r.a[1] = make_float2(t.z, t.w); return r;
+}
+template <int VEC> __device__ __forceinline__ void st_v(float2* p, const CV<VEC>& v);
+template <> __device__ __forceinline__ void st_v<1>(float2* p, const CV<1>& v) { *p = v.a[0]; }
+template <> __device__ __forceinline__ void st_v<2>(float2* p, const CV<2>& v) {
+    *reinterpret_cast<float4*>(p) = make_float4(v.a[0].x, v.a[0].y, v.a[1].x, v.a[1].y);
+}
+template <int VEC> __device__ __forceinline__ CV<VEC> zero_v() {
+    CV<VEC> r;
+#pragma unroll
+    for (int k = 0; k < VEC; ++k) r.a[k] = make_float2(0.f, 0.f);
+    return r;
+}
+
+// Block-level, fixed-order reduction of per-thread column sums into partials[tile][0..nb).
+// Slot (ty, tx, k) holds column (col0 + tx*VEC + k) % nb; thread j sums the slots of column j
+// in increasing (ty, position) order, so the result does not depend on scheduling.
+template <int VEC>
+__device__ __forceinline__ void block_column_sums(const double (&acc)[VEC], int col0, int nb,
+                                                  double* __restrict__ dst) {
+    extern __shared__ double red[];
+    const int TX = blockDim.x, TY = blockDim.y;
+    const int slot = (threadIdx.y * TX + threadIdx.x) * VEC;
+#pragma unroll
+    for (int k = 0; k < VEC; ++k) red[slot + k] = acc[k];
+    __syncthreads();
+    const int width = TX * VEC;
+    const int tid = threadIdx.y * TX + threadIdx.x;
+    for (int j = tid; j < nb; j += TX * TY) {
+        int t0 = j - col0;
+        if (t0 < 0) t0 += nb;
+        double s = 0.0;
+        for (int ty = 0; ty < TY; ++ty)
+            for (int t = t0; t < width; t += nb) s += red[ty * width + t];
+        dst[j] = s;
+    }
+}
+
+template <int VEC, int MODE>
+__global__ void __launch_bounds__(256)
+k_pass(const PassParams p) {
+    const int nb = p.nb;
+    const int RL = p.nx * nb;                               // complex elements per x-row
+    const int e0 = (blockIdx.x * blockDim.x + threadIdx.x) * VEC;
+    const int iy = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z0 = blockIdx.z * p.zc;
+    const int z1 = min(z0 + p.zc, p.nz);
+    const bool live = (e0 < RL) && (iy < p.ny);
+    const int col0 = (int)(((long long)blockIdx.x * blockDim.x * VEC) % nb);
+
+    double acc[VEC];
+#pragma unroll
+    for (int k = 0; k < VEC; ++k) acc[k] = 0.0;
+
+    if (live) {
+        const int ix = e0 / nb;
+        const int s0 = e0 - ix * nb;
+        float w2[VEC], ca[VEC], cb[VEC], cv[VEC], cx[VEC], cw[VEC];
+#pragma unroll
+        for (int k = 0; k < VEC; ++k) {
+            w2[k] = p.w2[s0 + k];
+            ca[k] = p.ca[s0 + k];
+            cb[k] = (MODE == MODE_A || MODE == MODE_F) ? p.cb[s0 + k] : 0.f;
+            cv[k] = (MODE == MODE_F) ? p.cv[s0 + k] : 0.f;
+            cx[k] = (MODE == MODE_F) ? p.cx[s0 + k] : 0.f;
+            cw[k] = (MODE == MODE_F) ? p.cw[s0 + k] : 0.f;
+        }
+        const bool has_xm = ix > 0, has_xp = ix < p.nx - 1;
+        const bool has_ym = iy > 0, has_yp = iy < p.ny - 1;
+        const size_t plane = (size_t)RL * p.ny;
+        const float gxy = fmaxf(p.gx[ix], p.gy[iy]);
+
+        size_t off = ((size_t)z0 * p.ny + iy) * RL + e0;
+        size_t moff = ((size_t)z0 * p.ny + iy) * p.nx + ix;
+        CV<VEC> prev = zero_v<VEC>(), cur, nxt;
+        cur = ldg_ro<VEC>(p.in + off);
+        if (MODE != MODE_INIT && z0 > 0) prev = ldg_ro<VEC>(p.in + off - plane);
+
+#pragma unroll 1
+        for (int z = z0; z < z1; ++z) {
+            nxt = zero_v<VEC>();
+            if (z + 1 < p.nz && (MODE != MODE_INIT || z + 1 < z1)) nxt = ldg_ro<VEC>(p.in + off + plane);
+            CV<VEC> r;
+            if (MODE != MODE_INIT) {
+                CV<VEC> xm = zero_v<VEC>(), xp = zero_v<VEC>(), ym = zero_v<VEC>(), yp = zero_v<VEC>();
+                if (has_xm) xm = ldg_ro<VEC>(p.in + off - nb);
+                if (has_xp) xp = ldg_ro<VEC>(p.in + off + nb);
+                if (has_ym) ym = ldg_ro<VEC>(p.in + off - RL);
+                if (has_yp) yp = ldg_ro<VEC>(p.in + off + RL);
+                CV<VEC> old, wv, xv;
+                if (MODE == MODE_A || MODE == MODE_F) old = ld_rw<VEC>(p.out + off);
+                if (MODE == MODE_F) { wv = ld_rw<VEC>(p.W + off); xv = ld_rw<VEC>(p.X + off); }
+                const float mc = __ldg(p.m + moff);
+                const float g = fmaxf(gxy, p.gz[z]);
+#pragma unroll
+                for (int k = 0; k < VEC; ++k) {
+                    const float wm = w2[k] * mc;
+                    const float dr = wm + p.m6ih2;          // Re diag = -6/h^2 + w^2 m
+                    const float di = p.sgn * wm * g;        // Im diag = +-w^2 m gamma
+                    const float sr = ((xm.a[k].x + xp.a[k].x) + (ym.a[k].x + yp.a[k].x)) + (prev.a[k].x + nxt.a[k].x);
+                    const float si = ((xm.a[k].y + xp.a[k].y) + (ym.a[k].y + yp.a[k].y)) + (prev.a[k].y + nxt.a[k].y);
+                    float ar = fmaf(p.ih2, sr, fmaf(dr, cur.a[k].x, -di * cur.a[k].y));
+                    float ai = fmaf(p.ih2, si, fmaf(dr, cur.a[k].y, di * cur.a[k].x));
+                    if (MODE == MODE_A || MODE == MODE_F) {
+                        ar = fmaf(ca[k], ar, -cb[k] * old.a[k].x);
+                        ai = fmaf(ca[k], ai, -cb[k] * old.a[k].y);
+                    } else {
+                        ar *= ca[k]; ai *= ca[k];
+                    }
+                    r.a[k] = make_float2(ar, ai);
+                    if (MODE == MODE_F) {
+                        xv.a[k].x = fmaf(cx[k], wv.a[k].x, xv.a[k].x);
+                        xv.a[k].y = fmaf(cx[k], wv.a[k].y, xv.a[k].y);
+                        wv.a[k].x = fmaf(cv[k], cur.a[k].x, -cw[k] * wv.a[k].x);
+                        wv.a[k].y = fmaf(cv[k], cur.a[k].y, -cw[k] * wv.a[k].y);
+                    }
+                }
+                if (MODE == MODE_F) { st_v<VEC>(p.X + off, xv); st_v<VEC>(p.W + off, wv); }
+            } else {
+#pragma unroll
+                for (int k = 0; k < VEC; ++k)
+                    r.a[k] = make_float2(ca[k] * cur.a[k].x, ca[k] * cur.a[k].y);
+            }
+            st_v<VEC>(p.out + off, r);
+            if (MODE != MODE_APPLY) {
+#pragma unroll
+                for (int k = 0; k < VEC; ++k)
+                    acc[k] += (double)fmaf(r.a[k].x, r.a[k].x, r.a[k].y * r.a[k].y);
+            }
+            prev = cur; cur = nxt;
+            off += plane;
+            moff += (size_t)p.nx * p.ny;
+        }
+    }
+    if (MODE != MODE_APPLY) {
+        const size_t tile = ((size_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+        block_column_sums<VEC>(acc, col0, nb, p.partials + tile * nb);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Receiver rows (P and P^T are exact indexing).
+
+// ybot[r][s] = x[rec[r]][s]            (bit-exact copy)
+__global__ void k_gather(const float2* __restrict__ x, const int* __restrict__ rec, int n_rec, int nb,
+                         float2* __restrict__ ybot) {
+    const long long n = (long long)n_rec * nb;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
+         i += (long long)gridDim.x * blockDim.x) {
+        const int r = (int)(i / nb), s = (int)(i - (long long)r * nb);
+        ybot[i] = x[(size_t)rec[r] * nb + s];
+    }
+}
+
+// x[rec[r]][s] += ybot[r][s]           (receivers are unique, so this is race-free)
+__global__ void k_scatter_add(float2* __restrict__ x, const int* __restrict__ rec, int n_rec, int nb,
+                              const float2* __restrict__ ybot) {
+    const long long n = (long long)n_rec * nb;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
+         i += (long long)gridDim.x * blockDim.x) {
+        const int r = (int)(i / nb), s = (int)(i - (long long)r * nb);
+        float2* d = x + (size_t)rec[r] * nb + s;
+        const float2 a = *d, b = ybot[i];
+        *d = make_float2(a.x + b.x, a.y + b.y);
+    }
+}
+
+// X += cx * W over the whole batch (last deferred update, wri_lsqr_end)
+__global__ void k_flush_x(float2* __restrict__ X, const float2* __restrict__ W,
+                          const float* __restrict__ cx, long long n, int nb) {
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
+         i += (long long)gridDim.x * blockDim.x) {
+        const float c = cx[(int)(i % nb)];
+        if (c != 0.f) {
+            const float2 w = W[i];
+            float2 x = X[i];
+            x.x = fmaf(c, w.x, x.x);
+            x.y = fmaf(c, w.y, x.y);
+            X[i] = x;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Per-column scalar recurrences + receiver rows, one block.  Phases:
+enum ScalPhase { PH_INIT_B = 0, PH_INIT_A = 1, PH_F = 2, PH_A = 3 };
+
+struct ScalParams {
+    const double* partials;   // [n_tiles][nb]
+    int n_tiles;
+    int nb, nb_max;
+    int n_rec;
+    const int* rec;           // [n_rec] cell indices
+    float2* V;                // [n_g][nb]
+    float2* U_bot;            // [n_rec][nb]
+    const float2* d;          // PH_INIT_B: data rows [n_rec][nb]
+    float* coef;              // [N_COEF][nb_max]
+    double* stat;             // [N_STAT][nb_max]
+    int* active;              // [nb]
+    int* iters;               // [nb]
+    const float* tol;         // [nb] or null
+    float* resnorms;          // [maxit+1][nb]
+    int* iters_out;           // [nb] or null
+    int k;                    // iteration number (PH_A), for resnorms / iters
+    int maxit;
+    float lambda;
+};
+
+// sum over tiles of partials[.][s] in fixed order; result for column s in colsum[s] (shared)
+__device__ __forceinline__ void reduce_partials(const ScalParams& p, double* scratch, double* colsum) {
+    const int nb = p.nb, T = blockDim.x;
+    const int G = max(1, T / nb);
+    for (int base = 0; base < nb; base += T) {           // nb > T handled in column chunks
+        const int ncol = min(nb - base, T);
+        const int g = threadIdx.x / ncol, s = base + threadIdx.x % ncol;
+        const int Gc = max(1, T / ncol);
+        double a = 0.0;
+        if (g < Gc)
+            for (int b = g; b < p.n_tiles; b += Gc) a += p.partials[(size_t)b * nb + s];
+        scratch[threadIdx.x] = a;
+        __syncthreads();
+        if (threadIdx.x < ncol) {
+            double t = 0.0;
+            for (int gg = 0; gg < Gc; ++gg) t += scratch[gg * ncol + threadIdx.x];
+            colsum[base + threadIdx.x] = t;
+        }
+        __syncthreads();
+    }
+    (void)G;
+}
+
+// fixed-order sum over receivers of |U_bot[r][s]|^2, added to colsum[s]
+__device__ __forceinline__ void add_receiver_norms(const ScalParams& p, double* scratch, double* colsum) {
+    const int nb = p.nb, T = blockDim.x;
+    for (int base = 0; base < nb; base += T) {
+        const int ncol = min(nb - base, T);
+        const int Gc = max(1, T / ncol);
+        const int g = threadIdx.x / ncol, s = base + threadIdx.x % ncol;
+        double a = 0.0;
+        if (g < Gc)
+            for (int r = g; r < p.n_rec; r += Gc) {
+                const float2 u = p.U_bot[(size_t)r * nb + s];
+                a += (double)fmaf(u.x, u.x, u.y * u.y);
+            }
+        scratch[threadIdx.x] = a;
+        __syncthreads();
+        if (threadIdx.x < ncol) {
+            double t = 0.0;
+            for (int gg = 0; gg < Gc; ++gg) t += scratch[gg * ncol + threadIdx.x];
+            colsum[base + threadIdx.x] += t;
+        }
+        __syncthreads();
+    }
+}
+
+template <int PHASE>
+__global__ void __launch_bounds__(1024)
+k_scalars(const ScalParams p) {
+    extern __shared__ double sh[];
+    double* scratch = sh;                   // [blockDim.x]
+    double* colsum = sh + blockDim.x;       // [nb]
+    const int nb = p.nb, NM = p.nb_max;
+    float* cf = p.coef;
+    double* st = p.stat;
+
+    const long long nrs = (long long)p.n_rec * nb;
+    if (PHASE == PH_INIT_B) {
+        // U_bot = d (exact copy), then beta1 = ||[lambda q ; d]||
+        for (long long i = threadIdx.x; i < nrs; i += blockDim.x) p.U_bot[i] = p.d[i];
+        __syncthreads();
+    }
+    if (PHASE == PH_F) {
+        // bottom rows of the forward pass just done:  U_bot <- cv * V[rec] - cb * U_bot
+        for (long long i = threadIdx.x; i < nrs; i += blockDim.x) {
+            const int r = (int)(i / nb), s = (int)(i - (long long)r * nb);
+            const float cv = cf[C_CV_F * NM + s], cb = cf[C_CB_F * NM + s];
+            const float2 v = p.V[(size_t)p.rec[r] * nb + s];
+            const float2 u = p.U_bot[i];
+            p.U_bot[i] = make_float2(fmaf(cv, v.x, -cb * u.x), fmaf(cv, v.y, -cb * u.y));
+        }
+        __syncthreads();
+    }
+    reduce_partials(p, scratch, colsum);
+    if (PHASE == PH_INIT_B || PHASE == PH_F) add_receiver_norms(p, scratch, colsum);
+
+    for (int s = threadIdx.x; s < nb; s += blockDim.x) {
+        const double nrm = sqrt(colsum[s]);
+        if (PHASE == PH_INIT_B) {
+            // beta1 u1 = b.  b = 0 => x = 0, nothing to iterate (reading C-7).
+            const double beta = nrm;
+            st[S_BETA * NM + s] = beta;
+            st[S_PHIBAR * NM + s] = beta;
+            st[S_ALPHA * NM + s] = 0.0;
+            st[S_RHOBAR * NM + s] = 0.0;
+            st[S_AR0 * NM + s] = 0.0;
+            const int act = beta > 0.0;
+            p.active[s] = act;
+            p.iters[s] = 0;
+            if (p.iters_out) p.iters_out[s] = 0;
+            p.resnorms[s] = (float)beta;
+            // first adjoint pass: V = (lambda/beta) A^H U + (1/beta) P^T U_bot, old V = 0 with cb = 1
+            cf[C_CA_A * NM + s] = act ? (float)((double)p.lambda / beta) : 0.f;
+            cf[C_CT_A * NM + s] = act ? (float)(1.0 / beta) : 0.f;
+            cf[C_CB_A * NM + s] = 1.f;
+            cf[C_CX * NM + s] = 0.f;
+            cf[C_CW * NM + s] = 0.f;
+        } else if (PHASE == PH_INIT_A) {
+            // alpha1 v1 = M^H u1 ; w1 = v1 ; phibar = beta1 ; rhobar = alpha1
+            const double alpha = nrm, beta = st[S_BETA * NM + s];
+            int act = p.active[s];
+            st[S_ALPHA * NM + s] = alpha;
+            st[S_RHOBAR * NM + s] = alpha;
+            st[S_AR0 * NM + s] = alpha * beta;
+            if (act && !(alpha > 0.0)) { act = 0; p.active[s] = 0; }
+            cf[C_CA_F * NM + s] = act ? (float)((double)p.lambda / alpha) : 0.f;
+            cf[C_CV_F * NM + s] = act ? (float)(1.0 / alpha) : 0.f;
+            cf[C_CB_F * NM + s] = act ? (float)(alpha / beta) : 0.f;
+        } else if (PHASE == PH_F) {
+            // beta_{k+1} = ||M v_k - alpha_k u_k||
+            const int act = p.active[s];
+            if (act) {
+                const double beta = nrm, alpha = st[S_ALPHA * NM + s];
+                st[S_BETA * NM + s] = beta;
+                const bool ok = beta > 0.0;
+                cf[C_CA_A * NM + s] = ok ? (float)((double)p.lambda / beta) : 0.f;
+                cf[C_CT_A * NM + s] = ok ? (float)(1.0 / beta) : 0.f;
+                cf[C_CB_A * NM + s] = ok ? (float)(beta / alpha) : 0.f;
+            } else {
+                cf[C_CA_A * NM + s] = 0.f; cf[C_CT_A * NM + s] = 0.f; cf[C_CB_A * NM + s] = 0.f;
+                cf[C_CX * NM + s] = 0.f;          // a stopped column's last x update has been applied
+            }
+        } else {  // PH_A
+            int act = p.active[s];
+            if (act) {
+                // alpha_{k+1} = ||M^H u_{k+1} - beta_{k+1} v_k||, then the plane rotation
+                const double alpha = nrm, beta = st[S_BETA * NM + s];
+                const double rhobar = st[S_RHOBAR * NM + s], phibar = st[S_PHIBAR * NM + s];
+                const double rho = hypot(rhobar, beta);
+                const double c = rhobar / rho, sn = beta / rho;
+                const double theta = sn * alpha;
+                const double phi = c * phibar;
+                const double phibar_n = sn * phibar;
+                st[S_ALPHA * NM + s] = alpha;
+                st[S_RHOBAR * NM + s] = -c * alpha;
+                st[S_PHIBAR * NM + s] = phibar_n;
+                p.iters[s] = p.k;
+                if (p.iters_out) p.iters_out[s] = p.k;
+                const double arnorm = phibar_n * alpha * fabs(c);
+                const float tol = p.tol ? p.tol[s] : 0.f;
+                bool stop = !(beta > 0.0) || !(alpha > 0.0);
+                if (tol > 0.f && arnorm <= (double)tol * st[S_AR0 * NM + s]) stop = true;
+                cf[C_CX * NM + s] = (float)(phi / rho);
+                if (stop) {
+                    act = 0; p.active[s] = 0;
+                    cf[C_CW * NM + s] = 0.f;
+                    cf[C_CA_F * NM + s] = 0.f; cf[C_CV_F * NM + s] = 0.f; cf[C_CB_F * NM + s] = 0.f;
+                } else {
+                    cf[C_CW * NM + s] = (float)(theta / rho);
+                    cf[C_CA_F * NM + s] = (float)((double)p.lambda / alpha);
+                    cf[C_CV_F * NM + s] = (float)(1.0 / alpha);
+                    cf[C_CB_F * NM + s] = (float)(alpha / beta);
+                }
+            } else {
+                cf[C_CW * NM + s] = 0.f;
+                cf[C_CA_F * NM + s] = 0.f; cf[C_CV_F * NM + s] = 0.f; cf[C_CB_F * NM + s] = 0.f;
+            }
+            p.resnorms[(size_t)p.k * nb + s] = (float)st[S_PHIBAR * NM + s];
+        }
+    }
+    __syncthreads();
+
+    if (PHASE == PH_INIT_B || PHASE == PH_F) {
+        // fold P^T into the coming adjoint pass:  V <- ca A^H U - cb (V - (ct/cb) P^T U_bot)
+        for (long long i = threadIdx.x; i < nrs; i += blockDim.x) {
+            const int r = (int)(i / nb), s = (int)(i - (long long)r * nb);
+            const float cb = cf[C_CB_A * NM + s];
+            if (cb != 0.f) {
+                const float f = cf[C_CT_A * NM + s] / cb;
+                const float2 u = p.U_bot[i];
+                float2* v = p.V + (size_t)p.rec[r] * nb + s;
+                float2 t = *v;
+                t.x = fmaf(-f, u.x, t.x);
+                t.y = fmaf(-f, u.y, t.y);
+                *v = t;
+            }
+        }
+    }
+}
+
+}  // namespace wri
