@@ -1,0 +1,333 @@
+#!/usr/bin/env python
+"""bench.py — whole-path throughput of libwri on BASELINE.json's headline workload.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+
+One "step" = one complete batched LSQR solve (Golub-Kahan start + maxit iterations + final x
+update) of the workload's 64 sources through the C ABI.  Metric: LSQR iterations x sources per
+second (sum of per-column iteration counts / time).  `value` is timed with the inputs resident
+in HBM; `e2e` is the same solve through wri_lsqr_batch_host with pinned HOST buffers (H2D of q, d
+and D2H of u, resnorms, iters inside the timed region).  N > 1 (torchrun): batch columns are
+independent systems, so every rank solves its own 64-source group with no
+collective on the data path (weak scaling); time = max over ranks.
+
+--impl reference times the complex128 CPU oracle (oracle/) on a bounded sample of the same
+workload; it is a deliberately plain program, reported as context.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import workloads  # noqa: E402
+
+METRIC = "lsqr_iterations_x_sources_per_s"
+UNIT = "iter*src/s"
+
+WORKLOADS = {
+    # BASELINE.json metric: "LSQR iterations.sources/s at 128^3 x 64 src" = configs[2], one
+    # frequency group (f = 6 Hz), 200 iterations
+    "config2_128cubed_x64src": dict(name="config2", freqs=(6.0,)),
+    "config2_128cubed_x192col": dict(name="config2"),
+    "config1_64cubed_x16src": dict(name="config1"),
+    "config3_vsp_200x200x160_x48src": dict(name="config3"),
+    "config4_256cubed_x32src": dict(name="config4"),
+}
+DEFAULT_WORKLOAD = "config2_128cubed_x64src"
+
+BYTES_PASS_F = 56   # per cell per source: reads v,u,w,x + writes u,w,x (complex64)  [DESIGN.md]
+BYTES_PASS_A = 24   # reads u,v + writes v
+BYTES_ITER = BYTES_PASS_F + BYTES_PASS_A
+
+
+def measured_hbm_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic_bytes():
+    """dram bytes (read + write) per pass-F launch from the committed ncu capture, or None."""
+    path = os.path.join(ROOT, "profiles", "traffic_pass_f.csv")
+    try:
+        with open(path) as f:
+            for line in f:
+                if line.startswith("#") or not line.strip():
+                    continue
+                k, v = line.strip().split(",")[:2]
+                if k == "dram_bytes_per_launch":
+                    return float(v)
+    except Exception:
+        pass
+    return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            parts = [p.strip() for p in ln.split(",")]
+            if len(parts) < 6:
+                continue
+            try:
+                sm.append(float(parts[0]))
+                mx.append(float(parts[1]))
+            except ValueError:
+                continue
+            for n, p in zip(names, parts[2:6]):
+                if p.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None,
+                "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+def oracle_sample(w, cores, iters):
+    """Time the CPU oracle as it stands on min(nb, cores) columns x `iters` iterations."""
+    from oracle import oracle as O
+    ncols = max(1, min(w.nb, cores))
+    cols = list(range(ncols))
+    rec = O.rec_cells(w.nx, w.ny, w.nz, w.rec_ijk)
+    ops = [O.Operator(w.nx, w.ny, w.nz, w.h, w.omegas[j], w.sponge_width, w.gamma_max, w.power, w.faces)
+           for j in w.omega_idx]
+    O.build()
+    t0 = time.perf_counter()
+    out = O.lsqr_batch(ops, w.m, w.lam, rec, w.Q, w.D, None, maxit=iters, threads=ncols, columns=cols)
+    dt = time.perf_counter() - t0
+    done = int(out["iters"].sum())
+    return done / dt, ncols, dt, "%d columns x %d LSQR iterations of %s (incl. Golub-Kahan start)" % (
+        ncols, iters, w.name)
+
+
+def oracle_iters_for(w):
+    # ~60 ns per cell per operator application, 2 applications per iteration -> ~10-20 s
+    per_iter = 2.6e-7 * w.ng
+    return int(max(4, min(64, round(12.0 / per_iter))))
+
+
+def run_reference(args, wl_name, w):
+    rank, world, _ = dist_env()
+    if rank != 0:
+        return
+    cores = os.cpu_count() or 1
+    iters = oracle_iters_for(w)
+    times, rate, ncols, sample = [], 0.0, 0, ""
+    for i in range(args.warmup + args.steps):
+        r, ncols, dt, sample = oracle_sample(w, cores, iters)
+        if i >= args.warmup:
+            times.append(dt)
+    total = ncols * iters * len(times)
+    value = total / sum(times)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sum(times) / len(times),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "c128",
+            "data": "synthetic",
+            "config": {"workload": wl_name, "grid": [w.nx, w.ny, w.nz], "nb": w.nb, "n_rec": w.n_rec,
+                       "maxit": w.maxit, "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": ncols, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args, wl_name, w):
+    import torch
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    use_dist = world > 1
+    if use_dist:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    from paper_2410_18429_b200 import Wri
+    ctx = Wri.from_workload(w, device=dev)
+    nb, maxit = w.nb, w.maxit
+    q = torch.from_numpy(w.Q).to(dev)
+    d = torch.from_numpy(w.D).to(dev)
+    tol = torch.from_numpy(w.tol).to(dev) if (w.tol > 0).any() else None
+    ctx.ensure_workspace(nb, host_staging=True)
+    out = ctx._outputs(nb, maxit, dev)
+
+    def barrier():
+        if use_dist:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step():
+        return ctx.lsqr_batch(q, d, w.lam, tol, maxit=maxit, omega_idx=w.omega_idx, out=out)
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    iters_per_step = int(out[2].sum().item())
+
+    # ---- device-resident timing (value) with per-kernel events and clock sampling
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ctx.profile_enable(True)
+    ctx.profile_read()
+    l0 = ctx.launch_count()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = ctx.launch_count() - l0
+    ms_f, n_f, ms_a, n_a = ctx.profile_read()
+    ctx.profile_enable(False)
+    clocks = sampler.stop() if rank == 0 else None
+
+    # ---- end-to-end timing through the host-buffer entry
+    qh = torch.from_numpy(w.Q).pin_memory()
+    dh = torch.from_numpy(w.D).pin_memory()
+    tolh = torch.from_numpy(w.tol).pin_memory() if tol is not None else None
+    outh = (torch.empty((w.ng, nb), dtype=torch.complex64).pin_memory(),
+            torch.empty((maxit + 1, nb), dtype=torch.float32).pin_memory(),
+            torch.empty(nb, dtype=torch.int32).pin_memory())
+    e2e_steps = max(1, min(args.steps, 3))
+    ctx.lsqr_batch_host(qh, dh, w.lam, tolh, maxit=maxit, omega_idx=w.omega_idx, out=outh)   # warm-up
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        ctx.lsqr_batch_host(qh, dh, w.lam, tolh, maxit=maxit, omega_idx=w.omega_idx, out=outh)
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    h2d = qh.numel() * 8 + dh.numel() * 8 + (tolh.numel() * 4 if tolh is not None else 0)
+    d2h = outh[0].numel() * 8 + outh[1].numel() * 4 + outh[2].numel() * 4
+    iters_e2e = int(outh[2].sum().item())
+
+    if use_dist:
+        t = torch.tensor([ms, e2e_s], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms, e2e_s = float(t[0]), float(t[1])
+        tot = torch.tensor([iters_per_step, iters_e2e, launches], dtype=torch.float64, device=dev)
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+        iters_all, iters_e2e_all, launches_all = float(tot[0]), float(tot[1]), int(tot[2])
+    else:
+        iters_all, iters_e2e_all, launches_all = iters_per_step, iters_e2e, launches
+
+    if rank == 0:
+        value = iters_all * args.steps / (ms * 1e-3)
+        peak, peak_src = measured_hbm_peak()
+        cells = w.ng * nb
+        bytes_f = BYTES_PASS_F * cells + 4 * w.ng
+        ach_f = bytes_f / (ms_f / max(n_f, 1) * 1e-3) / 1e9 if n_f else None
+        ach_a = (BYTES_PASS_A * cells + 4 * w.ng) / (ms_a / max(n_a, 1) * 1e-3) / 1e9 if n_a else None
+        # whole-iteration algorithmic bandwidth over the full step (includes start/end kernels)
+        ach_iter = BYTES_ITER * w.ng * iters_per_step * args.steps / (ms * 1e-3) / 1e9
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "c64", "data": "synthetic",
+            "config": {"workload": wl_name, "grid": [w.nx, w.ny, w.nz], "h": w.h, "nb": nb,
+                       "n_rec": w.n_rec, "freqs_hz": list(w.freqs), "lambda": w.lam, "maxit": maxit,
+                       "iters_per_step": iters_per_step, "sharding": "columns per rank, no collective",
+                       "l2": "working set %.1f GB per rank exceeds the 126 MB L2" % (4 * cells * 8 / 1e9)},
+            "clocks": clocks,
+            "e2e": {"value": iters_e2e_all * e2e_steps / e2e_s, "unit": UNIT,
+                    "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps},
+            "gpu_launches": launches_all,
+            "roofline": {"bound": "hbm", "kernel": "k_pass<MODE_F> (forward stencil + u axpy + x,w update + ||u||^2)",
+                         "achieved": ach_f, "peak": peak, "peak_source": peak_src, "unit": "GB/s",
+                         "frac": (ach_f / peak) if ach_f else None, "traffic": ncu_traffic_bytes(),
+                         "algorithmic_bytes_per_launch": bytes_f,
+                         "avg_launch_ms": ms_f / max(n_f, 1), "launches_timed": n_f,
+                         "pass_a": {"achieved": ach_a, "frac": (ach_a / peak) if ach_a else None,
+                                    "avg_launch_ms": ms_a / max(n_a, 1)},
+                         "whole_step": {"achieved": ach_iter, "frac": ach_iter / peak,
+                                        "frac_of_8000": ach_iter / 8000.0}},
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            cores = os.cpu_count() or 1
+            r, ncols, dt, sample = oracle_sample(w, cores, oracle_iters_for(w))
+            line["cpu_baseline"] = {"value": r, "unit": UNIT, "cores": ncols, "kind": "oracle",
+                                    "sample": sample, "seconds": dt}
+        print(json.dumps(line), flush=True)
+    if use_dist:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(WORKLOADS))
+    ap.add_argument("--maxit", type=int, default=None, help="override the workload's iteration count")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    spec = dict(WORKLOADS[args.workload])
+    w = workloads.make(spec.pop("name"), **spec)
+    if args.maxit:
+        w.maxit = args.maxit
+    if args.impl == "reference":
+        run_reference(args, args.workload, w)
+    else:
+        run_ours(args, args.workload, w)
+
+
+if __name__ == "__main__":
+    main()

@@ -67,6 +67,11 @@ struct wri_ctx {
     int* iters_out = nullptr;
     Tiling tl{};
     int64_t launches = 0;
+    // optional per-kernel timing (wri_profile_*)
+    bool profiling = false;
+    std::vector<cudaEvent_t> ev_pool;     // pairs: start, stop
+    std::vector<int> ev_kind;             // per pair: 0 = pass F, 1 = pass A
+    size_t ev_used = 0;                   // pairs in use
 };
 
 namespace {
@@ -150,12 +155,26 @@ PassParams base_params(const wri_ctx* c, int nb, const Tiling& t) {
 }
 
 template <int MODE>
-int launch_pass(wri_ctx* c, const PassParams& p, const Tiling& t) {
+int launch_pass(wri_ctx* c, const PassParams& p, const Tiling& t, bool timed = false) {
     const size_t smem = (MODE == MODE_APPLY) ? 0 : (size_t)t.block.x * t.block.y * t.vec * sizeof(double);
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (timed && c->profiling) {
+        if (c->ev_used * 2 == c->ev_pool.size()) {
+            cudaEvent_t a, b;
+            CK(cudaEventCreate(&a));
+            CK(cudaEventCreate(&b));
+            c->ev_pool.push_back(a); c->ev_pool.push_back(b); c->ev_kind.push_back(0);
+        }
+        e0 = c->ev_pool[2 * c->ev_used]; e1 = c->ev_pool[2 * c->ev_used + 1];
+        c->ev_kind[c->ev_used] = (MODE == MODE_F) ? 0 : 1;
+        c->ev_used++;
+        CK(cudaEventRecord(e0, c->stream));
+    }
     if (t.vec == 2) k_pass<2, MODE><<<t.grid, t.block, smem, c->stream>>>(p);
     else            k_pass<1, MODE><<<t.grid, t.block, smem, c->stream>>>(p);
     c->launches++;
     CK(cudaGetLastError());
+    if (e1) CK(cudaEventRecord(e1, c->stream));
     return WRI_OK;
 }
 
@@ -282,6 +301,7 @@ int wri_destroy(wri_ctx* c) {
     if (!c) return WRI_OK;
     cudaFree(c->gtab); cudaFree(c->rec); cudaFree(c->coef); cudaFree(c->stat);
     cudaFree(c->active); cudaFree(c->iters);
+    for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
     delete c;
     return WRI_OK;
 }
@@ -306,6 +326,25 @@ int wri_set_workspace(wri_ctx* c, void* ws_dev, size_t bytes) {
 }
 
 int64_t wri_launch_count(const wri_ctx* c) { return c ? c->launches : 0; }
+
+int wri_profile_enable(wri_ctx* c, int32_t on) {
+    if (!c) return WRI_ERR_ARG;
+    c->profiling = on != 0;
+    return WRI_OK;
+}
+
+int wri_profile_read(wri_ctx* c, double* ms_f, int64_t* n_f, double* ms_a, int64_t* n_a) {
+    if (!c || !ms_f || !n_f || !ms_a || !n_a) return WRI_ERR_ARG;
+    CK(cudaStreamSynchronize(c->stream));
+    *ms_f = *ms_a = 0.0; *n_f = *n_a = 0;
+    for (size_t i = 0; i < c->ev_used; ++i) {
+        float ms = 0.f;
+        CK(cudaEventElapsedTime(&ms, c->ev_pool[2 * i], c->ev_pool[2 * i + 1]));
+        if (c->ev_kind[i] == 0) { *ms_f += ms; ++*n_f; } else { *ms_a += ms; ++*n_a; }
+    }
+    c->ev_used = 0;
+    return WRI_OK;
+}
 
 int wri_apply_M(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, float lambda,
                 const void* x_dev, void* ytop_dev, void* ybot_dev) {
@@ -409,12 +448,12 @@ int wri_lsqr_iterate(wri_ctx* c, int32_t n_steps) {
         p.in = c->V; p.out = c->U; p.W = c->W; p.X = c->X; p.sgn = 1.f;
         p.ca = c->coef + C_CA_F * NM; p.cb = c->coef + C_CB_F * NM; p.cv = c->coef + C_CV_F * NM;
         p.cx = c->coef + C_CX * NM; p.cw = c->coef + C_CW * NM;
-        if ((rc = launch_pass<MODE_F>(c, p, c->tl))) return rc;
+        if ((rc = launch_pass<MODE_F>(c, p, c->tl, true))) return rc;
         if ((rc = launch_scalars<PH_F>(c, nullptr))) return rc;
         // pass A: V <- (lambda/beta) A^H U - (beta/alpha) V
         p.in = c->U; p.out = c->V; p.W = nullptr; p.X = nullptr; p.sgn = -1.f;
         p.ca = c->coef + C_CA_A * NM; p.cb = c->coef + C_CB_A * NM;
-        if ((rc = launch_pass<MODE_A>(c, p, c->tl))) return rc;
+        if ((rc = launch_pass<MODE_A>(c, p, c->tl, true))) return rc;
         if ((rc = launch_scalars<PH_A>(c, nullptr))) return rc;
     }
     return WRI_OK;
