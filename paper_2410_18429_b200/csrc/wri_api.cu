@@ -2,10 +2,12 @@
 // All arithmetic of the path runs in the kernels of wri_kernels.cuh; there is no CPU fallback.
 #include "../../include/wri.h"
 #include "wri_kernels.cuh"
+#include "wri_tma.cuh"
 
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 
@@ -67,6 +69,13 @@ struct wri_ctx {
     int* iters_out = nullptr;
     Tiling tl{};
     int64_t launches = 0;
+    // persistent TMA pass kernel (nb % 16 == 0): column chunk width, tiling, tensor maps
+    int num_sms = 0;
+    unsigned int* counter = nullptr;      // last-CTA ticket (device)
+    int tma_cb = 0;                       // 0 = not used for this solve
+    int tma_zc = 0, tma_ntx = 0, tma_nty = 0, tma_ntz = 0, tma_nchunk = 0, tma_tiles = 0, tma_grid = 0;
+    double* partials_tma = nullptr;       // [tma_grid][nb]
+    CUtensorMap tmU_halo{}, tmV_halo{}, tmU_ctr{}, tmV_ctr{}, tmW_ctr{}, tmX_ctr{};
     // optional per-kernel timing (wri_profile_*)
     bool profiling = false;
     std::vector<cudaEvent_t> ev_pool;     // pairs: start, stop
@@ -99,8 +108,10 @@ Tiling make_tiling(const wri_ctx* c, int nb) {
     return t;
 }
 
+constexpr int kMaxCtas = 512;          // upper bound on the persistent grid (>= SM count)
+
 struct WsLayout {
-    size_t U, V, W, U_bot, partials, Xs, Ds, tols, res, its, total;
+    size_t U, V, W, U_bot, partials, partials_tma, Xs, Ds, tols, res, its, total;
 };
 WsLayout ws_layout(const wri_ctx* c, int nb, int host_staging, int maxit_cap) {
     WsLayout L{};
@@ -113,6 +124,7 @@ WsLayout ws_layout(const wri_ctx* c, int nb, int host_staging, int maxit_cap) {
     L.W = o; o += vec;
     L.U_bot = o; o += bot;
     L.partials = o; o += align_up(t.n_tiles * nb * sizeof(double), 256);
+    L.partials_tma = o; o += align_up((size_t)kMaxCtas * nb * sizeof(double), 256);
     if (host_staging) {
         L.Xs = o; o += vec;
         L.Ds = o; o += bot;
@@ -195,6 +207,176 @@ int launch_scalars(wri_ctx* c, const float2* d) {
     c->launches++;
     CK(cudaGetLastError());
     return WRI_OK;
+}
+
+
+// ---- TMA path -------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
+                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                  CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void* ptr = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)ptr;
+    }
+    return fn;
+}
+
+// 4-D view (column, x, y, z) of a source-interleaved complex64 vector; one element = 8 bytes.
+// Out-of-range box elements are zero-filled (the Dirichlet closure of the stencil).
+int make_tmap(CUtensorMap* tm, const void* base, const wri_ctx* c, int nb, int cb, int bx, int by) {
+    EncodeTiledFn fn = get_encode_fn();
+    if (!fn) return cuda_fail(cudaErrorNotSupported, "cuTensorMapEncodeTiled lookup");
+    cuuint64_t gdim[4] = {(cuuint64_t)nb, (cuuint64_t)c->g.nx, (cuuint64_t)c->g.ny, (cuuint64_t)c->g.nz};
+    cuuint64_t gstr[3] = {(cuuint64_t)nb * 8, (cuuint64_t)nb * 8 * c->g.nx,
+                          (cuuint64_t)nb * 8 * c->g.nx * c->g.ny};
+    cuuint32_t box[4] = {(cuuint32_t)cb, (cuuint32_t)bx, (cuuint32_t)by, 1};
+    cuuint32_t estr[4] = {1, 1, 1, 1};
+    CUresult r = fn(tm, CU_TENSOR_MAP_DATA_TYPE_UINT64, 4, const_cast<void*>(base), gdim, gstr, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                    CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        snprintf(g_cuda_msg, sizeof g_cuda_msg, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+        return WRI_ERR_CUDA;
+    }
+    return WRI_OK;
+}
+
+typedef TileCfg<64, 4, 4> Cfg64;
+typedef TileCfg<32, 8, 4> Cfg32;
+typedef TileCfg<16, 8, 8> Cfg16;
+
+int tma_chunk_for(int nb) {
+    const char* off = getenv("WRI_NO_TMA");
+    if (off && off[0] == '1') return 0;
+    if (nb % 64 == 0) return 64;
+    if (nb % 32 == 0) return 32;
+    if (nb % 16 == 0) return 16;
+    return 0;
+}
+
+template <class Cfg, int MODE>
+size_t tma_smem_bytes(int nb) {
+    return (size_t)PassTraits<MODE>::NSTAGE * (Cfg::IN_BYTES + PassTraits<MODE>::NSTREAM * Cfg::CTR_BYTES) +
+           2 * PassTraits<MODE>::NSTAGE * 8 + (size_t)nb * 8 + (size_t)Cfg::NT * 2 * 8;
+}
+
+// tiling + tensor maps for the solve that is starting
+int tma_setup(wri_ctx* c) {
+    c->tma_cb = tma_chunk_for(c->nb);
+    if (!c->tma_cb) return WRI_OK;
+    if (!get_encode_fn()) { c->tma_cb = 0; return WRI_OK; }
+    int txc, tyc;
+    if (c->tma_cb == 64) { txc = Cfg64::TXC; tyc = Cfg64::TYC; }
+    else if (c->tma_cb == 32) { txc = Cfg32::TXC; tyc = Cfg32::TYC; }
+    else { txc = Cfg16::TXC; tyc = Cfg16::TYC; }
+    c->tma_nchunk = c->nb / c->tma_cb;
+    c->tma_ntx = (c->g.nx + txc - 1) / txc;
+    c->tma_nty = (c->g.ny + tyc - 1) / tyc;
+    const long long per_plane = (long long)c->tma_nchunk * c->tma_ntx * c->tma_nty;
+    int zc = std::min(c->g.nz, 32);
+    const char* zenv = getenv("WRI_ZC");
+    if (zenv && atoi(zenv) > 0) zc = std::min(c->g.nz, atoi(zenv));
+    else
+        while (zc > 8 && per_plane * ((c->g.nz + zc - 1) / zc) < 16LL * c->num_sms) zc = (zc + 1) / 2;
+    c->tma_zc = zc;
+    c->tma_ntz = (c->g.nz + zc - 1) / zc;
+    const long long tiles = per_plane * c->tma_ntz;
+    if (tiles > 0x7fffffffLL) { c->tma_cb = 0; return WRI_OK; }
+    c->tma_tiles = (int)tiles;
+    c->tma_grid = (int)std::min<long long>(tiles, std::min(c->num_sms, kMaxCtas));
+    int rc;
+    if ((rc = make_tmap(&c->tmU_halo, c->U, c, c->nb, c->tma_cb, txc + 2, tyc + 2))) return rc;
+    if ((rc = make_tmap(&c->tmV_halo, c->V, c, c->nb, c->tma_cb, txc + 2, tyc + 2))) return rc;
+    if ((rc = make_tmap(&c->tmU_ctr, c->U, c, c->nb, c->tma_cb, txc, tyc))) return rc;
+    if ((rc = make_tmap(&c->tmV_ctr, c->V, c, c->nb, c->tma_cb, txc, tyc))) return rc;
+    if ((rc = make_tmap(&c->tmW_ctr, c->W, c, c->nb, c->tma_cb, txc, tyc))) return rc;
+    if ((rc = make_tmap(&c->tmX_ctr, c->X, c, c->nb, c->tma_cb, txc, tyc))) return rc;
+    return WRI_OK;
+}
+
+ScalParams scal_params(const wri_ctx* c, const double* partials, int n_rows, const float2* d) {
+    ScalParams s{};
+    s.partials = partials;
+    s.n_tiles = n_rows;
+    s.nb = c->nb; s.nb_max = c->nb_max;
+    s.n_rec = c->n_rec; s.rec = c->rec;
+    s.V = c->V; s.U_bot = c->U_bot; s.d = d;
+    s.coef = c->coef; s.stat = c->stat; s.active = c->active; s.iters = c->iters;
+    s.tol = c->tol; s.resnorms = c->resnorms; s.iters_out = c->iters_out;
+    s.k = c->k; s.maxit = c->maxit; s.lambda = c->lambda;
+    return s;
+}
+
+template <class Cfg, int MODE>
+int launch_tma_cfg(wri_ctx* c, int phase) {
+    static size_t attr_bytes = 0;
+    const size_t smem = tma_smem_bytes<Cfg, MODE>(c->nb);
+    if (smem > attr_bytes) {
+        CK(cudaFuncSetAttribute(k_pass_tma<Cfg, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_bytes = smem;
+    }
+    const size_t NM = c->nb_max;
+    TmaPassParams p{};
+    p.m = c->m;
+    p.gx = c->gtab; p.gy = c->gtab + c->g.nx; p.gz = c->gtab + c->g.nx + c->g.ny;
+    p.w2 = c->coef + C_W2 * NM;
+    p.partials = c->partials_tma; p.counter = c->counter;
+    p.nx = c->g.nx; p.ny = c->g.ny; p.nz = c->g.nz; p.nb = c->nb;
+    p.zc = c->tma_zc; p.ntx = c->tma_ntx; p.nty = c->tma_nty; p.ntz = c->tma_ntz;
+    p.nchunk = c->tma_nchunk; p.n_tiles = c->tma_tiles;
+    p.ih2 = (float)(1.0 / (c->h * c->h));
+    p.m6ih2 = (float)(-6.0 / (c->h * c->h));
+    p.phase = phase;
+    p.fin = scal_params(c, c->partials_tma, c->tma_grid, nullptr);
+    const CUtensorMap *tin, *told;
+    if (MODE == MODE_F) {
+        p.out = c->U; p.W = c->W; p.X = c->X; p.sgn = 1.f;
+        p.ca = c->coef + C_CA_F * NM; p.cb = c->coef + C_CB_F * NM; p.cv = c->coef + C_CV_F * NM;
+        p.cx = c->coef + C_CX * NM; p.cw = c->coef + C_CW * NM;
+        tin = &c->tmV_halo; told = &c->tmU_ctr;
+    } else {
+        p.out = c->V; p.sgn = -1.f;
+        p.ca = c->coef + C_CA_A * NM; p.cb = c->coef + C_CB_A * NM;
+        p.cv = p.cx = p.cw = p.ca;
+        tin = &c->tmU_halo; told = &c->tmV_ctr;
+    }
+    cudaEvent_t e1 = nullptr;
+    if (c->profiling && phase != PH_INIT_A) {
+        if (c->ev_used * 2 == c->ev_pool.size()) {
+            cudaEvent_t a, b;
+            CK(cudaEventCreate(&a));
+            CK(cudaEventCreate(&b));
+            c->ev_pool.push_back(a); c->ev_pool.push_back(b); c->ev_kind.push_back(0);
+        }
+        cudaEvent_t e0 = c->ev_pool[2 * c->ev_used];
+        e1 = c->ev_pool[2 * c->ev_used + 1];
+        c->ev_kind[c->ev_used] = (MODE == MODE_F) ? 0 : 1;
+        c->ev_used++;
+        CK(cudaEventRecord(e0, c->stream));
+    }
+    k_pass_tma<Cfg, MODE><<<c->tma_grid, Cfg::NT + 32, smem, c->stream>>>(*tin, *told, c->tmW_ctr, c->tmX_ctr, p);
+    c->launches++;
+    CK(cudaGetLastError());
+    if (e1) CK(cudaEventRecord(e1, c->stream));
+    return WRI_OK;
+}
+
+template <int MODE>
+int launch_tma(wri_ctx* c, int phase) {
+    switch (c->tma_cb) {
+        case 64: return launch_tma_cfg<Cfg64, MODE>(c, phase);
+        case 32: return launch_tma_cfg<Cfg32, MODE>(c, phase);
+        default: return launch_tma_cfg<Cfg16, MODE>(c, phase);
+    }
 }
 
 int check_batch_args(const wri_ctx* c, int nb) {
@@ -292,6 +474,13 @@ int wri_create(wri_ctx** out, wri_grid grid, double h, int32_t n_omega, const do
     CKC(cudaMalloc(&c->iters, nb_max * sizeof(int)));
     CKC(cudaMemset(c->active, 0, nb_max * sizeof(int)));
     CKC(cudaMemset(c->iters, 0, nb_max * sizeof(int)));
+    CKC(cudaMalloc(&c->counter, sizeof(unsigned int)));
+    CKC(cudaMemset(c->counter, 0, sizeof(unsigned int)));
+    {
+        int dev = 0;
+        CKC(cudaGetDevice(&dev));
+        CKC(cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev));
+    }
 #undef CKC
     *out = c;
     return WRI_OK;
@@ -300,7 +489,7 @@ int wri_create(wri_ctx** out, wri_grid grid, double h, int32_t n_omega, const do
 int wri_destroy(wri_ctx* c) {
     if (!c) return WRI_OK;
     cudaFree(c->gtab); cudaFree(c->rec); cudaFree(c->coef); cudaFree(c->stat);
-    cudaFree(c->active); cudaFree(c->iters);
+    cudaFree(c->active); cudaFree(c->iters); cudaFree(c->counter);
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
     delete c;
     return WRI_OK;
@@ -409,9 +598,11 @@ int wri_lsqr_begin(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const 
     c->U = (float2*)(c->ws + L.U); c->V = (float2*)(c->ws + L.V); c->W = (float2*)(c->ws + L.W);
     c->U_bot = (float2*)(c->ws + L.U_bot);
     c->partials = (double*)(c->ws + L.partials);
+    c->partials_tma = (double*)(c->ws + L.partials_tma);
     c->X = (float2*)u_out_dev;
     c->tol = tol_dev; c->resnorms = resnorms_dev; c->iters_out = iters_dev;
     c->tl = make_tiling(c, nb);
+    if ((rc = tma_setup(c))) return rc;
     const size_t vbytes = c->ng * (size_t)nb * sizeof(float2);
     const size_t NM = c->nb_max;
 
@@ -426,10 +617,14 @@ int wri_lsqr_begin(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const 
     CK(cudaMemsetAsync(c->V, 0, vbytes, c->stream));
     if ((rc = launch_scalars<PH_INIT_B>(c, (const float2*)d_dev))) return rc;
     // alpha1 v1 = M^H u1
-    p.in = c->U; p.out = c->V; p.sgn = -1.f;
-    p.ca = c->coef + C_CA_A * NM; p.cb = c->coef + C_CB_A * NM;
-    if ((rc = launch_pass<MODE_A>(c, p, c->tl))) return rc;
-    if ((rc = launch_scalars<PH_INIT_A>(c, nullptr))) return rc;
+    if (c->tma_cb) {
+        if ((rc = launch_tma<MODE_A>(c, PH_INIT_A))) return rc;
+    } else {
+        p.in = c->U; p.out = c->V; p.sgn = -1.f;
+        p.ca = c->coef + C_CA_A * NM; p.cb = c->coef + C_CB_A * NM;
+        if ((rc = launch_pass<MODE_A>(c, p, c->tl))) return rc;
+        if ((rc = launch_scalars<PH_INIT_A>(c, nullptr))) return rc;
+    }
     c->solving = true;
     return WRI_OK;
 }
@@ -442,6 +637,12 @@ int wri_lsqr_iterate(wri_ctx* c, int32_t n_steps) {
     int rc;
     for (int i = 0; i < n_steps; ++i) {
         c->k++;
+        if (c->tma_cb) {
+            // two launches per iteration: the last CTA of each pass runs the scalar recurrences
+            if ((rc = launch_tma<MODE_F>(c, PH_F))) return rc;
+            if ((rc = launch_tma<MODE_A>(c, PH_A))) return rc;
+            continue;
+        }
         PassParams p = base_params(c, c->nb, c->tl);
         p.partials = c->partials;
         // pass F: U <- (lambda/alpha) A V - (alpha/beta) U ; deferred x, w updates

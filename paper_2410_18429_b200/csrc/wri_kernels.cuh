@@ -283,7 +283,7 @@ __device__ __forceinline__ void reduce_partials(const ScalParams& p, double* scr
         const int Gc = max(1, T / ncol);
         double a = 0.0;
         if (g < Gc)
-            for (int b = g; b < p.n_tiles; b += Gc) a += p.partials[(size_t)b * nb + s];
+            for (int b = g; b < p.n_tiles; b += Gc) a += __ldcg(p.partials + (size_t)b * nb + s);
         scratch[threadIdx.x] = a;
         __syncthreads();
         if (threadIdx.x < ncol) {
@@ -320,10 +320,10 @@ __device__ __forceinline__ void add_receiver_norms(const ScalParams& p, double* 
     }
 }
 
+// Runs in ONE block (any size): the standalone k_scalars kernel, or the last CTA of the
+// persistent pass kernel.  sh: (blockDim.x + nb) doubles of shared memory.
 template <int PHASE>
-__global__ void __launch_bounds__(1024)
-k_scalars(const ScalParams p) {
-    extern __shared__ double sh[];
+__device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) {
     double* scratch = sh;                   // [blockDim.x]
     double* colsum = sh + blockDim.x;       // [nb]
     const int nb = p.nb, NM = p.nb_max;
@@ -452,6 +452,13 @@ k_scalars(const ScalParams p) {
             }
         }
     }
+}
+
+template <int PHASE>
+__global__ void __launch_bounds__(1024)
+k_scalars(const ScalParams p) {
+    extern __shared__ double sh_scal[];
+    finalize_phase<PHASE>(p, sh_scal);
 }
 
 }  // namespace wri

@@ -1,0 +1,333 @@
+// wri_tma.cuh — persistent, TMA-fed stencil + LSQR pass for sm_100a (the hot kernel).
+//
+// One CTA per SM walks a fixed (static round-robin) list of tiles.  A tile is TXC x TYC cells
+// x CB batch columns, marched over zc planes.  A producer warp streams, per plane p,
+//     the stencil input tile with a one-cell x/y halo      box (CB, TXC+2, TYC+2, 1)
+//     the in-place streams of plane p-1 (old | W | X)      box (CB, TXC,   TYC,   1)
+// into a ring of shared-memory stages with cp.async.bulk.tensor (TMA).  Out-of-grid halo cells
+// and planes -1 / nz are zero-filled by the TMA unit, which IS the Dirichlet closure of the
+// 7-point stencil — no boundary branches in the kernel.  256 consumer threads keep the z
+// pipeline (c_{z-1}, c_z, in-plane neighbour sum n_z) in registers, so every stage is consumed
+// entirely at its own step, and write results straight to HBM with 128-bit stores.
+//
+// The squared-norm partials are accumulated per column in a fixed order (thread -> tile ->
+// CTA row of partials[]); the last CTA to finish reduces the rows, runs the per-column scalar
+// recurrences and the receiver rows (finalize_phase), so an LSQR iteration is two launches.
+#pragma once
+#include <cuda.h>
+#include "wri_kernels.cuh"
+
+namespace wri {
+
+template <int CB_, int TXC_, int TYC_>
+struct TileCfg {
+    static constexpr int CB = CB_, TXC = TXC_, TYC = TYC_;
+    static constexpr int NT = 256;                              // consumer threads
+    static constexpr int ITEMS = TXC * TYC * CB / 2;            // 16-byte items per plane
+    static constexpr int IPT = ITEMS / NT;                      // items per thread
+    static constexpr int IN_BYTES = (TXC + 2) * (TYC + 2) * CB * 8;
+    static constexpr int CTR_BYTES = TXC * TYC * CB * 8;
+    static_assert(ITEMS % NT == 0, "tile must give every consumer thread the same work");
+    static_assert(NT % (CB / 2) == 0, "a thread must keep one column pair");
+    static_assert(IN_BYTES % 128 == 0 && CTR_BYTES % 128 == 0, "TMA destinations need 128 B alignment");
+};
+
+template <int MODE> struct PassTraits;
+template <> struct PassTraits<MODE_F> { static constexpr int NSTREAM = 3, NSTAGE = 4; };
+template <> struct PassTraits<MODE_A> { static constexpr int NSTREAM = 1, NSTAGE = 6; };
+
+struct TmaPassParams {
+    float2* out;           // result vector (its old values arrive through tm_old)
+    float2* W;
+    float2* X;
+    const float* m;
+    const float *gx, *gy, *gz;
+    const float *w2, *ca, *cb, *cv, *cx, *cw;
+    double* partials;      // [gridDim.x][nb]
+    unsigned int* counter; // last-block ticket
+    int nx, ny, nz, nb;
+    int zc, ntx, nty, ntz, nchunk, n_tiles;
+    float ih2, m6ih2, sgn;
+    int phase;             // ScalPhase run by the last CTA
+    ScalParams fin;
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra LAB_DONE;\n"
+        "bra LAB_WAIT;\n"
+        "LAB_DONE:\n"
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* tm, uint32_t bar,
+                                            int c0, int c1, int c2, int c3) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes"
+        " [%0], [%1, {%3, %4, %5, %6}], [%2];" ::"r"(dst), "l"(tm), "r"(bar),
+        "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
+__device__ __forceinline__ void consumer_sync(int nthreads) {
+    asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory");
+}
+__device__ __forceinline__ float4 lds128(const unsigned char* base, int byte_off) {
+    return *reinterpret_cast<const float4*>(base + byte_off);
+}
+
+template <class Cfg, int MODE>
+__global__ void __launch_bounds__(Cfg::NT + 32, 1)
+k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUtensorMap tm_old,
+           const __grid_constant__ CUtensorMap tm_w, const __grid_constant__ CUtensorMap tm_x,
+           const TmaPassParams p) {
+    constexpr int CB = Cfg::CB, TXC = Cfg::TXC, TYC = Cfg::TYC, NT = Cfg::NT, IPT = Cfg::IPT;
+    constexpr int NSTREAM = PassTraits<MODE>::NSTREAM, NSTAGE = PassTraits<MODE>::NSTAGE;
+    constexpr int STAGE_BYTES = Cfg::IN_BYTES + NSTREAM * Cfg::CTR_BYTES;
+    constexpr int HP = CB / 2;                                  // column pairs per cell
+    constexpr int ROW_B = (TXC + 2) * CB * 8;                   // bytes per halo-tile row
+    constexpr int CELL_B = CB * 8;
+
+    extern __shared__ __align__(128) unsigned char smem[];
+    unsigned char* stages = smem;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + NSTAGE * STAGE_BYTES);   // full[NSTAGE], empty[NSTAGE]
+    double* colacc = reinterpret_cast<double*>(bars + 2 * NSTAGE);               // [nb]
+    double* red = colacc + p.nb;                                                  // [NT*2]
+    __shared__ unsigned int s_ticket;
+
+    const int tid = threadIdx.x;
+    const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + NSTAGE);
+
+    if (tid == 0) {
+        for (int s = 0; s < NSTAGE; ++s) {
+            mbar_init(full0 + 8 * s, 1);
+            mbar_init(empty0 + 8 * s, NT / 32);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    for (int j = tid; j < p.nb; j += blockDim.x) colacc[j] = 0.0;
+    __syncthreads();
+
+    if (tid >= NT) {
+        // ------------------------------------------------------------------ producer warp
+        // (all 32 lanes walk the loops together; lane 0 issues)
+        const bool issuer = (tid == NT);
+        int stage = 0;
+        uint32_t phase = 0;
+        for (int t = blockIdx.x; t < p.n_tiles; t += gridDim.x) {
+            int r = t;
+            const int chunk = r % p.nchunk; r /= p.nchunk;
+            const int tx = r % p.ntx; r /= p.ntx;
+            const int ty = r % p.nty;
+            const int tz = r / p.nty;
+            const int z0 = tz * p.zc, z1 = min(z0 + p.zc, p.nz);
+            const int c0 = chunk * CB, x0 = tx * TXC, y0 = ty * TYC;
+            for (int pl = z0 - 1; pl <= z1; ++pl) {
+                if (issuer) {
+                    mbar_wait(empty0 + 8 * stage, phase ^ 1);
+                    const bool streams = pl >= z0 + 1;
+                    const uint32_t fb = full0 + 8 * stage;
+                    mbar_expect_tx(fb, Cfg::IN_BYTES + (streams ? NSTREAM * Cfg::CTR_BYTES : 0));
+                    const uint32_t dst = smem_u32(stages + stage * STAGE_BYTES);
+                    tma_load_4d(dst, &tm_in, fb, c0, x0 - 1, y0 - 1, pl);
+                    if (streams) {
+                        tma_load_4d(dst + Cfg::IN_BYTES, &tm_old, fb, c0, x0, y0, pl - 1);
+                        if (MODE == MODE_F) {
+                            tma_load_4d(dst + Cfg::IN_BYTES + Cfg::CTR_BYTES, &tm_w, fb, c0, x0, y0, pl - 1);
+                            tma_load_4d(dst + Cfg::IN_BYTES + 2 * Cfg::CTR_BYTES, &tm_x, fb, c0, x0, y0, pl - 1);
+                        }
+                    }
+                }
+                __syncwarp();
+                if (++stage == NSTAGE) { stage = 0; phase ^= 1; }
+            }
+        }
+    } else {
+        // ------------------------------------------------------------------ consumers
+        const int cp = tid % HP;                                // column pair within the chunk
+        int stage = 0;
+        uint32_t phase = 0;
+        // static item geometry: item j of this thread is cell (cxj, cyj) of the tile
+        int sm_ctr[IPT];                                        // byte offset of the centre in the halo tile
+        int cxj[IPT], cyj[IPT];
+#pragma unroll
+        for (int j = 0; j < IPT; ++j) {
+            const int cell = (tid + j * NT) / HP;
+            cxj[j] = cell % TXC;
+            cyj[j] = cell / TXC;
+            sm_ctr[j] = (cyj[j] + 1) * ROW_B + (cxj[j] + 1) * CELL_B + cp * 16;
+        }
+
+        for (int t = blockIdx.x; t < p.n_tiles; t += gridDim.x) {
+            int r = t;
+            const int chunk = r % p.nchunk; r /= p.nchunk;
+            const int tx = r % p.ntx; r /= p.ntx;
+            const int ty = r % p.nty;
+            const int tz = r / p.nty;
+            const int z0 = tz * p.zc, z1 = min(z0 + p.zc, p.nz);
+            const int col = chunk * CB + cp * 2;
+
+            float w2[2], ca[2], cb[2], cv[2], cx[2], cw[2];
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                w2[e] = p.w2[col + e]; ca[e] = p.ca[col + e]; cb[e] = p.cb[col + e];
+                cv[e] = (MODE == MODE_F) ? p.cv[col + e] : 0.f;
+                cx[e] = (MODE == MODE_F) ? p.cx[col + e] : 0.f;
+                cw[e] = (MODE == MODE_F) ? p.cw[col + e] : 0.f;
+            }
+            bool valid[IPT];
+            float gxy[IPT], m_cur[IPT], m_nxt[IPT];
+            size_t goff[IPT];                                   // element offset of (cell, z0) in the vectors
+            size_t moff[IPT];
+            float4 c_prev[IPT], c_cur[IPT], n_cur[IPT];
+#pragma unroll
+            for (int j = 0; j < IPT; ++j) {
+                const int ix = tx * TXC + cxj[j], iy = ty * TYC + cyj[j];
+                valid[j] = ix < p.nx && iy < p.ny;
+                const int ixc = min(ix, p.nx - 1), iyc = min(iy, p.ny - 1);
+                gxy[j] = fmaxf(p.gx[ixc], p.gy[iyc]);
+                moff[j] = ((size_t)z0 * p.ny + iyc) * p.nx + ixc;
+                goff[j] = (((size_t)z0 * p.ny + iyc) * p.nx + ixc) * p.nb + col;
+                m_cur[j] = 0.f;
+                m_nxt[j] = 0.f;
+                c_prev[j] = c_cur[j] = n_cur[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+            }
+            double acc[2] = {0.0, 0.0};
+            const size_t plane_e = (size_t)p.nx * p.ny * p.nb;
+            const size_t plane_m = (size_t)p.nx * p.ny;
+
+            for (int pl = z0 - 1; pl <= z1; ++pl) {
+                // model value of plane pl (used one step later), issued before the wait
+                if (pl >= z0 && pl < z1) {
+#pragma unroll
+                    for (int j = 0; j < IPT; ++j) m_nxt[j] = __ldg(p.m + moff[j] + (size_t)(pl - z0) * plane_m);
+                }
+                mbar_wait(full0 + 8 * stage, phase);
+                const unsigned char* sb = stages + stage * STAGE_BYTES;
+                float4 c_new[IPT], n_new[IPT], o_old[IPT], o_w[IPT], o_x[IPT];
+                const bool emit = pl >= z0 + 1;
+#pragma unroll
+                for (int j = 0; j < IPT; ++j) {
+                    c_new[j] = lds128(sb, sm_ctr[j]);
+                    const float4 a = lds128(sb, sm_ctr[j] - CELL_B), b = lds128(sb, sm_ctr[j] + CELL_B);
+                    const float4 c = lds128(sb, sm_ctr[j] - ROW_B), d = lds128(sb, sm_ctr[j] + ROW_B);
+                    n_new[j] = make_float4((a.x + b.x) + (c.x + d.x), (a.y + b.y) + (c.y + d.y),
+                                           (a.z + b.z) + (c.z + d.z), (a.w + b.w) + (c.w + d.w));
+                    if (emit) {
+                        const int io = Cfg::IN_BYTES + (tid + j * NT) * 16;
+                        o_old[j] = lds128(sb, io);
+                        if (MODE == MODE_F) {
+                            o_w[j] = lds128(sb, io + Cfg::CTR_BYTES);
+                            o_x[j] = lds128(sb, io + 2 * Cfg::CTR_BYTES);
+                        }
+                    }
+                }
+                __syncwarp();
+                if ((tid & 31) == 0) mbar_arrive(empty0 + 8 * stage);
+                if (++stage == NSTAGE) { stage = 0; phase ^= 1; }
+
+                if (emit) {
+                    const int z = pl - 1;
+                    const float gzv = p.gz[z];
+#pragma unroll
+                    for (int j = 0; j < IPT; ++j) {
+                        const float g = fmaxf(gxy[j], gzv);
+                        const float4 cc = c_cur[j];
+                        // neighbour sums (x, y from this plane; z from the planes before / after)
+                        const float s0 = n_cur[j].x + (c_prev[j].x + c_new[j].x);
+                        const float s1 = n_cur[j].y + (c_prev[j].y + c_new[j].y);
+                        const float s2 = n_cur[j].z + (c_prev[j].z + c_new[j].z);
+                        const float s3 = n_cur[j].w + (c_prev[j].w + c_new[j].w);
+                        float4 rr;
+                        {
+                            const float wm = w2[0] * m_cur[j];
+                            const float dr = wm + p.m6ih2, di = p.sgn * wm * g;
+                            const float ar = fmaf(p.ih2, s0, fmaf(dr, cc.x, -di * cc.y));
+                            const float ai = fmaf(p.ih2, s1, fmaf(dr, cc.y, di * cc.x));
+                            rr.x = fmaf(ca[0], ar, -cb[0] * o_old[j].x);
+                            rr.y = fmaf(ca[0], ai, -cb[0] * o_old[j].y);
+                        }
+                        {
+                            const float wm = w2[1] * m_cur[j];
+                            const float dr = wm + p.m6ih2, di = p.sgn * wm * g;
+                            const float ar = fmaf(p.ih2, s2, fmaf(dr, cc.z, -di * cc.w));
+                            const float ai = fmaf(p.ih2, s3, fmaf(dr, cc.w, di * cc.z));
+                            rr.z = fmaf(ca[1], ar, -cb[1] * o_old[j].z);
+                            rr.w = fmaf(ca[1], ai, -cb[1] * o_old[j].w);
+                        }
+                        if (valid[j]) {
+                            const size_t off = goff[j] + (size_t)(z - z0) * plane_e;
+                            *reinterpret_cast<float4*>(p.out + off) = rr;
+                            acc[0] += (double)fmaf(rr.x, rr.x, rr.y * rr.y);
+                            acc[1] += (double)fmaf(rr.z, rr.z, rr.w * rr.w);
+                            if (MODE == MODE_F) {
+                                float4 xn, wn;
+                                xn.x = fmaf(cx[0], o_w[j].x, o_x[j].x);
+                                xn.y = fmaf(cx[0], o_w[j].y, o_x[j].y);
+                                xn.z = fmaf(cx[1], o_w[j].z, o_x[j].z);
+                                xn.w = fmaf(cx[1], o_w[j].w, o_x[j].w);
+                                wn.x = fmaf(cv[0], cc.x, -cw[0] * o_w[j].x);
+                                wn.y = fmaf(cv[0], cc.y, -cw[0] * o_w[j].y);
+                                wn.z = fmaf(cv[1], cc.z, -cw[1] * o_w[j].z);
+                                wn.w = fmaf(cv[1], cc.w, -cw[1] * o_w[j].w);
+                                *reinterpret_cast<float4*>(p.X + off) = xn;
+                                *reinterpret_cast<float4*>(p.W + off) = wn;
+                            }
+                        }
+                    }
+                }
+#pragma unroll
+                for (int j = 0; j < IPT; ++j) {
+                    c_prev[j] = c_cur[j]; c_cur[j] = c_new[j]; n_cur[j] = n_new[j];
+                    m_cur[j] = m_nxt[j];
+                }
+            }
+            // fold this tile's per-thread sums into the CTA's per-column sums, fixed order
+            red[tid * 2] = acc[0];
+            red[tid * 2 + 1] = acc[1];
+            consumer_sync(NT);
+            if (tid < CB) {
+                const int e = tid & 1, c2 = tid >> 1;
+                double s = 0.0;
+#pragma unroll 4
+                for (int k = 0; k < NT / HP; ++k) s += red[(c2 + k * HP) * 2 + e];
+                colacc[chunk * CB + tid] += s;
+            }
+            consumer_sync(NT);
+        }
+    }
+
+    // ---------------------------------------------------------------------- CTA epilogue
+    __syncthreads();
+    for (int j = tid; j < p.nb; j += blockDim.x) p.partials[(size_t)blockIdx.x * p.nb + j] = colacc[j];
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) s_ticket = atomicAdd(p.counter, 1u);
+    __syncthreads();
+    if (s_ticket == gridDim.x - 1) {
+        __threadfence();
+        double* sh = reinterpret_cast<double*>(smem);           // stages are idle now
+        switch (p.phase) {
+            case PH_INIT_A: finalize_phase<PH_INIT_A>(p.fin, sh); break;
+            case PH_F:      finalize_phase<PH_F>(p.fin, sh); break;
+            default:        finalize_phase<PH_A>(p.fin, sh); break;
+        }
+        __syncthreads();
+        if (tid == 0) *p.counter = 0u;
+    }
+}
+
+}  // namespace wri

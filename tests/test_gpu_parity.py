@@ -95,6 +95,11 @@ TF_CASES = [
     ("config1", dict(grid=(24, 20, 28), nb=4), 10),
     ("config2", dict(grid=(20, 33, 18), nb=3), 10),
     ("config3", dict(grid=(40, 40, 32), nb=6), 10),
+    # persistent TMA kernel: column chunks of 64 / 32 / 16, ragged tiles, mixed frequencies
+    ("config2", dict(grid=(21, 18, 37), nb=64), 5),
+    ("config4", dict(grid=(19, 22, 35), nb=32), 5),
+    ("config3", dict(grid=(27, 25, 20), nb=48), 5),
+    ("config1", dict(grid=(32, 32, 32), nb=16), 5),
 ]
 
 
@@ -178,14 +183,17 @@ def test_free_running_config1_50_iterations(torch_cuda):
         assert rel(u[:, j], ref["x"][:, j]) < 1e-3
 
 
-@pytest.mark.parametrize("name,kw", [
-    ("config2", dict(grid=(40, 36, 44), nb=6)),
-    ("config4", dict(grid=(48, 48, 48), nb=8)),
-    ("config3", dict(grid=(50, 50, 40), nb=12)),
+@pytest.mark.parametrize("name,kw,cols", [
+    ("config2", dict(grid=(40, 36, 44), nb=6), None),
+    ("config4", dict(grid=(48, 48, 48), nb=8), None),
+    ("config3", dict(grid=(50, 50, 40), nb=12), None),
+    ("config2", dict(grid=(45, 38, 70), nb=64), [0, 21, 42, 63]),      # TMA path, 3 z-chunks
+    ("config4", dict(grid=(40, 44, 36), nb=32), [0, 13, 31]),
+    ("config3", dict(grid=(50, 50, 40), nb=48), [0, 17, 47]),
 ])
-def test_free_running_scaled_configs(torch_cuda, name, kw):
+def test_free_running_scaled_configs(torch_cuda, name, kw, cols):
     w = workloads.make(name, **kw)
-    u, res, it, ref = _free_run(torch_cuda, w, 50)
+    u, res, it, ref = _free_run(torch_cuda, w, 50, cols=cols)
     for j in range(u.shape[1]):
         assert rel(res[:, j], ref["resnorms"][:, j]) < 1e-3
         assert rel(u[:, j], ref["x"][:, j]) < 1e-3
