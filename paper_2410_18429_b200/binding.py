@@ -45,7 +45,8 @@ _lib = None
 
 
 def lib_path() -> str:
-    return os.path.join(_HERE, "libwri.so")
+    # WRI_LIB: developer override to load a tuning variant built with build.build(out=...)
+    return os.environ.get("WRI_LIB") or os.path.join(_HERE, "libwri.so")
 
 
 def load_library():

@@ -73,9 +73,12 @@ struct wri_ctx {
     int num_sms = 0;
     unsigned int* counter = nullptr;      // last-CTA ticket (device)
     int tma_cb = 0;                       // 0 = not used for this solve
-    int tma_zc = 0, tma_ntx = 0, tma_nty = 0, tma_ntz = 0, tma_nchunk = 0, tma_tiles = 0, tma_grid = 0;
-    double* partials_tma = nullptr;       // [tma_grid][nb]
-    CUtensorMap tmU_halo{}, tmV_halo{}, tmU_ctr{}, tmV_ctr{}, tmW_ctr{}, tmX_ctr{};
+    struct TmaPlan {                      // one per pass (tile shapes may differ between F and A)
+        int txc = 0, tyc = 0, ntx = 0, nty = 0, ntz = 0, zc = 0, nchunk = 0, tiles = 0, grid = 0;
+        CUtensorMap in{}, old{}, w{}, x{}, m{};
+        int m_tma = 0;                    // model tile rides in the TMA stage
+    } planF, planA;
+    double* partials_tma = nullptr;       // [grid][nb]
     // optional per-kernel timing (wri_profile_*)
     bool profiling = false;
     std::vector<cudaEvent_t> ev_pool;     // pairs: start, stop
@@ -115,7 +118,8 @@ struct WsLayout {
 };
 WsLayout ws_layout(const wri_ctx* c, int nb, int host_staging, int maxit_cap) {
     WsLayout L{};
-    const size_t vec = align_up(c->ng * (size_t)nb * sizeof(float2), 256);
+    size_t vec = align_up(c->ng * (size_t)nb * sizeof(float2), 256);
+    if (const char* e = getenv("WRI_PAD")) vec += (size_t)atoll(e);
     const size_t bot = align_up((size_t)std::max(c->n_rec, 1) * nb * sizeof(float2), 256);
     const Tiling t = make_tiling(c, nb);
     size_t o = 0;
@@ -240,9 +244,11 @@ int make_tmap(CUtensorMap* tm, const void* base, const wri_ctx* c, int nb, int c
                           (cuuint64_t)nb * 8 * c->g.nx * c->g.ny};
     cuuint32_t box[4] = {(cuuint32_t)cb, (cuuint32_t)bx, (cuuint32_t)by, 1};
     cuuint32_t estr[4] = {1, 1, 1, 1};
+    CUtensorMapL2promotion promo = CU_TENSOR_MAP_L2_PROMOTION_L2_256B;
+    if (const char* e = getenv("WRI_L2PROMO")) promo = (CUtensorMapL2promotion)atoi(e);
     CUresult r = fn(tm, CU_TENSOR_MAP_DATA_TYPE_UINT64, 4, const_cast<void*>(base), gdim, gstr, box, estr,
                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                    CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                    promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
         snprintf(g_cuda_msg, sizeof g_cuda_msg, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
         return WRI_ERR_CUDA;
@@ -250,9 +256,32 @@ int make_tmap(CUtensorMap* tm, const void* base, const wri_ctx* c, int nb, int c
     return WRI_OK;
 }
 
-typedef TileCfg<64, 4, 4> Cfg64;
-typedef TileCfg<32, 8, 4> Cfg32;
-typedef TileCfg<16, 8, 8> Cfg16;
+// Tile shapes per column-chunk width and pass.  A tile row is TXC cells = TXC*CB*8 contiguous
+// bytes; TXC*TYC*CB = 1024 complex (F: 512 consumer threads, 1 item each; A: 256 x 2 items).
+#ifndef WRI_F_TX
+#define WRI_F_TX 4
+#endif
+#ifndef WRI_F_TY
+#define WRI_F_TY 4
+#endif
+#ifndef WRI_A_TX
+#define WRI_A_TX 4
+#endif
+#ifndef WRI_A_TY
+#define WRI_A_TY 4
+#endif
+#ifndef WRI_F_NT
+#define WRI_F_NT 512
+#endif
+#ifndef WRI_A_NT
+#define WRI_A_NT 256
+#endif
+template <int CB, int MODE> struct CfgFor {
+    static constexpr int S = 64 / CB;   // narrower chunks -> proportionally more cells per tile row
+    typedef TileCfg<CB, (MODE == MODE_F ? WRI_F_TX : WRI_A_TX) * (S >= 2 ? 2 : 1),
+                    (MODE == MODE_F ? WRI_F_TY : WRI_A_TY) * (S >= 4 ? 2 : 1),
+                    (MODE == MODE_F ? WRI_F_NT : WRI_A_NT)> type;
+};
 
 int tma_chunk_for(int nb) {
     const char* off = getenv("WRI_NO_TMA");
@@ -264,43 +293,81 @@ int tma_chunk_for(int nb) {
 }
 
 template <class Cfg, int MODE>
-size_t tma_smem_bytes(int nb) {
-    return (size_t)PassTraits<MODE>::NSTAGE * (Cfg::IN_BYTES + PassTraits<MODE>::NSTREAM * Cfg::CTR_BYTES) +
-           2 * PassTraits<MODE>::NSTAGE * 8 + (size_t)nb * 8 + (size_t)Cfg::NT * 2 * 8;
+size_t tma_smem_bytes(const wri_ctx* c) {
+    return (size_t)PassTraits<MODE>::NSTAGE *
+               (Cfg::IN_BYTES + PassTraits<MODE>::NSTREAM * Cfg::CTR_BYTES + Cfg::M_BYTES) +
+           2 * PassTraits<MODE>::NSTAGE * 8 + (size_t)c->nb * 8 + (size_t)Cfg::NT * 2 * 8 +
+           (size_t)(c->g.nx + c->g.ny + c->g.nz) * 4 + (size_t)6 * c->nb * 4;
 }
 
-// tiling + tensor maps for the solve that is starting
-int tma_setup(wri_ctx* c) {
-    c->tma_cb = tma_chunk_for(c->nb);
-    if (!c->tma_cb) return WRI_OK;
-    if (!get_encode_fn()) { c->tma_cb = 0; return WRI_OK; }
-    int txc, tyc;
-    if (c->tma_cb == 64) { txc = Cfg64::TXC; tyc = Cfg64::TYC; }
-    else if (c->tma_cb == 32) { txc = Cfg32::TXC; tyc = Cfg32::TYC; }
-    else { txc = Cfg16::TXC; tyc = Cfg16::TYC; }
-    c->tma_nchunk = c->nb / c->tma_cb;
-    c->tma_ntx = (c->g.nx + txc - 1) / txc;
-    c->tma_nty = (c->g.ny + tyc - 1) / tyc;
-    const long long per_plane = (long long)c->tma_nchunk * c->tma_ntx * c->tma_nty;
+// 3-D view (x, y, z) of the float32 model; needs a 16-byte row pitch
+int make_tmap_model(CUtensorMap* tm, const wri_ctx* c, int bx, int by) {
+    EncodeTiledFn fn = get_encode_fn();
+    if (!fn) return cuda_fail(cudaErrorNotSupported, "cuTensorMapEncodeTiled lookup");
+    cuuint64_t gdim[3] = {(cuuint64_t)c->g.nx, (cuuint64_t)c->g.ny, (cuuint64_t)c->g.nz};
+    cuuint64_t gstr[2] = {(cuuint64_t)c->g.nx * 4, (cuuint64_t)c->g.nx * 4 * c->g.ny};
+    cuuint32_t box[3] = {(cuuint32_t)bx, (cuuint32_t)by, 1};
+    cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = fn(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(c->m), gdim, gstr, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                    CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        snprintf(g_cuda_msg, sizeof g_cuda_msg, "cuTensorMapEncodeTiled(model) failed with CUresult %d", (int)r);
+        return WRI_ERR_CUDA;
+    }
+    return WRI_OK;
+}
+
+// tiling + tensor maps of one pass for the solve that is starting
+template <class Cfg>
+int tma_plan(wri_ctx* c, wri_ctx::TmaPlan& P, const void* in, const void* old, bool is_f) {
+    P.txc = Cfg::TXC; P.tyc = Cfg::TYC;
+    P.nchunk = c->nb / Cfg::CB;
+    P.ntx = (c->g.nx + P.txc - 1) / P.txc;
+    P.nty = (c->g.ny + P.tyc - 1) / P.tyc;
+    const long long per_plane = (long long)P.nchunk * P.ntx * P.nty;
     int zc = std::min(c->g.nz, 32);
     const char* zenv = getenv("WRI_ZC");
     if (zenv && atoi(zenv) > 0) zc = std::min(c->g.nz, atoi(zenv));
     else
         while (zc > 8 && per_plane * ((c->g.nz + zc - 1) / zc) < 16LL * c->num_sms) zc = (zc + 1) / 2;
-    c->tma_zc = zc;
-    c->tma_ntz = (c->g.nz + zc - 1) / zc;
-    const long long tiles = per_plane * c->tma_ntz;
-    if (tiles > 0x7fffffffLL) { c->tma_cb = 0; return WRI_OK; }
-    c->tma_tiles = (int)tiles;
-    c->tma_grid = (int)std::min<long long>(tiles, std::min(c->num_sms, kMaxCtas));
+    P.zc = zc;
+    P.ntz = (c->g.nz + zc - 1) / zc;
+    const long long tiles = per_plane * P.ntz;
+    if (tiles > 0x7fffffffLL) return WRI_ERR_ARG;
+    P.tiles = (int)tiles;
+    P.grid = (int)std::min<long long>(tiles, std::min(c->num_sms, kMaxCtas));
     int rc;
-    if ((rc = make_tmap(&c->tmU_halo, c->U, c, c->nb, c->tma_cb, txc + 2, tyc + 2))) return rc;
-    if ((rc = make_tmap(&c->tmV_halo, c->V, c, c->nb, c->tma_cb, txc + 2, tyc + 2))) return rc;
-    if ((rc = make_tmap(&c->tmU_ctr, c->U, c, c->nb, c->tma_cb, txc, tyc))) return rc;
-    if ((rc = make_tmap(&c->tmV_ctr, c->V, c, c->nb, c->tma_cb, txc, tyc))) return rc;
-    if ((rc = make_tmap(&c->tmW_ctr, c->W, c, c->nb, c->tma_cb, txc, tyc))) return rc;
-    if ((rc = make_tmap(&c->tmX_ctr, c->X, c, c->nb, c->tma_cb, txc, tyc))) return rc;
+    if ((rc = make_tmap(&P.in, in, c, c->nb, Cfg::CB, P.txc + 2, P.tyc + 2))) return rc;
+    if ((rc = make_tmap(&P.old, old, c, c->nb, Cfg::CB, P.txc, P.tyc))) return rc;
+    if (is_f) {
+        if ((rc = make_tmap(&P.w, c->W, c, c->nb, Cfg::CB, P.txc, P.tyc))) return rc;
+        if ((rc = make_tmap(&P.x, c->X, c, c->nb, Cfg::CB, P.txc, P.tyc))) return rc;
+    } else {
+        P.w = P.old; P.x = P.old;          // unused by pass A
+    }
+    P.m_tma = (c->g.nx % 4 == 0) && (P.txc % 4 == 0) && aligned16(c->m);
+    if (P.m_tma) { if ((rc = make_tmap_model(&P.m, c, P.txc, P.tyc))) return rc; }
+    else P.m = P.old;                       // unused placeholder
     return WRI_OK;
+}
+
+int tma_setup(wri_ctx* c) {
+    c->tma_cb = tma_chunk_for(c->nb);
+    if (!c->tma_cb) return WRI_OK;
+    if (!get_encode_fn()) { c->tma_cb = 0; return WRI_OK; }
+    int rc;
+    switch (c->tma_cb) {
+        case 64:
+            if ((rc = tma_plan<CfgFor<64, MODE_F>::type>(c, c->planF, c->V, c->U, true))) return rc;
+            return tma_plan<CfgFor<64, MODE_A>::type>(c, c->planA, c->U, c->V, false);
+        case 32:
+            if ((rc = tma_plan<CfgFor<32, MODE_F>::type>(c, c->planF, c->V, c->U, true))) return rc;
+            return tma_plan<CfgFor<32, MODE_A>::type>(c, c->planA, c->U, c->V, false);
+        default:
+            if ((rc = tma_plan<CfgFor<16, MODE_F>::type>(c, c->planF, c->V, c->U, true))) return rc;
+            return tma_plan<CfgFor<16, MODE_A>::type>(c, c->planA, c->U, c->V, false);
+    }
 }
 
 ScalParams scal_params(const wri_ctx* c, const double* partials, int n_rows, const float2* d) {
@@ -319,7 +386,8 @@ ScalParams scal_params(const wri_ctx* c, const double* partials, int n_rows, con
 template <class Cfg, int MODE>
 int launch_tma_cfg(wri_ctx* c, int phase) {
     static size_t attr_bytes = 0;
-    const size_t smem = tma_smem_bytes<Cfg, MODE>(c->nb);
+    const wri_ctx::TmaPlan& P = (MODE == MODE_F) ? c->planF : c->planA;
+    const size_t smem = tma_smem_bytes<Cfg, MODE>(c);
     if (smem > attr_bytes) {
         CK(cudaFuncSetAttribute(k_pass_tma<Cfg, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_bytes = smem;
@@ -331,23 +399,21 @@ int launch_tma_cfg(wri_ctx* c, int phase) {
     p.w2 = c->coef + C_W2 * NM;
     p.partials = c->partials_tma; p.counter = c->counter;
     p.nx = c->g.nx; p.ny = c->g.ny; p.nz = c->g.nz; p.nb = c->nb;
-    p.zc = c->tma_zc; p.ntx = c->tma_ntx; p.nty = c->tma_nty; p.ntz = c->tma_ntz;
-    p.nchunk = c->tma_nchunk; p.n_tiles = c->tma_tiles;
+    p.zc = P.zc; p.ntx = P.ntx; p.nty = P.nty; p.ntz = P.ntz;
+    p.nchunk = P.nchunk; p.n_tiles = P.tiles;
     p.ih2 = (float)(1.0 / (c->h * c->h));
     p.m6ih2 = (float)(-6.0 / (c->h * c->h));
     p.phase = phase;
-    p.fin = scal_params(c, c->partials_tma, c->tma_grid, nullptr);
-    const CUtensorMap *tin, *told;
+    p.m_tma = P.m_tma;
+    p.fin = scal_params(c, c->partials_tma, P.grid, nullptr);
     if (MODE == MODE_F) {
         p.out = c->U; p.W = c->W; p.X = c->X; p.sgn = 1.f;
         p.ca = c->coef + C_CA_F * NM; p.cb = c->coef + C_CB_F * NM; p.cv = c->coef + C_CV_F * NM;
         p.cx = c->coef + C_CX * NM; p.cw = c->coef + C_CW * NM;
-        tin = &c->tmV_halo; told = &c->tmU_ctr;
     } else {
         p.out = c->V; p.sgn = -1.f;
         p.ca = c->coef + C_CA_A * NM; p.cb = c->coef + C_CB_A * NM;
         p.cv = p.cx = p.cw = p.ca;
-        tin = &c->tmU_halo; told = &c->tmV_ctr;
     }
     cudaEvent_t e1 = nullptr;
     if (c->profiling && phase != PH_INIT_A) {
@@ -363,7 +429,7 @@ int launch_tma_cfg(wri_ctx* c, int phase) {
         c->ev_used++;
         CK(cudaEventRecord(e0, c->stream));
     }
-    k_pass_tma<Cfg, MODE><<<c->tma_grid, Cfg::NT + 32, smem, c->stream>>>(*tin, *told, c->tmW_ctr, c->tmX_ctr, p);
+    k_pass_tma<Cfg, MODE><<<P.grid, Cfg::NT + 32, smem, c->stream>>>(P.in, P.old, P.w, P.x, P.m, p);
     c->launches++;
     CK(cudaGetLastError());
     if (e1) CK(cudaEventRecord(e1, c->stream));
@@ -373,9 +439,9 @@ int launch_tma_cfg(wri_ctx* c, int phase) {
 template <int MODE>
 int launch_tma(wri_ctx* c, int phase) {
     switch (c->tma_cb) {
-        case 64: return launch_tma_cfg<Cfg64, MODE>(c, phase);
-        case 32: return launch_tma_cfg<Cfg32, MODE>(c, phase);
-        default: return launch_tma_cfg<Cfg16, MODE>(c, phase);
+        case 64: return launch_tma_cfg<typename CfgFor<64, MODE>::type, MODE>(c, phase);
+        case 32: return launch_tma_cfg<typename CfgFor<32, MODE>::type, MODE>(c, phase);
+        default: return launch_tma_cfg<typename CfgFor<16, MODE>::type, MODE>(c, phase);
     }
 }
 

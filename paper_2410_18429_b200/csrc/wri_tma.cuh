@@ -17,24 +17,35 @@
 #include <cuda.h>
 #include "wri_kernels.cuh"
 
+#ifndef WRI_HINTS
+#define WRI_HINTS 2     // 0 none, 1 streams evict_first, 2 + stencil input evict_last, 3 + output evict_last
+#endif
+
 namespace wri {
 
-template <int CB_, int TXC_, int TYC_>
+template <int CB_, int TXC_, int TYC_, int NT_>
 struct TileCfg {
     static constexpr int CB = CB_, TXC = TXC_, TYC = TYC_;
-    static constexpr int NT = 256;                              // consumer threads
+    static constexpr int NT = NT_;                              // consumer threads
     static constexpr int ITEMS = TXC * TYC * CB / 2;            // 16-byte items per plane
     static constexpr int IPT = ITEMS / NT;                      // items per thread
     static constexpr int IN_BYTES = (TXC + 2) * (TYC + 2) * CB * 8;
     static constexpr int CTR_BYTES = TXC * TYC * CB * 8;
+    static constexpr int M_BYTES = (TXC * TYC * 4 + 127) / 128 * 128;   // model tile (float per cell)
     static_assert(ITEMS % NT == 0, "tile must give every consumer thread the same work");
     static_assert(NT % (CB / 2) == 0, "a thread must keep one column pair");
     static_assert(IN_BYTES % 128 == 0 && CTR_BYTES % 128 == 0, "TMA destinations need 128 B alignment");
 };
 
 template <int MODE> struct PassTraits;
-template <> struct PassTraits<MODE_F> { static constexpr int NSTREAM = 3, NSTAGE = 4; };
-template <> struct PassTraits<MODE_A> { static constexpr int NSTREAM = 1, NSTAGE = 6; };
+#ifndef WRI_F_STAGES
+#define WRI_F_STAGES 3
+#endif
+#ifndef WRI_A_STAGES
+#define WRI_A_STAGES 6
+#endif
+template <> struct PassTraits<MODE_F> { static constexpr int NSTREAM = 3, NSTAGE = WRI_F_STAGES; };
+template <> struct PassTraits<MODE_A> { static constexpr int NSTREAM = 1, NSTAGE = WRI_A_STAGES; };
 
 struct TmaPassParams {
     float2* out;           // result vector (its old values arrive through tm_old)
@@ -48,6 +59,7 @@ struct TmaPassParams {
     int nx, ny, nz, nb;
     int zc, ntx, nty, ntz, nchunk, n_tiles;
     float ih2, m6ih2, sgn;
+    int m_tma;             // 1: the model tile rides in the TMA stage (needs nx % 4 == 0)
     int phase;             // ScalPhase run by the last CTA
     ScalParams fin;
 };
@@ -62,7 +74,11 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+#ifdef WRI_RELAXED_ARRIVE
+    asm volatile("mbarrier.arrive.relaxed.cta.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+#else
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+#endif
 }
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     asm volatile(
@@ -82,6 +98,36 @@ __device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* tm,
         " [%0], [%1, {%3, %4, %5, %6}], [%2];" ::"r"(dst), "l"(tm), "r"(bar),
         "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
 }
+// L2 eviction-priority policies: the in-place streams (old | W | X) are touched once per pass,
+// the stencil input is re-read by the neighbouring tiles and should outlive them in L2.
+__device__ __forceinline__ uint64_t policy_evict_first() {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ uint64_t policy_evict_last() {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ void tma_load_4d_hint(uint32_t dst, const CUtensorMap* tm, uint32_t bar,
+                                                 int c0, int c1, int c2, int c3, uint64_t pol) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint"
+        " [%0], [%1, {%3, %4, %5, %6}], [%2], %7;" ::"r"(dst), "l"(tm), "r"(bar),
+        "r"(c0), "r"(c1), "r"(c2), "r"(c3), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void stg128_hint(float2* ptr, const float4& v, uint64_t pol) {
+    asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1, %2, %3, %4}, %5;" ::"l"(ptr), "f"(v.x), "f"(v.y),
+                 "f"(v.z), "f"(v.w), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* tm, uint32_t bar,
+                                            int c0, int c1, int c2) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes"
+        " [%0], [%1, {%3, %4, %5}], [%2];" ::"r"(dst), "l"(tm), "r"(bar),
+        "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
 __device__ __forceinline__ void consumer_sync(int nthreads) {
     asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory");
 }
@@ -93,10 +139,11 @@ template <class Cfg, int MODE>
 __global__ void __launch_bounds__(Cfg::NT + 32, 1)
 k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CUtensorMap tm_old,
            const __grid_constant__ CUtensorMap tm_w, const __grid_constant__ CUtensorMap tm_x,
-           const TmaPassParams p) {
+           const __grid_constant__ CUtensorMap tm_m, const TmaPassParams p) {
     constexpr int CB = Cfg::CB, TXC = Cfg::TXC, TYC = Cfg::TYC, NT = Cfg::NT, IPT = Cfg::IPT;
     constexpr int NSTREAM = PassTraits<MODE>::NSTREAM, NSTAGE = PassTraits<MODE>::NSTAGE;
-    constexpr int STAGE_BYTES = Cfg::IN_BYTES + NSTREAM * Cfg::CTR_BYTES;
+    constexpr int M_OFF = Cfg::IN_BYTES + NSTREAM * Cfg::CTR_BYTES;
+    constexpr int STAGE_BYTES = M_OFF + Cfg::M_BYTES;
     constexpr int HP = CB / 2;                                  // column pairs per cell
     constexpr int ROW_B = (TXC + 2) * CB * 8;                   // bytes per halo-tile row
     constexpr int CELL_B = CB * 8;
@@ -106,6 +153,8 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + NSTAGE * STAGE_BYTES);   // full[NSTAGE], empty[NSTAGE]
     double* colacc = reinterpret_cast<double*>(bars + 2 * NSTAGE);               // [nb]
     double* red = colacc + p.nb;                                                  // [NT*2]
+    float* tab_g = reinterpret_cast<float*>(red + 2 * NT);                        // gx | gy | gz
+    float* tab_c = tab_g + (p.nx + p.ny + p.nz);                                  // w2|ca|cb|cv|cx|cw, [6][nb]
     __shared__ unsigned int s_ticket;
 
     const int tid = threadIdx.x;
@@ -118,13 +167,28 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    for (int j = tid; j < p.nb; j += blockDim.x) colacc[j] = 0.0;
+    for (int j = tid; j < p.nb; j += blockDim.x) {
+        colacc[j] = 0.0;
+        tab_c[j] = p.w2[j];
+        tab_c[p.nb + j] = p.ca[j];
+        tab_c[2 * p.nb + j] = p.cb[j];
+        tab_c[3 * p.nb + j] = (MODE == MODE_F) ? p.cv[j] : 0.f;
+        tab_c[4 * p.nb + j] = (MODE == MODE_F) ? p.cx[j] : 0.f;
+        tab_c[5 * p.nb + j] = (MODE == MODE_F) ? p.cw[j] : 0.f;
+    }
+    for (int j = tid; j < p.nx + p.ny + p.nz; j += blockDim.x) tab_g[j] = p.gx[j];   // gx|gy|gz are contiguous
     __syncthreads();
 
     if (tid >= NT) {
         // ------------------------------------------------------------------ producer warp
         // (all 32 lanes walk the loops together; lane 0 issues)
         const bool issuer = (tid == NT);
+#if WRI_HINTS >= 1
+        const uint64_t pol_stream = policy_evict_first();
+#endif
+#if WRI_HINTS >= 2
+        const uint64_t pol_in = policy_evict_last();
+#endif
         int stage = 0;
         uint32_t phase = 0;
         for (int t = blockIdx.x; t < p.n_tiles; t += gridDim.x) {
@@ -140,15 +204,29 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
                     mbar_wait(empty0 + 8 * stage, phase ^ 1);
                     const bool streams = pl >= z0 + 1;
                     const uint32_t fb = full0 + 8 * stage;
-                    mbar_expect_tx(fb, Cfg::IN_BYTES + (streams ? NSTREAM * Cfg::CTR_BYTES : 0));
+                    mbar_expect_tx(fb, Cfg::IN_BYTES + (streams ? NSTREAM * Cfg::CTR_BYTES +
+                                                            (p.m_tma ? TXC * TYC * 4 : 0) : 0));
                     const uint32_t dst = smem_u32(stages + stage * STAGE_BYTES);
+#if WRI_HINTS >= 2
+                    tma_load_4d_hint(dst, &tm_in, fb, c0, x0 - 1, y0 - 1, pl, pol_in);
+#else
                     tma_load_4d(dst, &tm_in, fb, c0, x0 - 1, y0 - 1, pl);
+#endif
                     if (streams) {
+#if WRI_HINTS >= 1
+                        tma_load_4d_hint(dst + Cfg::IN_BYTES, &tm_old, fb, c0, x0, y0, pl - 1, pol_stream);
+                        if (MODE == MODE_F) {
+                            tma_load_4d_hint(dst + Cfg::IN_BYTES + Cfg::CTR_BYTES, &tm_w, fb, c0, x0, y0, pl - 1, pol_stream);
+                            tma_load_4d_hint(dst + Cfg::IN_BYTES + 2 * Cfg::CTR_BYTES, &tm_x, fb, c0, x0, y0, pl - 1, pol_stream);
+                        }
+#else
                         tma_load_4d(dst + Cfg::IN_BYTES, &tm_old, fb, c0, x0, y0, pl - 1);
                         if (MODE == MODE_F) {
                             tma_load_4d(dst + Cfg::IN_BYTES + Cfg::CTR_BYTES, &tm_w, fb, c0, x0, y0, pl - 1);
                             tma_load_4d(dst + Cfg::IN_BYTES + 2 * Cfg::CTR_BYTES, &tm_x, fb, c0, x0, y0, pl - 1);
                         }
+#endif
+                        if (p.m_tma) tma_load_3d(dst + M_OFF, &tm_m, fb, x0, y0, pl - 1);
                     }
                 }
                 __syncwarp();
@@ -158,6 +236,10 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
     } else {
         // ------------------------------------------------------------------ consumers
         const int cp = tid % HP;                                // column pair within the chunk
+#if WRI_HINTS >= 1
+        const uint64_t pol_st = policy_evict_first();
+        const uint64_t pol_out = (WRI_HINTS >= 3) ? policy_evict_last() : pol_st;
+#endif
         int stage = 0;
         uint32_t phase = 0;
         // static item geometry: item j of this thread is cell (cxj, cyj) of the tile
@@ -183,10 +265,10 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
             float w2[2], ca[2], cb[2], cv[2], cx[2], cw[2];
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
-                w2[e] = p.w2[col + e]; ca[e] = p.ca[col + e]; cb[e] = p.cb[col + e];
-                cv[e] = (MODE == MODE_F) ? p.cv[col + e] : 0.f;
-                cx[e] = (MODE == MODE_F) ? p.cx[col + e] : 0.f;
-                cw[e] = (MODE == MODE_F) ? p.cw[col + e] : 0.f;
+                w2[e] = tab_c[col + e]; ca[e] = tab_c[p.nb + col + e]; cb[e] = tab_c[2 * p.nb + col + e];
+                cv[e] = tab_c[3 * p.nb + col + e];
+                cx[e] = tab_c[4 * p.nb + col + e];
+                cw[e] = tab_c[5 * p.nb + col + e];
             }
             bool valid[IPT];
             float gxy[IPT], m_cur[IPT], m_nxt[IPT];
@@ -198,7 +280,7 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
                 const int ix = tx * TXC + cxj[j], iy = ty * TYC + cyj[j];
                 valid[j] = ix < p.nx && iy < p.ny;
                 const int ixc = min(ix, p.nx - 1), iyc = min(iy, p.ny - 1);
-                gxy[j] = fmaxf(p.gx[ixc], p.gy[iyc]);
+                gxy[j] = fmaxf(tab_g[ixc], tab_g[p.nx + iyc]);
                 moff[j] = ((size_t)z0 * p.ny + iyc) * p.nx + ixc;
                 goff[j] = (((size_t)z0 * p.ny + iyc) * p.nx + ixc) * p.nb + col;
                 m_cur[j] = 0.f;
@@ -211,7 +293,7 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
 
             for (int pl = z0 - 1; pl <= z1; ++pl) {
                 // model value of plane pl (used one step later), issued before the wait
-                if (pl >= z0 && pl < z1) {
+                if (!p.m_tma && pl >= z0 && pl < z1) {
 #pragma unroll
                     for (int j = 0; j < IPT; ++j) m_nxt[j] = __ldg(p.m + moff[j] + (size_t)(pl - z0) * plane_m);
                 }
@@ -229,6 +311,8 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
                     if (emit) {
                         const int io = Cfg::IN_BYTES + (tid + j * NT) * 16;
                         o_old[j] = lds128(sb, io);
+                        if (p.m_tma)
+                            m_cur[j] = *reinterpret_cast<const float*>(sb + M_OFF + (cyj[j] * TXC + cxj[j]) * 4);
                         if (MODE == MODE_F) {
                             o_w[j] = lds128(sb, io + Cfg::CTR_BYTES);
                             o_x[j] = lds128(sb, io + 2 * Cfg::CTR_BYTES);
@@ -241,7 +325,7 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
 
                 if (emit) {
                     const int z = pl - 1;
-                    const float gzv = p.gz[z];
+                    const float gzv = tab_g[p.nx + p.ny + z];
 #pragma unroll
                     for (int j = 0; j < IPT; ++j) {
                         const float g = fmaxf(gxy[j], gzv);
@@ -270,7 +354,11 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
                         }
                         if (valid[j]) {
                             const size_t off = goff[j] + (size_t)(z - z0) * plane_e;
+#if WRI_HINTS >= 1
+                            stg128_hint(p.out + off, rr, pol_out);
+#else
                             *reinterpret_cast<float4*>(p.out + off) = rr;
+#endif
                             acc[0] += (double)fmaf(rr.x, rr.x, rr.y * rr.y);
                             acc[1] += (double)fmaf(rr.z, rr.z, rr.w * rr.w);
                             if (MODE == MODE_F) {
@@ -283,8 +371,13 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
                                 wn.y = fmaf(cv[0], cc.y, -cw[0] * o_w[j].y);
                                 wn.z = fmaf(cv[1], cc.z, -cw[1] * o_w[j].z);
                                 wn.w = fmaf(cv[1], cc.w, -cw[1] * o_w[j].w);
+#if WRI_HINTS >= 1
+                                stg128_hint(p.X + off, xn, pol_st);
+                                stg128_hint(p.W + off, wn, pol_st);
+#else
                                 *reinterpret_cast<float4*>(p.X + off) = xn;
                                 *reinterpret_cast<float4*>(p.W + off) = wn;
+#endif
                             }
                         }
                     }
@@ -292,7 +385,7 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
 #pragma unroll
                 for (int j = 0; j < IPT; ++j) {
                     c_prev[j] = c_cur[j]; c_cur[j] = c_new[j]; n_cur[j] = n_new[j];
-                    m_cur[j] = m_nxt[j];
+                    if (!p.m_tma) m_cur[j] = m_nxt[j];
                 }
             }
             // fold this tile's per-thread sums into the CTA's per-column sums, fixed order
