@@ -30,6 +30,9 @@ int cuda_fail(cudaError_t e, const char* what) {
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
+constexpr int kMaxCtas = 512;          // upper bound on the persistent grid (>= SM count)
+constexpr int kMinChunk = 16;          // narrowest column chunk of the TMA path
+
 struct Tiling {
     int vec;            // complex numbers per thread (2 = 128-bit accesses)
     dim3 block, grid;
@@ -51,6 +54,11 @@ struct wri_ctx {
     // library-owned device memory
     float* gtab = nullptr;       // gx | gy | gz
     int* rec = nullptr;          // [n_rec] cell indices
+    std::vector<int> rec_ijk;    // host copy [n_rec][3]
+    int* own_ptr = nullptr;      // [kMaxCtas + 1] pass A: CSR of the receivers inside each CTA's tiles
+    int4* own = nullptr;         // [n_rec * max chunks] {receiver, cell, tile, group size}
+    std::vector<int> h_own_ptr;
+    std::vector<int4> h_own;
     float* coef = nullptr;       // [N_COEF][nb_max]
     double* stat = nullptr;      // [N_STAT][nb_max]
     int* active = nullptr;       // [nb_max]
@@ -110,8 +118,6 @@ Tiling make_tiling(const wri_ctx* c, int nb) {
     t.n_tiles = (size_t)gx * gy * gz;
     return t;
 }
-
-constexpr int kMaxCtas = 512;          // upper bound on the persistent grid (>= SM count)
 
 struct WsLayout {
     size_t U, V, W, U_bot, partials, partials_tma, Xs, Ds, tols, res, its, total;
@@ -205,6 +211,7 @@ int launch_scalars(wri_ctx* c, const float2* d) {
     s.coef = c->coef; s.stat = c->stat; s.active = c->active; s.iters = c->iters;
     s.tol = c->tol; s.resnorms = c->resnorms; s.iters_out = c->iters_out;
     s.k = c->k; s.maxit = c->maxit; s.lambda = c->lambda;
+    s.rows_in_pass = c->tma_cb ? 1 : 0;
     const int T = 1024;
     const size_t smem = (size_t)(T + c->nb) * sizeof(double);
     k_scalars<PHASE><<<1, T, smem, c->stream>>>(s);
@@ -346,6 +353,39 @@ int tma_plan(wri_ctx* c, wri_ctx::TmaPlan& P, const void* in, const void* old, b
     } else {
         P.w = P.old; P.x = P.old;          // unused by pass A
     }
+    if (!is_f && c->n_rec) {
+        // receivers (x column chunks) inside each CTA's tiles, in the order the CTA walks its
+        // tiles (same tile numbering as the kernel)
+        const int G = P.grid, nent = c->n_rec * P.nchunk;
+        struct Ent { int cta, tile, r; };
+        std::vector<Ent> ents(nent);
+        for (int e = 0; e < nent; ++e) {
+            const int r = e / P.nchunk, chunk = e % P.nchunk;
+            const int tx = c->rec_ijk[3 * r] / P.txc, ty = c->rec_ijk[3 * r + 1] / P.tyc;
+            const int tz = c->rec_ijk[3 * r + 2] / P.zc;
+            const int t = (int)((((long long)tz * P.nty + ty) * P.ntx + tx) * P.nchunk + chunk);
+            ents[e] = {t % G, t, r};
+        }
+        std::sort(ents.begin(), ents.end(), [](const Ent& a, const Ent& b) {
+            return a.cta != b.cta ? a.cta < b.cta : a.tile != b.tile ? a.tile < b.tile : a.r < b.r;
+        });
+        c->h_own_ptr.assign(G + 1, 0);
+        c->h_own.resize(nent);
+        for (int e = 0; e < nent; ++e) c->h_own_ptr[ents[e].cta + 1]++;
+        for (int b = 0; b < G; ++b) c->h_own_ptr[b + 1] += c->h_own_ptr[b];
+        for (int e = 0; e < nent;) {
+            int f = e;
+            while (f < nent && ents[f].cta == ents[e].cta && ents[f].tile == ents[e].tile) ++f;
+            for (int j = e; j < f; ++j) {
+                const int r = ents[j].r;
+                const int cell = (c->rec_ijk[3 * r + 2] * c->g.ny + c->rec_ijk[3 * r + 1]) * c->g.nx + c->rec_ijk[3 * r];
+                c->h_own[j] = make_int4(r, cell, ents[j].tile, j == e ? f - e : 0);
+            }
+            e = f;
+        }
+        CK(cudaMemcpyAsync(c->own_ptr, c->h_own_ptr.data(), (G + 1) * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+        CK(cudaMemcpyAsync(c->own, c->h_own.data(), nent * sizeof(int4), cudaMemcpyHostToDevice, c->stream));
+    }
     P.m_tma = (c->g.nx % 4 == 0) && (P.txc % 4 == 0) && aligned16(c->m);
     if (P.m_tma) { if ((rc = make_tmap_model(&P.m, c, P.txc, P.tyc))) return rc; }
     else P.m = P.old;                       // unused placeholder
@@ -380,6 +420,7 @@ ScalParams scal_params(const wri_ctx* c, const double* partials, int n_rows, con
     s.coef = c->coef; s.stat = c->stat; s.active = c->active; s.iters = c->iters;
     s.tol = c->tol; s.resnorms = c->resnorms; s.iters_out = c->iters_out;
     s.k = c->k; s.maxit = c->maxit; s.lambda = c->lambda;
+    s.rows_in_pass = 1;
     return s;
 }
 
@@ -406,6 +447,8 @@ int launch_tma_cfg(wri_ctx* c, int phase) {
     p.phase = phase;
     p.m_tma = P.m_tma;
     p.fin = scal_params(c, c->partials_tma, P.grid, nullptr);
+    p.n_rec = c->n_rec; p.rec = c->rec; p.U_bot = c->U_bot; p.V = c->V;
+    p.ct = c->coef + C_CT_A * NM; p.own_ptr = c->own_ptr; p.own = c->own;
     if (MODE == MODE_F) {
         p.out = c->U; p.W = c->W; p.X = c->X; p.sgn = 1.f;
         p.ca = c->coef + C_CA_F * NM; p.cb = c->coef + C_CB_F * NM; p.cv = c->coef + C_CV_F * NM;
@@ -532,6 +575,9 @@ int wri_create(wri_ctx** out, wri_grid grid, double h, int32_t n_omega, const do
     CKC(cudaMemcpy(c->gtab, gt.data(), gt.size() * sizeof(float), cudaMemcpyHostToDevice));
     CKC(cudaMalloc(&c->rec, std::max(n_rec, 1) * sizeof(int)));
     if (n_rec) CKC(cudaMemcpy(c->rec, cells.data(), n_rec * sizeof(int), cudaMemcpyHostToDevice));
+    c->rec_ijk.assign(rec_ijk_host, rec_ijk_host + 3 * (size_t)n_rec);
+    CKC(cudaMalloc(&c->own_ptr, (kMaxCtas + 1) * sizeof(int)));
+    CKC(cudaMalloc(&c->own, (size_t)std::max(n_rec, 1) * (nb_max / kMinChunk + 1) * sizeof(int4)));
     CKC(cudaMalloc(&c->coef, (size_t)N_COEF * nb_max * sizeof(float)));
     CKC(cudaMemset(c->coef, 0, (size_t)N_COEF * nb_max * sizeof(float)));
     CKC(cudaMalloc(&c->stat, (size_t)N_STAT * nb_max * sizeof(double)));
@@ -556,6 +602,7 @@ int wri_destroy(wri_ctx* c) {
     if (!c) return WRI_OK;
     cudaFree(c->gtab); cudaFree(c->rec); cudaFree(c->coef); cudaFree(c->stat);
     cudaFree(c->active); cudaFree(c->iters); cudaFree(c->counter);
+    cudaFree(c->own_ptr); cudaFree(c->own);
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
     delete c;
     return WRI_OK;

@@ -271,6 +271,8 @@ struct ScalParams {
     int k;                    // iteration number (PH_A), for resnorms / iters
     int maxit;
     float lambda;
+    int rows_in_pass;         // 1: the pass kernels own the receiver rows (wri_tma.cuh); the
+                              //    finaliser only reduces partials and runs the recurrences
 };
 
 // sum over tiles of partials[.][s] in fixed order; result for column s in colsum[s] (shared)
@@ -282,8 +284,17 @@ __device__ __forceinline__ void reduce_partials(const ScalParams& p, double* scr
         const int g = threadIdx.x / ncol, s = base + threadIdx.x % ncol;
         const int Gc = max(1, T / ncol);
         double a = 0.0;
-        if (g < Gc)
-            for (int b = g; b < p.n_tiles; b += Gc) a += __ldcg(p.partials + (size_t)b * nb + s);
+        if (g < Gc) {
+            int b = g;
+            for (; b + 7 * Gc < p.n_tiles; b += 8 * Gc) {           // 8 loads in flight, added in order
+                double t[8];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) t[j] = __ldcg(p.partials + (size_t)(b + j * Gc) * nb + s);
+#pragma unroll
+                for (int j = 0; j < 8; ++j) a += t[j];
+            }
+            for (; b < p.n_tiles; b += Gc) a += __ldcg(p.partials + (size_t)b * nb + s);
+        }
         scratch[threadIdx.x] = a;
         __syncthreads();
         if (threadIdx.x < ncol) {
@@ -336,7 +347,7 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
         for (long long i = threadIdx.x; i < nrs; i += blockDim.x) p.U_bot[i] = p.d[i];
         __syncthreads();
     }
-    if (PHASE == PH_F) {
+    if (PHASE == PH_F && !p.rows_in_pass) {
         // bottom rows of the forward pass just done:  U_bot <- cv * V[rec] - cb * U_bot
         for (long long i = threadIdx.x; i < nrs; i += blockDim.x) {
             const int r = (int)(i / nb), s = (int)(i - (long long)r * nb);
@@ -348,7 +359,7 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
         __syncthreads();
     }
     reduce_partials(p, scratch, colsum);
-    if (PHASE == PH_INIT_B || PHASE == PH_F) add_receiver_norms(p, scratch, colsum);
+    if (PHASE == PH_INIT_B || (PHASE == PH_F && !p.rows_in_pass)) add_receiver_norms(p, scratch, colsum);
 
     for (int s = threadIdx.x; s < nb; s += blockDim.x) {
         const double nrm = sqrt(colsum[s]);
@@ -436,7 +447,7 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
     }
     __syncthreads();
 
-    if (PHASE == PH_INIT_B || PHASE == PH_F) {
+    if ((PHASE == PH_INIT_B || PHASE == PH_F) && !p.rows_in_pass) {
         // fold P^T into the coming adjoint pass:  V <- ca A^H U - cb (V - (ct/cb) P^T U_bot)
         for (long long i = threadIdx.x; i < nrs; i += blockDim.x) {
             const int r = (int)(i / nb), s = (int)(i - (long long)r * nb);

@@ -61,8 +61,43 @@ struct TmaPassParams {
     float ih2, m6ih2, sgn;
     int m_tma;             // 1: the model tile rides in the TMA stage (needs nx % 4 == 0)
     int phase;             // ScalPhase run by the last CTA
+    // receiver rows, spread over the CTAs (keeps them off the last CTA's serial tail)
+    int n_rec;
+    const int* rec;        // [n_rec] cell indices
+    float2* U_bot;         // [n_rec][nb]
+    const float2* V;       // pass F: the stencil input as a plain pointer (rows of P v)
+    const float* ct;       // pass A: [nb] scale of P^T U_bot
+    const int* own_ptr;    // pass A: [gridDim.x + 1] CSR over own
+    const int4* own;       // pass A: receivers inside this CTA's tiles, sorted by tile:
+                           //         {receiver, cell, tile, entries in this tile (at its first entry)};
+                           //         with column chunks, one entry per (receiver, chunk)
     ScalParams fin;
 };
+
+// rows x columns work with a fixed-order per-column sum: row i of `nrows`, local column s of
+// `ncols` -> fn(i, s) returns a double that is added to colacc[coloff(i) + s].  Rows are taken
+// NT/ncols at a time; within a round thread s adds the rows in increasing order, so the result
+// does not depend on scheduling.  Called by the NT consumer threads only (named barrier 1).
+template <int NT, class Fn, class Off>
+__device__ __forceinline__ void rows_by_columns(int nrows, int ncols, int tid, double* red, double* colacc,
+                                                Fn fn, Off coloff) {
+    for (int cbase = 0; cbase < ncols; cbase += NT) {
+        const int nc = min(ncols - cbase, NT);
+        const int rpr = NT / nc;                                // rows per round
+        const int i = tid / nc, s = cbase + tid % nc;
+        for (int row0 = 0; row0 < nrows; row0 += rpr) {
+            double a = 0.0;
+            if (i < rpr && row0 + i < nrows) a = fn(row0 + i, s);
+            red[tid] = a;
+            asm volatile("bar.sync 1, %0;" ::"r"(NT) : "memory");
+            if (tid < nc) {
+                const int nr = min(rpr, nrows - row0);
+                for (int j = 0; j < nr; ++j) colacc[coloff(row0 + j) + cbase + tid] += red[j * nc + tid];
+            }
+            asm volatile("bar.sync 1, %0;" ::"r"(NT) : "memory");
+        }
+    }
+}
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
     return (uint32_t)__cvta_generic_to_shared(p);
@@ -253,6 +288,33 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
             sm_ctr[j] = (cyj[j] + 1) * ROW_B + (cxj[j] + 1) * CELL_B + cp * 16;
         }
 
+        int own_cur = 0, own_end = 0;
+        int4 own_nxt = make_int4(-1, -1, -1, 0);
+        if (MODE == MODE_A && p.n_rec > 0) {
+            own_cur = p.own_ptr[blockIdx.x];
+            own_end = p.own_ptr[blockIdx.x + 1];
+            if (own_cur < own_end) own_nxt = __ldg(p.own + own_cur);
+        }
+        if (MODE == MODE_F && p.n_rec > (int)blockIdx.x) {
+            // receiver rows of u = M v - alpha u:  U_bot <- cv V[rec] - cb U_bot  (V is read-only in
+            // this pass), rows blockIdx.x, +gridDim.x, ...; their |.|^2 joins this CTA's column sums.
+            // Runs while the producer warp fills the pipeline.
+            const int nrows = (p.n_rec - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+            const int nb = p.nb;
+            rows_by_columns<NT>(nrows, nb, tid, red, colacc,
+                [&](int i, int s) -> double {
+                    const int r = blockIdx.x + i * gridDim.x;
+                    const size_t e = (size_t)r * nb + s;
+                    const float2 v = __ldcg(p.V + (size_t)p.rec[r] * nb + s);
+                    const float2 u = __ldcg(p.U_bot + e);
+                    const float cvs = tab_c[3 * nb + s], cbs = tab_c[2 * nb + s];
+                    const float2 n = make_float2(fmaf(cvs, v.x, -cbs * u.x), fmaf(cvs, v.y, -cbs * u.y));
+                    p.U_bot[e] = n;
+                    return (double)fmaf(n.x, n.x, n.y * n.y);
+                },
+                [](int) { return 0; });
+        }
+
         for (int t = blockIdx.x; t < p.n_tiles; t += gridDim.x) {
             int r = t;
             const int chunk = r % p.nchunk; r /= p.nchunk;
@@ -400,6 +462,26 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
                 colacc[chunk * CB + tid] += s;
             }
             consumer_sync(NT);
+            if (MODE == MODE_A && own_nxt.z == t) {
+                // P^T rows: the receivers inside the tile just written get  V += ct U_bot ; the
+                // squared-norm sums are corrected by |V + ct U_bot|^2 - |V|^2.
+                const int cnt = own_nxt.w, nb = p.nb;
+                rows_by_columns<NT>(cnt, CB, tid, red, colacc,
+                    [&](int i, int s) -> double {
+                        const int4 en = (i == 0) ? own_nxt : __ldg(p.own + own_cur + i);
+                        const int c = chunk * CB + s;
+                        float2* vp = p.out + (size_t)en.y * nb + c;
+                        const float2 v = __ldcg(vp);
+                        const float2 u = __ldcg(p.U_bot + (size_t)en.x * nb + c);
+                        const float cts = p.ct[c];
+                        const float2 n = make_float2(fmaf(cts, u.x, v.x), fmaf(cts, u.y, v.y));
+                        *vp = n;
+                        return ((double)n.x * n.x + (double)n.y * n.y) - (double)fmaf(v.x, v.x, v.y * v.y);
+                    },
+                    [&](int) { return chunk * CB; });
+                own_cur += cnt;
+                own_nxt = (own_cur < own_end) ? __ldg(p.own + own_cur) : make_int4(-1, -1, -1, 0);
+            }
         }
     }
 
