@@ -136,6 +136,19 @@ def dist_env():
     return rank, world, local
 
 
+def reduce_over_ranks(times, counts, dist=None, device=None):
+    """Whole-job aggregation for N ranks: times -> MAX over ranks, counts -> SUM over ranks.
+    (Columns are independent systems, so this is the only cross-rank traffic of the bench.)"""
+    if dist is None:
+        return list(times), list(counts)
+    import torch
+    t = torch.tensor(list(times), dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    c = torch.tensor(list(counts), dtype=torch.float64, device=device)
+    dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return [float(x) for x in t], [float(x) for x in c]
+
+
 def oracle_sample(w, cores, iters):
     """Time the CPU oracle as it stands on min(nb, cores) columns x `iters` iterations."""
     from oracle import oracle as O
@@ -257,15 +270,9 @@ def run_ours(args, wl_name, w):
     d2h = outh[0].numel() * 8 + outh[1].numel() * 4 + outh[2].numel() * 4
     iters_e2e = int(outh[2].sum().item())
 
-    if use_dist:
-        t = torch.tensor([ms, e2e_s], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms, e2e_s = float(t[0]), float(t[1])
-        tot = torch.tensor([iters_per_step, iters_e2e, launches], dtype=torch.float64, device=dev)
-        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
-        iters_all, iters_e2e_all, launches_all = float(tot[0]), float(tot[1]), int(tot[2])
-    else:
-        iters_all, iters_e2e_all, launches_all = iters_per_step, iters_e2e, launches
+    (ms, e2e_s), (iters_all, iters_e2e_all, launches_all) = reduce_over_ranks(
+        [ms, e2e_s], [iters_per_step, iters_e2e, launches], dist if use_dist else None, dev)
+    launches_all = int(launches_all)
 
     if rank == 0:
         value = iters_all * args.steps / (ms * 1e-3)
@@ -319,6 +326,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference" and dist_env()[0] != 0:
+        return                                   # the oracle arm runs on rank 0 alone
     spec = dict(WORKLOADS[args.workload])
     w = workloads.make(spec.pop("name"), **spec)
     if args.maxit:
