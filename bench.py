@@ -215,7 +215,7 @@ def run_ours(args, wl_name, w):
     q = torch.from_numpy(w.Q).to(dev)
     d = torch.from_numpy(w.D).to(dev)
     tol = torch.from_numpy(w.tol).to(dev) if (w.tol > 0).any() else None
-    ctx.ensure_workspace(nb, host_staging=True)
+    ctx.ensure_workspace(nb, host_staging=True, compaction=tol is not None)
     out = ctx._outputs(nb, maxit, dev)
 
     def barrier():

@@ -78,10 +78,15 @@ int wri_create(wri_ctx** out, wri_grid grid, double h,
 int wri_set_model(wri_ctx* ctx, const float* m_dev);
 
 /* Workspace for wri_lsqr_* at batch width nb (u, v, w vectors, receiver rows, reduction
- * partials).  host_staging != 0 adds room for the device copies wri_lsqr_batch_host needs.
+ * partials).  flags: WRI_WS_HOST_STAGING adds room for the device copies wri_lsqr_batch_host
+ * needs; WRI_WS_COMPACTION adds two more vectors so that converged columns can be compacted
+ * out of the working set when per-column tolerances are given (without it such a solve still
+ * stops early once every column has converged, but converged columns keep costing bandwidth).
  * The caller allocates (e.g. a torch uint8 tensor) and hands it over; it must stay alive and
  * untouched while a solve is in flight.                                                      */
-size_t wri_workspace_bytes(const wri_ctx* ctx, int32_t nb, int32_t host_staging);
+#define WRI_WS_HOST_STAGING 1
+#define WRI_WS_COMPACTION   2
+size_t wri_workspace_bytes(const wri_ctx* ctx, int32_t nb, int32_t flags);
 int    wri_set_workspace(wri_ctx* ctx, void* ws_dev, size_t bytes);
 
 /* y = M x: ytop = lambda * A x  (c64 [n_g][nb]),  ybot = x at the receiver
@@ -102,7 +107,12 @@ int wri_apply_MH(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_host, float 
  *   resnorms_dev float [maxit+1][nb]: ||b - M x_k|| for k = 0..maxit, held at the last value
  *                after a column stops (reading C-9)
  *   iters_dev    int32 [nb] iterations performed per column (may be NULL)
- * Equivalent to wri_lsqr_begin + wri_lsqr_iterate(maxit) + wri_lsqr_end.  Needs a workspace.  */
+ * Equivalent to wri_lsqr_begin + wri_lsqr_iterate(maxit) + wri_lsqr_end.  Needs a workspace.
+ * With tol_dev == NULL the call only enqueues work.  With tolerances the host reads the
+ * per-column active flags back every few iterations (one stream synchronisation each, about
+ * every 2 ms of device work): the solve returns as soon as every column has stopped, and
+ * stopped columns are compacted out of the working set (adaptive accuracy, PAPER.md:180-211;
+ * "the active mask shrinking as sources converge", BASELINE.json configs[3]).                */
 int wri_lsqr_batch(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_host,
                    const void* q_dev, const void* d_dev, float lambda,
                    const float* tol_dev, int32_t maxit,
@@ -134,7 +144,8 @@ int wri_lsqr_end(wri_ctx* ctx);
  *   (x_k also by wri_lsqr_end).
  * Pointers are into the caller's workspace / u_out buffer and the context's scalar block.    */
 typedef struct {
-    int32_t nb, k;                   /* batch width, iterations enqueued so far               */
+    int32_t nb, k;                   /* working batch width (shrinks when converged columns   */
+                                     /* are compacted away), iterations enqueued so far       */
     const void*   U_top;             /* c64 [n_g][nb]                                          */
     const void*   U_bot;             /* c64 [n_rec][nb]                                        */
     const void*   V;                 /* c64 [n_g][nb]                                          */

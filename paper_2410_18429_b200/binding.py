@@ -40,6 +40,8 @@ WRI_ERR_RECEIVER_DUP = -3
 WRI_ERR_WORKSPACE = -4
 WRI_ERR_CUDA = -5
 WRI_ERR_STATE = -6
+WRI_WS_HOST_STAGING = 1
+WRI_WS_COMPACTION = 2
 
 _lib = None
 
@@ -152,11 +154,15 @@ class Wri:
             pass
 
     # ---- workspace
-    def workspace_bytes(self, nb, host_staging=False):
-        return int(self._lib.wri_workspace_bytes(self._h, int(nb), int(bool(host_staging))))
+    def workspace_bytes(self, nb, host_staging=False, compaction=False):
+        flags = (WRI_WS_HOST_STAGING if host_staging else 0) | (WRI_WS_COMPACTION if compaction else 0)
+        return int(self._lib.wri_workspace_bytes(self._h, int(nb), flags))
 
-    def ensure_workspace(self, nb, host_staging=False):
-        need = self.workspace_bytes(nb, host_staging)
+    def ensure_workspace(self, nb, host_staging=False, compaction=False):
+        # sticky: a workspace once sized for host staging / compaction keeps that room
+        self._ws_hs = getattr(self, "_ws_hs", False) or bool(host_staging)
+        self._ws_cp = getattr(self, "_ws_cp", False) or bool(compaction)
+        need = self.workspace_bytes(nb, self._ws_hs, self._ws_cp)
         if self._ws is None or self._ws.numel() < need:
             self._ws = None
             self._ws = self._torch.empty(need, dtype=self._torch.uint8, device=self.m.device)
@@ -195,7 +201,7 @@ class Wri:
 
     def lsqr_batch(self, q, d, lam, tol=None, maxit=50, omega_idx=None, out=None):
         nb = q.shape[1]
-        self.ensure_workspace(nb)
+        self.ensure_workspace(nb, compaction=tol is not None)
         u, res, it = out if out is not None else self._outputs(nb, maxit, q.device)
         keep, oi = _i32(omega_idx)
         _ck(self._lib.wri_lsqr_batch(self._h, nb, oi, _dptr(q), _dptr(d), float(lam), _dptr(tol),
@@ -206,7 +212,7 @@ class Wri:
         """Host-buffer entry: q, d, tol and the outputs are CPU tensors (pinned for speed)."""
         t = self._torch
         nb = q.shape[1]
-        self.ensure_workspace(nb, host_staging=True)
+        self.ensure_workspace(nb, host_staging=True, compaction=tol is not None)
         if out is None:
             out = (t.empty((self.ng, nb), dtype=t.complex64).pin_memory(),
                    t.empty((maxit + 1, nb), dtype=t.float32).pin_memory(),
@@ -219,7 +225,7 @@ class Wri:
 
     def lsqr_begin(self, q, d, lam, tol=None, maxit=50, omega_idx=None):
         nb = q.shape[1]
-        self.ensure_workspace(nb)
+        self.ensure_workspace(nb, compaction=tol is not None)
         u, res, it = self._outputs(nb, maxit, q.device)
         keep, oi = _i32(omega_idx)
         self._keep = [q, d, tol, u, res, it]

@@ -59,16 +59,31 @@ struct wri_ctx {
     int4* own = nullptr;         // [n_rec * max chunks] {receiver, cell, tile, group size}
     std::vector<int> h_own_ptr;
     std::vector<int4> h_own;
-    float* coef = nullptr;       // [N_COEF][nb_max]
+    float* coef = nullptr;       // [N_COEF][nb_max]   current bank of the per-column scalars
     double* stat = nullptr;      // [N_STAT][nb_max]
     int* active = nullptr;       // [nb_max]
     int* iters = nullptr;        // [nb_max]
+    float* coef_alt = nullptr;   // second bank: column compaction gathers into it and swaps
+    double* stat_alt = nullptr;
+    int* active_alt = nullptr;
+    int* iters_alt = nullptr;
+    int* colmap = nullptr;       // [nb_max] working column -> caller's column (-1 = padding)
+    int* idx = nullptr;          // [3][nb_max] scratch: gather map | retire source | retire destination
+    int* h_active = nullptr;     // pinned host copy of the active flags
     // caller's workspace
     char* ws = nullptr;
     size_t ws_bytes = 0;
     // solve in flight
     bool solving = false;
-    int nb = 0, k = 0, maxit = 0;
+    int nb = 0, k = 0, maxit = 0;   // nb = WORKING width (shrinks when converged columns are compacted away)
+    int nb0 = 0;                    // caller's batch width
+    bool packed = false;            // X lives in the workspace (after the first compaction); else X = u_out
+    bool can_compact = false, all_done = false;
+    int check_every = 0;            // iterations between host looks at the active flags (0 = never)
+    std::vector<int> h_colmap;      // host copy of colmap
+    std::vector<char> retired;      // per caller's column: x and history are final in the caller's buffers
+    std::vector<float2*> free_slots;   // workspace vector slots not holding a live vector
+    float2 *U_bot_alt = nullptr, *u_out = nullptr;
     float lambda = 0;
     float2 *U = nullptr, *V = nullptr, *W = nullptr, *X = nullptr, *U_bot = nullptr;
     double* partials = nullptr;
@@ -120,12 +135,12 @@ Tiling make_tiling(const wri_ctx* c, int nb) {
 }
 
 struct WsLayout {
-    size_t U, V, W, U_bot, partials, partials_tma, Xs, Ds, tols, res, its, total;
+    size_t U, V, W, U_bot, partials, partials_tma, Xs, Ds, tols, res, its, B3, B4, U_bot2, total;
 };
-WsLayout ws_layout(const wri_ctx* c, int nb, int host_staging, int maxit_cap) {
+enum { WS_HOST_STAGING = 1, WS_COMPACTION = 2 };
+WsLayout ws_layout(const wri_ctx* c, int nb, int flags, int maxit_cap) {
     WsLayout L{};
-    size_t vec = align_up(c->ng * (size_t)nb * sizeof(float2), 256);
-    if (const char* e = getenv("WRI_PAD")) vec += (size_t)atoll(e);
+    const size_t vec = align_up(c->ng * (size_t)nb * sizeof(float2), 256);
     const size_t bot = align_up((size_t)std::max(c->n_rec, 1) * nb * sizeof(float2), 256);
     const Tiling t = make_tiling(c, nb);
     size_t o = 0;
@@ -135,12 +150,17 @@ WsLayout ws_layout(const wri_ctx* c, int nb, int host_staging, int maxit_cap) {
     L.U_bot = o; o += bot;
     L.partials = o; o += align_up(t.n_tiles * nb * sizeof(double), 256);
     L.partials_tma = o; o += align_up((size_t)kMaxCtas * nb * sizeof(double), 256);
-    if (host_staging) {
+    if (flags & WS_HOST_STAGING) {
         L.Xs = o; o += vec;
         L.Ds = o; o += bot;
         L.tols = o; o += align_up((size_t)nb * sizeof(float), 256);
         L.res = o; o += align_up((size_t)(maxit_cap + 1) * nb * sizeof(float), 256);
         L.its = o; o += align_up((size_t)nb * sizeof(int), 256);
+    }
+    if (flags & WS_COMPACTION) {
+        L.B3 = o; o += vec;
+        L.B4 = o; o += vec;
+        L.U_bot2 = o; o += bot;
     }
     L.total = o;
     return L;
@@ -212,6 +232,8 @@ int launch_scalars(wri_ctx* c, const float2* d) {
     s.tol = c->tol; s.resnorms = c->resnorms; s.iters_out = c->iters_out;
     s.k = c->k; s.maxit = c->maxit; s.lambda = c->lambda;
     s.rows_in_pass = c->tma_cb ? 1 : 0;
+    s.colmap = c->packed ? c->colmap : nullptr;
+    s.nb_out = c->nb0;
     const int T = 1024;
     const size_t smem = (size_t)(T + c->nb) * sizeof(double);
     k_scalars<PHASE><<<1, T, smem, c->stream>>>(s);
@@ -290,10 +312,16 @@ template <int CB, int MODE> struct CfgFor {
                     (MODE == MODE_F ? WRI_F_NT : WRI_A_NT)> type;
 };
 
+// 48 columns: 4 x 4 cells x 48 columns = 768 complex per plane, 384 (F) / 192 (A) consumer threads
+template <int MODE> struct CfgFor<48, MODE> {
+    typedef TileCfg<48, 4, 4, (MODE == MODE_F ? 384 : 192)> type;
+};
+
 int tma_chunk_for(int nb) {
     const char* off = getenv("WRI_NO_TMA");
     if (off && off[0] == '1') return 0;
     if (nb % 64 == 0) return 64;
+    if (nb % 48 == 0) return 48;
     if (nb % 32 == 0) return 32;
     if (nb % 16 == 0) return 16;
     return 0;
@@ -401,6 +429,9 @@ int tma_setup(wri_ctx* c) {
         case 64:
             if ((rc = tma_plan<CfgFor<64, MODE_F>::type>(c, c->planF, c->V, c->U, true))) return rc;
             return tma_plan<CfgFor<64, MODE_A>::type>(c, c->planA, c->U, c->V, false);
+        case 48:
+            if ((rc = tma_plan<CfgFor<48, MODE_F>::type>(c, c->planF, c->V, c->U, true))) return rc;
+            return tma_plan<CfgFor<48, MODE_A>::type>(c, c->planA, c->U, c->V, false);
         case 32:
             if ((rc = tma_plan<CfgFor<32, MODE_F>::type>(c, c->planF, c->V, c->U, true))) return rc;
             return tma_plan<CfgFor<32, MODE_A>::type>(c, c->planA, c->U, c->V, false);
@@ -421,6 +452,8 @@ ScalParams scal_params(const wri_ctx* c, const double* partials, int n_rows, con
     s.tol = c->tol; s.resnorms = c->resnorms; s.iters_out = c->iters_out;
     s.k = c->k; s.maxit = c->maxit; s.lambda = c->lambda;
     s.rows_in_pass = 1;
+    s.colmap = c->packed ? c->colmap : nullptr;
+    s.nb_out = c->nb0;
     return s;
 }
 
@@ -483,6 +516,7 @@ template <int MODE>
 int launch_tma(wri_ctx* c, int phase) {
     switch (c->tma_cb) {
         case 64: return launch_tma_cfg<typename CfgFor<64, MODE>::type, MODE>(c, phase);
+        case 48: return launch_tma_cfg<typename CfgFor<48, MODE>::type, MODE>(c, phase);
         case 32: return launch_tma_cfg<typename CfgFor<32, MODE>::type, MODE>(c, phase);
         default: return launch_tma_cfg<typename CfgFor<16, MODE>::type, MODE>(c, phase);
     }
@@ -586,6 +620,13 @@ int wri_create(wri_ctx** out, wri_grid grid, double h, int32_t n_omega, const do
     CKC(cudaMalloc(&c->iters, nb_max * sizeof(int)));
     CKC(cudaMemset(c->active, 0, nb_max * sizeof(int)));
     CKC(cudaMemset(c->iters, 0, nb_max * sizeof(int)));
+    CKC(cudaMalloc(&c->coef_alt, (size_t)N_COEF * nb_max * sizeof(float)));
+    CKC(cudaMalloc(&c->stat_alt, (size_t)N_STAT * nb_max * sizeof(double)));
+    CKC(cudaMalloc(&c->active_alt, nb_max * sizeof(int)));
+    CKC(cudaMalloc(&c->iters_alt, nb_max * sizeof(int)));
+    CKC(cudaMalloc(&c->colmap, nb_max * sizeof(int)));
+    CKC(cudaMalloc(&c->idx, (size_t)3 * nb_max * sizeof(int)));
+    CKC(cudaMallocHost(&c->h_active, nb_max * sizeof(int)));
     CKC(cudaMalloc(&c->counter, sizeof(unsigned int)));
     CKC(cudaMemset(c->counter, 0, sizeof(unsigned int)));
     {
@@ -603,6 +644,9 @@ int wri_destroy(wri_ctx* c) {
     cudaFree(c->gtab); cudaFree(c->rec); cudaFree(c->coef); cudaFree(c->stat);
     cudaFree(c->active); cudaFree(c->iters); cudaFree(c->counter);
     cudaFree(c->own_ptr); cudaFree(c->own);
+    cudaFree(c->coef_alt); cudaFree(c->stat_alt); cudaFree(c->active_alt); cudaFree(c->iters_alt);
+    cudaFree(c->colmap); cudaFree(c->idx);
+    if (c->h_active) cudaFreeHost(c->h_active);
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
     delete c;
     return WRI_OK;
@@ -614,9 +658,9 @@ int wri_set_model(wri_ctx* c, const float* m_dev) {
     return WRI_OK;
 }
 
-size_t wri_workspace_bytes(const wri_ctx* c, int32_t nb, int32_t host_staging) {
+size_t wri_workspace_bytes(const wri_ctx* c, int32_t nb, int32_t flags) {
     if (!c || nb <= 0 || nb > c->nb_max) return 0;
-    return ws_layout(c, nb, host_staging, kHostMaxitCap).total;
+    return ws_layout(c, nb, flags & (WS_HOST_STAGING | WS_COMPACTION), kHostMaxitCap).total;
 }
 
 int wri_set_workspace(wri_ctx* c, void* ws_dev, size_t bytes) {
@@ -694,28 +738,53 @@ int wri_apply_MH(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, float la
     return WRI_OK;
 }
 
-int wri_lsqr_begin(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const void* q_dev,
-                   const void* d_dev, float lambda, const float* tol_dev, int32_t maxit,
-                   void* u_out_dev, float* resnorms_dev, int32_t* iters_dev) {
+// ---- solver entries ----------------------------------------------------------------------------
+}  // extern "C"
+
+namespace {
+
+int lsqr_begin_impl(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const void* q_dev,
+                    const void* d_dev, float lambda, const float* tol_dev, int32_t maxit,
+                    void* u_out_dev, float* resnorms_dev, int32_t* iters_dev, bool host_staged) {
     int rc = check_batch_args(c, nb);
     if (rc) return rc;
     if (!q_dev || (c->n_rec && !d_dev) || !u_out_dev || !resnorms_dev || maxit < 0 ||
         !aligned16(q_dev) || !aligned16(u_out_dev) || q_dev == u_out_dev)
         return WRI_ERR_ARG;
     if (!c->ws) return WRI_ERR_WORKSPACE;
-    const WsLayout L = ws_layout(c, nb, 0, 0);
-    if (c->ws_bytes < L.total) return WRI_ERR_WORKSPACE;
+    const int base_flags = host_staged ? WS_HOST_STAGING : 0;
+    if (c->ws_bytes < ws_layout(c, nb, base_flags, kHostMaxitCap).total) return WRI_ERR_WORKSPACE;
+    const WsLayout L = ws_layout(c, nb, base_flags | WS_COMPACTION, kHostMaxitCap);
     if ((rc = upload_columns(c, nb, omega_idx_host, lambda))) return rc;
 
-    c->nb = nb; c->k = 0; c->maxit = maxit; c->lambda = lambda;
+    c->nb = nb; c->nb0 = nb; c->k = 0; c->maxit = maxit; c->lambda = lambda;
+    c->packed = false; c->all_done = false;
     c->U = (float2*)(c->ws + L.U); c->V = (float2*)(c->ws + L.V); c->W = (float2*)(c->ws + L.W);
     c->U_bot = (float2*)(c->ws + L.U_bot);
     c->partials = (double*)(c->ws + L.partials);
     c->partials_tma = (double*)(c->ws + L.partials_tma);
-    c->X = (float2*)u_out_dev;
+    c->X = (float2*)u_out_dev; c->u_out = (float2*)u_out_dev;
     c->tol = tol_dev; c->resnorms = resnorms_dev; c->iters_out = iters_dev;
     c->tl = make_tiling(c, nb);
     if ((rc = tma_setup(c))) return rc;
+    // Convergence is watched from the host only when tolerances are given: every check_every
+    // iterations (~2 ms of device work) the active flags are read back; converged columns are
+    // compacted away when the workspace has room for it and the batch is on the TMA path.
+    c->can_compact = tol_dev && c->tma_cb && c->ws_bytes >= L.total && !getenv("WRI_NO_COMPACT");
+    c->check_every = 0;
+    if (tol_dev) {
+        const double t_iter = 80.0 * (double)c->ng * nb / 6.0e12;
+        c->check_every = (int)std::min(32.0, std::max(1.0, std::ceil(2.0e-3 / t_iter)));
+    }
+    c->free_slots.clear();
+    if (c->can_compact) {
+        c->free_slots.push_back((float2*)(c->ws + L.B3));
+        c->free_slots.push_back((float2*)(c->ws + L.B4));
+        c->U_bot_alt = (float2*)(c->ws + L.U_bot2);
+    }
+    c->h_colmap.resize(nb);
+    for (int s = 0; s < nb; ++s) c->h_colmap[s] = s;
+    c->retired.assign(nb, 0);
     const size_t vbytes = c->ng * (size_t)nb * sizeof(float2);
     const size_t NM = c->nb_max;
 
@@ -742,33 +811,138 @@ int wri_lsqr_begin(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const 
     return WRI_OK;
 }
 
+inline unsigned blocks_for(long long n) { return (unsigned)std::min<long long>((n + 255) / 256, 148 * 16); }
+
+// x and history of the listed working columns become final in the caller's buffers:
+// u_out[:, dst] = X[:, src] + cx[src] W[:, src]; resnorms rows k+1..maxit held at phibar.
+int retire_columns(wri_ctx* c, const std::vector<int>& src, const std::vector<int>& dst) {
+    const int n = (int)src.size();
+    if (!n) return WRI_OK;
+    const size_t NM = c->nb_max;
+    int* d_src = c->idx + NM;
+    int* d_dst = c->idx + 2 * NM;
+    CK(cudaMemcpyAsync(d_src, src.data(), n * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(d_dst, dst.data(), n * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    k_retire_cols<<<blocks_for((long long)c->ng * n), 256, 0, c->stream>>>(
+        c->u_out, c->X, c->W, c->coef + C_CX * NM, d_src, d_dst, n, (long long)c->ng, c->nb, c->nb0);
+    c->launches++;
+    CK(cudaGetLastError());
+    if (c->k < c->maxit) {
+        k_hold_history<<<blocks_for((long long)(c->maxit - c->k) * n), 256, 0, c->stream>>>(
+            c->resnorms, c->stat + S_PHIBAR * NM, d_src, d_dst, n, c->k + 1, c->maxit, c->nb0);
+        c->launches++;
+        CK(cudaGetLastError());
+    }
+    for (int t = 0; t < n; ++t) c->retired[dst[t]] = 1;
+    return WRI_OK;
+}
+
+int round_up16(int n) { return (n + 15) / 16 * 16; }
+
+// Re-pack the working set to the columns still active (plus zero padding up to a multiple of 16).
+int compact_columns(wri_ctx* c, const int* act) {
+    std::vector<int> keep, rs, rd;
+    for (int j = 0; j < c->nb; ++j) {
+        const int so = c->h_colmap[j];
+        if (act[j]) keep.push_back(j);
+        else if (so >= 0 && !c->retired[so]) { rs.push_back(j); rd.push_back(so); }
+    }
+    const int new_nb = round_up16((int)keep.size());
+    if (new_nb >= c->nb) return WRI_OK;
+    int rc = retire_columns(c, rs, rd);
+    if (rc) return rc;
+    std::vector<int> map(new_nb, -1), cm(new_nb, -1);
+    for (size_t i = 0; i < keep.size(); ++i) { map[i] = keep[i]; cm[i] = c->h_colmap[keep[i]]; }
+    const size_t NM = c->nb_max;
+    CK(cudaMemcpyAsync(c->idx, map.data(), new_nb * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(c->colmap, cm.data(), new_nb * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    // vectors: gather each into a free slot, then its old slot becomes free (X = u_out is the caller's)
+    float2** vecs[4] = {&c->U, &c->V, &c->W, &c->X};
+    for (int i = 0; i < 4; ++i) {
+        if (c->free_slots.empty()) return WRI_ERR_STATE;
+        float2* dst = c->free_slots.front();
+        c->free_slots.erase(c->free_slots.begin());
+        float2* src = *vecs[i];
+        k_gather_cols<<<blocks_for((long long)c->ng * new_nb), 256, 0, c->stream>>>(
+            dst, src, c->idx, (long long)c->ng, new_nb, c->nb);
+        c->launches++;
+        CK(cudaGetLastError());
+        if (!(i == 3 && !c->packed)) c->free_slots.push_back(src);
+        *vecs[i] = dst;
+    }
+    if (c->n_rec) {
+        k_gather_cols<<<blocks_for((long long)c->n_rec * new_nb), 256, 0, c->stream>>>(
+            c->U_bot_alt, c->U_bot, c->idx, (long long)c->n_rec, new_nb, c->nb);
+        c->launches++;
+        CK(cudaGetLastError());
+        std::swap(c->U_bot, c->U_bot_alt);
+    }
+    k_gather_scalars<<<(new_nb + 127) / 128, 128, 0, c->stream>>>(
+        c->coef_alt, c->coef, c->stat_alt, c->stat, c->active_alt, c->active, c->iters_alt, c->iters,
+        c->idx, new_nb, (int)NM);
+    c->launches++;
+    CK(cudaGetLastError());
+    std::swap(c->coef, c->coef_alt); std::swap(c->stat, c->stat_alt);
+    std::swap(c->active, c->active_alt); std::swap(c->iters, c->iters_alt);
+    c->h_colmap = cm;
+    c->nb = new_nb;
+    c->packed = true;
+    c->tl = make_tiling(c, new_nb);
+    return tma_setup(c);
+}
+
+// host look at the active flags: early exit when every column has stopped, compaction when the
+// active count has dropped below the next multiple of 16
+int check_active(wri_ctx* c) {
+    CK(cudaMemcpyAsync(c->h_active, c->active, c->nb * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    int n_act = 0;
+    for (int j = 0; j < c->nb; ++j) n_act += c->h_active[j] != 0;
+    if (n_act == 0) { c->all_done = true; return WRI_OK; }
+    if (c->can_compact && round_up16(n_act) < c->nb) return compact_columns(c, c->h_active);
+    return WRI_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int wri_lsqr_begin(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const void* q_dev,
+                   const void* d_dev, float lambda, const float* tol_dev, int32_t maxit,
+                   void* u_out_dev, float* resnorms_dev, int32_t* iters_dev) {
+    return lsqr_begin_impl(c, nb, omega_idx_host, q_dev, d_dev, lambda, tol_dev, maxit, u_out_dev,
+                           resnorms_dev, iters_dev, false);
+}
+
 int wri_lsqr_iterate(wri_ctx* c, int32_t n_steps) {
     if (!c || n_steps < 0) return WRI_ERR_ARG;
     if (!c->solving) return WRI_ERR_STATE;
     if (c->k + n_steps > c->maxit) return WRI_ERR_ARG;
-    const size_t NM = c->nb_max;
     int rc;
-    for (int i = 0; i < n_steps; ++i) {
+    for (int i = 0; i < n_steps && !c->all_done; ++i) {
         c->k++;
+        const size_t NM = c->nb_max;
         if (c->tma_cb) {
             // two launches per iteration: the last CTA of each pass runs the scalar recurrences
             if ((rc = launch_tma<MODE_F>(c, PH_F))) return rc;
             if ((rc = launch_tma<MODE_A>(c, PH_A))) return rc;
-            continue;
+        } else {
+            PassParams p = base_params(c, c->nb, c->tl);
+            p.partials = c->partials;
+            // pass F: U <- (lambda/alpha) A V - (alpha/beta) U ; deferred x, w updates
+            p.in = c->V; p.out = c->U; p.W = c->W; p.X = c->X; p.sgn = 1.f;
+            p.ca = c->coef + C_CA_F * NM; p.cb = c->coef + C_CB_F * NM; p.cv = c->coef + C_CV_F * NM;
+            p.cx = c->coef + C_CX * NM; p.cw = c->coef + C_CW * NM;
+            if ((rc = launch_pass<MODE_F>(c, p, c->tl, true))) return rc;
+            if ((rc = launch_scalars<PH_F>(c, nullptr))) return rc;
+            // pass A: V <- (lambda/beta) A^H U - (beta/alpha) V
+            p.in = c->U; p.out = c->V; p.W = nullptr; p.X = nullptr; p.sgn = -1.f;
+            p.ca = c->coef + C_CA_A * NM; p.cb = c->coef + C_CB_A * NM;
+            if ((rc = launch_pass<MODE_A>(c, p, c->tl, true))) return rc;
+            if ((rc = launch_scalars<PH_A>(c, nullptr))) return rc;
         }
-        PassParams p = base_params(c, c->nb, c->tl);
-        p.partials = c->partials;
-        // pass F: U <- (lambda/alpha) A V - (alpha/beta) U ; deferred x, w updates
-        p.in = c->V; p.out = c->U; p.W = c->W; p.X = c->X; p.sgn = 1.f;
-        p.ca = c->coef + C_CA_F * NM; p.cb = c->coef + C_CB_F * NM; p.cv = c->coef + C_CV_F * NM;
-        p.cx = c->coef + C_CX * NM; p.cw = c->coef + C_CW * NM;
-        if ((rc = launch_pass<MODE_F>(c, p, c->tl, true))) return rc;
-        if ((rc = launch_scalars<PH_F>(c, nullptr))) return rc;
-        // pass A: V <- (lambda/beta) A^H U - (beta/alpha) V
-        p.in = c->U; p.out = c->V; p.W = nullptr; p.X = nullptr; p.sgn = -1.f;
-        p.ca = c->coef + C_CA_A * NM; p.cb = c->coef + C_CB_A * NM;
-        if ((rc = launch_pass<MODE_A>(c, p, c->tl, true))) return rc;
-        if ((rc = launch_scalars<PH_A>(c, nullptr))) return rc;
+        if (c->check_every && c->k % c->check_every == 0 && c->k < c->maxit)
+            if ((rc = check_active(c))) return rc;
     }
     return WRI_OK;
 }
@@ -776,11 +950,23 @@ int wri_lsqr_iterate(wri_ctx* c, int32_t n_steps) {
 int wri_lsqr_end(wri_ctx* c) {
     if (!c) return WRI_ERR_ARG;
     if (!c->solving) return WRI_ERR_STATE;
-    const long long n = (long long)c->ng * c->nb;
     const size_t NM = c->nb_max;
-    k_flush_x<<<148 * 8, 256, 0, c->stream>>>(c->X, c->W, c->coef + C_CX * NM, n, c->nb);
-    c->launches++;
-    CK(cudaGetLastError());
+    int rc;
+    if (!c->packed && c->k == c->maxit) {
+        // X is the caller's buffer: apply the last deferred update in place
+        const long long n = (long long)c->ng * c->nb;
+        k_flush_x<<<148 * 8, 256, 0, c->stream>>>(c->X, c->W, c->coef + C_CX * NM, n, c->nb);
+        c->launches++;
+        CK(cudaGetLastError());
+    } else {
+        // stopped early and / or compacted: every column not yet final is retired now
+        std::vector<int> rs, rd;
+        for (int j = 0; j < c->nb; ++j) {
+            const int so = c->h_colmap[j];
+            if (so >= 0 && !c->retired[so]) { rs.push_back(j); rd.push_back(so); }
+        }
+        if ((rc = retire_columns(c, rs, rd))) return rc;
+    }
     CK(cudaMemsetAsync(c->coef + C_CX * NM, 0, c->nb * sizeof(float), c->stream));
     c->solving = false;
     return WRI_OK;
@@ -805,7 +991,7 @@ int wri_lsqr_batch_host(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, c
         maxit > kHostMaxitCap)
         return WRI_ERR_ARG;
     if (!c->ws) return WRI_ERR_WORKSPACE;
-    const WsLayout L = ws_layout(c, nb, 1, kHostMaxitCap);
+    const WsLayout L = ws_layout(c, nb, WS_HOST_STAGING, kHostMaxitCap);
     if (c->ws_bytes < L.total) return WRI_ERR_WORKSPACE;
     const size_t vbytes = c->ng * (size_t)nb * sizeof(float2);
     const size_t dbytes = (size_t)c->n_rec * nb * sizeof(float2);
@@ -814,13 +1000,15 @@ int wri_lsqr_batch_host(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, c
     float* tols = (float*)(c->ws + L.tols);
     float* res = (float*)(c->ws + L.res);
     int* its = (int*)(c->ws + L.its);
-    // q is staged in the V slot: wri_lsqr_begin consumes q before it clears V
+    // q is staged in the V slot: the start consumes q before it clears V
     float2* Qs = (float2*)(c->ws + L.V);
     CK(cudaMemcpyAsync(Qs, q_host, vbytes, cudaMemcpyHostToDevice, c->stream));
     if (dbytes) CK(cudaMemcpyAsync(Ds, d_host, dbytes, cudaMemcpyHostToDevice, c->stream));
     if (tol_host) CK(cudaMemcpyAsync(tols, tol_host, nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));
-    rc = wri_lsqr_batch(c, nb, omega_idx_host, Qs, Ds, lambda, tol_host ? tols : nullptr, maxit, Xs, res, its);
+    rc = lsqr_begin_impl(c, nb, omega_idx_host, Qs, Ds, lambda, tol_host ? tols : nullptr, maxit, Xs, res, its, true);
     if (rc) return rc;
+    if ((rc = wri_lsqr_iterate(c, maxit))) { c->solving = false; return rc; }
+    if ((rc = wri_lsqr_end(c))) return rc;
     CK(cudaMemcpyAsync(u_out_host, Xs, vbytes, cudaMemcpyDeviceToHost, c->stream));
     CK(cudaMemcpyAsync(resnorms_host, res, (size_t)(maxit + 1) * nb * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
     if (iters_host) CK(cudaMemcpyAsync(iters_host, its, nb * sizeof(int), cudaMemcpyDeviceToHost, c->stream));

@@ -273,6 +273,8 @@ struct ScalParams {
     float lambda;
     int rows_in_pass;         // 1: the pass kernels own the receiver rows (wri_tma.cuh); the
                               //    finaliser only reduces partials and runs the recurrences
+    const int* colmap;        // [nb] working column -> caller's column (-1 = padding); null = identity
+    int nb_out;               // caller's batch width: row stride of resnorms
 };
 
 // sum over tiles of partials[.][s] in fixed order; result for column s in colsum[s] (shared)
@@ -374,7 +376,7 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
             const int act = beta > 0.0;
             p.active[s] = act;
             p.iters[s] = 0;
-            if (p.iters_out) p.iters_out[s] = 0;
+            if (p.iters_out) p.iters_out[s] = 0;      // start phases always run on the identity map
             p.resnorms[s] = (float)beta;
             // first adjoint pass: V = (lambda/beta) A^H U + (1/beta) P^T U_bot, old V = 0 with cb = 1
             cf[C_CA_A * NM + s] = act ? (float)((double)p.lambda / beta) : 0.f;
@@ -409,6 +411,7 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
             }
         } else {  // PH_A
             int act = p.active[s];
+            const int so = p.colmap ? p.colmap[s] : s;       // caller's column of working column s
             if (act) {
                 // alpha_{k+1} = ||M^H u_{k+1} - beta_{k+1} v_k||, then the plane rotation
                 const double alpha = nrm, beta = st[S_BETA * NM + s];
@@ -422,9 +425,9 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
                 st[S_RHOBAR * NM + s] = -c * alpha;
                 st[S_PHIBAR * NM + s] = phibar_n;
                 p.iters[s] = p.k;
-                if (p.iters_out) p.iters_out[s] = p.k;
+                if (p.iters_out) p.iters_out[so] = p.k;
                 const double arnorm = phibar_n * alpha * fabs(c);
-                const float tol = p.tol ? p.tol[s] : 0.f;
+                const float tol = p.tol ? p.tol[so] : 0.f;
                 bool stop = !(beta > 0.0) || !(alpha > 0.0);
                 if (tol > 0.f && arnorm <= (double)tol * st[S_AR0 * NM + s]) stop = true;
                 cf[C_CX * NM + s] = (float)(phi / rho);
@@ -442,7 +445,7 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
                 cf[C_CW * NM + s] = 0.f;
                 cf[C_CA_F * NM + s] = 0.f; cf[C_CV_F * NM + s] = 0.f; cf[C_CB_F * NM + s] = 0.f;
             }
-            p.resnorms[(size_t)p.k * nb + s] = (float)st[S_PHIBAR * NM + s];
+            if (so >= 0) p.resnorms[(size_t)p.k * p.nb_out + so] = (float)st[S_PHIBAR * NM + s];
         }
     }
     __syncthreads();
@@ -462,6 +465,73 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
                 *v = t;
             }
         }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Column compaction (shrinking active mask): converged columns leave the
+// working set, the remaining ones are re-packed to a narrower source-interleaved layout.
+
+// dst[c][j] = src[c][map[j]] (map[j] < 0 -> 0), widths nb_dst <= nb_src; dst and src are distinct buffers
+__global__ void k_gather_cols(float2* __restrict__ dst, const float2* __restrict__ src,
+                              const int* __restrict__ map, long long n_rows, int nb_dst, int nb_src) {
+    const long long n = n_rows * nb_dst;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
+         i += (long long)gridDim.x * blockDim.x) {
+        const long long c = i / nb_dst;
+        const int j = (int)(i - c * nb_dst);
+        const int m = map[j];
+        dst[i] = m >= 0 ? __ldcs(src + c * nb_src + m) : make_float2(0.f, 0.f);
+    }
+}
+
+// Retire columns: u_out[c][dst_col[t]] = X[c][src_col[t]] + cx[src_col[t]] * W[c][src_col[t]]
+// (the column's last deferred x update), t < n_ret.  X may be u_out itself (same column).
+__global__ void k_retire_cols(float2* u_out, const float2* X, const float2* __restrict__ W,
+                              const float* __restrict__ cx, const int* __restrict__ src_col,
+                              const int* __restrict__ dst_col, int n_ret, long long n_rows, int nb_src,
+                              int nb_out) {
+    const long long n = n_rows * n_ret;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
+         i += (long long)gridDim.x * blockDim.x) {
+        const long long c = i / n_ret;
+        const int t = (int)(i - c * n_ret);
+        const int js = src_col[t];
+        const float a = cx[js];
+        float2 x = X[c * nb_src + js];
+        if (a != 0.f) {
+            const float2 w = W[c * nb_src + js];
+            x.x = fmaf(a, w.x, x.x);
+            x.y = fmaf(a, w.y, x.y);
+        }
+        u_out[c * nb_out + dst_col[t]] = x;
+    }
+}
+
+// history of retired columns is held at the stop value (reading C-9): rows k0..maxit
+__global__ void k_hold_history(float* __restrict__ resnorms, const double* __restrict__ phibar,
+                               const int* __restrict__ src_col, const int* __restrict__ dst_col, int n_ret,
+                               int k0, int maxit, int nb_out) {
+    const long long n = (long long)(maxit - k0 + 1) * n_ret;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
+         i += (long long)gridDim.x * blockDim.x) {
+        const int row = (int)(i / n_ret), t = (int)(i - (long long)row * n_ret);
+        resnorms[(size_t)(k0 + row) * nb_out + dst_col[t]] = (float)phibar[src_col[t]];
+    }
+}
+
+// per-column scalar rows follow the vectors: dst bank <- src bank through map (padding -> 0 / inactive)
+__global__ void k_gather_scalars(float* __restrict__ coef_dst, const float* __restrict__ coef_src,
+                                 double* __restrict__ stat_dst, const double* __restrict__ stat_src,
+                                 int* __restrict__ act_dst, const int* __restrict__ act_src,
+                                 int* __restrict__ it_dst, const int* __restrict__ it_src,
+                                 const int* __restrict__ map, int nb_dst, int nb_max) {
+    for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < nb_dst; j += gridDim.x * blockDim.x) {
+        const int m = map[j];
+        for (int r = 0; r < N_COEF; ++r) coef_dst[r * nb_max + j] = m >= 0 ? coef_src[r * nb_max + m] : 0.f;
+        for (int r = 0; r < N_STAT; ++r) stat_dst[r * nb_max + j] = m >= 0 ? stat_src[r * nb_max + m] : 0.0;
+        act_dst[j] = m >= 0 ? act_src[m] : 0;
+        it_dst[j] = m >= 0 ? it_src[m] : 0;
     }
 }
 

@@ -254,6 +254,60 @@ def test_adaptive_masks_config3(torch_cuda):
         assert np.all(res[k:, s] == res[k, s])               # history held after the stop
 
 
+def test_column_compaction_matches_uncompacted_and_oracle(torch_cuda, monkeypatch):
+    """48 columns on the TMA path with tolerances spread over two decades: converged columns are
+    compacted out of the working set (48 -> 32 -> 16 columns) and the solve returns once all have
+    stopped.  Stop iterations, wavefields and histories must match the same solve without
+    compaction and the oracle."""
+    torch = torch_cuda
+    w = workloads.make("config3", grid=(50, 50, 40), nb=48)
+    rng = np.random.Generator(np.random.PCG64(5))
+    w.tol[:] = (10.0 ** rng.uniform(-2.0, -0.7, w.nb)).astype(np.float32)
+    w.tol[7] = 0.0                                           # one column runs to maxit
+    maxit = 90
+    q, d = torch.from_numpy(w.Q).cuda(), torch.from_numpy(w.D).cuda()
+    tol = torch.from_numpy(w.tol).cuda()
+
+    def run(no_compact):
+        if no_compact:
+            monkeypatch.setenv("WRI_NO_COMPACT", "1")
+        else:
+            monkeypatch.delenv("WRI_NO_COMPACT", raising=False)
+        ctx = _wri(w)
+        out = [t.cpu().numpy() for t in ctx.lsqr_batch(q, d, w.lam, tol, maxit=maxit, omega_idx=w.omega_idx)]
+        return out, ctx.lsqr_peek()["nb"], ctx.launch_count()
+
+    (u, res, it), nb_end, n1 = run(False)
+    (u0, res0, it0), nb_end0, n0 = run(True)
+    assert nb_end0 == 48 and nb_end == 16                    # the working set really shrank
+    assert np.array_equal(it, it0) and it[7] == maxit and len(set(it.tolist())) > 8
+    assert np.isfinite(u.view(np.float32)).all()
+    for s in range(w.nb):
+        assert rel(u[:, s], u0[:, s]) < 2e-5, s
+        assert rel(res[:, s], res0[:, s]) < 1e-6, s
+        assert np.all(res[it[s]:, s] == res[it[s], s])       # history held after the stop
+    rec = O.rec_cells(w.nx, w.ny, w.nz, w.rec_ijk)
+    ops = ops_for(w)
+    for s in (0, 7, 19, 33, 47):
+        ref = O.lsqr(ops[s], w.m, w.lam, rec, w.Q[:, s], w.D[:, s], tol=float(w.tol[s]), maxit=maxit)
+        assert abs(int(it[s]) - int(ref["iters"])) <= 2, (s, it[s], ref["iters"])
+        same = O.lsqr(ops[s], w.m, w.lam, rec, w.Q[:, s], w.D[:, s], tol=0.0, maxit=int(it[s]))
+        lim = 1e-3 if it[s] <= 60 else 5e-2
+        assert rel(u[:, s], same["x"]) < lim, (s, it[s])
+        assert rel(res[:it[s] + 1, s], same["resnorms"]) < 5e-3
+
+    # every column converges early: the solve stops before maxit and still fills the history
+    w.tol[:] = 5e-2
+    tol2 = torch.from_numpy(w.tol).cuda()
+    ctx = _wri(w)
+    u2, res2, it2 = [t.cpu().numpy() for t in ctx.lsqr_batch(q, d, w.lam, tol2, maxit=maxit, omega_idx=w.omega_idx)]
+    assert it2.max() < maxit and ctx.lsqr_peek()["k"] < maxit
+    for s in (0, 21, 47):
+        same = O.lsqr(ops[s], w.m, w.lam, rec, w.Q[:, s], w.D[:, s], tol=0.0, maxit=int(it2[s]))
+        assert rel(u2[:, s], same["x"]) < 1e-3
+        assert np.all(res2[it2[s]:, s] == res2[it2[s], s]) and res2[maxit, s] > 0
+
+
 def test_degenerate_columns_and_determinism(torch_cuda):
     """b = 0 column -> x = 0, iters = 0, no NaN anywhere; no receivers; two runs bit-identical."""
     torch = torch_cuda
