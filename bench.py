@@ -247,7 +247,7 @@ def run_ours(args, wl_name, w):
     barrier()
     ms = e0.elapsed_time(e1)
     launches = ctx.launch_count() - l0
-    ms_f, n_f, ms_a, n_a = ctx.profile_read()
+    ms_f, n_f, cols_f, ms_a, n_a, cols_a = ctx.profile_read()
     ctx.profile_enable(False)
     clocks = sampler.stop() if rank == 0 else None
 
@@ -278,9 +278,11 @@ def run_ours(args, wl_name, w):
         value = iters_all * args.steps / (ms * 1e-3)
         peak, peak_src = measured_hbm_peak()
         cells = w.ng * nb
-        bytes_f = BYTES_PASS_F * cells + 4 * w.ng
+        # bytes per launch from the widths the launches really had (compaction narrows the batch)
+        bytes_f = (BYTES_PASS_F * w.ng * cols_f + 4 * w.ng * n_f) / max(n_f, 1)
+        bytes_a = (BYTES_PASS_A * w.ng * cols_a + 4 * w.ng * n_a) / max(n_a, 1)
         ach_f = bytes_f / (ms_f / max(n_f, 1) * 1e-3) / 1e9 if n_f else None
-        ach_a = (BYTES_PASS_A * cells + 4 * w.ng) / (ms_a / max(n_a, 1) * 1e-3) / 1e9 if n_a else None
+        ach_a = bytes_a / (ms_a / max(n_a, 1) * 1e-3) / 1e9 if n_a else None
         # whole-iteration algorithmic bandwidth over the full step (includes start/end kernels)
         ach_iter = BYTES_ITER * w.ng * iters_per_step * args.steps / (ms * 1e-3) / 1e9
         line = {
@@ -297,9 +299,11 @@ def run_ours(args, wl_name, w):
             "gpu_launches": launches_all,
             "roofline": {"bound": "hbm", "kernel": "k_pass<MODE_F> (forward stencil + u axpy + x,w update + ||u||^2)",
                          "achieved": ach_f, "peak": peak, "peak_source": peak_src, "unit": "GB/s",
-                         "frac": (ach_f / peak) if ach_f else None, "traffic": ncu_traffic_bytes(),
+                         "frac": (ach_f / peak) if ach_f else None,
+                         "traffic": ncu_traffic_bytes() if wl_name == DEFAULT_WORKLOAD else None,
                          "algorithmic_bytes_per_launch": bytes_f,
                          "avg_launch_ms": ms_f / max(n_f, 1), "launches_timed": n_f,
+                         "avg_columns_per_launch": cols_f / max(n_f, 1),
                          "pass_a": {"achieved": ach_a, "frac": (ach_a / peak) if ach_a else None,
                                     "avg_launch_ms": ms_a / max(n_a, 1)},
                          "whole_step": {"achieved": ach_iter, "frac": ach_iter / peak,

@@ -169,12 +169,13 @@ int64_t wri_launch_count(const wri_ctx* ctx);
 
 /* Per-kernel timing for the roofline report: while enabled, the two stencil passes of every
  * LSQR iteration are bracketed by CUDA events on the context's stream.  wri_profile_read
- * synchronises the stream, returns the summed durations (ms) and launch counts of pass F
- * (forward operator + x/w update) and pass A (adjoint operator) since the last read, and
- * resets the counters.                                                                       */
+ * synchronises the stream and returns, for pass F (forward operator + x/w update) and pass A
+ * (adjoint operator) since the last read: the summed durations (ms), the launch counts and the
+ * summed working batch widths of those launches (so that bytes moved = bytes per cell-column
+ * x n_g x cols even when compaction narrows the batch); then resets the counters.           */
 int wri_profile_enable(wri_ctx* ctx, int32_t on);
-int wri_profile_read(wri_ctx* ctx, double* ms_pass_f, int64_t* n_pass_f,
-                     double* ms_pass_a, int64_t* n_pass_a);
+int wri_profile_read(wri_ctx* ctx, double* ms_pass_f, int64_t* n_pass_f, int64_t* cols_pass_f,
+                     double* ms_pass_a, int64_t* n_pass_a, int64_t* cols_pass_a);
 
 int wri_destroy(wri_ctx* ctx);
 

@@ -79,7 +79,7 @@ def load_library():
     lib.wri_launch_count.argtypes = [P]
     lib.wri_launch_count.restype = C.c_int64
     lib.wri_profile_enable.argtypes = [P, I32]
-    lib.wri_profile_read.argtypes = [P, P, P, P, P]
+    lib.wri_profile_read.argtypes = [P, P, P, P, P, P, P]
     lib.wri_destroy.argtypes = [P]
     lib.wri_strerror.argtypes = [C.c_int]
     lib.wri_strerror.restype = C.c_char_p
@@ -269,11 +269,13 @@ class Wri:
         _ck(self._lib.wri_profile_enable(self._h, int(bool(on))))
 
     def profile_read(self):
-        """(ms_pass_f, n_pass_f, ms_pass_a, n_pass_a) since the last read; synchronises."""
+        """(ms_pass_f, n_pass_f, cols_pass_f, ms_pass_a, n_pass_a, cols_pass_a) since the last read;
+        synchronises."""
         mf, ma = C.c_double(), C.c_double()
-        nf, na = C.c_int64(), C.c_int64()
-        _ck(self._lib.wri_profile_read(self._h, C.byref(mf), C.byref(nf), C.byref(ma), C.byref(na)))
-        return mf.value, nf.value, ma.value, na.value
+        nf, na, cf, ca = C.c_int64(), C.c_int64(), C.c_int64(), C.c_int64()
+        _ck(self._lib.wri_profile_read(self._h, C.byref(mf), C.byref(nf), C.byref(cf), C.byref(ma),
+                                       C.byref(na), C.byref(ca)))
+        return mf.value, nf.value, cf.value, ma.value, na.value, ca.value
 
     def launch_count(self):
         return int(self._lib.wri_launch_count(self._h))

@@ -31,7 +31,7 @@ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 constexpr int kMaxCtas = 512;          // upper bound on the persistent grid (>= SM count)
-constexpr int kMinChunk = 16;          // narrowest column chunk of the TMA path
+constexpr int kMinChunk = 4;           // narrowest column chunk of the TMA path
 
 struct Tiling {
     int vec;            // complex numbers per thread (2 = 128-bit accesses)
@@ -100,12 +100,14 @@ struct wri_ctx {
         int txc = 0, tyc = 0, ntx = 0, nty = 0, ntz = 0, zc = 0, nchunk = 0, tiles = 0, grid = 0;
         CUtensorMap in{}, old{}, w{}, x{}, m{};
         int m_tma = 0;                    // model tile rides in the TMA stage
+        int merged = 0;                   // tensor maps fold (column, x)
     } planF, planA;
     double* partials_tma = nullptr;       // [grid][nb]
     // optional per-kernel timing (wri_profile_*)
     bool profiling = false;
     std::vector<cudaEvent_t> ev_pool;     // pairs: start, stop
     std::vector<int> ev_kind;             // per pair: 0 = pass F, 1 = pass A
+    std::vector<int> ev_cols;             // per pair: working batch width of that launch
     size_t ev_used = 0;                   // pairs in use
 };
 
@@ -205,10 +207,11 @@ int launch_pass(wri_ctx* c, const PassParams& p, const Tiling& t, bool timed = f
             cudaEvent_t a, b;
             CK(cudaEventCreate(&a));
             CK(cudaEventCreate(&b));
-            c->ev_pool.push_back(a); c->ev_pool.push_back(b); c->ev_kind.push_back(0);
+            c->ev_pool.push_back(a); c->ev_pool.push_back(b); c->ev_kind.push_back(0); c->ev_cols.push_back(0);
         }
         e0 = c->ev_pool[2 * c->ev_used]; e1 = c->ev_pool[2 * c->ev_used + 1];
         c->ev_kind[c->ev_used] = (MODE == MODE_F) ? 0 : 1;
+        c->ev_cols[c->ev_used] = c->nb;
         c->ev_used++;
         CK(cudaEventRecord(e0, c->stream));
     }
@@ -265,13 +268,21 @@ EncodeTiledFn get_encode_fn() {
 
 // 4-D view (column, x, y, z) of a source-interleaved complex64 vector; one element = 8 bytes.
 // Out-of-range box elements are zero-filled (the Dirichlet closure of the stencil).
-int make_tmap(CUtensorMap* tm, const void* base, const wri_ctx* c, int nb, int cb, int bx, int by) {
+// merged (nb == cb only): (column, x) folded into one dimension of nb*nx contiguous elements, so a box
+// row is cb*bx elements (<= 256) — narrow chunks would otherwise move 32-128 byte rows
+int make_tmap(CUtensorMap* tm, const void* base, const wri_ctx* c, int nb, int cb, int bx, int by,
+              bool merged = false) {
     EncodeTiledFn fn = get_encode_fn();
     if (!fn) return cuda_fail(cudaErrorNotSupported, "cuTensorMapEncodeTiled lookup");
     cuuint64_t gdim[4] = {(cuuint64_t)nb, (cuuint64_t)c->g.nx, (cuuint64_t)c->g.ny, (cuuint64_t)c->g.nz};
     cuuint64_t gstr[3] = {(cuuint64_t)nb * 8, (cuuint64_t)nb * 8 * c->g.nx,
                           (cuuint64_t)nb * 8 * c->g.nx * c->g.ny};
     cuuint32_t box[4] = {(cuuint32_t)cb, (cuuint32_t)bx, (cuuint32_t)by, 1};
+    if (merged) {
+        gdim[0] = (cuuint64_t)nb * c->g.nx; gdim[1] = (cuuint64_t)c->g.ny; gdim[2] = (cuuint64_t)c->g.nz; gdim[3] = 1;
+        gstr[0] = (cuuint64_t)nb * 8 * c->g.nx; gstr[1] = gstr[0] * c->g.ny; gstr[2] = gstr[1] * c->g.nz;
+        box[0] = (cuuint32_t)(cb * bx); box[1] = (cuuint32_t)by; box[2] = 1; box[3] = 1;
+    }
     cuuint32_t estr[4] = {1, 1, 1, 1};
     CUtensorMapL2promotion promo = CU_TENSOR_MAP_L2_PROMOTION_L2_256B;
     if (const char* e = getenv("WRI_L2PROMO")) promo = (CUtensorMapL2promotion)atoi(e);
@@ -309,12 +320,30 @@ template <int CB, int MODE> struct CfgFor {
     static constexpr int S = 64 / CB;   // narrower chunks -> proportionally more cells per tile row
     typedef TileCfg<CB, (MODE == MODE_F ? WRI_F_TX : WRI_A_TX) * (S >= 2 ? 2 : 1),
                     (MODE == MODE_F ? WRI_F_TY : WRI_A_TY) * (S >= 4 ? 2 : 1),
-                    (MODE == MODE_F ? WRI_F_NT : WRI_A_NT)> type;
+                    (MODE == MODE_F ? WRI_F_NT : WRI_A_NT), PassTraits<MODE>::NSTAGE> type;
 };
 
-// 48 columns: 4 x 4 cells x 48 columns = 768 complex per plane, 384 (F) / 192 (A) consumer threads
+// 48 columns: 4 x 4 cells x 48 columns = 768 complex per plane, 384 consumer threads (one item each)
+#ifndef WRI_F48_NT
+#define WRI_F48_NT 384
+#endif
+#ifndef WRI_A48_NT
+#define WRI_A48_NT 384
+#endif
+#ifndef WRI_A48_STAGES
+#define WRI_A48_STAGES 8
+#endif
 template <int MODE> struct CfgFor<48, MODE> {
-    typedef TileCfg<48, 4, 4, (MODE == MODE_F ? 384 : 192)> type;
+    typedef TileCfg<48, 4, 4, (MODE == MODE_F ? WRI_F48_NT : WRI_A48_NT),
+                    (MODE == MODE_F ? PassTraits<MODE_F>::NSTAGE : WRI_A48_STAGES)> type;
+};
+
+// 8 / 4 columns (the tail of a shrinking batch): 16 x 8 / 16 x 16 cells, always one chunk per cell
+template <int MODE> struct CfgFor<8, MODE> {
+    typedef TileCfg<8, 16, 8, (MODE == MODE_F ? WRI_F_NT : WRI_A_NT), PassTraits<MODE>::NSTAGE> type;
+};
+template <int MODE> struct CfgFor<4, MODE> {
+    typedef TileCfg<4, 16, 16, (MODE == MODE_F ? WRI_F_NT : WRI_A_NT), PassTraits<MODE>::NSTAGE> type;
 };
 
 int tma_chunk_for(int nb) {
@@ -324,14 +353,15 @@ int tma_chunk_for(int nb) {
     if (nb % 48 == 0) return 48;
     if (nb % 32 == 0) return 32;
     if (nb % 16 == 0) return 16;
+    if (nb == 8 || nb == 4) return nb;
     return 0;
 }
 
 template <class Cfg, int MODE>
 size_t tma_smem_bytes(const wri_ctx* c) {
-    return (size_t)PassTraits<MODE>::NSTAGE *
+    return (size_t)Cfg::NSTAGE *
                (Cfg::IN_BYTES + PassTraits<MODE>::NSTREAM * Cfg::CTR_BYTES + Cfg::M_BYTES) +
-           2 * PassTraits<MODE>::NSTAGE * 8 + (size_t)c->nb * 8 + (size_t)Cfg::NT * 2 * 8 +
+           2 * Cfg::NSTAGE * 8 + (size_t)c->nb * 8 + (size_t)Cfg::NT * 2 * 8 +
            (size_t)(c->g.nx + c->g.ny + c->g.nz) * 4 + (size_t)6 * c->nb * 4;
 }
 
@@ -373,11 +403,13 @@ int tma_plan(wri_ctx* c, wri_ctx::TmaPlan& P, const void* in, const void* old, b
     P.tiles = (int)tiles;
     P.grid = (int)std::min<long long>(tiles, std::min(c->num_sms, kMaxCtas));
     int rc;
-    if ((rc = make_tmap(&P.in, in, c, c->nb, Cfg::CB, P.txc + 2, P.tyc + 2))) return rc;
-    if ((rc = make_tmap(&P.old, old, c, c->nb, Cfg::CB, P.txc, P.tyc))) return rc;
+    const bool mg = P.nchunk == 1 && Cfg::CB * (P.txc + 2) <= 256 && !getenv("WRI_NO_MERGE");
+    P.merged = mg;
+    if ((rc = make_tmap(&P.in, in, c, c->nb, Cfg::CB, P.txc + 2, P.tyc + 2, mg))) return rc;
+    if ((rc = make_tmap(&P.old, old, c, c->nb, Cfg::CB, P.txc, P.tyc, mg))) return rc;
     if (is_f) {
-        if ((rc = make_tmap(&P.w, c->W, c, c->nb, Cfg::CB, P.txc, P.tyc))) return rc;
-        if ((rc = make_tmap(&P.x, c->X, c, c->nb, Cfg::CB, P.txc, P.tyc))) return rc;
+        if ((rc = make_tmap(&P.w, c->W, c, c->nb, Cfg::CB, P.txc, P.tyc, mg))) return rc;
+        if ((rc = make_tmap(&P.x, c->X, c, c->nb, Cfg::CB, P.txc, P.tyc, mg))) return rc;
     } else {
         P.w = P.old; P.x = P.old;          // unused by pass A
     }
@@ -435,6 +467,12 @@ int tma_setup(wri_ctx* c) {
         case 32:
             if ((rc = tma_plan<CfgFor<32, MODE_F>::type>(c, c->planF, c->V, c->U, true))) return rc;
             return tma_plan<CfgFor<32, MODE_A>::type>(c, c->planA, c->U, c->V, false);
+        case 8:
+            if ((rc = tma_plan<CfgFor<8, MODE_F>::type>(c, c->planF, c->V, c->U, true))) return rc;
+            return tma_plan<CfgFor<8, MODE_A>::type>(c, c->planA, c->U, c->V, false);
+        case 4:
+            if ((rc = tma_plan<CfgFor<4, MODE_F>::type>(c, c->planF, c->V, c->U, true))) return rc;
+            return tma_plan<CfgFor<4, MODE_A>::type>(c, c->planA, c->U, c->V, false);
         default:
             if ((rc = tma_plan<CfgFor<16, MODE_F>::type>(c, c->planF, c->V, c->U, true))) return rc;
             return tma_plan<CfgFor<16, MODE_A>::type>(c, c->planA, c->U, c->V, false);
@@ -479,6 +517,7 @@ int launch_tma_cfg(wri_ctx* c, int phase) {
     p.m6ih2 = (float)(-6.0 / (c->h * c->h));
     p.phase = phase;
     p.m_tma = P.m_tma;
+    p.merged = P.merged;
     p.fin = scal_params(c, c->partials_tma, P.grid, nullptr);
     p.n_rec = c->n_rec; p.rec = c->rec; p.U_bot = c->U_bot; p.V = c->V;
     p.ct = c->coef + C_CT_A * NM; p.own_ptr = c->own_ptr; p.own = c->own;
@@ -497,11 +536,12 @@ int launch_tma_cfg(wri_ctx* c, int phase) {
             cudaEvent_t a, b;
             CK(cudaEventCreate(&a));
             CK(cudaEventCreate(&b));
-            c->ev_pool.push_back(a); c->ev_pool.push_back(b); c->ev_kind.push_back(0);
+            c->ev_pool.push_back(a); c->ev_pool.push_back(b); c->ev_kind.push_back(0); c->ev_cols.push_back(0);
         }
         cudaEvent_t e0 = c->ev_pool[2 * c->ev_used];
         e1 = c->ev_pool[2 * c->ev_used + 1];
         c->ev_kind[c->ev_used] = (MODE == MODE_F) ? 0 : 1;
+        c->ev_cols[c->ev_used] = c->nb;
         c->ev_used++;
         CK(cudaEventRecord(e0, c->stream));
     }
@@ -518,6 +558,8 @@ int launch_tma(wri_ctx* c, int phase) {
         case 64: return launch_tma_cfg<typename CfgFor<64, MODE>::type, MODE>(c, phase);
         case 48: return launch_tma_cfg<typename CfgFor<48, MODE>::type, MODE>(c, phase);
         case 32: return launch_tma_cfg<typename CfgFor<32, MODE>::type, MODE>(c, phase);
+        case 8: return launch_tma_cfg<typename CfgFor<8, MODE>::type, MODE>(c, phase);
+        case 4: return launch_tma_cfg<typename CfgFor<4, MODE>::type, MODE>(c, phase);
         default: return launch_tma_cfg<typename CfgFor<16, MODE>::type, MODE>(c, phase);
     }
 }
@@ -679,14 +721,16 @@ int wri_profile_enable(wri_ctx* c, int32_t on) {
     return WRI_OK;
 }
 
-int wri_profile_read(wri_ctx* c, double* ms_f, int64_t* n_f, double* ms_a, int64_t* n_a) {
-    if (!c || !ms_f || !n_f || !ms_a || !n_a) return WRI_ERR_ARG;
+int wri_profile_read(wri_ctx* c, double* ms_f, int64_t* n_f, int64_t* cols_f, double* ms_a, int64_t* n_a,
+                     int64_t* cols_a) {
+    if (!c || !ms_f || !n_f || !cols_f || !ms_a || !n_a || !cols_a) return WRI_ERR_ARG;
     CK(cudaStreamSynchronize(c->stream));
-    *ms_f = *ms_a = 0.0; *n_f = *n_a = 0;
+    *ms_f = *ms_a = 0.0; *n_f = *n_a = 0; *cols_f = *cols_a = 0;
     for (size_t i = 0; i < c->ev_used; ++i) {
         float ms = 0.f;
         CK(cudaEventElapsedTime(&ms, c->ev_pool[2 * i], c->ev_pool[2 * i + 1]));
-        if (c->ev_kind[i] == 0) { *ms_f += ms; ++*n_f; } else { *ms_a += ms; ++*n_a; }
+        if (c->ev_kind[i] == 0) { *ms_f += ms; ++*n_f; *cols_f += c->ev_cols[i]; }
+        else { *ms_a += ms; ++*n_a; *cols_a += c->ev_cols[i]; }
     }
     c->ev_used = 0;
     return WRI_OK;
@@ -837,7 +881,8 @@ int retire_columns(wri_ctx* c, const std::vector<int>& src, const std::vector<in
     return WRI_OK;
 }
 
-int round_up16(int n) { return (n + 15) / 16 * 16; }
+// working widths the TMA path serves: 4, 8, then multiples of 16
+int round_up16(int n) { return n <= 4 ? 4 : n <= 8 ? 8 : (n + 15) / 16 * 16; }
 
 // Re-pack the working set to the columns still active (plus zero padding up to a multiple of 16).
 int compact_columns(wri_ctx* c, const int* act) {

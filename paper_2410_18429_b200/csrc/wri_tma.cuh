@@ -23,10 +23,11 @@
 
 namespace wri {
 
-template <int CB_, int TXC_, int TYC_, int NT_>
+template <int CB_, int TXC_, int TYC_, int NT_, int NSTAGE_>
 struct TileCfg {
     static constexpr int CB = CB_, TXC = TXC_, TYC = TYC_;
     static constexpr int NT = NT_;                              // consumer threads
+    static constexpr int NSTAGE = NSTAGE_;                      // depth of the shared-memory ring
     static constexpr int ITEMS = TXC * TYC * CB / 2;            // 16-byte items per plane
     static constexpr int IPT = ITEMS / NT;                      // items per thread
     static constexpr int IN_BYTES = (TXC + 2) * (TYC + 2) * CB * 8;
@@ -44,7 +45,7 @@ template <int MODE> struct PassTraits;
 #ifndef WRI_A_STAGES
 #define WRI_A_STAGES 6
 #endif
-template <> struct PassTraits<MODE_F> { static constexpr int NSTREAM = 3, NSTAGE = WRI_F_STAGES; };
+template <> struct PassTraits<MODE_F> { static constexpr int NSTREAM = 3, NSTAGE = WRI_F_STAGES; };   // default depths
 template <> struct PassTraits<MODE_A> { static constexpr int NSTREAM = 1, NSTAGE = WRI_A_STAGES; };
 
 struct TmaPassParams {
@@ -60,6 +61,7 @@ struct TmaPassParams {
     int zc, ntx, nty, ntz, nchunk, n_tiles;
     float ih2, m6ih2, sgn;
     int m_tma;             // 1: the model tile rides in the TMA stage (needs nx % 4 == 0)
+    int merged;            // 1: tensor maps fold (column, x) into one dimension (nchunk == 1)
     int phase;             // ScalPhase run by the last CTA
     // receiver rows, spread over the CTAs (keeps them off the last CTA's serial tail)
     int n_rec;
@@ -176,7 +178,7 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
            const __grid_constant__ CUtensorMap tm_w, const __grid_constant__ CUtensorMap tm_x,
            const __grid_constant__ CUtensorMap tm_m, const TmaPassParams p) {
     constexpr int CB = Cfg::CB, TXC = Cfg::TXC, TYC = Cfg::TYC, NT = Cfg::NT, IPT = Cfg::IPT;
-    constexpr int NSTREAM = PassTraits<MODE>::NSTREAM, NSTAGE = PassTraits<MODE>::NSTAGE;
+    constexpr int NSTREAM = PassTraits<MODE>::NSTREAM, NSTAGE = Cfg::NSTAGE;
     constexpr int M_OFF = Cfg::IN_BYTES + NSTREAM * Cfg::CTR_BYTES;
     constexpr int STAGE_BYTES = M_OFF + Cfg::M_BYTES;
     constexpr int HP = CB / 2;                                  // column pairs per cell
@@ -218,6 +220,9 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
         // ------------------------------------------------------------------ producer warp
         // (all 32 lanes walk the loops together; lane 0 issues)
         const bool issuer = (tid == NT);
+        // merged maps (narrow chunks, one chunk per cell): the column index is folded into x, so a
+        // box row is CB*(TXC+2) contiguous elements instead of CB:  (x*CB, y, z, 0)
+        const bool mg = p.merged != 0;
 #if WRI_HINTS >= 1
         const uint64_t pol_stream = policy_evict_first();
 #endif
@@ -243,22 +248,22 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
                                                             (p.m_tma ? TXC * TYC * 4 : 0) : 0));
                     const uint32_t dst = smem_u32(stages + stage * STAGE_BYTES);
 #if WRI_HINTS >= 2
-                    tma_load_4d_hint(dst, &tm_in, fb, c0, x0 - 1, y0 - 1, pl, pol_in);
+                    tma_load_4d_hint(dst, &tm_in, fb, mg ? (x0 - 1) * CB : c0, mg ? y0 - 1 : x0 - 1, mg ? pl : y0 - 1, mg ? 0 : pl, pol_in);
 #else
-                    tma_load_4d(dst, &tm_in, fb, c0, x0 - 1, y0 - 1, pl);
+                    tma_load_4d(dst, &tm_in, fb, mg ? (x0 - 1) * CB : c0, mg ? y0 - 1 : x0 - 1, mg ? pl : y0 - 1, mg ? 0 : pl);
 #endif
                     if (streams) {
 #if WRI_HINTS >= 1
-                        tma_load_4d_hint(dst + Cfg::IN_BYTES, &tm_old, fb, c0, x0, y0, pl - 1, pol_stream);
+                        tma_load_4d_hint(dst + Cfg::IN_BYTES, &tm_old, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1, pol_stream);
                         if (MODE == MODE_F) {
-                            tma_load_4d_hint(dst + Cfg::IN_BYTES + Cfg::CTR_BYTES, &tm_w, fb, c0, x0, y0, pl - 1, pol_stream);
-                            tma_load_4d_hint(dst + Cfg::IN_BYTES + 2 * Cfg::CTR_BYTES, &tm_x, fb, c0, x0, y0, pl - 1, pol_stream);
+                            tma_load_4d_hint(dst + Cfg::IN_BYTES + Cfg::CTR_BYTES, &tm_w, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1, pol_stream);
+                            tma_load_4d_hint(dst + Cfg::IN_BYTES + 2 * Cfg::CTR_BYTES, &tm_x, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1, pol_stream);
                         }
 #else
-                        tma_load_4d(dst + Cfg::IN_BYTES, &tm_old, fb, c0, x0, y0, pl - 1);
+                        tma_load_4d(dst + Cfg::IN_BYTES, &tm_old, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1);
                         if (MODE == MODE_F) {
-                            tma_load_4d(dst + Cfg::IN_BYTES + Cfg::CTR_BYTES, &tm_w, fb, c0, x0, y0, pl - 1);
-                            tma_load_4d(dst + Cfg::IN_BYTES + 2 * Cfg::CTR_BYTES, &tm_x, fb, c0, x0, y0, pl - 1);
+                            tma_load_4d(dst + Cfg::IN_BYTES + Cfg::CTR_BYTES, &tm_w, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1);
+                            tma_load_4d(dst + Cfg::IN_BYTES + 2 * Cfg::CTR_BYTES, &tm_x, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1);
                         }
 #endif
                         if (p.m_tma) tma_load_3d(dst + M_OFF, &tm_m, fb, x0, y0, pl - 1);

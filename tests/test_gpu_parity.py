@@ -100,6 +100,8 @@ TF_CASES = [
     ("config4", dict(grid=(19, 22, 35), nb=32), 5),
     ("config3", dict(grid=(27, 25, 20), nb=48), 5),
     ("config1", dict(grid=(32, 32, 32), nb=16), 5),
+    ("config1", dict(grid=(21, 34, 19), nb=8), 4),
+    ("config2", dict(grid=(30, 17, 22), nb=4), 4),
 ]
 
 
@@ -190,6 +192,9 @@ def test_free_running_config1_50_iterations(torch_cuda):
     ("config2", dict(grid=(45, 38, 70), nb=64), [0, 21, 42, 63]),      # TMA path, 3 z-chunks
     ("config4", dict(grid=(40, 44, 36), nb=32), [0, 13, 31]),
     ("config3", dict(grid=(50, 50, 40), nb=48), [0, 17, 47]),
+    ("config1", dict(grid=(45, 38, 36), nb=16), [0, 9, 15]),           # merged (column, x) tensor maps
+    ("config1", dict(grid=(37, 41, 40), nb=8), None),                  # 8- and 4-column tiles
+    ("config4", dict(grid=(33, 35, 34), nb=4), None),
 ])
 def test_free_running_scaled_configs(torch_cuda, name, kw, cols):
     w = workloads.make(name, **kw)
@@ -256,7 +261,7 @@ def test_adaptive_masks_config3(torch_cuda):
 
 def test_column_compaction_matches_uncompacted_and_oracle(torch_cuda, monkeypatch):
     """48 columns on the TMA path with tolerances spread over two decades: converged columns are
-    compacted out of the working set (48 -> 32 -> 16 columns) and the solve returns once all have
+    compacted out of the working set (48 -> 32 -> 16 -> 8 -> 4 columns) and the solve returns once all have
     stopped.  Stop iterations, wavefields and histories must match the same solve without
     compaction and the oracle."""
     torch = torch_cuda
@@ -279,7 +284,7 @@ def test_column_compaction_matches_uncompacted_and_oracle(torch_cuda, monkeypatc
 
     (u, res, it), nb_end, n1 = run(False)
     (u0, res0, it0), nb_end0, n0 = run(True)
-    assert nb_end0 == 48 and nb_end == 16                    # the working set really shrank
+    assert nb_end0 == 48 and nb_end == 4                     # the working set really shrank (48 -> ... -> 4)
     assert np.array_equal(it, it0) and it[7] == maxit and len(set(it.tolist())) > 8
     assert np.isfinite(u.view(np.float32)).all()
     for s in range(w.nb):
