@@ -51,6 +51,17 @@ class _RefState(C.Structure):
                 ("stop", C.c_int32)]
 
 
+class _RefStateSF(C.Structure):
+    _fields_ = [("u_top", C.c_void_p), ("u_bot", C.c_void_p), ("v", C.c_void_p),
+                ("w", C.c_void_p), ("x", C.c_void_p),
+                ("v_a", C.c_double * 2), ("w_a", C.c_double * 2), ("x_a", C.c_double * 2),
+                ("alpha", C.c_double), ("beta", C.c_double),
+                ("rhobar", C.c_double), ("phibar", C.c_double),
+                ("rho", C.c_double), ("c", C.c_double), ("s", C.c_double),
+                ("theta", C.c_double), ("phi", C.c_double), ("arnorm", C.c_double),
+                ("stop", C.c_int32)]
+
+
 _lib = None
 
 
@@ -69,8 +80,19 @@ def _L():
         lib.ref_lsqr.argtypes = [C.POINTER(_RefOp), P, C.c_double, C.c_int32, P, P, P,
                                  C.c_double, C.c_int32, P, P, P, P, C.c_int32]
         lib.ref_lsqr.restype = C.c_int32
+        I64 = C.c_int64
+        lib.ref_apply_S.argtypes = [C.POINTER(_RefOp), P, C.c_double, C.c_int32, P, I64, P, P, P, P]
+        lib.ref_apply_SH.argtypes = [C.POINTER(_RefOp), P, C.c_double, C.c_int32, P, I64, P, P, P, P]
+        lib.ref_lsqr_sf_step.argtypes = [C.POINTER(_RefOp), P, C.c_double, C.c_int32, P, I64,
+                                         C.POINTER(_RefStateSF)]
+        lib.ref_lsqr_sf.argtypes = [C.POINTER(_RefOp), P, C.c_double, C.c_int32, P, I64, P,
+                                    C.c_double, C.c_int32, P, P, P, P]
+        lib.ref_lsqr_sf.restype = C.c_int32
+        lib.ref_objective_gradient.argtypes = [C.POINTER(_RefOp), P, C.c_double, C.c_int32, P, I64,
+                                               P, P, P, P, P, P, P]
         for f in (lib.ref_gamma, lib.ref_apply_A, lib.ref_apply_AH, lib.ref_apply_M,
-                  lib.ref_apply_MH, lib.ref_lsqr_step):
+                  lib.ref_apply_MH, lib.ref_lsqr_step, lib.ref_apply_S, lib.ref_apply_SH,
+                  lib.ref_lsqr_sf_step, lib.ref_objective_gradient):
             f.restype = None
         _lib = lib
     return _lib
@@ -229,3 +251,122 @@ def lsqr_batch(ops, m, lam: float, rec: np.ndarray, Q, D, tols=None, maxit: int 
             "resnorms": np.stack([o["resnorms"] for o in outs], axis=1),
             "arnorms": np.stack([o["arnorms"] for o in outs], axis=1),
             "iters": np.array([o["iters"] for o in outs], dtype=np.int32)}
+
+
+# ---------------------------------------------------------------------------------------------
+# Source-free system S = [lam A, -lam e; P, 0], x = [u; alpha], b = [0; d]
+
+def _drec(d, rec):
+    return _c128(d, rec.size) if rec.size else np.zeros(1, dtype=np.complex128)
+
+
+def apply_S(op: Operator, m, lam: float, rec: np.ndarray, src: int, u, a):
+    m = _f64(m, op.ng)
+    u = _c128(u, op.ng)
+    rec = np.ascontiguousarray(rec, dtype=np.int64)
+    a = np.array([a], dtype=np.complex128)
+    ytop = np.empty(op.ng, dtype=np.complex128)
+    ybot = np.empty(max(rec.size, 1), dtype=np.complex128)
+    _L().ref_apply_S(C.byref(op._c()), _ptr(m), float(lam), rec.size, _ptr(rec), int(src), _ptr(u),
+                     _ptr(a), _ptr(ytop), _ptr(ybot))
+    return ytop, ybot[:rec.size]
+
+
+def apply_SH(op: Operator, m, lam: float, rec: np.ndarray, src: int, ytop, ybot):
+    m = _f64(m, op.ng)
+    rec = np.ascontiguousarray(rec, dtype=np.int64)
+    ytop = _c128(ytop, op.ng)
+    ybot = _drec(ybot, rec)
+    xu = np.empty(op.ng, dtype=np.complex128)
+    xa = np.empty(1, dtype=np.complex128)
+    _L().ref_apply_SH(C.byref(op._c()), _ptr(m), float(lam), rec.size, _ptr(rec), int(src),
+                      _ptr(ytop), _ptr(ybot), _ptr(xu), _ptr(xa))
+    return xu, complex(xa[0])
+
+
+def lsqr_sf(op: Operator, m, lam: float, rec: np.ndarray, src: int, d, tol: float = 0.0,
+            maxit: int = 50) -> dict:
+    """One column of LSQR on min ||S [u; alpha] - [0; d]||, x0 = 0."""
+    m = _f64(m, op.ng)
+    rec = np.ascontiguousarray(rec, dtype=np.int64)
+    d = _drec(d, rec)
+    x = np.empty(op.ng, dtype=np.complex128)
+    xa = np.zeros(1, dtype=np.complex128)
+    res = np.empty(maxit + 1, dtype=np.float64)
+    ar = np.empty(maxit + 1, dtype=np.float64)
+    it = _L().ref_lsqr_sf(C.byref(op._c()), _ptr(m), float(lam), rec.size, _ptr(rec), int(src),
+                          _ptr(d), float(tol), int(maxit), _ptr(x), _ptr(xa), _ptr(res), _ptr(ar))
+    return {"x": x, "alpha_src": complex(xa[0]), "resnorms": res, "arnorms": ar, "iters": int(it)}
+
+
+def lsqr_sf_step(op: Operator, m, lam: float, rec: np.ndarray, src: int, state: dict) -> dict:
+    """One LSQR iteration on a normalised source-free state: the keys of lsqr_step plus the
+    alpha entries v_a, w_a, x_a of v, w, x."""
+    m = _f64(m, op.ng)
+    rec = np.ascontiguousarray(rec, dtype=np.int64)
+    arrs = {k: _c128(state[k], op.ng).copy() for k in ("u_top", "v", "w", "x")}
+    arrs["u_bot"] = _drec(state["u_bot"], rec).copy()
+    st = _RefStateSF()
+    for k, a in arrs.items():
+        setattr(st, k, a.ctypes.data)
+    for k in ("v_a", "w_a", "x_a"):
+        z = complex(state[k])
+        getattr(st, k)[0] = z.real
+        getattr(st, k)[1] = z.imag
+    for k in ("alpha", "beta", "rhobar", "phibar"):
+        setattr(st, k, float(state[k]))
+    _L().ref_lsqr_sf_step(C.byref(op._c()), _ptr(m), float(lam), rec.size, _ptr(rec), int(src),
+                          C.byref(st))
+    out = dict(arrs)
+    out["u_bot"] = arrs["u_bot"][:rec.size]
+    for k in ("v_a", "w_a", "x_a"):
+        out[k] = complex(getattr(st, k)[0], getattr(st, k)[1])
+    for k in ("alpha", "beta", "rhobar", "phibar", "rho", "c", "s", "theta", "phi", "arnorm"):
+        out[k] = getattr(st, k)
+    out["stop"] = int(st.stop)
+    return out
+
+
+def lsqr_sf_batch(ops, m, lam: float, rec: np.ndarray, src_cells, D, tols=None, maxit: int = 50,
+                  threads: int = 1, columns=None) -> dict:
+    """Column loop of lsqr_sf over D[n_r, nb]; src_cells[nb] = source node of each column."""
+    D = np.asarray(D)
+    nb = len(src_cells)
+    cols = list(range(nb)) if columns is None else list(columns)
+    tols = np.zeros(nb) if tols is None else np.asarray(tols, dtype=np.float64)
+
+    def one(s):
+        return lsqr_sf(ops[s], m, lam, rec, int(src_cells[s]), D[:, s] if D.size else D.reshape(0),
+                       tol=float(tols[s]), maxit=maxit)
+
+    if threads > 1 and len(cols) > 1:
+        _L()
+        with ThreadPoolExecutor(max_workers=threads) as ex:
+            outs = list(ex.map(one, cols))
+    else:
+        outs = [one(s) for s in cols]
+    return {"x": np.stack([o["x"] for o in outs], axis=1),
+            "alpha_src": np.array([o["alpha_src"] for o in outs], dtype=np.complex128),
+            "resnorms": np.stack([o["resnorms"] for o in outs], axis=1),
+            "arnorms": np.stack([o["arnorms"] for o in outs], axis=1),
+            "iters": np.array([o["iters"] for o in outs], dtype=np.int32)}
+
+
+def objective_gradient(op: Operator, m, lam: float, rec: np.ndarray, u, d, q=None, src: int = -1,
+                       alpha_src: complex = 0.0, g=None):
+    """f_pde = lam^2/2 ||A u - q - alpha e||^2, f_data = 1/2 ||P u - d||^2 and, when g (float64
+    [n_g]) is given, g += lam^2 omega^2 Re[conj((1+i gamma) u) r]  (eq. 4, 9)."""
+    m = _f64(m, op.ng)
+    rec = np.ascontiguousarray(rec, dtype=np.int64)
+    u = _c128(u, op.ng)
+    d = _drec(d, rec)
+    qq = _c128(q, op.ng) if q is not None else None
+    a = np.array([alpha_src], dtype=np.complex128)
+    fp = C.c_double(0.0)
+    fd = C.c_double(0.0)
+    if g is not None:
+        assert g.dtype == np.float64 and g.flags.c_contiguous and g.size == op.ng
+    _L().ref_objective_gradient(C.byref(op._c()), _ptr(m), float(lam), rec.size, _ptr(rec), int(src),
+                                _ptr(a), _ptr(qq) if qq is not None else None, _ptr(u), _ptr(d),
+                                C.byref(fp), C.byref(fd), _ptr(g) if g is not None else None)
+    return fp.value, fd.value

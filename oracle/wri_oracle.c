@@ -36,7 +36,8 @@
  * One column (one source/frequency) per call; complex numbers are C99
  * double complex (re, im pairs in memory).
  *
- * Pins (tests/test_oracle_*.py): adjoint dot test, closed-form eigenpairs
+ * Pins (tests/test_oracle_*.py; the source-free and gradient functions at the
+ * end of this file list theirs in their own headers): adjoint dot test, closed-form eigenpairs
  * (periodic plane wave, Dirichlet sine modes), printed sponge values, dense
  * LAPACK least squares on 8^3, SciPy LSQR, CGLS, estimate-vs-true residuals,
  * monotone ||r||, consistent system, breakdown cases.
@@ -330,4 +331,247 @@ int32_t ref_lsqr(const ref_op *op, const double *m, double lambda, int32_t n_rec
     free(gamma); free(tmp_top); free(tmp_bot);
     free(st.u_top); free(st.u_bot); free(st.v); free(st.w);
     return iters;
+}
+
+/* ===========================================================================
+ * Source-free system: the system the paper actually
+ * states, PAPER.md:76-85 (eq. 4-6), with the source weight alpha UNKNOWN:
+ *
+ *     S = [ lambda A   -lambda e ]      x = [ u     ]      b = [ 0 ]
+ *         [ P           0        ]          [ alpha ]          [ d ]
+ *
+ * e = real unit vector at the source node `src` ("e_i is a unit
+ * vector representing the location of the i-th source").
+ *   ref_apply_S    S [u; a]   = [ lambda (A u - a e) ; P u ]
+ *   ref_apply_SH   S^H [yt;yb] = [ lambda A^H yt + P^T yb ; -lambda yt[src] ]
+ *                  (e is real, so e^H yt = yt[src]; conjugate transpose per
+ *                  reading C-2)
+ *   ref_lsqr_sf    the same Paige & Saunders recurrences as ref_lsqr on S, b;
+ *                  norms run over the stacked vectors including the alpha entry
+ *   ref_lsqr_sf_step  one loop body on a caller-supplied state
+ * Pins (tests/test_oracle_sf.py): adjoint dot test, dense LAPACK least squares
+ * on 8^3 incl. the alpha entry, recovery of alpha_true on consistent data,
+ * SciPy LSQR on the assembled sparse S, agreement with ref_lsqr when the alpha
+ * column is removed.
+ * ======================================================================== */
+
+static void apply_S_g(const ref_op *op, const double *m, const double *gamma, double lambda,
+                      int32_t n_rec, const int64_t *rec, int64_t src, const zc *u, zc a,
+                      zc *ytop, zc *ybot) {
+    size_t ng = (size_t)op->nx * op->ny * op->nz;
+    apply_A_impl(op, m, gamma, u, ytop, 0);
+    ytop[src] -= a;                                  /* A u - alpha e            */
+    for (size_t c = 0; c < ng; ++c) ytop[c] *= lambda;
+    for (int32_t r = 0; r < n_rec; ++r) ybot[r] = u[rec[r]];
+}
+
+static void apply_SH_g(const ref_op *op, const double *m, const double *gamma, double lambda,
+                       int32_t n_rec, const int64_t *rec, int64_t src, const zc *ytop,
+                       const zc *ybot, zc *xu, zc *xa) {
+    size_t ng = (size_t)op->nx * op->ny * op->nz;
+    apply_A_impl(op, m, gamma, ytop, xu, 1);
+    for (size_t c = 0; c < ng; ++c) xu[c] *= lambda;
+    for (int32_t r = 0; r < n_rec; ++r) xu[rec[r]] += ybot[r];
+    *xa = -lambda * ytop[src];                       /* (-lambda e)^H y_top      */
+}
+
+void ref_apply_S(const ref_op *op, const double *m, double lambda, int32_t n_rec,
+                 const int64_t *rec, int64_t src, const zc *u, const zc *a, zc *ytop, zc *ybot) {
+    size_t ng = (size_t)op->nx * op->ny * op->nz;
+    double *gamma = (double *)malloc(ng * sizeof(double));
+    ref_gamma(op, gamma);
+    apply_S_g(op, m, gamma, lambda, n_rec, rec, src, u, *a, ytop, ybot);
+    free(gamma);
+}
+
+void ref_apply_SH(const ref_op *op, const double *m, double lambda, int32_t n_rec,
+                  const int64_t *rec, int64_t src, const zc *ytop, const zc *ybot, zc *xu, zc *xa) {
+    size_t ng = (size_t)op->nx * op->ny * op->nz;
+    double *gamma = (double *)malloc(ng * sizeof(double));
+    ref_gamma(op, gamma);
+    apply_SH_g(op, m, gamma, lambda, n_rec, rec, src, ytop, ybot, xu, xa);
+    free(gamma);
+}
+
+/* LSQR state of one source-free column: the x-space vectors v, w, x carry one
+ * more complex entry (the alpha component), all NORMALISED as in ref_state. */
+typedef struct {
+    zc *u_top;      /* [n_g]   */
+    zc *u_bot;      /* [n_rec] */
+    zc *v;          /* [n_g]   */
+    zc *w;          /* [n_g]   */
+    zc *x;          /* [n_g]   */
+    zc v_a, w_a, x_a;               /* alpha entries of v, w, x */
+    double alpha, beta, rhobar, phibar;     /* LSQR scalars (alpha here is Golub-Kahan's, */
+                                            /* not the source weight)                     */
+    double rho, c, s, theta, phi, arnorm;
+    int32_t stop;
+} ref_state_sf;
+
+static double abs2(zc z) { return creal(z) * creal(z) + cimag(z) * cimag(z); }
+
+/* One LSQR iteration on S (same loop body and order as lsqr_step_g). */
+static void lsqr_sf_step_g(const ref_op *op, const double *m, const double *gamma, double lambda,
+                           int32_t n_rec, const int64_t *rec, int64_t src, ref_state_sf *st,
+                           zc *tmp_top, zc *tmp_bot) {
+    size_t ng = (size_t)op->nx * op->ny * op->nz;
+    double alpha = st->alpha, beta;
+    zc tmp_a;
+
+    apply_S_g(op, m, gamma, lambda, n_rec, rec, src, st->v, st->v_a, tmp_top, tmp_bot);
+    for (size_t i = 0; i < ng; ++i) st->u_top[i] = tmp_top[i] - alpha * st->u_top[i];
+    for (int32_t r = 0; r < n_rec; ++r) st->u_bot[r] = tmp_bot[r] - alpha * st->u_bot[r];
+    beta = norm2(st->u_top, ng, st->u_bot, (size_t)n_rec);
+
+    if (beta > 0.0) {
+        for (size_t i = 0; i < ng; ++i) st->u_top[i] /= beta;
+        for (int32_t r = 0; r < n_rec; ++r) st->u_bot[r] /= beta;
+        apply_SH_g(op, m, gamma, lambda, n_rec, rec, src, st->u_top, st->u_bot, tmp_top, &tmp_a);
+        for (size_t i = 0; i < ng; ++i) st->v[i] = tmp_top[i] - beta * st->v[i];
+        st->v_a = tmp_a - beta * st->v_a;
+        double nv = norm2(st->v, ng, NULL, 0);
+        alpha = sqrt(nv * nv + abs2(st->v_a));
+        if (alpha > 0.0) {
+            for (size_t i = 0; i < ng; ++i) st->v[i] /= alpha;
+            st->v_a /= alpha;
+        }
+    } else {
+        alpha = 0.0;
+    }
+
+    double rho = hypot(st->rhobar, beta);
+    double c = st->rhobar / rho;
+    double s = beta / rho;
+    double theta = s * alpha;
+    double phi = c * st->phibar;
+    st->rhobar = -c * alpha;
+    st->phibar = s * st->phibar;
+
+    double t1 = phi / rho, t2 = theta / rho;
+    for (size_t i = 0; i < ng; ++i) {
+        st->x[i] += t1 * st->w[i];
+        st->w[i] = st->v[i] - t2 * st->w[i];
+    }
+    st->x_a += t1 * st->w_a;
+    st->w_a = st->v_a - t2 * st->w_a;
+    st->alpha = alpha;
+    st->beta = beta;
+    st->rho = rho; st->c = c; st->s = s; st->theta = theta; st->phi = phi;
+    st->arnorm = st->phibar * alpha * fabs(c);
+    st->stop = (beta == 0.0) ? 1 : (alpha == 0.0 ? 2 : 0);
+}
+
+void ref_lsqr_sf_step(const ref_op *op, const double *m, double lambda, int32_t n_rec,
+                      const int64_t *rec, int64_t src, ref_state_sf *st) {
+    size_t ng = (size_t)op->nx * op->ny * op->nz;
+    double *gamma = (double *)malloc(ng * sizeof(double));
+    zc *tmp_top = (zc *)malloc(ng * sizeof(zc));
+    zc *tmp_bot = (zc *)malloc(((size_t)n_rec + 1) * sizeof(zc));
+    ref_gamma(op, gamma);
+    lsqr_sf_step_g(op, m, gamma, lambda, n_rec, rec, src, st, tmp_top, tmp_bot);
+    free(gamma); free(tmp_top); free(tmp_bot);
+}
+
+/* LSQR on  min_x || S x - b ||,  b = [0 ; d],  x0 = 0.
+ * Same stop rule, histories and hold-last convention as ref_lsqr.  x_u [n_g] and
+ * x_a [1] receive the wavefield and the source-weight estimate.  Returns the
+ * number of iterations performed. */
+int32_t ref_lsqr_sf(const ref_op *op, const double *m, double lambda, int32_t n_rec,
+                    const int64_t *rec, int64_t src, const zc *d, double tol, int32_t maxit,
+                    zc *x_u, zc *x_a, double *resnorms, double *arnorms) {
+    size_t ng = (size_t)op->nx * op->ny * op->nz;
+    double *gamma = (double *)malloc(ng * sizeof(double));
+    zc *tmp_top = (zc *)malloc(ng * sizeof(zc));
+    zc *tmp_bot = (zc *)malloc(((size_t)n_rec + 1) * sizeof(zc));
+    ref_state_sf st;
+    memset(&st, 0, sizeof st);
+    st.u_top = (zc *)malloc(ng * sizeof(zc));
+    st.u_bot = (zc *)malloc(((size_t)n_rec + 1) * sizeof(zc));
+    st.v = (zc *)malloc(ng * sizeof(zc));
+    st.w = (zc *)malloc(ng * sizeof(zc));
+    st.x = x_u;
+    ref_gamma(op, gamma);
+    int32_t iters = 0;
+
+    for (size_t i = 0; i < ng; ++i) { st.u_top[i] = 0.0; x_u[i] = 0.0; }     /* b_top = 0 */
+    for (int32_t r = 0; r < n_rec; ++r) st.u_bot[r] = d[r];
+    double beta = norm2(st.u_top, ng, st.u_bot, (size_t)n_rec);
+    double ar0 = 0.0, last_r = beta, last_ar = 0.0;
+    resnorms[0] = beta;
+    if (arnorms) arnorms[0] = 0.0;
+
+    if (beta > 0.0) {
+        for (int32_t r = 0; r < n_rec; ++r) st.u_bot[r] /= beta;
+        apply_SH_g(op, m, gamma, lambda, n_rec, rec, src, st.u_top, st.u_bot, st.v, &st.v_a);
+        double nv = norm2(st.v, ng, NULL, 0);
+        double alpha = sqrt(nv * nv + abs2(st.v_a));
+        ar0 = alpha * beta;
+        last_ar = ar0;
+        if (arnorms) arnorms[0] = ar0;
+        if (alpha > 0.0) {
+            for (size_t i = 0; i < ng; ++i) { st.v[i] /= alpha; st.w[i] = st.v[i]; }
+            st.v_a /= alpha; st.w_a = st.v_a;
+            st.alpha = alpha; st.beta = beta; st.phibar = beta; st.rhobar = alpha;
+            for (int32_t k = 1; k <= maxit; ++k) {
+                lsqr_sf_step_g(op, m, gamma, lambda, n_rec, rec, src, &st, tmp_top, tmp_bot);
+                iters = k;
+                last_r = st.phibar; last_ar = st.arnorm;
+                resnorms[k] = last_r;
+                if (arnorms) arnorms[k] = last_ar;
+                if (st.stop) break;
+                if (tol > 0.0 && st.arnorm <= tol * ar0) break;
+            }
+        }
+    }
+    *x_a = st.x_a;
+    for (int32_t k = iters + 1; k <= maxit; ++k) {
+        resnorms[k] = last_r;
+        if (arnorms) arnorms[k] = last_ar;
+    }
+    free(gamma); free(tmp_top); free(tmp_bot);
+    free(st.u_top); free(st.u_bot); free(st.v); free(st.w);
+    return iters;
+}
+
+/* ===========================================================================
+ * Objective and gradient of the reduced problem,
+ * PAPER.md:71-76 (eq. 4), 98-110 (eq. 8-9), for ONE column at a given (u, alpha):
+ *
+ *   r      = A(m) u - q - alpha e                    (q dense and/or alpha e; either may be absent)
+ *   f_pde  = 1/2 lambda^2 || r ||^2                  (eq. 5: the 1/2 covers both terms of eq. 4)
+ *   f_data = 1/2 || P u - d ||^2
+ *   g[c]  += lambda^2 omega^2 Re[ conj((1 + i gamma_c) u_c) r_c ]
+ *
+ * Eq. 9 prints  lambda^2 omega^2 diag(conj(u)) (A u - alpha e)  for the paper's
+ * real-coefficient A = omega^2 diag(m) + Laplacian; m is real, so the real part
+ * is meant, and with the sponge of this build dA/dm_c = omega^2 (1 + i gamma_c),
+ * which gives the factor above (it reduces to eq. 9 where gamma = 0).  By
+ * variable projection this partial derivative at the minimiser
+ * (u-bar, alpha-bar) IS the gradient of f4(m); "does not involve additional PDE
+ * solvers".  g is ACCUMULATED (the paper sums over sources and frequencies).
+ * Pins (tests/test_oracle_sf.py): central finite differences of f in m at fixed
+ * (u, alpha); finite differences of f4(m) through a converged solve on 6^3.
+ * ======================================================================== */
+void ref_objective_gradient(const ref_op *op, const double *m, double lambda, int32_t n_rec,
+                            const int64_t *rec, int64_t src /* < 0: none */, const zc *alpha_src,
+                            const zc *q /* may be NULL */, const zc *u, const zc *d,
+                            double *f_pde, double *f_data, double *g /* [n_g], += ; may be NULL */) {
+    size_t ng = (size_t)op->nx * op->ny * op->nz;
+    double *gamma = (double *)malloc(ng * sizeof(double));
+    zc *r = (zc *)malloc(ng * sizeof(zc));
+    ref_gamma(op, gamma);
+    apply_A_impl(op, m, gamma, u, r, 0);
+    if (q) for (size_t c = 0; c < ng; ++c) r[c] -= q[c];
+    if (src >= 0) r[src] -= *alpha_src;
+    double sp = 0.0, sd = 0.0;
+    for (size_t c = 0; c < ng; ++c) sp += abs2(r[c]);
+    for (int32_t k = 0; k < n_rec; ++k) sd += abs2(u[rec[k]] - d[k]);
+    *f_pde = 0.5 * lambda * lambda * sp;
+    *f_data = 0.5 * sd;
+    if (g) {
+        const double w2 = op->omega * op->omega;
+        for (size_t c = 0; c < ng; ++c)
+            g[c] += lambda * lambda * w2 * creal(conj((1.0 + I * gamma[c]) * u[c]) * r[c]);
+    }
+    free(gamma); free(r);
 }
