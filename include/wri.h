@@ -118,6 +118,39 @@ int wri_lsqr_batch(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_host,
                    const float* tol_dev, int32_t maxit,
                    void* u_out_dev, float* resnorms_dev, int32_t* iters_dev);
 
+/* ---- Source-free system (the system the paper states, eq. 4-6) ---------------
+ *
+ *     S = [ lambda A   -lambda e ]      x = [ u     ]      b = [ lambda q ]   (paper: q = 0)
+ *         [ P           0        ]          [ alpha ]          [ d        ]
+ *
+ * The source weight alpha of every column is one more complex unknown; e is the real unit
+ * vector at that column's source node.  S^H y = [lambda A^H y_top + P^T y_bot ;
+ * -lambda y_top[src]].  All norms run over the stacked vectors including the alpha entry.
+ *   src_ijk_host  [nb][3] = (ix,iy,iz) source node per batch column (columns of one source at
+ *                 several frequencies repeat it); outside the grid -> WRI_ERR_ARG
+ *   xalpha / alpha_out   c64 [nb], device
+ *   q_dev         may be NULL (the paper's b = [0; d]); given, it is a known part of the source
+ * wri_apply_S / wri_apply_SH are the operator entries; wri_lsqr_sf_* mirror wri_lsqr_* (same
+ * stop rule, histories, compaction, stepping through wri_lsqr_iterate / _end / _peek), and
+ * alpha_out_dev receives the source-weight estimate of x_k (the paper's on-the-fly source
+ * estimation).                                                                    */
+int wri_apply_S (wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_host, const int32_t* src_ijk_host,
+                 float lambda, const void* x_dev, const void* xalpha_dev, void* ytop_dev, void* ybot_dev);
+int wri_apply_SH(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_host, const int32_t* src_ijk_host,
+                 float lambda, const void* ytop_dev, const void* ybot_dev, void* x_dev, void* xalpha_dev);
+int wri_lsqr_sf_batch(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_host, const int32_t* src_ijk_host,
+                      const void* q_dev, const void* d_dev, float lambda, const float* tol_dev,
+                      int32_t maxit, void* u_out_dev, void* alpha_out_dev, float* resnorms_dev,
+                      int32_t* iters_dev);
+int wri_lsqr_sf_begin(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_host, const int32_t* src_ijk_host,
+                      const void* q_dev, const void* d_dev, float lambda, const float* tol_dev,
+                      int32_t maxit, void* u_out_dev, void* alpha_out_dev, float* resnorms_dev,
+                      int32_t* iters_dev);
+int wri_lsqr_sf_batch_host(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_host,
+                           const int32_t* src_ijk_host, const void* q_host, const void* d_host,
+                           float lambda, const float* tol_host, int32_t maxit, void* u_out_host,
+                           void* alpha_out_host, float* resnorms_host, int32_t* iters_host);
+
 /* Same solve with HOST buffers: copies q, d (and tol) to the device, solves, copies u_out,
  * resnorms and iters back, then synchronises the stream.  Needs a workspace sized with
  * host_staging = 1.  Pinned host memory makes the copies asynchronous but is not required.   */
@@ -161,6 +194,11 @@ typedef struct {
                                      /*      w_{k+1} = V/alpha - cw * W                        */
     const int32_t* active;           /* [nb] 1 while the column iterates                       */
     const int32_t* iters;            /* [nb]                                                   */
+    int32_t nb_max;                  /* row stride of sf_state                                 */
+    const double* sf_state;          /* source-free solves (else NULL): [6][nb_max] rows        */
+                                     /* Re v_a, Im v_a, Re w_a, Im w_a, Re x_a, Im x_a — the     */
+                                     /* alpha entries of V (un-normalised like V), of w_{k+1}   */
+                                     /* and of x_k (these two are NOT deferred)                 */
 } wri_lsqr_view;
 int wri_lsqr_peek(const wri_ctx* ctx, wri_lsqr_view* view);
 

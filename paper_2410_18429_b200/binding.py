@@ -30,7 +30,8 @@ class wri_lsqr_view(C.Structure):
                 ("W", C.c_void_p), ("X", C.c_void_p),
                 ("alpha", C.c_void_p), ("beta", C.c_void_p), ("rhobar", C.c_void_p),
                 ("phibar", C.c_void_p), ("ar0", C.c_void_p), ("cx", C.c_void_p), ("cw", C.c_void_p),
-                ("active", C.c_void_p), ("iters", C.c_void_p)]
+                ("active", C.c_void_p), ("iters", C.c_void_p),
+                ("nb_max", C.c_int32), ("sf_state", C.c_void_p)]
 
 
 WRI_OK = 0
@@ -73,6 +74,12 @@ def load_library():
     lib.wri_lsqr_batch.argtypes = solve
     lib.wri_lsqr_batch_host.argtypes = solve
     lib.wri_lsqr_begin.argtypes = solve
+    lib.wri_apply_S.argtypes = [P, I32, P, P, F32, P, P, P, P]
+    lib.wri_apply_SH.argtypes = [P, I32, P, P, F32, P, P, P, P]
+    solve_sf = [P, I32, P, P, P, P, F32, P, I32, P, P, P, P]
+    lib.wri_lsqr_sf_batch.argtypes = solve_sf
+    lib.wri_lsqr_sf_begin.argtypes = solve_sf
+    lib.wri_lsqr_sf_batch_host.argtypes = solve_sf
     lib.wri_lsqr_iterate.argtypes = [P, I32]
     lib.wri_lsqr_end.argtypes = [P]
     lib.wri_lsqr_peek.argtypes = [P, C.POINTER(wri_lsqr_view)]
@@ -191,6 +198,30 @@ class Wri:
         _ck(self._lib.wri_apply_MH(self._h, nb, oi, float(lam), _dptr(ytop), _dptr(ybot), _dptr(x)))
         return x
 
+    def apply_S(self, x, xalpha, lam, src_ijk, omega_idx=None):
+        """S [x; xalpha] of the source-free system: (ytop, ybot)."""
+        t = self._torch
+        nb = x.shape[1]
+        ytop = t.empty_like(x)
+        ybot = t.empty((self.n_rec, nb), dtype=t.complex64, device=x.device)
+        keep, oi = _i32(omega_idx)
+        keep2, si = _i32(src_ijk)
+        _ck(self._lib.wri_apply_S(self._h, nb, oi, si, float(lam), _dptr(x), _dptr(xalpha), _dptr(ytop),
+                                  _dptr(ybot)))
+        return ytop, ybot
+
+    def apply_SH(self, ytop, ybot, lam, src_ijk, omega_idx=None):
+        """S^H [ytop; ybot]: (x, xalpha)."""
+        t = self._torch
+        nb = ytop.shape[1]
+        x = t.empty_like(ytop)
+        xa = t.empty(nb, dtype=t.complex64, device=ytop.device)
+        keep, oi = _i32(omega_idx)
+        keep2, si = _i32(src_ijk)
+        _ck(self._lib.wri_apply_SH(self._h, nb, oi, si, float(lam), _dptr(ytop), _dptr(ybot), _dptr(x),
+                                   _dptr(xa)))
+        return x, xa
+
     # ---- solver
     def _outputs(self, nb, maxit, device):
         t = self._torch
@@ -233,6 +264,49 @@ class Wri:
                                      int(maxit), _dptr(u), _dptr(res), _dptr(it)))
         return u, res, it
 
+    # ---- source-free system (unknown source weight per column)
+    def lsqr_sf_batch(self, d, lam, src_ijk, tol=None, maxit=50, omega_idx=None, q=None):
+        t = self._torch
+        nb = d.shape[1]
+        self.ensure_workspace(nb, compaction=tol is not None)
+        u, res, it = self._outputs(nb, maxit, d.device)
+        a = t.empty(nb, dtype=t.complex64, device=d.device)
+        keep, oi = _i32(omega_idx)
+        keep2, si = _i32(src_ijk)
+        _ck(self._lib.wri_lsqr_sf_batch(self._h, nb, oi, si, _dptr(q), _dptr(d), float(lam), _dptr(tol),
+                                        int(maxit), _dptr(u), _dptr(a), _dptr(res), _dptr(it)))
+        return u, a, res, it
+
+    def lsqr_sf_batch_host(self, d, lam, src_ijk, tol=None, maxit=50, omega_idx=None, q=None, out=None):
+        t = self._torch
+        nb = d.shape[1]
+        self.ensure_workspace(nb, host_staging=True, compaction=tol is not None)
+        if out is None:
+            out = (t.empty((self.ng, nb), dtype=t.complex64).pin_memory(),
+                   t.empty(nb, dtype=t.complex64).pin_memory(),
+                   t.empty((maxit + 1, nb), dtype=t.float32).pin_memory(),
+                   t.empty(nb, dtype=t.int32).pin_memory())
+        u, a, res, it = out
+        keep, oi = _i32(omega_idx)
+        keep2, si = _i32(src_ijk)
+        _ck(self._lib.wri_lsqr_sf_batch_host(self._h, nb, oi, si, _dptr(q), _dptr(d), float(lam),
+                                             _dptr(tol), int(maxit), _dptr(u), _dptr(a), _dptr(res),
+                                             _dptr(it)))
+        return u, a, res, it
+
+    def lsqr_sf_begin(self, d, lam, src_ijk, tol=None, maxit=50, omega_idx=None, q=None):
+        t = self._torch
+        nb = d.shape[1]
+        self.ensure_workspace(nb, compaction=tol is not None)
+        u, res, it = self._outputs(nb, maxit, d.device)
+        a = t.empty(nb, dtype=t.complex64, device=d.device)
+        keep, oi = _i32(omega_idx)
+        keep2, si = _i32(src_ijk)
+        self._keep = [q, d, tol, u, a, res, it]
+        _ck(self._lib.wri_lsqr_sf_begin(self._h, nb, oi, si, _dptr(q), _dptr(d), float(lam), _dptr(tol),
+                                        int(maxit), _dptr(u), _dptr(a), _dptr(res), _dptr(it)))
+        return u, a, res, it
+
     def lsqr_iterate(self, n_steps=1):
         _ck(self._lib.wri_lsqr_iterate(self._h, int(n_steps)))
 
@@ -263,6 +337,11 @@ class Wri:
         out["cw"] = grab(v.cw, (nb,), np.float32)
         out["active"] = grab(v.active, (nb,), np.int32)
         out["iters"] = grab(v.iters, (nb,), np.int32)
+        if v.sf_state:
+            sf = grab(v.sf_state, (6, v.nb_max), np.float64)[:, :nb]
+            out["v_a"] = sf[0] + 1j * sf[1]
+            out["w_a"] = sf[2] + 1j * sf[3]
+            out["x_a"] = sf[4] + 1j * sf[5]
         return out
 
     def profile_enable(self, on=True):

@@ -67,6 +67,9 @@ struct wri_ctx {
     double* stat_alt = nullptr;
     int* active_alt = nullptr;
     int* iters_alt = nullptr;
+    int* src = nullptr;          // [nb_max] source cell per caller's column (source-free system)
+    bool sf = false;             // the solve in flight has the extra source-weight unknown
+    float2* alpha_out = nullptr; // caller's [nb] source-weight estimates (source-free system)
     int* colmap = nullptr;       // [nb_max] working column -> caller's column (-1 = padding)
     int* idx = nullptr;          // [3][nb_max] scratch: gather map | retire source | retire destination
     int* h_active = nullptr;     // pinned host copy of the active flags
@@ -137,7 +140,7 @@ Tiling make_tiling(const wri_ctx* c, int nb) {
 }
 
 struct WsLayout {
-    size_t U, V, W, U_bot, partials, partials_tma, Xs, Ds, tols, res, its, B3, B4, U_bot2, total;
+    size_t U, V, W, U_bot, partials, partials_tma, Xs, Ds, tols, res, its, alphas, B3, B4, U_bot2, total;
 };
 enum { WS_HOST_STAGING = 1, WS_COMPACTION = 2 };
 WsLayout ws_layout(const wri_ctx* c, int nb, int flags, int maxit_cap) {
@@ -158,6 +161,7 @@ WsLayout ws_layout(const wri_ctx* c, int nb, int flags, int maxit_cap) {
         L.tols = o; o += align_up((size_t)nb * sizeof(float), 256);
         L.res = o; o += align_up((size_t)(maxit_cap + 1) * nb * sizeof(float), 256);
         L.its = o; o += align_up((size_t)nb * sizeof(int), 256);
+        L.alphas = o; o += align_up((size_t)nb * sizeof(float2), 256);
     }
     if (flags & WS_COMPACTION) {
         L.B3 = o; o += vec;
@@ -180,6 +184,19 @@ int upload_columns(wri_ctx* c, int nb, const int32_t* omega_idx, float lambda) {
     CK(cudaMemcpyAsync(c->coef + C_W2 * NM, w2.data(), nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));
     CK(cudaMemcpyAsync(c->coef + C_ONE * NM, one.data(), nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));
     CK(cudaMemcpyAsync(c->coef + C_LAM * NM, lam.data(), nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    return WRI_OK;
+}
+
+// source nodes of the source-free system, one per batch column -> c->src (cell indices)
+int upload_sources(wri_ctx* c, int nb, const int32_t* src_ijk) {
+    std::vector<int> cells(nb);
+    for (int s = 0; s < nb; ++s) {
+        const int ix = src_ijk[3 * s], iy = src_ijk[3 * s + 1], iz = src_ijk[3 * s + 2];
+        if (ix < 0 || ix >= c->g.nx || iy < 0 || iy >= c->g.ny || iz < 0 || iz >= c->g.nz) return WRI_ERR_ARG;
+        cells[s] = (iz * c->g.ny + iy) * c->g.nx + ix;
+    }
+    CK(cudaMemcpyAsync(c->src, cells.data(), nb * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaStreamSynchronize(c->stream));        // cells is a local
     return WRI_OK;
 }
 
@@ -223,20 +240,12 @@ int launch_pass(wri_ctx* c, const PassParams& p, const Tiling& t, bool timed = f
     return WRI_OK;
 }
 
+ScalParams scal_params(const wri_ctx* c, const double* partials, int n_rows, const float2* d);
+
 template <int PHASE>
 int launch_scalars(wri_ctx* c, const float2* d) {
-    ScalParams s{};
-    s.partials = c->partials;
-    s.n_tiles = (int)c->tl.n_tiles;
-    s.nb = c->nb; s.nb_max = c->nb_max;
-    s.n_rec = c->n_rec; s.rec = c->rec;
-    s.V = c->V; s.U_bot = c->U_bot; s.d = d;
-    s.coef = c->coef; s.stat = c->stat; s.active = c->active; s.iters = c->iters;
-    s.tol = c->tol; s.resnorms = c->resnorms; s.iters_out = c->iters_out;
-    s.k = c->k; s.maxit = c->maxit; s.lambda = c->lambda;
+    ScalParams s = scal_params(c, c->partials, (int)c->tl.n_tiles, d);
     s.rows_in_pass = c->tma_cb ? 1 : 0;
-    s.colmap = c->packed ? c->colmap : nullptr;
-    s.nb_out = c->nb0;
     const int T = 1024;
     const size_t smem = (size_t)(T + c->nb) * sizeof(double);
     k_scalars<PHASE><<<1, T, smem, c->stream>>>(s);
@@ -492,6 +501,9 @@ ScalParams scal_params(const wri_ctx* c, const double* partials, int n_rows, con
     s.rows_in_pass = 1;
     s.colmap = c->packed ? c->colmap : nullptr;
     s.nb_out = c->nb0;
+    s.src = c->sf ? c->src : nullptr;
+    s.U = c->U;
+    s.alpha_out = c->sf ? c->alpha_out : nullptr;
     return s;
 }
 
@@ -667,6 +679,7 @@ int wri_create(wri_ctx** out, wri_grid grid, double h, int32_t n_omega, const do
     CKC(cudaMalloc(&c->active_alt, nb_max * sizeof(int)));
     CKC(cudaMalloc(&c->iters_alt, nb_max * sizeof(int)));
     CKC(cudaMalloc(&c->colmap, nb_max * sizeof(int)));
+    CKC(cudaMalloc(&c->src, nb_max * sizeof(int)));
     CKC(cudaMalloc(&c->idx, (size_t)3 * nb_max * sizeof(int)));
     CKC(cudaMallocHost(&c->h_active, nb_max * sizeof(int)));
     CKC(cudaMalloc(&c->counter, sizeof(unsigned int)));
@@ -687,7 +700,7 @@ int wri_destroy(wri_ctx* c) {
     cudaFree(c->active); cudaFree(c->iters); cudaFree(c->counter);
     cudaFree(c->own_ptr); cudaFree(c->own);
     cudaFree(c->coef_alt); cudaFree(c->stat_alt); cudaFree(c->active_alt); cudaFree(c->iters_alt);
-    cudaFree(c->colmap); cudaFree(c->idx);
+    cudaFree(c->colmap); cudaFree(c->idx); cudaFree(c->src);
     if (c->h_active) cudaFreeHost(c->h_active);
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
     delete c;
@@ -782,6 +795,32 @@ int wri_apply_MH(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, float la
     return WRI_OK;
 }
 
+int wri_apply_S(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const int32_t* src_ijk_host,
+                float lambda, const void* x_dev, const void* xalpha_dev, void* ytop_dev, void* ybot_dev) {
+    if (!src_ijk_host || !xalpha_dev) return WRI_ERR_ARG;
+    int rc = wri_apply_M(c, nb, omega_idx_host, lambda, x_dev, ytop_dev, ybot_dev);
+    if (rc) return rc;
+    if ((rc = upload_sources(c, nb, src_ijk_host))) return rc;
+    k_src_forward<<<(nb + 127) / 128, 128, 0, c->stream>>>((float2*)ytop_dev, c->src, nb, lambda,
+                                                          (const float2*)xalpha_dev);
+    c->launches++;
+    CK(cudaGetLastError());
+    return WRI_OK;
+}
+
+int wri_apply_SH(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const int32_t* src_ijk_host,
+                 float lambda, const void* ytop_dev, const void* ybot_dev, void* x_dev, void* xalpha_dev) {
+    if (!src_ijk_host || !xalpha_dev) return WRI_ERR_ARG;
+    int rc = wri_apply_MH(c, nb, omega_idx_host, lambda, ytop_dev, ybot_dev, x_dev);
+    if (rc) return rc;
+    if ((rc = upload_sources(c, nb, src_ijk_host))) return rc;
+    k_src_adjoint<<<(nb + 127) / 128, 128, 0, c->stream>>>((const float2*)ytop_dev, c->src, nb, lambda,
+                                                          (float2*)xalpha_dev);
+    c->launches++;
+    CK(cudaGetLastError());
+    return WRI_OK;
+}
+
 // ---- solver entries ----------------------------------------------------------------------------
 }  // extern "C"
 
@@ -789,17 +828,22 @@ namespace {
 
 int lsqr_begin_impl(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const void* q_dev,
                     const void* d_dev, float lambda, const float* tol_dev, int32_t maxit,
-                    void* u_out_dev, float* resnorms_dev, int32_t* iters_dev, bool host_staged) {
+                    void* u_out_dev, float* resnorms_dev, int32_t* iters_dev, bool host_staged,
+                    const int32_t* src_ijk_host = nullptr, void* alpha_out_dev = nullptr) {
     int rc = check_batch_args(c, nb);
     if (rc) return rc;
-    if (!q_dev || (c->n_rec && !d_dev) || !u_out_dev || !resnorms_dev || maxit < 0 ||
-        !aligned16(q_dev) || !aligned16(u_out_dev) || q_dev == u_out_dev)
+    const bool sf = src_ijk_host != nullptr;          // source-free system: q may be absent (b_top = 0)
+    if ((!q_dev && !sf) || (c->n_rec && !d_dev) || !u_out_dev || !resnorms_dev || maxit < 0 ||
+        (q_dev && !aligned16(q_dev)) || !aligned16(u_out_dev) || q_dev == u_out_dev || (sf && !alpha_out_dev))
         return WRI_ERR_ARG;
     if (!c->ws) return WRI_ERR_WORKSPACE;
     const int base_flags = host_staged ? WS_HOST_STAGING : 0;
     if (c->ws_bytes < ws_layout(c, nb, base_flags, kHostMaxitCap).total) return WRI_ERR_WORKSPACE;
     const WsLayout L = ws_layout(c, nb, base_flags | WS_COMPACTION, kHostMaxitCap);
     if ((rc = upload_columns(c, nb, omega_idx_host, lambda))) return rc;
+    if (sf && (rc = upload_sources(c, nb, src_ijk_host))) return rc;
+    c->sf = sf;
+    c->alpha_out = (float2*)alpha_out_dev;
 
     c->nb = nb; c->nb0 = nb; c->k = 0; c->maxit = maxit; c->lambda = lambda;
     c->packed = false; c->all_done = false;
@@ -837,7 +881,12 @@ int lsqr_begin_impl(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const
     PassParams p = base_params(c, nb, c->tl);
     p.partials = c->partials;
     p.in = (const float2*)q_dev; p.out = c->U; p.ca = c->coef + C_LAM * NM;
-    if ((rc = launch_pass<MODE_INIT>(c, p, c->tl))) return rc;
+    if (q_dev) {
+        if ((rc = launch_pass<MODE_INIT>(c, p, c->tl))) return rc;
+    } else {
+        CK(cudaMemsetAsync(c->U, 0, vbytes, c->stream));
+        CK(cudaMemsetAsync(c->partials, 0, c->tl.n_tiles * nb * sizeof(double), c->stream));
+    }
     CK(cudaMemsetAsync(c->X, 0, vbytes, c->stream));
     CK(cudaMemsetAsync(c->W, 0, vbytes, c->stream));
     CK(cudaMemsetAsync(c->V, 0, vbytes, c->stream));
@@ -959,6 +1008,15 @@ int wri_lsqr_begin(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const 
                            resnorms_dev, iters_dev, false);
 }
 
+int wri_lsqr_sf_begin(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const int32_t* src_ijk_host,
+                      const void* q_dev, const void* d_dev, float lambda, const float* tol_dev,
+                      int32_t maxit, void* u_out_dev, void* alpha_out_dev, float* resnorms_dev,
+                      int32_t* iters_dev) {
+    if (!src_ijk_host) return WRI_ERR_ARG;
+    return lsqr_begin_impl(c, nb, omega_idx_host, q_dev, d_dev, lambda, tol_dev, maxit, u_out_dev,
+                           resnorms_dev, iters_dev, false, src_ijk_host, alpha_out_dev);
+}
+
 int wri_lsqr_iterate(wri_ctx* c, int32_t n_steps) {
     if (!c || n_steps < 0) return WRI_ERR_ARG;
     if (!c->solving) return WRI_ERR_STATE;
@@ -1027,13 +1085,30 @@ int wri_lsqr_batch(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const 
     return wri_lsqr_end(c);
 }
 
-int wri_lsqr_batch_host(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const void* q_host,
-                        const void* d_host, float lambda, const float* tol_host, int32_t maxit,
-                        void* u_out_host, float* resnorms_host, int32_t* iters_host) {
+int wri_lsqr_sf_batch(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const int32_t* src_ijk_host,
+                      const void* q_dev, const void* d_dev, float lambda, const float* tol_dev,
+                      int32_t maxit, void* u_out_dev, void* alpha_out_dev, float* resnorms_dev,
+                      int32_t* iters_dev) {
+    int rc = wri_lsqr_sf_begin(c, nb, omega_idx_host, src_ijk_host, q_dev, d_dev, lambda, tol_dev, maxit,
+                               u_out_dev, alpha_out_dev, resnorms_dev, iters_dev);
+    if (rc) return rc;
+    if ((rc = wri_lsqr_iterate(c, maxit))) { c->solving = false; return rc; }
+    return wri_lsqr_end(c);
+}
+
+}  // extern "C"
+
+namespace {
+
+int lsqr_batch_host_impl(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const int32_t* src_ijk_host,
+                         const void* q_host, const void* d_host, float lambda, const float* tol_host,
+                         int32_t maxit, void* u_out_host, void* alpha_out_host, float* resnorms_host,
+                         int32_t* iters_host) {
     int rc = check_batch_args(c, nb);
     if (rc) return rc;
-    if (!q_host || (c->n_rec && !d_host) || !u_out_host || !resnorms_host || maxit < 0 ||
-        maxit > kHostMaxitCap)
+    const bool sf = src_ijk_host != nullptr;
+    if ((!q_host && !sf) || (c->n_rec && !d_host) || !u_out_host || !resnorms_host || maxit < 0 ||
+        maxit > kHostMaxitCap || (sf && !alpha_out_host))
         return WRI_ERR_ARG;
     if (!c->ws) return WRI_ERR_WORKSPACE;
     const WsLayout L = ws_layout(c, nb, WS_HOST_STAGING, kHostMaxitCap);
@@ -1046,19 +1121,43 @@ int wri_lsqr_batch_host(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, c
     float* res = (float*)(c->ws + L.res);
     int* its = (int*)(c->ws + L.its);
     // q is staged in the V slot: the start consumes q before it clears V
-    float2* Qs = (float2*)(c->ws + L.V);
-    CK(cudaMemcpyAsync(Qs, q_host, vbytes, cudaMemcpyHostToDevice, c->stream));
+    float2* Qs = q_host ? (float2*)(c->ws + L.V) : nullptr;
+    float2* As = (float2*)(c->ws + L.alphas);
+    if (Qs) CK(cudaMemcpyAsync(Qs, q_host, vbytes, cudaMemcpyHostToDevice, c->stream));
     if (dbytes) CK(cudaMemcpyAsync(Ds, d_host, dbytes, cudaMemcpyHostToDevice, c->stream));
     if (tol_host) CK(cudaMemcpyAsync(tols, tol_host, nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));
-    rc = lsqr_begin_impl(c, nb, omega_idx_host, Qs, Ds, lambda, tol_host ? tols : nullptr, maxit, Xs, res, its, true);
+    rc = lsqr_begin_impl(c, nb, omega_idx_host, Qs, Ds, lambda, tol_host ? tols : nullptr, maxit, Xs, res, its,
+                         true, src_ijk_host, sf ? As : nullptr);
     if (rc) return rc;
     if ((rc = wri_lsqr_iterate(c, maxit))) { c->solving = false; return rc; }
     if ((rc = wri_lsqr_end(c))) return rc;
     CK(cudaMemcpyAsync(u_out_host, Xs, vbytes, cudaMemcpyDeviceToHost, c->stream));
     CK(cudaMemcpyAsync(resnorms_host, res, (size_t)(maxit + 1) * nb * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
     if (iters_host) CK(cudaMemcpyAsync(iters_host, its, nb * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    if (sf) CK(cudaMemcpyAsync(alpha_out_host, As, nb * sizeof(float2), cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
     return WRI_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int wri_lsqr_batch_host(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const void* q_host,
+                        const void* d_host, float lambda, const float* tol_host, int32_t maxit,
+                        void* u_out_host, float* resnorms_host, int32_t* iters_host) {
+    if (!q_host) return WRI_ERR_ARG;
+    return lsqr_batch_host_impl(c, nb, omega_idx_host, nullptr, q_host, d_host, lambda, tol_host, maxit,
+                                u_out_host, nullptr, resnorms_host, iters_host);
+}
+
+int wri_lsqr_sf_batch_host(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const int32_t* src_ijk_host,
+                           const void* q_host, const void* d_host, float lambda, const float* tol_host,
+                           int32_t maxit, void* u_out_host, void* alpha_out_host, float* resnorms_host,
+                           int32_t* iters_host) {
+    if (!src_ijk_host) return WRI_ERR_ARG;
+    return lsqr_batch_host_impl(c, nb, omega_idx_host, src_ijk_host, q_host, d_host, lambda, tol_host, maxit,
+                                u_out_host, alpha_out_host, resnorms_host, iters_host);
 }
 
 int wri_lsqr_peek(const wri_ctx* c, wri_lsqr_view* v) {
@@ -1073,6 +1172,8 @@ int wri_lsqr_peek(const wri_ctx* c, wri_lsqr_view* v) {
     v->cx = c->coef + C_CX * NM;
     v->cw = c->coef + C_CW * NM;
     v->active = c->active; v->iters = c->iters;
+    v->nb_max = c->nb_max;
+    v->sf_state = c->sf ? c->stat + S_VA_RE * NM : nullptr;
     return WRI_OK;
 }
 

@@ -23,7 +23,10 @@ enum PassMode { MODE_APPLY = 0, MODE_A = 1, MODE_F = 2, MODE_INIT = 3 };
 // per-column float coefficients, one row of nb_max each
 enum Coef { C_CA_F = 0, C_CB_F, C_CV_F, C_CX, C_CW, C_CA_A, C_CB_A, C_CT_A, C_W2, C_ONE, C_LAM, N_COEF };
 // per-column double state, one row of nb_max each
-enum Stat { S_ALPHA = 0, S_BETA, S_RHOBAR, S_PHIBAR, S_AR0, N_STAT };
+// (S_VA.. S_XA: the source-weight entries of V, W, X in the source-free system, re/im pairs;
+//  V's entry is stored un-normalised like V itself)
+enum Stat { S_ALPHA = 0, S_BETA, S_RHOBAR, S_PHIBAR, S_AR0,
+            S_VA_RE, S_VA_IM, S_WA_RE, S_WA_IM, S_XA_RE, S_XA_IM, N_STAT };
 
 struct PassParams {
     const float2* in;      // stencil input [n_g][nb]
@@ -232,6 +235,27 @@ __global__ void k_scatter_add(float2* __restrict__ x, const int* __restrict__ re
     }
 }
 
+// Source column of S = [lambda A, -lambda e; P, 0] (eq. 6), one entry per batch column:
+//   forward : ytop[src[s]][s] -= lambda * a[s]            (after ytop = lambda A x)
+//   adjoint : xa[s] = -lambda * ytop[src[s]][s]           (e is a real unit vector)
+__global__ void k_src_forward(float2* __restrict__ ytop, const int* __restrict__ src, int nb, float lambda,
+                              const float2* __restrict__ a) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s < nb) {
+        float2* y = ytop + (size_t)src[s] * nb + s;
+        const float2 t = *y, as = a[s];
+        *y = make_float2(fmaf(-lambda, as.x, t.x), fmaf(-lambda, as.y, t.y));
+    }
+}
+__global__ void k_src_adjoint(const float2* __restrict__ ytop, const int* __restrict__ src, int nb, float lambda,
+                              float2* __restrict__ xa) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s < nb) {
+        const float2 t = ytop[(size_t)src[s] * nb + s];
+        xa[s] = make_float2(-lambda * t.x, -lambda * t.y);
+    }
+}
+
 // X += cx * W over the whole batch (last deferred update, wri_lsqr_end)
 __global__ void k_flush_x(float2* __restrict__ X, const float2* __restrict__ W,
                           const float* __restrict__ cx, long long n, int nb) {
@@ -275,6 +299,10 @@ struct ScalParams {
                               //    finaliser only reduces partials and runs the recurrences
     const int* colmap;        // [nb] working column -> caller's column (-1 = padding); null = identity
     int nb_out;               // caller's batch width: row stride of resnorms
+    // source-free system S = [lambda A, -lambda e; P, 0]: one more unknown per column
+    const int* src;           // [nb_out] source cell of the CALLER's column, or null (known-source system)
+    float2* U;                // [n_g][nb] top rows of u (its source-node entry takes the -lambda e column)
+    float2* alpha_out;        // [nb_out] source-weight estimate of x_k, c64
 };
 
 // sum over tiles of partials[.][s] in fixed order; result for column s in colsum[s] (shared)
@@ -364,8 +392,33 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
     if (PHASE == PH_INIT_B || (PHASE == PH_F && !p.rows_in_pass)) add_receiver_norms(p, scratch, colsum);
 
     for (int s = threadIdx.x; s < nb; s += blockDim.x) {
-        const double nrm = sqrt(colsum[s]);
+        const int so = p.colmap ? p.colmap[s] : s;           // caller's column of working column s
+        const int sc = (p.src && so >= 0) ? p.src[so] : -1;  // source cell (source-free system) or -1
+        double cs = colsum[s];
+        if (sc >= 0 && PHASE != PH_INIT_B && p.active[s]) {
+            // the extra column -lambda e of S and its row of S^H (one entry per column):
+            double va_re = st[S_VA_RE * NM + s], va_im = st[S_VA_IM * NM + s];
+            float2* up = p.U + (size_t)sc * nb + s;
+            const float2 o = __ldcg(up);
+            if (PHASE == PH_F) {
+                // u_top[src] -= (lambda/alpha) v_a ; the squared norm follows by the difference
+                const double ca = (double)cf[C_CA_F * NM + s];
+                const float2 n = make_float2((float)((double)o.x - ca * va_re), (float)((double)o.y - ca * va_im));
+                *up = n;
+                cs += ((double)n.x * n.x + (double)n.y * n.y) - ((double)o.x * o.x + (double)o.y * o.y);
+            } else {
+                // v_a <- -(lambda/beta) u_top[src] - (beta/alpha) v_a  (first pass: old v_a = 0)
+                const double ca = (double)cf[C_CA_A * NM + s], cb = (double)cf[C_CB_A * NM + s];
+                va_re = -ca * (double)o.x - cb * va_re;
+                va_im = -ca * (double)o.y - cb * va_im;
+                st[S_VA_RE * NM + s] = va_re; st[S_VA_IM * NM + s] = va_im;
+                cs += va_re * va_re + va_im * va_im;
+            }
+        }
+        const double nrm = sqrt(fmax(cs, 0.0));
         if (PHASE == PH_INIT_B) {
+            for (int r = S_VA_RE; r <= S_XA_IM; ++r) st[r * NM + s] = 0.0;
+            if (p.alpha_out) p.alpha_out[s] = make_float2(0.f, 0.f);
             // beta1 u1 = b.  b = 0 => x = 0, nothing to iterate (reading C-7).
             const double beta = nrm;
             st[S_BETA * NM + s] = beta;
@@ -395,6 +448,10 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
             cf[C_CA_F * NM + s] = act ? (float)((double)p.lambda / alpha) : 0.f;
             cf[C_CV_F * NM + s] = act ? (float)(1.0 / alpha) : 0.f;
             cf[C_CB_F * NM + s] = act ? (float)(alpha / beta) : 0.f;
+            if (sc >= 0) {                                    // w1 = v1, x0 = 0
+                st[S_WA_RE * NM + s] = act ? st[S_VA_RE * NM + s] / alpha : 0.0;
+                st[S_WA_IM * NM + s] = act ? st[S_VA_IM * NM + s] / alpha : 0.0;
+            }
         } else if (PHASE == PH_F) {
             // beta_{k+1} = ||M v_k - alpha_k u_k||
             const int act = p.active[s];
@@ -411,7 +468,6 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
             }
         } else {  // PH_A
             int act = p.active[s];
-            const int so = p.colmap ? p.colmap[s] : s;       // caller's column of working column s
             if (act) {
                 // alpha_{k+1} = ||M^H u_{k+1} - beta_{k+1} v_k||, then the plane rotation
                 const double alpha = nrm, beta = st[S_BETA * NM + s];
@@ -431,6 +487,19 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
                 bool stop = !(beta > 0.0) || !(alpha > 0.0);
                 if (tol > 0.f && arnorm <= (double)tol * st[S_AR0 * NM + s]) stop = true;
                 cf[C_CX * NM + s] = (float)(phi / rho);
+                if (sc >= 0) {
+                    // the alpha entries of x and w are updated at once (the vectors' updates are
+                    // deferred to the next pass F):  x_a += (phi/rho) w_a ; w_a = v_a/alpha - (theta/rho) w_a
+                    const double t1 = phi / rho, t2 = theta / rho;
+                    const double wr = st[S_WA_RE * NM + s], wi = st[S_WA_IM * NM + s];
+                    const double xr = st[S_XA_RE * NM + s] + t1 * wr, xi = st[S_XA_IM * NM + s] + t1 * wi;
+                    st[S_XA_RE * NM + s] = xr; st[S_XA_IM * NM + s] = xi;
+                    if (!stop) {
+                        st[S_WA_RE * NM + s] = st[S_VA_RE * NM + s] / alpha - t2 * wr;
+                        st[S_WA_IM * NM + s] = st[S_VA_IM * NM + s] / alpha - t2 * wi;
+                    }
+                    if (p.alpha_out) p.alpha_out[so] = make_float2((float)xr, (float)xi);
+                }
                 if (stop) {
                     act = 0; p.active[s] = 0;
                     cf[C_CW * NM + s] = 0.f;

@@ -31,3 +31,13 @@ def gpu_state_column(st, s):
                 w=v - float(st["cw"][s]) * W,
                 x=st["X"][:, s].astype(np.complex128) + float(st["cx"][s]) * W,
                 alpha=alpha, beta=beta, rhobar=float(st["rhobar"][s]), phibar=float(st["phibar"][s]))
+
+
+def gpu_state_column_sf(st, s):
+    """Same for a source-free solve: adds the alpha entries of v, w, x (sf_state of
+    wri_lsqr_view: v_a un-normalised like V; w_a and x_a are not deferred)."""
+    g = gpu_state_column(st, s)
+    g["v_a"] = complex(st["v_a"][s]) / g["alpha"]
+    g["w_a"] = complex(st["w_a"][s])
+    g["x_a"] = complex(st["x_a"][s])
+    return g
