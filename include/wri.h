@@ -151,6 +151,23 @@ int wri_lsqr_sf_batch_host(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_ho
                            float lambda, const float* tol_host, int32_t maxit, void* u_out_host,
                            void* alpha_out_host, float* resnorms_host, int32_t* iters_host);
 
+/* Objective and gradient of the reduced problem at given wavefields (eq. 4,
+ * 98-110 eq. 8-9; "does not involve additional PDE solvers"), per batch column s:
+ *     r_s       = A u_s - q_s - alpha_s e_s
+ *     f_pde[s]  = 1/2 lambda^2 || r_s ||^2          f_data[s] = 1/2 || P u_s - d_s ||^2
+ *     g[c]     += sum_s lambda^2 omega_s^2 Re[ conj((1 + i gamma_c) u_cs) r_cs ]
+ * f_pde + f_data = f2 of eq. 4 (= 1/2 ||S x - b||^2, eq. 5); g is eq. 9 with dA/dm_c =
+ * omega^2 (1 + i gamma_c) of this build's sponge (equal to the printed formula where gamma = 0;
+ * the real part is implied, m is real).  The sum over the batch is the paper's sum over sources
+ * and frequencies; g_dev (float32 [n_g]) is ACCUMULATED so that several batches add up — clear
+ * it first; NULL skips the gradient.  src_ijk_host/alpha_dev (c64 [nb]) and q_dev are each
+ * optional: the source-free solve passes the first pair, the known-source solve passes q_dev.
+ * f_pde_dev, f_data_dev: double [nb].  Needs a workspace; nb <= 1024.  Bit-reproducible.       */
+int wri_objective_gradient(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_host,
+                           const int32_t* src_ijk_host, const void* alpha_dev, const void* q_dev,
+                           const void* u_dev, const void* d_dev, float lambda,
+                           double* f_pde_dev, double* f_data_dev, float* g_dev);
+
 /* Same solve with HOST buffers: copies q, d (and tol) to the device, solves, copies u_out,
  * resnorms and iters back, then synchronises the stream.  Needs a workspace sized with
  * host_staging = 1.  Pinned host memory makes the copies asynchronous but is not required.   */

@@ -80,6 +80,7 @@ def load_library():
     lib.wri_lsqr_sf_batch.argtypes = solve_sf
     lib.wri_lsqr_sf_begin.argtypes = solve_sf
     lib.wri_lsqr_sf_batch_host.argtypes = solve_sf
+    lib.wri_objective_gradient.argtypes = [P, I32, P, P, P, P, P, P, F32, P, P, P]
     lib.wri_lsqr_iterate.argtypes = [P, I32]
     lib.wri_lsqr_end.argtypes = [P]
     lib.wri_lsqr_peek.argtypes = [P, C.POINTER(wri_lsqr_view)]
@@ -306,6 +307,19 @@ class Wri:
         _ck(self._lib.wri_lsqr_sf_begin(self._h, nb, oi, si, _dptr(q), _dptr(d), float(lam), _dptr(tol),
                                         int(maxit), _dptr(u), _dptr(a), _dptr(res), _dptr(it)))
         return u, a, res, it
+
+    def objective_gradient(self, u, d, lam, omega_idx=None, q=None, src_ijk=None, alpha=None, g=None):
+        """(f_pde [nb], f_data [nb]) float64 tensors; g (float32 [n_g]) is accumulated in place."""
+        t = self._torch
+        nb = u.shape[1]
+        self.ensure_workspace(nb)
+        fp = t.empty(nb, dtype=t.float64, device=u.device)
+        fd = t.empty(nb, dtype=t.float64, device=u.device)
+        keep, oi = _i32(omega_idx)
+        keep2, si = _i32(src_ijk)
+        _ck(self._lib.wri_objective_gradient(self._h, nb, oi, si, _dptr(alpha), _dptr(q), _dptr(u), _dptr(d),
+                                             float(lam), _dptr(fp), _dptr(fd), _dptr(g)))
+        return fp, fd
 
     def lsqr_iterate(self, n_steps=1):
         _ck(self._lib.wri_lsqr_iterate(self._h, int(n_steps)))

@@ -139,6 +139,33 @@ Tiling make_tiling(const wri_ctx* c, int nb) {
     return t;
 }
 
+// Thread mapping of k_grad: the TPC = nb / vec threads of one cell sit side by side in a block row.
+struct GradTiling { Tiling t; int tpc; int shuffle; bool ok; };
+GradTiling make_grad_tiling(const wri_ctx* c, int nb) {
+    GradTiling G{};
+    G.t.vec = (nb % 2 == 0) ? 2 : 1;
+    G.tpc = nb / G.t.vec;
+    G.ok = G.tpc <= 512;
+    if (!G.ok) return G;
+    G.shuffle = G.tpc <= 32 && (G.tpc & (G.tpc - 1)) == 0;
+    const int tx = G.shuffle ? 128 : G.tpc * std::max(1, 128 / G.tpc);
+    int ty = std::max(1, 256 / tx);
+    while (ty > 1 && ty / 2 >= c->g.ny) ty /= 2;
+    if (G.shuffle && (tx * ty) % 32) ty = 1;
+    G.t.block = dim3(tx, ty, 1);
+    const long long row_threads = (long long)c->g.nx * G.tpc;
+    const unsigned gx = (unsigned)((row_threads + tx - 1) / tx);
+    const unsigned gy = (unsigned)((c->g.ny + ty - 1) / ty);
+    int zc = c->g.nz;
+    const long long want = 148LL * 4 * 16;
+    while (zc > 8 && (long long)gx * gy * ((c->g.nz + zc - 1) / zc) < want) zc = (zc + 1) / 2;
+    G.t.zc = zc;
+    const unsigned gz = (unsigned)((c->g.nz + zc - 1) / zc);
+    G.t.grid = dim3(gx, gy, gz);
+    G.t.n_tiles = (size_t)gx * gy * gz;
+    return G;
+}
+
 struct WsLayout {
     size_t U, V, W, U_bot, partials, partials_tma, Xs, Ds, tols, res, its, alphas, B3, B4, U_bot2, total;
 };
@@ -153,7 +180,8 @@ WsLayout ws_layout(const wri_ctx* c, int nb, int flags, int maxit_cap) {
     L.V = o; o += vec;
     L.W = o; o += vec;
     L.U_bot = o; o += bot;
-    L.partials = o; o += align_up(t.n_tiles * nb * sizeof(double), 256);
+    const GradTiling gt = make_grad_tiling(c, nb);
+    L.partials = o; o += align_up(std::max(t.n_tiles, gt.ok ? gt.t.n_tiles : 0) * nb * sizeof(double), 256);
     L.partials_tma = o; o += align_up((size_t)kMaxCtas * nb * sizeof(double), 256);
     if (flags & WS_HOST_STAGING) {
         L.Xs = o; o += vec;
@@ -816,6 +844,50 @@ int wri_apply_SH(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const in
     if ((rc = upload_sources(c, nb, src_ijk_host))) return rc;
     k_src_adjoint<<<(nb + 127) / 128, 128, 0, c->stream>>>((const float2*)ytop_dev, c->src, nb, lambda,
                                                           (float2*)xalpha_dev);
+    c->launches++;
+    CK(cudaGetLastError());
+    return WRI_OK;
+}
+
+int wri_objective_gradient(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host,
+                           const int32_t* src_ijk_host, const void* alpha_dev, const void* q_dev,
+                           const void* u_dev, const void* d_dev, float lambda, double* f_pde_dev,
+                           double* f_data_dev, float* g_dev) {
+    int rc = check_batch_args(c, nb);
+    if (rc) return rc;
+    if (!u_dev || !aligned16(u_dev) || (q_dev && !aligned16(q_dev)) || (c->n_rec && !d_dev) || !f_pde_dev ||
+        !f_data_dev || (src_ijk_host && !alpha_dev))
+        return WRI_ERR_ARG;
+    if (c->solving) return WRI_ERR_STATE;
+    const GradTiling G = make_grad_tiling(c, nb);
+    if (!G.ok) return WRI_ERR_ARG;
+    if (!c->ws) return WRI_ERR_WORKSPACE;
+    const WsLayout L = ws_layout(c, nb, 0, kHostMaxitCap);
+    if (c->ws_bytes < L.total) return WRI_ERR_WORKSPACE;
+    if ((rc = upload_columns(c, nb, omega_idx_host, lambda))) return rc;
+    if (src_ijk_host && (rc = upload_sources(c, nb, src_ijk_host))) return rc;
+    GradParams p{};
+    p.u = (const float2*)u_dev; p.q = (const float2*)q_dev;
+    p.src = src_ijk_host ? c->src : nullptr; p.alpha = (const float2*)alpha_dev;
+    p.m = c->m;
+    p.gx = c->gtab; p.gy = c->gtab + c->g.nx; p.gz = c->gtab + c->g.nx + c->g.ny;
+    p.w2 = c->coef + C_W2 * (size_t)c->nb_max;
+    p.g = g_dev;
+    p.partials = (double*)(c->ws + L.partials);
+    p.nx = c->g.nx; p.ny = c->g.ny; p.nz = c->g.nz; p.nb = nb; p.zc = G.t.zc;
+    p.tpc = G.tpc; p.shuffle = G.shuffle;
+    p.ih2 = (float)(1.0 / (c->h * c->h));
+    p.m6ih2 = (float)(-6.0 / (c->h * c->h));
+    p.lam2 = lambda * lambda;
+    const size_t smem = (size_t)G.t.block.x * G.t.block.y * G.t.vec * sizeof(double);
+    if (G.t.vec == 2) k_grad<2><<<G.t.grid, G.t.block, smem, c->stream>>>(p);
+    else              k_grad<1><<<G.t.grid, G.t.block, smem, c->stream>>>(p);
+    c->launches++;
+    CK(cudaGetLastError());
+    k_objective<<<1, 1024, 1024 * sizeof(double), c->stream>>>(p.partials, (int)G.t.n_tiles, nb, p.u,
+                                                             (const float2*)d_dev, c->rec, c->n_rec,
+                                                             (double)lambda * (double)lambda, f_pde_dev,
+                                                             f_data_dev);
     c->launches++;
     CK(cudaGetLastError());
     return WRI_OK;

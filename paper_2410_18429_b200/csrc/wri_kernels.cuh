@@ -604,6 +604,167 @@ __global__ void k_gather_scalars(float* __restrict__ coef_dst, const float* __re
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Objective and gradient of the reduced problem (eq. 4, 98-110 eq. 8-9), at given
+// wavefields u (and source weights):   r = A u - q - alpha e,
+//   f_pde[s]  = 1/2 lambda^2 ||r_s||^2,   f_data[s] = 1/2 ||P u_s - d_s||^2,
+//   g[c]     += sum_s lambda^2 omega_s^2 Re[ conj((1 + i gamma_c) u_cs) r_cs ]
+// (eq. 9 with dA/dm_c = omega^2 (1 + i gamma_c) of this build's sponge; the sum over the batch
+// columns is the paper's sum over sources and frequencies).  Same thread mapping and z march as
+// k_pass; the threads of one cell are TPC = nb / VEC consecutive threads of a block row (the
+// host makes blockDim.x a multiple of TPC), reduced in a fixed order — warp shuffles when TPC is
+// a power of two <= 32, shared memory otherwise — so g is bit-reproducible.
+struct GradParams {
+    const float2* u;       // [n_g][nb]
+    const float2* q;       // [n_g][nb] or null
+    const int* src;        // [nb] source cells or null
+    const float2* alpha;   // [nb] source weights (with src)
+    const float* m;
+    const float *gx, *gy, *gz;
+    const float* w2;       // [nb]
+    float* g;              // [n_g], accumulated; may be null
+    double* partials;      // [n_tiles][nb] sums of |r|^2
+    int nx, ny, nz, nb, zc;
+    int tpc;               // threads per cell
+    int shuffle;           // 1: tpc is a power of two <= 32
+    float ih2, m6ih2, lam2;
+};
+
+template <int VEC>
+__global__ void __launch_bounds__(512)
+k_grad(const GradParams p) {
+    extern __shared__ double red[];                          // block_column_sums scratch; reused per plane
+    const int nb = p.nb;
+    const int RL = p.nx * nb;
+    const int e0 = (blockIdx.x * blockDim.x + threadIdx.x) * VEC;
+    const int iy = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z0 = blockIdx.z * p.zc;
+    const int z1 = min(z0 + p.zc, p.nz);
+    const bool live = (e0 < RL) && (iy < p.ny);
+    const int tlin = threadIdx.y * blockDim.x + threadIdx.x;
+    float* gsm = reinterpret_cast<float*>(red);              // [blockDim.x * blockDim.y] per-thread g terms
+
+    double acc[VEC];
+#pragma unroll
+    for (int k = 0; k < VEC; ++k) acc[k] = 0.0;
+
+    const int ix = live ? e0 / nb : 0;
+    const int s0 = live ? e0 - ix * nb : 0;
+    float w2[VEC];
+    int srcc[VEC];
+    float2 al[VEC];
+#pragma unroll
+    for (int k = 0; k < VEC; ++k) {
+        w2[k] = live ? p.w2[s0 + k] : 0.f;
+        srcc[k] = (live && p.src) ? p.src[s0 + k] : -1;
+        al[k] = (live && p.src) ? p.alpha[s0 + k] : make_float2(0.f, 0.f);
+    }
+    const bool has_xm = ix > 0, has_xp = ix < p.nx - 1;
+    const bool has_ym = iy > 0, has_yp = iy < p.ny - 1;
+    const size_t plane = (size_t)RL * p.ny;
+    const float gxy = live ? fmaxf(p.gx[ix], p.gy[iy]) : 0.f;
+    size_t off = live ? ((size_t)z0 * p.ny + iy) * RL + e0 : 0;
+    size_t cell = live ? ((size_t)z0 * p.ny + iy) * p.nx + ix : 0;
+    CV<VEC> prev = zero_v<VEC>(), cur = zero_v<VEC>(), nxt;
+    if (live) {
+        cur = ldg_ro<VEC>(p.u + off);
+        if (z0 > 0) prev = ldg_ro<VEC>(p.u + off - plane);
+    }
+
+#pragma unroll 1
+    for (int z = z0; z < z1; ++z) {
+        float gterm = 0.f;
+        if (live) {
+            nxt = zero_v<VEC>();
+            if (z + 1 < p.nz) nxt = ldg_ro<VEC>(p.u + off + plane);
+            CV<VEC> xm = zero_v<VEC>(), xp = zero_v<VEC>(), ym = zero_v<VEC>(), yp = zero_v<VEC>();
+            if (has_xm) xm = ldg_ro<VEC>(p.u + off - nb);
+            if (has_xp) xp = ldg_ro<VEC>(p.u + off + nb);
+            if (has_ym) ym = ldg_ro<VEC>(p.u + off - RL);
+            if (has_yp) yp = ldg_ro<VEC>(p.u + off + RL);
+            CV<VEC> qv = zero_v<VEC>();
+            if (p.q) qv = ld_rw<VEC>(p.q + off);
+            const float mc = __ldg(p.m + cell);
+            const float gam = fmaxf(gxy, p.gz[z]);
+#pragma unroll
+            for (int k = 0; k < VEC; ++k) {
+                const float wm = w2[k] * mc;
+                const float dr = wm + p.m6ih2, di = wm * gam;
+                const float sr = ((xm.a[k].x + xp.a[k].x) + (ym.a[k].x + yp.a[k].x)) + (prev.a[k].x + nxt.a[k].x);
+                const float si = ((xm.a[k].y + xp.a[k].y) + (ym.a[k].y + yp.a[k].y)) + (prev.a[k].y + nxt.a[k].y);
+                float rr = fmaf(p.ih2, sr, fmaf(dr, cur.a[k].x, -di * cur.a[k].y)) - qv.a[k].x;
+                float ri = fmaf(p.ih2, si, fmaf(dr, cur.a[k].y, di * cur.a[k].x)) - qv.a[k].y;
+                if ((int)cell == srcc[k]) { rr -= al[k].x; ri -= al[k].y; }
+                acc[k] += (double)fmaf(rr, rr, ri * ri);
+                // Re[conj((1 + i gamma) u) r] = Re t + gamma Im t,  t = conj(u) r
+                const float tr = fmaf(cur.a[k].x, rr, cur.a[k].y * ri);
+                const float ti = fmaf(cur.a[k].x, ri, -cur.a[k].y * rr);
+                gterm = fmaf(w2[k], fmaf(gam, ti, tr), gterm);
+            }
+            prev = cur; cur = nxt;
+        }
+        if (p.g) {
+            if (p.shuffle) {
+                for (int d = p.tpc >> 1; d > 0; d >>= 1) gterm += __shfl_down_sync(0xffffffffu, gterm, d, p.tpc);
+                if (live && (threadIdx.x % p.tpc) == 0) p.g[cell] += p.lam2 * gterm;
+            } else {
+                gsm[tlin] = gterm;
+                __syncthreads();
+                if (live && (threadIdx.x % p.tpc) == 0) {
+                    float t = 0.f;
+                    for (int j = 0; j < p.tpc; ++j) t += gsm[tlin + j];
+                    p.g[cell] += p.lam2 * t;
+                }
+                __syncthreads();
+            }
+        }
+        off += plane;
+        cell += (size_t)p.nx * p.ny;
+    }
+    const size_t tile = ((size_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+    const int col0 = (int)(((long long)blockIdx.x * blockDim.x * VEC) % nb);
+    __syncthreads();
+    block_column_sums<VEC>(acc, col0, nb, p.partials + tile * nb);
+}
+
+// f_pde[s] = 1/2 lambda^2 sum_tiles partials[.][s];  f_data[s] = 1/2 sum_r |u[rec_r][s] - d[r][s]|^2
+// One block; fixed summation order.
+__global__ void __launch_bounds__(1024)
+k_objective(const double* __restrict__ partials, int n_tiles, int nb, const float2* __restrict__ u,
+            const float2* __restrict__ d, const int* __restrict__ rec, int n_rec, double lam2,
+            double* __restrict__ f_pde, double* __restrict__ f_data) {
+    extern __shared__ double sh_obj[];                       // [blockDim.x]
+    const int T = blockDim.x;
+    for (int base = 0; base < nb; base += T) {
+        const int ncol = min(nb - base, T);
+        const int Gc = max(1, T / ncol);
+        const int g = threadIdx.x / ncol, s = base + threadIdx.x % ncol;
+        for (int pass = 0; pass < 2; ++pass) {
+            double a = 0.0;
+            if (g < Gc) {
+                if (pass == 0) {
+                    for (int b = g; b < n_tiles; b += Gc) a += __ldcg(partials + (size_t)b * nb + s);
+                } else {
+                    for (int r = g; r < n_rec; r += Gc) {
+                        const float2 uv = u[(size_t)rec[r] * nb + s], dv = d[(size_t)r * nb + s];
+                        const double er = (double)uv.x - (double)dv.x, ei = (double)uv.y - (double)dv.y;
+                        a += er * er + ei * ei;
+                    }
+                }
+            }
+            sh_obj[threadIdx.x] = a;
+            __syncthreads();
+            if (threadIdx.x < ncol) {
+                double t = 0.0;
+                for (int gg = 0; gg < Gc; ++gg) t += sh_obj[gg * ncol + threadIdx.x];
+                if (pass == 0) f_pde[base + threadIdx.x] = 0.5 * lam2 * t;
+                else f_data[base + threadIdx.x] = 0.5 * t;
+            }
+            __syncthreads();
+        }
+    }
+}
+
 template <int PHASE>
 __global__ void __launch_bounds__(1024)
 k_scalars(const ScalParams p) {
