@@ -270,6 +270,41 @@ def run_ours(args, wl_name, w):
     d2h = outh[0].numel() * 8 + outh[1].numel() * 4 + outh[2].numel() * 4
     iters_e2e = int(outh[2].sum().item())
 
+    # ---- the same workload through the paper's own source-free system (unknown source weight per
+    #      column, eq. 4-6) and one objective + gradient evaluation (eq. 8-9); context lines, N = 1 only
+    extras = None
+    if world == 1 and not args.no_extras and w.src_ijk is not None:
+        extras = {}
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+        ctx.lsqr_sf_batch(d, w.lam, w.src_ijk, tol, maxit=maxit, omega_idx=w.omega_idx)      # warm-up
+        torch.cuda.synchronize()
+        ev[0].record()
+        n_sf = 2
+        for _ in range(n_sf):
+            u_sf, a_sf, _, it_sf = ctx.lsqr_sf_batch(d, w.lam, w.src_ijk, tol, maxit=maxit, omega_idx=w.omega_idx)
+        ev[1].record()
+        torch.cuda.synchronize()
+        ms_sf = ev[0].elapsed_time(ev[1]) / n_sf
+        extras["sourcefree_lsqr"] = {"value": int(it_sf.sum().item()) / (ms_sf * 1e-3), "unit": UNIT,
+                                     "ms_per_step": ms_sf, "system": "S = [lam A, -lam e; P, 0], b = [0; d]"}
+        g = torch.zeros(w.ng, dtype=torch.float32, device=dev)
+        ctx.objective_gradient(u_sf, d, w.lam, omega_idx=w.omega_idx, src_ijk=w.src_ijk, alpha=a_sf, g=g)
+        torch.cuda.synchronize()
+        n_g = 5
+        ev[2].record()
+        for _ in range(n_g):
+            ctx.objective_gradient(u_sf, d, w.lam, omega_idx=w.omega_idx, src_ijk=w.src_ijk, alpha=a_sf, g=g)
+        ev[3].record()
+        torch.cuda.synchronize()
+        ms_g = ev[2].elapsed_time(ev[3]) / n_g
+        bytes_g = (8 * nb + 4 + 8) * w.ng          # u read once, m read, g read + written
+        peak_g, _ = measured_hbm_peak()
+        extras["objective_gradient"] = {"ms": ms_g, "algorithmic_bytes": bytes_g,
+                                        "achieved": bytes_g / (ms_g * 1e-3) / 1e9, "unit": "GB/s",
+                                        "frac": bytes_g / (ms_g * 1e-3) / 1e9 / peak_g,
+                                        "kernel": "k_grad + k_objective (eq. 9 fused with the stencil residual)"}
+        del u_sf, g
+
     (ms, e2e_s), (iters_all, iters_e2e_all, launches_all) = reduce_over_ranks(
         [ms, e2e_s], [iters_per_step, iters_e2e, launches], dist if use_dist else None, dev)
     launches_all = int(launches_all)
@@ -297,7 +332,7 @@ def run_ours(args, wl_name, w):
             "e2e": {"value": iters_e2e_all * e2e_steps / e2e_s, "unit": UNIT,
                     "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps},
             "gpu_launches": launches_all,
-            "roofline": {"bound": "hbm", "kernel": "k_pass<MODE_F> (forward stencil + u axpy + x,w update + ||u||^2)",
+            "roofline": {"bound": "hbm", "kernel": "k_pass_tma<MODE_F> (forward stencil + u axpy + x,w update + ||u||^2)",
                          "achieved": ach_f, "peak": peak, "peak_source": peak_src, "unit": "GB/s",
                          "frac": (ach_f / peak) if ach_f else None,
                          "traffic": ncu_traffic_bytes() if wl_name == DEFAULT_WORKLOAD else None,
@@ -309,6 +344,8 @@ def run_ours(args, wl_name, w):
                          "whole_step": {"achieved": ach_iter, "frac": ach_iter / peak,
                                         "frac_of_8000": ach_iter / 8000.0}},
         }
+        if extras:
+            line["extras"] = extras
         if world == 1 and not args.no_cpu_baseline:
             cores = os.cpu_count() or 1
             r, ncols, dt, sample = oracle_sample(w, cores, oracle_iters_for(w))
@@ -328,6 +365,8 @@ def main():
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(WORKLOADS))
     ap.add_argument("--maxit", type=int, default=None, help="override the workload's iteration count")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true",
+                    help="skip the source-free solve and the objective/gradient context lines")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference" and dist_env()[0] != 0:

@@ -30,6 +30,7 @@ int cuda_fail(cudaError_t e, const char* what) {
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
+inline unsigned blocks_for(long long n) { return (unsigned)std::min<long long>((n + 255) / 256, 148 * 16); }
 constexpr int kMaxCtas = 512;          // upper bound on the persistent grid (>= SM count)
 constexpr int kMinChunk = 4;           // narrowest column chunk of the TMA path
 
@@ -104,7 +105,7 @@ struct wri_ctx {
         CUtensorMap in{}, old{}, w{}, x{}, m{};
         int m_tma = 0;                    // model tile rides in the TMA stage
         int merged = 0;                   // tensor maps fold (column, x)
-    } planF, planA;
+    } planF, planA, planG;
     double* partials_tma = nullptr;       // [grid][nb]
     // optional per-kernel timing (wri_profile_*)
     bool profiling = false;
@@ -157,7 +158,7 @@ GradTiling make_grad_tiling(const wri_ctx* c, int nb) {
     const unsigned gx = (unsigned)((row_threads + tx - 1) / tx);
     const unsigned gy = (unsigned)((c->g.ny + ty - 1) / ty);
     int zc = c->g.nz;
-    const long long want = 148LL * 4 * 16;
+    const long long want = 148LL * 4 * 4;
     while (zc > 8 && (long long)gx * gy * ((c->g.nz + zc - 1) / zc) < want) zc = (zc + 1) / 2;
     G.t.zc = zc;
     const unsigned gz = (unsigned)((c->g.nz + zc - 1) / zc);
@@ -167,7 +168,7 @@ GradTiling make_grad_tiling(const wri_ctx* c, int nb) {
 }
 
 struct WsLayout {
-    size_t U, V, W, U_bot, partials, partials_tma, Xs, Ds, tols, res, its, alphas, B3, B4, U_bot2, total;
+    size_t U, V, W, U_bot, partials, partials_tma, gscratch, Xs, Ds, tols, res, its, alphas, B3, B4, U_bot2, total;
 };
 enum { WS_HOST_STAGING = 1, WS_COMPACTION = 2 };
 WsLayout ws_layout(const wri_ctx* c, int nb, int flags, int maxit_cap) {
@@ -183,6 +184,7 @@ WsLayout ws_layout(const wri_ctx* c, int nb, int flags, int maxit_cap) {
     const GradTiling gt = make_grad_tiling(c, nb);
     L.partials = o; o += align_up(std::max(t.n_tiles, gt.ok ? gt.t.n_tiles : 0) * nb * sizeof(double), 256);
     L.partials_tma = o; o += align_up((size_t)kMaxCtas * nb * sizeof(double), 256);
+    L.gscratch = o; o += align_up(c->ng * sizeof(float), 256);       // one batch's gradient (TMA path)
     if (flags & WS_HOST_STAGING) {
         L.Xs = o; o += vec;
         L.Ds = o; o += bot;
@@ -223,8 +225,8 @@ int upload_sources(wri_ctx* c, int nb, const int32_t* src_ijk) {
         if (ix < 0 || ix >= c->g.nx || iy < 0 || iy >= c->g.ny || iz < 0 || iz >= c->g.nz) return WRI_ERR_ARG;
         cells[s] = (iz * c->g.ny + iy) * c->g.nx + ix;
     }
+    // pageable source: the call returns once the data sits in the driver's staging buffer
     CK(cudaMemcpyAsync(c->src, cells.data(), nb * sizeof(int), cudaMemcpyHostToDevice, c->stream));
-    CK(cudaStreamSynchronize(c->stream));        // cells is a local
     return WRI_OK;
 }
 
@@ -351,7 +353,7 @@ int make_tmap(CUtensorMap* tm, const void* base, const wri_ctx* c, int nb, int c
 #define WRI_F_NT 512
 #endif
 #ifndef WRI_A_NT
-#define WRI_A_NT 256
+#define WRI_A_NT 512
 #endif
 template <int CB, int MODE> struct CfgFor {
     static constexpr int S = 64 / CB;   // narrower chunks -> proportionally more cells per tile row
@@ -422,7 +424,8 @@ int make_tmap_model(CUtensorMap* tm, const wri_ctx* c, int bx, int by) {
 
 // tiling + tensor maps of one pass for the solve that is starting
 template <class Cfg>
-int tma_plan(wri_ctx* c, wri_ctx::TmaPlan& P, const void* in, const void* old, bool is_f) {
+int tma_plan(wri_ctx* c, wri_ctx::TmaPlan& P, const void* in, const void* old, bool is_f,
+             bool rec_lists = true) {
     P.txc = Cfg::TXC; P.tyc = Cfg::TYC;
     P.nchunk = c->nb / Cfg::CB;
     P.ntx = (c->g.nx + P.txc - 1) / P.txc;
@@ -450,7 +453,7 @@ int tma_plan(wri_ctx* c, wri_ctx::TmaPlan& P, const void* in, const void* old, b
     } else {
         P.w = P.old; P.x = P.old;          // unused by pass A
     }
-    if (!is_f && c->n_rec) {
+    if (!is_f && c->n_rec && rec_lists) {
         // receivers (x column chunks) inside each CTA's tiles, in the order the CTA walks its
         // tiles (same tile numbering as the kernel)
         const int G = P.grid, nent = c->n_rec * P.nchunk;
@@ -602,6 +605,44 @@ int launch_tma(wri_ctx* c, int phase) {
         case 4: return launch_tma_cfg<typename CfgFor<4, MODE>::type, MODE>(c, phase);
         default: return launch_tma_cfg<typename CfgFor<16, MODE>::type, MODE>(c, phase);
     }
+}
+
+// objective + gradient through the TMA pipeline (one chunk per cell, power-of-two column pairs)
+template <int CB>
+int launch_tma_grad(wri_ctx* c, const float2* u, const float2* q, const int* src, const float2* alpha,
+                    float* g, float lambda) {
+    // pass A's tile shape, 512 consumer threads (one item each): this pass is bound by
+    // instruction issue, not by DRAM, and 4 warps per scheduler hide the shared-memory latency
+    typedef typename CfgFor<CB, MODE_A>::type CfgA;
+    typedef TileCfg<CB, CfgA::TXC, CfgA::TYC, WRI_F_NT, WRI_A_STAGES> Cfg;
+    int rc = tma_plan<Cfg>(c, c->planG, u, q ? q : u, false, false);
+    if (rc) return rc;
+    static size_t attr_bytes = 0;
+    const wri_ctx::TmaPlan& P = c->planG;
+    const size_t smem = tma_smem_bytes<Cfg, MODE_G>(c);
+    if (smem > attr_bytes) {
+        CK(cudaFuncSetAttribute(k_pass_tma<Cfg, MODE_G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_bytes = smem;
+    }
+    const size_t NM = c->nb_max;
+    TmaPassParams p{};
+    p.m = c->m;
+    p.gx = c->gtab; p.gy = c->gtab + c->g.nx; p.gz = c->gtab + c->g.nx + c->g.ny;
+    p.w2 = c->coef + C_W2 * NM;
+    p.ca = p.cb = p.cv = p.cx = p.cw = p.w2;      // unused by MODE_G
+    p.partials = c->partials_tma; p.counter = c->counter;
+    p.nx = c->g.nx; p.ny = c->g.ny; p.nz = c->g.nz; p.nb = c->nb;
+    p.zc = P.zc; p.ntx = P.ntx; p.nty = P.nty; p.ntz = P.ntz;
+    p.nchunk = P.nchunk; p.n_tiles = P.tiles;
+    p.ih2 = (float)(1.0 / (c->h * c->h));
+    p.m6ih2 = (float)(-6.0 / (c->h * c->h));
+    p.sgn = 1.f;
+    p.m_tma = P.m_tma; p.merged = P.merged;
+    p.has_q = q != nullptr; p.gsrc = src; p.galpha = alpha; p.g = g; p.lam2 = lambda * lambda;
+    k_pass_tma<Cfg, MODE_G><<<P.grid, Cfg::NT + 32, smem, c->stream>>>(P.in, P.old, P.old, P.old, P.m, p);
+    c->launches++;
+    CK(cudaGetLastError());
+    return WRI_OK;
 }
 
 int check_batch_args(const wri_ctx* c, int nb) {
@@ -879,12 +920,39 @@ int wri_objective_gradient(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host
     p.ih2 = (float)(1.0 / (c->h * c->h));
     p.m6ih2 = (float)(-6.0 / (c->h * c->h));
     p.lam2 = lambda * lambda;
-    const size_t smem = (size_t)G.t.block.x * G.t.block.y * G.t.vec * sizeof(double);
-    if (G.t.vec == 2) k_grad<2><<<G.t.grid, G.t.block, smem, c->stream>>>(p);
-    else              k_grad<1><<<G.t.grid, G.t.block, smem, c->stream>>>(p);
-    c->launches++;
-    CK(cudaGetLastError());
-    k_objective<<<1, 1024, 1024 * sizeof(double), c->stream>>>(p.partials, (int)G.t.n_tiles, nb, p.u,
+    // TMA pipeline when the batch is one power-of-two chunk per cell (64 / 32 / 16 / 8 / 4 columns);
+    // the generic kernel otherwise (odd widths, 48, several chunks)
+    int cb = tma_chunk_for(nb);
+    if (cb == 48 || cb != nb || !get_encode_fn() || getenv("WRI_GRAD_GENERIC")) cb = 0;
+    int n_rows = (int)G.t.n_tiles;
+    if (cb) {
+        c->nb = nb;
+        c->partials_tma = (double*)(c->ws + L.partials_tma);
+        float* g_user = g_dev;
+        if (g_dev) g_dev = (float*)(c->ws + L.gscratch);
+        switch (cb) {
+            case 64: rc = launch_tma_grad<64>(c, p.u, p.q, p.src, p.alpha, g_dev, lambda); break;
+            case 32: rc = launch_tma_grad<32>(c, p.u, p.q, p.src, p.alpha, g_dev, lambda); break;
+            case 16: rc = launch_tma_grad<16>(c, p.u, p.q, p.src, p.alpha, g_dev, lambda); break;
+            case 8:  rc = launch_tma_grad<8>(c, p.u, p.q, p.src, p.alpha, g_dev, lambda); break;
+            default: rc = launch_tma_grad<4>(c, p.u, p.q, p.src, p.alpha, g_dev, lambda); break;
+        }
+        if (rc) return rc;
+        if (g_user) {
+            k_add_f32<<<blocks_for((long long)c->ng), 256, 0, c->stream>>>(g_user, g_dev, (long long)c->ng);
+            c->launches++;
+            CK(cudaGetLastError());
+        }
+        p.partials = c->partials_tma;
+        n_rows = c->planG.grid;
+    } else {
+        const size_t smem = (size_t)G.t.block.x * G.t.block.y * G.t.vec * sizeof(double);
+        if (G.t.vec == 2) k_grad<2><<<G.t.grid, G.t.block, smem, c->stream>>>(p);
+        else              k_grad<1><<<G.t.grid, G.t.block, smem, c->stream>>>(p);
+        c->launches++;
+        CK(cudaGetLastError());
+    }
+    k_objective<<<(nb + OBJ_CPB - 1) / OBJ_CPB, 1024, 1024 * sizeof(double), c->stream>>>(p.partials, n_rows, nb, p.u,
                                                              (const float2*)d_dev, c->rec, c->n_rec,
                                                              (double)lambda * (double)lambda, f_pde_dev,
                                                              f_data_dev);
@@ -976,7 +1044,6 @@ int lsqr_begin_impl(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const
     return WRI_OK;
 }
 
-inline unsigned blocks_for(long long n) { return (unsigned)std::min<long long>((n + 255) / 256, 148 * 16); }
 
 // x and history of the listed working columns become final in the caller's buffers:
 // u_out[:, dst] = X[:, src] + cx[src] W[:, src]; resnorms rows k+1..maxit held at phibar.

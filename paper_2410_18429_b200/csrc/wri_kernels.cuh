@@ -18,7 +18,7 @@
 
 namespace wri {
 
-enum PassMode { MODE_APPLY = 0, MODE_A = 1, MODE_F = 2, MODE_INIT = 3 };
+enum PassMode { MODE_APPLY = 0, MODE_A = 1, MODE_F = 2, MODE_INIT = 3, MODE_G = 4 };
 
 // per-column float coefficients, one row of nb_max each
 enum Coef { C_CA_F = 0, C_CB_F, C_CV_F, C_CX, C_CW, C_CA_A, C_CB_A, C_CT_A, C_W2, C_ONE, C_LAM, N_COEF };
@@ -727,41 +727,56 @@ k_grad(const GradParams p) {
     block_column_sums<VEC>(acc, col0, nb, p.partials + tile * nb);
 }
 
+// g += t  (the batch's gradient from the TMA pass into the caller's accumulated gradient)
+__global__ void k_add_f32(float* __restrict__ g, const float* __restrict__ t, long long n) {
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
+         i += (long long)gridDim.x * blockDim.x)
+        g[i] += t[i];
+}
+
 // f_pde[s] = 1/2 lambda^2 sum_tiles partials[.][s];  f_data[s] = 1/2 sum_r |u[rec_r][s] - d[r][s]|^2
-// One block; fixed summation order.
+// Block b owns OBJ_CPB consecutive columns (T / OBJ_CPB row groups each); fixed summation order.
+constexpr int OBJ_CPB = 8;
 __global__ void __launch_bounds__(1024)
 k_objective(const double* __restrict__ partials, int n_tiles, int nb, const float2* __restrict__ u,
             const float2* __restrict__ d, const int* __restrict__ rec, int n_rec, double lam2,
             double* __restrict__ f_pde, double* __restrict__ f_data) {
     extern __shared__ double sh_obj[];                       // [blockDim.x]
     const int T = blockDim.x;
-    for (int base = 0; base < nb; base += T) {
-        const int ncol = min(nb - base, T);
-        const int Gc = max(1, T / ncol);
-        const int g = threadIdx.x / ncol, s = base + threadIdx.x % ncol;
-        for (int pass = 0; pass < 2; ++pass) {
-            double a = 0.0;
-            if (g < Gc) {
-                if (pass == 0) {
-                    for (int b = g; b < n_tiles; b += Gc) a += __ldcg(partials + (size_t)b * nb + s);
-                } else {
-                    for (int r = g; r < n_rec; r += Gc) {
-                        const float2 uv = u[(size_t)rec[r] * nb + s], dv = d[(size_t)r * nb + s];
-                        const double er = (double)uv.x - (double)dv.x, ei = (double)uv.y - (double)dv.y;
-                        a += er * er + ei * ei;
-                    }
+    const int base = blockIdx.x * OBJ_CPB;
+    const int ncol = min(nb - base, OBJ_CPB);
+    const int Gc = T / OBJ_CPB;
+    const int g = threadIdx.x / OBJ_CPB, cl = threadIdx.x % OBJ_CPB, s = base + cl;
+    for (int pass = 0; pass < 2; ++pass) {
+        double a = 0.0;
+        if (cl < ncol) {
+            if (pass == 0) {
+                int b = g;
+                for (; b + 7 * Gc < n_tiles; b += 8 * Gc) {          // 8 loads in flight, added in order
+                    double t[8];
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) t[j] = __ldcg(partials + (size_t)(b + j * Gc) * nb + s);
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) a += t[j];
+                }
+                for (; b < n_tiles; b += Gc) a += __ldcg(partials + (size_t)b * nb + s);
+            } else {
+                for (int r = g; r < n_rec; r += Gc) {
+                    const float2 uv = u[(size_t)rec[r] * nb + s], dv = d[(size_t)r * nb + s];
+                    const double er = (double)uv.x - (double)dv.x, ei = (double)uv.y - (double)dv.y;
+                    a += er * er + ei * ei;
                 }
             }
-            sh_obj[threadIdx.x] = a;
-            __syncthreads();
-            if (threadIdx.x < ncol) {
-                double t = 0.0;
-                for (int gg = 0; gg < Gc; ++gg) t += sh_obj[gg * ncol + threadIdx.x];
-                if (pass == 0) f_pde[base + threadIdx.x] = 0.5 * lam2 * t;
-                else f_data[base + threadIdx.x] = 0.5 * t;
-            }
-            __syncthreads();
         }
+        sh_obj[threadIdx.x] = a;
+        __syncthreads();
+        if (threadIdx.x < ncol) {
+            double t = 0.0;
+            for (int gg = 0; gg < Gc; ++gg) t += sh_obj[gg * OBJ_CPB + threadIdx.x];
+            if (pass == 0) f_pde[base + threadIdx.x] = 0.5 * lam2 * t;
+            else f_data[base + threadIdx.x] = 0.5 * t;
+        }
+        __syncthreads();
     }
 }
 

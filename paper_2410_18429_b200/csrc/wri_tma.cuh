@@ -47,6 +47,7 @@ template <int MODE> struct PassTraits;
 #endif
 template <> struct PassTraits<MODE_F> { static constexpr int NSTREAM = 3, NSTAGE = WRI_F_STAGES; };   // default depths
 template <> struct PassTraits<MODE_A> { static constexpr int NSTREAM = 1, NSTAGE = WRI_A_STAGES; };
+template <> struct PassTraits<MODE_G> { static constexpr int NSTREAM = 1, NSTAGE = WRI_A_STAGES; };   // stream = q (optional)
 
 struct TmaPassParams {
     float2* out;           // result vector (its old values arrive through tm_old)
@@ -74,6 +75,12 @@ struct TmaPassParams {
                            //         {receiver, cell, tile, entries in this tile (at its first entry)};
                            //         with column chunks, one entry per (receiver, chunk)
     ScalParams fin;
+    // MODE_G (objective + gradient, eq. 4 / 9): out is unused; the optional stream is q
+    int has_q;
+    const int* gsrc;       // [nb] source cells or null
+    const float2* galpha;  // [nb] source weights (with gsrc)
+    float* g;              // [n_g] this batch's gradient (overwritten) or null
+    float lam2;
 };
 
 // rows x columns work with a fixed-order per-column sum: row i of `nrows`, local column s of
@@ -243,8 +250,9 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
                 if (issuer) {
                     mbar_wait(empty0 + 8 * stage, phase ^ 1);
                     const bool streams = pl >= z0 + 1;
+                    const bool old_stream = (MODE != MODE_G) || p.has_q;
                     const uint32_t fb = full0 + 8 * stage;
-                    mbar_expect_tx(fb, Cfg::IN_BYTES + (streams ? NSTREAM * Cfg::CTR_BYTES +
+                    mbar_expect_tx(fb, Cfg::IN_BYTES + (streams ? (old_stream ? NSTREAM * Cfg::CTR_BYTES : 0) +
                                                             (p.m_tma ? TXC * TYC * 4 : 0) : 0));
                     const uint32_t dst = smem_u32(stages + stage * STAGE_BYTES);
 #if WRI_HINTS >= 2
@@ -254,12 +262,14 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
 #endif
                     if (streams) {
 #if WRI_HINTS >= 1
+                        if (old_stream)
                         tma_load_4d_hint(dst + Cfg::IN_BYTES, &tm_old, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1, pol_stream);
                         if (MODE == MODE_F) {
                             tma_load_4d_hint(dst + Cfg::IN_BYTES + Cfg::CTR_BYTES, &tm_w, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1, pol_stream);
                             tma_load_4d_hint(dst + Cfg::IN_BYTES + 2 * Cfg::CTR_BYTES, &tm_x, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1, pol_stream);
                         }
 #else
+                        if (old_stream)
                         tma_load_4d(dst + Cfg::IN_BYTES, &tm_old, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1);
                         if (MODE == MODE_F) {
                             tma_load_4d(dst + Cfg::IN_BYTES + Cfg::CTR_BYTES, &tm_w, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1);
@@ -337,6 +347,12 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
                 cx[e] = tab_c[4 * p.nb + col + e];
                 cw[e] = tab_c[5 * p.nb + col + e];
             }
+            int gsrc0 = -1, gsrc1 = -1;
+            float2 gal0 = make_float2(0.f, 0.f), gal1 = gal0;
+            if (MODE == MODE_G && p.gsrc) {
+                gsrc0 = p.gsrc[col]; gsrc1 = p.gsrc[col + 1];
+                gal0 = p.galpha[col]; gal1 = p.galpha[col + 1];
+            }
             bool valid[IPT];
             float gxy[IPT], m_cur[IPT], m_nxt[IPT];
             size_t goff[IPT];                                   // element offset of (cell, z0) in the vectors
@@ -377,7 +393,7 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
                                            (a.z + b.z) + (c.z + d.z), (a.w + b.w) + (c.w + d.w));
                     if (emit) {
                         const int io = Cfg::IN_BYTES + (tid + j * NT) * 16;
-                        o_old[j] = lds128(sb, io);
+                        o_old[j] = (MODE != MODE_G || p.has_q) ? lds128(sb, io) : make_float4(0.f, 0.f, 0.f, 0.f);
                         if (p.m_tma)
                             m_cur[j] = *reinterpret_cast<const float*>(sb + M_OFF + (cyj[j] * TXC + cxj[j]) * 4);
                         if (MODE == MODE_F) {
@@ -402,6 +418,42 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
                         const float s1 = n_cur[j].y + (c_prev[j].y + c_new[j].y);
                         const float s2 = n_cur[j].z + (c_prev[j].z + c_new[j].z);
                         const float s3 = n_cur[j].w + (c_prev[j].w + c_new[j].w);
+                        if (MODE == MODE_G) {
+                            // r = A u - q - alpha e;  |r|^2 sums;  g[c] += lam^2 sum_s w2_s (Re t + gamma Im t),
+                            // t = conj(u) r  (= Re[conj((1 + i gamma) u) r], eq. 9 with this build's sponge)
+                            const int cell = (int)(moff[j] + (size_t)(z - z0) * plane_m);
+                            float gterm = 0.f;
+                            {
+                                const float wm = w2[0] * m_cur[j];
+                                const float dr = wm + p.m6ih2, di = wm * g;
+                                float r_re = fmaf(p.ih2, s0, fmaf(dr, cc.x, -di * cc.y)) - o_old[j].x;
+                                float r_im = fmaf(p.ih2, s1, fmaf(dr, cc.y, di * cc.x)) - o_old[j].y;
+                                if (cell == gsrc0) { r_re -= gal0.x; r_im -= gal0.y; }
+                                if (valid[j]) acc[0] += (double)fmaf(r_re, r_re, r_im * r_im);
+                                const float tr = fmaf(cc.x, r_re, cc.y * r_im), ti = fmaf(cc.x, r_im, -cc.y * r_re);
+                                gterm = w2[0] * fmaf(g, ti, tr);
+                            }
+                            {
+                                const float wm = w2[1] * m_cur[j];
+                                const float dr = wm + p.m6ih2, di = wm * g;
+                                float r_re = fmaf(p.ih2, s2, fmaf(dr, cc.z, -di * cc.w)) - o_old[j].z;
+                                float r_im = fmaf(p.ih2, s3, fmaf(dr, cc.w, di * cc.z)) - o_old[j].w;
+                                if (cell == gsrc1) { r_re -= gal1.x; r_im -= gal1.y; }
+                                if (valid[j]) acc[1] += (double)fmaf(r_re, r_re, r_im * r_im);
+                                const float tr = fmaf(cc.z, r_re, cc.w * r_im), ti = fmaf(cc.z, r_im, -cc.w * r_re);
+                                gterm = fmaf(w2[1], fmaf(g, ti, tr), gterm);
+                            }
+                            if (p.g) {
+                                // the HP threads of one cell are consecutive lanes (HP is a power of two <= 32)
+#pragma unroll
+                                for (int dlt = HP >> 1; dlt > 0; dlt >>= 1)
+                                    gterm += __shfl_down_sync(0xffffffffu, gterm, dlt, HP);
+                                // pure store (no load in the pipeline's critical path): this batch's
+                                // gradient goes to a scratch array, k_add_f32 accumulates it afterwards
+                                if (cp == 0 && valid[j]) p.g[cell] = p.lam2 * gterm;
+                            }
+                            continue;
+                        }
                         float4 rr;
                         {
                             const float wm = w2[0] * m_cur[j];
@@ -500,6 +552,7 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
     if (s_ticket == gridDim.x - 1) {
         __threadfence();
         double* sh = reinterpret_cast<double*>(smem);           // stages are idle now
+        if (MODE != MODE_G)
         switch (p.phase) {
             case PH_INIT_A: finalize_phase<PH_INIT_A>(p.fin, sh); break;
             case PH_F:      finalize_phase<PH_F>(p.fin, sh); break;
