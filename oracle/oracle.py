@@ -85,8 +85,8 @@ def _L():
         lib.ref_apply_SH.argtypes = [C.POINTER(_RefOp), P, C.c_double, C.c_int32, P, I64, P, P, P, P]
         lib.ref_lsqr_sf_step.argtypes = [C.POINTER(_RefOp), P, C.c_double, C.c_int32, P, I64,
                                          C.POINTER(_RefStateSF)]
-        lib.ref_lsqr_sf.argtypes = [C.POINTER(_RefOp), P, C.c_double, C.c_int32, P, I64, P,
-                                    C.c_double, C.c_int32, P, P, P, P]
+        lib.ref_lsqr_sf.argtypes = [C.POINTER(_RefOp), P, C.c_double, C.c_int32, P, I64, P, P,
+                                    C.c_double, C.c_double, C.c_int32, P, P, P, P]
         lib.ref_lsqr_sf.restype = C.c_int32
         lib.ref_objective_gradient.argtypes = [C.POINTER(_RefOp), P, C.c_double, C.c_int32, P, I64,
                                                P, P, P, P, P, P, P]
@@ -285,18 +285,37 @@ def apply_SH(op: Operator, m, lam: float, rec: np.ndarray, src: int, ytop, ybot)
 
 
 def lsqr_sf(op: Operator, m, lam: float, rec: np.ndarray, src: int, d, tol: float = 0.0,
-            maxit: int = 50) -> dict:
-    """One column of LSQR on min ||S [u; alpha] - [0; d]||, x0 = 0."""
+            maxit: int = 50, q=None, ar_ref: float = 0.0) -> dict:
+    """One column of LSQR on min ||S [u; alpha] - [lam q; d]||, x0 = 0 (q = None: the paper's
+    b = [0; d]).  ar_ref > 0 replaces alpha1*beta1 as the reference of the stop rule."""
     m = _f64(m, op.ng)
     rec = np.ascontiguousarray(rec, dtype=np.int64)
     d = _drec(d, rec)
+    qq = _c128(q, op.ng) if q is not None else None
     x = np.empty(op.ng, dtype=np.complex128)
     xa = np.zeros(1, dtype=np.complex128)
     res = np.empty(maxit + 1, dtype=np.float64)
     ar = np.empty(maxit + 1, dtype=np.float64)
     it = _L().ref_lsqr_sf(C.byref(op._c()), _ptr(m), float(lam), rec.size, _ptr(rec), int(src),
-                          _ptr(d), float(tol), int(maxit), _ptr(x), _ptr(xa), _ptr(res), _ptr(ar))
+                          _ptr(qq) if qq is not None else None, _ptr(d), float(tol), float(ar_ref),
+                          int(maxit), _ptr(x), _ptr(xa), _ptr(res), _ptr(ar))
     return {"x": x, "alpha_src": complex(xa[0]), "resnorms": res, "arnorms": ar, "iters": int(it)}
+
+
+def lsqr_sf_warm(op: Operator, m, lam: float, rec: np.ndarray, src: int, d, x0, a0, tol: float = 0.0,
+                 maxit: int = 50, q=None, ar_ref: float = 0.0) -> dict:
+    """Warm start (Algorithm 1 leaves x0 free), written out as its definition:
+    r0 = b - S [x0; a0];  [dx; da] = LSQR on S with right-hand side r0 from zero;  x = x0 + dx.
+    resnorms[k] is then ||b - S x_k|| of the ORIGINAL system."""
+    x0 = _c128(x0, op.ng)
+    t, bb = apply_S(op, m, lam, rec, src, x0, a0)
+    b_top = (lam * _c128(q, op.ng) if q is not None else np.zeros(op.ng, dtype=np.complex128))
+    r_top = b_top - t
+    r_bot = _drec(d, np.ascontiguousarray(rec, dtype=np.int64))[:np.size(rec)] - bb
+    out = lsqr_sf(op, m, lam, rec, src, r_bot, tol=tol, maxit=maxit, q=r_top / lam, ar_ref=ar_ref)
+    out["x"] = x0 + out["x"]
+    out["alpha_src"] = complex(a0) + out["alpha_src"]
+    return out
 
 
 def lsqr_sf_step(op: Operator, m, lam: float, rec: np.ndarray, src: int, state: dict) -> dict:

@@ -472,12 +472,15 @@ void ref_lsqr_sf_step(const ref_op *op, const double *m, double lambda, int32_t 
     free(gamma); free(tmp_top); free(tmp_bot);
 }
 
-/* LSQR on  min_x || S x - b ||,  b = [0 ; d],  x0 = 0.
- * Same stop rule, histories and hold-last convention as ref_lsqr.  x_u [n_g] and
- * x_a [1] receive the wavefield and the source-weight estimate.  Returns the
- * number of iterations performed. */
+/* LSQR on  min_x || S x - b ||,  b = [lambda q ; d]  (the paper's b = [0 ; d] is q = NULL),
+ * x0 = 0.  Same histories and hold-last convention as ref_lsqr.
+ * Stop rule: arnorm_k <= tol * ar_ref, with ar_ref = alpha1*beta1 of THIS system when the
+ * argument is <= 0 (reading C-6), else the caller's reference (warm starts, reading C-17:
+ * the tolerance stays relative to the cold problem's ||S^H b||).  x_u [n_g] and x_a [1]
+ * receive the wavefield and the source-weight estimate.  Returns the iterations performed. */
 int32_t ref_lsqr_sf(const ref_op *op, const double *m, double lambda, int32_t n_rec,
-                    const int64_t *rec, int64_t src, const zc *d, double tol, int32_t maxit,
+                    const int64_t *rec, int64_t src, const zc *q, const zc *d, double tol,
+                    double ar_ref, int32_t maxit,
                     zc *x_u, zc *x_a, double *resnorms, double *arnorms) {
     size_t ng = (size_t)op->nx * op->ny * op->nz;
     double *gamma = (double *)malloc(ng * sizeof(double));
@@ -493,7 +496,7 @@ int32_t ref_lsqr_sf(const ref_op *op, const double *m, double lambda, int32_t n_
     ref_gamma(op, gamma);
     int32_t iters = 0;
 
-    for (size_t i = 0; i < ng; ++i) { st.u_top[i] = 0.0; x_u[i] = 0.0; }     /* b_top = 0 */
+    for (size_t i = 0; i < ng; ++i) { st.u_top[i] = q ? lambda * q[i] : 0.0; x_u[i] = 0.0; }
     for (int32_t r = 0; r < n_rec; ++r) st.u_bot[r] = d[r];
     double beta = norm2(st.u_top, ng, st.u_bot, (size_t)n_rec);
     double ar0 = 0.0, last_r = beta, last_ar = 0.0;
@@ -501,13 +504,14 @@ int32_t ref_lsqr_sf(const ref_op *op, const double *m, double lambda, int32_t n_
     if (arnorms) arnorms[0] = 0.0;
 
     if (beta > 0.0) {
+        for (size_t i = 0; i < ng; ++i) st.u_top[i] /= beta;
         for (int32_t r = 0; r < n_rec; ++r) st.u_bot[r] /= beta;
         apply_SH_g(op, m, gamma, lambda, n_rec, rec, src, st.u_top, st.u_bot, st.v, &st.v_a);
         double nv = norm2(st.v, ng, NULL, 0);
         double alpha = sqrt(nv * nv + abs2(st.v_a));
-        ar0 = alpha * beta;
-        last_ar = ar0;
-        if (arnorms) arnorms[0] = ar0;
+        last_ar = alpha * beta;
+        if (arnorms) arnorms[0] = last_ar;
+        ar0 = ar_ref > 0.0 ? ar_ref : alpha * beta;
         if (alpha > 0.0) {
             for (size_t i = 0; i < ng; ++i) { st.v[i] /= alpha; st.w[i] = st.v[i]; }
             st.v_a /= alpha; st.w_a = st.v_a;

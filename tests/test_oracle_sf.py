@@ -278,3 +278,44 @@ def test_gradient_of_the_reduced_objective_by_variable_projection():
     eps = 1e-4
     fd = (f4(m + eps * dm)[0] - f4(m - eps * dm)[0]) / (2 * eps)
     assert fd == pytest.approx(float(g @ dm), rel=1e-5)
+
+
+# ---------------------------------------------------------------- known part of the source, warm start
+def test_sf_with_a_known_source_part_and_warm_start(tiny):
+    """b = [lam q; d] with the weight still unknown, and x0 != 0 (Algorithm 1 leaves x0 free):
+    both must land on LAPACK's minimiser; a warm start from zero is the cold start; a warm start
+    at the minimiser has nothing left to do once the stop rule refers to the cold ||S^H b||."""
+    op, m, rec, src, lam, d, S = tiny
+    rng = _rng(46)
+    q = _cn(rng, op.ng) * 1e-3
+    b = np.concatenate([lam * q, d])
+    x_ls = np.linalg.lstsq(S, b, rcond=None)[0]
+    cold = O.lsqr_sf(op, m, lam, rec, src, d, tol=0.0, maxit=700, q=q)
+    x = np.concatenate([cold["x"], [cold["alpha_src"]]])
+    assert np.linalg.norm(x - x_ls) < 1e-9 * np.linalg.norm(x_ls)
+    assert cold["resnorms"][0] == pytest.approx(np.linalg.norm(b), rel=1e-14)
+    # warm start from zero = cold start (up to the rounding of (lam q) / lam * lam)
+    w0 = O.lsqr_sf_warm(op, m, lam, rec, src, d, np.zeros(op.ng), 0.0, maxit=5, q=q)
+    c0 = O.lsqr_sf(op, m, lam, rec, src, d, maxit=5, q=q)
+    assert np.linalg.norm(w0["x"] - c0["x"]) < 1e-10 * np.linalg.norm(c0["x"])
+    assert np.allclose(w0["resnorms"], c0["resnorms"], rtol=1e-12)
+    # warm start from a random point converges to the same minimiser; resnorms[0] = ||b - S x0||
+    x0, a0 = _cn(rng, op.ng), complex(_cn(rng, 1)[0])
+    warm = O.lsqr_sf_warm(op, m, lam, rec, src, d, x0, a0, maxit=700, q=q)
+    xw = np.concatenate([warm["x"], [warm["alpha_src"]]])
+    assert np.linalg.norm(xw - x_ls) < 1e-9 * np.linalg.norm(x_ls)
+    assert warm["resnorms"][0] == pytest.approx(np.linalg.norm(b - S @ np.concatenate([x0, [a0]])), rel=1e-12)
+    # from a partly converged iterate, with the cold reference: fewer iterations than the cold solve
+    tol = 1e-6
+    full = O.lsqr_sf(op, m, lam, rec, src, d, tol=tol, maxit=700, q=q)
+    part = O.lsqr_sf(op, m, lam, rec, src, d, tol=1e-3, maxit=700, q=q)
+    ar_cold = full["arnorms"][0]
+    cont = O.lsqr_sf_warm(op, m, lam, rec, src, d, part["x"], part["alpha_src"], tol=tol, maxit=700, q=q,
+                          ar_ref=ar_cold)
+    assert 0 < cont["iters"] < full["iters"]
+    r = b - S @ np.concatenate([cont["x"], [cont["alpha_src"]]])
+    assert np.linalg.norm(S.conj().T @ r) <= 1.01 * tol * ar_cold
+    # at the minimiser nothing is left: the first look at the rule stops it
+    done = O.lsqr_sf_warm(op, m, lam, rec, src, d, x_ls[:-1], x_ls[-1], tol=tol, maxit=50, q=q, ar_ref=ar_cold)
+    assert done["iters"] <= 1
+    assert np.linalg.norm(done["x"] - x_ls[:-1]) < 1e-9 * np.linalg.norm(x_ls)
