@@ -168,6 +168,25 @@ int wri_objective_gradient(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_ho
                            const void* u_dev, const void* d_dev, float lambda,
                            double* f_pde_dev, double* f_data_dev, float* g_dev);
 
+/* Options of the solves that follow (all wri_lsqr_* / wri_lsqr_sf_* begin and batch entries);
+ * sticky until set again, NULL restores the defaults (all zero).
+ *   warm_start   1: u_out_dev (and alpha_out_dev) hold x0 (alpha0) on entry.  Algorithm 1 leaves
+ *                x0 free; the solve runs LSQR on the residual system
+ *                r0 = b - S x0 and accumulates into x0, so x_k = x0 + dx_k and resnorms[k] =
+ *                ||b - S x_k|| of the original system.  Used to re-solve after a model update
+ *                or with a tighter tolerance (Algorithm 2).
+ *   ar_ref_dev   double [nb] or NULL: reference of the stop rule, ||S^H r_k|| <= tol * ar_ref
+ *                (default: this solve's own alpha1*beta1 = ||S^H r0||).  A warm start passes the
+ *                cold solve's value so that tol keeps its meaning (reading C-17).
+ *   ar0_out_dev  double [nb] or NULL: receives alpha1*beta1 of the solve.
+ * The device arrays must stay valid while a solve is in flight.                                  */
+typedef struct {
+    int32_t       warm_start;
+    const double* ar_ref_dev;
+    double*       ar0_out_dev;
+} wri_lsqr_opts;
+int wri_lsqr_set_opts(wri_ctx* ctx, const wri_lsqr_opts* opts);
+
 /* Same solve with HOST buffers: copies q, d (and tol) to the device, solves, copies u_out,
  * resnorms and iters back, then synchronises the stream.  Needs a workspace sized with
  * host_staging = 1.  Pinned host memory makes the copies asynchronous but is not required.   */

@@ -24,6 +24,10 @@ class wri_sponge(C.Structure):
                 ("faces", C.c_uint32)]
 
 
+class wri_lsqr_opts(C.Structure):
+    _fields_ = [("warm_start", C.c_int32), ("ar_ref_dev", C.c_void_p), ("ar0_out_dev", C.c_void_p)]
+
+
 class wri_lsqr_view(C.Structure):
     _fields_ = [("nb", C.c_int32), ("k", C.c_int32),
                 ("U_top", C.c_void_p), ("U_bot", C.c_void_p), ("V", C.c_void_p),
@@ -81,6 +85,7 @@ def load_library():
     lib.wri_lsqr_sf_begin.argtypes = solve_sf
     lib.wri_lsqr_sf_batch_host.argtypes = solve_sf
     lib.wri_objective_gradient.argtypes = [P, I32, P, P, P, P, P, P, F32, P, P, P]
+    lib.wri_lsqr_set_opts.argtypes = [P, C.POINTER(wri_lsqr_opts)]
     lib.wri_lsqr_iterate.argtypes = [P, I32]
     lib.wri_lsqr_end.argtypes = [P]
     lib.wri_lsqr_peek.argtypes = [P, C.POINTER(wri_lsqr_view)]
@@ -265,13 +270,25 @@ class Wri:
                                      int(maxit), _dptr(u), _dptr(res), _dptr(it)))
         return u, res, it
 
+    def set_opts(self, warm_start=False, ar_ref=None, ar0_out=None):
+        """Options of the solves that follow: warm start from the contents of the output buffers,
+        reference of the stop rule (float64 [nb] CUDA tensor), receiver of alpha1*beta1."""
+        self._opt_keep = (ar_ref, ar0_out)
+        o = wri_lsqr_opts(int(bool(warm_start)), _dptr(ar_ref), _dptr(ar0_out))
+        _ck(self._lib.wri_lsqr_set_opts(self._h, C.byref(o)))
+
     # ---- source-free system (unknown source weight per column)
-    def lsqr_sf_batch(self, d, lam, src_ijk, tol=None, maxit=50, omega_idx=None, q=None):
+    def lsqr_sf_batch(self, d, lam, src_ijk, tol=None, maxit=50, omega_idx=None, q=None, out=None):
+        """out = (u, alpha, resnorms, iters) to reuse buffers; with set_opts(warm_start=True) u and
+        alpha hold the start point on entry."""
         t = self._torch
         nb = d.shape[1]
         self.ensure_workspace(nb, compaction=tol is not None)
-        u, res, it = self._outputs(nb, maxit, d.device)
-        a = t.empty(nb, dtype=t.complex64, device=d.device)
+        if out is not None:
+            u, a, res, it = out
+        else:
+            u, res, it = self._outputs(nb, maxit, d.device)
+            a = t.empty(nb, dtype=t.complex64, device=d.device)
         keep, oi = _i32(omega_idx)
         keep2, si = _i32(src_ijk)
         _ck(self._lib.wri_lsqr_sf_batch(self._h, nb, oi, si, _dptr(q), _dptr(d), float(lam), _dptr(tol),

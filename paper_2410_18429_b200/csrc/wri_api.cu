@@ -71,6 +71,7 @@ struct wri_ctx {
     int* src = nullptr;          // [nb_max] source cell per caller's column (source-free system)
     bool sf = false;             // the solve in flight has the extra source-weight unknown
     float2* alpha_out = nullptr; // caller's [nb] source-weight estimates (source-free system)
+    wri_lsqr_opts opts{};        // warm start / stop-rule reference for the next solves (wri_lsqr_set_opts)
     int* colmap = nullptr;       // [nb_max] working column -> caller's column (-1 = padding)
     int* idx = nullptr;          // [3][nb_max] scratch: gather map | retire source | retire destination
     int* h_active = nullptr;     // pinned host copy of the active flags
@@ -204,7 +205,7 @@ WsLayout ws_layout(const wri_ctx* c, int nb, int flags, int maxit_cap) {
 constexpr int kHostMaxitCap = 4096;   // resnorm staging rows reserved for wri_lsqr_batch_host
 
 int upload_columns(wri_ctx* c, int nb, const int32_t* omega_idx, float lambda) {
-    std::vector<float> w2(nb), one(nb, 1.f), lam(nb, lambda);
+    std::vector<float> w2(nb), one(nb, 1.f), lam(nb, lambda), nlam(nb, -lambda), mone(nb, -1.f);
     for (int s = 0; s < nb; ++s) {
         const int j = omega_idx ? omega_idx[s] : 0;
         if (j < 0 || j >= (int)c->omega.size()) return WRI_ERR_ARG;
@@ -214,6 +215,8 @@ int upload_columns(wri_ctx* c, int nb, const int32_t* omega_idx, float lambda) {
     CK(cudaMemcpyAsync(c->coef + C_W2 * NM, w2.data(), nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));
     CK(cudaMemcpyAsync(c->coef + C_ONE * NM, one.data(), nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));
     CK(cudaMemcpyAsync(c->coef + C_LAM * NM, lam.data(), nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(c->coef + C_NLAM * NM, nlam.data(), nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(c->coef + C_MONE * NM, mone.data(), nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));
     return WRI_OK;
 }
 
@@ -535,6 +538,10 @@ ScalParams scal_params(const wri_ctx* c, const double* partials, int n_rows, con
     s.src = c->sf ? c->src : nullptr;
     s.U = c->U;
     s.alpha_out = c->sf ? c->alpha_out : nullptr;
+    s.warm = c->opts.warm_start;
+    s.X = c->X;
+    s.ar_ref = c->opts.ar_ref_dev;
+    s.ar0_out = c->opts.ar0_out_dev;
     return s;
 }
 
@@ -795,6 +802,13 @@ int wri_set_workspace(wri_ctx* c, void* ws_dev, size_t bytes) {
     return WRI_OK;
 }
 
+int wri_lsqr_set_opts(wri_ctx* c, const wri_lsqr_opts* opts) {
+    if (!c) return WRI_ERR_ARG;
+    if (c->solving) return WRI_ERR_STATE;
+    c->opts = opts ? *opts : wri_lsqr_opts{};
+    return WRI_OK;
+}
+
 int64_t wri_launch_count(const wri_ctx* c) { return c ? c->launches : 0; }
 
 int wri_profile_enable(wri_ctx* c, int32_t on) {
@@ -1027,7 +1041,15 @@ int lsqr_begin_impl(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const
         CK(cudaMemsetAsync(c->U, 0, vbytes, c->stream));
         CK(cudaMemsetAsync(c->partials, 0, c->tl.n_tiles * nb * sizeof(double), c->stream));
     }
-    CK(cudaMemsetAsync(c->X, 0, vbytes, c->stream));
+    if (c->opts.warm_start) {
+        // warm start: u_out holds x0; top rows of r0 = b - S x0:  U <- U - lambda A x0  (and its ||.||^2)
+        PassParams r = p;
+        r.in = c->X; r.out = c->U; r.sgn = 1.f;
+        r.ca = c->coef + C_NLAM * NM; r.cb = c->coef + C_MONE * NM;
+        if ((rc = launch_pass<MODE_A>(c, r, c->tl))) return rc;
+    } else {
+        CK(cudaMemsetAsync(c->X, 0, vbytes, c->stream));
+    }
     CK(cudaMemsetAsync(c->W, 0, vbytes, c->stream));
     CK(cudaMemsetAsync(c->V, 0, vbytes, c->stream));
     if ((rc = launch_scalars<PH_INIT_B>(c, (const float2*)d_dev))) return rc;
@@ -1262,6 +1284,10 @@ int lsqr_batch_host_impl(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, 
     // q is staged in the V slot: the start consumes q before it clears V
     float2* Qs = q_host ? (float2*)(c->ws + L.V) : nullptr;
     float2* As = (float2*)(c->ws + L.alphas);
+    if (c->opts.warm_start) {                 // x0 (alpha0) arrive in the output buffers
+        CK(cudaMemcpyAsync(Xs, u_out_host, vbytes, cudaMemcpyHostToDevice, c->stream));
+        if (sf) CK(cudaMemcpyAsync(As, alpha_out_host, nb * sizeof(float2), cudaMemcpyHostToDevice, c->stream));
+    }
     if (Qs) CK(cudaMemcpyAsync(Qs, q_host, vbytes, cudaMemcpyHostToDevice, c->stream));
     if (dbytes) CK(cudaMemcpyAsync(Ds, d_host, dbytes, cudaMemcpyHostToDevice, c->stream));
     if (tol_host) CK(cudaMemcpyAsync(tols, tol_host, nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));

@@ -21,7 +21,7 @@ namespace wri {
 enum PassMode { MODE_APPLY = 0, MODE_A = 1, MODE_F = 2, MODE_INIT = 3, MODE_G = 4 };
 
 // per-column float coefficients, one row of nb_max each
-enum Coef { C_CA_F = 0, C_CB_F, C_CV_F, C_CX, C_CW, C_CA_A, C_CB_A, C_CT_A, C_W2, C_ONE, C_LAM, N_COEF };
+enum Coef { C_CA_F = 0, C_CB_F, C_CV_F, C_CX, C_CW, C_CA_A, C_CB_A, C_CT_A, C_W2, C_ONE, C_LAM, C_NLAM, C_MONE, N_COEF };
 // per-column double state, one row of nb_max each
 // (S_VA.. S_XA: the source-weight entries of V, W, X in the source-free system, re/im pairs;
 //  V's entry is stored un-normalised like V itself)
@@ -303,6 +303,11 @@ struct ScalParams {
     const int* src;           // [nb_out] source cell of the CALLER's column, or null (known-source system)
     float2* U;                // [n_g][nb] top rows of u (its source-node entry takes the -lambda e column)
     float2* alpha_out;        // [nb_out] source-weight estimate of x_k, c64
+    // warm start (x0 in X / alpha_out on entry) and the reference of the stop rule
+    int warm;
+    const float2* X;          // [n_g][nb] x0 (PH_INIT_B: receiver rows of the residual)
+    const double* ar_ref;     // [nb] or null: arnorm_k <= tol * ar_ref instead of tol * alpha1 beta1
+    double* ar0_out;          // [nb] or null: alpha1 beta1 of this solve
 };
 
 // sum over tiles of partials[.][s] in fixed order; result for column s in colsum[s] (shared)
@@ -374,7 +379,16 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
     const long long nrs = (long long)p.n_rec * nb;
     if (PHASE == PH_INIT_B) {
         // U_bot = d (exact copy), then beta1 = ||[lambda q ; d]||
-        for (long long i = threadIdx.x; i < nrs; i += blockDim.x) p.U_bot[i] = p.d[i];
+        if (!p.warm) {
+            for (long long i = threadIdx.x; i < nrs; i += blockDim.x) p.U_bot[i] = p.d[i];
+        } else {
+            // warm start: bottom rows of r0 = b - S x0, i.e. d - x0 at the receiver nodes
+            for (long long i = threadIdx.x; i < nrs; i += blockDim.x) {
+                const int r = (int)(i / nb), s = (int)(i - (long long)r * nb);
+                const float2 dv = p.d[i], xv = p.X[(size_t)p.rec[r] * nb + s];
+                p.U_bot[i] = make_float2(dv.x - xv.x, dv.y - xv.y);
+            }
+        }
         __syncthreads();
     }
     if (PHASE == PH_F && !p.rows_in_pass) {
@@ -415,10 +429,23 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
                 cs += va_re * va_re + va_im * va_im;
             }
         }
-        const double nrm = sqrt(fmax(cs, 0.0));
         if (PHASE == PH_INIT_B) {
             for (int r = S_VA_RE; r <= S_XA_IM; ++r) st[r * NM + s] = 0.0;
-            if (p.alpha_out) p.alpha_out[s] = make_float2(0.f, 0.f);
+            if (p.alpha_out && !p.warm) p.alpha_out[s] = make_float2(0.f, 0.f);
+            if (p.warm && sc >= 0) {
+                // r0_top = lam q - lam (A x0 - a0 e): the pass before left lam q - lam A x0 in U
+                const float2 a0 = p.alpha_out[s];
+                st[S_XA_RE * NM + s] = (double)a0.x; st[S_XA_IM * NM + s] = (double)a0.y;
+                float2* up = p.U + (size_t)sc * nb + s;
+                const float2 o = __ldcg(up);
+                const float2 n = make_float2((float)((double)o.x + (double)p.lambda * a0.x),
+                                             (float)((double)o.y + (double)p.lambda * a0.y));
+                *up = n;
+                cs += ((double)n.x * n.x + (double)n.y * n.y) - ((double)o.x * o.x + (double)o.y * o.y);
+            }
+        }
+        const double nrm = sqrt(fmax(cs, 0.0));
+        if (PHASE == PH_INIT_B) {
             // beta1 u1 = b.  b = 0 => x = 0, nothing to iterate (reading C-7).
             const double beta = nrm;
             st[S_BETA * NM + s] = beta;
@@ -443,7 +470,8 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
             int act = p.active[s];
             st[S_ALPHA * NM + s] = alpha;
             st[S_RHOBAR * NM + s] = alpha;
-            st[S_AR0 * NM + s] = alpha * beta;
+            st[S_AR0 * NM + s] = (p.ar_ref && p.ar_ref[s] > 0.0) ? p.ar_ref[s] : alpha * beta;
+            if (p.ar0_out) p.ar0_out[s] = alpha * beta;
             if (act && !(alpha > 0.0)) { act = 0; p.active[s] = 0; }
             cf[C_CA_F * NM + s] = act ? (float)((double)p.lambda / alpha) : 0.f;
             cf[C_CV_F * NM + s] = act ? (float)(1.0 / alpha) : 0.f;

@@ -272,3 +272,69 @@ def test_sf_known_part_of_the_source_and_bad_source_node(torch_cuda):
     with pytest.raises(WriError) as e:
         ctx.lsqr_sf_batch(d, w.lam, bad, None, maxit=2, omega_idx=w.omega_idx)
     assert e.value.code == WRI_ERR_ARG
+
+
+@pytest.mark.parametrize("name,kw", [
+    ("config1", dict(grid=(32, 32, 32), nb=16)),       # TMA path
+    ("config2", dict(grid=(20, 33, 18), nb=3)),        # generic path
+])
+def test_sf_warm_start_and_stop_rule_reference(torch_cuda, name, kw):
+    """Warm start (wri_lsqr_set_opts): the start of the residual system (r0 = b - S x0, teacher-forced
+    against the oracle's operator), x_k = x0 + dx_k against the oracle's warm start for k <= 3, the
+    history is ||b - S x_k|| of the original system, and continuing a loose solve to a tight
+    tolerance with the cold reference needs fewer iterations than the cold tight solve."""
+    torch = torch_cuda
+    w = workloads.make(name, **kw)
+    ctx = _wri(w)
+    rec, src = O.rec_cells(w.nx, w.ny, w.nz, w.rec_ijk), _src_cells(w)
+    ops = ops_for(w)
+    rng = np.random.Generator(np.random.PCG64(29))
+    d, q = torch.from_numpy(w.D).cuda(), torch.from_numpy(w.Q).cuda()
+    x0 = (_cn(rng, (w.ng, w.nb)) * np.float32(1e-2)).astype(np.complex64)
+    a0 = (_cn(rng, (w.nb,)) * np.float32(1e-2)).astype(np.complex64)
+    K = 3
+    ctx.set_opts(warm_start=True)
+    out = (torch.from_numpy(x0).cuda(), torch.from_numpy(a0).cuda(),
+           torch.empty((K + 1, w.nb), dtype=torch.float32, device="cuda"),
+           torch.empty(w.nb, dtype=torch.int32, device="cuda"))
+    u, a, res, it = ctx.lsqr_sf_batch(d, w.lam, w.src_ijk, None, maxit=K, omega_idx=w.omega_idx, q=q, out=out)
+    torch.cuda.synchronize()
+    u, a, res = u.cpu().numpy(), a.cpu().numpy(), res.cpu().numpy()
+    for s in sorted(set([0, w.nb // 2, w.nb - 1])):
+        ref = O.lsqr_sf_warm(ops[s], w.m, w.lam, rec, src[s], w.D[:, s], x0[:, s], a0[s], maxit=K, q=w.Q[:, s])
+        assert rel(res[:, s], ref["resnorms"]) < 1e-3
+        assert rel(u[:, s], ref["x"]) < 1e-3
+        assert abs(a[s] - ref["alpha_src"]) < 1e-3 * math.sqrt(np.linalg.norm(ref["x"]) ** 2 + abs(ref["alpha_src"]) ** 2)
+        # resnorms[0] is the residual of the ORIGINAL system at x0
+        t, b = O.apply_S(ops[s], w.m, w.lam, rec, src[s], x0[:, s], a0[s])
+        r0 = math.sqrt(np.linalg.norm(w.lam * w.Q[:, s].astype(complex) - t) ** 2
+                       + np.linalg.norm(w.D[:, s].astype(complex) - b) ** 2)
+        assert res[0, s] == pytest.approx(r0, rel=1e-5)
+
+    # loose solve, then continue to a tight tolerance with the cold reference
+    ctx.set_opts(ar0_out=torch.zeros(w.nb, dtype=torch.float64, device="cuda"))
+    ar0 = ctx._opt_keep[1]
+    maxit = 150
+    loose = torch.full((w.nb,), 3e-2, dtype=torch.float32, device="cuda")
+    tight = torch.full((w.nb,), 3e-3, dtype=torch.float32, device="cuda")
+    ul, al, resl, itl = ctx.lsqr_sf_batch(d, w.lam, w.src_ijk, loose, maxit=maxit, omega_idx=w.omega_idx)
+    torch.cuda.synchronize()
+    ar_cold = ar0.clone()
+    assert (ar_cold > 0).all()
+    ctx.set_opts()
+    ut, at, rest, itt = ctx.lsqr_sf_batch(d, w.lam, w.src_ijk, tight, maxit=maxit, omega_idx=w.omega_idx)
+    ctx.set_opts(warm_start=True, ar_ref=ar_cold)
+    out = (ul.clone(), al.clone(), torch.empty_like(resl), torch.empty_like(itl))
+    uc, ac, resc, itc = ctx.lsqr_sf_batch(d, w.lam, w.src_ijk, tight, maxit=maxit, omega_idx=w.omega_idx, out=out)
+    torch.cuda.synchronize()
+    ctx.set_opts()
+    itl, itt, itc = itl.cpu().numpy(), itt.cpu().numpy(), itc.cpu().numpy()
+    assert (itl < itt).all() and (itt < maxit).all()
+    assert (itc < itt).all(), (itl, itt, itc)
+    # the continued solution satisfies the tight rule (oracle arithmetic) and starts where the loose one ended
+    uc, ac, resc = uc.cpu().numpy(), ac.cpu().numpy(), resc.cpu().numpy()
+    for s in (0, w.nb - 1):
+        r_true, ar_true = _true_residuals(w, ops[s], rec, src[s], s, uc[:, s], ac[s])
+        assert ar_true <= 1.5 * 3e-3 * float(ar_cold[s])
+        assert resc[0, s] == pytest.approx(float(resl[itl[s], s]), rel=1e-4)
+        assert abs(resc[itc[s], s] / r_true - 1.0) < 1e-3
