@@ -303,7 +303,18 @@ def run_ours(args, wl_name, w):
                                         "achieved": bytes_g / (ms_g * 1e-3) / 1e9, "unit": "GB/s",
                                         "frac": bytes_g / (ms_g * 1e-3) / 1e9 / peak_g,
                                         "kernel": "k_grad + k_objective (eq. 9 fused with the stencil residual)"}
-        del u_sf, g
+        # one misfit evaluation (Algorithm 2 lines 4-5; the unit the paper times in Table 1):
+        # source-free solve of every column to a tolerance + objective + gradient, one C-ABI call
+        eps_m = 1e-2
+        ctx.misfit_sf(d, w.lam, w.src_ijk, eps_m, maxit, omega_idx=w.omega_idx, g=g)           # warm-up
+        t0 = time.perf_counter()
+        mf = ctx.misfit_sf(d, w.lam, w.src_ijk, eps_m, maxit, omega_idx=w.omega_idx, g=g)       # synchronises (f)
+        s_m = time.perf_counter() - t0
+        it_m = int(mf["iters"].sum().item())
+        extras["misfit_evaluation"] = {"ms": s_m * 1e3, "eps": eps_m, "lsqr_iterations_x_sources": it_m,
+                                       "value": it_m / s_m, "unit": UNIT, "f": mf["f"],
+                                       "timing": "host wall clock around wri_misfit_sf (it ends with a stream sync)"}
+        del u_sf, g, mf
 
     (ms, e2e_s), (iters_all, iters_e2e_all, launches_all) = reduce_over_ranks(
         [ms, e2e_s], [iters_per_step, iters_e2e, launches], dist if use_dist else None, dev)

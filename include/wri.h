@@ -105,7 +105,7 @@ int wri_apply_MH(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_host, float 
  *                tol_s <= 0 (or NULL) runs exactly maxit iterations
  *   u_out_dev    c64 [n_g][nb]     the wavefields x_k at each column's stop iteration
  *   resnorms_dev float [maxit+1][nb]: ||b - M x_k|| for k = 0..maxit, held at the last value
- *                after a column stops (reading C-9)
+ *                after a column stops (reading C-9); may be NULL (no history wanted)
  *   iters_dev    int32 [nb] iterations performed per column (may be NULL)
  * Equivalent to wri_lsqr_begin + wri_lsqr_iterate(maxit) + wri_lsqr_end.  Needs a workspace.
  * With tol_dev == NULL the call only enqueues work.  With tolerances the host reads the
@@ -186,6 +186,69 @@ typedef struct {
     double*       ar0_out_dev;
 } wri_lsqr_opts;
 int wri_lsqr_set_opts(wri_ctx* ctx, const wri_lsqr_opts* opts);
+
+/* ---- Misfit evaluation and the adaptive outer step (Algorithm 2) -------------
+ *
+ * wri_misfit_sf — one misfit evaluation of the source-free problem for a group of nb columns
+ * ("a single misfit function calculation", the unit of the paper's Table 1):
+ *     x_bar_s = argmin || S_s x - [0; d_s] ||   by LSQR, every column to the tolerance eps (eq. 7)
+ *     f_pde[s], f_data[s], g += ...             as wri_objective_gradient at (u_bar, alpha_bar) (eq. 8-9)
+ *   eps        LSQR tolerance of every column (0: exactly maxit iterations)
+ *   warm       1: u_dev / alpha_dev hold a start point and ar0_dev the cold solve's alpha1*beta1
+ *              (the stop rule stays relative to it, reading C-17); 0: cold solve, ar0_dev (may be
+ *              NULL) receives alpha1*beta1
+ *   u_dev      c64 [n_g][nb], alpha_dev c64 [nb]: the minimisers on return
+ *   g_dev      float [n_g], ACCUMULATED (clear it first), or NULL for the objective alone
+ *   iters_dev  int32 [nb] or NULL
+ *   f_host     HOST double or NULL: sum_s (f_pde + f_data), summed in column order; asking for it
+ *              synchronises the stream
+ * Needs a workspace (with WRI_WS_COMPACTION room converged columns are compacted away).
+ *
+ * wri_awri_step — lines 4-14 of Algorithm 2 for one group of columns and the model in m_dev:
+ *     4-5  x_bar, f, g at m with tolerance eps            7-8  x_tilde, f_tilde at m_tilde
+ *     6    m_tilde = update(m, g)                          9-11 f_tilde > f: eps <- eps/2, back to 4
+ *                                                          13   else m <- m_tilde
+ * The quasi-Newton direction of line 6 is the caller's (l-BFGS is outside this library):
+ * opts->update(user, m_dev, g_dev, m_trial_dev, cuda_stream) must ENQUEUE the computation of
+ * m_trial on the given stream and return 0; with update == NULL the built-in steepest-descent
+ * update m_tilde = clamp(m - step * g, m_min, m_max) is used.  Algorithm 2 does not bound the
+ * "go back" loop: after max_halvings halvings the step is reported as rejected and m_dev is left
+ * unchanged (reading C-20).  warm_restart = 1 continues the re-solve of line 4 from x_bar.
+ * The comparison of line 9 is made on the host in double (one stream synchronisation per
+ * evaluation).  During the call the context's model pointer is switched between m_dev and
+ * m_trial_dev and restored on return.
+ *   m_dev        float [n_g]: m^(k) on entry, m^(k+1) on return if accepted
+ *   m_trial_dev  float [n_g] scratch (the last trial model on return)
+ *   g_dev        float [n_g]: gradient at m^(k) with the final eps (overwritten)
+ *   u_dev, alpha_dev / u_trial_dev, alpha_trial_dev   wavefields and source weights at m^(k) / m_tilde
+ *   f_cols_dev   double [2][nb]: f_pde | f_data per column at m^(k)
+ *   report       HOST                                                                          */
+#define WRI_AWRI_MAX_TRACE 16
+typedef int (*wri_update_fn)(void* user, const float* m_dev, const float* g_dev, float* m_trial_dev,
+                             void* cuda_stream);
+typedef struct {
+    int32_t       max_halvings;     /* < WRI_AWRI_MAX_TRACE                                      */
+    int32_t       warm_restart;
+    wri_update_fn update;           /* NULL: built-in steepest descent with the fields below     */
+    void*         user;
+    float         step, m_min, m_max;
+} wri_awri_opts;
+typedef struct {
+    int32_t accepted, n_halvings, n_trace;
+    float   eps;                    /* tolerance in force at the end                              */
+    double  f, f_trial;             /* of the last round                                          */
+    int64_t lsqr_iters;             /* column iterations spent by all solves of the step          */
+    float   trace_eps[WRI_AWRI_MAX_TRACE];
+    double  trace_f[WRI_AWRI_MAX_TRACE], trace_f_trial[WRI_AWRI_MAX_TRACE];
+} wri_awri_report;
+int wri_misfit_sf(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_host, const int32_t* src_ijk_host,
+                  const void* d_dev, float lambda, float eps, int32_t maxit, int32_t warm,
+                  void* u_dev, void* alpha_dev, double* ar0_dev, double* f_pde_dev, double* f_data_dev,
+                  float* g_dev, int32_t* iters_dev, double* f_host);
+int wri_awri_step(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_host, const int32_t* src_ijk_host,
+                  const void* d_dev, float lambda, float eps, int32_t maxit, const wri_awri_opts* opts,
+                  float* m_dev, float* m_trial_dev, float* g_dev, void* u_dev, void* alpha_dev,
+                  void* u_trial_dev, void* alpha_trial_dev, double* f_cols_dev, wri_awri_report* report);
 
 /* Same solve with HOST buffers: copies q, d (and tol) to the device, solves, copies u_out,
  * resnorms and iters back, then synchronises the stream.  Needs a workspace sized with

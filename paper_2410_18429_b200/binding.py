@@ -38,6 +38,22 @@ class wri_lsqr_view(C.Structure):
                 ("nb_max", C.c_int32), ("sf_state", C.c_void_p)]
 
 
+WRI_AWRI_MAX_TRACE = 16
+wri_update_fn = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p)
+
+
+class wri_awri_opts(C.Structure):
+    _fields_ = [("max_halvings", C.c_int32), ("warm_restart", C.c_int32), ("update", wri_update_fn),
+                ("user", C.c_void_p), ("step", C.c_float), ("m_min", C.c_float), ("m_max", C.c_float)]
+
+
+class wri_awri_report(C.Structure):
+    _fields_ = [("accepted", C.c_int32), ("n_halvings", C.c_int32), ("n_trace", C.c_int32),
+                ("eps", C.c_float), ("f", C.c_double), ("f_trial", C.c_double), ("lsqr_iters", C.c_int64),
+                ("trace_eps", C.c_float * WRI_AWRI_MAX_TRACE), ("trace_f", C.c_double * WRI_AWRI_MAX_TRACE),
+                ("trace_f_trial", C.c_double * WRI_AWRI_MAX_TRACE)]
+
+
 WRI_OK = 0
 WRI_ERR_ARG = -1
 WRI_ERR_RECEIVER_RANGE = -2
@@ -86,6 +102,9 @@ def load_library():
     lib.wri_lsqr_sf_batch_host.argtypes = solve_sf
     lib.wri_objective_gradient.argtypes = [P, I32, P, P, P, P, P, P, F32, P, P, P]
     lib.wri_lsqr_set_opts.argtypes = [P, C.POINTER(wri_lsqr_opts)]
+    lib.wri_misfit_sf.argtypes = [P, I32, P, P, P, F32, F32, I32, I32, P, P, P, P, P, P, P, P]
+    lib.wri_awri_step.argtypes = [P, I32, P, P, P, F32, F32, I32, C.POINTER(wri_awri_opts), P, P, P, P, P, P, P,
+                                  P, C.POINTER(wri_awri_report)]
     lib.wri_lsqr_iterate.argtypes = [P, I32]
     lib.wri_lsqr_end.argtypes = [P]
     lib.wri_lsqr_peek.argtypes = [P, C.POINTER(wri_lsqr_view)]
@@ -337,6 +356,72 @@ class Wri:
         _ck(self._lib.wri_objective_gradient(self._h, nb, oi, si, _dptr(alpha), _dptr(q), _dptr(u), _dptr(d),
                                              float(lam), _dptr(fp), _dptr(fd), _dptr(g)))
         return fp, fd
+
+    def misfit_sf(self, d, lam, src_ijk, eps, maxit, omega_idx=None, g=None, warm=None, want_f=True):
+        """One misfit evaluation (wri_misfit_sf).  warm = (u, alpha, ar0) from an earlier evaluation
+        continues from it.  Returns dict(u, alpha, ar0, f_pde, f_data, iters, f); f is a host float
+        (None with want_f=False: then nothing synchronises)."""
+        t = self._torch
+        nb = d.shape[1]
+        self.ensure_workspace(nb, compaction=eps > 0)
+        if warm is not None:
+            u, a, ar0 = warm
+        else:
+            u = t.empty((self.ng, nb), dtype=t.complex64, device=d.device)
+            a = t.empty(nb, dtype=t.complex64, device=d.device)
+            ar0 = t.empty(nb, dtype=t.float64, device=d.device)
+        fp = t.empty(nb, dtype=t.float64, device=d.device)
+        fd = t.empty(nb, dtype=t.float64, device=d.device)
+        it = t.empty(nb, dtype=t.int32, device=d.device)
+        f = C.c_double(0.0)
+        keep, oi = _i32(omega_idx)
+        keep2, si = _i32(src_ijk)
+        _ck(self._lib.wri_misfit_sf(self._h, nb, oi, si, _dptr(d), float(lam), float(eps), int(maxit),
+                                    int(warm is not None), _dptr(u), _dptr(a), _dptr(ar0), _dptr(fp),
+                                    _dptr(fd), _dptr(g), _dptr(it), C.byref(f) if want_f else None))
+        return dict(u=u, alpha=a, ar0=ar0, f_pde=fp, f_data=fd, iters=it, f=f.value if want_f else None)
+
+    def awri_step(self, m, d, lam, src_ijk, eps, maxit, omega_idx=None, max_halvings=8, warm_restart=False,
+                  update=None, step=0.0, m_min=0.0, m_max=float("inf")):
+        """Lines 4-14 of Algorithm 2 (wri_awri_step) on the model tensor m (float32 [n_g], updated in
+        place when the step is accepted).  update(m, g, m_trial): enqueue m_trial on the current
+        stream (torch ops on the three tensors); None = built-in clamp(m - step g, m_min, m_max)."""
+        t = self._torch
+        nb = d.shape[1]
+        self.ensure_workspace(nb, compaction=True)
+        dev = d.device
+        m_trial = t.empty_like(m)
+        g = t.empty(self.ng, dtype=t.float32, device=dev)
+        u, ut = (t.empty((self.ng, nb), dtype=t.complex64, device=dev) for _ in range(2))
+        a, at = (t.empty(nb, dtype=t.complex64, device=dev) for _ in range(2))
+        fc = t.empty((2, nb), dtype=t.float64, device=dev)
+        err = []
+
+        def _cb(user, m_ptr, g_ptr, mt_ptr, stream):
+            try:
+                update(m, g, m_trial)
+                return 0
+            except Exception as e:                      # never raise across the C ABI
+                err.append(e)
+                return 1
+
+        cb = wri_update_fn(_cb) if update is not None else wri_update_fn()
+        o = wri_awri_opts(int(max_halvings), int(bool(warm_restart)), cb, None, float(step), float(m_min),
+                          float(m_max))
+        rep = wri_awri_report()
+        keep, oi = _i32(omega_idx)
+        keep2, si = _i32(src_ijk)
+        rc = self._lib.wri_awri_step(self._h, nb, oi, si, _dptr(d), float(lam), float(eps), int(maxit),
+                                     C.byref(o), _dptr(m), _dptr(m_trial), _dptr(g), _dptr(u), _dptr(a),
+                                     _dptr(ut), _dptr(at), _dptr(fc), C.byref(rep))
+        if err:
+            raise err[0]
+        _ck(rc)
+        n = rep.n_trace
+        return dict(accepted=bool(rep.accepted), n_halvings=rep.n_halvings, eps=rep.eps, f=rep.f,
+                    f_trial=rep.f_trial, lsqr_iters=rep.lsqr_iters, g=g, m_trial=m_trial, u=u, alpha=a,
+                    u_trial=ut, alpha_trial=at, f_cols=fc,
+                    trace=[(rep.trace_eps[i], rep.trace_f[i], rep.trace_f_trial[i]) for i in range(n)])
 
     def lsqr_iterate(self, n_steps=1):
         _ck(self._lib.wri_lsqr_iterate(self._h, int(n_steps)))

@@ -75,6 +75,12 @@ struct wri_ctx {
     int* colmap = nullptr;       // [nb_max] working column -> caller's column (-1 = padding)
     int* idx = nullptr;          // [3][nb_max] scratch: gather map | retire source | retire destination
     int* h_active = nullptr;     // pinned host copy of the active flags
+    // misfit evaluation / Algorithm 2 step (wri_misfit_sf, wri_awri_step)
+    float* aw_tol = nullptr;     // [nb_max] the uniform tolerance eps of a misfit evaluation
+    double* aw_f = nullptr;      // [2][nb_max] f_pde | f_data of the trial evaluation
+    double* aw_ar0 = nullptr;    // [nb_max] alpha1*beta1 of the cold solve at the current model
+    int* aw_iters = nullptr;     // [nb_max]
+    double* h_aw = nullptr;      // pinned: [2][nb_max] doubles followed by [nb_max] ints
     // caller's workspace
     char* ws = nullptr;
     size_t ws_bytes = 0;
@@ -758,6 +764,11 @@ int wri_create(wri_ctx** out, wri_grid grid, double h, int32_t n_omega, const do
     CKC(cudaMalloc(&c->src, nb_max * sizeof(int)));
     CKC(cudaMalloc(&c->idx, (size_t)3 * nb_max * sizeof(int)));
     CKC(cudaMallocHost(&c->h_active, nb_max * sizeof(int)));
+    CKC(cudaMalloc(&c->aw_tol, nb_max * sizeof(float)));
+    CKC(cudaMalloc(&c->aw_f, (size_t)2 * nb_max * sizeof(double)));
+    CKC(cudaMalloc(&c->aw_ar0, nb_max * sizeof(double)));
+    CKC(cudaMalloc(&c->aw_iters, nb_max * sizeof(int)));
+    CKC(cudaMallocHost(&c->h_aw, (size_t)nb_max * (2 * sizeof(double) + sizeof(int))));
     CKC(cudaMalloc(&c->counter, sizeof(unsigned int)));
     CKC(cudaMemset(c->counter, 0, sizeof(unsigned int)));
     {
@@ -778,6 +789,8 @@ int wri_destroy(wri_ctx* c) {
     cudaFree(c->coef_alt); cudaFree(c->stat_alt); cudaFree(c->active_alt); cudaFree(c->iters_alt);
     cudaFree(c->colmap); cudaFree(c->idx); cudaFree(c->src);
     if (c->h_active) cudaFreeHost(c->h_active);
+    cudaFree(c->aw_tol); cudaFree(c->aw_f); cudaFree(c->aw_ar0); cudaFree(c->aw_iters);
+    if (c->h_aw) cudaFreeHost(c->h_aw);
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
     delete c;
     return WRI_OK;
@@ -987,7 +1000,7 @@ int lsqr_begin_impl(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const
     int rc = check_batch_args(c, nb);
     if (rc) return rc;
     const bool sf = src_ijk_host != nullptr;          // source-free system: q may be absent (b_top = 0)
-    if ((!q_dev && !sf) || (c->n_rec && !d_dev) || !u_out_dev || !resnorms_dev || maxit < 0 ||
+    if ((!q_dev && !sf) || (c->n_rec && !d_dev) || !u_out_dev || maxit < 0 ||
         (q_dev && !aligned16(q_dev)) || !aligned16(u_out_dev) || q_dev == u_out_dev || (sf && !alpha_out_dev))
         return WRI_ERR_ARG;
     if (!c->ws) return WRI_ERR_WORKSPACE;
@@ -1081,7 +1094,7 @@ int retire_columns(wri_ctx* c, const std::vector<int>& src, const std::vector<in
         c->u_out, c->X, c->W, c->coef + C_CX * NM, d_src, d_dst, n, (long long)c->ng, c->nb, c->nb0);
     c->launches++;
     CK(cudaGetLastError());
-    if (c->k < c->maxit) {
+    if (c->k < c->maxit && c->resnorms) {
         k_hold_history<<<blocks_for((long long)(c->maxit - c->k) * n), 256, 0, c->stream>>>(
             c->resnorms, c->stat + S_PHIBAR * NM, d_src, d_dst, n, c->k + 1, c->maxit, c->nb0);
         c->launches++;
@@ -1340,6 +1353,123 @@ int wri_lsqr_peek(const wri_ctx* c, wri_lsqr_view* v) {
     v->nb_max = c->nb_max;
     v->sf_state = c->sf ? c->stat + S_VA_RE * NM : nullptr;
     return WRI_OK;
+}
+
+}  // extern "C"
+
+// ---- misfit evaluation and one outer iteration of Algorithm 2 -------------------------------------
+namespace {
+
+// Lines 4-5 (or 7-8) of Algorithm 2 for one group of columns: source-free solve to tolerance eps,
+// then eq. 8-9 at the solution.  f_host (optional) receives sum_s (f_pde + f_data), iters_host the
+// column iterations spent; either one makes the call synchronise the stream.
+int misfit_impl(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const int32_t* src_ijk_host,
+                const void* d_dev, float lambda, float eps, int32_t maxit, int32_t warm, void* u_dev,
+                void* alpha_dev, double* ar0_dev, double* f_pde_dev, double* f_data_dev, float* g_dev,
+                int32_t* iters_dev, double* f_host, int64_t* iters_host) {
+    int rc = check_batch_args(c, nb);
+    if (rc) return rc;
+    if (!src_ijk_host || !u_dev || !alpha_dev || !f_pde_dev || !f_data_dev || !(eps >= 0.f) || maxit < 0 ||
+        (warm && !ar0_dev))
+        return WRI_ERR_ARG;
+    if (c->solving) return WRI_ERR_STATE;
+    std::vector<float> tol(nb, eps);
+    CK(cudaMemcpyAsync(c->aw_tol, tol.data(), nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    int32_t* its = iters_dev ? iters_dev : c->aw_iters;
+    const wri_lsqr_opts saved = c->opts;
+    c->opts = wri_lsqr_opts{};
+    if (warm) { c->opts.warm_start = 1; c->opts.ar_ref_dev = ar0_dev; }
+    else c->opts.ar0_out_dev = ar0_dev;
+    rc = wri_lsqr_sf_batch(c, nb, omega_idx_host, src_ijk_host, nullptr, d_dev, lambda,
+                           eps > 0.f ? c->aw_tol : nullptr, maxit, u_dev, alpha_dev, nullptr, its);
+    c->opts = saved;
+    if (rc) return rc;
+    if ((rc = wri_objective_gradient(c, nb, omega_idx_host, src_ijk_host, alpha_dev, nullptr, u_dev, d_dev,
+                                     lambda, f_pde_dev, f_data_dev, g_dev)))
+        return rc;
+    if (f_host || iters_host) {
+        double* hf = c->h_aw;
+        int* hi = reinterpret_cast<int*>(c->h_aw + 2 * (size_t)c->nb_max);
+        CK(cudaMemcpyAsync(hf, f_pde_dev, nb * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        CK(cudaMemcpyAsync(hf + c->nb_max, f_data_dev, nb * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        CK(cudaMemcpyAsync(hi, its, nb * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+        CK(cudaStreamSynchronize(c->stream));
+        double f = 0.0;
+        int64_t n = 0;
+        for (int s = 0; s < nb; ++s) { f += hf[s] + hf[c->nb_max + s]; n += hi[s]; }   // fixed order
+        if (f_host) *f_host = f;
+        if (iters_host) *iters_host = n;
+    }
+    return WRI_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int wri_misfit_sf(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const int32_t* src_ijk_host,
+                  const void* d_dev, float lambda, float eps, int32_t maxit, int32_t warm, void* u_dev,
+                  void* alpha_dev, double* ar0_dev, double* f_pde_dev, double* f_data_dev, float* g_dev,
+                  int32_t* iters_dev, double* f_host) {
+    return misfit_impl(c, nb, omega_idx_host, src_ijk_host, d_dev, lambda, eps, maxit, warm, u_dev, alpha_dev,
+                       ar0_dev, f_pde_dev, f_data_dev, g_dev, iters_dev, f_host, nullptr);
+}
+
+int wri_awri_step(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const int32_t* src_ijk_host,
+                  const void* d_dev, float lambda, float eps, int32_t maxit, const wri_awri_opts* o,
+                  float* m_dev, float* m_trial_dev, float* g_dev, void* u_dev, void* alpha_dev,
+                  void* u_trial_dev, void* alpha_trial_dev, double* f_cols_dev, wri_awri_report* rep) {
+    int rc = check_batch_args(c, nb);
+    if (rc) return rc;
+    if (!o || !m_dev || !m_trial_dev || !g_dev || !u_dev || !alpha_dev || !u_trial_dev || !alpha_trial_dev ||
+        !f_cols_dev || !rep || !(eps > 0.f) || o->max_halvings < 0 || o->max_halvings >= WRI_AWRI_MAX_TRACE ||
+        m_dev == m_trial_dev || u_dev == u_trial_dev)
+        return WRI_ERR_ARG;
+    if (c->solving) return WRI_ERR_STATE;
+    const float* m_saved = c->m;
+    auto leave = [&](int code) { c->m = m_saved; return code; };
+    memset(rep, 0, sizeof *rep);
+    double* f_pde = f_cols_dev;
+    double* f_data = f_cols_dev + nb;
+    for (int h = 0;; ++h) {
+        // line 4-5: x-bar, f, g at the current model (after a "go back": optionally continued from x-bar)
+        double f = 0.0, f_trial = 0.0;
+        int64_t it0 = 0, it1 = 0;
+        c->m = m_dev;
+        CK(cudaMemsetAsync(g_dev, 0, c->ng * sizeof(float), c->stream));
+        const int warm = (o->warm_restart && h > 0) ? 1 : 0;
+        if ((rc = misfit_impl(c, nb, omega_idx_host, src_ijk_host, d_dev, lambda, eps, maxit, warm, u_dev,
+                              alpha_dev, c->aw_ar0, f_pde, f_data, g_dev, nullptr, &f, &it0)))
+            return leave(rc);
+        // line 6: the trial model
+        if (o->update) {
+            if (o->update(o->user, m_dev, g_dev, m_trial_dev, (void*)c->stream) != 0) return leave(WRI_ERR_ARG);
+        } else {
+            k_model_step<<<blocks_for((long long)c->ng), 256, 0, c->stream>>>(
+                m_trial_dev, m_dev, g_dev, o->step, o->m_min, o->m_max, (long long)c->ng);
+            c->launches++;
+            CK(cudaGetLastError());
+        }
+        // line 7-8: x-tilde and f-tilde at the trial model (cold solve, objective only)
+        c->m = m_trial_dev;
+        if ((rc = misfit_impl(c, nb, omega_idx_host, src_ijk_host, d_dev, lambda, eps, maxit, 0, u_trial_dev,
+                              alpha_trial_dev, nullptr, c->aw_f, c->aw_f + c->nb_max, nullptr, nullptr,
+                              &f_trial, &it1)))
+            return leave(rc);
+        c->m = m_dev;
+        rep->trace_eps[h] = eps; rep->trace_f[h] = f; rep->trace_f_trial[h] = f_trial;
+        rep->n_trace = h + 1;
+        rep->f = f; rep->f_trial = f_trial; rep->eps = eps; rep->n_halvings = h;
+        rep->lsqr_iters += it0 + it1;
+        if (!(f_trial > f)) {                               // line 9 / 12-13
+            CK(cudaMemcpyAsync(m_dev, m_trial_dev, c->ng * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
+            rep->accepted = 1;
+            break;
+        }
+        if (h == o->max_halvings) break;                    // reading C-20: give up, model unchanged
+        eps *= 0.5f;                                        // line 10-11
+    }
+    return leave(WRI_OK);
 }
 
 }  // extern "C"

@@ -457,7 +457,7 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
             p.active[s] = act;
             p.iters[s] = 0;
             if (p.iters_out) p.iters_out[s] = 0;      // start phases always run on the identity map
-            p.resnorms[s] = (float)beta;
+            if (p.resnorms) p.resnorms[s] = (float)beta;
             // first adjoint pass: V = (lambda/beta) A^H U + (1/beta) P^T U_bot, old V = 0 with cb = 1
             cf[C_CA_A * NM + s] = act ? (float)((double)p.lambda / beta) : 0.f;
             cf[C_CT_A * NM + s] = act ? (float)(1.0 / beta) : 0.f;
@@ -542,7 +542,7 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
                 cf[C_CW * NM + s] = 0.f;
                 cf[C_CA_F * NM + s] = 0.f; cf[C_CV_F * NM + s] = 0.f; cf[C_CB_F * NM + s] = 0.f;
             }
-            if (so >= 0) p.resnorms[(size_t)p.k * p.nb_out + so] = (float)st[S_PHIBAR * NM + s];
+            if (so >= 0 && p.resnorms) p.resnorms[(size_t)p.k * p.nb_out + so] = (float)st[S_PHIBAR * NM + s];
         }
     }
     __syncthreads();
@@ -753,6 +753,15 @@ k_grad(const GradParams p) {
     const int col0 = (int)(((long long)blockIdx.x * blockDim.x * VEC) % nb);
     __syncthreads();
     block_column_sums<VEC>(acc, col0, nb, p.partials + tile * nb);
+}
+
+// trial model of Algorithm 2 line 6 with the built-in steepest-descent update:
+// m_trial = clamp(m - step * g, m_min, m_max)   (the l-BFGS direction is the caller's)
+__global__ void k_model_step(float* __restrict__ m_trial, const float* __restrict__ m, const float* __restrict__ g,
+                             float step, float m_min, float m_max, long long n) {
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
+         i += (long long)gridDim.x * blockDim.x)
+        m_trial[i] = fminf(fmaxf(fmaf(-step, g[i], m[i]), m_min), m_max);
 }
 
 // g += t  (the batch's gradient from the TMA pass into the caller's accumulated gradient)

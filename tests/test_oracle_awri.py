@@ -1,0 +1,138 @@
+"""Pins of oracle/awri.py (CPU only): the misfit evaluation of eq. 7-9 summed over a group of
+columns, and lines 4-14 of Algorithm 2.
+
+The misfit and its gradient are checked against dense LAPACK least squares and finite
+differences of the reduced objective (nothing of the oracle's formulas is re-typed); the
+accept / halve / give-up logic against what Algorithm 2 prescribes on cases built so that each
+branch is taken: a descent step (accepted at once, first-order decrease t ||g||^2), an ascent
+step (never accepted: eps halves max_halvings times, model unchanged), and a case where the
+loose tolerance rejects a good step and the halved one accepts it.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import awri as A
+from oracle import oracle as O
+
+
+def _cn(rng, n):
+    return (rng.standard_normal(n) + 1j * rng.standard_normal(n)) / math.sqrt(2)
+
+
+def _problem(shape, n_rec, nb, seed, L=2, h=10.0, freqs=(5.0, 7.0)):
+    rng = np.random.Generator(np.random.PCG64(seed))
+    ops = [O.Operator(shape[0], shape[1], shape[2], h, 2 * math.pi * freqs[s % len(freqs)], L)
+           for s in range(nb)]
+    ng = ops[0].ng
+    v = rng.uniform(1500.0, 4500.0, ng)
+    m = 1.0 / v ** 2
+    rec = np.sort(rng.choice(ng, size=n_rec, replace=False)).astype(np.int64)
+    src = rng.choice(ng, size=nb, replace=False).astype(np.int64)
+    D = np.stack([_cn(rng, n_rec) for _ in range(nb)], axis=1)
+    return ops, m, rec, src, D, rng
+
+
+def _dense_S(op, m, lam, rec, src):
+    n = op.ng
+    S = np.zeros((n + rec.size, n + 1), dtype=complex)
+    e = np.zeros(n, complex)
+    for j in range(n):
+        e[j] = 1.0
+        t, b = O.apply_M(op, m, lam, rec, e)
+        S[:n, j], S[n:, j] = t, b
+        e[j] = 0.0
+    S[src, n] = -lam
+    return S
+
+
+def _f4_lapack(ops, m, lam, rec, src, D):
+    """eq. 8 through LAPACK: sum over columns of 1/2 min_x ||S x - [0; d]||^2."""
+    f = 0.0
+    for s, op in enumerate(ops):
+        S = _dense_S(op, m, lam, rec, int(src[s]))
+        b = np.concatenate([np.zeros(op.ng), D[:, s]])
+        x = np.linalg.lstsq(S, b, rcond=None)[0]
+        f += 0.5 * np.linalg.norm(S @ x - b) ** 2
+    return f
+
+
+def test_misfit_is_the_sum_over_columns_of_the_reduced_objective():
+    ops, m, rec, src, D, rng = _problem((6, 6, 5), 8, 2, seed=51)
+    lam = 15.0
+    out = A.misfit_sf(ops, m, lam, rec, src, D, eps=1e-13, maxit=3000)
+    assert out["f"] == pytest.approx(_f4_lapack(ops, m, lam, rec, src, D), rel=1e-9)
+    assert out["f"] == pytest.approx(out["f_cols"].sum(), rel=1e-15)
+    # eq. 9 summed over the group = derivative of eq. 8 (variable projection), by central differences
+    dm = rng.standard_normal(m.size) * m.mean()
+    e = 1e-4
+    fd = (_f4_lapack(ops, m + e * dm, lam, rec, src, D) - _f4_lapack(ops, m - e * dm, lam, rec, src, D)) / (2 * e)
+    assert fd == pytest.approx(float(out["g"] @ dm), rel=1e-5)
+    # a looser tolerance stops earlier and leaves a larger objective (LSQR's ||r_k|| is monotone)
+    loose = A.misfit_sf(ops, m, lam, rec, src, D, eps=1e-1, maxit=3000)
+    assert (loose["iters"] < out["iters"]).all() and loose["f"] > out["f"]
+    # warm start from the loose solution with the cold reference reaches the tight tolerance too
+    warm = A.misfit_sf(ops, m, lam, rec, src, D, eps=1e-13, maxit=3000, x0=loose["U"], a0=loose["alpha"],
+                       ar_ref=loose["ar0"])
+    assert warm["f"] == pytest.approx(out["f"], rel=1e-9)
+    assert np.array_equal(warm["ar0"], loose["ar0"])
+
+
+@pytest.fixture(scope="module")
+def group():
+    ops, m, rec, src, D, rng = _problem((10, 9, 8), 14, 3, seed=6)
+    lam = 20.0
+    g = A.misfit_sf(ops, m, lam, rec, src, D, eps=1e-10, maxit=2000)["g"]
+    return ops, m, rec, src, D, lam, g
+
+
+def _steepest(m, g_ref, t_rel, sign=-1.0):
+    t = t_rel * np.abs(m).mean() / np.abs(g_ref).max()
+    return (lambda mm, gg: np.float32(mm + sign * t * gg).astype(np.float64)), t
+
+
+def test_descent_step_is_accepted_at_once(group):
+    ops, m, rec, src, D, lam, g = group
+    upd, t = _steepest(m, g, 1e-3)
+    r = A.awri_step(ops, m, lam, rec, src, D, eps=1e-9, maxit=2000, update=upd, max_halvings=3)
+    assert r["accepted"] and r["n_halvings"] == 0 and r["eps"] == 1e-9
+    assert len(r["trace"]) == 1
+    assert np.array_equal(r["m"], upd(m, r["g"]))
+    # first-order decrease of the reduced objective along -g: f - f_trial = t ||g||^2 (1 + O(t))
+    assert r["f"] - r["f_trial"] == pytest.approx(t * float(r["g"] @ r["g"]), rel=2e-2)
+
+
+def test_ascent_step_halves_the_tolerance_until_the_cap(group):
+    ops, m, rec, src, D, lam, g = group
+    upd, _ = _steepest(m, g, 1e-1, sign=+1.0)
+    H = 3
+    r = A.awri_step(ops, m, lam, rec, src, D, eps=1e-6, maxit=2000, update=upd, max_halvings=H)
+    assert not r["accepted"] and r["n_halvings"] == H
+    assert r["eps"] == pytest.approx(1e-6 / 2 ** H, rel=1e-15)
+    assert [e for e, _, _ in r["trace"]] == pytest.approx([1e-6 / 2 ** h for h in range(H + 1)], rel=1e-15)
+    assert all(ft > f for _, f, ft in r["trace"])
+    assert r["m"] is m or np.array_equal(r["m"], m)          # line 13 not reached: model unchanged
+
+
+def test_loose_tolerance_rejects_a_good_step_and_the_halved_one_accepts(group):
+    """Found by scanning eps on this seeded group: at eps = 0.08466 one column of the trial model
+    stops an iteration earlier than at m, so f_trial > f although the step is a descent step;
+    with eps/2 the step is accepted (lines 9-13).  Margins of both decisions are > 1e-3 of f."""
+    ops, m, rec, src, D, lam, g = group
+    upd, _ = _steepest(m, g, 1e-1)
+    eps0 = 0.08466
+    r = A.awri_step(ops, m, lam, rec, src, D, eps=eps0, maxit=400, update=upd, max_halvings=6)
+    assert r["accepted"] and r["n_halvings"] == 1 and r["eps"] == pytest.approx(eps0 / 2, rel=1e-15)
+    (e0, f0, ft0), (e1, f1, ft1) = r["trace"]
+    assert ft0 > f0 and ft1 < f1
+    assert min(abs(ft0 - f0) / f0, abs(ft1 - f1) / f1) > 1e-3
+    assert f1 < f0                                            # the tighter solve lowers the objective
+    # the accepted model is the update from the gradient of the LAST (eps/2) evaluation
+    g1 = A.misfit_sf(ops, m, lam, rec, src, D, eps=eps0 / 2, maxit=400)["g"]
+    assert np.array_equal(r["m"], upd(m, g1))
+    # going back to line 4 with a warm start is allowed (x0 is free): the re-solve then starts from
+    # the loose solution and spends fewer iterations on it than a cold one
+    rw = A.awri_step(ops, m, lam, rec, src, D, eps=eps0, maxit=400, update=upd, max_halvings=6, warm=True)
+    assert rw["trace"][0] == r["trace"][0]
+    assert rw["accepted"]
