@@ -551,6 +551,19 @@ ScalParams scal_params(const wri_ctx* c, const double* partials, int n_rows, con
     return s;
 }
 
+// Ring depth per pass and plan.  Measured on B200 (profiles/r01_v6_stages.md): the adjoint pass is
+// sensitive to the prefetch distance (more stages in flight cost L2 hits on the stencil halo), with
+// the optimum at 6 stages for one 64- or 48-column chunk per cell and 5 otherwise; pass F at 3
+// (2 for 32-column chunks).
+template <class Cfg, int MODE>
+int ring_depth(int nchunk) {
+    int n = (MODE == MODE_F) ? (Cfg::CB == 32 ? 2 : 3)
+                             : ((Cfg::CB == 64 && nchunk == 1) || Cfg::CB == 48 || MODE == MODE_G) ? 6 : 5;
+    if (const char* e = getenv(MODE == MODE_F ? "WRI_F_NSTAGE" : "WRI_A_NSTAGE"))
+        if (atoi(e) > 0) n = atoi(e);
+    return std::max(2, std::min(n, (int)Cfg::NSTAGE));
+}
+
 template <class Cfg, int MODE>
 int launch_tma_cfg(wri_ctx* c, int phase) {
     static size_t attr_bytes = 0;
@@ -572,6 +585,7 @@ int launch_tma_cfg(wri_ctx* c, int phase) {
     p.ih2 = (float)(1.0 / (c->h * c->h));
     p.m6ih2 = (float)(-6.0 / (c->h * c->h));
     p.phase = phase;
+    p.nstage = ring_depth<Cfg, MODE>(P.nchunk);
     p.m_tma = P.m_tma;
     p.merged = P.merged;
     p.fin = scal_params(c, c->partials_tma, P.grid, nullptr);
@@ -651,6 +665,7 @@ int launch_tma_grad(wri_ctx* c, const float2* u, const float2* q, const int* src
     p.m6ih2 = (float)(-6.0 / (c->h * c->h));
     p.sgn = 1.f;
     p.m_tma = P.m_tma; p.merged = P.merged;
+    p.nstage = ring_depth<Cfg, MODE_G>(P.nchunk);
     p.has_q = q != nullptr; p.gsrc = src; p.galpha = alpha; p.g = g; p.lam2 = lambda * lambda;
     k_pass_tma<Cfg, MODE_G><<<P.grid, Cfg::NT + 32, smem, c->stream>>>(P.in, P.old, P.old, P.old, P.m, p);
     c->launches++;

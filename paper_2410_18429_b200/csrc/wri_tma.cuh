@@ -27,7 +27,7 @@ template <int CB_, int TXC_, int TYC_, int NT_, int NSTAGE_>
 struct TileCfg {
     static constexpr int CB = CB_, TXC = TXC_, TYC = TYC_;
     static constexpr int NT = NT_;                              // consumer threads
-    static constexpr int NSTAGE = NSTAGE_;                      // depth of the shared-memory ring
+    static constexpr int NSTAGE = NSTAGE_;                      // LARGEST depth of the shared-memory ring (p.nstage <= NSTAGE is used)
     static constexpr int ITEMS = TXC * TYC * CB / 2;            // 16-byte items per plane
     static constexpr int IPT = ITEMS / NT;                      // items per thread
     static constexpr int IN_BYTES = (TXC + 2) * (TYC + 2) * CB * 8;
@@ -38,14 +38,17 @@ struct TileCfg {
     static_assert(IN_BYTES % 128 == 0 && CTR_BYTES % 128 == 0, "TMA destinations need 128 B alignment");
 };
 
+struct TrueT { static constexpr bool value = true; };
+struct FalseT { static constexpr bool value = false; };
+
 template <int MODE> struct PassTraits;
 #ifndef WRI_F_STAGES
-#define WRI_F_STAGES 3
+#define WRI_F_STAGES 4
 #endif
 #ifndef WRI_A_STAGES
-#define WRI_A_STAGES 6
+#define WRI_A_STAGES 7
 #endif
-template <> struct PassTraits<MODE_F> { static constexpr int NSTREAM = 3, NSTAGE = WRI_F_STAGES; };   // default depths
+template <> struct PassTraits<MODE_F> { static constexpr int NSTREAM = 3, NSTAGE = WRI_F_STAGES; };   // largest depths
 template <> struct PassTraits<MODE_A> { static constexpr int NSTREAM = 1, NSTAGE = WRI_A_STAGES; };
 template <> struct PassTraits<MODE_G> { static constexpr int NSTREAM = 1, NSTAGE = WRI_A_STAGES; };   // stream = q (optional)
 
@@ -64,6 +67,7 @@ struct TmaPassParams {
     int m_tma;             // 1: the model tile rides in the TMA stage (needs nx % 4 == 0)
     int merged;            // 1: tensor maps fold (column, x) into one dimension (nchunk == 1)
     int phase;             // ScalPhase run by the last CTA
+    int nstage;            // ring depth in use (<= Cfg::NSTAGE), chosen per plan by the host
     // receiver rows, spread over the CTAs (keeps them off the last CTA's serial tail)
     int n_rec;
     const int* rec;        // [n_rec] cell indices
@@ -280,7 +284,7 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
                     }
                 }
                 __syncwarp();
-                if (++stage == NSTAGE) { stage = 0; phase ^= 1; }
+                if (++stage == p.nstage) { stage = 0; phase ^= 1; }
             }
         }
     } else {
@@ -330,7 +334,13 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
                 [](int) { return 0; });
         }
 
-        for (int t = blockIdx.x; t < p.n_tiles; t += gridDim.x) {
+        // One tile, marched over its planes.  M_TMA / HAS_OLD are compile-time copies of p.m_tma and of
+        // "the old-vector stream is present" so that the plane loop carries no such branches.  The
+        // three centre planes (z-1, z, z+1) rotate through three register sets by NAME (the loop is
+        // unrolled by three), the in-plane neighbour sum is overwritten after its use: no register
+        // copies per plane.  |.|^2 is summed in fp32 over the <= 32 planes of the tile, then in fp64.
+        auto run_tile = [&](auto m_tma_c, auto has_old_c, const int t, double (&acc)[2], int& chunk_out) {
+            constexpr bool M_TMA = decltype(m_tma_c)::value, HAS_OLD = decltype(has_old_c)::value;
             int r = t;
             const int chunk = r % p.nchunk; r /= p.nchunk;
             const int tx = r % p.ntx; r /= p.ntx;
@@ -338,6 +348,7 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
             const int tz = r / p.nty;
             const int z0 = tz * p.zc, z1 = min(z0 + p.zc, p.nz);
             const int col = chunk * CB + cp * 2;
+            chunk_out = chunk;
 
             float w2[2], ca[2], cb[2], cv[2], cx[2], cw[2];
 #pragma unroll
@@ -355,34 +366,36 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
             }
             bool valid[IPT];
             float gxy[IPT], m_cur[IPT], m_nxt[IPT];
-            size_t goff[IPT];                                   // element offset of (cell, z0) in the vectors
-            size_t moff[IPT];
-            float4 c_prev[IPT], c_cur[IPT], n_cur[IPT];
+            size_t off[IPT];                                    // element offset of (cell, plane being emitted)
+            int cell[IPT];                                      // its cell index
+            float4 cA[IPT], cB[IPT], cC[IPT], n_cur[IPT];
 #pragma unroll
             for (int j = 0; j < IPT; ++j) {
                 const int ix = tx * TXC + cxj[j], iy = ty * TYC + cyj[j];
                 valid[j] = ix < p.nx && iy < p.ny;
                 const int ixc = min(ix, p.nx - 1), iyc = min(iy, p.ny - 1);
                 gxy[j] = fmaxf(tab_g[ixc], tab_g[p.nx + iyc]);
-                moff[j] = ((size_t)z0 * p.ny + iyc) * p.nx + ixc;
-                goff[j] = (((size_t)z0 * p.ny + iyc) * p.nx + ixc) * p.nb + col;
+                cell[j] = (z0 * p.ny + iyc) * p.nx + ixc;
+                off[j] = (size_t)cell[j] * p.nb + col;
                 m_cur[j] = 0.f;
                 m_nxt[j] = 0.f;
-                c_prev[j] = c_cur[j] = n_cur[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+                cA[j] = cB[j] = cC[j] = n_cur[j] = make_float4(0.f, 0.f, 0.f, 0.f);
             }
-            double acc[2] = {0.0, 0.0};
+            float acc32[2] = {0.f, 0.f};
             const size_t plane_e = (size_t)p.nx * p.ny * p.nb;
-            const size_t plane_m = (size_t)p.nx * p.ny;
+            const int plane_m = p.nx * p.ny;
+            const float* gz_tab = tab_g + p.nx + p.ny;
 
-            for (int pl = z0 - 1; pl <= z1; ++pl) {
-                // model value of plane pl (used one step later), issued before the wait
-                if (!p.m_tma && pl >= z0 && pl < z1) {
+            // step pl: c_new <- centre of plane pl; emit plane pl-1 from (c_prev, c_cur, c_new, n_cur);
+            // then n_cur <- in-plane neighbour sum of plane pl
+            auto plane = [&](const int pl, float4 (&c_prev)[IPT], float4 (&c_cur)[IPT], float4 (&c_new)[IPT]) {
+                if (!M_TMA && pl >= z0 && pl < z1) {
 #pragma unroll
-                    for (int j = 0; j < IPT; ++j) m_nxt[j] = __ldg(p.m + moff[j] + (size_t)(pl - z0) * plane_m);
+                    for (int j = 0; j < IPT; ++j) m_nxt[j] = __ldg(p.m + cell[j] + (pl > z0 ? plane_m : 0));
                 }
                 mbar_wait(full0 + 8 * stage, phase);
                 const unsigned char* sb = stages + stage * STAGE_BYTES;
-                float4 c_new[IPT], n_new[IPT], o_old[IPT], o_w[IPT], o_x[IPT];
+                float4 n_new[IPT], o_old[IPT], o_w[IPT], o_x[IPT];
                 const bool emit = pl >= z0 + 1;
 #pragma unroll
                 for (int j = 0; j < IPT; ++j) {
@@ -393,22 +406,22 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
                                            (a.z + b.z) + (c.z + d.z), (a.w + b.w) + (c.w + d.w));
                     if (emit) {
                         const int io = Cfg::IN_BYTES + (tid + j * NT) * 16;
-                        o_old[j] = (MODE != MODE_G || p.has_q) ? lds128(sb, io) : make_float4(0.f, 0.f, 0.f, 0.f);
-                        if (p.m_tma)
+                        o_old[j] = HAS_OLD ? lds128(sb, io) : make_float4(0.f, 0.f, 0.f, 0.f);
+                        if (M_TMA)
                             m_cur[j] = *reinterpret_cast<const float*>(sb + M_OFF + (cyj[j] * TXC + cxj[j]) * 4);
-                        if (MODE == MODE_F) {
-                            o_w[j] = lds128(sb, io + Cfg::CTR_BYTES);
-                            o_x[j] = lds128(sb, io + 2 * Cfg::CTR_BYTES);
-                        }
                     }
                 }
-                __syncwarp();
-                if ((tid & 31) == 0) mbar_arrive(empty0 + 8 * stage);
-                if (++stage == NSTAGE) { stage = 0; phase ^= 1; }
+                // pass A / G: the stage is free once its loads are done.  Pass F reads W and X from
+                // the stage just before it uses them (fewer live registers) and releases it after.
+                auto release = [&]() {
+                    __syncwarp();
+                    if ((tid & 31) == 0) mbar_arrive(empty0 + 8 * stage);
+                    if (++stage == p.nstage) { stage = 0; phase ^= 1; }
+                };
+                if (MODE != MODE_F) release();
 
                 if (emit) {
-                    const int z = pl - 1;
-                    const float gzv = tab_g[p.nx + p.ny + z];
+                    const float gzv = gz_tab[pl - 1];
 #pragma unroll
                     for (int j = 0; j < IPT; ++j) {
                         const float g = fmaxf(gxy[j], gzv);
@@ -421,15 +434,14 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
                         if (MODE == MODE_G) {
                             // r = A u - q - alpha e;  |r|^2 sums;  g[c] += lam^2 sum_s w2_s (Re t + gamma Im t),
                             // t = conj(u) r  (= Re[conj((1 + i gamma) u) r], eq. 9 with this build's sponge)
-                            const int cell = (int)(moff[j] + (size_t)(z - z0) * plane_m);
                             float gterm = 0.f;
                             {
                                 const float wm = w2[0] * m_cur[j];
                                 const float dr = wm + p.m6ih2, di = wm * g;
                                 float r_re = fmaf(p.ih2, s0, fmaf(dr, cc.x, -di * cc.y)) - o_old[j].x;
                                 float r_im = fmaf(p.ih2, s1, fmaf(dr, cc.y, di * cc.x)) - o_old[j].y;
-                                if (cell == gsrc0) { r_re -= gal0.x; r_im -= gal0.y; }
-                                if (valid[j]) acc[0] += (double)fmaf(r_re, r_re, r_im * r_im);
+                                if (cell[j] == gsrc0) { r_re -= gal0.x; r_im -= gal0.y; }
+                                if (valid[j]) acc32[0] += fmaf(r_re, r_re, r_im * r_im);
                                 const float tr = fmaf(cc.x, r_re, cc.y * r_im), ti = fmaf(cc.x, r_im, -cc.y * r_re);
                                 gterm = w2[0] * fmaf(g, ti, tr);
                             }
@@ -438,8 +450,8 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
                                 const float dr = wm + p.m6ih2, di = wm * g;
                                 float r_re = fmaf(p.ih2, s2, fmaf(dr, cc.z, -di * cc.w)) - o_old[j].z;
                                 float r_im = fmaf(p.ih2, s3, fmaf(dr, cc.w, di * cc.z)) - o_old[j].w;
-                                if (cell == gsrc1) { r_re -= gal1.x; r_im -= gal1.y; }
-                                if (valid[j]) acc[1] += (double)fmaf(r_re, r_re, r_im * r_im);
+                                if (cell[j] == gsrc1) { r_re -= gal1.x; r_im -= gal1.y; }
+                                if (valid[j]) acc32[1] += fmaf(r_re, r_re, r_im * r_im);
                                 const float tr = fmaf(cc.z, r_re, cc.w * r_im), ti = fmaf(cc.z, r_im, -cc.w * r_re);
                                 gterm = fmaf(w2[1], fmaf(g, ti, tr), gterm);
                             }
@@ -450,62 +462,89 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
                                     gterm += __shfl_down_sync(0xffffffffu, gterm, dlt, HP);
                                 // pure store (no load in the pipeline's critical path): this batch's
                                 // gradient goes to a scratch array, k_add_f32 accumulates it afterwards
-                                if (cp == 0 && valid[j]) p.g[cell] = p.lam2 * gterm;
+                                if (cp == 0 && valid[j]) p.g[cell[j]] = p.lam2 * gterm;
                             }
-                            continue;
-                        }
-                        float4 rr;
-                        {
-                            const float wm = w2[0] * m_cur[j];
-                            const float dr = wm + p.m6ih2, di = p.sgn * wm * g;
-                            const float ar = fmaf(p.ih2, s0, fmaf(dr, cc.x, -di * cc.y));
-                            const float ai = fmaf(p.ih2, s1, fmaf(dr, cc.y, di * cc.x));
-                            rr.x = fmaf(ca[0], ar, -cb[0] * o_old[j].x);
-                            rr.y = fmaf(ca[0], ai, -cb[0] * o_old[j].y);
-                        }
-                        {
-                            const float wm = w2[1] * m_cur[j];
-                            const float dr = wm + p.m6ih2, di = p.sgn * wm * g;
-                            const float ar = fmaf(p.ih2, s2, fmaf(dr, cc.z, -di * cc.w));
-                            const float ai = fmaf(p.ih2, s3, fmaf(dr, cc.w, di * cc.z));
-                            rr.z = fmaf(ca[1], ar, -cb[1] * o_old[j].z);
-                            rr.w = fmaf(ca[1], ai, -cb[1] * o_old[j].w);
-                        }
-                        if (valid[j]) {
-                            const size_t off = goff[j] + (size_t)(z - z0) * plane_e;
+                        } else {
+                            float4 rr;
+                            {
+                                const float wm = w2[0] * m_cur[j];
+                                const float dr = wm + p.m6ih2, di = p.sgn * wm * g;
+                                const float ar = fmaf(p.ih2, s0, fmaf(dr, cc.x, -di * cc.y));
+                                const float ai = fmaf(p.ih2, s1, fmaf(dr, cc.y, di * cc.x));
+                                rr.x = fmaf(ca[0], ar, -cb[0] * o_old[j].x);
+                                rr.y = fmaf(ca[0], ai, -cb[0] * o_old[j].y);
+                            }
+                            {
+                                const float wm = w2[1] * m_cur[j];
+                                const float dr = wm + p.m6ih2, di = p.sgn * wm * g;
+                                const float ar = fmaf(p.ih2, s2, fmaf(dr, cc.z, -di * cc.w));
+                                const float ai = fmaf(p.ih2, s3, fmaf(dr, cc.w, di * cc.z));
+                                rr.z = fmaf(ca[1], ar, -cb[1] * o_old[j].z);
+                                rr.w = fmaf(ca[1], ai, -cb[1] * o_old[j].w);
+                            }
+                            if (valid[j]) {
 #if WRI_HINTS >= 1
-                            stg128_hint(p.out + off, rr, pol_out);
+                                stg128_hint(p.out + off[j], rr, pol_out);
 #else
-                            *reinterpret_cast<float4*>(p.out + off) = rr;
+                                *reinterpret_cast<float4*>(p.out + off[j]) = rr;
 #endif
-                            acc[0] += (double)fmaf(rr.x, rr.x, rr.y * rr.y);
-                            acc[1] += (double)fmaf(rr.z, rr.z, rr.w * rr.w);
-                            if (MODE == MODE_F) {
-                                float4 xn, wn;
-                                xn.x = fmaf(cx[0], o_w[j].x, o_x[j].x);
-                                xn.y = fmaf(cx[0], o_w[j].y, o_x[j].y);
-                                xn.z = fmaf(cx[1], o_w[j].z, o_x[j].z);
-                                xn.w = fmaf(cx[1], o_w[j].w, o_x[j].w);
-                                wn.x = fmaf(cv[0], cc.x, -cw[0] * o_w[j].x);
-                                wn.y = fmaf(cv[0], cc.y, -cw[0] * o_w[j].y);
-                                wn.z = fmaf(cv[1], cc.z, -cw[1] * o_w[j].z);
-                                wn.w = fmaf(cv[1], cc.w, -cw[1] * o_w[j].w);
+                                acc32[0] += fmaf(rr.x, rr.x, rr.y * rr.y);
+                                acc32[1] += fmaf(rr.z, rr.z, rr.w * rr.w);
+                                if (MODE == MODE_F) {
+                                    const int io = Cfg::IN_BYTES + (tid + j * NT) * 16;
+                                    o_w[j] = lds128(sb, io + Cfg::CTR_BYTES);
+                                    o_x[j] = lds128(sb, io + 2 * Cfg::CTR_BYTES);
+                                    float4 xn, wn;
+                                    xn.x = fmaf(cx[0], o_w[j].x, o_x[j].x);
+                                    xn.y = fmaf(cx[0], o_w[j].y, o_x[j].y);
+                                    xn.z = fmaf(cx[1], o_w[j].z, o_x[j].z);
+                                    xn.w = fmaf(cx[1], o_w[j].w, o_x[j].w);
+                                    wn.x = fmaf(cv[0], cc.x, -cw[0] * o_w[j].x);
+                                    wn.y = fmaf(cv[0], cc.y, -cw[0] * o_w[j].y);
+                                    wn.z = fmaf(cv[1], cc.z, -cw[1] * o_w[j].z);
+                                    wn.w = fmaf(cv[1], cc.w, -cw[1] * o_w[j].w);
 #if WRI_HINTS >= 1
-                                stg128_hint(p.X + off, xn, pol_st);
-                                stg128_hint(p.W + off, wn, pol_st);
+                                    stg128_hint(p.X + off[j], xn, pol_st);
+                                    stg128_hint(p.W + off[j], wn, pol_st);
 #else
-                                *reinterpret_cast<float4*>(p.X + off) = xn;
-                                *reinterpret_cast<float4*>(p.W + off) = wn;
+                                    *reinterpret_cast<float4*>(p.X + off[j]) = xn;
+                                    *reinterpret_cast<float4*>(p.W + off[j]) = wn;
 #endif
+                                }
                             }
                         }
+                        off[j] += plane_e;
+                        cell[j] += plane_m;
                     }
                 }
+                if (MODE == MODE_F) release();
 #pragma unroll
                 for (int j = 0; j < IPT; ++j) {
-                    c_prev[j] = c_cur[j]; c_cur[j] = c_new[j]; n_cur[j] = n_new[j];
-                    if (!p.m_tma) m_cur[j] = m_nxt[j];
+                    n_cur[j] = n_new[j];
+                    if (!M_TMA) m_cur[j] = m_nxt[j];
                 }
+            };
+            for (int pl = z0 - 1; pl <= z1; pl += 3) {
+                plane(pl, cA, cB, cC);
+                if (pl + 1 > z1) break;
+                plane(pl + 1, cB, cC, cA);
+                if (pl + 2 > z1) break;
+                plane(pl + 2, cC, cA, cB);
+            }
+            acc[0] = (double)acc32[0];
+            acc[1] = (double)acc32[1];
+        };
+
+        for (int t = blockIdx.x; t < p.n_tiles; t += gridDim.x) {
+            double acc[2];
+            int chunk;
+            const bool has_old = (MODE != MODE_G) || p.has_q;
+            if (p.m_tma) {
+                if (has_old) run_tile(TrueT{}, TrueT{}, t, acc, chunk);
+                else         run_tile(TrueT{}, FalseT{}, t, acc, chunk);
+            } else {
+                if (has_old) run_tile(FalseT{}, TrueT{}, t, acc, chunk);
+                else         run_tile(FalseT{}, FalseT{}, t, acc, chunk);
             }
             // fold this tile's per-thread sums into the CTA's per-column sums, fixed order
             red[tid * 2] = acc[0];
