@@ -1011,9 +1011,14 @@ namespace {
 int lsqr_begin_impl(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const void* q_dev,
                     const void* d_dev, float lambda, const float* tol_dev, int32_t maxit,
                     void* u_out_dev, float* resnorms_dev, int32_t* iters_dev, bool host_staged,
-                    const int32_t* src_ijk_host = nullptr, void* alpha_out_dev = nullptr) {
+                    const int32_t* src_ijk_host = nullptr, void* alpha_out_dev = nullptr,
+                    int col0 = 0, int nbw = 0) {
+    // col0, nbw: a GROUPED solve works on the caller's columns [col0, col0 + nbw) only, in a compact
+    // nbw-wide working set of its own (nbw = 0: all nb columns, working set = the caller's layout)
     int rc = check_batch_args(c, nb);
     if (rc) return rc;
+    const bool grouped = nbw > 0 && nbw < nb;
+    if (!grouped) { col0 = 0; nbw = nb; }
     const bool sf = src_ijk_host != nullptr;          // source-free system: q may be absent (b_top = 0)
     if ((!q_dev && !sf) || (c->n_rec && !d_dev) || !u_out_dev || maxit < 0 ||
         (q_dev && !aligned16(q_dev)) || !aligned16(u_out_dev) || q_dev == u_out_dev || (sf && !alpha_out_dev))
@@ -1022,52 +1027,87 @@ int lsqr_begin_impl(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const
     const int base_flags = host_staged ? WS_HOST_STAGING : 0;
     if (c->ws_bytes < ws_layout(c, nb, base_flags, kHostMaxitCap).total) return WRI_ERR_WORKSPACE;
     const WsLayout L = ws_layout(c, nb, base_flags | WS_COMPACTION, kHostMaxitCap);
-    if ((rc = upload_columns(c, nb, omega_idx_host, lambda))) return rc;
+    if ((rc = upload_columns(c, nbw, omega_idx_host ? omega_idx_host + col0 : nullptr, lambda))) return rc;
     if (sf && (rc = upload_sources(c, nb, src_ijk_host))) return rc;
     c->sf = sf;
     c->alpha_out = (float2*)alpha_out_dev;
 
-    c->nb = nb; c->nb0 = nb; c->k = 0; c->maxit = maxit; c->lambda = lambda;
-    c->packed = false; c->all_done = false;
-    c->U = (float2*)(c->ws + L.U); c->V = (float2*)(c->ws + L.V); c->W = (float2*)(c->ws + L.W);
+    c->nb = nbw; c->nb0 = nb; c->k = 0; c->maxit = maxit; c->lambda = lambda;
+    c->packed = grouped; c->all_done = false;
     c->U_bot = (float2*)(c->ws + L.U_bot);
     c->partials = (double*)(c->ws + L.partials);
     c->partials_tma = (double*)(c->ws + L.partials_tma);
-    c->X = (float2*)u_out_dev; c->u_out = (float2*)u_out_dev;
+    c->u_out = (float2*)u_out_dev;
+    c->free_slots.clear();
+    const bool ws_compact = c->ws_bytes >= L.total;           // the two spare vectors are there
+    if (!grouped) {
+        c->U = (float2*)(c->ws + L.U); c->V = (float2*)(c->ws + L.V); c->W = (float2*)(c->ws + L.W);
+        c->X = (float2*)u_out_dev;
+        if (ws_compact) {
+            c->free_slots.push_back((float2*)(c->ws + L.B3));
+            c->free_slots.push_back((float2*)(c->ws + L.B4));
+            c->U_bot_alt = (float2*)(c->ws + L.U_bot2);
+        }
+    } else {
+        // nbw-wide slots carved out of the nb-wide vector regions; the V region is skipped when the
+        // host entry has staged q there (it must survive until the last group has started)
+        const size_t slot = align_up(c->ng * (size_t)nbw * sizeof(float2), 256);
+        const size_t region = align_up(c->ng * (size_t)nb * sizeof(float2), 256);
+        std::vector<float2*> slots;
+        size_t bases[5] = {L.U, L.V, L.W, L.B3, L.B4};
+        for (int rgn = 0; rgn < (ws_compact ? 5 : 3); ++rgn) {
+            if (rgn == 1 && host_staged && q_dev) continue;
+            for (size_t o = 0; o + slot <= region; o += slot) slots.push_back((float2*)(c->ws + bases[rgn] + o));
+        }
+        if (slots.size() < 4) return WRI_ERR_WORKSPACE;
+        c->U = slots[0]; c->V = slots[1]; c->W = slots[2]; c->X = slots[3];
+        for (size_t i = 4; i < slots.size(); ++i) c->free_slots.push_back(slots[i]);
+        // the receiver-row region holds nb columns: first half the rows, second half the spare
+        c->U_bot_alt = c->U_bot + (size_t)std::max(c->n_rec, 1) * nbw;
+        std::vector<int> cm(nbw);
+        for (int j = 0; j < nbw; ++j) cm[j] = col0 + j;
+        CK(cudaMemcpyAsync(c->colmap, cm.data(), nbw * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    }
     c->tol = tol_dev; c->resnorms = resnorms_dev; c->iters_out = iters_dev;
-    c->tl = make_tiling(c, nb);
+    c->tl = make_tiling(c, nbw);
     if ((rc = tma_setup(c))) return rc;
     // Convergence is watched from the host only when tolerances are given: every check_every
     // iterations (~2 ms of device work) the active flags are read back; converged columns are
     // compacted away when the workspace has room for it and the batch is on the TMA path.
-    c->can_compact = tol_dev && c->tma_cb && c->ws_bytes >= L.total && !getenv("WRI_NO_COMPACT");
+    c->can_compact = tol_dev && c->tma_cb && c->free_slots.size() >= 2 && !getenv("WRI_NO_COMPACT");
     c->check_every = 0;
     if (tol_dev) {
-        const double t_iter = 80.0 * (double)c->ng * nb / 6.0e12;
+        const double t_iter = 80.0 * (double)c->ng * nbw / 6.0e12;
         c->check_every = (int)std::min(32.0, std::max(1.0, std::ceil(2.0e-3 / t_iter)));
     }
-    c->free_slots.clear();
-    if (c->can_compact) {
-        c->free_slots.push_back((float2*)(c->ws + L.B3));
-        c->free_slots.push_back((float2*)(c->ws + L.B4));
-        c->U_bot_alt = (float2*)(c->ws + L.U_bot2);
-    }
-    c->h_colmap.resize(nb);
-    for (int s = 0; s < nb; ++s) c->h_colmap[s] = s;
+    c->h_colmap.resize(nbw);
+    for (int s = 0; s < nbw; ++s) c->h_colmap[s] = col0 + s;
     c->retired.assign(nb, 0);
-    const size_t vbytes = c->ng * (size_t)nb * sizeof(float2);
+    const size_t vbytes = c->ng * (size_t)nbw * sizeof(float2);
     const size_t NM = c->nb_max;
 
     // beta1 u1 = b = [lambda q ; d]   (q is consumed before V is cleared: the host entry
     // stages q in the V slot)
-    PassParams p = base_params(c, nb, c->tl);
+    PassParams p = base_params(c, nbw, c->tl);
     p.partials = c->partials;
     p.in = (const float2*)q_dev; p.out = c->U; p.ca = c->coef + C_LAM * NM;
+    auto gather_in = [&](float2* dst, const void* src) -> int {      // dst[:, j] = src[:, col0 + j]
+        k_gather_cols<<<blocks_for((long long)c->ng * nbw), 256, 0, c->stream>>>(
+            dst, (const float2*)src, c->colmap, (long long)c->ng, nbw, nb);
+        c->launches++;
+        CK(cudaGetLastError());
+        return WRI_OK;
+    };
+    if (grouped && c->opts.warm_start && (rc = gather_in(c->X, u_out_dev))) return rc;
     if (q_dev) {
+        if (grouped) {                    // the group's columns of q, compact, in the (still unused) W slot
+            if ((rc = gather_in(c->W, q_dev))) return rc;
+            p.in = c->W;
+        }
         if ((rc = launch_pass<MODE_INIT>(c, p, c->tl))) return rc;
     } else {
         CK(cudaMemsetAsync(c->U, 0, vbytes, c->stream));
-        CK(cudaMemsetAsync(c->partials, 0, c->tl.n_tiles * nb * sizeof(double), c->stream));
+        CK(cudaMemsetAsync(c->partials, 0, c->tl.n_tiles * nbw * sizeof(double), c->stream));
     }
     if (c->opts.warm_start) {
         // warm start: u_out holds x0; top rows of r0 = b - S x0:  U <- U - lambda A x0  (and its ||.||^2)
@@ -1186,6 +1226,32 @@ int check_active(wri_ctx* c) {
     return WRI_OK;
 }
 
+// A batch wider than one 64-column chunk per cell is solved as successive 64-column GROUPS, each in a
+// compact working set of its own (columns are independent systems; reading C-9: a
+// column's result does not depend on its batch).  With several chunks per cell a tile row is a 512-byte
+// piece of a wider cell record and the passes reach 0.84-0.88 of the copy bandwidth; compact groups
+// run at the single-chunk rate (0.92).  The stepping entries keep all columns in lock-step.
+int group_width(const wri_ctx* c, int nb) {
+    if (getenv("WRI_NO_GROUPS")) return 0;
+    return (nb > 64 && nb % 64 == 0 && tma_chunk_for(64) == 64 && get_encode_fn()) ? 64 : 0;
+}
+
+int solve_groups(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const void* q_dev, const void* d_dev,
+                 float lambda, const float* tol_dev, int32_t maxit, void* u_out_dev, float* resnorms_dev,
+                 int32_t* iters_dev, bool host_staged, const int32_t* src_ijk_host, void* alpha_out_dev) {
+    int rc = check_batch_args(c, nb);
+    if (rc) return rc;
+    const int gw = group_width(c, nb);
+    for (int col0 = 0; col0 < nb; col0 += (gw ? gw : nb)) {
+        if ((rc = lsqr_begin_impl(c, nb, omega_idx_host, q_dev, d_dev, lambda, tol_dev, maxit, u_out_dev,
+                                  resnorms_dev, iters_dev, host_staged, src_ijk_host, alpha_out_dev, col0, gw)))
+            return rc;
+        if ((rc = wri_lsqr_iterate(c, maxit))) { c->solving = false; return rc; }
+        if ((rc = wri_lsqr_end(c))) return rc;
+    }
+    return WRI_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -1267,22 +1333,17 @@ int wri_lsqr_end(wri_ctx* c) {
 int wri_lsqr_batch(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const void* q_dev,
                    const void* d_dev, float lambda, const float* tol_dev, int32_t maxit,
                    void* u_out_dev, float* resnorms_dev, int32_t* iters_dev) {
-    int rc = wri_lsqr_begin(c, nb, omega_idx_host, q_dev, d_dev, lambda, tol_dev, maxit, u_out_dev,
-                            resnorms_dev, iters_dev);
-    if (rc) return rc;
-    if ((rc = wri_lsqr_iterate(c, maxit))) { c->solving = false; return rc; }
-    return wri_lsqr_end(c);
+    return solve_groups(c, nb, omega_idx_host, q_dev, d_dev, lambda, tol_dev, maxit, u_out_dev, resnorms_dev,
+                        iters_dev, false, nullptr, nullptr);
 }
 
 int wri_lsqr_sf_batch(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const int32_t* src_ijk_host,
                       const void* q_dev, const void* d_dev, float lambda, const float* tol_dev,
                       int32_t maxit, void* u_out_dev, void* alpha_out_dev, float* resnorms_dev,
                       int32_t* iters_dev) {
-    int rc = wri_lsqr_sf_begin(c, nb, omega_idx_host, src_ijk_host, q_dev, d_dev, lambda, tol_dev, maxit,
-                               u_out_dev, alpha_out_dev, resnorms_dev, iters_dev);
-    if (rc) return rc;
-    if ((rc = wri_lsqr_iterate(c, maxit))) { c->solving = false; return rc; }
-    return wri_lsqr_end(c);
+    if (!src_ijk_host) return WRI_ERR_ARG;
+    return solve_groups(c, nb, omega_idx_host, q_dev, d_dev, lambda, tol_dev, maxit, u_out_dev, resnorms_dev,
+                        iters_dev, false, src_ijk_host, alpha_out_dev);
 }
 
 }  // extern "C"
@@ -1319,11 +1380,9 @@ int lsqr_batch_host_impl(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, 
     if (Qs) CK(cudaMemcpyAsync(Qs, q_host, vbytes, cudaMemcpyHostToDevice, c->stream));
     if (dbytes) CK(cudaMemcpyAsync(Ds, d_host, dbytes, cudaMemcpyHostToDevice, c->stream));
     if (tol_host) CK(cudaMemcpyAsync(tols, tol_host, nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));
-    rc = lsqr_begin_impl(c, nb, omega_idx_host, Qs, Ds, lambda, tol_host ? tols : nullptr, maxit, Xs, res, its,
-                         true, src_ijk_host, sf ? As : nullptr);
-    if (rc) return rc;
-    if ((rc = wri_lsqr_iterate(c, maxit))) { c->solving = false; return rc; }
-    if ((rc = wri_lsqr_end(c))) return rc;
+    if ((rc = solve_groups(c, nb, omega_idx_host, Qs, Ds, lambda, tol_host ? tols : nullptr, maxit, Xs, res, its,
+                           true, src_ijk_host, sf ? As : nullptr)))
+        return rc;
     CK(cudaMemcpyAsync(u_out_host, Xs, vbytes, cudaMemcpyDeviceToHost, c->stream));
     CK(cudaMemcpyAsync(resnorms_host, res, (size_t)(maxit + 1) * nb * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
     if (iters_host) CK(cudaMemcpyAsync(iters_host, its, nb * sizeof(int), cudaMemcpyDeviceToHost, c->stream));

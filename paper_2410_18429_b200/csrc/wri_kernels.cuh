@@ -379,15 +379,17 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
     const long long nrs = (long long)p.n_rec * nb;
     if (PHASE == PH_INIT_B) {
         // U_bot = d (exact copy), then beta1 = ||[lambda q ; d]||
-        if (!p.warm) {
-            for (long long i = threadIdx.x; i < nrs; i += blockDim.x) p.U_bot[i] = p.d[i];
-        } else {
-            // warm start: bottom rows of r0 = b - S x0, i.e. d - x0 at the receiver nodes
-            for (long long i = threadIdx.x; i < nrs; i += blockDim.x) {
-                const int r = (int)(i / nb), s = (int)(i - (long long)r * nb);
-                const float2 dv = p.d[i], xv = p.X[(size_t)p.rec[r] * nb + s];
-                p.U_bot[i] = make_float2(dv.x - xv.x, dv.y - xv.y);
+        // (d is the CALLER's [n_rec][nb_out] array: a grouped solve works on a subset of its columns)
+        for (long long i = threadIdx.x; i < nrs; i += blockDim.x) {
+            const int r = (int)(i / nb), s = (int)(i - (long long)r * nb);
+            const int so = p.colmap ? p.colmap[s] : s;
+            float2 dv = so >= 0 ? p.d[(size_t)r * p.nb_out + so] : make_float2(0.f, 0.f);
+            if (p.warm) {
+                // warm start: bottom rows of r0 = b - S x0, i.e. d - x0 at the receiver nodes
+                const float2 xv = p.X[(size_t)p.rec[r] * nb + s];
+                dv = make_float2(dv.x - xv.x, dv.y - xv.y);
             }
+            p.U_bot[i] = dv;
         }
         __syncthreads();
     }
@@ -431,10 +433,10 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
         }
         if (PHASE == PH_INIT_B) {
             for (int r = S_VA_RE; r <= S_XA_IM; ++r) st[r * NM + s] = 0.0;
-            if (p.alpha_out && !p.warm) p.alpha_out[s] = make_float2(0.f, 0.f);
+            if (p.alpha_out && !p.warm && so >= 0) p.alpha_out[so] = make_float2(0.f, 0.f);
             if (p.warm && sc >= 0) {
                 // r0_top = lam q - lam (A x0 - a0 e): the pass before left lam q - lam A x0 in U
-                const float2 a0 = p.alpha_out[s];
+                const float2 a0 = p.alpha_out[so];
                 st[S_XA_RE * NM + s] = (double)a0.x; st[S_XA_IM * NM + s] = (double)a0.y;
                 float2* up = p.U + (size_t)sc * nb + s;
                 const float2 o = __ldcg(up);
@@ -456,8 +458,8 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
             const int act = beta > 0.0;
             p.active[s] = act;
             p.iters[s] = 0;
-            if (p.iters_out) p.iters_out[s] = 0;      // start phases always run on the identity map
-            if (p.resnorms) p.resnorms[s] = (float)beta;
+            if (p.iters_out && so >= 0) p.iters_out[so] = 0;
+            if (p.resnorms && so >= 0) p.resnorms[so] = (float)beta;
             // first adjoint pass: V = (lambda/beta) A^H U + (1/beta) P^T U_bot, old V = 0 with cb = 1
             cf[C_CA_A * NM + s] = act ? (float)((double)p.lambda / beta) : 0.f;
             cf[C_CT_A * NM + s] = act ? (float)(1.0 / beta) : 0.f;
@@ -470,8 +472,8 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
             int act = p.active[s];
             st[S_ALPHA * NM + s] = alpha;
             st[S_RHOBAR * NM + s] = alpha;
-            st[S_AR0 * NM + s] = (p.ar_ref && p.ar_ref[s] > 0.0) ? p.ar_ref[s] : alpha * beta;
-            if (p.ar0_out) p.ar0_out[s] = alpha * beta;
+            st[S_AR0 * NM + s] = (p.ar_ref && so >= 0 && p.ar_ref[so] > 0.0) ? p.ar_ref[so] : alpha * beta;
+            if (p.ar0_out && so >= 0) p.ar0_out[so] = alpha * beta;
             if (act && !(alpha > 0.0)) { act = 0; p.active[s] = 0; }
             cf[C_CA_F * NM + s] = act ? (float)((double)p.lambda / alpha) : 0.f;
             cf[C_CV_F * NM + s] = act ? (float)(1.0 / alpha) : 0.f;

@@ -359,3 +359,79 @@ def test_no_receivers_and_host_entry(torch_cuda):
     b = [t.numpy() for t in ctx.lsqr_batch_host(qh, dh, w.lam, None, maxit=15, omega_idx=w.omega_idx)]
     for x, y in zip(a, b):
         assert np.array_equal(x, y)
+
+
+def test_wide_batches_are_solved_in_64_column_groups(torch_cuda, monkeypatch):
+    """nb = 128: wri_lsqr_batch works through two compact 64-column groups.
+    Each group must give exactly what a separate solve of those 64 columns gives (a column's
+    result does not depend on its batch, C-9), the lock-step 128-column solve (WRI_NO_GROUPS) the
+    same within rounding, the oracle within 1e-3; with tolerances, the source-free system, a warm
+    start and the host entry as well."""
+    torch = torch_cuda
+    w = workloads.make("config2", grid=(24, 28, 40), nb=128)
+    K = 30
+    q, d = torch.from_numpy(w.Q).cuda(), torch.from_numpy(w.D).cuda()
+    ctx = _wri(w)
+    u, res, it = ctx.lsqr_batch(q, d, w.lam, None, maxit=K, omega_idx=w.omega_idx)
+    torch.cuda.synchronize()
+    assert (it.cpu().numpy() == K).all()
+    for g in range(2):
+        sl = slice(64 * g, 64 * g + 64)
+        ug, rg, _ = ctx.lsqr_batch(q[:, sl].contiguous(), d[:, sl].contiguous(), w.lam, None, maxit=K,
+                                   omega_idx=w.omega_idx[sl])
+        assert torch.equal(torch.view_as_real(u[:, sl]), torch.view_as_real(ug))
+        assert torch.equal(res[:, sl], rg)
+    monkeypatch.setenv("WRI_NO_GROUPS", "1")
+    u1, res1, _ = ctx.lsqr_batch(q, d, w.lam, None, maxit=K, omega_idx=w.omega_idx)
+    torch.cuda.synchronize()
+    monkeypatch.delenv("WRI_NO_GROUPS")
+    assert rel(u.cpu().numpy(), u1.cpu().numpy()) < 1e-5
+    assert rel(res.cpu().numpy(), res1.cpu().numpy()) < 1e-6
+    rec = O.rec_cells(w.nx, w.ny, w.nz, w.rec_ijk)
+    cols = [0, 63, 64, 127]
+    ref = O.lsqr_batch(ops_for(w), w.m, w.lam, rec, w.Q, w.D, None, maxit=K, threads=4, columns=cols)
+    for j, s in enumerate(cols):
+        assert rel(res[:, s].cpu().numpy(), ref["resnorms"][:, j]) < 1e-3
+        assert rel(u[:, s].cpu().numpy(), ref["x"][:, j]) < 1e-3
+
+    # per-column tolerances: groups compact on their own; same stop iterations as the lock-step solve
+    rng = np.random.Generator(np.random.PCG64(5))
+    tolh = (10.0 ** rng.uniform(-2.5, -0.5, w.nb)).astype(np.float32)
+    tolh[7] = 0.0
+    tol = torch.from_numpy(tolh).cuda()
+    ut, rt, itt = ctx.lsqr_batch(q, d, w.lam, tol, maxit=80, omega_idx=w.omega_idx)
+    torch.cuda.synchronize()
+    monkeypatch.setenv("WRI_NO_GROUPS", "1")
+    ut1, rt1, itt1 = ctx.lsqr_batch(q, d, w.lam, tol, maxit=80, omega_idx=w.omega_idx)
+    torch.cuda.synchronize()
+    monkeypatch.delenv("WRI_NO_GROUPS")
+    assert torch.equal(itt, itt1) and int(itt[7]) == 80 and len(set(itt.cpu().tolist())) > 8
+    assert rel(ut.cpu().numpy(), ut1.cpu().numpy()) < 1e-5
+    assert rel(rt.cpu().numpy(), rt1.cpu().numpy()) < 1e-6
+
+    # source-free system, then a warm continuation with the cold reference, grouped vs lock-step
+    outs = {}
+    for mode in ("groups", "lockstep"):
+        if mode == "lockstep":
+            monkeypatch.setenv("WRI_NO_GROUPS", "1")
+        ar0 = torch.zeros(w.nb, dtype=torch.float64, device="cuda")
+        ctx.set_opts(ar0_out=ar0)
+        us, al, rs, its = ctx.lsqr_sf_batch(d, w.lam, w.src_ijk, None, maxit=12, omega_idx=w.omega_idx)
+        ctx.set_opts(warm_start=True, ar_ref=ar0)
+        us2, al2, rs2, its2 = ctx.lsqr_sf_batch(d, w.lam, w.src_ijk, None, maxit=8, omega_idx=w.omega_idx,
+                                                out=(us.clone(), al.clone(),
+                                                     torch.empty((9, w.nb), dtype=torch.float32, device="cuda"),
+                                                     torch.empty(w.nb, dtype=torch.int32, device="cuda")))
+        ctx.set_opts()
+        torch.cuda.synchronize()
+        outs[mode] = [t.cpu().numpy() for t in (us, al, rs, us2, al2, rs2, ar0)]
+        if mode == "lockstep":
+            monkeypatch.delenv("WRI_NO_GROUPS")
+    for a, b in zip(outs["groups"], outs["lockstep"]):
+        assert rel(a, b) < 2e-5
+    assert np.all(outs["groups"][5][-1] < outs["groups"][2][-1])       # the continuation went on converging
+
+    # host entry
+    qh, dh = torch.from_numpy(w.Q).pin_memory(), torch.from_numpy(w.D).pin_memory()
+    uh, rh, ith = ctx.lsqr_batch_host(qh, dh, w.lam, None, maxit=K, omega_idx=w.omega_idx)
+    assert np.array_equal(uh.numpy(), u.cpu().numpy()) and np.array_equal(rh.numpy(), res.cpu().numpy())
