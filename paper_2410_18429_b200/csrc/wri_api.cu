@@ -32,7 +32,7 @@ inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 
 
 inline unsigned blocks_for(long long n) { return (unsigned)std::min<long long>((n + 255) / 256, 148 * 16); }
 constexpr int kMaxCtas = 512;          // upper bound on the persistent grid (>= SM count)
-constexpr int kMinChunk = 4;           // narrowest column chunk of the TMA path
+constexpr int kMinChunk = 2;           // narrowest column chunk of the TMA path
 
 struct Tiling {
     int vec;            // complex numbers per thread (2 = 128-bit accesses)
@@ -393,22 +393,37 @@ template <int MODE> struct CfgFor<8, MODE> {
 template <int MODE> struct CfgFor<4, MODE> {
     typedef TileCfg<4, 16, 16, (MODE == MODE_F ? WRI_F_NT : WRI_A_NT), PassTraits<MODE>::NSTAGE> type;
 };
+// 56 / 40 / 24 columns (widths a shrinking batch passes through): one item per consumer thread
+template <int MODE> struct CfgFor<56, MODE> {
+    typedef TileCfg<56, 4, 4, 448, (MODE == MODE_F ? PassTraits<MODE_F>::NSTAGE : WRI_A48_STAGES)> type;
+};
+template <int MODE> struct CfgFor<40, MODE> {
+    typedef TileCfg<40, 4, 4, 320, (MODE == MODE_F ? PassTraits<MODE_F>::NSTAGE : WRI_A48_STAGES)> type;
+};
+template <int MODE> struct CfgFor<24, MODE> {
+    typedef TileCfg<24, 8, 4, 384, (MODE == MODE_F ? PassTraits<MODE_F>::NSTAGE : WRI_A48_STAGES)> type;
+};
+// 2 columns (one 16-byte item per cell): 32 x 16 cells
+template <int MODE> struct CfgFor<2, MODE> {
+    typedef TileCfg<2, 32, 16, (MODE == MODE_F ? WRI_F_NT : WRI_A_NT), PassTraits<MODE>::NSTAGE> type;
+};
 
 int tma_chunk_for(int nb) {
     const char* off = getenv("WRI_NO_TMA");
     if (off && off[0] == '1') return 0;
     if (nb % 64 == 0) return 64;
+    if (nb == 56 || nb == 40 || nb == 24) return nb;
     if (nb % 48 == 0) return 48;
     if (nb % 32 == 0) return 32;
     if (nb % 16 == 0) return 16;
-    if (nb == 8 || nb == 4) return nb;
+    if (nb == 8 || nb == 4 || nb == 2) return nb;
     return 0;
 }
 
 template <class Cfg, int MODE>
 size_t tma_smem_bytes(const wri_ctx* c) {
     return (size_t)Cfg::NSTAGE *
-               (Cfg::IN_BYTES + PassTraits<MODE>::NSTREAM * Cfg::CTR_BYTES + Cfg::M_BYTES) +
+               (Cfg::IN_SPAN + PassTraits<MODE>::NSTREAM * Cfg::CTR_BYTES + Cfg::M_BYTES) +
            2 * Cfg::NSTAGE * 8 + (size_t)c->nb * 8 + (size_t)Cfg::NT * 2 * 8 +
            (size_t)(c->g.nx + c->g.ny + c->g.nz) * 4 + (size_t)6 * c->nb * 4;
 }
@@ -522,6 +537,18 @@ int tma_setup(wri_ctx* c) {
         case 4:
             if ((rc = tma_plan<CfgFor<4, MODE_F>::type>(c, c->planF, c->V, c->U, true))) return rc;
             return tma_plan<CfgFor<4, MODE_A>::type>(c, c->planA, c->U, c->V, false);
+        case 2:
+            if ((rc = tma_plan<CfgFor<2, MODE_F>::type>(c, c->planF, c->V, c->U, true))) return rc;
+            return tma_plan<CfgFor<2, MODE_A>::type>(c, c->planA, c->U, c->V, false);
+        case 56:
+            if ((rc = tma_plan<CfgFor<56, MODE_F>::type>(c, c->planF, c->V, c->U, true))) return rc;
+            return tma_plan<CfgFor<56, MODE_A>::type>(c, c->planA, c->U, c->V, false);
+        case 40:
+            if ((rc = tma_plan<CfgFor<40, MODE_F>::type>(c, c->planF, c->V, c->U, true))) return rc;
+            return tma_plan<CfgFor<40, MODE_A>::type>(c, c->planA, c->U, c->V, false);
+        case 24:
+            if ((rc = tma_plan<CfgFor<24, MODE_F>::type>(c, c->planF, c->V, c->U, true))) return rc;
+            return tma_plan<CfgFor<24, MODE_A>::type>(c, c->planA, c->U, c->V, false);
         default:
             if ((rc = tma_plan<CfgFor<16, MODE_F>::type>(c, c->planF, c->V, c->U, true))) return rc;
             return tma_plan<CfgFor<16, MODE_A>::type>(c, c->planA, c->U, c->V, false);
@@ -630,6 +657,10 @@ int launch_tma(wri_ctx* c, int phase) {
         case 32: return launch_tma_cfg<typename CfgFor<32, MODE>::type, MODE>(c, phase);
         case 8: return launch_tma_cfg<typename CfgFor<8, MODE>::type, MODE>(c, phase);
         case 4: return launch_tma_cfg<typename CfgFor<4, MODE>::type, MODE>(c, phase);
+        case 2: return launch_tma_cfg<typename CfgFor<2, MODE>::type, MODE>(c, phase);
+        case 56: return launch_tma_cfg<typename CfgFor<56, MODE>::type, MODE>(c, phase);
+        case 40: return launch_tma_cfg<typename CfgFor<40, MODE>::type, MODE>(c, phase);
+        case 24: return launch_tma_cfg<typename CfgFor<24, MODE>::type, MODE>(c, phase);
         default: return launch_tma_cfg<typename CfgFor<16, MODE>::type, MODE>(c, phase);
     }
 }
@@ -965,7 +996,7 @@ int wri_objective_gradient(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host
     // TMA pipeline when the batch is one power-of-two chunk per cell (64 / 32 / 16 / 8 / 4 columns);
     // the generic kernel otherwise (odd widths, 48, several chunks)
     int cb = tma_chunk_for(nb);
-    if (cb == 48 || cb != nb || !get_encode_fn() || getenv("WRI_GRAD_GENERIC")) cb = 0;
+    if ((cb & (cb - 1)) || cb == 2 || cb != nb || !get_encode_fn() || getenv("WRI_GRAD_GENERIC")) cb = 0;
     int n_rows = (int)G.t.n_tiles;
     if (cb) {
         c->nb = nb;
@@ -1159,10 +1190,10 @@ int retire_columns(wri_ctx* c, const std::vector<int>& src, const std::vector<in
     return WRI_OK;
 }
 
-// working widths the TMA path serves: 4, 8, then multiples of 16
-int round_up16(int n) { return n <= 4 ? 4 : n <= 8 ? 8 : (n + 15) / 16 * 16; }
+// working widths the TMA path serves: 2, 4, multiples of 8 up to 64, then multiples of 16
+int round_up16(int n) { return n <= 2 ? 2 : n <= 4 ? 4 : n <= 64 ? (n + 7) / 8 * 8 : (n + 15) / 16 * 16; }
 
-// Re-pack the working set to the columns still active (plus zero padding up to a multiple of 16).
+// Re-pack the working set to the columns still active (plus zero padding up to the next supported width).
 int compact_columns(wri_ctx* c, const int* act) {
     std::vector<int> keep, rs, rd;
     for (int j = 0; j < c->nb; ++j) {
@@ -1215,7 +1246,7 @@ int compact_columns(wri_ctx* c, const int* act) {
 }
 
 // host look at the active flags: early exit when every column has stopped, compaction when the
-// active count has dropped below the next multiple of 16
+// active count has dropped below the next supported width
 int check_active(wri_ctx* c) {
     CK(cudaMemcpyAsync(c->h_active, c->active, c->nb * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));

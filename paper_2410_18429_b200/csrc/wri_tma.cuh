@@ -30,12 +30,13 @@ struct TileCfg {
     static constexpr int NSTAGE = NSTAGE_;                      // LARGEST depth of the shared-memory ring (p.nstage <= NSTAGE is used)
     static constexpr int ITEMS = TXC * TYC * CB / 2;            // 16-byte items per plane
     static constexpr int IPT = ITEMS / NT;                      // items per thread
-    static constexpr int IN_BYTES = (TXC + 2) * (TYC + 2) * CB * 8;
+    static constexpr int IN_BYTES = (TXC + 2) * (TYC + 2) * CB * 8;   // bytes the halo box delivers
+    static constexpr int IN_SPAN = (IN_BYTES + 127) / 128 * 128;       // room it takes in a stage (TMA destinations: 128 B)
     static constexpr int CTR_BYTES = TXC * TYC * CB * 8;
     static constexpr int M_BYTES = (TXC * TYC * 4 + 127) / 128 * 128;   // model tile (float per cell)
     static_assert(ITEMS % NT == 0, "tile must give every consumer thread the same work");
     static_assert(NT % (CB / 2) == 0, "a thread must keep one column pair");
-    static_assert(IN_BYTES % 128 == 0 && CTR_BYTES % 128 == 0, "TMA destinations need 128 B alignment");
+    static_assert(CTR_BYTES % 128 == 0, "TMA destinations need 128 B alignment");
 };
 
 struct TrueT { static constexpr bool value = true; };
@@ -190,7 +191,7 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
            const __grid_constant__ CUtensorMap tm_m, const TmaPassParams p) {
     constexpr int CB = Cfg::CB, TXC = Cfg::TXC, TYC = Cfg::TYC, NT = Cfg::NT, IPT = Cfg::IPT;
     constexpr int NSTREAM = PassTraits<MODE>::NSTREAM, NSTAGE = Cfg::NSTAGE;
-    constexpr int M_OFF = Cfg::IN_BYTES + NSTREAM * Cfg::CTR_BYTES;
+    constexpr int M_OFF = Cfg::IN_SPAN + NSTREAM * Cfg::CTR_BYTES;
     constexpr int STAGE_BYTES = M_OFF + Cfg::M_BYTES;
     constexpr int HP = CB / 2;                                  // column pairs per cell
     constexpr int ROW_B = (TXC + 2) * CB * 8;                   // bytes per halo-tile row
@@ -267,17 +268,17 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
                     if (streams) {
 #if WRI_HINTS >= 1
                         if (old_stream)
-                        tma_load_4d_hint(dst + Cfg::IN_BYTES, &tm_old, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1, pol_stream);
+                        tma_load_4d_hint(dst + Cfg::IN_SPAN, &tm_old, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1, pol_stream);
                         if (MODE == MODE_F) {
-                            tma_load_4d_hint(dst + Cfg::IN_BYTES + Cfg::CTR_BYTES, &tm_w, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1, pol_stream);
-                            tma_load_4d_hint(dst + Cfg::IN_BYTES + 2 * Cfg::CTR_BYTES, &tm_x, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1, pol_stream);
+                            tma_load_4d_hint(dst + Cfg::IN_SPAN + Cfg::CTR_BYTES, &tm_w, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1, pol_stream);
+                            tma_load_4d_hint(dst + Cfg::IN_SPAN + 2 * Cfg::CTR_BYTES, &tm_x, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1, pol_stream);
                         }
 #else
                         if (old_stream)
-                        tma_load_4d(dst + Cfg::IN_BYTES, &tm_old, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1);
+                        tma_load_4d(dst + Cfg::IN_SPAN, &tm_old, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1);
                         if (MODE == MODE_F) {
-                            tma_load_4d(dst + Cfg::IN_BYTES + Cfg::CTR_BYTES, &tm_w, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1);
-                            tma_load_4d(dst + Cfg::IN_BYTES + 2 * Cfg::CTR_BYTES, &tm_x, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1);
+                            tma_load_4d(dst + Cfg::IN_SPAN + Cfg::CTR_BYTES, &tm_w, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1);
+                            tma_load_4d(dst + Cfg::IN_SPAN + 2 * Cfg::CTR_BYTES, &tm_x, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1);
                         }
 #endif
                         if (p.m_tma) tma_load_3d(dst + M_OFF, &tm_m, fb, x0, y0, pl - 1);
@@ -405,7 +406,7 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
                     n_new[j] = make_float4((a.x + b.x) + (c.x + d.x), (a.y + b.y) + (c.y + d.y),
                                            (a.z + b.z) + (c.z + d.z), (a.w + b.w) + (c.w + d.w));
                     if (emit) {
-                        const int io = Cfg::IN_BYTES + (tid + j * NT) * 16;
+                        const int io = Cfg::IN_SPAN + (tid + j * NT) * 16;
                         o_old[j] = HAS_OLD ? lds128(sb, io) : make_float4(0.f, 0.f, 0.f, 0.f);
                         if (M_TMA)
                             m_cur[j] = *reinterpret_cast<const float*>(sb + M_OFF + (cyj[j] * TXC + cxj[j]) * 4);
@@ -491,7 +492,7 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
                                 acc32[0] += fmaf(rr.x, rr.x, rr.y * rr.y);
                                 acc32[1] += fmaf(rr.z, rr.z, rr.w * rr.w);
                                 if (MODE == MODE_F) {
-                                    const int io = Cfg::IN_BYTES + (tid + j * NT) * 16;
+                                    const int io = Cfg::IN_SPAN + (tid + j * NT) * 16;
                                     o_w[j] = lds128(sb, io + Cfg::CTR_BYTES);
                                     o_x[j] = lds128(sb, io + 2 * Cfg::CTR_BYTES);
                                     float4 xn, wn;
