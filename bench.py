@@ -204,7 +204,8 @@ def run_ours(args, wl_name, w):
         raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-    use_dist = world > 1
+    # WRI_BENCH_DIST1=1 (developer switch): take the N > 1 code path with one rank under torchrun
+    use_dist = world > 1 or os.environ.get("WRI_BENCH_DIST1") == "1"
     if use_dist:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
@@ -315,6 +316,32 @@ def run_ours(args, wl_name, w):
                                        "value": it_m / s_m, "unit": UNIT, "f": mf["f"],
                                        "timing": "host wall clock around wri_misfit_sf (it ends with a stream sync)"}
         del u_sf, g, mf
+
+    # ---- N > 1: the misfit of all ranks' columns with its one collective, the all-reduce of the
+    #      gradient and the objective (eq. 8-9 are sums over sources and frequencies); context line
+    if use_dist and not args.no_extras and w.src_ijk is not None:
+        try:
+            from paper_2410_18429_b200.sharded import ShardedMisfit
+
+            def evaluate(lo, hi, eps, mit, g, warm):          # every rank owns one nb-column group
+                o = ctx.misfit_sf(d, w.lam, w.src_ijk, eps, mit, omega_idx=w.omega_idx, g=g)
+                return o["f"], int(o["iters"].sum().item()), None
+
+            sm = ShardedMisfit(nb * world, evaluate, w.ng, dev, dist)
+            sm.misfit(1e-2, maxit)                               # warm-up (NCCL communicator, workspace)
+            barrier()
+            t0 = time.perf_counter()
+            f_all, g_all, it_all, _ = sm.misfit(1e-2, maxit)
+            barrier()
+            s_sm = time.perf_counter() - t0
+            extras = extras or {}
+            extras["sharded_misfit"] = {"ms": s_sm * 1e3, "eps": 1e-2, "columns": nb * world,
+                                        "lsqr_iterations_x_sources": it_all, "value": it_all / s_sm, "unit": UNIT,
+                                        "f": f_all, "collective": "all-reduce of g (float32 [n_g]) and f over NCCL",
+                                        "g_norm": float(g_all.double().norm().item())}
+        except Exception as e:                                   # a context line must never cost the bench line
+            extras = extras or {}
+            extras["sharded_misfit"] = {"error": repr(e)}
 
     (ms, e2e_s), (iters_all, iters_e2e_all, launches_all) = reduce_over_ranks(
         [ms, e2e_s], [iters_per_step, iters_e2e, launches], dist if use_dist else None, dev)

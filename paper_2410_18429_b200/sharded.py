@@ -1,0 +1,104 @@
+"""Column sharding of the misfit evaluation over N ranks (one process per GPU, torch.distributed).
+
+The systems S_ij are independent across sources and frequencies, so every rank
+solves its own block of batch columns with no exchange inside LSQR.  The objective and the gradient
+are SUMS over sources and frequencies (eq. 8-9): one all-reduce of the float32
+[n_g] gradient and of the objective per misfit evaluation is the only collective of the method
+(NCCL over NVLink on GPUs; 8 MB at 128^3 against >= 60 ms of solves, so it is not fused into a
+kernel).  Every rank ends up with the same f and g, hence takes the same accept / reject decision
+in Algorithm 2 without further communication.
+
+Plumbing only: the arithmetic of a rank's block runs in libwri (Wri.misfit_sf); `evaluate` is
+injectable so that the reduction logic can be exercised on CPU ranks (gloo) in the tests.
+"""
+from __future__ import annotations
+
+
+def column_range(nb: int, rank: int, world: int):
+    """Contiguous block [lo, hi) of the nb batch columns owned by `rank`; blocks differ by at most one."""
+    base, rem = divmod(int(nb), int(world))
+    lo = rank * base + min(rank, rem)
+    return lo, lo + base + (1 if rank < rem else 0)
+
+
+class ShardedMisfit:
+    """f4(m) = sum over ALL columns of 1/2 ||S x_bar - b||^2 and its gradient on N ranks.
+
+    evaluate(lo, hi, eps, maxit, g, warm) -> (f_local: float, iters_local: int, state)
+        the rank-local misfit of columns [lo, hi): adds the block's gradient into g (a float32
+        [n_g] tensor on the rank's device, cleared by this class) and returns the block's objective;
+        `warm` is the state a previous call returned (or None), for warm restarts.
+    dist: torch.distributed (initialised) or None for a single process.
+    """
+
+    def __init__(self, nb_total, evaluate, n_g, device, dist=None):
+        import torch
+        self._t = torch
+        self.dist = dist if (dist is not None and dist.is_initialized()) else None
+        self.rank = self.dist.get_rank() if self.dist else 0
+        self.world = self.dist.get_world_size() if self.dist else 1
+        self.nb_total = int(nb_total)
+        self.lo, self.hi = column_range(nb_total, self.rank, self.world)
+        self.evaluate = evaluate
+        self.g = torch.zeros(int(n_g), dtype=torch.float32, device=device)
+
+    def misfit(self, eps, maxit, want_gradient=True, warm=None):
+        """Returns (f, g, iters, state): f and iters summed over all ranks, g all-reduced in place
+        (None when want_gradient is False), state = this rank's warm-start state."""
+        t = self._t
+        g = self.g if want_gradient else None
+        if g is not None:
+            g.zero_()
+        if self.hi > self.lo:
+            f_loc, it_loc, state = self.evaluate(self.lo, self.hi, eps, maxit, g, warm)
+        else:
+            f_loc, it_loc, state = 0.0, 0, None              # more ranks than columns
+        if self.dist:
+            s = t.tensor([float(f_loc), float(it_loc)], dtype=t.float64, device=self.g.device)
+            self.dist.all_reduce(s, op=self.dist.ReduceOp.SUM)
+            if g is not None:
+                self.dist.all_reduce(g, op=self.dist.ReduceOp.SUM)
+            f_loc, it_loc = float(s[0]), int(round(float(s[1])))
+        return float(f_loc), g, int(it_loc), state
+
+    def awri_step(self, m, eps, maxit, update, set_model, max_halvings=8, warm_restart=False):
+        """Lines 4-14 of Algorithm 2 with the sums of lines 5 and 8 taken over all ranks.
+
+        m: this rank's replica of the model (a tensor, updated in place when the step is accepted);
+        update(m, g, m_trial) fills m_trial; set_model(tensor) points the rank's solver at a model.
+        Every rank computes the same f, f_trial and therefore the same decision.  Returns a dict
+        like Wri.awri_step (accepted, n_halvings, eps, f, f_trial, lsqr_iters, trace)."""
+        m_trial = m.clone()
+        trace, total, state = [], 0, None
+        accepted = False
+        f = ft = 0.0
+        h = 0
+        for h in range(int(max_halvings) + 1):
+            set_model(m)
+            f, g, it0, state = self.misfit(eps, maxit, True, state if (warm_restart and h > 0) else None)
+            update(m, g, m_trial)
+            set_model(m_trial)
+            ft, _, it1, _ = self.misfit(eps, maxit, False, None)
+            set_model(m)
+            total += it0 + it1
+            trace.append((eps, f, ft))
+            if not (ft > f):
+                m.copy_(m_trial)
+                accepted = True
+                break
+            if h == max_halvings:
+                break
+            eps *= 0.5
+        return dict(accepted=accepted, n_halvings=h, eps=eps, f=f, f_trial=ft, lsqr_iters=total, trace=trace)
+
+
+def wri_evaluator(ctx, d, lam, src_ijk, omega_idx):
+    """evaluate() for ShardedMisfit on a GPU rank: Wri.misfit_sf on the rank's block of columns.
+    d [n_rec, nb_total] (complex64, device), src_ijk [nb_total, 3], omega_idx [nb_total]."""
+
+    def evaluate(lo, hi, eps, maxit, g, warm):
+        out = ctx.misfit_sf(d[:, lo:hi].contiguous(), lam, src_ijk[lo:hi], eps, maxit,
+                            omega_idx=None if omega_idx is None else omega_idx[lo:hi], g=g, warm=warm)
+        return out["f"], int(out["iters"].sum().item()), (out["u"], out["alpha"], out["ar0"])
+
+    return evaluate
