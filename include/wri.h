@@ -168,6 +168,15 @@ int wri_objective_gradient(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_ho
                            const void* u_dev, const void* d_dev, float lambda,
                            double* f_pde_dev, double* f_data_dev, float* g_dev);
 
+/* Per-source receiver sets P_i ("P_i is the restriction operator for source i").
+ * mask_dev: uint8 [n_rec][nb], 1 = receiver r records batch column s, 0 = that row is absent from
+ * P_s: its entry of P_s v is 0, its datum d[r][s] is ignored, P_s^T adds nothing there.  Sticky for
+ * every later call of batch width nb (apply, solve, objective / gradient, misfit); other widths are
+ * refused with WRI_ERR_ARG while a mask is set; NULL restores "every receiver records every column"
+ * (the default, north_star's shared P).  The array is BORROWED: it must stay valid and unchanged
+ * while calls that use it are in flight.                                                        */
+int wri_set_receiver_mask(wri_ctx* ctx, int32_t nb, const uint8_t* mask_dev);
+
 /* Options of the solves that follow (all wri_lsqr_* / wri_lsqr_sf_* begin and batch entries);
  * sticky until set again, NULL restores the defaults (all zero).
  *   warm_start   1: u_out_dev (and alpha_out_dev) hold x0 (alpha0) on entry.  Algorithm 1 leaves

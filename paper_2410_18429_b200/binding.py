@@ -102,6 +102,7 @@ def load_library():
     lib.wri_lsqr_sf_batch_host.argtypes = solve_sf
     lib.wri_objective_gradient.argtypes = [P, I32, P, P, P, P, P, P, F32, P, P, P]
     lib.wri_lsqr_set_opts.argtypes = [P, C.POINTER(wri_lsqr_opts)]
+    lib.wri_set_receiver_mask.argtypes = [P, I32, P]
     lib.wri_misfit_sf.argtypes = [P, I32, P, P, P, F32, F32, I32, I32, P, P, P, P, P, P, P, P]
     lib.wri_awri_step.argtypes = [P, I32, P, P, P, F32, F32, I32, C.POINTER(wri_awri_opts), P, P, P, P, P, P, P,
                                   P, C.POINTER(wri_awri_report)]
@@ -295,6 +296,11 @@ class Wri:
         self._opt_keep = (ar_ref, ar0_out)
         o = wri_lsqr_opts(int(bool(warm_start)), _dptr(ar_ref), _dptr(ar0_out))
         _ck(self._lib.wri_lsqr_set_opts(self._h, C.byref(o)))
+
+    def set_receiver_mask(self, mask):
+        """Per-source receiver sets: mask uint8 [n_rec, nb] CUDA tensor (1 = recorded), None = all."""
+        self._rmask_keep = mask
+        _ck(self._lib.wri_set_receiver_mask(self._h, 0 if mask is None else int(mask.shape[1]), _dptr(mask)))
 
     # ---- source-free system (unknown source weight per column)
     def lsqr_sf_batch(self, d, lam, src_ijk, tol=None, maxit=50, omega_idx=None, q=None, out=None):

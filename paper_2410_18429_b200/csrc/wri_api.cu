@@ -72,6 +72,8 @@ struct wri_ctx {
     bool sf = false;             // the solve in flight has the extra source-weight unknown
     float2* alpha_out = nullptr; // caller's [nb] source-weight estimates (source-free system)
     wri_lsqr_opts opts{};        // warm start / stop-rule reference for the next solves (wri_lsqr_set_opts)
+    const unsigned char* rmask = nullptr;   // per-source receiver sets [n_rec][rmask_nb] (wri_set_receiver_mask)
+    int rmask_nb = 0;
     int* colmap = nullptr;       // [nb_max] working column -> caller's column (-1 = padding)
     int* idx = nullptr;          // [3][nb_max] scratch: gather map | retire source | retire destination
     int* h_active = nullptr;     // pinned host copy of the active flags
@@ -575,6 +577,7 @@ ScalParams scal_params(const wri_ctx* c, const double* partials, int n_rows, con
     s.X = c->X;
     s.ar_ref = c->opts.ar_ref_dev;
     s.ar0_out = c->opts.ar0_out_dev;
+    s.rmask = c->rmask;
     return s;
 }
 
@@ -707,6 +710,7 @@ int launch_tma_grad(wri_ctx* c, const float2* u, const float2* q, const int* src
 int check_batch_args(const wri_ctx* c, int nb) {
     if (!c) return WRI_ERR_ARG;
     if (nb <= 0 || nb > c->nb_max) return WRI_ERR_ARG;
+    if (c->rmask && c->rmask_nb != nb) return WRI_ERR_ARG;       // the receiver mask was given for another width
     if ((long long)c->ng * nb > 0x7fffffffLL * 1LL) return WRI_ERR_ARG;   // element indices stay below 2^31
     return WRI_OK;
 }
@@ -861,6 +865,14 @@ int wri_set_workspace(wri_ctx* c, void* ws_dev, size_t bytes) {
     return WRI_OK;
 }
 
+int wri_set_receiver_mask(wri_ctx* c, int32_t nb, const uint8_t* mask_dev) {
+    if (!c || (mask_dev && (nb <= 0 || nb > c->nb_max))) return WRI_ERR_ARG;
+    if (c->solving) return WRI_ERR_STATE;
+    c->rmask = mask_dev;
+    c->rmask_nb = mask_dev ? nb : 0;
+    return WRI_OK;
+}
+
 int wri_lsqr_set_opts(wri_ctx* c, const wri_lsqr_opts* opts) {
     if (!c) return WRI_ERR_ARG;
     if (c->solving) return WRI_ERR_STATE;
@@ -907,7 +919,7 @@ int wri_apply_M(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, float lam
     if (c->n_rec) {
         const long long n = (long long)c->n_rec * nb;
         k_gather<<<(unsigned)std::min<long long>((n + 255) / 256, 1184), 256, 0, c->stream>>>(
-            (const float2*)x_dev, c->rec, c->n_rec, nb, (float2*)ybot_dev);
+            (const float2*)x_dev, c->rec, c->n_rec, nb, (float2*)ybot_dev, c->rmask);
         c->launches++;
         CK(cudaGetLastError());
     }
@@ -930,7 +942,7 @@ int wri_apply_MH(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, float la
     if (c->n_rec) {
         const long long n = (long long)c->n_rec * nb;
         k_scatter_add<<<(unsigned)std::min<long long>((n + 255) / 256, 1184), 256, 0, c->stream>>>(
-            (float2*)x_dev, c->rec, c->n_rec, nb, (const float2*)ybot_dev);
+            (float2*)x_dev, c->rec, c->n_rec, nb, (const float2*)ybot_dev, c->rmask);
         c->launches++;
         CK(cudaGetLastError());
     }
@@ -1028,7 +1040,7 @@ int wri_objective_gradient(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host
     k_objective<<<(nb + OBJ_CPB - 1) / OBJ_CPB, 1024, 1024 * sizeof(double), c->stream>>>(p.partials, n_rows, nb, p.u,
                                                              (const float2*)d_dev, c->rec, c->n_rec,
                                                              (double)lambda * (double)lambda, f_pde_dev,
-                                                             f_data_dev);
+                                                             f_data_dev, c->rmask);
     c->launches++;
     CK(cudaGetLastError());
     return WRI_OK;

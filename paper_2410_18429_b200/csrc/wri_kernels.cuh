@@ -211,24 +211,27 @@ k_pass(const PassParams p) {
 // ---------------------------------------------------------------------------------------------
 // Receiver rows (P and P^T are exact indexing).
 
+// Per-source receiver sets P_s ("P_i"): rmask[r][s] = 1 when receiver r records column s,
+// 0 when that row is absent from P_s (its entry of P_s v is 0 and its datum is ignored); null = all.
 // ybot[r][s] = x[rec[r]][s]            (bit-exact copy)
 __global__ void k_gather(const float2* __restrict__ x, const int* __restrict__ rec, int n_rec, int nb,
-                         float2* __restrict__ ybot) {
+                         float2* __restrict__ ybot, const unsigned char* __restrict__ rmask) {
     const long long n = (long long)n_rec * nb;
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
          i += (long long)gridDim.x * blockDim.x) {
         const int r = (int)(i / nb), s = (int)(i - (long long)r * nb);
-        ybot[i] = x[(size_t)rec[r] * nb + s];
+        ybot[i] = (!rmask || rmask[i]) ? x[(size_t)rec[r] * nb + s] : make_float2(0.f, 0.f);
     }
 }
 
 // x[rec[r]][s] += ybot[r][s]           (receivers are unique, so this is race-free)
 __global__ void k_scatter_add(float2* __restrict__ x, const int* __restrict__ rec, int n_rec, int nb,
-                              const float2* __restrict__ ybot) {
+                              const float2* __restrict__ ybot, const unsigned char* __restrict__ rmask) {
     const long long n = (long long)n_rec * nb;
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
          i += (long long)gridDim.x * blockDim.x) {
         const int r = (int)(i / nb), s = (int)(i - (long long)r * nb);
+        if (rmask && !rmask[i]) continue;
         float2* d = x + (size_t)rec[r] * nb + s;
         const float2 a = *d, b = ybot[i];
         *d = make_float2(a.x + b.x, a.y + b.y);
@@ -308,6 +311,7 @@ struct ScalParams {
     const float2* X;          // [n_g][nb] x0 (PH_INIT_B: receiver rows of the residual)
     const double* ar_ref;     // [nb] or null: arnorm_k <= tol * ar_ref instead of tol * alpha1 beta1
     double* ar0_out;          // [nb] or null: alpha1 beta1 of this solve
+    const unsigned char* rmask;   // [n_rec][nb_out] per-source receiver sets by the CALLER's column, or null
 };
 
 // sum over tiles of partials[.][s] in fixed order; result for column s in colsum[s] (shared)
@@ -389,6 +393,7 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
                 const float2 xv = p.X[(size_t)p.rec[r] * nb + s];
                 dv = make_float2(dv.x - xv.x, dv.y - xv.y);
             }
+            if (p.rmask && so >= 0 && !p.rmask[(size_t)r * p.nb_out + so]) dv = make_float2(0.f, 0.f);
             p.U_bot[i] = dv;
         }
         __syncthreads();
@@ -400,7 +405,9 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
             const float cv = cf[C_CV_F * NM + s], cb = cf[C_CB_F * NM + s];
             const float2 v = p.V[(size_t)p.rec[r] * nb + s];
             const float2 u = p.U_bot[i];
-            p.U_bot[i] = make_float2(fmaf(cv, v.x, -cb * u.x), fmaf(cv, v.y, -cb * u.y));
+            const int so = p.colmap ? p.colmap[s] : s;
+            const bool on = !p.rmask || so < 0 || p.rmask[(size_t)r * p.nb_out + so];
+            p.U_bot[i] = on ? make_float2(fmaf(cv, v.x, -cb * u.x), fmaf(cv, v.y, -cb * u.y)) : make_float2(0.f, 0.f);
         }
         __syncthreads();
     }
@@ -779,7 +786,7 @@ constexpr int OBJ_CPB = 8;
 __global__ void __launch_bounds__(1024)
 k_objective(const double* __restrict__ partials, int n_tiles, int nb, const float2* __restrict__ u,
             const float2* __restrict__ d, const int* __restrict__ rec, int n_rec, double lam2,
-            double* __restrict__ f_pde, double* __restrict__ f_data) {
+            double* __restrict__ f_pde, double* __restrict__ f_data, const unsigned char* __restrict__ rmask) {
     extern __shared__ double sh_obj[];                       // [blockDim.x]
     const int T = blockDim.x;
     const int base = blockIdx.x * OBJ_CPB;
@@ -801,6 +808,7 @@ k_objective(const double* __restrict__ partials, int n_tiles, int nb, const floa
                 for (; b < n_tiles; b += Gc) a += __ldcg(partials + (size_t)b * nb + s);
             } else {
                 for (int r = g; r < n_rec; r += Gc) {
+                    if (rmask && !rmask[(size_t)r * nb + s]) continue;
                     const float2 uv = u[(size_t)rec[r] * nb + s], dv = d[(size_t)r * nb + s];
                     const double er = (double)uv.x - (double)dv.x, ei = (double)uv.y - (double)dv.y;
                     a += er * er + ei * ei;

@@ -328,7 +328,11 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
                     const float2 v = __ldcg(p.V + (size_t)p.rec[r] * nb + s);
                     const float2 u = __ldcg(p.U_bot + e);
                     const float cvs = tab_c[3 * nb + s], cbs = tab_c[2 * nb + s];
-                    const float2 n = make_float2(fmaf(cvs, v.x, -cbs * u.x), fmaf(cvs, v.y, -cbs * u.y));
+                    float2 n = make_float2(fmaf(cvs, v.x, -cbs * u.x), fmaf(cvs, v.y, -cbs * u.y));
+                    if (p.fin.rmask) {                                  // per-source receiver sets
+                        const int so = p.fin.colmap ? p.fin.colmap[s] : s;
+                        if (so >= 0 && !p.fin.rmask[(size_t)r * p.fin.nb_out + so]) n = make_float2(0.f, 0.f);
+                    }
                     p.U_bot[e] = n;
                     return (double)fmaf(n.x, n.x, n.y * n.y);
                 },
