@@ -86,8 +86,8 @@ def test_config2_128cubed_x64src_50_iterations(torch_cuda):
 
 
 def test_config2_128cubed_x192col_three_frequencies(torch_cuda):
-    """configs[2] in full: 64 sources x {4, 6, 8} Hz in one 192-column batch (three 64-column
-    chunks per cell); one column per frequency against the oracle, 25 iterations."""
+    """configs[2] in full: 64 sources x {4, 6, 8} Hz in one 192-column batch (solved as three compact
+    64-column groups); one column per frequency against the oracle, 25 iterations."""
     w = workloads.make("config2")
     assert w.nb == 192 and len(set(w.omega_idx.tolist())) == 3
     _fixed_k_case(torch_cuda, w, 25, [5, 100, 191], threads=3)
@@ -150,4 +150,64 @@ def test_config3_vsp_adaptive_full_size(torch_cuda):
         assert abs(k - k_ref) <= 2, (s, k, k_ref)
         assert rel(resh[:k + 1, s], same["resnorms"][:k + 1]) < 1e-3, s
         assert rel(u[:, s].cpu().numpy(), same["x"]) < 1e-3, s
+    ctx.close()
+
+
+def test_config2_128cubed_x64src_source_free_and_misfit(torch_cuda):
+    """The headline grid and batch width through the paper's own system (source weight unknown,
+    b = [0; d]) and one misfit evaluation (solve to a tolerance + eq. 8-9), in bench.py's launch
+    configuration.  Sampled columns against the oracle where complex64 can follow it (k <= 3, C-16);
+    every column through oracle-independent properties; the group gradient against the oracle's
+    eq. 9 evaluated on the GPU's own wavefields (all 64 columns)."""
+    torch = torch_cuda
+    w = workloads.make("config2", freqs=(6.0,))
+    ctx = _wri(w)
+    rec = O.rec_cells(w.nx, w.ny, w.nz, w.rec_ijk)
+    srcc = O.rec_cells(w.nx, w.ny, w.nz, w.src_ijk)
+    ops = ops_for(w)
+    d = torch.from_numpy(w.D).cuda()
+    m64 = w.m.astype(np.float64)
+    # three free-running iterations: x and the history follow the oracle
+    u3, a3, res3, _ = ctx.lsqr_sf_batch(d, w.lam, w.src_ijk, None, maxit=3, omega_idx=w.omega_idx)
+    torch.cuda.synchronize()
+    cols = [0, 31, 63]
+    for s in cols:
+        r = O.lsqr_sf(ops[s], m64, w.lam, rec, int(srcc[s]), w.D[:, s], tol=0.0, maxit=3)
+        assert rel(res3[:, s].cpu().numpy(), r["resnorms"]) < 1e-3, s
+        assert rel(u3[:, s].cpu().numpy(), r["x"]) < 1e-3, s
+        assert abs(complex(a3[s].item()) - r["alpha_src"]) <= 1e-3 * abs(r["alpha_src"]), s
+    # misfit evaluation at eps = 1e-2
+    eps, maxit = 1e-2, 200
+    g = torch.zeros(w.ng, dtype=torch.float32, device="cuda")
+    out = ctx.misfit_sf(d, w.lam, w.src_ijk, eps, maxit, omega_idx=w.omega_idx, g=g)
+    it = out["iters"].cpu().numpy()
+    assert it.min() >= 1 and it.max() < maxit
+    f_cols = (out["f_pde"] + out["f_data"]).cpu().numpy()
+    assert out["f"] == pytest.approx(float(f_cols.sum()), rel=1e-12)
+    u, al = out["u"].cpu().numpy(), out["alpha"].cpu().numpy()
+    gsum = np.zeros(w.ng)
+
+    def one(s):
+        gs = np.zeros(w.ng)
+        fp, fd = O.objective_gradient(ops[s], m64, w.lam, rec, u[:, s].astype(complex), w.D[:, s],
+                                      src=int(srcc[s]), alpha_src=complex(al[s]), g=gs)
+        return s, fp + fd, gs
+
+    from concurrent.futures import ThreadPoolExecutor
+    with ThreadPoolExecutor(8) as ex:
+        for s, f_true, gs in ex.map(one, range(w.nb)):
+            assert f_cols[s] == pytest.approx(f_true, rel=1e-5), s          # honest objective, every column
+            gsum += gs
+    assert rel(g.cpu().numpy(), gsum) < 1e-5
+    # the stop rule holds in oracle arithmetic (sampled columns), and the oracle stops in the same band
+    ar0 = out["ar0"].cpu().numpy()
+    for s in cols:
+        t, b = O.apply_S(ops[s], m64, w.lam, rec, int(srcc[s]), u[:, s].astype(complex), complex(al[s]))
+        xu, xa = O.apply_SH(ops[s], m64, w.lam, rec, int(srcc[s]), -t, w.D[:, s].astype(complex) - b)
+        ar_true = float(np.sqrt(np.vdot(xu, xu).real + abs(xa) ** 2))
+        assert ar_true <= 1.05 * eps * ar0[s], s
+        r = O.lsqr_sf(ops[s], m64, w.lam, rec, int(srcc[s]), w.D[:, s], tol=eps, maxit=maxit)
+        assert abs(int(it[s]) - r["iters"]) <= max(2, int(0.4 * r["iters"])), (s, it[s], r["iters"])
+        assert f_cols[s] == pytest.approx(0.5 * r["resnorms"][r["iters"]] ** 2, rel=5e-3), s
+        assert ar0[s] == pytest.approx(r["arnorms"][0], rel=1e-5), s
     ctx.close()
