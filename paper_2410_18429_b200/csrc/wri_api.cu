@@ -9,6 +9,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <utility>
 #include <vector>
 
 using namespace wri;
@@ -122,6 +123,7 @@ struct wri_ctx {
     std::vector<int> ev_kind;             // per pair: 0 = pass F, 1 = pass A
     std::vector<int> ev_cols;             // per pair: working batch width of that launch
     size_t ev_used = 0;                   // pairs in use
+    std::vector<std::pair<const void*, size_t>> smem_ok;   // kernels already granted their dynamic smem size
 };
 
 namespace {
@@ -422,6 +424,21 @@ int tma_chunk_for(int nb) {
     return 0;
 }
 
+// opt-in to > 48 KB of dynamic shared memory, once per (context, kernel, size): the attribute is per
+// device, so it is not cached in a process-wide static
+int allow_smem(wri_ctx* c, const void* fn, size_t bytes) {
+    for (auto& e : c->smem_ok)
+        if (e.first == fn) {
+            if (e.second >= bytes) return WRI_OK;
+            CK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+            e.second = bytes;
+            return WRI_OK;
+        }
+    CK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    c->smem_ok.emplace_back(fn, bytes);
+    return WRI_OK;
+}
+
 template <class Cfg, int MODE>
 size_t tma_smem_bytes(const wri_ctx* c) {
     return (size_t)Cfg::NSTAGE *
@@ -596,13 +613,10 @@ int ring_depth(int nchunk) {
 
 template <class Cfg, int MODE>
 int launch_tma_cfg(wri_ctx* c, int phase) {
-    static size_t attr_bytes = 0;
     const wri_ctx::TmaPlan& P = (MODE == MODE_F) ? c->planF : c->planA;
     const size_t smem = tma_smem_bytes<Cfg, MODE>(c);
-    if (smem > attr_bytes) {
-        CK(cudaFuncSetAttribute(k_pass_tma<Cfg, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_bytes = smem;
-    }
+    int rc_attr = allow_smem(c, (const void*)k_pass_tma<Cfg, MODE>, smem);
+    if (rc_attr) return rc_attr;
     const size_t NM = c->nb_max;
     TmaPassParams p{};
     p.m = c->m;
@@ -678,13 +692,9 @@ int launch_tma_grad(wri_ctx* c, const float2* u, const float2* q, const int* src
     typedef TileCfg<CB, CfgA::TXC, CfgA::TYC, WRI_F_NT, WRI_A_STAGES> Cfg;
     int rc = tma_plan<Cfg>(c, c->planG, u, q ? q : u, false, false);
     if (rc) return rc;
-    static size_t attr_bytes = 0;
     const wri_ctx::TmaPlan& P = c->planG;
     const size_t smem = tma_smem_bytes<Cfg, MODE_G>(c);
-    if (smem > attr_bytes) {
-        CK(cudaFuncSetAttribute(k_pass_tma<Cfg, MODE_G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_bytes = smem;
-    }
+    if ((rc = allow_smem(c, (const void*)k_pass_tma<Cfg, MODE_G>, smem))) return rc;
     const size_t NM = c->nb_max;
     TmaPassParams p{};
     p.m = c->m;
