@@ -304,6 +304,28 @@ def run_ours(args, wl_name, w):
                                         "achieved": bytes_g / (ms_g * 1e-3) / 1e9, "unit": "GB/s",
                                         "frac": bytes_g / (ms_g * 1e-3) / 1e9 / peak_g,
                                         "kernel": "k_grad + k_objective (eq. 9 fused with the stencil residual)"}
+        # the operator entries on their own (wri_apply_M / wri_apply_MH): read x, write y = 16 B per cell-column
+        ev2 = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+        yb = torch.empty((w.n_rec, nb), dtype=torch.complex64, device=dev)
+        ctx.apply_M(u_sf, w.lam, w.omega_idx); ctx.apply_MH(u_sf, yb, w.lam, w.omega_idx)
+        torch.cuda.synchronize()
+        n_ap = 5
+        ev2[0].record()
+        for _ in range(n_ap):
+            ctx.apply_M(u_sf, w.lam, w.omega_idx)
+        ev2[1].record()
+        ev2[2].record()
+        for _ in range(n_ap):
+            ctx.apply_MH(u_sf, yb, w.lam, w.omega_idx)
+        ev2[3].record()
+        torch.cuda.synchronize()
+        bytes_ap = (16 * nb + 4) * w.ng
+        for nm, a, b in (("apply_M", 0, 1), ("apply_MH", 2, 3)):
+            ms_ap = ev2[a].elapsed_time(ev2[b]) / n_ap
+            extras[nm] = {"ms": ms_ap, "algorithmic_bytes": bytes_ap, "achieved": bytes_ap / (ms_ap * 1e-3) / 1e9,
+                          "unit": "GB/s", "frac": bytes_ap / (ms_ap * 1e-3) / 1e9 / peak_g,
+                          "note": "includes the output allocation of the Python binding"}
+        del yb
         # one misfit evaluation (Algorithm 2 lines 4-5; the unit the paper times in Table 1):
         # source-free solve of every column to a tolerance + objective + gradient, one C-ABI call
         eps_m = 1e-2

@@ -629,6 +629,7 @@ int launch_tma_cfg(wri_ctx* c, int phase) {
     p.ih2 = (float)(1.0 / (c->h * c->h));
     p.m6ih2 = (float)(-6.0 / (c->h * c->h));
     p.phase = phase;
+    p.has_q = 1;                                   // the in-place (old) stream is there
     p.nstage = ring_depth<Cfg, MODE>(P.nchunk);
     p.m_tma = P.m_tma;
     p.merged = P.merged;
@@ -715,6 +716,70 @@ int launch_tma_grad(wri_ctx* c, const float2* u, const float2* q, const int* src
     c->launches++;
     CK(cudaGetLastError());
     return WRI_OK;
+}
+
+// out = lambda * A in (sgn = +1) or lambda * A^H in (sgn = -1) through the TMA pipeline: pass A's kernel
+// without its in-place stream, scalar phase and receiver rows.  No workspace is touched.
+template <int CB>
+int launch_tma_apply(wri_ctx* c, const float2* in, float2* out, float sgn) {
+    typedef typename CfgFor<CB, MODE_A>::type Cfg;
+    int rc = tma_plan<Cfg>(c, c->planG, in, in, false, false);
+    if (rc) return rc;
+    const wri_ctx::TmaPlan& P = c->planG;
+    const size_t smem = tma_smem_bytes<Cfg, MODE_A>(c);
+    if ((rc = allow_smem(c, (const void*)k_pass_tma<Cfg, MODE_A>, smem))) return rc;
+    const size_t NM = c->nb_max;
+    TmaPassParams p{};
+    p.m = c->m;
+    p.gx = c->gtab; p.gy = c->gtab + c->g.nx; p.gz = c->gtab + c->g.nx + c->g.ny;
+    p.w2 = c->coef + C_W2 * NM;
+    p.ca = c->coef + C_LAM * NM;
+    p.cb = p.cv = p.cx = p.cw = p.ca;                 // unused without the in-place stream
+    p.partials = nullptr; p.counter = c->counter;
+    p.nx = c->g.nx; p.ny = c->g.ny; p.nz = c->g.nz; p.nb = c->nb;
+    p.zc = P.zc; p.ntx = P.ntx; p.nty = P.nty; p.ntz = P.ntz;
+    p.nchunk = P.nchunk; p.n_tiles = P.tiles;
+    p.ih2 = (float)(1.0 / (c->h * c->h));
+    p.m6ih2 = (float)(-6.0 / (c->h * c->h));
+    p.sgn = sgn;
+    p.phase = -1; p.has_q = 0; p.n_rec = 0;
+    p.m_tma = P.m_tma; p.merged = P.merged;
+    p.nstage = ring_depth<Cfg, MODE_A>(P.nchunk);
+    p.out = out;
+    k_pass_tma<Cfg, MODE_A><<<P.grid, Cfg::NT + 32, smem, c->stream>>>(P.in, P.old, P.old, P.old, P.m, p);
+    c->launches++;
+    CK(cudaGetLastError());
+    return WRI_OK;
+}
+
+// operator part of wri_apply_M / _MH: TMA pipeline when the width has a tile configuration, else k_pass
+int apply_operator(wri_ctx* c, int nb, const float2* in, float2* out, float sgn) {
+    const int cb = (c->solving || getenv("WRI_APPLY_GENERIC") || !get_encode_fn()) ? 0 : tma_chunk_for(nb);
+    if (cb) {
+        const int nb_saved = c->nb;
+        c->nb = nb;
+        int rc;
+        switch (cb) {
+            case 64: rc = launch_tma_apply<64>(c, in, out, sgn); break;
+            case 56: rc = launch_tma_apply<56>(c, in, out, sgn); break;
+            case 48: rc = launch_tma_apply<48>(c, in, out, sgn); break;
+            case 40: rc = launch_tma_apply<40>(c, in, out, sgn); break;
+            case 32: rc = launch_tma_apply<32>(c, in, out, sgn); break;
+            case 24: rc = launch_tma_apply<24>(c, in, out, sgn); break;
+            case 16: rc = launch_tma_apply<16>(c, in, out, sgn); break;
+            case 8:  rc = launch_tma_apply<8>(c, in, out, sgn); break;
+            case 4:  rc = launch_tma_apply<4>(c, in, out, sgn); break;
+            default: rc = launch_tma_apply<2>(c, in, out, sgn); break;
+        }
+        c->nb = nb_saved;
+        return rc;
+    }
+    const Tiling t = make_tiling(c, nb);
+    PassParams p = base_params(c, nb, t);
+    p.in = in; p.out = out;
+    p.ca = c->coef + C_LAM * (size_t)c->nb_max;
+    p.sgn = sgn;
+    return launch_pass<MODE_APPLY>(c, p, t);
 }
 
 int check_batch_args(const wri_ctx* c, int nb) {
@@ -920,12 +985,7 @@ int wri_apply_M(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, float lam
     if (!x_dev || !ytop_dev || (c->n_rec && !ybot_dev) || !aligned16(x_dev) || !aligned16(ytop_dev))
         return WRI_ERR_ARG;
     if ((rc = upload_columns(c, nb, omega_idx_host, lambda))) return rc;
-    const Tiling t = make_tiling(c, nb);
-    PassParams p = base_params(c, nb, t);
-    p.in = (const float2*)x_dev; p.out = (float2*)ytop_dev;
-    p.ca = c->coef + C_LAM * (size_t)c->nb_max;
-    p.sgn = 1.f;
-    if ((rc = launch_pass<MODE_APPLY>(c, p, t))) return rc;
+    if ((rc = apply_operator(c, nb, (const float2*)x_dev, (float2*)ytop_dev, 1.f))) return rc;
     if (c->n_rec) {
         const long long n = (long long)c->n_rec * nb;
         k_gather<<<(unsigned)std::min<long long>((n + 255) / 256, 1184), 256, 0, c->stream>>>(
@@ -943,12 +1003,7 @@ int wri_apply_MH(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, float la
     if (!x_dev || !ytop_dev || (c->n_rec && !ybot_dev) || !aligned16(x_dev) || !aligned16(ytop_dev))
         return WRI_ERR_ARG;
     if ((rc = upload_columns(c, nb, omega_idx_host, lambda))) return rc;
-    const Tiling t = make_tiling(c, nb);
-    PassParams p = base_params(c, nb, t);
-    p.in = (const float2*)ytop_dev; p.out = (float2*)x_dev;
-    p.ca = c->coef + C_LAM * (size_t)c->nb_max;
-    p.sgn = -1.f;
-    if ((rc = launch_pass<MODE_APPLY>(c, p, t))) return rc;
+    if ((rc = apply_operator(c, nb, (const float2*)ytop_dev, (float2*)x_dev, -1.f))) return rc;
     if (c->n_rec) {
         const long long n = (long long)c->n_rec * nb;
         k_scatter_add<<<(unsigned)std::min<long long>((n + 255) / 256, 1184), 256, 0, c->stream>>>(

@@ -81,7 +81,8 @@ struct TmaPassParams {
                            //         with column chunks, one entry per (receiver, chunk)
     ScalParams fin;
     // MODE_G (objective + gradient, eq. 4 / 9): out is unused; the optional stream is q
-    int has_q;
+    int has_q;             // MODE_A / MODE_G: the second stream (old vector / q) is present; 0 = plain operator
+                           // application out = ca * A in (wri_apply_M / _MH through this pipeline)
     const int* gsrc;       // [nb] source cells or null
     const float2* galpha;  // [nb] source weights (with gsrc)
     float* g;              // [n_g] this batch's gradient (overwritten) or null
@@ -255,7 +256,7 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
                 if (issuer) {
                     mbar_wait(empty0 + 8 * stage, phase ^ 1);
                     const bool streams = pl >= z0 + 1;
-                    const bool old_stream = (MODE != MODE_G) || p.has_q;
+                    const bool old_stream = (MODE == MODE_F) || p.has_q;
                     const uint32_t fb = full0 + 8 * stage;
                     mbar_expect_tx(fb, Cfg::IN_BYTES + (streams ? (old_stream ? NSTREAM * Cfg::CTR_BYTES : 0) +
                                                             (p.m_tma ? TXC * TYC * 4 : 0) : 0));
@@ -543,7 +544,7 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
         for (int t = blockIdx.x; t < p.n_tiles; t += gridDim.x) {
             double acc[2];
             int chunk;
-            const bool has_old = (MODE != MODE_G) || p.has_q;
+            const bool has_old = (MODE == MODE_F) || p.has_q;
             if (p.m_tma) {
                 if (has_old) run_tile(TrueT{}, TrueT{}, t, acc, chunk);
                 else         run_tile(TrueT{}, FalseT{}, t, acc, chunk);
@@ -588,7 +589,8 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
 
     // ---------------------------------------------------------------------- CTA epilogue
     __syncthreads();
-    for (int j = tid; j < p.nb; j += blockDim.x) p.partials[(size_t)blockIdx.x * p.nb + j] = colacc[j];
+    if (p.partials)
+        for (int j = tid; j < p.nb; j += blockDim.x) p.partials[(size_t)blockIdx.x * p.nb + j] = colacc[j];
     __threadfence();
     __syncthreads();
     if (tid == 0) s_ticket = atomicAdd(p.counter, 1u);
@@ -596,7 +598,7 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
     if (s_ticket == gridDim.x - 1) {
         __threadfence();
         double* sh = reinterpret_cast<double*>(smem);           // stages are idle now
-        if (MODE != MODE_G)
+        if (MODE != MODE_G && p.phase >= 0)                     // phase < 0: no scalar phase (operator application)
         switch (p.phase) {
             case PH_INIT_A: finalize_phase<PH_INIT_A>(p.fin, sh); break;
             case PH_F:      finalize_phase<PH_F>(p.fin, sh); break;
