@@ -267,6 +267,31 @@ int wri_lsqr_batch_host(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_host,
                         const float* tol_host, int32_t maxit,
                         void* u_out_host, float* resnorms_host, int32_t* iters_host);
 
+/* Pipelined host-buffer solves.  An inversion walks through many source groups / frequencies
+ * (PAPER.md:221); with HOST buffers the copies of one solve (q in, u out: 2 x n_g*nb*8 bytes) can
+ * ride under the neighbouring solves: while solve i runs, the inputs of solve i+1 are uploaded and
+ * the results of solve i-1 downloaded, on two copy streams of the library's own.
+ *   wri_host_pipeline_bytes / wri_set_host_pipeline   two staging slots (q, d, x, tol, history per
+ *                slot) in a device buffer the caller allocates for batch widths up to nb; NULL drops it
+ *   wri_lsqr_batch_host_async / wri_lsqr_sf_batch_host_async   same arguments and results as the
+ *                _host entries, but the call returns once everything is ENQUEUED (with tolerances:
+ *                once the solve itself has finished); the host buffers — PINNED memory, or nothing
+ *                overlaps — must stay valid, and the outputs must not be read, until wri_host_wait
+ *   wri_host_wait   blocks until every enqueued solve has delivered its results
+ * Solves still execute one after the other on the context's stream, so results are those of the
+ * _host entries bit for bit.  Call wri_host_wait before using any other entry of the context.   */
+size_t wri_host_pipeline_bytes(const wri_ctx* ctx, int32_t nb);
+int    wri_set_host_pipeline(wri_ctx* ctx, int32_t nb, void* buf_dev, size_t bytes);
+int    wri_lsqr_batch_host_async(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_host,
+                                 const void* q_host, const void* d_host, float lambda,
+                                 const float* tol_host, int32_t maxit,
+                                 void* u_out_host, float* resnorms_host, int32_t* iters_host);
+int    wri_lsqr_sf_batch_host_async(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_host,
+                                    const int32_t* src_ijk_host, const void* q_host, const void* d_host,
+                                    float lambda, const float* tol_host, int32_t maxit, void* u_out_host,
+                                    void* alpha_out_host, float* resnorms_host, int32_t* iters_host);
+int    wri_host_wait(wri_ctx* ctx);
+
 /* Stepping form of the same solve (outer drivers, teacher-forced parity tests).
  *   begin   : Golub-Kahan start  beta1 u1 = b, alpha1 v1 = M^H u1, w1 = v1, x0 = 0
  *   iterate : n_steps more iterations (total must not exceed maxit)

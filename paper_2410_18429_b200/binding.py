@@ -93,6 +93,11 @@ def load_library():
     solve = [P, I32, P, P, P, F32, P, I32, P, P, P]
     lib.wri_lsqr_batch.argtypes = solve
     lib.wri_lsqr_batch_host.argtypes = solve
+    lib.wri_lsqr_batch_host_async.argtypes = solve
+    lib.wri_host_pipeline_bytes.argtypes = [P, I32]
+    lib.wri_host_pipeline_bytes.restype = C.c_size_t
+    lib.wri_set_host_pipeline.argtypes = [P, I32, P, C.c_size_t]
+    lib.wri_host_wait.argtypes = [P]
     lib.wri_lsqr_begin.argtypes = solve
     lib.wri_apply_S.argtypes = [P, I32, P, P, F32, P, P, P, P]
     lib.wri_apply_SH.argtypes = [P, I32, P, P, F32, P, P, P, P]
@@ -100,6 +105,7 @@ def load_library():
     lib.wri_lsqr_sf_batch.argtypes = solve_sf
     lib.wri_lsqr_sf_begin.argtypes = solve_sf
     lib.wri_lsqr_sf_batch_host.argtypes = solve_sf
+    lib.wri_lsqr_sf_batch_host_async.argtypes = solve_sf
     lib.wri_objective_gradient.argtypes = [P, I32, P, P, P, P, P, P, F32, P, P, P]
     lib.wri_lsqr_set_opts.argtypes = [P, C.POINTER(wri_lsqr_opts)]
     lib.wri_set_receiver_mask.argtypes = [P, I32, P]
@@ -279,6 +285,37 @@ class Wri:
         _ck(self._lib.wri_lsqr_batch_host(self._h, nb, oi, _dptr(q), _dptr(d), float(lam), _dptr(tol),
                                           int(maxit), _dptr(u), _dptr(res), _dptr(it)))
         return u, res, it
+
+    def ensure_host_pipeline(self, nb):
+        """Device staging for the pipelined host-buffer entries (two slots)."""
+        need = int(self._lib.wri_host_pipeline_bytes(self._h, int(nb)))
+        buf = getattr(self, "_pipe", None)
+        if buf is None or buf.numel() < need or getattr(self, "_pipe_nb", 0) < nb:
+            self._pipe = self._torch.empty(need, dtype=self._torch.uint8, device=self.m.device)
+            self._pipe_nb = int(nb)
+            _ck(self._lib.wri_set_host_pipeline(self._h, int(nb), _dptr(self._pipe), self._pipe.numel()))
+
+    def lsqr_batch_host_async(self, q, d, lam, tol=None, maxit=50, omega_idx=None, out=None):
+        """Pipelined host-buffer solve: returns after enqueue; q, d, tol and out = (u, resnorms,
+        iters) are PINNED CPU tensors that must stay alive, and out unread, until host_wait()."""
+        t = self._torch
+        nb = q.shape[1]
+        self.ensure_workspace(nb, compaction=tol is not None)
+        self.ensure_host_pipeline(nb)
+        if out is None:
+            out = (t.empty((self.ng, nb), dtype=t.complex64).pin_memory(),
+                   t.empty((maxit + 1, nb), dtype=t.float32).pin_memory(),
+                   t.empty(nb, dtype=t.int32).pin_memory())
+        u, res, it = out
+        keep, oi = _i32(omega_idx)
+        self._async_keep = getattr(self, "_async_keep", []) + [(q, d, tol, u, res, it)]
+        _ck(self._lib.wri_lsqr_batch_host_async(self._h, nb, oi, _dptr(q), _dptr(d), float(lam), _dptr(tol),
+                                                int(maxit), _dptr(u), _dptr(res), _dptr(it)))
+        return u, res, it
+
+    def host_wait(self):
+        _ck(self._lib.wri_host_wait(self._h))
+        self._async_keep = []
 
     def lsqr_begin(self, q, d, lam, tol=None, maxit=50, omega_idx=None):
         nb = q.shape[1]

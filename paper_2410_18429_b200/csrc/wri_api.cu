@@ -124,6 +124,15 @@ struct wri_ctx {
     std::vector<int> ev_cols;             // per pair: working batch width of that launch
     size_t ev_used = 0;                   // pairs in use
     std::vector<std::pair<const void*, size_t>> smem_ok;   // kernels already granted their dynamic smem size
+    // pipelined host-buffer solves (wri_set_host_pipeline): two staging slots, copy streams, events
+    struct PipeSlot {
+        float2 *Q = nullptr, *D = nullptr, *X = nullptr, *alpha = nullptr;
+        float *tol = nullptr, *res = nullptr;
+        int* its = nullptr;
+        cudaEvent_t ev_in = nullptr, ev_solve = nullptr, ev_out = nullptr;
+    } pipe[2];
+    cudaStream_t s_in = nullptr, s_out = nullptr;
+    int pipe_nb = 0, pipe_next = 0;       // width the staging was sized for (0 = no pipeline), next slot
 };
 
 namespace {
@@ -917,6 +926,13 @@ int wri_destroy(wri_ctx* c) {
     cudaFree(c->aw_tol); cudaFree(c->aw_f); cudaFree(c->aw_ar0); cudaFree(c->aw_iters);
     if (c->h_aw) cudaFreeHost(c->h_aw);
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
+    for (auto& sl : c->pipe) {
+        if (sl.ev_in) cudaEventDestroy(sl.ev_in);
+        if (sl.ev_solve) cudaEventDestroy(sl.ev_solve);
+        if (sl.ev_out) cudaEventDestroy(sl.ev_out);
+    }
+    if (c->s_in) cudaStreamDestroy(c->s_in);
+    if (c->s_out) cudaStreamDestroy(c->s_out);
     delete c;
     return WRI_OK;
 }
@@ -1534,6 +1550,134 @@ int wri_lsqr_peek(const wri_ctx* c, wri_lsqr_view* v) {
     v->active = c->active; v->iters = c->iters;
     v->nb_max = c->nb_max;
     v->sf_state = c->sf ? c->stat + S_VA_RE * NM : nullptr;
+    return WRI_OK;
+}
+
+}  // extern "C"
+
+// ---- pipelined host-buffer solves ------------------------------------------------------------------
+namespace {
+
+struct PipeLayout { size_t Q, D, X, alpha, tol, res, its, slot; };
+PipeLayout pipe_layout(const wri_ctx* c, int nb) {
+    PipeLayout L{};
+    const size_t vec = align_up(c->ng * (size_t)nb * sizeof(float2), 256);
+    const size_t bot = align_up((size_t)std::max(c->n_rec, 1) * nb * sizeof(float2), 256);
+    size_t o = 0;
+    L.Q = o; o += vec;
+    L.X = o; o += vec;
+    L.D = o; o += bot;
+    L.alpha = o; o += align_up((size_t)nb * sizeof(float2), 256);
+    L.tol = o; o += align_up((size_t)nb * sizeof(float), 256);
+    L.res = o; o += align_up((size_t)(kHostMaxitCap + 1) * nb * sizeof(float), 256);
+    L.its = o; o += align_up((size_t)nb * sizeof(int), 256);
+    L.slot = o;
+    return L;
+}
+
+int host_async_impl(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const int32_t* src_ijk_host,
+                    const void* q_host, const void* d_host, float lambda, const float* tol_host, int32_t maxit,
+                    void* u_out_host, void* alpha_out_host, float* resnorms_host, int32_t* iters_host) {
+    int rc = check_batch_args(c, nb);
+    if (rc) return rc;
+    const bool sf = src_ijk_host != nullptr;
+    if ((!q_host && !sf) || (c->n_rec && !d_host) || !u_out_host || !resnorms_host || maxit < 0 ||
+        maxit > kHostMaxitCap || (sf && !alpha_out_host))
+        return WRI_ERR_ARG;
+    if (!c->pipe_nb || nb > c->pipe_nb) return WRI_ERR_WORKSPACE;
+    if (!c->ws) return WRI_ERR_WORKSPACE;
+    wri_ctx::PipeSlot& S = c->pipe[c->pipe_next];
+    c->pipe_next ^= 1;
+    const size_t vbytes = c->ng * (size_t)nb * sizeof(float2);
+    const size_t dbytes = (size_t)c->n_rec * nb * sizeof(float2);
+    // inputs: the slot's previous solve has consumed them and its results have left
+    CK(cudaStreamWaitEvent(c->s_in, S.ev_solve, 0));
+    CK(cudaStreamWaitEvent(c->s_in, S.ev_out, 0));
+    if (c->opts.warm_start) {
+        CK(cudaMemcpyAsync(S.X, u_out_host, vbytes, cudaMemcpyHostToDevice, c->s_in));
+        if (sf) CK(cudaMemcpyAsync(S.alpha, alpha_out_host, nb * sizeof(float2), cudaMemcpyHostToDevice, c->s_in));
+    }
+    if (q_host) CK(cudaMemcpyAsync(S.Q, q_host, vbytes, cudaMemcpyHostToDevice, c->s_in));
+    if (dbytes) CK(cudaMemcpyAsync(S.D, d_host, dbytes, cudaMemcpyHostToDevice, c->s_in));
+    if (tol_host) CK(cudaMemcpyAsync(S.tol, tol_host, nb * sizeof(float), cudaMemcpyHostToDevice, c->s_in));
+    CK(cudaEventRecord(S.ev_in, c->s_in));
+    // the solve, on the context's stream
+    CK(cudaStreamWaitEvent(c->stream, S.ev_in, 0));
+    CK(cudaStreamWaitEvent(c->stream, S.ev_out, 0));
+    if ((rc = solve_groups(c, nb, omega_idx_host, q_host ? S.Q : nullptr, S.D, lambda, tol_host ? S.tol : nullptr,
+                           maxit, S.X, S.res, S.its, false, src_ijk_host, sf ? S.alpha : nullptr)))
+        return rc;
+    CK(cudaEventRecord(S.ev_solve, c->stream));
+    // results
+    CK(cudaStreamWaitEvent(c->s_out, S.ev_solve, 0));
+    CK(cudaMemcpyAsync(u_out_host, S.X, vbytes, cudaMemcpyDeviceToHost, c->s_out));
+    CK(cudaMemcpyAsync(resnorms_host, S.res, (size_t)(maxit + 1) * nb * sizeof(float), cudaMemcpyDeviceToHost, c->s_out));
+    if (iters_host) CK(cudaMemcpyAsync(iters_host, S.its, nb * sizeof(int), cudaMemcpyDeviceToHost, c->s_out));
+    if (sf) CK(cudaMemcpyAsync(alpha_out_host, S.alpha, nb * sizeof(float2), cudaMemcpyDeviceToHost, c->s_out));
+    CK(cudaEventRecord(S.ev_out, c->s_out));
+    return WRI_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t wri_host_pipeline_bytes(const wri_ctx* c, int32_t nb) {
+    if (!c || nb <= 0 || nb > c->nb_max) return 0;
+    return 2 * pipe_layout(c, nb).slot;
+}
+
+int wri_set_host_pipeline(wri_ctx* c, int32_t nb, void* buf_dev, size_t bytes) {
+    if (!c) return WRI_ERR_ARG;
+    if (c->solving) return WRI_ERR_STATE;
+    if (c->s_out) { CK(cudaStreamSynchronize(c->s_out)); CK(cudaStreamSynchronize(c->s_in)); }
+    if (!buf_dev) { c->pipe_nb = 0; return WRI_OK; }
+    if (nb <= 0 || nb > c->nb_max || !aligned16(buf_dev)) return WRI_ERR_ARG;
+    const PipeLayout L = pipe_layout(c, nb);
+    if (bytes < 2 * L.slot) return WRI_ERR_WORKSPACE;
+    if (!c->s_in) {
+        CK(cudaStreamCreateWithFlags(&c->s_in, cudaStreamNonBlocking));
+        CK(cudaStreamCreateWithFlags(&c->s_out, cudaStreamNonBlocking));
+        for (auto& sl : c->pipe) {
+            CK(cudaEventCreateWithFlags(&sl.ev_in, cudaEventDisableTiming));
+            CK(cudaEventCreateWithFlags(&sl.ev_solve, cudaEventDisableTiming));
+            CK(cudaEventCreateWithFlags(&sl.ev_out, cudaEventDisableTiming));
+        }
+    }
+    for (int i = 0; i < 2; ++i) {
+        char* b = (char*)buf_dev + (size_t)i * L.slot;
+        wri_ctx::PipeSlot& S = c->pipe[i];
+        S.Q = (float2*)(b + L.Q); S.X = (float2*)(b + L.X); S.D = (float2*)(b + L.D);
+        S.alpha = (float2*)(b + L.alpha); S.tol = (float*)(b + L.tol); S.res = (float*)(b + L.res);
+        S.its = (int*)(b + L.its);
+    }
+    c->pipe_nb = nb;
+    c->pipe_next = 0;
+    return WRI_OK;
+}
+
+int wri_lsqr_batch_host_async(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const void* q_host,
+                              const void* d_host, float lambda, const float* tol_host, int32_t maxit,
+                              void* u_out_host, float* resnorms_host, int32_t* iters_host) {
+    if (!q_host) return WRI_ERR_ARG;
+    return host_async_impl(c, nb, omega_idx_host, nullptr, q_host, d_host, lambda, tol_host, maxit, u_out_host,
+                           nullptr, resnorms_host, iters_host);
+}
+
+int wri_lsqr_sf_batch_host_async(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host,
+                                 const int32_t* src_ijk_host, const void* q_host, const void* d_host,
+                                 float lambda, const float* tol_host, int32_t maxit, void* u_out_host,
+                                 void* alpha_out_host, float* resnorms_host, int32_t* iters_host) {
+    if (!src_ijk_host) return WRI_ERR_ARG;
+    return host_async_impl(c, nb, omega_idx_host, src_ijk_host, q_host, d_host, lambda, tol_host, maxit,
+                           u_out_host, alpha_out_host, resnorms_host, iters_host);
+}
+
+int wri_host_wait(wri_ctx* c) {
+    if (!c) return WRI_ERR_ARG;
+    if (c->s_in) CK(cudaStreamSynchronize(c->s_in));
+    CK(cudaStreamSynchronize(c->stream));
+    if (c->s_out) CK(cudaStreamSynchronize(c->s_out));
     return WRI_OK;
 }
 

@@ -30,7 +30,9 @@ def test_every_declared_symbol_is_exported(lib):
             "wri_lsqr_begin", "wri_lsqr_iterate", "wri_lsqr_end", "wri_lsqr_peek",
             "wri_set_model", "wri_launch_count", "wri_apply_S", "wri_apply_SH", "wri_lsqr_sf_batch",
             "wri_lsqr_sf_begin", "wri_lsqr_sf_batch_host", "wri_objective_gradient", "wri_lsqr_set_opts",
-            "wri_misfit_sf", "wri_awri_step", "wri_set_receiver_mask"} <= set(names)
+            "wri_misfit_sf", "wri_awri_step", "wri_set_receiver_mask",
+            "wri_host_pipeline_bytes", "wri_set_host_pipeline", "wri_lsqr_batch_host_async",
+            "wri_lsqr_sf_batch_host_async", "wri_host_wait"} <= set(names)
     for n in names:
         assert hasattr(lib, n), n
 

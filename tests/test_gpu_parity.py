@@ -443,3 +443,32 @@ def test_wide_batches_are_solved_in_64_column_groups(torch_cuda, monkeypatch):
     qh, dh = torch.from_numpy(w.Q).pin_memory(), torch.from_numpy(w.D).pin_memory()
     uh, rh, ith = ctx.lsqr_batch_host(qh, dh, w.lam, None, maxit=K, omega_idx=w.omega_idx)
     assert np.array_equal(uh.numpy(), u.cpu().numpy()) and np.array_equal(rh.numpy(), res.cpu().numpy())
+
+
+def test_pipelined_host_entry_equals_the_serial_one(torch_cuda):
+    """wri_lsqr_batch_host_async: four solves with different inputs enqueued back to back (uploads
+    and downloads ride under the neighbouring solves on the library's copy streams); after
+    wri_host_wait every result equals the serial host entry's bit for bit; with tolerances and a
+    128-column (grouped) batch as well."""
+    torch = torch_cuda
+    w = workloads.make("config2", grid=(24, 28, 40), nb=128)
+    ctx = _wri(w)
+    rng = np.random.Generator(np.random.PCG64(3))
+    K = 12
+    ins, outs = [], []
+    tolh = (10.0 ** rng.uniform(-2.0, -0.7, w.nb)).astype(np.float32)
+    for i in range(4):
+        scale = np.float32(1.0 + 0.25 * i)
+        q = torch.from_numpy((w.Q * scale).astype(np.complex64)).pin_memory()
+        d = torch.from_numpy(np.roll(w.D, i, axis=1).copy()).pin_memory()
+        tol = torch.from_numpy(tolh).pin_memory() if i == 2 else None
+        ins.append((q, d, tol))
+    for q, d, tol in ins:                                        # all enqueued before anything is read
+        outs.append(ctx.lsqr_batch_host_async(q, d, w.lam, tol, maxit=K, omega_idx=w.omega_idx))
+    ctx.host_wait()
+    for (q, d, tol), (u, res, it) in zip(ins, outs):
+        us, rs, its = ctx.lsqr_batch_host(q, d, w.lam, tol, maxit=K, omega_idx=w.omega_idx)
+        assert np.array_equal(u.numpy(), us.numpy())
+        assert np.array_equal(res.numpy(), rs.numpy()) and np.array_equal(it.numpy(), its.numpy())
+    assert len(set(outs[2][2].numpy().tolist())) > 3             # the tolerance case really stopped early
+    assert not np.array_equal(outs[0][0].numpy(), outs[1][0].numpy())
