@@ -472,3 +472,45 @@ def test_pipelined_host_entry_equals_the_serial_one(torch_cuda):
         assert np.array_equal(res.numpy(), rs.numpy()) and np.array_equal(it.numpy(), its.numpy())
     assert len(set(outs[2][2].numpy().tolist())) > 3             # the tolerance case really stopped early
     assert not np.array_equal(outs[0][0].numpy(), outs[1][0].numpy())
+
+
+def test_two_contexts_and_a_side_stream(torch_cuda):
+    """Two contexts (different grids, widths, receiver sets) used alternately, one of them on a
+    non-default CUDA stream: each gives what it gives alone (no state shared between contexts; all
+    work of a context is enqueued on the stream given at create)."""
+    torch = torch_cuda
+    from paper_2410_18429_b200 import Wri
+    wa = workloads.make("config1", grid=(32, 28, 24), nb=16)
+    wb = workloads.make("config3", grid=(26, 30, 22), nb=48)
+    side = torch.cuda.Stream()
+    ca = _wri(wa)
+    with torch.cuda.stream(side):
+        mb = torch.from_numpy(wb.m).cuda()
+        cb = Wri((wb.nx, wb.ny, wb.nz), wb.h, wb.omegas, mb, wb.sponge_width, wb.rec_ijk, wb.nb,
+                 stream=side.cuda_stream)
+        qb, db = torch.from_numpy(wb.Q).cuda(), torch.from_numpy(wb.D).cuda()
+    qa, da = torch.from_numpy(wa.Q).cuda(), torch.from_numpy(wa.D).cuda()
+    side.synchronize()
+    K = 10
+    ua0, ra0, _ = ca.lsqr_batch(qa, da, wa.lam, None, maxit=K, omega_idx=wa.omega_idx)
+    torch.cuda.synchronize()
+    with torch.cuda.stream(side):
+        ub0, rb0, _ = cb.lsqr_batch(qb, db, wb.lam, None, maxit=K, omega_idx=wb.omega_idx)
+    side.synchronize()
+    ua0, ra0, ub0, rb0 = (t.clone() for t in (ua0, ra0, ub0, rb0))
+    # interleaved, stepping entries, both in flight at once
+    ua, ra, _ = ca.lsqr_begin(qa, da, wa.lam, None, maxit=K, omega_idx=wa.omega_idx)
+    with torch.cuda.stream(side):
+        ub, rb, _ = cb.lsqr_begin(qb, db, wb.lam, None, maxit=K, omega_idx=wb.omega_idx)
+    for _ in range(K // 2):
+        ca.lsqr_iterate(2)
+        cb.lsqr_iterate(2)
+    ca.lsqr_end()
+    cb.lsqr_end()
+    torch.cuda.synchronize()
+    side.synchronize()
+    assert torch.equal(ra, ra0) and torch.equal(torch.view_as_real(ua), torch.view_as_real(ua0))
+    assert torch.equal(rb, rb0) and torch.equal(torch.view_as_real(ub), torch.view_as_real(ub0))
+    rec = O.rec_cells(wb.nx, wb.ny, wb.nz, wb.rec_ijk)
+    ref = O.lsqr(ops_for(wb)[5], wb.m, wb.lam, rec, wb.Q[:, 5], wb.D[:, 5], tol=0.0, maxit=K)
+    assert rel(ub[:, 5].cpu().numpy(), ref["x"]) < 1e-3 and rel(rb[:, 5].cpu().numpy(), ref["resnorms"]) < 1e-3
