@@ -117,6 +117,7 @@ struct wri_ctx {
         int merged = 0;                   // tensor maps fold (column, x)
     } planF, planA, planG;
     double* partials_tma = nullptr;       // [grid][nb]
+    bool wx_zero = false;                 // W, X not cleared: the first pass F must not read them
     // optional per-kernel timing (wri_profile_*)
     bool profiling = false;
     std::vector<cudaEvent_t> ev_pool;     // pairs: start, stop
@@ -638,7 +639,9 @@ int launch_tma_cfg(wri_ctx* c, int phase) {
     p.ih2 = (float)(1.0 / (c->h * c->h));
     p.m6ih2 = (float)(-6.0 / (c->h * c->h));
     p.phase = phase;
-    p.has_q = 1;                                   // the in-place (old) stream is there
+    // streams known to be zero are neither cleared nor read: V in the start's adjoint pass, W and X in the
+    // first forward pass of a cold batch solve (c->wx_zero)
+    p.has_q = (MODE == MODE_A) ? (phase != PH_INIT_A) : (MODE == MODE_F ? !c->wx_zero : 1);
     p.nstage = ring_depth<Cfg, MODE>(P.nchunk);
     p.m_tma = P.m_tma;
     p.merged = P.merged;
@@ -1136,7 +1139,7 @@ int lsqr_begin_impl(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const
                     const void* d_dev, float lambda, const float* tol_dev, int32_t maxit,
                     void* u_out_dev, float* resnorms_dev, int32_t* iters_dev, bool host_staged,
                     const int32_t* src_ijk_host = nullptr, void* alpha_out_dev = nullptr,
-                    int col0 = 0, int nbw = 0) {
+                    int col0 = 0, int nbw = 0, bool lazy_start = false) {
     // col0, nbw: a GROUPED solve works on the caller's columns [col0, col0 + nbw) only, in a compact
     // nbw-wide working set of its own (nbw = 0: all nb columns, working set = the caller's layout)
     int rc = check_batch_args(c, nb);
@@ -1239,11 +1242,15 @@ int lsqr_begin_impl(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const
         r.in = c->X; r.out = c->U; r.sgn = 1.f;
         r.ca = c->coef + C_NLAM * NM; r.cb = c->coef + C_MONE * NM;
         if ((rc = launch_pass<MODE_A>(c, r, c->tl))) return rc;
-    } else {
-        CK(cudaMemsetAsync(c->X, 0, vbytes, c->stream));
     }
-    CK(cudaMemsetAsync(c->W, 0, vbytes, c->stream));
-    CK(cudaMemsetAsync(c->V, 0, vbytes, c->stream));
+    // x0 = 0, w = 0, v = 0.  On the TMA path V is not read by the start's adjoint pass, and in a cold
+    // batch solve of at least one iteration (lazy_start) W and X are not read by the first forward pass,
+    // which writes them: no clearing needed.  (The stepping entries clear everything: their state can
+    // be looked at before the first iteration.)
+    c->wx_zero = lazy_start && c->tma_cb && !c->opts.warm_start && maxit >= 1;
+    if (!c->opts.warm_start && !c->wx_zero) CK(cudaMemsetAsync(c->X, 0, vbytes, c->stream));
+    if (!c->wx_zero) CK(cudaMemsetAsync(c->W, 0, vbytes, c->stream));
+    if (!c->tma_cb) CK(cudaMemsetAsync(c->V, 0, vbytes, c->stream));
     if ((rc = launch_scalars<PH_INIT_B>(c, (const float2*)d_dev))) return rc;
     // alpha1 v1 = M^H u1
     if (c->tma_cb) {
@@ -1368,7 +1375,7 @@ int solve_groups(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const vo
     const int gw = group_width(c, nb);
     for (int col0 = 0; col0 < nb; col0 += (gw ? gw : nb)) {
         if ((rc = lsqr_begin_impl(c, nb, omega_idx_host, q_dev, d_dev, lambda, tol_dev, maxit, u_out_dev,
-                                  resnorms_dev, iters_dev, host_staged, src_ijk_host, alpha_out_dev, col0, gw)))
+                                  resnorms_dev, iters_dev, host_staged, src_ijk_host, alpha_out_dev, col0, gw, true)))
             return rc;
         if ((rc = wri_lsqr_iterate(c, maxit))) { c->solving = false; return rc; }
         if ((rc = wri_lsqr_end(c))) return rc;
@@ -1407,6 +1414,7 @@ int wri_lsqr_iterate(wri_ctx* c, int32_t n_steps) {
         if (c->tma_cb) {
             // two launches per iteration: the last CTA of each pass runs the scalar recurrences
             if ((rc = launch_tma<MODE_F>(c, PH_F))) return rc;
+            c->wx_zero = false;
             if ((rc = launch_tma<MODE_A>(c, PH_A))) return rc;
         } else {
             PassParams p = base_params(c, c->nb, c->tl);

@@ -82,6 +82,8 @@ struct TmaPassParams {
     ScalParams fin;
     // MODE_G (objective + gradient, eq. 4 / 9): out is unused; the optional stream is q
     int has_q;             // MODE_A / MODE_G: the second stream (old vector / q) is present; 0 = plain operator
+                           // MODE_F: the W and X streams are read; 0 = they are known to be zero (first pass of a
+                           // cold solve: they are written, never read, so they need no clearing beforehand)
                            // application out = ca * A in (wri_apply_M / _MH through this pipeline)
     const int* gsrc;       // [nb] source cells or null
     const float2* galpha;  // [nb] source weights (with gsrc)
@@ -257,8 +259,9 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
                     mbar_wait(empty0 + 8 * stage, phase ^ 1);
                     const bool streams = pl >= z0 + 1;
                     const bool old_stream = (MODE == MODE_F) || p.has_q;
+                    const bool wx_streams = (MODE == MODE_F) && p.has_q;     // F's first pass of a cold solve: W = X = 0
                     const uint32_t fb = full0 + 8 * stage;
-                    mbar_expect_tx(fb, Cfg::IN_BYTES + (streams ? (old_stream ? NSTREAM * Cfg::CTR_BYTES : 0) +
+                    mbar_expect_tx(fb, Cfg::IN_BYTES + (streams ? (old_stream ? (wx_streams || MODE != MODE_F ? NSTREAM : 1) * Cfg::CTR_BYTES : 0) +
                                                             (p.m_tma ? TXC * TYC * 4 : 0) : 0));
                     const uint32_t dst = smem_u32(stages + stage * STAGE_BYTES);
 #if WRI_HINTS >= 2
@@ -270,14 +273,14 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
 #if WRI_HINTS >= 1
                         if (old_stream)
                         tma_load_4d_hint(dst + Cfg::IN_SPAN, &tm_old, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1, pol_stream);
-                        if (MODE == MODE_F) {
+                        if (wx_streams) {
                             tma_load_4d_hint(dst + Cfg::IN_SPAN + Cfg::CTR_BYTES, &tm_w, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1, pol_stream);
                             tma_load_4d_hint(dst + Cfg::IN_SPAN + 2 * Cfg::CTR_BYTES, &tm_x, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1, pol_stream);
                         }
 #else
                         if (old_stream)
                         tma_load_4d(dst + Cfg::IN_SPAN, &tm_old, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1);
-                        if (MODE == MODE_F) {
+                        if (wx_streams) {
                             tma_load_4d(dst + Cfg::IN_SPAN + Cfg::CTR_BYTES, &tm_w, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1);
                             tma_load_4d(dst + Cfg::IN_SPAN + 2 * Cfg::CTR_BYTES, &tm_x, fb, mg ? x0 * CB : c0, mg ? y0 : x0, mg ? pl - 1 : y0, mg ? 0 : pl - 1);
                         }
@@ -498,8 +501,12 @@ k_pass_tma(const __grid_constant__ CUtensorMap tm_in, const __grid_constant__ CU
                                 acc32[1] += fmaf(rr.z, rr.z, rr.w * rr.w);
                                 if (MODE == MODE_F) {
                                     const int io = Cfg::IN_SPAN + (tid + j * NT) * 16;
-                                    o_w[j] = lds128(sb, io + Cfg::CTR_BYTES);
-                                    o_x[j] = lds128(sb, io + 2 * Cfg::CTR_BYTES);
+                                    if (p.has_q) {
+                                        o_w[j] = lds128(sb, io + Cfg::CTR_BYTES);
+                                        o_x[j] = lds128(sb, io + 2 * Cfg::CTR_BYTES);
+                                    } else {
+                                        o_w[j] = o_x[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+                                    }
                                     float4 xn, wn;
                                     xn.x = fmaf(cx[0], o_w[j].x, o_x[j].x);
                                     xn.y = fmaf(cx[0], o_w[j].y, o_x[j].y);
