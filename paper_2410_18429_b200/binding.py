@@ -313,6 +313,27 @@ class Wri:
                                                 int(maxit), _dptr(u), _dptr(res), _dptr(it)))
         return u, res, it
 
+    def lsqr_sf_batch_host_async(self, d, lam, src_ijk, tol=None, maxit=50, omega_idx=None, q=None, out=None):
+        """Pipelined host-buffer solve of the source-free system; out = (u, alpha, resnorms, iters),
+        pinned CPU tensors; see lsqr_batch_host_async."""
+        t = self._torch
+        nb = d.shape[1]
+        self.ensure_workspace(nb, compaction=tol is not None)
+        self.ensure_host_pipeline(nb)
+        if out is None:
+            out = (t.empty((self.ng, nb), dtype=t.complex64).pin_memory(),
+                   t.empty(nb, dtype=t.complex64).pin_memory(),
+                   t.empty((maxit + 1, nb), dtype=t.float32).pin_memory(),
+                   t.empty(nb, dtype=t.int32).pin_memory())
+        u, a, res, it = out
+        keep, oi = _i32(omega_idx)
+        keep2, si = _i32(src_ijk)
+        self._async_keep = getattr(self, "_async_keep", []) + [(q, d, tol, u, a, res, it)]
+        _ck(self._lib.wri_lsqr_sf_batch_host_async(self._h, nb, oi, si, _dptr(q), _dptr(d), float(lam),
+                                                   _dptr(tol), int(maxit), _dptr(u), _dptr(a), _dptr(res),
+                                                   _dptr(it)))
+        return u, a, res, it
+
     def host_wait(self):
         _ck(self._lib.wri_host_wait(self._h))
         self._async_keep = []

@@ -472,6 +472,17 @@ def test_pipelined_host_entry_equals_the_serial_one(torch_cuda):
         assert np.array_equal(res.numpy(), rs.numpy()) and np.array_equal(it.numpy(), its.numpy())
     assert len(set(outs[2][2].numpy().tolist())) > 3             # the tolerance case really stopped early
     assert not np.array_equal(outs[0][0].numpy(), outs[1][0].numpy())
+    # the source-free system through the pipeline, a known-source solve in between
+    sf = [ctx.lsqr_sf_batch_host_async(ins[i][1], w.lam, w.src_ijk, None, maxit=K, omega_idx=w.omega_idx)
+          for i in (0, 1)]
+    mid = ctx.lsqr_batch_host_async(ins[3][0], ins[3][1], w.lam, None, maxit=K, omega_idx=w.omega_idx)
+    sf.append(ctx.lsqr_sf_batch_host_async(ins[2][1], w.lam, w.src_ijk, None, maxit=K, omega_idx=w.omega_idx))
+    ctx.host_wait()
+    assert np.array_equal(mid[0].numpy(), outs[3][0].numpy())
+    for i, (u, a, res, it) in zip((0, 1, 2), sf):
+        us, as_, rs, its = ctx.lsqr_sf_batch_host(ins[i][1], w.lam, w.src_ijk, None, maxit=K, omega_idx=w.omega_idx)
+        assert np.array_equal(u.numpy(), us.numpy()) and np.array_equal(a.numpy(), as_.numpy())
+        assert np.array_equal(res.numpy(), rs.numpy()) and np.array_equal(it.numpy(), its.numpy())
 
 
 def test_two_contexts_and_a_side_stream(torch_cuda):
