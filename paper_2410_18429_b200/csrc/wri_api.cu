@@ -610,12 +610,20 @@ ScalParams scal_params(const wri_ctx* c, const double* partials, int n_rows, con
 
 // Ring depth per pass and plan.  Measured on B200 (profiles/r01_v6_stages.md): the adjoint pass is
 // sensitive to the prefetch distance (more stages in flight cost L2 hits on the stencil halo), with
-// the optimum at 6 stages for one 64- or 48-column chunk per cell and 5 otherwise; pass F at 3
-// (2 for 32-column chunks).
+// the optimum near 130-160 KB of stages in flight: 6 stages for one 64-column chunk per cell, 5 for 32
+// columns or several chunks, 7-8 for the narrower widths with their smaller stages; pass F at 3 (2 for
+// 32-column chunks, 4 for 40).
 template <class Cfg, int MODE>
 int ring_depth(int nchunk) {
-    int n = (MODE == MODE_F) ? (Cfg::CB == 32 ? 2 : 3)
-                             : ((Cfg::CB == 64 && nchunk == 1) || Cfg::CB == 48 || MODE == MODE_G) ? 6 : 5;
+    int n;
+    if (MODE == MODE_F) n = Cfg::CB == 32 ? 2 : Cfg::CB == 40 ? 4 : 3;
+    else if (MODE == MODE_G) n = 6;
+    else if (Cfg::CB == 64) n = nchunk == 1 ? 6 : 5;
+    else if (Cfg::CB == 32) n = 5;
+    else if (Cfg::CB == 56) n = 6;
+    else if (Cfg::CB == 48) n = 7;
+    else if (Cfg::CB == 40 || Cfg::CB == 24) n = 8;
+    else n = 7;                                   // 16, 8, 4, 2 columns: small stages, deeper ring
     if (const char* e = getenv(MODE == MODE_F ? "WRI_F_NSTAGE" : "WRI_A_NSTAGE"))
         if (atoi(e) > 0) n = atoi(e);
     return std::max(2, std::min(n, (int)Cfg::NSTAGE));
