@@ -617,7 +617,7 @@ template <class Cfg, int MODE>
 int ring_depth(int nchunk) {
     int n;
     if (MODE == MODE_F) n = Cfg::CB == 32 ? 2 : Cfg::CB == 40 ? 4 : 3;
-    else if (MODE == MODE_G) n = 6;
+    else if (MODE == MODE_G) n = Cfg::NSTAGE;     // one light stream: the deepest ring the stage layout allows
     else if (Cfg::CB == 64) n = nchunk == 1 ? 6 : 5;
     else if (Cfg::CB == 32) n = 5;
     else if (Cfg::CB == 56) n = 6;
@@ -764,7 +764,7 @@ int launch_tma_apply(wri_ctx* c, const float2* in, float2* out, float sgn) {
     p.sgn = sgn;
     p.phase = -1; p.has_q = 0; p.n_rec = 0;
     p.m_tma = P.m_tma; p.merged = P.merged;
-    p.nstage = ring_depth<Cfg, MODE_A>(P.nchunk);
+    p.nstage = Cfg::NSTAGE;                           // no in-place stream: the deepest ring (measured 7 > 6 > 5)
     p.out = out;
     k_pass_tma<Cfg, MODE_A><<<P.grid, Cfg::NT + 32, smem, c->stream>>>(P.in, P.old, P.old, P.old, P.m, p);
     c->launches++;
