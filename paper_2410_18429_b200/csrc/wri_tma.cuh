@@ -6,13 +6,16 @@
 //     the in-place streams of plane p-1 (old | W | X)      box (CB, TXC,   TYC,   1)
 // into a ring of shared-memory stages with cp.async.bulk.tensor (TMA).  Out-of-grid halo cells
 // and planes -1 / nz are zero-filled by the TMA unit, which IS the Dirichlet closure of the
-// 7-point stencil — no boundary branches in the kernel.  256 consumer threads keep the z
-// pipeline (c_{z-1}, c_z, in-plane neighbour sum n_z) in registers, so every stage is consumed
-// entirely at its own step, and write results straight to HBM with 128-bit stores.
+// 7-point stencil — no boundary branches in the kernel.  The consumer threads (one 16-byte item
+// each, up to 512) keep the z pipeline (c_{z-1}, c_z, in-plane neighbour sum n_z) in registers, so
+// every stage is consumed entirely at its own step, and write results straight to HBM with 128-bit
+// stores.  The ring depth in use is a run-time parameter (TmaPassParams::nstage <= Cfg::NSTAGE).
 //
 // The squared-norm partials are accumulated per column in a fixed order (thread -> tile ->
-// CTA row of partials[]); the last CTA to finish reduces the rows, runs the per-column scalar
-// recurrences and the receiver rows (finalize_phase), so an LSQR iteration is two launches.
+// CTA row of partials[]); the last CTA to finish reduces the rows and runs the per-column scalar
+// recurrences (finalize_phase), so an LSQR iteration is two launches.  Receiver rows: pass F's
+// prologue (P v) and a per-tile correction in pass A (P^T).  The same kernel serves the
+// objective / gradient pass (MODE_G) and, without its in-place stream, the operator entries.
 #pragma once
 #include <cuda.h>
 #include "wri_kernels.cuh"
