@@ -78,6 +78,16 @@ def load_library():
     if _lib is not None:
         return _lib
     path = lib_path()
+    if not os.path.exists(path) and not os.environ.get("WRI_LIB"):
+        # the in-tree library is missing (fresh checkout): build it with nvcc, loudly; never a CPU fallback
+        import sys
+        sys.stderr.write("paper_2410_18429_b200: libwri.so missing, building it with nvcc for sm_100a ...\n")
+        try:
+            from . import build as _build
+            _build.build()
+        except Exception as e:
+            raise WriError(WRI_ERR_CUDA, "libwri.so is not built and building it failed (%s); run python -m "
+                                         "paper_2410_18429_b200.build; there is no CPU fallback" % (e,))
     if not os.path.exists(path):
         raise WriError(WRI_ERR_CUDA, "libwri.so is not built (run python -m paper_2410_18429_b200.build); "
                                      "there is no CPU fallback")
