@@ -98,7 +98,10 @@ int wri_apply_M(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_host, float l
 int wri_apply_MH(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_host, float lambda,
                  const void* ytop_dev, const void* ybot_dev, void* x_dev);
 
-/* wri_lsqr_batch — nb independent LSQR solves in lock-step, b_s = [lambda q_s ; d_s], x0 = 0.
+/* wri_lsqr_batch — nb independent LSQR solves, b_s = [lambda q_s ; d_s], x0 = 0.  Up to 64 columns run in
+ * lock-step (two kernel launches per iteration for all of them); a wider batch whose width is a multiple
+ * of 64 is worked through as successive 64-column groups, each in a compact working set inside the same
+ * workspace (columns are independent systems, so a column's result does not depend on the grouping).
  *   q_dev        c64 [n_g][nb]     d_dev  c64 [n_rec][nb]
  *   tol_dev      float [nb] or NULL; column s stops at the first k with
  *                ||M^H r_k|| / ||M^H b|| <= tol_s  (LSQR's running estimate, reading C-6);
