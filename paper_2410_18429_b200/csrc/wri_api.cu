@@ -9,6 +9,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <type_traits>
 #include <utility>
 #include <vector>
 
@@ -546,43 +547,34 @@ int tma_plan(wri_ctx* c, wri_ctx::TmaPlan& P, const void* in, const void* old, b
     return WRI_OK;
 }
 
+// One place that turns the run-time column-chunk width into its tile configuration: f is called with
+// std::integral_constant<int, CB> for the CB that tma_chunk_for() returned.
+template <class F>
+int dispatch_cb(int cb, F&& f) {
+    switch (cb) {
+        case 64: return f(std::integral_constant<int, 64>{});
+        case 56: return f(std::integral_constant<int, 56>{});
+        case 48: return f(std::integral_constant<int, 48>{});
+        case 40: return f(std::integral_constant<int, 40>{});
+        case 32: return f(std::integral_constant<int, 32>{});
+        case 24: return f(std::integral_constant<int, 24>{});
+        case 8:  return f(std::integral_constant<int, 8>{});
+        case 4:  return f(std::integral_constant<int, 4>{});
+        case 2:  return f(std::integral_constant<int, 2>{});
+        default: return f(std::integral_constant<int, 16>{});
+    }
+}
+
 int tma_setup(wri_ctx* c) {
     c->tma_cb = tma_chunk_for(c->nb);
     if (!c->tma_cb) return WRI_OK;
     if (!get_encode_fn()) { c->tma_cb = 0; return WRI_OK; }
-    int rc;
-    switch (c->tma_cb) {
-        case 64:
-            if ((rc = tma_plan<CfgFor<64, MODE_F>::type>(c, c->planF, c->V, c->U, true))) return rc;
-            return tma_plan<CfgFor<64, MODE_A>::type>(c, c->planA, c->U, c->V, false);
-        case 48:
-            if ((rc = tma_plan<CfgFor<48, MODE_F>::type>(c, c->planF, c->V, c->U, true))) return rc;
-            return tma_plan<CfgFor<48, MODE_A>::type>(c, c->planA, c->U, c->V, false);
-        case 32:
-            if ((rc = tma_plan<CfgFor<32, MODE_F>::type>(c, c->planF, c->V, c->U, true))) return rc;
-            return tma_plan<CfgFor<32, MODE_A>::type>(c, c->planA, c->U, c->V, false);
-        case 8:
-            if ((rc = tma_plan<CfgFor<8, MODE_F>::type>(c, c->planF, c->V, c->U, true))) return rc;
-            return tma_plan<CfgFor<8, MODE_A>::type>(c, c->planA, c->U, c->V, false);
-        case 4:
-            if ((rc = tma_plan<CfgFor<4, MODE_F>::type>(c, c->planF, c->V, c->U, true))) return rc;
-            return tma_plan<CfgFor<4, MODE_A>::type>(c, c->planA, c->U, c->V, false);
-        case 2:
-            if ((rc = tma_plan<CfgFor<2, MODE_F>::type>(c, c->planF, c->V, c->U, true))) return rc;
-            return tma_plan<CfgFor<2, MODE_A>::type>(c, c->planA, c->U, c->V, false);
-        case 56:
-            if ((rc = tma_plan<CfgFor<56, MODE_F>::type>(c, c->planF, c->V, c->U, true))) return rc;
-            return tma_plan<CfgFor<56, MODE_A>::type>(c, c->planA, c->U, c->V, false);
-        case 40:
-            if ((rc = tma_plan<CfgFor<40, MODE_F>::type>(c, c->planF, c->V, c->U, true))) return rc;
-            return tma_plan<CfgFor<40, MODE_A>::type>(c, c->planA, c->U, c->V, false);
-        case 24:
-            if ((rc = tma_plan<CfgFor<24, MODE_F>::type>(c, c->planF, c->V, c->U, true))) return rc;
-            return tma_plan<CfgFor<24, MODE_A>::type>(c, c->planA, c->U, c->V, false);
-        default:
-            if ((rc = tma_plan<CfgFor<16, MODE_F>::type>(c, c->planF, c->V, c->U, true))) return rc;
-            return tma_plan<CfgFor<16, MODE_A>::type>(c, c->planA, c->U, c->V, false);
-    }
+    return dispatch_cb(c->tma_cb, [&](auto cb) -> int {
+        constexpr int CB = decltype(cb)::value;
+        int rc = tma_plan<typename CfgFor<CB, MODE_F>::type>(c, c->planF, c->V, c->U, true);
+        if (rc) return rc;
+        return tma_plan<typename CfgFor<CB, MODE_A>::type>(c, c->planA, c->U, c->V, false);
+    });
 }
 
 ScalParams scal_params(const wri_ctx* c, const double* partials, int n_rows, const float2* d) {
@@ -690,18 +682,9 @@ int launch_tma_cfg(wri_ctx* c, int phase) {
 
 template <int MODE>
 int launch_tma(wri_ctx* c, int phase) {
-    switch (c->tma_cb) {
-        case 64: return launch_tma_cfg<typename CfgFor<64, MODE>::type, MODE>(c, phase);
-        case 48: return launch_tma_cfg<typename CfgFor<48, MODE>::type, MODE>(c, phase);
-        case 32: return launch_tma_cfg<typename CfgFor<32, MODE>::type, MODE>(c, phase);
-        case 8: return launch_tma_cfg<typename CfgFor<8, MODE>::type, MODE>(c, phase);
-        case 4: return launch_tma_cfg<typename CfgFor<4, MODE>::type, MODE>(c, phase);
-        case 2: return launch_tma_cfg<typename CfgFor<2, MODE>::type, MODE>(c, phase);
-        case 56: return launch_tma_cfg<typename CfgFor<56, MODE>::type, MODE>(c, phase);
-        case 40: return launch_tma_cfg<typename CfgFor<40, MODE>::type, MODE>(c, phase);
-        case 24: return launch_tma_cfg<typename CfgFor<24, MODE>::type, MODE>(c, phase);
-        default: return launch_tma_cfg<typename CfgFor<16, MODE>::type, MODE>(c, phase);
-    }
+    return dispatch_cb(c->tma_cb, [&](auto cb) -> int {
+        return launch_tma_cfg<typename CfgFor<decltype(cb)::value, MODE>::type, MODE>(c, phase);
+    });
 }
 
 // objective + gradient through the TMA pipeline (one chunk per cell, power-of-two column pairs)
@@ -779,19 +762,9 @@ int apply_operator(wri_ctx* c, int nb, const float2* in, float2* out, float sgn)
     if (cb) {
         const int nb_saved = c->nb;
         c->nb = nb;
-        int rc;
-        switch (cb) {
-            case 64: rc = launch_tma_apply<64>(c, in, out, sgn); break;
-            case 56: rc = launch_tma_apply<56>(c, in, out, sgn); break;
-            case 48: rc = launch_tma_apply<48>(c, in, out, sgn); break;
-            case 40: rc = launch_tma_apply<40>(c, in, out, sgn); break;
-            case 32: rc = launch_tma_apply<32>(c, in, out, sgn); break;
-            case 24: rc = launch_tma_apply<24>(c, in, out, sgn); break;
-            case 16: rc = launch_tma_apply<16>(c, in, out, sgn); break;
-            case 8:  rc = launch_tma_apply<8>(c, in, out, sgn); break;
-            case 4:  rc = launch_tma_apply<4>(c, in, out, sgn); break;
-            default: rc = launch_tma_apply<2>(c, in, out, sgn); break;
-        }
+        const int rc = dispatch_cb(cb, [&](auto t) -> int {
+            return launch_tma_apply<decltype(t)::value>(c, in, out, sgn);
+        });
         c->nb = nb_saved;
         return rc;
     }
