@@ -486,8 +486,14 @@ int tma_plan(wri_ctx* c, wri_ctx::TmaPlan& P, const void* in, const void* old, b
     P.ntx = (c->g.nx + P.txc - 1) / P.txc;
     P.nty = (c->g.ny + P.tyc - 1) / P.tyc;
     const long long per_plane = (long long)P.nchunk * P.ntx * P.nty;
-    int zc = std::min(c->g.nz, 32);
-    const char* zenv = getenv("WRI_ZC");
+    // planes per tile: 32, except pass F with one 64-column chunk per cell: 16 — measured
+    // (profiles/r01_v6_stages.md): shorter tiles shorten the time between the waves of tiles, so more of
+    // the halo shared across a wave boundary is still in L2, at the price of two more halo planes per
+    // tile; at 128^3 x 64 pass F gains (0.929 -> 0.947), pass A loses (0.938 -> 0.907), and at 32 or 48
+    // columns (256^3, 200x200x160) F does not gain either.  WRI_ZC / WRI_ZC_F / WRI_ZC_A override.
+    int zc = std::min(c->g.nz, (is_f && Cfg::CB == 64 && P.nchunk == 1) ? 16 : 32);
+    const char* zenv = getenv(is_f ? "WRI_ZC_F" : "WRI_ZC_A");
+    if (!zenv) zenv = getenv("WRI_ZC");
     if (zenv && atoi(zenv) > 0) zc = std::min(c->g.nz, atoi(zenv));
     else
         while (zc > 8 && per_plane * ((c->g.nz + zc - 1) / zc) < 16LL * c->num_sms) zc = (zc + 1) / 2;
