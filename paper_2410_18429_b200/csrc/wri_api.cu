@@ -491,7 +491,8 @@ int tma_plan(wri_ctx* c, wri_ctx::TmaPlan& P, const void* in, const void* old, b
     // the halo shared across a wave boundary is still in L2, at the price of two more halo planes per
     // tile; at 128^3 x 64 pass F gains (0.929 -> 0.947), pass A loses (0.938 -> 0.907), and at 32 or 48
     // columns (256^3, 200x200x160) F does not gain either.  WRI_ZC / WRI_ZC_F / WRI_ZC_A override.
-    int zc = std::min(c->g.nz, (is_f && Cfg::CB == 64 && P.nchunk == 1) ? 16 : 32);
+    // (pass F at 32 columns: 128 planes, 0.945 -> 0.957 at 256^3 x 32)
+    int zc = std::min(c->g.nz, (is_f && Cfg::CB == 64 && P.nchunk == 1) ? 16 : (is_f && Cfg::CB == 32) ? 128 : 32);
     const char* zenv = getenv(is_f ? "WRI_ZC_F" : "WRI_ZC_A");
     if (!zenv) zenv = getenv("WRI_ZC");
     if (zenv && atoi(zenv) > 0) zc = std::min(c->g.nz, atoi(zenv));
