@@ -38,7 +38,8 @@ class _RefOp(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
                 ("h", C.c_double), ("omega", C.c_double),
                 ("sponge_width", C.c_int32), ("gamma_max", C.c_double),
-                ("power", C.c_int32), ("faces", C.c_uint32), ("periodic", C.c_int32)]
+                ("power", C.c_int32), ("faces", C.c_uint32), ("periodic", C.c_int32),
+                ("stencil", C.c_int32), ("round_c64", C.c_int32)]
 
 
 class _RefState(C.Structure):
@@ -111,6 +112,8 @@ class Operator:
     power: int = 2
     faces: int = 0x3F
     periodic: bool = False   # test-only boundary rule for the plane-wave pin
+    stencil: int = 0         # 0: 7-point star, 1: 27-point box (reading C-23)
+    round_c64: bool = False  # test-only: LSQR vectors stored in complex64 (attainable-floor emulation)
 
     @property
     def ng(self) -> int:
@@ -119,7 +122,8 @@ class Operator:
     def _c(self) -> _RefOp:
         return _RefOp(self.nx, self.ny, self.nz, float(self.h), float(self.omega),
                       int(self.sponge_width), float(self.gamma_max), int(self.power),
-                      int(self.faces), int(bool(self.periodic)))
+                      int(self.faces), int(bool(self.periodic)), int(self.stencil),
+                      int(bool(self.round_c64)))
 
 
 def _f64(a, n):

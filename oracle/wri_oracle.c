@@ -16,15 +16,17 @@
  *                  ("A_j(m) = omega_j^2 diag(m) + Delta"); 2nd-order 7-point
  *                  stencil and the (1+i gamma) sponge are fixed by
  *                  BASELINE.json north_star; zero (Dirichlet) outside the grid,
- *                  DESIGN.md reading C-3.
+ *                  DESIGN.md reading C-3.  op->stencil = 1 selects the 27-point
+ *                  box discretisation of the same Laplacian (SURVEY.md §8(f)
+ *                  NEXT-4, reading C-23), written out as its definition.
  *   ref_apply_M    M v = [lambda A v ; P v], PAPER.md:78-85 (eq. 5-6) with the
  *                  source weight fixed (reading C-5); P = sampling of receiver
  *                  nodes.
  *   ref_apply_MH   M^H y = lambda A^H y_top + P^T y_bot (PAPER.md:95, 118 write
- *                  "T"; conjugate transpose is meant, reading C-2).  A^H is
- *                  written out here as its own stencil (conjugated diagonal),
- *                  not derived from ref_apply_A, so the adjoint dot test pins
- *                  both.
+ *                  "T"; conjugate transpose is meant, reading C-2).  A and A^H
+ *                  share one stencil routine (apply_A_impl) with a flag that
+ *                  conjugates the diagonal; the adjoint dot test and
+ *                  test_adjoint_of_A_alone_and_symmetry pin that flag.
  *   ref_lsqr       Paige & Saunders (1982) LSQR, the algorithm the paper names
  *                  and cites.  Algorithm 1 as
  *                  printed is garbled (reading C-1); the recurrences below are
@@ -40,7 +42,12 @@
  * end of this file list theirs in their own headers): adjoint dot test, closed-form eigenpairs
  * (periodic plane wave, Dirichlet sine modes), printed sponge values, dense
  * LAPACK least squares on 8^3, SciPy LSQR, CGLS, estimate-vs-true residuals,
- * monotone ||r||, consistent system, breakdown cases.
+ * monotone ||r||, consistent system, breakdown cases.  27-point stencil
+ * (tests/test_oracle_stencil27.py): closed-form symbol on the periodic box and on
+ * Dirichlet sine modes, second-order convergence to the continuous Laplacian,
+ * dot test, dense least squares.  round_c64 (tests/test_oracle_c64floor.py):
+ * flag off is bit-identical to the plain solver; with it the iterates stay
+ * within float32 rounding of the plain ones on a well-conditioned problem.
  * Unpinned: nothing in this file.  (Free-running complex64-vs-complex128
  * agreement on configs[0] is a property of the problem, C-12.)
  */
@@ -61,6 +68,10 @@ typedef struct {
     int32_t power;       /* exponent of the profile                           */
     uint32_t faces;      /* bit0..5 = x-,x+,y-,y+,z-,z+                        */
     int32_t periodic;    /* TEST ONLY: wrap neighbours (closed-form pin P2a)  */
+    int32_t stencil;     /* 0: 7-point star (north_star); 1: 27-point box, reading C-23 */
+    int32_t round_c64;   /* TEST ONLY: LSQR keeps u, v, w, x in complex64 STORAGE (rounded
+                          * after every step; all arithmetic stays complex128) — the
+                          * attainable floor of a complex64 solver, SURVEY C-12(iii)       */
 } ref_op;
 
 /* depth into the sponge along one axis, in cells: max(L - i, i - (n-1-L), 0)
@@ -118,10 +129,25 @@ static void apply_A_impl(const ref_op *op, const double *m, const double *gamma,
         for (int iy = 0; iy < ny; ++iy)
             for (int ix = 0; ix < nx; ++ix) {
                 size_t c = ((size_t)iz * ny + iy) * nx + ix;
-                zc lap = nb(op, v, ix - 1, iy, iz) + nb(op, v, ix + 1, iy, iz) +
-                         nb(op, v, ix, iy - 1, iz) + nb(op, v, ix, iy + 1, iz) +
-                         nb(op, v, ix, iy, iz - 1) + nb(op, v, ix, iy, iz + 1) -
-                         6.0 * v[c];
+                zc lap;
+                if (op->stencil == 1) {
+                    /* 27-point box stencil (reading C-23): the member of the family
+                     *   h^2 Lap_h = a0 v_c + a1 sum(6 faces) + a2 sum(12 edges) + a3 sum(8 corners)
+                     * that is consistent (a0 + 6 a1 + 12 a2 + 8 a3 = 0, a1 + 4 a2 + 4 a3 = 1), has an
+                     * isotropic leading error term (a2 + 2 a3 = 1/6) and a3 = 1/30:
+                     *   a0 = -128/30, a1 = 14/30, a2 = 3/30, a3 = 1/30. */
+                    zc sum[4] = {0.0, 0.0, 0.0, 0.0};
+                    for (int dz = -1; dz <= 1; ++dz)
+                        for (int dy = -1; dy <= 1; ++dy)
+                            for (int dx = -1; dx <= 1; ++dx)
+                                sum[(dx != 0) + (dy != 0) + (dz != 0)] += nb(op, v, ix + dx, iy + dy, iz + dz);
+                    lap = (-128.0 * sum[0] + 14.0 * sum[1] + 3.0 * sum[2] + 1.0 * sum[3]) / 30.0;
+                } else {
+                    lap = nb(op, v, ix - 1, iy, iz) + nb(op, v, ix + 1, iy, iz) +
+                          nb(op, v, ix, iy - 1, iz) + nb(op, v, ix, iy + 1, iz) +
+                          nb(op, v, ix, iy, iz - 1) + nb(op, v, ix, iy, iz + 1) -
+                          6.0 * v[c];
+                }
                 zc mass = w2 * m[c] * (1.0 + I * gamma[c]);
                 if (conj_diag) mass = conj(mass);
                 y[c] = lap * ih2 + mass * v[c];
@@ -188,6 +214,12 @@ static double norm2(const zc *a, size_t na, const zc *b, size_t nb_) {
     return sqrt(s);
 }
 
+/* TEST ONLY (op->round_c64): complex64 storage of a vector — each component is
+ * rounded to float and promoted back. */
+static void round_vec(zc *a, size_t n) {
+    for (size_t i = 0; i < n; ++i) a[i] = (double)(float)creal(a[i]) + I * (double)(float)cimag(a[i]);
+}
+
 /* LSQR state of one column, all vectors NORMALISED as in Paige & Saunders:
  * ||u|| = ||v|| = 1 (unless broken down). */
 typedef struct {
@@ -244,6 +276,10 @@ static void lsqr_step_g(const ref_op *op, const double *m, const double *gamma, 
     for (size_t i = 0; i < ng; ++i) {
         st->x[i] += t1 * st->w[i];
         st->w[i] = st->v[i] - t2 * st->w[i];
+    }
+    if (op->round_c64) {
+        round_vec(st->u_top, ng); round_vec(st->u_bot, (size_t)n_rec);
+        round_vec(st->v, ng); round_vec(st->w, ng); round_vec(st->x, ng);
     }
     st->alpha = alpha;
     st->beta = beta;
@@ -310,6 +346,10 @@ int32_t ref_lsqr(const ref_op *op, const double *m, double lambda, int32_t n_rec
         if (arnorms) arnorms[0] = ar0;
         if (alpha > 0.0) {
             for (size_t i = 0; i < ng; ++i) { st.v[i] /= alpha; st.w[i] = st.v[i]; }
+            if (op->round_c64) {
+                round_vec(st.u_top, ng); round_vec(st.u_bot, (size_t)n_rec);
+                round_vec(st.v, ng); round_vec(st.w, ng);
+            }
             st.alpha = alpha; st.beta = beta; st.phibar = beta; st.rhobar = alpha;
             for (int32_t k = 1; k <= maxit; ++k) {
                 lsqr_step_g(op, m, gamma, lambda, n_rec, rec, &st, tmp_top, tmp_bot);
@@ -454,6 +494,10 @@ static void lsqr_sf_step_g(const ref_op *op, const double *m, const double *gamm
     }
     st->x_a += t1 * st->w_a;
     st->w_a = st->v_a - t2 * st->w_a;
+    if (op->round_c64) {          /* the alpha entries live in double on the GPU too: not rounded */
+        round_vec(st->u_top, ng); round_vec(st->u_bot, (size_t)n_rec);
+        round_vec(st->v, ng); round_vec(st->w, ng); round_vec(st->x, ng);
+    }
     st->alpha = alpha;
     st->beta = beta;
     st->rho = rho; st->c = c; st->s = s; st->theta = theta; st->phi = phi;
@@ -515,6 +559,10 @@ int32_t ref_lsqr_sf(const ref_op *op, const double *m, double lambda, int32_t n_
         if (alpha > 0.0) {
             for (size_t i = 0; i < ng; ++i) { st.v[i] /= alpha; st.w[i] = st.v[i]; }
             st.v_a /= alpha; st.w_a = st.v_a;
+            if (op->round_c64) {
+                round_vec(st.u_top, ng); round_vec(st.u_bot, (size_t)n_rec);
+                round_vec(st.v, ng); round_vec(st.w, ng);
+            }
             st.alpha = alpha; st.beta = beta; st.phibar = beta; st.rhobar = alpha;
             for (int32_t k = 1; k <= maxit; ++k) {
                 lsqr_sf_step_g(op, m, gamma, lambda, n_rec, rec, src, &st, tmp_top, tmp_bot);
