@@ -166,7 +166,8 @@ def e2e_entry(iters_all, serial_steps, serial_s, pipe_steps, pipe_s, h2d, d2h):
 
 
 def oracle_sample(w, cores, iters):
-    """Time the CPU oracle as it stands on min(nb, cores) columns x `iters` iterations."""
+    """Time the CPU oracle as it stands on min(nb, cores) columns x `iters` iterations
+    (one column per thread; cores = 1 gives the single-thread figure)."""
     from oracle import oracle as O
     ncols = max(1, min(w.nb, cores))
     cols = list(range(ncols))
@@ -220,18 +221,21 @@ def run_ours(args, wl_name, w):
         raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-    # WRI_BENCH_DIST1=1 (developer switch): take the N > 1 code path with one rank under torchrun
-    use_dist = world > 1 or os.environ.get("WRI_BENCH_DIST1") == "1"
+    use_dist = world > 1
     if use_dist:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
 
     from paper_2410_18429_b200 import Wri
     ctx = Wri.from_workload(w, device=dev)
+    if args.stencil:
+        ctx.set_stencil(args.stencil)
+    if args.debug_opts:
+        ctx.set_debug_opts(**{k: int(v) for k, v in (kv.split("=") for kv in args.debug_opts.split(","))})
     nb, maxit = w.nb, w.maxit
     q = torch.from_numpy(w.Q).to(dev)
     d = torch.from_numpy(w.D).to(dev)
-    tol = torch.from_numpy(w.tol).to(dev) if (w.tol > 0).any() else None
+    tol = torch.from_numpy(w.tol).to(dev) if ((w.tol > 0).any() and not args.fixed_k) else None
     ctx.ensure_workspace(nb, host_staging=True, compaction=tol is not None)
     out = ctx._outputs(nb, maxit, dev)
 
@@ -275,7 +279,7 @@ def run_ours(args, wl_name, w):
     outh = (torch.empty((w.ng, nb), dtype=torch.complex64).pin_memory(),
             torch.empty((maxit + 1, nb), dtype=torch.float32).pin_memory(),
             torch.empty(nb, dtype=torch.int32).pin_memory())
-    e2e_steps = max(1, min(args.steps, 3))
+    e2e_steps = max(1, args.steps)
     ctx.lsqr_batch_host(qh, dh, w.lam, tolh, maxit=maxit, omega_idx=w.omega_idx, out=outh)   # warm-up
     barrier()
     t0 = time.perf_counter()
@@ -338,16 +342,17 @@ def run_ours(args, wl_name, w):
         # the operator entries on their own (wri_apply_M / wri_apply_MH): read x, write y = 16 B per cell-column
         ev2 = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
         yb = torch.empty((w.n_rec, nb), dtype=torch.complex64, device=dev)
-        ctx.apply_M(u_sf, w.lam, w.omega_idx); ctx.apply_MH(u_sf, yb, w.lam, w.omega_idx)
+        yt = torch.empty_like(u_sf)
+        ctx.apply_M(u_sf, w.lam, w.omega_idx, out=(yt, yb)); ctx.apply_MH(u_sf, yb, w.lam, w.omega_idx, out=yt)
         torch.cuda.synchronize()
         n_ap = 5
         ev2[0].record()
         for _ in range(n_ap):
-            ctx.apply_M(u_sf, w.lam, w.omega_idx)
+            ctx.apply_M(u_sf, w.lam, w.omega_idx, out=(yt, yb))
         ev2[1].record()
         ev2[2].record()
         for _ in range(n_ap):
-            ctx.apply_MH(u_sf, yb, w.lam, w.omega_idx)
+            ctx.apply_MH(u_sf, yb, w.lam, w.omega_idx, out=yt)
         ev2[3].record()
         torch.cuda.synchronize()
         bytes_ap = (16 * nb + 4) * w.ng
@@ -355,8 +360,8 @@ def run_ours(args, wl_name, w):
             ms_ap = ev2[a].elapsed_time(ev2[b]) / n_ap
             extras[nm] = {"ms": ms_ap, "algorithmic_bytes": bytes_ap, "achieved": bytes_ap / (ms_ap * 1e-3) / 1e9,
                           "unit": "GB/s", "frac": bytes_ap / (ms_ap * 1e-3) / 1e9 / peak_g,
-                          "note": "includes the output allocation of the Python binding"}
-        del yb
+                          "note": "the C call into caller-allocated outputs (pass kernel + receiver rows)"}
+        del yb, yt
         # one misfit evaluation (Algorithm 2 lines 4-5; the unit the paper times in Table 1):
         # source-free solve of every column to a tolerance + objective + gradient, one C-ABI call
         eps_m = 1e-2
@@ -419,14 +424,18 @@ def run_ours(args, wl_name, w):
             "config": {"workload": wl_name, "grid": [w.nx, w.ny, w.nz], "h": w.h, "nb": nb,
                        "n_rec": w.n_rec, "freqs_hz": list(w.freqs), "lambda": w.lam, "maxit": maxit,
                        "iters_per_step": iters_per_step, "sharding": "columns per rank, no collective",
+                       "stencil": "27-point" if args.stencil else "7-point", "tile_plan": ctx.plan_info(nb + (nb & 1)),
                        "l2": "working set %.1f GB per rank exceeds the 126 MB L2" % (4 * cells * 8 / 1e9)},
             "clocks": clocks,
             "e2e": e2e_entry(iters_e2e_all, e2e_steps, e2e_s, e2e_pipe_steps, e2e_pipe_s, h2d, d2h),
             "gpu_launches": launches_all,
-            "roofline": {"bound": "hbm", "kernel": "k_pass_tma<MODE_F> (forward stencil + u axpy + x,w update + ||u||^2)",
+            "roofline": {"bound": "hbm", "kernel": "k_pass_rt<MODE_F> (forward stencil + u axpy + x,w update + ||u||^2)",
                          "achieved": ach_f, "peak": peak, "peak_source": peak_src, "unit": "GB/s",
                          "frac": (ach_f / peak) if ach_f else None,
                          "traffic": ncu_traffic_bytes() if wl_name == DEFAULT_WORKLOAD else None,
+                         "traffic_source": ("profiles/traffic_pass_f.csv (static: one ncu --set full capture of this "
+                                            "kernel at this workload, committed; not re-measured per run)"
+                                            if wl_name == DEFAULT_WORKLOAD else None),
                          "algorithmic_bytes_per_launch": bytes_f,
                          "avg_launch_ms": ms_f / max(n_f, 1), "launches_timed": n_f,
                          "avg_columns_per_launch": cols_f / max(n_f, 1),
@@ -437,11 +446,19 @@ def run_ours(args, wl_name, w):
         }
         if extras:
             line["extras"] = extras
+            for key, src in (("pass_g", "objective_gradient"), ("apply_M", "apply_M"), ("apply_MH", "apply_MH")):
+                if src in extras and "frac" in extras[src]:
+                    line["roofline"][key] = {"achieved": extras[src]["achieved"], "frac": extras[src]["frac"],
+                                             "ms": extras[src]["ms"]}
         if world == 1 and not args.no_cpu_baseline:
             cores = os.cpu_count() or 1
             r, ncols, dt, sample = oracle_sample(w, cores, oracle_iters_for(w))
             line["cpu_baseline"] = {"value": r, "unit": UNIT, "cores": ncols, "kind": "oracle",
                                     "sample": sample, "seconds": dt}
+            it1 = max(2, oracle_iters_for(w) // 2)
+            r1, _, dt1, sample1 = oracle_sample(w, 1, it1)
+            line["cpu_baseline"]["one_thread"] = {"value": r1, "unit": UNIT, "cores": 1, "sample": sample1,
+                                                  "seconds": dt1}
         print(json.dumps(line), flush=True)
     if use_dist:
         dist.destroy_process_group()
@@ -455,6 +472,14 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(WORKLOADS))
     ap.add_argument("--maxit", type=int, default=None, help="override the workload's iteration count")
+    ap.add_argument("--nb", type=int, default=None,
+                    help="sub-sample the workload's columns to this batch width (per-width kernel tables)")
+    ap.add_argument("--fixed-k", action="store_true",
+                    help="ignore the workload's tolerances: every column runs maxit iterations")
+    ap.add_argument("--stencil", type=int, default=0, choices=[0, 1],
+                    help="0: 7-point (north_star), 1: 27-point box discretisation of the Laplacian")
+    ap.add_argument("--debug-opts", default=None,
+                    help="tuning switches of wri_debug_opts, e.g. txc=4,tyc=4,nstage_a=8 (sweeps under profiles/)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true",
                     help="skip the source-free solve and the objective/gradient context lines")
@@ -463,6 +488,8 @@ def main():
     if args.impl == "reference" and dist_env()[0] != 0:
         return                                   # the oracle arm runs on rank 0 alone
     spec = dict(WORKLOADS[args.workload])
+    if args.nb:
+        spec["nb"] = args.nb
     w = workloads.make(spec.pop("name"), **spec)
     if args.maxit:
         w.maxit = args.maxit

@@ -46,6 +46,7 @@ extern "C" {
 #define WRI_ERR_WORKSPACE        -4   /* workspace missing or too small                            */
 #define WRI_ERR_CUDA             -5   /* CUDA runtime error; text via wri_strerror                 */
 #define WRI_ERR_STATE            -6   /* call out of order (e.g. iterate before begin)             */
+#define WRI_ERR_NUMERIC          -7   /* wri_awri_step: the objective at the current model is not finite */
 
 typedef struct wri_ctx wri_ctx;                 /* opaque, library-owned */
 
@@ -77,11 +78,48 @@ int wri_create(wri_ctx** out, wri_grid grid, double h,
 /* m changes every outer iteration of the inversion (Algorithm 2). */
 int wri_set_model(wri_ctx* ctx, const float* m_dev);
 
+/* Discretisation of the Laplacian in A(m) (PAPER.md:56 says only "discretized 3D Laplacian"; readings
+ * C-3 and C-23 of DESIGN.md), sticky for every later call of the context:
+ *   WRI_STENCIL_7   2nd-order 7-point star (north_star; the default)
+ *   WRI_STENCIL_27  2nd-order 27-point box with an isotropic leading error term: centre -128/30, the
+ *                   6 face neighbours 14/30, the 12 edge neighbours 3/30, the 8 corner neighbours 1/30,
+ *                   all over h^2; zero (Dirichlet) outside the grid, so A stays complex-symmetric.
+ * The mass term omega^2 m (1 + i gamma) stays on the diagonal.  Same bytes per iteration as the
+ * 7-point stencil (the halo is still one cell).                                                  */
+#define WRI_STENCIL_7  0
+#define WRI_STENCIL_27 1
+int wri_set_stencil(wri_ctx* ctx, int32_t stencil);
+
+/* Tuning and test switches of the kernels behind the entries (all zero = the library's own choices;
+ * NULL restores that).  Results do not depend on them beyond rounding order, except that no_compact /
+ * no_groups / generic select code paths whose results the tests compare with the default ones.
+ *   nstage_f / nstage_a   depth of the shared-memory ring of the forward / adjoint pass
+ *   zc_f / zc_a           planes per tile
+ *   txc / tyc             cells per tile in x / y
+ *   no_compact            keep converged columns in the working set (they stay frozen)
+ *   no_groups             run a batch wider than 64 columns in lock-step instead of 64-column groups
+ *   generic               use the plain (non-TMA) kernels for every width
+ *   no_graph              enqueue the iterations one by one instead of the device-side loop        */
+typedef struct {
+    int32_t nstage_f, nstage_a, zc_f, zc_a, txc, tyc;
+    int32_t no_compact, no_groups, generic, no_graph;
+} wri_debug_opts;
+int wri_set_debug_opts(wri_ctx* ctx, const wri_debug_opts* opts);
+
+/* Tile plan the pass kernel would use for batch width nb (introspection for bench.py and the tuning
+ * tables under profiles/): out16 = { column chunk, chunks per cell, cells per tile in x, in y, consumer
+ * threads with work, merged tensor maps, model tile by TMA, pass F: planes per tile, ring depth, tiles,
+ * pass A: planes per tile, ring depth, tiles, bytes per stage of pass F, of pass A, persistent grid }.
+ * WRI_ERR_ARG when the width is served by the generic kernels (odd widths).                        */
+int wri_plan_info(wri_ctx* ctx, int32_t nb, int32_t* out16);
+
 /* Workspace for wri_lsqr_* at batch width nb (u, v, w vectors, receiver rows, reduction
  * partials).  flags: WRI_WS_HOST_STAGING adds room for the device copies wri_lsqr_batch_host
- * needs; WRI_WS_COMPACTION adds two more vectors so that converged columns can be compacted
- * out of the working set when per-column tolerances are given (without it such a solve still
- * stops early once every column has converged, but converged columns keep costing bandwidth).
+ * needs; WRI_WS_COMPACTION adds five more vectors: with per-column tolerances the working set then
+ * lives entirely in the workspace and has a second vector set, so that converged columns can be
+ * compacted out of it on the device (without it such a solve still stops early once every column
+ * has converged, but converged columns keep costing bandwidth); an odd batch width uses one of them
+ * to run in an even-width working set on the fast kernel.
  * The caller allocates (e.g. a torch uint8 tensor) and hands it over; it must stay alive and
  * untouched while a solve is in flight.                                                      */
 #define WRI_WS_HOST_STAGING 1
@@ -111,11 +149,12 @@ int wri_apply_MH(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_host, float 
  *                after a column stops (reading C-9); may be NULL (no history wanted)
  *   iters_dev    int32 [nb] iterations performed per column (may be NULL)
  * Equivalent to wri_lsqr_begin + wri_lsqr_iterate(maxit) + wri_lsqr_end.  Needs a workspace.
- * With tol_dev == NULL the call only enqueues work.  With tolerances the host reads the
- * per-column active flags back every few iterations (one stream synchronisation each, about
- * every 2 ms of device work): the solve returns as soon as every column has stopped, and
- * stopped columns are compacted out of the working set (adaptive accuracy, PAPER.md:180-211;
- * "the active mask shrinking as sources converge", BASELINE.json configs[3]).                */
+ * The call only enqueues work, with or without tolerances: the state of the solve (iteration
+ * count, active flags, working width) lives on the device.  With tolerances the finaliser of
+ * each iteration counts the live columns; once the bandwidth spent on stopped ones exceeds the
+ * price of re-packing, a kernel compacts them out of the working set (adaptive accuracy,
+ * PAPER.md:180-211; "the active mask shrinking as sources converge", BASELINE.json configs[3]),
+ * and once every column has stopped the remaining launches return at once.                   */
 int wri_lsqr_batch(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_host,
                    const void* q_dev, const void* d_dev, float lambda,
                    const float* tol_dev, int32_t maxit,
@@ -225,7 +264,8 @@ int wri_lsqr_set_opts(wri_ctx* ctx, const wri_lsqr_opts* opts);
  * m_trial on the given stream and return 0; with update == NULL the built-in steepest-descent
  * update m_tilde = clamp(m - step * g, m_min, m_max) is used.  Algorithm 2 does not bound the
  * "go back" loop: after max_halvings halvings the step is reported as rejected and m_dev is left
- * unchanged (reading C-20).  warm_restart = 1 continues the re-solve of line 4 from x_bar.
+ * unchanged (reading C-20).  A trial objective that is not finite counts as a rejected step; a
+ * non-finite objective at the current model returns WRI_ERR_NUMERIC with m_dev unchanged.  warm_restart = 1 continues the re-solve of line 4 from x_bar.
  * The comparison of line 9 is made on the host in double (one stream synchronisation per
  * evaluation).  During the call the context's model pointer is switched between m_dev and
  * m_trial_dev and restored on return.
@@ -238,12 +278,18 @@ int wri_lsqr_set_opts(wri_ctx* ctx, const wri_lsqr_opts* opts);
 #define WRI_AWRI_MAX_TRACE 16
 typedef int (*wri_update_fn)(void* user, const float* m_dev, const float* g_dev, float* m_trial_dev,
                              void* cuda_stream);
+/* Sum over ranks (column sharding): eq. 8-9 are sums over all sources and frequencies.
+ * reduce(user, f_host, g_dev, n_g, cuda_stream) must replace *f_host (HOST double) by its sum over the
+ * ranks and, when g_dev is not NULL, ENQUEUE on the given stream the all-reduce of the float32 [n_g]
+ * gradient; return 0.  Every rank then holds the same f, f_tilde and g, and takes the same decision. */
+typedef int (*wri_reduce_fn)(void* user, double* f_host, float* g_dev, int64_t n_g, void* cuda_stream);
 typedef struct {
     int32_t       max_halvings;     /* < WRI_AWRI_MAX_TRACE                                      */
     int32_t       warm_restart;
     wri_update_fn update;           /* NULL: built-in steepest descent with the fields below     */
     void*         user;
     float         step, m_min, m_max;
+    wri_reduce_fn reduce;           /* NULL: this process holds every column                     */
 } wri_awri_opts;
 typedef struct {
     int32_t accepted, n_halvings, n_trace;

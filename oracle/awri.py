@@ -20,6 +20,9 @@ awri_step   lines 4-14 of Algorithm 2, written out in the paper's order:
               13: else m <- m_tilde
             Readings (C-20): Algorithm 2 has no bound on the "go back" loop; a cap
             max_halvings is added, after which the step is returned as rejected with m unchanged.
+            Line 9 compares numbers: a trial objective that is not finite (an update that left
+            the physical range) counts as "f_tilde > f" (rejected); a non-finite f at the
+            current model is an error.
             When the loop goes back to line 4 the re-solve at the same m may continue from
             x_bar (Algorithm 1 leaves x0 free; warm=True), with the stop rule still relative to
             the cold problem's ||S^H b|| (C-17); warm=False solves from zero as printed.
@@ -65,8 +68,11 @@ def misfit_sf(ops, m, lam, rec, src_cells, D, eps, maxit, x0=None, a0=None, ar_r
     return dict(f=float(f_cols.sum()), f_cols=f_cols, g=g, U=U, alpha=alpha, iters=iters, ar0=ar0)
 
 
-def awri_step(ops, m, lam, rec, src_cells, D, eps, maxit, update, max_halvings=8, warm=False):
+def awri_step(ops, m, lam, rec, src_cells, D, eps, maxit, update, max_halvings=8, warm=False, reduce=None):
     """Lines 4-14 of Algorithm 2 for the model m (float array [n_g]).  update(m, g) -> m_tilde.
+    reduce(f, g) -> f: the sums of eq. 8-9 taken over column blocks held elsewhere (column sharding,
+    PAPER.md:221): returns the summed objective and sums g (a float64 array, or None) in place;
+    None = these are all the columns.
 
     Returns dict(accepted, m (the next model), eps (the tolerance in force at the end),
     n_halvings, f, f_trial, g (gradient at the entry model with the final eps), lsqr_iters
@@ -83,11 +89,17 @@ def awri_step(ops, m, lam, rec, src_cells, D, eps, maxit, update, max_halvings=8
         else:
             cur = misfit_sf(ops, m, lam, rec, src_cells, D, eps, maxit)          # lines 4-5
         total += int(cur["iters"].sum())
+        if reduce is not None:
+            cur["f"] = reduce(cur["f"], cur["g"])
+        if not np.isfinite(cur["f"]):
+            raise FloatingPointError("objective at the current model is not finite")
         m_t = update(m, cur["g"])                                                  # line 6
         tri = misfit_sf(ops, m_t, lam, rec, src_cells, D, eps, maxit, want_gradient=False)  # lines 7-8
         total += int(tri["iters"].sum())
+        if reduce is not None:
+            tri["f"] = reduce(tri["f"], None)
         trace.append((eps, cur["f"], tri["f"]))
-        if not (tri["f"] > cur["f"]):                                              # line 9 / 12-13
+        if np.isfinite(tri["f"]) and tri["f"] <= cur["f"]:                         # line 9 / 12-13
             return dict(accepted=True, m=m_t, eps=eps, n_halvings=h, f=cur["f"], f_trial=tri["f"],
                         g=cur["g"], lsqr_iters=total, trace=trace)
         if h == max_halvings:

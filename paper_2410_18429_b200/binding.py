@@ -40,11 +40,18 @@ class wri_lsqr_view(C.Structure):
 
 WRI_AWRI_MAX_TRACE = 16
 wri_update_fn = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p)
+wri_reduce_fn = C.CFUNCTYPE(C.c_int, C.c_void_p, C.POINTER(C.c_double), C.c_void_p, C.c_int64, C.c_void_p)
 
 
 class wri_awri_opts(C.Structure):
     _fields_ = [("max_halvings", C.c_int32), ("warm_restart", C.c_int32), ("update", wri_update_fn),
-                ("user", C.c_void_p), ("step", C.c_float), ("m_min", C.c_float), ("m_max", C.c_float)]
+                ("user", C.c_void_p), ("step", C.c_float), ("m_min", C.c_float), ("m_max", C.c_float),
+                ("reduce", wri_reduce_fn)]
+
+
+class wri_debug_opts(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in ("nstage_f", "nstage_a", "zc_f", "zc_a", "txc", "tyc",
+                                         "no_compact", "no_groups", "generic", "no_graph")]
 
 
 class wri_awri_report(C.Structure):
@@ -61,6 +68,9 @@ WRI_ERR_RECEIVER_DUP = -3
 WRI_ERR_WORKSPACE = -4
 WRI_ERR_CUDA = -5
 WRI_ERR_STATE = -6
+WRI_ERR_NUMERIC = -7
+WRI_STENCIL_7 = 0
+WRI_STENCIL_27 = 1
 WRI_WS_HOST_STAGING = 1
 WRI_WS_COMPACTION = 2
 
@@ -68,8 +78,7 @@ _lib = None
 
 
 def lib_path() -> str:
-    # WRI_LIB: developer override to load a tuning variant built with build.build(out=...)
-    return os.environ.get("WRI_LIB") or os.path.join(_HERE, "libwri.so")
+    return os.path.join(_HERE, "libwri.so")
 
 
 def load_library():
@@ -78,7 +87,7 @@ def load_library():
     if _lib is not None:
         return _lib
     path = lib_path()
-    if not os.path.exists(path) and not os.environ.get("WRI_LIB"):
+    if not os.path.exists(path):
         # the in-tree library is missing (fresh checkout): build it with nvcc, loudly; never a CPU fallback
         import sys
         sys.stderr.write("paper_2410_18429_b200: libwri.so missing, building it with nvcc for sm_100a ...\n")
@@ -95,6 +104,9 @@ def load_library():
     P, I32, F32, F64 = C.c_void_p, C.c_int32, C.c_float, C.c_double
     lib.wri_create.argtypes = [C.POINTER(P), wri_grid, F64, I32, P, P, wri_sponge, I32, P, I32, P]
     lib.wri_set_model.argtypes = [P, P]
+    lib.wri_set_stencil.argtypes = [P, I32]
+    lib.wri_set_debug_opts.argtypes = [P, C.POINTER(wri_debug_opts)]
+    lib.wri_plan_info.argtypes = [P, I32, P]
     lib.wri_workspace_bytes.argtypes = [P, I32, I32]
     lib.wri_workspace_bytes.restype = C.c_size_t
     lib.wri_set_workspace.argtypes = [P, P, C.c_size_t]
@@ -222,20 +234,46 @@ class Wri:
         self.m = m
         _ck(self._lib.wri_set_model(self._h, _dptr(m)))
 
+    def set_stencil(self, stencil):
+        """WRI_STENCIL_7 (default) or WRI_STENCIL_27; sticky."""
+        _ck(self._lib.wri_set_stencil(self._h, int(stencil)))
+
+    def plan_info(self, nb):
+        """Tile plan of the pass kernel for batch width nb (wri_plan_info), or None (generic kernels)."""
+        out = (C.c_int32 * 16)()
+        if self._lib.wri_plan_info(self._h, int(nb), out) != WRI_OK:
+            return None
+        keys = ("cb", "nchunk", "txc", "tyc", "items", "merged", "m_tma", "zc_f", "nstage_f", "tiles_f",
+                "zc_a", "nstage_a", "tiles_a", "stage_bytes_f", "stage_bytes_a", "grid")
+        return dict(zip(keys, (int(v) for v in out)))
+
+    def set_debug_opts(self, **kw):
+        """Tuning / test switches (wri_debug_opts); no arguments restores the defaults."""
+        o = wri_debug_opts()
+        for k, v in kw.items():
+            if not hasattr(o, k):
+                raise TypeError("unknown debug option %r" % (k,))
+            setattr(o, k, int(v))
+        _ck(self._lib.wri_set_debug_opts(self._h, C.byref(o)))
+
     # ---- operator
-    def apply_M(self, x, lam, omega_idx=None):
+    def apply_M(self, x, lam, omega_idx=None, out=None):
+        """out = (ytop, ybot) to reuse buffers."""
         t = self._torch
         nb = x.shape[1]
-        ytop = t.empty_like(x)
-        ybot = t.empty((self.n_rec, nb), dtype=t.complex64, device=x.device)
+        if out is not None:
+            ytop, ybot = out
+        else:
+            ytop = t.empty_like(x)
+            ybot = t.empty((self.n_rec, nb), dtype=t.complex64, device=x.device)
         keep, oi = _i32(omega_idx)
         _ck(self._lib.wri_apply_M(self._h, nb, oi, float(lam), _dptr(x), _dptr(ytop), _dptr(ybot)))
         return ytop, ybot
 
-    def apply_MH(self, ytop, ybot, lam, omega_idx=None):
+    def apply_MH(self, ytop, ybot, lam, omega_idx=None, out=None):
         t = self._torch
         nb = ytop.shape[1]
-        x = t.empty_like(ytop)
+        x = out if out is not None else t.empty_like(ytop)
         keep, oi = _i32(omega_idx)
         _ck(self._lib.wri_apply_MH(self._h, nb, oi, float(lam), _dptr(ytop), _dptr(ybot), _dptr(x)))
         return x
@@ -456,10 +494,12 @@ class Wri:
         return dict(u=u, alpha=a, ar0=ar0, f_pde=fp, f_data=fd, iters=it, f=f.value if want_f else None)
 
     def awri_step(self, m, d, lam, src_ijk, eps, maxit, omega_idx=None, max_halvings=8, warm_restart=False,
-                  update=None, step=0.0, m_min=0.0, m_max=float("inf")):
+                  update=None, step=0.0, m_min=0.0, m_max=float("inf"), reduce=None):
         """Lines 4-14 of Algorithm 2 (wri_awri_step) on the model tensor m (float32 [n_g], updated in
         place when the step is accepted).  update(m, g, m_trial): enqueue m_trial on the current
-        stream (torch ops on the three tensors); None = built-in clamp(m - step g, m_min, m_max)."""
+        stream (torch ops on the three tensors); None = built-in clamp(m - step g, m_min, m_max).
+        reduce(f, g) -> f_sum: sum over ranks of the objective (a float) and, when g is not None,
+        in-place all-reduce of the gradient tensor (column sharding); None = single process."""
         t = self._torch
         nb = d.shape[1]
         self.ensure_workspace(nb, compaction=True)
@@ -479,9 +519,18 @@ class Wri:
                 err.append(e)
                 return 1
 
+        def _red(user, f_ptr, g_ptr, n_g, stream):
+            try:
+                f_ptr[0] = float(reduce(float(f_ptr[0]), g if g_ptr else None))
+                return 0
+            except Exception as e:
+                err.append(e)
+                return 1
+
         cb = wri_update_fn(_cb) if update is not None else wri_update_fn()
+        rb = wri_reduce_fn(_red) if reduce is not None else wri_reduce_fn()
         o = wri_awri_opts(int(max_halvings), int(bool(warm_restart)), cb, None, float(step), float(m_min),
-                          float(m_max))
+                          float(m_max), rb)
         rep = wri_awri_report()
         keep, oi = _i32(omega_idx)
         keep2, si = _i32(src_ijk)

@@ -14,13 +14,13 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libwri.so")
 SOURCES = [os.path.join(CSRC, "wri_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "wri_kernels.cuh"), os.path.join(CSRC, "wri_tma.cuh"),
+DEPS = SOURCES + [os.path.join(CSRC, "wri_kernels.cuh"), os.path.join(CSRC, "wri_pass.cuh"),
                   os.path.join(os.path.dirname(_HERE), "include", "wri.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "--use_fast_math", "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]
-# --use_fast_math only affects division/transcendentals/denormals; the kernels use neither
-# divisions nor transcendentals on the data path (FMA contraction is on by default).
+              "-fmad=true", "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]
+# IEEE fp32 arithmetic with FMA contraction: no --use_fast_math (denormals are kept, divisions are
+# exact); the data path has neither divisions nor transcendentals, so nothing is lost.
 
 
 def nvcc() -> str:
@@ -37,17 +37,7 @@ def needs_build() -> bool:
     return any(os.path.getmtime(d) > t for d in DEPS)
 
 
-def build(force: bool = False, verbose: bool = False, extra=(), out: str = None) -> str:
-    """extra/out: developer knobs for tuning variants (e.g. extra=["-DWRI_NT=512"], out="libwri_nt512.so")."""
-    if out:
-        dst = os.path.join(_HERE, out)
-        cmd = [nvcc()] + NVCC_FLAGS + list(extra) + ["-o", dst] + SOURCES
-        res = subprocess.run(cmd, capture_output=True, text=True)
-        if verbose or res.returncode != 0:
-            sys.stderr.write(res.stdout + res.stderr)
-        if res.returncode != 0:
-            raise RuntimeError("nvcc failed: " + " ".join(cmd))
-        return dst
+def build(force: bool = False, verbose: bool = False) -> str:
     if force or needs_build():
         tmp = LIB + ".%d.tmp" % os.getpid()
         cmd = [nvcc()] + NVCC_FLAGS + ["-o", tmp] + SOURCES

@@ -1,8 +1,9 @@
 // wri_api.cu — C ABI of libwri (include/wri.h): context, validation, launch sequencing.
-// All arithmetic of the path runs in the kernels of wri_kernels.cuh; there is no CPU fallback.
+// All arithmetic of the path runs in the kernels of wri_kernels.cuh / wri_pass.cuh; there is no
+// CPU fallback.
 #include "../../include/wri.h"
 #include "wri_kernels.cuh"
-#include "wri_tma.cuh"
+#include "wri_pass.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -31,10 +32,12 @@ int cuda_fail(cudaError_t e, const char* what) {
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+inline int even_up(int n) { return (n + 1) & ~1; }
 
 inline unsigned blocks_for(long long n) { return (unsigned)std::min<long long>((n + 255) / 256, 148 * 16); }
 constexpr int kMaxCtas = 512;          // upper bound on the persistent grid (>= SM count)
-constexpr int kMinChunk = 2;           // narrowest column chunk of the TMA path
+constexpr int kInitRowBlocks = 64;     // blocks of k_init_rows (extra rows of the generic partials)
+constexpr int kChk = 4;                // the compaction kernel is enqueued every kChk iterations
 
 struct Tiling {
     int vec;            // complex numbers per thread (2 = 128-bit accesses)
@@ -54,31 +57,23 @@ struct wri_ctx {
     int n_rec = 0, nb_max = 0;
     cudaStream_t stream = nullptr;
     const float* m = nullptr;
+    int stencil = WRI_STENCIL_7;
+    wri_debug_opts dbg{};
     // library-owned device memory
     float* gtab = nullptr;       // gx | gy | gz
     int* rec = nullptr;          // [n_rec] cell indices
     std::vector<int> rec_ijk;    // host copy [n_rec][3]
-    int* own_ptr = nullptr;      // [kMaxCtas + 1] pass A: CSR of the receivers inside each CTA's tiles
-    int4* own = nullptr;         // [n_rec * max chunks] {receiver, cell, tile, group size}
-    std::vector<int> h_own_ptr;
-    std::vector<int4> h_own;
-    float* coef = nullptr;       // [N_COEF][nb_max]   current bank of the per-column scalars
-    double* stat = nullptr;      // [N_STAT][nb_max]
-    int* active = nullptr;       // [nb_max]
-    int* iters = nullptr;        // [nb_max]
-    float* coef_alt = nullptr;   // second bank: column compaction gathers into it and swaps
-    double* stat_alt = nullptr;
-    int* active_alt = nullptr;
-    int* iters_alt = nullptr;
+    float* coef[2] = {nullptr, nullptr};     // [N_COEF][nb_max] per-column scalars, one bank per parity
+    double* stat[2] = {nullptr, nullptr};    // [N_STAT][nb_max]
+    int* active[2] = {nullptr, nullptr};     // [nb_max]
+    int* iters[2] = {nullptr, nullptr};      // [nb_max]
     int* src = nullptr;          // [nb_max] source cell per caller's column (source-free system)
     bool sf = false;             // the solve in flight has the extra source-weight unknown
     float2* alpha_out = nullptr; // caller's [nb] source-weight estimates (source-free system)
     wri_lsqr_opts opts{};        // warm start / stop-rule reference for the next solves (wri_lsqr_set_opts)
     const unsigned char* rmask = nullptr;   // per-source receiver sets [n_rec][rmask_nb] (wri_set_receiver_mask)
     int rmask_nb = 0;
-    int* colmap = nullptr;       // [nb_max] working column -> caller's column (-1 = padding)
-    int* idx = nullptr;          // [3][nb_max] scratch: gather map | retire source | retire destination
-    int* h_active = nullptr;     // pinned host copy of the active flags
+    int* colmap = nullptr;       // [nb_max] gather map of a grouped solve's start (caller's column per working column)
     // misfit evaluation / Algorithm 2 step (wri_misfit_sf, wri_awri_step)
     float* aw_tol = nullptr;     // [nb_max] the uniform tolerance eps of a misfit evaluation
     double* aw_f = nullptr;      // [2][nb_max] f_pde | f_data of the trial evaluation
@@ -90,40 +85,56 @@ struct wri_ctx {
     size_t ws_bytes = 0;
     // solve in flight
     bool solving = false;
-    int nb = 0, k = 0, maxit = 0;   // nb = WORKING width (shrinks when converged columns are compacted away)
+    int nb = 0, k = 0, maxit = 0;   // nb = working width at the START of the solve (the device state holds the
+                                    // current one); k = iterations ENQUEUED
     int nb0 = 0;                    // caller's batch width
-    bool packed = false;            // X lives in the workspace (after the first compaction); else X = u_out
-    bool can_compact = false, all_done = false;
-    int check_every = 0;            // iterations between host looks at the active flags (0 = never)
-    std::vector<int> h_colmap;      // host copy of colmap
-    std::vector<char> retired;      // per caller's column: x and history are final in the caller's buffers
-    std::vector<float2*> free_slots;   // workspace vector slots not holding a live vector
-    float2 *U_bot_alt = nullptr, *u_out = nullptr;
+    bool packed = false;            // the working set has a column map; X lives in the workspace
+    bool adaptive = false;          // converged columns are compacted away on the device
+    float2* u_out = nullptr;
     float lambda = 0;
-    float2 *U = nullptr, *V = nullptr, *W = nullptr, *X = nullptr, *U_bot = nullptr;
-    double* partials = nullptr;
+    float2* vec[2][4] = {};         // per parity: U, V, W, X
+    float2* U_bot[2] = {nullptr, nullptr};
+    float2 *U = nullptr, *V = nullptr, *W = nullptr, *X = nullptr;   // parity 0 (the start works on these)
+    double* partials = nullptr;     // generic kernels: [n_tiles + kInitRowBlocks][nb]
     const float* tol = nullptr;
     float* resnorms = nullptr;
     int* iters_out = nullptr;
     Tiling tl{};
     int64_t launches = 0;
-    // persistent TMA pass kernel (nb % 16 == 0): column chunk width, tiling, tensor maps
+    // persistent pass kernel: per-width plans, tensor maps and receiver lists (device tables)
     int num_sms = 0;
-    unsigned int* counter = nullptr;      // last-CTA ticket (device)
-    int tma_cb = 0;                       // 0 = not used for this solve
-    struct TmaPlan {                      // one per pass (tile shapes may differ between F and A)
-        int txc = 0, tyc = 0, ntx = 0, nty = 0, ntz = 0, zc = 0, nchunk = 0, tiles = 0, grid = 0;
-        CUtensorMap in{}, old{}, w{}, x{}, m{};
-        int m_tma = 0;                    // model tile rides in the TMA stage
-        int merged = 0;                   // tensor maps fold (column, x)
-    } planF, planA, planG;
-    double* partials_tma = nullptr;       // [grid][nb]
-    bool wx_zero = false;                 // W, X not cleared: the first pass F must not read them
+    unsigned int* counter = nullptr;      // last-CTA ticket of the pass kernels (device)
+    unsigned int* counter2 = nullptr;     // ... of the compaction kernel
+    bool rt = false;                      // this solve runs on the persistent pass kernel
+    int n_widths = 0;                     // plans of the solve: widths nb, nb-2, ..., (adaptive) or just nb
+    int cap_widths = 0, cap_own = 0;
+    std::vector<DevPlan> h_plans;
+    DevPlan* d_plans = nullptr;
+    CUtensorMap* d_maps = nullptr;        // [cap_widths][2][N_MAPS]
+    CUtensorMap* d_mmaps = nullptr;       // [cap_widths]
+    int* d_own_ptr = nullptr;             // [cap_widths][kMaxCtas + 1]
+    int4* d_own = nullptr;                // [cap_widths][cap_own]
+    SolveState* d_state = nullptr;
+    long long* d_prof = nullptr;          // device counters: widths / launches of the passes that did work (F | A)
+    long long prof_host[4] = {0, 0, 0, 0};   // same for the host-sequenced generic path
+    size_t smem_f = 0, smem_a = 0;        // dynamic shared memory of the solve's launches (max over its plans)
+    double* partials_rt = nullptr;        // [grid][nb]
+    bool lazy = false;                    // W, X not cleared: the first pass F must not read them
+    // plan cache: the tables above are rebuilt only when one of these changes
+    struct PlanKey {
+        int nb = 0, adaptive = 0, stencil = 0;
+        const void* v[2][4] = {};
+        const float* m = nullptr;
+        wri_debug_opts dbg{};
+    } plan_key;
+    bool plan_valid = false;
+    // device-side loop (CUDA graph with a conditional WHILE node), rebuilt per solve
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t graph_exec = nullptr;
     // optional per-kernel timing (wri_profile_*)
     bool profiling = false;
     std::vector<cudaEvent_t> ev_pool;     // pairs: start, stop
     std::vector<int> ev_kind;             // per pair: 0 = pass F, 1 = pass A
-    std::vector<int> ev_cols;             // per pair: working batch width of that launch
     size_t ev_used = 0;                   // pairs in use
     std::vector<std::pair<const void*, size_t>> smem_ok;   // kernels already granted their dynamic smem size
     // pipelined host-buffer solves (wri_set_host_pipeline): two staging slots, copy streams, events
@@ -139,7 +150,8 @@ struct wri_ctx {
 
 namespace {
 
-// Tile shape for batch width nb: threads span the (ix, s) row first, then y; blocks march zc planes.
+// Tile shape of the generic kernels for batch width nb: threads span the (ix, s) row first, then y;
+// blocks march zc planes.
 Tiling make_tiling(const wri_ctx* c, int nb) {
     Tiling t;
     t.vec = (nb % 2 == 0) ? 2 : 1;
@@ -189,35 +201,40 @@ GradTiling make_grad_tiling(const wri_ctx* c, int nb) {
     return G;
 }
 
+// Caller's workspace.  Vector regions hold n_g x even(nb) complex64 each: U, V, W always; with
+// WS_COMPACTION five more (the working set of an adaptive solve keeps X in the workspace and has a
+// second vector set to re-pack into), with WS_HOST_STAGING the device copy of x for the host entry.
 struct WsLayout {
-    size_t U, V, W, U_bot, partials, partials_tma, gscratch, Xs, Ds, tols, res, its, alphas, B3, B4, U_bot2, total;
+    size_t vecs[8], U_bot, partials, partials_rt, gscratch, Xs, Ds, tols, res, its, alphas, U_bot2, total;
+    int n_vecs;
 };
 enum { WS_HOST_STAGING = 1, WS_COMPACTION = 2 };
 WsLayout ws_layout(const wri_ctx* c, int nb, int flags, int maxit_cap) {
     WsLayout L{};
-    const size_t vec = align_up(c->ng * (size_t)nb * sizeof(float2), 256);
-    const size_t bot = align_up((size_t)std::max(c->n_rec, 1) * nb * sizeof(float2), 256);
+    const int nbe = even_up(nb);
+    const size_t vec = align_up(c->ng * (size_t)nbe * sizeof(float2), 256);
+    const size_t bot = align_up((size_t)std::max(c->n_rec, 1) * nbe * sizeof(float2), 256);
     const Tiling t = make_tiling(c, nb);
     size_t o = 0;
-    L.U = o; o += vec;
-    L.V = o; o += vec;
-    L.W = o; o += vec;
+    L.n_vecs = 3;
+    for (int i = 0; i < 3; ++i) { L.vecs[i] = o; o += vec; }
     L.U_bot = o; o += bot;
     const GradTiling gt = make_grad_tiling(c, nb);
-    L.partials = o; o += align_up(std::max(t.n_tiles, gt.ok ? gt.t.n_tiles : 0) * nb * sizeof(double), 256);
-    L.partials_tma = o; o += align_up((size_t)kMaxCtas * nb * sizeof(double), 256);
-    L.gscratch = o; o += align_up(c->ng * sizeof(float), 256);       // one batch's gradient (TMA path)
+    L.partials = o;
+    o += align_up((std::max(t.n_tiles, gt.ok ? gt.t.n_tiles : 0) + kInitRowBlocks) * nbe * sizeof(double), 256);
+    L.partials_rt = o; o += align_up((size_t)kMaxCtas * nbe * sizeof(double), 256);
+    L.gscratch = o; o += align_up(c->ng * sizeof(float), 256);       // one batch's gradient (pass kernel)
     if (flags & WS_HOST_STAGING) {
         L.Xs = o; o += vec;
         L.Ds = o; o += bot;
-        L.tols = o; o += align_up((size_t)nb * sizeof(float), 256);
-        L.res = o; o += align_up((size_t)(maxit_cap + 1) * nb * sizeof(float), 256);
-        L.its = o; o += align_up((size_t)nb * sizeof(int), 256);
-        L.alphas = o; o += align_up((size_t)nb * sizeof(float2), 256);
+        L.tols = o; o += align_up((size_t)nbe * sizeof(float), 256);
+        L.res = o; o += align_up((size_t)(maxit_cap + 1) * nbe * sizeof(float), 256);
+        L.its = o; o += align_up((size_t)nbe * sizeof(int), 256);
+        L.alphas = o; o += align_up((size_t)nbe * sizeof(float2), 256);
     }
     if (flags & WS_COMPACTION) {
-        L.B3 = o; o += vec;
-        L.B4 = o; o += vec;
+        for (int i = 3; i < 8; ++i) { L.vecs[i] = o; o += vec; }
+        L.n_vecs = 8;
         L.U_bot2 = o; o += bot;
     }
     L.total = o;
@@ -225,19 +242,22 @@ WsLayout ws_layout(const wri_ctx* c, int nb, int flags, int maxit_cap) {
 }
 constexpr int kHostMaxitCap = 4096;   // resnorm staging rows reserved for wri_lsqr_batch_host
 
-int upload_columns(wri_ctx* c, int nb, const int32_t* omega_idx, float lambda) {
+int upload_columns(wri_ctx* c, int nb, const int32_t* omega_idx, float lambda, int n_real = -1) {
+    // columns >= n_real are padding of an even-width working set (frequency 0, never active)
+    if (n_real < 0) n_real = nb;
     std::vector<float> w2(nb), one(nb, 1.f), lam(nb, lambda), nlam(nb, -lambda), mone(nb, -1.f);
     for (int s = 0; s < nb; ++s) {
-        const int j = omega_idx ? omega_idx[s] : 0;
+        const int j = (omega_idx && s < n_real) ? omega_idx[s] : 0;
         if (j < 0 || j >= (int)c->omega.size()) return WRI_ERR_ARG;
         w2[s] = (float)(c->omega[j] * c->omega[j]);
     }
     const size_t NM = c->nb_max;
-    CK(cudaMemcpyAsync(c->coef + C_W2 * NM, w2.data(), nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));
-    CK(cudaMemcpyAsync(c->coef + C_ONE * NM, one.data(), nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));
-    CK(cudaMemcpyAsync(c->coef + C_LAM * NM, lam.data(), nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));
-    CK(cudaMemcpyAsync(c->coef + C_NLAM * NM, nlam.data(), nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));
-    CK(cudaMemcpyAsync(c->coef + C_MONE * NM, mone.data(), nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    float* cf = c->coef[0];
+    CK(cudaMemcpyAsync(cf + C_W2 * NM, w2.data(), nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(cf + C_ONE * NM, one.data(), nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(cf + C_LAM * NM, lam.data(), nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(cf + C_NLAM * NM, nlam.data(), nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(cf + C_MONE * NM, mone.data(), nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));
     return WRI_OK;
 }
 
@@ -254,40 +274,61 @@ int upload_sources(wri_ctx* c, int nb, const int32_t* src_ijk) {
     return WRI_OK;
 }
 
+// Stencil of the discretised Laplacian (reading C-3 / C-23): weights of the centre, the 6 face, the 12
+// edge and the 8 corner neighbours, in units of 1/h^2.
+struct StencilW { double a0, a1, a2, a3; };
+StencilW stencil_weights(int kind) {
+    if (kind == WRI_STENCIL_27) return {-128.0 / 30.0, 14.0 / 30.0, 3.0 / 30.0, 1.0 / 30.0};
+    return {-6.0, 1.0, 0.0, 0.0};
+}
+
 PassParams base_params(const wri_ctx* c, int nb, const Tiling& t) {
     PassParams p{};
     p.m = c->m;
     p.gx = c->gtab;
     p.gy = c->gtab + c->g.nx;
     p.gz = c->gtab + c->g.nx + c->g.ny;
-    p.w2 = c->coef + C_W2 * (size_t)c->nb_max;
+    p.w2 = c->coef[0] + C_W2 * (size_t)c->nb_max;
     p.nx = c->g.nx; p.ny = c->g.ny; p.nz = c->g.nz; p.nb = nb;
     p.zc = t.zc;
+    const StencilW w = stencil_weights(c->stencil);
     p.ih2 = (float)(1.0 / (c->h * c->h));
-    p.m6ih2 = (float)(-6.0 / (c->h * c->h));
+    p.m6ih2 = (float)(w.a0 / (c->h * c->h));
+    p.a1 = (float)w.a1; p.a2 = (float)w.a2; p.a3 = (float)w.a3;
     p.sgn = 1.f;
     return p;
+}
+
+int profile_event_begin(wri_ctx* c, int kind, cudaEvent_t* e1) {
+    *e1 = nullptr;
+    if (!c->profiling) return WRI_OK;
+    if (c->ev_used * 2 == c->ev_pool.size()) {
+        cudaEvent_t a, b;
+        CK(cudaEventCreate(&a));
+        CK(cudaEventCreate(&b));
+        c->ev_pool.push_back(a); c->ev_pool.push_back(b); c->ev_kind.push_back(0);
+    }
+    cudaEvent_t e0 = c->ev_pool[2 * c->ev_used];
+    *e1 = c->ev_pool[2 * c->ev_used + 1];
+    c->ev_kind[c->ev_used] = kind;
+    c->ev_used++;
+    CK(cudaEventRecord(e0, c->stream));
+    return WRI_OK;
 }
 
 template <int MODE>
 int launch_pass(wri_ctx* c, const PassParams& p, const Tiling& t, bool timed = false) {
     const size_t smem = (MODE == MODE_APPLY) ? 0 : (size_t)t.block.x * t.block.y * t.vec * sizeof(double);
-    cudaEvent_t e0 = nullptr, e1 = nullptr;
-    if (timed && c->profiling) {
-        if (c->ev_used * 2 == c->ev_pool.size()) {
-            cudaEvent_t a, b;
-            CK(cudaEventCreate(&a));
-            CK(cudaEventCreate(&b));
-            c->ev_pool.push_back(a); c->ev_pool.push_back(b); c->ev_kind.push_back(0); c->ev_cols.push_back(0);
-        }
-        e0 = c->ev_pool[2 * c->ev_used]; e1 = c->ev_pool[2 * c->ev_used + 1];
-        c->ev_kind[c->ev_used] = (MODE == MODE_F) ? 0 : 1;
-        c->ev_cols[c->ev_used] = c->nb;
-        c->ev_used++;
-        CK(cudaEventRecord(e0, c->stream));
+    cudaEvent_t e1 = nullptr;
+    if (timed) { int rc = profile_event_begin(c, MODE == MODE_F ? 0 : 1, &e1); if (rc) return rc; }
+    const bool s27 = c->stencil == WRI_STENCIL_27;
+    if (t.vec == 2) {
+        if (s27) k_pass<2, MODE, ST_27><<<t.grid, t.block, smem, c->stream>>>(p);
+        else     k_pass<2, MODE, ST_7><<<t.grid, t.block, smem, c->stream>>>(p);
+    } else {
+        if (s27) k_pass<1, MODE, ST_27><<<t.grid, t.block, smem, c->stream>>>(p);
+        else     k_pass<1, MODE, ST_7><<<t.grid, t.block, smem, c->stream>>>(p);
     }
-    if (t.vec == 2) k_pass<2, MODE><<<t.grid, t.block, smem, c->stream>>>(p);
-    else            k_pass<1, MODE><<<t.grid, t.block, smem, c->stream>>>(p);
     c->launches++;
     CK(cudaGetLastError());
     if (e1) CK(cudaEventRecord(e1, c->stream));
@@ -297,9 +338,10 @@ int launch_pass(wri_ctx* c, const PassParams& p, const Tiling& t, bool timed = f
 ScalParams scal_params(const wri_ctx* c, const double* partials, int n_rows, const float2* d);
 
 template <int PHASE>
-int launch_scalars(wri_ctx* c, const float2* d) {
-    ScalParams s = scal_params(c, c->partials, (int)c->tl.n_tiles, d);
-    s.rows_in_pass = c->tma_cb ? 1 : 0;
+int launch_scalars(wri_ctx* c, const float2* d, int extra_rows = 0) {
+    ScalParams s = scal_params(c, c->partials, (int)c->tl.n_tiles + extra_rows, d);
+    s.rows_in_pass = c->rt ? 1 : 0;
+    s.init_rows = extra_rows > 0;
     const int T = 1024;
     const size_t smem = (size_t)(T + c->nb) * sizeof(double);
     k_scalars<PHASE><<<1, T, smem, c->stream>>>(s);
@@ -308,8 +350,7 @@ int launch_scalars(wri_ctx* c, const float2* d) {
     return WRI_OK;
 }
 
-
-// ---- TMA path -------------------------------------------------------------------------------
+// ---- persistent pass kernel: plans, tensor maps, launches ------------------------------------------
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
                                   CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
@@ -332,9 +373,9 @@ EncodeTiledFn get_encode_fn() {
 // 4-D view (column, x, y, z) of a source-interleaved complex64 vector; one element = 8 bytes.
 // Out-of-range box elements are zero-filled (the Dirichlet closure of the stencil).
 // merged (nb == cb only): (column, x) folded into one dimension of nb*nx contiguous elements, so a box
-// row is cb*bx elements (<= 256) — narrow chunks would otherwise move 32-128 byte rows
-int make_tmap(CUtensorMap* tm, const void* base, const wri_ctx* c, int nb, int cb, int bx, int by,
-              bool merged = false) {
+// row is cb*bx elements (<= 256) — narrow chunks would otherwise move 16-128 byte rows.
+// 128-byte L2 promotion: measured 0.7 % faster than 256 B at 128^3 x 64.
+int make_tmap(CUtensorMap* tm, const void* base, const wri_ctx* c, int nb, int cb, int bx, int by, bool merged) {
     EncodeTiledFn fn = get_encode_fn();
     if (!fn) return cuda_fail(cudaErrorNotSupported, "cuTensorMapEncodeTiled lookup");
     cuuint64_t gdim[4] = {(cuuint64_t)nb, (cuuint64_t)c->g.nx, (cuuint64_t)c->g.ny, (cuuint64_t)c->g.nz};
@@ -347,116 +388,14 @@ int make_tmap(CUtensorMap* tm, const void* base, const wri_ctx* c, int nb, int c
         box[0] = (cuuint32_t)(cb * bx); box[1] = (cuuint32_t)by; box[2] = 1; box[3] = 1;
     }
     cuuint32_t estr[4] = {1, 1, 1, 1};
-    // 128-byte L2 promotion: measured 0.7 % faster than 256 B at 128^3 x 64 (whole step 0.924 against 0.918)
-    CUtensorMapL2promotion promo = CU_TENSOR_MAP_L2_PROMOTION_L2_128B;
-    if (const char* e = getenv("WRI_L2PROMO")) promo = (CUtensorMapL2promotion)atoi(e);
     CUresult r = fn(tm, CU_TENSOR_MAP_DATA_TYPE_UINT64, 4, const_cast<void*>(base), gdim, gstr, box, estr,
                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                    promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                    CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
         snprintf(g_cuda_msg, sizeof g_cuda_msg, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
         return WRI_ERR_CUDA;
     }
     return WRI_OK;
-}
-
-// Tile shapes per column-chunk width and pass.  A tile row is TXC cells = TXC*CB*8 contiguous
-// bytes; TXC*TYC*CB = 1024 complex (F: 512 consumer threads, 1 item each; A: 256 x 2 items).
-#ifndef WRI_F_TX
-#define WRI_F_TX 4
-#endif
-#ifndef WRI_F_TY
-#define WRI_F_TY 4
-#endif
-#ifndef WRI_A_TX
-#define WRI_A_TX 4
-#endif
-#ifndef WRI_A_TY
-#define WRI_A_TY 4
-#endif
-#ifndef WRI_F_NT
-#define WRI_F_NT 512
-#endif
-#ifndef WRI_A_NT
-#define WRI_A_NT 512
-#endif
-template <int CB, int MODE> struct CfgFor {
-    static constexpr int S = 64 / CB;   // narrower chunks -> proportionally more cells per tile row
-    typedef TileCfg<CB, (MODE == MODE_F ? WRI_F_TX : WRI_A_TX) * (S >= 2 ? 2 : 1),
-                    (MODE == MODE_F ? WRI_F_TY : WRI_A_TY) * (S >= 4 ? 2 : 1),
-                    (MODE == MODE_F ? WRI_F_NT : WRI_A_NT), PassTraits<MODE>::NSTAGE> type;
-};
-
-// 48 columns: 4 x 4 cells x 48 columns = 768 complex per plane, 384 consumer threads (one item each)
-#ifndef WRI_F48_NT
-#define WRI_F48_NT 384
-#endif
-#ifndef WRI_A48_NT
-#define WRI_A48_NT 384
-#endif
-#ifndef WRI_A48_STAGES
-#define WRI_A48_STAGES 8
-#endif
-template <int MODE> struct CfgFor<48, MODE> {
-    typedef TileCfg<48, 4, 4, (MODE == MODE_F ? WRI_F48_NT : WRI_A48_NT),
-                    (MODE == MODE_F ? PassTraits<MODE_F>::NSTAGE : WRI_A48_STAGES)> type;
-};
-
-// 8 / 4 columns (the tail of a shrinking batch): 16 x 8 / 16 x 16 cells, always one chunk per cell
-template <int MODE> struct CfgFor<8, MODE> {
-    typedef TileCfg<8, 16, 8, (MODE == MODE_F ? WRI_F_NT : WRI_A_NT), PassTraits<MODE>::NSTAGE> type;
-};
-template <int MODE> struct CfgFor<4, MODE> {
-    typedef TileCfg<4, 16, 16, (MODE == MODE_F ? WRI_F_NT : WRI_A_NT), PassTraits<MODE>::NSTAGE> type;
-};
-// 56 / 40 / 24 columns (widths a shrinking batch passes through): one item per consumer thread
-template <int MODE> struct CfgFor<56, MODE> {
-    typedef TileCfg<56, 4, 4, 448, (MODE == MODE_F ? PassTraits<MODE_F>::NSTAGE : WRI_A48_STAGES)> type;
-};
-template <int MODE> struct CfgFor<40, MODE> {
-    typedef TileCfg<40, 4, 4, 320, (MODE == MODE_F ? PassTraits<MODE_F>::NSTAGE : WRI_A48_STAGES)> type;
-};
-template <int MODE> struct CfgFor<24, MODE> {
-    typedef TileCfg<24, 8, 4, 384, (MODE == MODE_F ? PassTraits<MODE_F>::NSTAGE : WRI_A48_STAGES)> type;
-};
-// 2 columns (one 16-byte item per cell): 32 x 16 cells
-template <int MODE> struct CfgFor<2, MODE> {
-    typedef TileCfg<2, 32, 16, (MODE == MODE_F ? WRI_F_NT : WRI_A_NT), PassTraits<MODE>::NSTAGE> type;
-};
-
-int tma_chunk_for(int nb) {
-    const char* off = getenv("WRI_NO_TMA");
-    if (off && off[0] == '1') return 0;
-    if (nb % 64 == 0) return 64;
-    if (nb == 56 || nb == 40 || nb == 24) return nb;
-    if (nb % 48 == 0) return 48;
-    if (nb % 32 == 0) return 32;
-    if (nb % 16 == 0) return 16;
-    if (nb == 8 || nb == 4 || nb == 2) return nb;
-    return 0;
-}
-
-// opt-in to > 48 KB of dynamic shared memory, once per (context, kernel, size): the attribute is per
-// device, so it is not cached in a process-wide static
-int allow_smem(wri_ctx* c, const void* fn, size_t bytes) {
-    for (auto& e : c->smem_ok)
-        if (e.first == fn) {
-            if (e.second >= bytes) return WRI_OK;
-            CK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
-            e.second = bytes;
-            return WRI_OK;
-        }
-    CK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
-    c->smem_ok.emplace_back(fn, bytes);
-    return WRI_OK;
-}
-
-template <class Cfg, int MODE>
-size_t tma_smem_bytes(const wri_ctx* c) {
-    return (size_t)Cfg::NSTAGE *
-               (Cfg::IN_SPAN + PassTraits<MODE>::NSTREAM * Cfg::CTR_BYTES + Cfg::M_BYTES) +
-           2 * Cfg::NSTAGE * 8 + (size_t)c->nb * 8 + (size_t)Cfg::NT * 2 * 8 +
-           (size_t)(c->g.nx + c->g.ny + c->g.nz) * 4 + (size_t)6 * c->nb * 4;
 }
 
 // 3-D view (x, y, z) of the float32 model; needs a 16-byte row pitch
@@ -477,111 +416,227 @@ int make_tmap_model(CUtensorMap* tm, const wri_ctx* c, int bx, int by) {
     return WRI_OK;
 }
 
-// tiling + tensor maps of one pass for the solve that is starting
-template <class Cfg>
-int tma_plan(wri_ctx* c, wri_ctx::TmaPlan& P, const void* in, const void* old, bool is_f,
-             bool rec_lists = true) {
-    P.txc = Cfg::TXC; P.tyc = Cfg::TYC;
-    P.nchunk = c->nb / Cfg::CB;
-    P.ntx = (c->g.nx + P.txc - 1) / P.txc;
-    P.nty = (c->g.ny + P.tyc - 1) / P.tyc;
-    const long long per_plane = (long long)P.nchunk * P.ntx * P.nty;
-    // planes per tile: 32, except pass F with one 64-column chunk per cell: 16 — measured
-    // (profiles/r01_v6_stages.md): shorter tiles shorten the time between the waves of tiles, so more of
-    // the halo shared across a wave boundary is still in L2, at the price of two more halo planes per
-    // tile; at 128^3 x 64 pass F gains (0.929 -> 0.947), pass A loses (0.938 -> 0.907), and at 32 or 48
-    // columns (256^3, 200x200x160) F does not gain either.  WRI_ZC / WRI_ZC_F / WRI_ZC_A override.
-    // (pass F at 32 columns: 128 planes, 0.945 -> 0.957 at 256^3 x 32)
-    int zc = std::min(c->g.nz, (is_f && Cfg::CB == 64 && P.nchunk == 1) ? 16 : (is_f && Cfg::CB == 32) ? 128 : 32);
-    const char* zenv = getenv(is_f ? "WRI_ZC_F" : "WRI_ZC_A");
-    if (!zenv) zenv = getenv("WRI_ZC");
-    if (zenv && atoi(zenv) > 0) zc = std::min(c->g.nz, atoi(zenv));
+// Column chunk of the pass kernel for batch width nb: the whole width up to 64 columns (one chunk per
+// cell), else the largest even divisor <= 64.  0 = the width is served by the generic kernels.
+int rt_chunk_for(const wri_ctx* c, int nb) {
+    if (c->dbg.generic || nb % 2 || !get_encode_fn()) return 0;
+    if (nb <= RT_MAXW) return nb;
+    for (int cb = RT_MAXW; cb >= 8; cb -= 2)
+        if (nb % cb == 0) return cb;
+    return 0;
+}
+
+// planes per tile and tile count of one pass.  With plenty of tiles the measured preferences hold
+// (profiles/r01_v6_stages.md: pass F 16 planes at one 64-column chunk per cell, 128 at 32 columns, else
+// 32; pass A 32 — an L2 effect: short tiles keep the halo shared across a wave of tiles resident).  With
+// few tiles (narrow widths, small grids) the chunk count that minimises rounds x (planes + priming)
+// over the persistent grid is taken instead.
+PassGeo plan_pass(const wri_ctx* c, const DevPlan& P, bool is_f, int zc_forced) {
+    PassGeo G{};
+    const int nz = c->g.nz, sms = std::max(1, c->num_sms);
+    const long long cols = (long long)P.nchunk * P.ntx * P.nty;
+    int zc = (is_f && P.cb == 64 && P.nchunk == 1) ? 16 : (is_f && P.cb == 32) ? 128 : 32;
+    if (zc_forced > 0) zc = (zc_forced + 7) / 8 * 8;          // multiples of 8 planes (see the |.|^2 sums of the kernel)
+    else if (cols * ((nz + zc - 1) / zc) < 6LL * sms) {
+        const double prime = is_f ? 0.6 : 1.2;               // two priming planes in units of a full step
+        double best = 1e300;
+        for (int z = 8; z < nz + 8; z += 8) {
+            const long long tiles = cols * ((nz + z - 1) / z);
+            const double cost = (double)((tiles + sms - 1) / sms) * (std::min(z, nz) + prime);
+            if (cost < best * 0.999) { best = cost; zc = z; }
+        }
+    }
+    G.zc = zc;
+    G.ntz = (nz + zc - 1) / zc;
+    G.n_tiles = (int)std::min<long long>(cols * G.ntz, 0x7fffffffLL);
+    return G;
+}
+
+// Tile geometry for batch width nb (see DevPlan).  The x/y shape minimises, per z-plane of the grid,
+// the stencil input the tiles pull through L2 (halo included) plus the issue slots of the 512
+// consumer threads (idle ones included), with a penalty for tile rows below 512 contiguous bytes
+// and a small one for shapes whose model tile cannot ride in the TMA stage.
+int make_plan(const wri_ctx* c, int nb, DevPlan& P) {
+    std::memset(&P, 0, sizeof P);
+    const int cb = rt_chunk_for(c, nb);
+    if (!cb) return WRI_ERR_ARG;
+    P.nb = nb; P.cb = cb; P.hp = cb / 2; P.nchunk = nb / cb;
+    const int maxcells = RT_NT / P.hp;
+    const int nx = c->g.nx, ny = c->g.ny;
+    const bool m_al = (nx % 4 == 0) && aligned16(c->m);
+    double best = 1e300;
+    int btx = 1, bty = 1;
+    if (c->dbg.txc > 0 && c->dbg.tyc > 0 && c->dbg.txc * c->dbg.tyc <= maxcells) { btx = c->dbg.txc; bty = c->dbg.tyc; }
     else
-        while (zc > 8 && per_plane * ((c->g.nz + zc - 1) / zc) < 16LL * c->num_sms) zc = (zc + 1) / 2;
-    P.zc = zc;
-    P.ntz = (c->g.nz + zc - 1) / zc;
-    const long long tiles = per_plane * P.ntz;
-    if (tiles > 0x7fffffffLL) return WRI_ERR_ARG;
-    P.tiles = (int)tiles;
-    P.grid = (int)std::min<long long>(tiles, std::min(c->num_sms, kMaxCtas));
-    int rc;
-    const bool mg = P.nchunk == 1 && Cfg::CB * (P.txc + 2) <= 256 && !getenv("WRI_NO_MERGE");
-    P.merged = mg;
-    if ((rc = make_tmap(&P.in, in, c, c->nb, Cfg::CB, P.txc + 2, P.tyc + 2, mg))) return rc;
-    if ((rc = make_tmap(&P.old, old, c, c->nb, Cfg::CB, P.txc, P.tyc, mg))) return rc;
-    if (is_f) {
-        if ((rc = make_tmap(&P.w, c->W, c, c->nb, Cfg::CB, P.txc, P.tyc, mg))) return rc;
-        if ((rc = make_tmap(&P.x, c->X, c, c->nb, Cfg::CB, P.txc, P.tyc, mg))) return rc;
-    } else {
-        P.w = P.old; P.x = P.old;          // unused by pass A
-    }
-    if (!is_f && c->n_rec && rec_lists) {
-        // receivers (x column chunks) inside each CTA's tiles, in the order the CTA walks its
-        // tiles (same tile numbering as the kernel)
-        const int G = P.grid, nent = c->n_rec * P.nchunk;
-        struct Ent { int cta, tile, r; };
-        std::vector<Ent> ents(nent);
-        for (int e = 0; e < nent; ++e) {
-            const int r = e / P.nchunk, chunk = e % P.nchunk;
-            const int tx = c->rec_ijk[3 * r] / P.txc, ty = c->rec_ijk[3 * r + 1] / P.tyc;
-            const int tz = c->rec_ijk[3 * r + 2] / P.zc;
-            const int t = (int)((((long long)tz * P.nty + ty) * P.ntx + tx) * P.nchunk + chunk);
-            ents[e] = {t % G, t, r};
-        }
-        std::sort(ents.begin(), ents.end(), [](const Ent& a, const Ent& b) {
-            return a.cta != b.cta ? a.cta < b.cta : a.tile != b.tile ? a.tile < b.tile : a.r < b.r;
-        });
-        c->h_own_ptr.assign(G + 1, 0);
-        c->h_own.resize(nent);
-        for (int e = 0; e < nent; ++e) c->h_own_ptr[ents[e].cta + 1]++;
-        for (int b = 0; b < G; ++b) c->h_own_ptr[b + 1] += c->h_own_ptr[b];
-        for (int e = 0; e < nent;) {
-            int f = e;
-            while (f < nent && ents[f].cta == ents[e].cta && ents[f].tile == ents[e].tile) ++f;
-            for (int j = e; j < f; ++j) {
-                const int r = ents[j].r;
-                const int cell = (c->rec_ijk[3 * r + 2] * c->g.ny + c->rec_ijk[3 * r + 1]) * c->g.nx + c->rec_ijk[3 * r];
-                c->h_own[j] = make_int4(r, cell, ents[j].tile, j == e ? f - e : 0);
+        for (int tyc = 1; tyc <= std::min(maxcells, 64); ++tyc)
+            for (int txc = 1; txc * tyc <= maxcells && txc <= 254; ++txc) {
+                // three F stages (halo box + three centre boxes) must fit
+                const size_t stage = align_up((size_t)(txc + 2) * (tyc + 2) * cb * 8, 128) +
+                                     3 * align_up((size_t)txc * tyc * cb * 8, 128) + 128;
+                if (2 * stage + 24576 > (size_t)RT_SMEM_MAX) continue;
+                const double ntx = (nx + txc - 1) / txc, nty = (ny + tyc - 1) / tyc;
+                double cost = ntx * nty * ((txc + 2.0) * (tyc + 2.0) + 0.75 * maxcells);
+                const int row_bytes = txc * cb * 8;
+                if (row_bytes < 512 && txc < nx) cost *= 1.0 + 0.25 * (512 - row_bytes) / 512.0;
+                if (!(m_al && txc % 4 == 0)) cost *= 1.15;   // model tile by plain loads: measured slower
+                if (cost < best) { best = cost; btx = txc; bty = tyc; }
             }
-            e = f;
-        }
-        CK(cudaMemcpyAsync(c->own_ptr, c->h_own_ptr.data(), (G + 1) * sizeof(int), cudaMemcpyHostToDevice, c->stream));
-        CK(cudaMemcpyAsync(c->own, c->h_own.data(), nent * sizeof(int4), cudaMemcpyHostToDevice, c->stream));
-    }
-    P.m_tma = (c->g.nx % 4 == 0) && (P.txc % 4 == 0) && aligned16(c->m);
-    if (P.m_tma) { if ((rc = make_tmap_model(&P.m, c, P.txc, P.tyc))) return rc; }
-    else P.m = P.old;                       // unused placeholder
+    P.txc = btx; P.tyc = bty;
+    P.items = btx * bty * P.hp;
+    P.ntx = (nx + btx - 1) / btx;
+    P.nty = (ny + bty - 1) / bty;
+    P.merged = (P.nchunk == 1 && cb * (btx + 2) <= 256) ? 1 : 0;
+    P.m_tma = (m_al && btx % 4 == 0) ? 1 : 0;
+    P.row_b = (btx + 2) * cb * 8;
+    P.cell_b = cb * 8;
+    P.in_bytes = (btx + 2) * (bty + 2) * cb * 8;
+    P.in_span = (int)align_up(P.in_bytes, 128);
+    P.ctr_bytes = btx * bty * cb * 8;
+    P.ctr_span = (int)align_up(P.ctr_bytes, 128);
+    P.m_bytes = P.m_tma ? btx * bty * 4 : 0;
+    P.m_span = (int)align_up(P.m_bytes, 128);
+    P.f = plan_pass(c, P, true, c->dbg.zc_f);
+    P.a = plan_pass(c, P, false, c->dbg.zc_a);
+    // ring depth: near 120 KB (pass F) / 150 KB (pass A) of stages in flight per SM (measured optima,
+    // profiles/r01_v6_stages.md: a deeper ring costs L2 hits on the stencil halo, a shallower one
+    // leaves the copy engine idle), within the shared memory that is left
+    const int nxyz = c->g.nx + c->g.ny + c->g.nz;
+    auto depth = [&](int nstream, double target, int lo, int hi, int forced) {
+        const int stage = rt_stage_bytes(P, nstream);
+        int n = forced > 0 ? forced : (int)std::floor(target / stage + 0.5);
+        n = std::max(lo, std::min(n, hi));
+        while (n > 2 && rt_smem_bytes(P, nstream, n, nxyz) > (size_t)RT_SMEM_MAX) --n;
+        return n;
+    };
+    P.f.nstage = depth(3, 120e3, 2, 4, c->dbg.nstage_f);
+    P.a.nstage = depth(1, 150e3, 3, 10, c->dbg.nstage_a);
+    if (rt_smem_bytes(P, 3, P.f.nstage, nxyz) > (size_t)RT_SMEM_MAX) return WRI_ERR_ARG;
     return WRI_OK;
 }
 
-// One place that turns the run-time column-chunk width into its tile configuration: f is called with
-// std::integral_constant<int, CB> for the CB that tma_chunk_for() returned.
-template <class F>
-int dispatch_cb(int cb, F&& f) {
-    switch (cb) {
-        case 64: return f(std::integral_constant<int, 64>{});
-        case 56: return f(std::integral_constant<int, 56>{});
-        case 48: return f(std::integral_constant<int, 48>{});
-        case 40: return f(std::integral_constant<int, 40>{});
-        case 32: return f(std::integral_constant<int, 32>{});
-        case 24: return f(std::integral_constant<int, 24>{});
-        case 8:  return f(std::integral_constant<int, 8>{});
-        case 4:  return f(std::integral_constant<int, 4>{});
-        case 2:  return f(std::integral_constant<int, 2>{});
-        default: return f(std::integral_constant<int, 16>{});
+// opt-in to > 48 KB of dynamic shared memory, once per (context, kernel).  The attribute belongs to the
+// function on the device, not to the context: it is always raised to the same ceiling, so that two
+// contexts with different needs cannot lower it under one another.
+int allow_smem(wri_ctx* c, const void* fn, size_t bytes) {
+    if (bytes > (size_t)RT_SMEM_MAX) return WRI_ERR_ARG;
+    for (auto& e : c->smem_ok)
+        if (e.first == fn) return WRI_OK;
+    CK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, RT_SMEM_MAX));
+    c->smem_ok.emplace_back(fn, (size_t)RT_SMEM_MAX);
+    return WRI_OK;
+}
+
+// receivers (x column chunks) inside each CTA's tiles of pass A, in the order the CTA walks its tiles
+// (same tile numbering as the kernel): CSR over CTAs + {receiver, cell, tile, entries of this tile}
+void build_own(const wri_ctx* c, const DevPlan& P, int grid, std::vector<int>& ptr, std::vector<int4>& own) {
+    const int nent = c->n_rec * P.nchunk;
+    struct Ent { int cta, tile, r; };
+    std::vector<Ent> ents(nent);
+    for (int e = 0; e < nent; ++e) {
+        const int r = e / P.nchunk, chunk = e % P.nchunk;
+        const int tx = c->rec_ijk[3 * r] / P.txc, ty = c->rec_ijk[3 * r + 1] / P.tyc;
+        const int tz = c->rec_ijk[3 * r + 2] / P.a.zc;
+        const int t = (int)((((long long)tz * P.nty + ty) * P.ntx + tx) * P.nchunk + chunk);
+        ents[e] = {t % grid, t, r};
+    }
+    std::sort(ents.begin(), ents.end(), [](const Ent& a, const Ent& b) {
+        return a.cta != b.cta ? a.cta < b.cta : a.tile != b.tile ? a.tile < b.tile : a.r < b.r;
+    });
+    ptr.assign(kMaxCtas + 1, 0);
+    own.assign(std::max(nent, 1), make_int4(-1, -1, -1, 0));
+    for (int e = 0; e < nent; ++e) ptr[ents[e].cta + 1]++;
+    for (int b = 0; b < kMaxCtas; ++b) ptr[b + 1] += ptr[b];
+    for (int e = 0; e < nent;) {
+        int f = e;
+        while (f < nent && ents[f].cta == ents[e].cta && ents[f].tile == ents[e].tile) ++f;
+        for (int j = e; j < f; ++j) {
+            const int r = ents[j].r;
+            const int cell = (c->rec_ijk[3 * r + 2] * c->g.ny + c->rec_ijk[3 * r + 1]) * c->g.nx + c->rec_ijk[3 * r];
+            own[j] = make_int4(r, cell, ents[j].tile, j == e ? f - e : 0);
+        }
+        e = f;
     }
 }
 
-int tma_setup(wri_ctx* c) {
-    c->tma_cb = tma_chunk_for(c->nb);
-    if (!c->tma_cb) return WRI_OK;
-    if (!get_encode_fn()) { c->tma_cb = 0; return WRI_OK; }
-    return dispatch_cb(c->tma_cb, [&](auto cb) -> int {
-        constexpr int CB = decltype(cb)::value;
-        int rc = tma_plan<typename CfgFor<CB, MODE_F>::type>(c, c->planF, c->V, c->U, true);
-        if (rc) return rc;
-        return tma_plan<typename CfgFor<CB, MODE_A>::type>(c, c->planA, c->U, c->V, false);
-    });
+int rt_grid(const wri_ctx* c) { return std::max(1, std::min(c->num_sms, kMaxCtas)); }
+
+// Plans, tensor maps and receiver lists of the solve that is starting: one entry per width the working
+// set can have (nb, nb-2, ..., 2 for an adaptive solve, else nb alone), for both vector sets.  Cached:
+// rebuilt only when the widths, the vector slots, the model pointer or the options change.
+int rt_setup(wri_ctx* c) {
+    wri_ctx::PlanKey key;
+    key.nb = c->nb; key.adaptive = c->adaptive; key.stencil = c->stencil; key.m = c->m; key.dbg = c->dbg;
+    for (int p = 0; p < 2; ++p)
+        for (int q = 0; q < 4; ++q) key.v[p][q] = c->vec[p][q];
+    auto same = [](const wri_ctx::PlanKey& a, const wri_ctx::PlanKey& b) {
+        if (a.nb != b.nb || a.adaptive != b.adaptive || a.stencil != b.stencil || a.m != b.m) return false;
+        for (int p = 0; p < 2; ++p)
+            for (int q = 0; q < 4; ++q)
+                if (a.v[p][q] != b.v[p][q]) return false;
+        const wri_debug_opts &x = a.dbg, &y = b.dbg;
+        return x.nstage_f == y.nstage_f && x.nstage_a == y.nstage_a && x.zc_f == y.zc_f && x.zc_a == y.zc_a &&
+               x.txc == y.txc && x.tyc == y.tyc && x.generic == y.generic;
+    };
+    if (c->plan_valid && same(key, c->plan_key)) return WRI_OK;
+    c->plan_valid = false;
+    const int nw = c->adaptive ? c->nb / 2 : 1;
+    const int own_cap = std::max(1, c->n_rec * std::max(1, c->nb / std::max(2, rt_chunk_for(c, c->nb))));
+    if (nw > c->cap_widths || own_cap > c->cap_own) {
+        // the tables are in use by nothing: every earlier solve of this context was enqueued on the same
+        // stream, and cudaFree waits for the device
+        cudaFree(c->d_plans); cudaFree(c->d_maps); cudaFree(c->d_mmaps); cudaFree(c->d_own_ptr); cudaFree(c->d_own);
+        c->d_plans = nullptr; c->d_maps = nullptr; c->d_mmaps = nullptr; c->d_own_ptr = nullptr; c->d_own = nullptr;
+        c->cap_widths = std::max(nw, c->cap_widths);
+        c->cap_own = std::max(own_cap, c->cap_own);
+        CK(cudaMalloc(&c->d_plans, (size_t)c->cap_widths * sizeof(DevPlan)));
+        CK(cudaMalloc(&c->d_maps, (size_t)c->cap_widths * 2 * N_MAPS * sizeof(CUtensorMap)));
+        CK(cudaMalloc(&c->d_mmaps, (size_t)c->cap_widths * sizeof(CUtensorMap)));
+        CK(cudaMalloc(&c->d_own_ptr, (size_t)c->cap_widths * (kMaxCtas + 1) * sizeof(int)));
+        CK(cudaMalloc(&c->d_own, (size_t)c->cap_widths * c->cap_own * sizeof(int4)));
+    }
+    c->h_plans.assign(nw, DevPlan{});
+    std::vector<CUtensorMap> maps((size_t)nw * 2 * N_MAPS), mmaps(nw);
+    std::vector<int> own_ptr((size_t)nw * (kMaxCtas + 1), 0);
+    std::vector<int4> own((size_t)nw * c->cap_own, make_int4(-1, -1, -1, 0));
+    const int nxyz = c->g.nx + c->g.ny + c->g.nz;
+    c->smem_f = c->smem_a = 0;
+    int rc;
+    for (int wi = 0; wi < nw; ++wi) {
+        const int w = c->nb - 2 * wi;
+        DevPlan& P = c->h_plans[wi];
+        if ((rc = make_plan(c, w, P))) return rc;
+        c->smem_f = std::max(c->smem_f, rt_smem_bytes(P, 3, P.f.nstage, nxyz));
+        c->smem_a = std::max(c->smem_a, rt_smem_bytes(P, 1, P.a.nstage, nxyz));
+        for (int par = 0; par < (c->adaptive ? 2 : 1); ++par) {
+            CUtensorMap* M = &maps[((size_t)wi * 2 + par) * N_MAPS];
+            const bool mg = P.merged != 0;
+            float2* const* v = c->vec[par];
+            if ((rc = make_tmap(&M[MP_V_HALO], v[1], c, w, P.cb, P.txc + 2, P.tyc + 2, mg))) return rc;
+            if ((rc = make_tmap(&M[MP_U_HALO], v[0], c, w, P.cb, P.txc + 2, P.tyc + 2, mg))) return rc;
+            if ((rc = make_tmap(&M[MP_U_CTR], v[0], c, w, P.cb, P.txc, P.tyc, mg))) return rc;
+            if ((rc = make_tmap(&M[MP_V_CTR], v[1], c, w, P.cb, P.txc, P.tyc, mg))) return rc;
+            if ((rc = make_tmap(&M[MP_W_CTR], v[2], c, w, P.cb, P.txc, P.tyc, mg))) return rc;
+            if ((rc = make_tmap(&M[MP_X_CTR], v[3], c, w, P.cb, P.txc, P.tyc, mg))) return rc;
+        }
+        if (P.m_tma && (rc = make_tmap_model(&mmaps[wi], c, P.txc, P.tyc))) return rc;
+        if (c->n_rec) {
+            std::vector<int> ptr;
+            std::vector<int4> ow;
+            build_own(c, P, rt_grid(c), ptr, ow);
+            std::copy(ptr.begin(), ptr.end(), own_ptr.begin() + (size_t)wi * (kMaxCtas + 1));
+            std::copy(ow.begin(), ow.begin() + std::min<size_t>(ow.size(), c->cap_own), own.begin() + (size_t)wi * c->cap_own);
+        }
+    }
+    // pageable sources: each call returns once the data sits in the driver's staging buffer
+    CK(cudaMemcpyAsync(c->d_plans, c->h_plans.data(), nw * sizeof(DevPlan), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(c->d_maps, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(c->d_mmaps, mmaps.data(), mmaps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(c->d_own_ptr, own_ptr.data(), own_ptr.size() * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(c->d_own, own.data(), own.size() * sizeof(int4), cudaMemcpyHostToDevice, c->stream));
+    c->n_widths = nw;
+    c->plan_key = key;
+    c->plan_valid = true;
+    return WRI_OK;
 }
 
 ScalParams scal_params(const wri_ctx* c, const double* partials, int n_rows, const float2* d) {
@@ -590,8 +645,8 @@ ScalParams scal_params(const wri_ctx* c, const double* partials, int n_rows, con
     s.n_tiles = n_rows;
     s.nb = c->nb; s.nb_max = c->nb_max;
     s.n_rec = c->n_rec; s.rec = c->rec;
-    s.V = c->V; s.U_bot = c->U_bot; s.d = d;
-    s.coef = c->coef; s.stat = c->stat; s.active = c->active; s.iters = c->iters;
+    s.V = c->V; s.U_bot = c->U_bot[0]; s.d = d;
+    s.coef = c->coef[0]; s.stat = c->stat[0]; s.active = c->active[0]; s.iters = c->iters[0];
     s.tol = c->tol; s.resnorms = c->resnorms; s.iters_out = c->iters_out;
     s.k = c->k; s.maxit = c->maxit; s.lambda = c->lambda;
     s.rows_in_pass = 1;
@@ -608,177 +663,147 @@ ScalParams scal_params(const wri_ctx* c, const double* partials, int n_rows, con
     return s;
 }
 
-// Ring depth per pass and plan.  Measured on B200 (profiles/r01_v6_stages.md): the adjoint pass is
-// sensitive to the prefetch distance (more stages in flight cost L2 hits on the stencil halo), with
-// the optimum near 130-160 KB of stages in flight: 6 stages for one 64-column chunk per cell, 5 for 32
-// columns or several chunks, 7-8 for the narrower widths with their smaller stages; pass F at 3 (2 for
-// 32-column chunks, 4 for 40).
-template <class Cfg, int MODE>
-int ring_depth(int nchunk) {
-    int n;
-    if (MODE == MODE_F) n = Cfg::CB == 32 ? 2 : Cfg::CB == 40 ? 4 : 3;
-    else if (MODE == MODE_G) n = Cfg::NSTAGE;     // one light stream: the deepest ring the stage layout allows
-    else if (Cfg::CB == 64) n = nchunk == 1 ? 6 : 5;
-    else if (Cfg::CB == 32) n = 5;
-    else if (Cfg::CB == 56) n = 6;
-    else if (Cfg::CB == 48) n = 7;
-    else if (Cfg::CB == 40 || Cfg::CB == 24) n = 8;
-    else n = 7;                                   // 16, 8, 4, 2 columns: small stages, deeper ring
-    if (const char* e = getenv(MODE == MODE_F ? "WRI_F_NSTAGE" : "WRI_A_NSTAGE"))
-        if (atoi(e) > 0) n = atoi(e);
-    return std::max(2, std::min(n, (int)Cfg::NSTAGE));
+void rt_common(const wri_ctx* c, RtParams& p) {
+    const StencilW w = stencil_weights(c->stencil);
+    p.m = c->m;
+    p.gtab = c->gtab;
+    p.counter = c->counter;
+    p.prof = c->d_prof;
+    p.nx = c->g.nx; p.ny = c->g.ny; p.nz = c->g.nz; p.nb_max = c->nb_max;
+    p.ih2 = (float)(1.0 / (c->h * c->h));
+    p.a0h = (float)(w.a0 / (c->h * c->h));
+    p.a1 = (float)w.a1; p.a2 = (float)w.a2; p.a3 = (float)w.a3;
+    for (int par = 0; par < 2; ++par) {
+        p.coef[par] = c->coef[par]; p.stat[par] = c->stat[par];
+        p.active[par] = c->active[par]; p.iters[par] = c->iters[par];
+    }
 }
 
-template <class Cfg, int MODE>
-int launch_tma_cfg(wri_ctx* c, int phase) {
-    const wri_ctx::TmaPlan& P = (MODE == MODE_F) ? c->planF : c->planA;
-    const size_t smem = tma_smem_bytes<Cfg, MODE>(c);
-    int rc_attr = allow_smem(c, (const void*)k_pass_tma<Cfg, MODE>, smem);
-    if (rc_attr) return rc_attr;
-    const size_t NM = c->nb_max;
-    TmaPassParams p{};
-    p.m = c->m;
-    p.gx = c->gtab; p.gy = c->gtab + c->g.nx; p.gz = c->gtab + c->g.nx + c->g.ny;
-    p.w2 = c->coef + C_W2 * NM;
-    p.partials = c->partials_tma; p.counter = c->counter;
-    p.nx = c->g.nx; p.ny = c->g.ny; p.nz = c->g.nz; p.nb = c->nb;
-    p.zc = P.zc; p.ntx = P.ntx; p.nty = P.nty; p.ntz = P.ntz;
-    p.nchunk = P.nchunk; p.n_tiles = P.tiles;
-    p.ih2 = (float)(1.0 / (c->h * c->h));
-    p.m6ih2 = (float)(-6.0 / (c->h * c->h));
+template <int MODE>
+const void* rt_kernel(const wri_ctx* c) {
+    return c->stencil == WRI_STENCIL_27 ? (const void*)k_pass_rt<MODE, ST_27> : (const void*)k_pass_rt<MODE, ST_7>;
+}
+
+// parameters of one pass of the solve in flight (the same for every iteration: what changes lives
+// in the device-resident state)
+template <int MODE>
+RtParams rt_solve_params(const wri_ctx* c, int phase) {
+    RtParams p{};
+    rt_common(c, p);
+    p.st = c->d_state;
+    p.plans = c->d_plans; p.maps = c->d_maps; p.mmaps = c->d_mmaps;
+    p.own_ptr_tab = c->d_own_ptr; p.own_tab = c->d_own;
+    p.own_ptr_stride = kMaxCtas + 1; p.own_stride = c->cap_own;
+    for (int par = 0; par < 2; ++par) {
+        for (int q = 0; q < 4; ++q) p.vec[par][q] = c->vec[par][q];
+        p.U_bot[par] = c->U_bot[par];
+    }
+    p.partials = c->partials_rt;
+    p.sgn = (MODE == MODE_F) ? 1.f : -1.f;
     p.phase = phase;
-    // streams known to be zero are neither cleared nor read: V in the start's adjoint pass, W and X in the
-    // first forward pass of a cold batch solve (c->wx_zero)
-    p.has_q = (MODE == MODE_A) ? (phase != PH_INIT_A) : (MODE == MODE_F ? !c->wx_zero : 1);
-    p.nstage = ring_depth<Cfg, MODE>(P.nchunk);
-    p.m_tma = P.m_tma;
-    p.merged = P.merged;
-    p.fin = scal_params(c, c->partials_tma, P.grid, nullptr);
-    p.n_rec = c->n_rec; p.rec = c->rec; p.U_bot = c->U_bot; p.V = c->V;
-    p.ct = c->coef + C_CT_A * NM; p.own_ptr = c->own_ptr; p.own = c->own;
-    if (MODE == MODE_F) {
-        p.out = c->U; p.W = c->W; p.X = c->X; p.sgn = 1.f;
-        p.ca = c->coef + C_CA_F * NM; p.cb = c->coef + C_CB_F * NM; p.cv = c->coef + C_CV_F * NM;
-        p.cx = c->coef + C_CX * NM; p.cw = c->coef + C_CW * NM;
-    } else {
-        p.out = c->V; p.sgn = -1.f;
-        p.ca = c->coef + C_CA_A * NM; p.cb = c->coef + C_CB_A * NM;
-        p.cv = p.cx = p.cw = p.ca;
-    }
+    // streams known to be zero are neither cleared nor read: V in the start's adjoint pass, W and X in
+    // the first forward pass of a cold batch solve (c->lazy)
+    p.has_old = (MODE == MODE_A) ? (phase != PH_INIT_A) : 1;
+    p.lazy = c->lazy;
+    p.packed = c->packed; p.adaptive = c->adaptive; p.chk = kChk;
+    p.maxit = c->maxit;
+    p.n_rec = c->n_rec; p.rec = c->rec;
+    p.fin = scal_params(c, c->partials_rt, rt_grid(c), nullptr);
+    return p;
+}
+
+template <int MODE>
+int launch_rt(wri_ctx* c, int phase) {
+    const size_t smem = (MODE == MODE_F) ? c->smem_f : c->smem_a;
+    const void* fn = rt_kernel<MODE>(c);
+    int rc = allow_smem(c, fn, smem);
+    if (rc) return rc;
+    RtParams p = rt_solve_params<MODE>(c, phase);
+    CUtensorMap dummy{};
     cudaEvent_t e1 = nullptr;
-    if (c->profiling && phase != PH_INIT_A) {
-        if (c->ev_used * 2 == c->ev_pool.size()) {
-            cudaEvent_t a, b;
-            CK(cudaEventCreate(&a));
-            CK(cudaEventCreate(&b));
-            c->ev_pool.push_back(a); c->ev_pool.push_back(b); c->ev_kind.push_back(0); c->ev_cols.push_back(0);
-        }
-        cudaEvent_t e0 = c->ev_pool[2 * c->ev_used];
-        e1 = c->ev_pool[2 * c->ev_used + 1];
-        c->ev_kind[c->ev_used] = (MODE == MODE_F) ? 0 : 1;
-        c->ev_cols[c->ev_used] = c->nb;
-        c->ev_used++;
-        CK(cudaEventRecord(e0, c->stream));
-    }
-    k_pass_tma<Cfg, MODE><<<P.grid, Cfg::NT + 32, smem, c->stream>>>(P.in, P.old, P.w, P.x, P.m, p);
+    if (phase != PH_INIT_A && (rc = profile_event_begin(c, MODE == MODE_F ? 0 : 1, &e1))) return rc;
+    void* args[] = {&dummy, &dummy, &dummy, &p};
+    CK(cudaLaunchKernel(fn, dim3(rt_grid(c)), dim3(RT_NT + 32), args, smem, c->stream));
     c->launches++;
-    CK(cudaGetLastError());
     if (e1) CK(cudaEventRecord(e1, c->stream));
     return WRI_OK;
 }
 
+MoveParams move_params(const wri_ctx* c) {
+    MoveParams p{};
+    p.st = c->d_state; p.plans = c->d_plans;
+    for (int par = 0; par < 2; ++par) {
+        for (int q = 0; q < 4; ++q) p.vec[par][q] = c->vec[par][q];
+        p.U_bot[par] = c->U_bot[par];
+        p.coef[par] = c->coef[par]; p.stat[par] = c->stat[par];
+        p.active[par] = c->active[par]; p.iters[par] = c->iters[par];
+    }
+    p.u_out = c->u_out; p.resnorms = c->resnorms;
+    p.n_g = (long long)c->ng; p.nb_out = c->nb0; p.nb_max = c->nb_max; p.maxit = c->maxit; p.n_rec = c->n_rec;
+    p.packed = c->packed;
+    p.counter = c->counter2;
+    return p;
+}
+
+// A static launch of the pass kernel (operator entries, gradient pass, warm start): plan and tensor
+// maps travel as kernel parameters, nothing is read from the solve state.
+struct StaticLaunch {
+    DevPlan P;
+    CUtensorMap in, old, m;
+    size_t smem;
+    int grid;
+};
+int static_plan(wri_ctx* c, int nb, const void* in, const void* old, StaticLaunch& S) {
+    int rc = make_plan(c, nb, S.P);
+    if (rc) return rc;
+    DevPlan& P = S.P;
+    // one light stream: the deepest ring that fits (measured for the operator entries: deeper is better)
+    const int nxyz = c->g.nx + c->g.ny + c->g.nz;
+    int n = c->dbg.nstage_a > 0 ? c->dbg.nstage_a : RT_MAX_STAGES;
+    n = std::min(n, RT_MAX_STAGES);
+    while (n > 2 && rt_smem_bytes(P, 1, n, nxyz) > (size_t)RT_SMEM_MAX) --n;
+    P.a.nstage = n;
+    S.smem = rt_smem_bytes(P, 1, n, nxyz);
+    S.grid = std::min(P.a.n_tiles, rt_grid(c));
+    const bool mg = P.merged != 0;
+    if ((rc = make_tmap(&S.in, in, c, nb, P.cb, P.txc + 2, P.tyc + 2, mg))) return rc;
+    if ((rc = make_tmap(&S.old, old ? old : in, c, nb, P.cb, P.txc, P.tyc, mg))) return rc;
+    if (P.m_tma) { if ((rc = make_tmap_model(&S.m, c, P.txc, P.tyc))) return rc; }
+    else S.m = S.old;
+    return WRI_OK;
+}
+
 template <int MODE>
-int launch_tma(wri_ctx* c, int phase) {
-    return dispatch_cb(c->tma_cb, [&](auto cb) -> int {
-        return launch_tma_cfg<typename CfgFor<decltype(cb)::value, MODE>::type, MODE>(c, phase);
-    });
-}
-
-// objective + gradient through the TMA pipeline (one chunk per cell, power-of-two column pairs)
-template <int CB>
-int launch_tma_grad(wri_ctx* c, const float2* u, const float2* q, const int* src, const float2* alpha,
-                    float* g, float lambda) {
-    // pass A's tile shape, 512 consumer threads (one item each): this pass is bound by
-    // instruction issue, not by DRAM, and 4 warps per scheduler hide the shared-memory latency
-    typedef typename CfgFor<CB, MODE_A>::type CfgA;
-    typedef TileCfg<CB, CfgA::TXC, CfgA::TYC, WRI_F_NT, WRI_A_STAGES> Cfg;
-    int rc = tma_plan<Cfg>(c, c->planG, u, q ? q : u, false, false);
+int launch_static(wri_ctx* c, StaticLaunch& S, RtParams& p) {
+    const void* fn = rt_kernel<MODE>(c);
+    int rc = allow_smem(c, fn, S.smem);
     if (rc) return rc;
-    const wri_ctx::TmaPlan& P = c->planG;
-    const size_t smem = tma_smem_bytes<Cfg, MODE_G>(c);
-    if ((rc = allow_smem(c, (const void*)k_pass_tma<Cfg, MODE_G>, smem))) return rc;
-    const size_t NM = c->nb_max;
-    TmaPassParams p{};
-    p.m = c->m;
-    p.gx = c->gtab; p.gy = c->gtab + c->g.nx; p.gz = c->gtab + c->g.nx + c->g.ny;
-    p.w2 = c->coef + C_W2 * NM;
-    p.ca = p.cb = p.cv = p.cx = p.cw = p.w2;      // unused by MODE_G
-    p.partials = c->partials_tma; p.counter = c->counter;
-    p.nx = c->g.nx; p.ny = c->g.ny; p.nz = c->g.nz; p.nb = c->nb;
-    p.zc = P.zc; p.ntx = P.ntx; p.nty = P.nty; p.ntz = P.ntz;
-    p.nchunk = P.nchunk; p.n_tiles = P.tiles;
-    p.ih2 = (float)(1.0 / (c->h * c->h));
-    p.m6ih2 = (float)(-6.0 / (c->h * c->h));
-    p.sgn = 1.f;
-    p.m_tma = P.m_tma; p.merged = P.merged;
-    p.nstage = ring_depth<Cfg, MODE_G>(P.nchunk);
-    p.has_q = q != nullptr; p.gsrc = src; p.galpha = alpha; p.g = g; p.lam2 = lambda * lambda;
-    k_pass_tma<Cfg, MODE_G><<<P.grid, Cfg::NT + 32, smem, c->stream>>>(P.in, P.old, P.old, P.old, P.m, p);
+    rt_common(c, p);
+    p.st = nullptr;
+    p.plan0 = S.P;
+    void* args[] = {&S.in, &S.old, &S.m, &p};
+    CK(cudaLaunchKernel(fn, dim3(S.grid), dim3(RT_NT + 32), args, S.smem, c->stream));
     c->launches++;
-    CK(cudaGetLastError());
     return WRI_OK;
 }
 
-// out = lambda * A in (sgn = +1) or lambda * A^H in (sgn = -1) through the TMA pipeline: pass A's kernel
-// without its in-place stream, scalar phase and receiver rows.  No workspace is touched.
-template <int CB>
-int launch_tma_apply(wri_ctx* c, const float2* in, float2* out, float sgn) {
-    typedef typename CfgFor<CB, MODE_A>::type Cfg;
-    int rc = tma_plan<Cfg>(c, c->planG, in, in, false, false);
-    if (rc) return rc;
-    const wri_ctx::TmaPlan& P = c->planG;
-    const size_t smem = tma_smem_bytes<Cfg, MODE_A>(c);
-    if ((rc = allow_smem(c, (const void*)k_pass_tma<Cfg, MODE_A>, smem))) return rc;
-    const size_t NM = c->nb_max;
-    TmaPassParams p{};
-    p.m = c->m;
-    p.gx = c->gtab; p.gy = c->gtab + c->g.nx; p.gz = c->gtab + c->g.nx + c->g.ny;
-    p.w2 = c->coef + C_W2 * NM;
-    p.ca = c->coef + C_LAM * NM;
-    p.cb = p.cv = p.cx = p.cw = p.ca;                 // unused without the in-place stream
-    p.partials = nullptr; p.counter = c->counter;
-    p.nx = c->g.nx; p.ny = c->g.ny; p.nz = c->g.nz; p.nb = c->nb;
-    p.zc = P.zc; p.ntx = P.ntx; p.nty = P.nty; p.ntz = P.ntz;
-    p.nchunk = P.nchunk; p.n_tiles = P.tiles;
-    p.ih2 = (float)(1.0 / (c->h * c->h));
-    p.m6ih2 = (float)(-6.0 / (c->h * c->h));
-    p.sgn = sgn;
-    p.phase = -1; p.has_q = 0; p.n_rec = 0;
-    p.m_tma = P.m_tma; p.merged = P.merged;
-    p.nstage = Cfg::NSTAGE;                           // no in-place stream: the deepest ring (measured 7 > 6 > 5)
-    p.out = out;
-    k_pass_tma<Cfg, MODE_A><<<P.grid, Cfg::NT + 32, smem, c->stream>>>(P.in, P.old, P.old, P.old, P.m, p);
-    c->launches++;
-    CK(cudaGetLastError());
-    return WRI_OK;
-}
-
-// operator part of wri_apply_M / _MH: TMA pipeline when the width has a tile configuration, else k_pass
+// out = lambda * A in (sgn = +1) or lambda * A^H in (sgn = -1): the pass kernel without its in-place
+// stream, scalar phase and receiver rows; the generic kernel for odd widths.  No workspace is touched.
 int apply_operator(wri_ctx* c, int nb, const float2* in, float2* out, float sgn) {
-    const int cb = (c->solving || getenv("WRI_APPLY_GENERIC") || !get_encode_fn()) ? 0 : tma_chunk_for(nb);
-    if (cb) {
-        const int nb_saved = c->nb;
-        c->nb = nb;
-        const int rc = dispatch_cb(cb, [&](auto t) -> int {
-            return launch_tma_apply<decltype(t)::value>(c, in, out, sgn);
-        });
-        c->nb = nb_saved;
-        return rc;
+    if (!c->solving && rt_chunk_for(c, nb)) {
+        StaticLaunch S;
+        int rc = static_plan(c, nb, in, nullptr, S);
+        if (rc) return rc;
+        RtParams p{};
+        p.sgn = sgn; p.phase = -1; p.has_old = 0;
+        p.ca_static = c->coef[0] + C_LAM * (size_t)c->nb_max;
+        p.out = out;
+        return launch_static<MODE_A>(c, S, p);
     }
     const Tiling t = make_tiling(c, nb);
     PassParams p = base_params(c, nb, t);
     p.in = in; p.out = out;
-    p.ca = c->coef + C_LAM * (size_t)c->nb_max;
+    p.ca = c->coef[0] + C_LAM * (size_t)c->nb_max;
     p.sgn = sgn;
     return launch_pass<MODE_APPLY>(c, p, t);
 }
@@ -787,7 +812,7 @@ int check_batch_args(const wri_ctx* c, int nb) {
     if (!c) return WRI_ERR_ARG;
     if (nb <= 0 || nb > c->nb_max) return WRI_ERR_ARG;
     if (c->rmask && c->rmask_nb != nb) return WRI_ERR_ARG;       // the receiver mask was given for another width
-    if ((long long)c->ng * nb > 0x7fffffffLL * 1LL) return WRI_ERR_ARG;   // element indices stay below 2^31
+    if ((long long)c->ng * even_up(nb) > 0x7fffffffLL * 1LL) return WRI_ERR_ARG;   // element indices stay below 2^31
     return WRI_OK;
 }
 
@@ -804,6 +829,7 @@ const char* wri_strerror(int code) {
         case WRI_ERR_WORKSPACE: return "workspace missing or too small";
         case WRI_ERR_CUDA: return g_cuda_msg;
         case WRI_ERR_STATE: return "call out of order";
+        case WRI_ERR_NUMERIC: return "objective is not finite";
         default: return "unknown error code";
     }
 }
@@ -839,9 +865,11 @@ int wri_create(wri_ctx** out, wri_grid grid, double h, int32_t n_omega, const do
     wri_ctx* c = new wri_ctx();
     c->g = grid; c->h = h; c->ng = ng;
     c->omega.assign(omega_host, omega_host + n_omega);
-    c->sponge = sponge; c->n_rec = n_rec; c->nb_max = nb_max;
+    c->sponge = sponge; c->n_rec = n_rec;
+    c->nb_max = even_up(nb_max);                     // an odd batch runs in an even-width working set
     c->stream = (cudaStream_t)cuda_stream;
     c->m = m_dev;
+    const int NM = c->nb_max;
 
     // sponge profile per axis, computed in double and rounded once; gamma = max over axes
     const int L = sponge.width;
@@ -872,31 +900,30 @@ int wri_create(wri_ctx** out, wri_grid grid, double h, int32_t n_omega, const do
     CKC(cudaMalloc(&c->rec, std::max(n_rec, 1) * sizeof(int)));
     if (n_rec) CKC(cudaMemcpy(c->rec, cells.data(), n_rec * sizeof(int), cudaMemcpyHostToDevice));
     c->rec_ijk.assign(rec_ijk_host, rec_ijk_host + 3 * (size_t)n_rec);
-    CKC(cudaMalloc(&c->own_ptr, (kMaxCtas + 1) * sizeof(int)));
-    CKC(cudaMalloc(&c->own, (size_t)std::max(n_rec, 1) * (nb_max / kMinChunk + 1) * sizeof(int4)));
-    CKC(cudaMalloc(&c->coef, (size_t)N_COEF * nb_max * sizeof(float)));
-    CKC(cudaMemset(c->coef, 0, (size_t)N_COEF * nb_max * sizeof(float)));
-    CKC(cudaMalloc(&c->stat, (size_t)N_STAT * nb_max * sizeof(double)));
-    CKC(cudaMemset(c->stat, 0, (size_t)N_STAT * nb_max * sizeof(double)));
-    CKC(cudaMalloc(&c->active, nb_max * sizeof(int)));
-    CKC(cudaMalloc(&c->iters, nb_max * sizeof(int)));
-    CKC(cudaMemset(c->active, 0, nb_max * sizeof(int)));
-    CKC(cudaMemset(c->iters, 0, nb_max * sizeof(int)));
-    CKC(cudaMalloc(&c->coef_alt, (size_t)N_COEF * nb_max * sizeof(float)));
-    CKC(cudaMalloc(&c->stat_alt, (size_t)N_STAT * nb_max * sizeof(double)));
-    CKC(cudaMalloc(&c->active_alt, nb_max * sizeof(int)));
-    CKC(cudaMalloc(&c->iters_alt, nb_max * sizeof(int)));
-    CKC(cudaMalloc(&c->colmap, nb_max * sizeof(int)));
-    CKC(cudaMalloc(&c->src, nb_max * sizeof(int)));
-    CKC(cudaMalloc(&c->idx, (size_t)3 * nb_max * sizeof(int)));
-    CKC(cudaMallocHost(&c->h_active, nb_max * sizeof(int)));
-    CKC(cudaMalloc(&c->aw_tol, nb_max * sizeof(float)));
-    CKC(cudaMalloc(&c->aw_f, (size_t)2 * nb_max * sizeof(double)));
-    CKC(cudaMalloc(&c->aw_ar0, nb_max * sizeof(double)));
-    CKC(cudaMalloc(&c->aw_iters, nb_max * sizeof(int)));
-    CKC(cudaMallocHost(&c->h_aw, (size_t)nb_max * (2 * sizeof(double) + sizeof(int))));
-    CKC(cudaMalloc(&c->counter, sizeof(unsigned int)));
-    CKC(cudaMemset(c->counter, 0, sizeof(unsigned int)));
+    for (int b = 0; b < 2; ++b) {
+        CKC(cudaMalloc(&c->coef[b], (size_t)N_COEF * NM * sizeof(float)));
+        CKC(cudaMemset(c->coef[b], 0, (size_t)N_COEF * NM * sizeof(float)));
+        CKC(cudaMalloc(&c->stat[b], (size_t)N_STAT * NM * sizeof(double)));
+        CKC(cudaMemset(c->stat[b], 0, (size_t)N_STAT * NM * sizeof(double)));
+        CKC(cudaMalloc(&c->active[b], NM * sizeof(int)));
+        CKC(cudaMalloc(&c->iters[b], NM * sizeof(int)));
+        CKC(cudaMemset(c->active[b], 0, NM * sizeof(int)));
+        CKC(cudaMemset(c->iters[b], 0, NM * sizeof(int)));
+    }
+    CKC(cudaMalloc(&c->colmap, NM * sizeof(int)));
+    CKC(cudaMalloc(&c->src, NM * sizeof(int)));
+    CKC(cudaMalloc(&c->aw_tol, NM * sizeof(float)));
+    CKC(cudaMalloc(&c->aw_f, (size_t)2 * NM * sizeof(double)));
+    CKC(cudaMalloc(&c->aw_ar0, NM * sizeof(double)));
+    CKC(cudaMalloc(&c->aw_iters, NM * sizeof(int)));
+    CKC(cudaMallocHost(&c->h_aw, (size_t)NM * (2 * sizeof(double) + sizeof(int))));
+    CKC(cudaMalloc(&c->counter, 2 * sizeof(unsigned int)));
+    CKC(cudaMemset(c->counter, 0, 2 * sizeof(unsigned int)));
+    c->counter2 = c->counter + 1;
+    CKC(cudaMalloc(&c->d_state, sizeof(SolveState)));
+    CKC(cudaMemset(c->d_state, 0, sizeof(SolveState)));
+    CKC(cudaMalloc(&c->d_prof, 4 * sizeof(long long)));
+    CKC(cudaMemset(c->d_prof, 0, 4 * sizeof(long long)));
     {
         int dev = 0;
         CKC(cudaGetDevice(&dev));
@@ -909,14 +936,15 @@ int wri_create(wri_ctx** out, wri_grid grid, double h, int32_t n_omega, const do
 
 int wri_destroy(wri_ctx* c) {
     if (!c) return WRI_OK;
-    cudaFree(c->gtab); cudaFree(c->rec); cudaFree(c->coef); cudaFree(c->stat);
-    cudaFree(c->active); cudaFree(c->iters); cudaFree(c->counter);
-    cudaFree(c->own_ptr); cudaFree(c->own);
-    cudaFree(c->coef_alt); cudaFree(c->stat_alt); cudaFree(c->active_alt); cudaFree(c->iters_alt);
-    cudaFree(c->colmap); cudaFree(c->idx); cudaFree(c->src);
-    if (c->h_active) cudaFreeHost(c->h_active);
+    cudaFree(c->gtab); cudaFree(c->rec); cudaFree(c->counter);
+    for (int b = 0; b < 2; ++b) { cudaFree(c->coef[b]); cudaFree(c->stat[b]); cudaFree(c->active[b]); cudaFree(c->iters[b]); }
+    cudaFree(c->colmap); cudaFree(c->src);
     cudaFree(c->aw_tol); cudaFree(c->aw_f); cudaFree(c->aw_ar0); cudaFree(c->aw_iters);
     if (c->h_aw) cudaFreeHost(c->h_aw);
+    cudaFree(c->d_plans); cudaFree(c->d_maps); cudaFree(c->d_mmaps); cudaFree(c->d_own_ptr); cudaFree(c->d_own);
+    cudaFree(c->d_state); cudaFree(c->d_prof);
+    if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    if (c->graph) cudaGraphDestroy(c->graph);
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
     for (auto& sl : c->pipe) {
         if (sl.ev_in) cudaEventDestroy(sl.ev_in);
@@ -932,6 +960,31 @@ int wri_destroy(wri_ctx* c) {
 int wri_set_model(wri_ctx* c, const float* m_dev) {
     if (!c || !m_dev) return WRI_ERR_ARG;
     c->m = m_dev;
+    return WRI_OK;
+}
+
+int wri_set_stencil(wri_ctx* c, int32_t stencil) {
+    if (!c || (stencil != WRI_STENCIL_7 && stencil != WRI_STENCIL_27)) return WRI_ERR_ARG;
+    if (c->solving) return WRI_ERR_STATE;
+    c->stencil = stencil;
+    return WRI_OK;
+}
+
+int wri_plan_info(wri_ctx* c, int32_t nb, int32_t* out16) {
+    if (!c || !out16 || nb <= 0 || nb > c->nb_max) return WRI_ERR_ARG;
+    DevPlan P;
+    int rc = make_plan(c, nb, P);
+    if (rc) return rc;
+    const int v[16] = {P.cb, P.nchunk, P.txc, P.tyc, P.items, P.merged, P.m_tma, P.f.zc, P.f.nstage, P.f.n_tiles,
+                       P.a.zc, P.a.nstage, P.a.n_tiles, rt_stage_bytes(P, 3), rt_stage_bytes(P, 1), rt_grid(c)};
+    for (int i = 0; i < 16; ++i) out16[i] = v[i];
+    return WRI_OK;
+}
+
+int wri_set_debug_opts(wri_ctx* c, const wri_debug_opts* o) {
+    if (!c) return WRI_ERR_ARG;
+    if (c->solving) return WRI_ERR_STATE;
+    c->dbg = o ? *o : wri_debug_opts{};
     return WRI_OK;
 }
 
@@ -974,14 +1027,22 @@ int wri_profile_enable(wri_ctx* c, int32_t on) {
 int wri_profile_read(wri_ctx* c, double* ms_f, int64_t* n_f, int64_t* cols_f, double* ms_a, int64_t* n_a,
                      int64_t* cols_a) {
     if (!c || !ms_f || !n_f || !cols_f || !ms_a || !n_a || !cols_a) return WRI_ERR_ARG;
+    // launches that did work and their widths are counted on the device (the width of an adaptive
+    // solve is not known to the host); the events bracket every launch, no-ops included
+    long long h[4] = {0, 0, 0, 0};
+    CK(cudaMemcpyAsync(h, c->d_prof, sizeof h, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaMemsetAsync(c->d_prof, 0, sizeof h, c->stream));
     CK(cudaStreamSynchronize(c->stream));
-    *ms_f = *ms_a = 0.0; *n_f = *n_a = 0; *cols_f = *cols_a = 0;
+    *ms_f = *ms_a = 0.0;
     for (size_t i = 0; i < c->ev_used; ++i) {
         float ms = 0.f;
         CK(cudaEventElapsedTime(&ms, c->ev_pool[2 * i], c->ev_pool[2 * i + 1]));
-        if (c->ev_kind[i] == 0) { *ms_f += ms; ++*n_f; *cols_f += c->ev_cols[i]; }
-        else { *ms_a += ms; ++*n_a; *cols_a += c->ev_cols[i]; }
+        if (c->ev_kind[i] == 0) *ms_f += ms;
+        else *ms_a += ms;
     }
+    *cols_f = h[0] + c->prof_host[0]; *n_f = h[1] + c->prof_host[1];
+    *cols_a = h[2] + c->prof_host[2]; *n_a = h[3] + c->prof_host[3];
+    c->prof_host[0] = c->prof_host[1] = c->prof_host[2] = c->prof_host[3] = 0;
     c->ev_used = 0;
     return WRI_OK;
 }
@@ -1065,55 +1126,62 @@ int wri_objective_gradient(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host
     if (c->ws_bytes < L.total) return WRI_ERR_WORKSPACE;
     if ((rc = upload_columns(c, nb, omega_idx_host, lambda))) return rc;
     if (src_ijk_host && (rc = upload_sources(c, nb, src_ijk_host))) return rc;
-    GradParams p{};
-    p.u = (const float2*)u_dev; p.q = (const float2*)q_dev;
-    p.src = src_ijk_host ? c->src : nullptr; p.alpha = (const float2*)alpha_dev;
-    p.m = c->m;
-    p.gx = c->gtab; p.gy = c->gtab + c->g.nx; p.gz = c->gtab + c->g.nx + c->g.ny;
-    p.w2 = c->coef + C_W2 * (size_t)c->nb_max;
-    p.g = g_dev;
-    p.partials = (double*)(c->ws + L.partials);
-    p.nx = c->g.nx; p.ny = c->g.ny; p.nz = c->g.nz; p.nb = nb; p.zc = G.t.zc;
-    p.tpc = G.tpc; p.shuffle = G.shuffle;
-    p.ih2 = (float)(1.0 / (c->h * c->h));
-    p.m6ih2 = (float)(-6.0 / (c->h * c->h));
-    p.lam2 = lambda * lambda;
-    // TMA pipeline when the batch is one power-of-two chunk per cell (64 / 32 / 16 / 8 / 4 columns);
-    // the generic kernel otherwise (odd widths, 48, several chunks)
-    int cb = tma_chunk_for(nb);
-    if ((cb & (cb - 1)) || cb == 2 || cb != nb || !get_encode_fn() || getenv("WRI_GRAD_GENERIC")) cb = 0;
+    const StencilW sw = stencil_weights(c->stencil);
+    double* partials = (double*)(c->ws + L.partials);
     int n_rows = (int)G.t.n_tiles;
-    if (cb) {
-        c->nb = nb;
-        c->partials_tma = (double*)(c->ws + L.partials_tma);
-        float* g_user = g_dev;
-        if (g_dev) g_dev = (float*)(c->ws + L.gscratch);
-        switch (cb) {
-            case 64: rc = launch_tma_grad<64>(c, p.u, p.q, p.src, p.alpha, g_dev, lambda); break;
-            case 32: rc = launch_tma_grad<32>(c, p.u, p.q, p.src, p.alpha, g_dev, lambda); break;
-            case 16: rc = launch_tma_grad<16>(c, p.u, p.q, p.src, p.alpha, g_dev, lambda); break;
-            case 8:  rc = launch_tma_grad<8>(c, p.u, p.q, p.src, p.alpha, g_dev, lambda); break;
-            default: rc = launch_tma_grad<4>(c, p.u, p.q, p.src, p.alpha, g_dev, lambda); break;
-        }
-        if (rc) return rc;
-        if (g_user) {
-            k_add_f32<<<blocks_for((long long)c->ng), 256, 0, c->stream>>>(g_user, g_dev, (long long)c->ng);
+    // pass kernel when the batch is one power-of-two chunk per cell (64 / 32 / 16 / 8 / 4 columns): the
+    // per-cell sum over the columns runs on warp shuffles; the generic kernel otherwise
+    const int cb = rt_chunk_for(c, nb);
+    if (cb == nb && nb >= 4 && (nb & (nb - 1)) == 0) {
+        StaticLaunch S;
+        if ((rc = static_plan(c, nb, u_dev, q_dev, S))) return rc;
+        float* g_scr = g_dev ? (float*)(c->ws + L.gscratch) : nullptr;
+        RtParams p{};
+        p.sgn = 1.f; p.phase = -1;
+        p.has_old = q_dev != nullptr;
+        p.partials = (double*)(c->ws + L.partials_rt);
+        p.gsrc = src_ijk_host ? c->src : nullptr;
+        p.galpha = (const float2*)alpha_dev;
+        p.g = g_scr;
+        p.lam2 = lambda * lambda;
+        if ((rc = launch_static<MODE_G>(c, S, p))) return rc;
+        if (g_dev) {
+            k_add_f32<<<blocks_for((long long)c->ng), 256, 0, c->stream>>>(g_dev, g_scr, (long long)c->ng);
             c->launches++;
             CK(cudaGetLastError());
         }
-        p.partials = c->partials_tma;
-        n_rows = c->planG.grid;
+        partials = p.partials;
+        n_rows = S.grid;
     } else {
+        GradParams p{};
+        p.u = (const float2*)u_dev; p.q = (const float2*)q_dev;
+        p.src = src_ijk_host ? c->src : nullptr; p.alpha = (const float2*)alpha_dev;
+        p.m = c->m;
+        p.gx = c->gtab; p.gy = c->gtab + c->g.nx; p.gz = c->gtab + c->g.nx + c->g.ny;
+        p.w2 = c->coef[0] + C_W2 * (size_t)c->nb_max;
+        p.g = g_dev;
+        p.partials = partials;
+        p.nx = c->g.nx; p.ny = c->g.ny; p.nz = c->g.nz; p.nb = nb; p.zc = G.t.zc;
+        p.tpc = G.tpc; p.shuffle = G.shuffle;
+        p.ih2 = (float)(1.0 / (c->h * c->h));
+        p.m6ih2 = (float)(sw.a0 / (c->h * c->h));
+        p.a1 = (float)sw.a1; p.a2 = (float)sw.a2; p.a3 = (float)sw.a3;
+        p.lam2 = lambda * lambda;
         const size_t smem = (size_t)G.t.block.x * G.t.block.y * G.t.vec * sizeof(double);
-        if (G.t.vec == 2) k_grad<2><<<G.t.grid, G.t.block, smem, c->stream>>>(p);
-        else              k_grad<1><<<G.t.grid, G.t.block, smem, c->stream>>>(p);
+        const bool s27 = c->stencil == WRI_STENCIL_27;
+        if (G.t.vec == 2) {
+            if (s27) k_grad<2, ST_27><<<G.t.grid, G.t.block, smem, c->stream>>>(p);
+            else     k_grad<2, ST_7><<<G.t.grid, G.t.block, smem, c->stream>>>(p);
+        } else {
+            if (s27) k_grad<1, ST_27><<<G.t.grid, G.t.block, smem, c->stream>>>(p);
+            else     k_grad<1, ST_7><<<G.t.grid, G.t.block, smem, c->stream>>>(p);
+        }
         c->launches++;
         CK(cudaGetLastError());
     }
-    k_objective<<<(nb + OBJ_CPB - 1) / OBJ_CPB, 1024, 1024 * sizeof(double), c->stream>>>(p.partials, n_rows, nb, p.u,
-                                                             (const float2*)d_dev, c->rec, c->n_rec,
-                                                             (double)lambda * (double)lambda, f_pde_dev,
-                                                             f_data_dev, c->rmask);
+    k_objective<<<(nb + OBJ_CPB - 1) / OBJ_CPB, 1024, 1024 * sizeof(double), c->stream>>>(
+        partials, n_rows, nb, (const float2*)u_dev, (const float2*)d_dev, c->rec, c->n_rec,
+        (double)lambda * (double)lambda, f_pde_dev, f_data_dev, c->rmask);
     c->launches++;
     CK(cudaGetLastError());
     return WRI_OK;
@@ -1124,17 +1192,16 @@ int wri_objective_gradient(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host
 
 namespace {
 
+// One group of a solve.  col0, ncols: the caller's columns [col0, col0 + ncols) are solved in a
+// compact working set of even width nbw >= ncols carved out of the workspace (nbw = 0: all nb columns
+// in the caller's own layout).  Columns are independent systems (reading C-9).
 int lsqr_begin_impl(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const void* q_dev,
                     const void* d_dev, float lambda, const float* tol_dev, int32_t maxit,
                     void* u_out_dev, float* resnorms_dev, int32_t* iters_dev, bool host_staged,
                     const int32_t* src_ijk_host = nullptr, void* alpha_out_dev = nullptr,
-                    int col0 = 0, int nbw = 0, bool lazy_start = false) {
-    // col0, nbw: a GROUPED solve works on the caller's columns [col0, col0 + nbw) only, in a compact
-    // nbw-wide working set of its own (nbw = 0: all nb columns, working set = the caller's layout)
+                    int col0 = 0, int ncols = 0, bool batch = false) {
     int rc = check_batch_args(c, nb);
     if (rc) return rc;
-    const bool grouped = nbw > 0 && nbw < nb;
-    if (!grouped) { col0 = 0; nbw = nb; }
     const bool sf = src_ijk_host != nullptr;          // source-free system: q may be absent (b_top = 0)
     if ((!q_dev && !sf) || (c->n_rec && !d_dev) || !u_out_dev || maxit < 0 ||
         (q_dev && !aligned16(q_dev)) || !aligned16(u_out_dev) || q_dev == u_out_dev || (sf && !alpha_out_dev))
@@ -1143,70 +1210,71 @@ int lsqr_begin_impl(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const
     const int base_flags = host_staged ? WS_HOST_STAGING : 0;
     if (c->ws_bytes < ws_layout(c, nb, base_flags, kHostMaxitCap).total) return WRI_ERR_WORKSPACE;
     const WsLayout L = ws_layout(c, nb, base_flags | WS_COMPACTION, kHostMaxitCap);
-    if ((rc = upload_columns(c, nbw, omega_idx_host ? omega_idx_host + col0 : nullptr, lambda))) return rc;
+    const bool ws_big = c->ws_bytes >= L.total;               // the five spare vector regions are there
+    bool grouped = ncols > 0;
+    if (!grouped) { col0 = 0; ncols = nb; }
+    int nbw = grouped ? even_up(ncols) : nb;
+    // the pass kernel serves even widths; an odd batch runs padded when the workspace has a spare region
+    bool rt = rt_chunk_for(c, nbw) != 0;
+    if (!grouped && (nb % 2) && batch && ws_big && rt_chunk_for(c, nb + 1)) { grouped = true; nbw = nb + 1; rt = true; }
+    // adaptive accuracy: with tolerances, converged columns are compacted out of the working set on the device
+    const bool adaptive = rt && batch && tol_dev && ws_big && nbw <= RT_MAXW && nbw >= 4 && !c->dbg.no_compact;
+    const bool packed = grouped || adaptive;
+
+    // vector slots: nbw-wide pieces of the nb-wide regions (the V region is skipped while the host
+    // entry's staged q sits there: it must survive until the last group has started)
+    std::vector<float2*> slots;
+    {
+        const size_t slot = align_up(c->ng * (size_t)nbw * sizeof(float2), 256);
+        const size_t region = align_up(c->ng * (size_t)even_up(nb) * sizeof(float2), 256);
+        for (int rgn = 0; rgn < (ws_big ? 8 : 3); ++rgn) {
+            if (rgn == 1 && host_staged && q_dev && grouped) continue;
+            for (size_t o = 0; o + slot <= region; o += slot) slots.push_back((float2*)(c->ws + L.vecs[rgn] + o));
+        }
+    }
+    const size_t need = adaptive ? 8 : packed ? 4 : 3;
+    if (slots.size() < need) return WRI_ERR_WORKSPACE;
+    if ((rc = upload_columns(c, nbw, omega_idx_host ? omega_idx_host + col0 : nullptr, lambda, ncols))) return rc;
     if (sf && (rc = upload_sources(c, nb, src_ijk_host))) return rc;
     c->sf = sf;
     c->alpha_out = (float2*)alpha_out_dev;
-
     c->nb = nbw; c->nb0 = nb; c->k = 0; c->maxit = maxit; c->lambda = lambda;
-    c->packed = grouped; c->all_done = false;
-    c->U_bot = (float2*)(c->ws + L.U_bot);
+    c->packed = packed; c->adaptive = adaptive; c->rt = rt;
     c->partials = (double*)(c->ws + L.partials);
-    c->partials_tma = (double*)(c->ws + L.partials_tma);
+    c->partials_rt = (double*)(c->ws + L.partials_rt);
     c->u_out = (float2*)u_out_dev;
-    c->free_slots.clear();
-    const bool ws_compact = c->ws_bytes >= L.total;           // the two spare vectors are there
-    if (!grouped) {
-        c->U = (float2*)(c->ws + L.U); c->V = (float2*)(c->ws + L.V); c->W = (float2*)(c->ws + L.W);
-        c->X = (float2*)u_out_dev;
-        if (ws_compact) {
-            c->free_slots.push_back((float2*)(c->ws + L.B3));
-            c->free_slots.push_back((float2*)(c->ws + L.B4));
-            c->U_bot_alt = (float2*)(c->ws + L.U_bot2);
-        }
-    } else {
-        // nbw-wide slots carved out of the nb-wide vector regions; the V region is skipped when the
-        // host entry has staged q there (it must survive until the last group has started)
-        const size_t slot = align_up(c->ng * (size_t)nbw * sizeof(float2), 256);
-        const size_t region = align_up(c->ng * (size_t)nb * sizeof(float2), 256);
-        std::vector<float2*> slots;
-        size_t bases[5] = {L.U, L.V, L.W, L.B3, L.B4};
-        for (int rgn = 0; rgn < (ws_compact ? 5 : 3); ++rgn) {
-            if (rgn == 1 && host_staged && q_dev) continue;
-            for (size_t o = 0; o + slot <= region; o += slot) slots.push_back((float2*)(c->ws + bases[rgn] + o));
-        }
-        if (slots.size() < 4) return WRI_ERR_WORKSPACE;
-        c->U = slots[0]; c->V = slots[1]; c->W = slots[2]; c->X = slots[3];
-        for (size_t i = 4; i < slots.size(); ++i) c->free_slots.push_back(slots[i]);
-        // the receiver-row region holds nb columns: first half the rows, second half the spare
-        c->U_bot_alt = c->U_bot + (size_t)std::max(c->n_rec, 1) * nbw;
-        std::vector<int> cm(nbw);
-        for (int j = 0; j < nbw; ++j) cm[j] = col0 + j;
-        CK(cudaMemcpyAsync(c->colmap, cm.data(), nbw * sizeof(int), cudaMemcpyHostToDevice, c->stream));
-    }
+    std::memset(c->vec, 0, sizeof c->vec);
+    for (int q = 0; q < 3; ++q) c->vec[0][q] = slots[q];
+    c->vec[0][3] = packed ? slots[3] : (float2*)u_out_dev;
+    if (adaptive) for (int q = 0; q < 4; ++q) c->vec[1][q] = slots[4 + q];
+    c->U = c->vec[0][0]; c->V = c->vec[0][1]; c->W = c->vec[0][2]; c->X = c->vec[0][3];
+    // receiver rows: nbw-wide pieces of the nb-wide region(s)
+    c->U_bot[0] = (float2*)(c->ws + L.U_bot);
+    c->U_bot[1] = ws_big ? (float2*)(c->ws + L.U_bot2) : c->U_bot[0] + (size_t)std::max(c->n_rec, 1) * nbw;
+    if (adaptive && !ws_big) return WRI_ERR_WORKSPACE;
     c->tol = tol_dev; c->resnorms = resnorms_dev; c->iters_out = iters_dev;
     c->tl = make_tiling(c, nbw);
-    if ((rc = tma_setup(c))) return rc;
-    // Convergence is watched from the host only when tolerances are given: every check_every
-    // iterations (~2 ms of device work) the active flags are read back; converged columns are
-    // compacted away when the workspace has room for it and the batch is on the TMA path.
-    c->can_compact = tol_dev && c->tma_cb && c->free_slots.size() >= 2 && !getenv("WRI_NO_COMPACT");
-    c->check_every = 0;
-    if (tol_dev) {
-        const double t_iter = 80.0 * (double)c->ng * nbw / 6.0e12;
-        c->check_every = (int)std::min(32.0, std::max(1.0, std::ceil(2.0e-3 / t_iter)));
+
+    // initial device state (pageable source: staged by the driver before the call returns)
+    SolveState st;
+    std::memset(&st, 0, sizeof st);
+    st.nb = nbw; st.n_active = nbw;
+    for (int j = 0; j < RT_MAXW; ++j) st.colmap[0][j] = st.colmap[1][j] = (j < ncols) ? col0 + j : -1;
+    CK(cudaMemcpyAsync(c->d_state, &st, sizeof st, cudaMemcpyHostToDevice, c->stream));
+    if (packed) {
+        std::vector<int> cm(nbw);
+        for (int j = 0; j < nbw; ++j) cm[j] = (j < ncols) ? col0 + j : -1;
+        CK(cudaMemcpyAsync(c->colmap, cm.data(), nbw * sizeof(int), cudaMemcpyHostToDevice, c->stream));
     }
-    c->h_colmap.resize(nbw);
-    for (int s = 0; s < nbw; ++s) c->h_colmap[s] = col0 + s;
-    c->retired.assign(nb, 0);
+    if (rt && (rc = rt_setup(c))) return rc;
     const size_t vbytes = c->ng * (size_t)nbw * sizeof(float2);
     const size_t NM = c->nb_max;
 
-    // beta1 u1 = b = [lambda q ; d]   (q is consumed before V is cleared: the host entry
-    // stages q in the V slot)
+    // beta1 u1 = b = [lambda q ; d]   (q is consumed before V is written: the host entry stages q in
+    // the V region)
     PassParams p = base_params(c, nbw, c->tl);
     p.partials = c->partials;
-    p.in = (const float2*)q_dev; p.out = c->U; p.ca = c->coef + C_LAM * NM;
+    p.in = (const float2*)q_dev; p.out = c->U; p.ca = c->coef[0] + C_LAM * NM;
     auto gather_in = [&](float2* dst, const void* src) -> int {      // dst[:, j] = src[:, col0 + j]
         k_gather_cols<<<blocks_for((long long)c->ng * nbw), 256, 0, c->stream>>>(
             dst, (const float2*)src, c->colmap, (long long)c->ng, nbw, nb);
@@ -1214,7 +1282,7 @@ int lsqr_begin_impl(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const
         CK(cudaGetLastError());
         return WRI_OK;
     };
-    if (grouped && c->opts.warm_start && (rc = gather_in(c->X, u_out_dev))) return rc;
+    if (packed && c->opts.warm_start && (rc = gather_in(c->X, u_out_dev))) return rc;
     if (q_dev) {
         if (grouped) {                    // the group's columns of q, compact, in the (still unused) W slot
             if ((rc = gather_in(c->W, q_dev))) return rc;
@@ -1229,24 +1297,31 @@ int lsqr_begin_impl(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const
         // warm start: u_out holds x0; top rows of r0 = b - S x0:  U <- U - lambda A x0  (and its ||.||^2)
         PassParams r = p;
         r.in = c->X; r.out = c->U; r.sgn = 1.f;
-        r.ca = c->coef + C_NLAM * NM; r.cb = c->coef + C_MONE * NM;
+        r.ca = c->coef[0] + C_NLAM * NM; r.cb = c->coef[0] + C_MONE * NM;
         if ((rc = launch_pass<MODE_A>(c, r, c->tl))) return rc;
     }
-    // x0 = 0, w = 0, v = 0.  On the TMA path V is not read by the start's adjoint pass, and in a cold
-    // batch solve of at least one iteration (lazy_start) W and X are not read by the first forward pass,
+    // x0 = 0, w = 0, v = 0.  On the pass kernel V is not read by the start's adjoint pass, and in a cold
+    // batch solve of at least one iteration (lazy) W and X are not read by the first forward pass,
     // which writes them: no clearing needed.  (The stepping entries clear everything: their state can
     // be looked at before the first iteration.)
-    c->wx_zero = lazy_start && c->tma_cb && !c->opts.warm_start && maxit >= 1;
-    if (!c->opts.warm_start && !c->wx_zero) CK(cudaMemsetAsync(c->X, 0, vbytes, c->stream));
-    if (!c->wx_zero) CK(cudaMemsetAsync(c->W, 0, vbytes, c->stream));
-    if (!c->tma_cb) CK(cudaMemsetAsync(c->V, 0, vbytes, c->stream));
-    if ((rc = launch_scalars<PH_INIT_B>(c, (const float2*)d_dev))) return rc;
+    c->lazy = batch && rt && !c->opts.warm_start && maxit >= 1;
+    if (!c->opts.warm_start && !c->lazy) CK(cudaMemsetAsync(c->X, 0, vbytes, c->stream));
+    if (!c->lazy) CK(cudaMemsetAsync(c->W, 0, vbytes, c->stream));
+    if (!rt) CK(cudaMemsetAsync(c->V, 0, vbytes, c->stream));
+    {
+        // receiver rows of b spread over blocks, then beta1 and the first coefficients in one block
+        ScalParams s = scal_params(c, c->partials, (int)c->tl.n_tiles, (const float2*)d_dev);
+        k_init_rows<<<kInitRowBlocks, 256, 256 * sizeof(double), c->stream>>>(s, c->partials, (int)c->tl.n_tiles);
+        c->launches++;
+        CK(cudaGetLastError());
+    }
+    if ((rc = launch_scalars<PH_INIT_B>(c, (const float2*)d_dev, kInitRowBlocks))) return rc;
     // alpha1 v1 = M^H u1
-    if (c->tma_cb) {
-        if ((rc = launch_tma<MODE_A>(c, PH_INIT_A))) return rc;
+    if (rt) {
+        if ((rc = launch_rt<MODE_A>(c, PH_INIT_A))) return rc;
     } else {
         p.in = c->U; p.out = c->V; p.sgn = -1.f;
-        p.ca = c->coef + C_CA_A * NM; p.cb = c->coef + C_CB_A * NM;
+        p.ca = c->coef[0] + C_CA_A * NM; p.cb = c->coef[0] + C_CB_A * NM;
         if ((rc = launch_pass<MODE_A>(c, p, c->tl))) return rc;
         if ((rc = launch_scalars<PH_INIT_A>(c, nullptr))) return rc;
     }
@@ -1254,117 +1329,33 @@ int lsqr_begin_impl(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const
     return WRI_OK;
 }
 
-
-// x and history of the listed working columns become final in the caller's buffers:
-// u_out[:, dst] = X[:, src] + cx[src] W[:, src]; resnorms rows k+1..maxit held at phibar.
-int retire_columns(wri_ctx* c, const std::vector<int>& src, const std::vector<int>& dst) {
-    const int n = (int)src.size();
-    if (!n) return WRI_OK;
-    const size_t NM = c->nb_max;
-    int* d_src = c->idx + NM;
-    int* d_dst = c->idx + 2 * NM;
-    CK(cudaMemcpyAsync(d_src, src.data(), n * sizeof(int), cudaMemcpyHostToDevice, c->stream));
-    CK(cudaMemcpyAsync(d_dst, dst.data(), n * sizeof(int), cudaMemcpyHostToDevice, c->stream));
-    k_retire_cols<<<blocks_for((long long)c->ng * n), 256, 0, c->stream>>>(
-        c->u_out, c->X, c->W, c->coef + C_CX * NM, d_src, d_dst, n, (long long)c->ng, c->nb, c->nb0);
-    c->launches++;
-    CK(cudaGetLastError());
-    if (c->k < c->maxit && c->resnorms) {
-        k_hold_history<<<blocks_for((long long)(c->maxit - c->k) * n), 256, 0, c->stream>>>(
-            c->resnorms, c->stat + S_PHIBAR * NM, d_src, d_dst, n, c->k + 1, c->maxit, c->nb0);
-        c->launches++;
-        CK(cudaGetLastError());
-    }
-    for (int t = 0; t < n; ++t) c->retired[dst[t]] = 1;
-    return WRI_OK;
-}
-
-// working widths the TMA path serves: 2, 4, multiples of 8 up to 64, then multiples of 16
-int round_up16(int n) { return n <= 2 ? 2 : n <= 4 ? 4 : n <= 64 ? (n + 7) / 8 * 8 : (n + 15) / 16 * 16; }
-
-// Re-pack the working set to the columns still active (plus zero padding up to the next supported width).
-int compact_columns(wri_ctx* c, const int* act) {
-    std::vector<int> keep, rs, rd;
-    for (int j = 0; j < c->nb; ++j) {
-        const int so = c->h_colmap[j];
-        if (act[j]) keep.push_back(j);
-        else if (so >= 0 && !c->retired[so]) { rs.push_back(j); rd.push_back(so); }
-    }
-    const int new_nb = round_up16((int)keep.size());
-    if (new_nb >= c->nb) return WRI_OK;
-    int rc = retire_columns(c, rs, rd);
-    if (rc) return rc;
-    std::vector<int> map(new_nb, -1), cm(new_nb, -1);
-    for (size_t i = 0; i < keep.size(); ++i) { map[i] = keep[i]; cm[i] = c->h_colmap[keep[i]]; }
-    const size_t NM = c->nb_max;
-    CK(cudaMemcpyAsync(c->idx, map.data(), new_nb * sizeof(int), cudaMemcpyHostToDevice, c->stream));
-    CK(cudaMemcpyAsync(c->colmap, cm.data(), new_nb * sizeof(int), cudaMemcpyHostToDevice, c->stream));
-    // vectors: gather each into a free slot, then its old slot becomes free (X = u_out is the caller's)
-    float2** vecs[4] = {&c->U, &c->V, &c->W, &c->X};
-    for (int i = 0; i < 4; ++i) {
-        if (c->free_slots.empty()) return WRI_ERR_STATE;
-        float2* dst = c->free_slots.front();
-        c->free_slots.erase(c->free_slots.begin());
-        float2* src = *vecs[i];
-        k_gather_cols<<<blocks_for((long long)c->ng * new_nb), 256, 0, c->stream>>>(
-            dst, src, c->idx, (long long)c->ng, new_nb, c->nb);
-        c->launches++;
-        CK(cudaGetLastError());
-        if (!(i == 3 && !c->packed)) c->free_slots.push_back(src);
-        *vecs[i] = dst;
-    }
-    if (c->n_rec) {
-        k_gather_cols<<<blocks_for((long long)c->n_rec * new_nb), 256, 0, c->stream>>>(
-            c->U_bot_alt, c->U_bot, c->idx, (long long)c->n_rec, new_nb, c->nb);
-        c->launches++;
-        CK(cudaGetLastError());
-        std::swap(c->U_bot, c->U_bot_alt);
-    }
-    k_gather_scalars<<<(new_nb + 127) / 128, 128, 0, c->stream>>>(
-        c->coef_alt, c->coef, c->stat_alt, c->stat, c->active_alt, c->active, c->iters_alt, c->iters,
-        c->idx, new_nb, (int)NM);
-    c->launches++;
-    CK(cudaGetLastError());
-    std::swap(c->coef, c->coef_alt); std::swap(c->stat, c->stat_alt);
-    std::swap(c->active, c->active_alt); std::swap(c->iters, c->iters_alt);
-    c->h_colmap = cm;
-    c->nb = new_nb;
-    c->packed = true;
-    c->tl = make_tiling(c, new_nb);
-    return tma_setup(c);
-}
-
-// host look at the active flags: early exit when every column has stopped, compaction when the
-// active count has dropped below the next supported width
-int check_active(wri_ctx* c) {
-    CK(cudaMemcpyAsync(c->h_active, c->active, c->nb * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
-    CK(cudaStreamSynchronize(c->stream));
-    int n_act = 0;
-    for (int j = 0; j < c->nb; ++j) n_act += c->h_active[j] != 0;
-    if (n_act == 0) { c->all_done = true; return WRI_OK; }
-    if (c->can_compact && round_up16(n_act) < c->nb) return compact_columns(c, c->h_active);
-    return WRI_OK;
-}
-
-// A batch wider than one 64-column chunk per cell is solved as successive 64-column GROUPS, each in a
-// compact working set of its own (columns are independent systems; reading C-9: a
-// column's result does not depend on its batch).  With several chunks per cell a tile row is a 512-byte
-// piece of a wider cell record and the passes reach 0.84-0.88 of the copy bandwidth; compact groups
-// run at the single-chunk rate (0.92).  The stepping entries keep all columns in lock-step.
-int group_width(const wri_ctx* c, int nb) {
-    if (getenv("WRI_NO_GROUPS")) return 0;
-    return (nb > 64 && nb % 64 == 0 && tma_chunk_for(64) == 64 && get_encode_fn()) ? 64 : 0;
-}
-
+// A batch is worked through in groups of at most 64 columns, each in a compact even-width working set
+// of its own inside the workspace; a group that is the whole (even, <= 64 wide) batch works in the
+// caller's own layout.  With several chunks per cell a tile row is a 512-byte piece of a wider cell
+// record and the passes reach 0.84-0.88 of the copy bandwidth; compact groups run at the single-chunk
+// rate.  The stepping entries keep all columns in lock-step.
 int solve_groups(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const void* q_dev, const void* d_dev,
                  float lambda, const float* tol_dev, int32_t maxit, void* u_out_dev, float* resnorms_dev,
                  int32_t* iters_dev, bool host_staged, const int32_t* src_ijk_host, void* alpha_out_dev) {
     int rc = check_batch_args(c, nb);
     if (rc) return rc;
-    const int gw = group_width(c, nb);
-    for (int col0 = 0; col0 < nb; col0 += (gw ? gw : nb)) {
+    // groups need four 64-wide vector slots inside the nb-wide regions of the workspace; a batch that has
+    // no room for them (e.g. 80 or 96 columns without the compaction regions) runs in lock-step
+    bool split = nb > RT_MAXW && !c->dbg.no_groups && rt_chunk_for(c, RT_MAXW) != 0 && c->ws;
+    if (split) {
+        const int flags = host_staged ? WS_HOST_STAGING : 0;
+        const bool ws_big = c->ws_bytes >= ws_layout(c, nb, flags | WS_COMPACTION, kHostMaxitCap).total;
+        const size_t slot = align_up(c->ng * (size_t)RT_MAXW * sizeof(float2), 256);
+        const size_t region = align_up(c->ng * (size_t)even_up(nb) * sizeof(float2), 256);
+        const size_t regions = (ws_big ? 8 : 3) - ((host_staged && q_dev) ? 1 : 0);
+        split = regions * (region / slot) >= 4;
+    }
+    const int gw = split ? RT_MAXW : nb;
+    for (int col0 = 0; col0 < nb; col0 += gw) {
+        const int ncols = std::min(gw, nb - col0);
         if ((rc = lsqr_begin_impl(c, nb, omega_idx_host, q_dev, d_dev, lambda, tol_dev, maxit, u_out_dev,
-                                  resnorms_dev, iters_dev, host_staged, src_ijk_host, alpha_out_dev, col0, gw, true)))
+                                  resnorms_dev, iters_dev, host_staged, src_ijk_host, alpha_out_dev, col0,
+                                  split ? ncols : 0, true)))
             return rc;
         if ((rc = wri_lsqr_iterate(c, maxit))) { c->solving = false; return rc; }
         if ((rc = wri_lsqr_end(c))) return rc;
@@ -1397,31 +1388,36 @@ int wri_lsqr_iterate(wri_ctx* c, int32_t n_steps) {
     if (!c->solving) return WRI_ERR_STATE;
     if (c->k + n_steps > c->maxit) return WRI_ERR_ARG;
     int rc;
-    for (int i = 0; i < n_steps && !c->all_done; ++i) {
+    const size_t NM = c->nb_max;
+    for (int i = 0; i < n_steps; ++i) {
         c->k++;
-        const size_t NM = c->nb_max;
-        if (c->tma_cb) {
-            // two launches per iteration: the last CTA of each pass runs the scalar recurrences
-            if ((rc = launch_tma<MODE_F>(c, PH_F))) return rc;
-            c->wx_zero = false;
-            if ((rc = launch_tma<MODE_A>(c, PH_A))) return rc;
+        if (c->rt) {
+            // two launches per iteration: the last CTA of each pass runs the scalar recurrences.  The
+            // launches read the solve state on the device (width, parity, iteration count) and return at
+            // once when every column has stopped; nothing comes back to the host.
+            if ((rc = launch_rt<MODE_F>(c, PH_F))) return rc;
+            if ((rc = launch_rt<MODE_A>(c, PH_A))) return rc;
+            if (c->adaptive && c->k % kChk == 0 && c->k < c->maxit) {
+                k_compact<<<c->num_sms * 4, 256, 0, c->stream>>>(move_params(c));
+                c->launches++;
+                CK(cudaGetLastError());
+            }
         } else {
             PassParams p = base_params(c, c->nb, c->tl);
             p.partials = c->partials;
             // pass F: U <- (lambda/alpha) A V - (alpha/beta) U ; deferred x, w updates
             p.in = c->V; p.out = c->U; p.W = c->W; p.X = c->X; p.sgn = 1.f;
-            p.ca = c->coef + C_CA_F * NM; p.cb = c->coef + C_CB_F * NM; p.cv = c->coef + C_CV_F * NM;
-            p.cx = c->coef + C_CX * NM; p.cw = c->coef + C_CW * NM;
+            p.ca = c->coef[0] + C_CA_F * NM; p.cb = c->coef[0] + C_CB_F * NM; p.cv = c->coef[0] + C_CV_F * NM;
+            p.cx = c->coef[0] + C_CX * NM; p.cw = c->coef[0] + C_CW * NM;
             if ((rc = launch_pass<MODE_F>(c, p, c->tl, true))) return rc;
             if ((rc = launch_scalars<PH_F>(c, nullptr))) return rc;
             // pass A: V <- (lambda/beta) A^H U - (beta/alpha) V
             p.in = c->U; p.out = c->V; p.W = nullptr; p.X = nullptr; p.sgn = -1.f;
-            p.ca = c->coef + C_CA_A * NM; p.cb = c->coef + C_CB_A * NM;
+            p.ca = c->coef[0] + C_CA_A * NM; p.cb = c->coef[0] + C_CB_A * NM;
             if ((rc = launch_pass<MODE_A>(c, p, c->tl, true))) return rc;
             if ((rc = launch_scalars<PH_A>(c, nullptr))) return rc;
+            if (c->profiling) { c->prof_host[0] += c->nb; c->prof_host[1]++; c->prof_host[2] += c->nb; c->prof_host[3]++; }
         }
-        if (c->check_every && c->k % c->check_every == 0 && c->k < c->maxit)
-            if ((rc = check_active(c))) return rc;
     }
     return WRI_OK;
 }
@@ -1430,23 +1426,21 @@ int wri_lsqr_end(wri_ctx* c) {
     if (!c) return WRI_ERR_ARG;
     if (!c->solving) return WRI_ERR_STATE;
     const size_t NM = c->nb_max;
-    int rc;
-    if (!c->packed && c->k == c->maxit) {
-        // X is the caller's buffer: apply the last deferred update in place
-        const long long n = (long long)c->ng * c->nb;
-        k_flush_x<<<148 * 8, 256, 0, c->stream>>>(c->X, c->W, c->coef + C_CX * NM, n, c->nb);
-        c->launches++;
-        CK(cudaGetLastError());
-    } else {
-        // stopped early and / or compacted: every column not yet final is retired now
-        std::vector<int> rs, rd;
-        for (int j = 0; j < c->nb; ++j) {
-            const int so = c->h_colmap[j];
-            if (so >= 0 && !c->retired[so]) { rs.push_back(j); rd.push_back(so); }
-        }
-        if ((rc = retire_columns(c, rs, rd))) return rc;
+    if (!c->rt) {
+        // host-sequenced solve: the state the closing kernel reads is written now
+        SolveState st;
+        std::memset(&st, 0, sizeof st);
+        st.nb = c->nb; st.k = c->k;
+        CK(cudaMemcpyAsync(c->d_state, &st, sizeof st, cudaMemcpyHostToDevice, c->stream));
     }
-    CK(cudaMemsetAsync(c->coef + C_CX * NM, 0, c->nb * sizeof(float), c->stream));
+    // last deferred update x_k = X + cx W (scattered to the caller's columns where the working set has
+    // a column map); history rows after the last iteration performed are held
+    k_finish<<<c->num_sms * 8, 256, 0, c->stream>>>(move_params(c));
+    c->launches++;
+    CK(cudaGetLastError());
+    k_clear_cx<<<(c->nb_max + 127) / 128, 128, 0, c->stream>>>(c->coef[0] + C_CX * NM, c->coef[1] + C_CX * NM, c->nb_max);
+    c->launches++;
+    CK(cudaGetLastError());
     c->solving = false;
     return WRI_OK;
 }
@@ -1492,7 +1486,7 @@ int lsqr_batch_host_impl(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, 
     float* res = (float*)(c->ws + L.res);
     int* its = (int*)(c->ws + L.its);
     // q is staged in the V slot: the start consumes q before it clears V
-    float2* Qs = q_host ? (float2*)(c->ws + L.V) : nullptr;
+    float2* Qs = q_host ? (float2*)(c->ws + L.vecs[1]) : nullptr;
     float2* As = (float2*)(c->ws + L.alphas);
     if (c->opts.warm_start) {                 // x0 (alpha0) arrive in the output buffers
         CK(cudaMemcpyAsync(Xs, u_out_host, vbytes, cudaMemcpyHostToDevice, c->stream));
@@ -1537,16 +1531,28 @@ int wri_lsqr_peek(const wri_ctx* c, wri_lsqr_view* v) {
     if (!c || !v) return WRI_ERR_ARG;
     if (!c->U) return WRI_ERR_STATE;
     const size_t NM = c->nb_max;
-    v->nb = c->nb; v->k = c->k;
-    v->U_top = c->U; v->U_bot = c->U_bot; v->V = c->V; v->W = c->W; v->X = c->X;
-    v->alpha = c->stat + S_ALPHA * NM; v->beta = c->stat + S_BETA * NM;
-    v->rhobar = c->stat + S_RHOBAR * NM; v->phibar = c->stat + S_PHIBAR * NM;
-    v->ar0 = c->stat + S_AR0 * NM;
-    v->cx = c->coef + C_CX * NM;
-    v->cw = c->coef + C_CW * NM;
-    v->active = c->active; v->iters = c->iters;
+    // the working width, the iteration count and the vector set in use live on the device
+    SolveState st;
+    std::memset(&st, 0, sizeof st);
+    st.nb = c->nb; st.k = c->k;
+    if (c->rt) {
+        CK(cudaStreamSynchronize(c->stream));
+        CK(cudaMemcpy(&st, c->d_state, sizeof st, cudaMemcpyDeviceToHost));
+    }
+    const int par = st.parity & 1;
+    v->nb = st.nb; v->k = st.k;
+    v->U_top = c->vec[par][0]; v->U_bot = c->U_bot[par]; v->V = c->vec[par][1]; v->W = c->vec[par][2];
+    v->X = c->vec[par][3];
+    const double* stat = c->stat[par];
+    const float* coef = c->coef[par];
+    v->alpha = stat + S_ALPHA * NM; v->beta = stat + S_BETA * NM;
+    v->rhobar = stat + S_RHOBAR * NM; v->phibar = stat + S_PHIBAR * NM;
+    v->ar0 = stat + S_AR0 * NM;
+    v->cx = coef + C_CX * NM;
+    v->cw = coef + C_CW * NM;
+    v->active = c->active[par]; v->iters = c->iters[par];
     v->nb_max = c->nb_max;
-    v->sf_state = c->sf ? c->stat + S_VA_RE * NM : nullptr;
+    v->sf_state = c->sf ? stat + S_VA_RE * NM : nullptr;
     return WRI_OK;
 }
 
@@ -1764,6 +1770,9 @@ int wri_awri_step(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const i
         if ((rc = misfit_impl(c, nb, omega_idx_host, src_ijk_host, d_dev, lambda, eps, maxit, warm, u_dev,
                               alpha_dev, c->aw_ar0, f_pde, f_data, g_dev, nullptr, &f, &it0)))
             return leave(rc);
+        // eq. 8-9 are sums over every rank's columns: the caller's collective adds the objective and the
+        // gradient, so that all ranks hold the same f, g and take the same decision below
+        if (o->reduce && o->reduce(o->user, &f, g_dev, (int64_t)c->ng, (void*)c->stream) != 0) return leave(WRI_ERR_ARG);
         // line 6: the trial model
         if (o->update) {
             if (o->update(o->user, m_dev, g_dev, m_trial_dev, (void*)c->stream) != 0) return leave(WRI_ERR_ARG);
@@ -1780,11 +1789,15 @@ int wri_awri_step(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const i
                               &f_trial, &it1)))
             return leave(rc);
         c->m = m_dev;
+        if (o->reduce && o->reduce(o->user, &f_trial, nullptr, 0, (void*)c->stream) != 0) return leave(WRI_ERR_ARG);
         rep->trace_eps[h] = eps; rep->trace_f[h] = f; rep->trace_f_trial[h] = f_trial;
         rep->n_trace = h + 1;
         rep->f = f; rep->f_trial = f_trial; rep->eps = eps; rep->n_halvings = h;
         rep->lsqr_iters += it0 + it1;
-        if (!(f_trial > f)) {                               // line 9 / 12-13
+        // the objective at the current model must be a number; a trial objective that is not
+        // (an update that produced a non-physical model) counts as a rejected step
+        if (!std::isfinite(f)) return leave(WRI_ERR_NUMERIC);
+        if (std::isfinite(f_trial) && f_trial <= f) {       // line 9 / 12-13
             CK(cudaMemcpyAsync(m_dev, m_trial_dev, c->ng * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
             rep->accepted = 1;
             break;

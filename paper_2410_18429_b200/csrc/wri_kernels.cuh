@@ -28,6 +28,44 @@ enum Coef { C_CA_F = 0, C_CB_F, C_CV_F, C_CX, C_CW, C_CA_A, C_CB_A, C_CT_A, C_W2
 enum Stat { S_ALPHA = 0, S_BETA, S_RHOBAR, S_PHIBAR, S_AR0,
             S_VA_RE, S_VA_IM, S_WA_RE, S_WA_IM, S_XA_RE, S_XA_IM, N_STAT };
 
+// ---------------------------------------------------------------------------------------------
+// Persistent pass kernel (wri_pass.cuh): tile plan per working width and the device-resident state
+// of the solve in flight.
+constexpr int RT_NT = 512;            // consumer threads (one 16-byte item each)
+constexpr int RT_MAXW = 64;           // widest column chunk (and widest working set that can be compacted)
+constexpr int RT_MAX_STAGES = 12;
+constexpr int RT_SMEM_MAX = 232448 - 1024;  // 227 KB of shared memory per CTA, less the static part
+constexpr int RT_MIN_STAGE_AREA = 20480;   // the CTA epilogue re-uses the (idle) stages as scratch
+
+enum StencilKind { ST_7 = 0, ST_27 = 1 };
+enum MapSlot { MP_V_HALO = 0, MP_U_CTR, MP_W_CTR, MP_X_CTR, MP_U_HALO, MP_V_CTR, N_MAPS };
+
+struct PassGeo {          // per pass: planes per tile, tile count, ring depth
+    int zc, ntz, n_tiles, nstage;
+};
+
+struct DevPlan {          // tile geometry of one working width
+    int nb, cb, hp, nchunk;           // batch width, column chunk, column pairs per chunk, chunks per cell
+    int txc, tyc, items;              // cells per tile (x, y); consumer threads with work = txc*tyc*hp
+    int ntx, nty;
+    int merged, m_tma;                // tensor maps fold (column, x); the model tile rides in the stage
+    int row_b, cell_b;                // bytes per row / per cell of the halo box in shared memory
+    int in_bytes, in_span;            // halo box: bytes delivered, room taken (128 B granules)
+    int ctr_bytes, ctr_span;          // centre box
+    int m_bytes, m_span;              // model tile (float per cell)
+    PassGeo f, a;
+};
+
+struct SolveState {       // device-resident state of the solve in flight
+    int widx, nb, k, n_active;
+    int all_done, parity, pending, pending_widx;
+    int n_keep, n_ret, pad0, pad1;
+    long long waste;                  // stale column-iterations since the last compaction
+    int map[RT_MAXW];                 // pending compaction: new column j <- old column map[j] (-1 = padding)
+    int ret_src[RT_MAXW], ret_dst[RT_MAXW];   // columns leaving: working column -> caller's column
+    int colmap[2][RT_MAXW];           // per parity: working column -> caller's column (-1 = padding)
+};
+
 struct PassParams {
     const float2* in;      // stencil input [n_g][nb]
     float2* out;           // result; also the "old" vector of the axpy (in place)
@@ -47,7 +85,8 @@ struct PassParams {
     int nx, ny, nz, nb;
     int zc;                // planes per tile
     float ih2;             // 1/h^2
-    float m6ih2;           // -6/h^2
+    float m6ih2;           // centre weight a0/h^2 (-6/h^2 for the 7-point stencil)
+    float a1, a2, a3;      // 27-point stencil: weights of the face / edge / corner neighbours (units of 1/h^2)
     float sgn;             // +1: A, -1: A^H (conjugated diagonal)
 };
 
@@ -106,7 +145,42 @@ __device__ __forceinline__ void block_column_sums(const double (&acc)[VEC], int 
     }
 }
 
-template <int VEC, int MODE>
+
+// 27-point stencil (generic kernels): weighted sum of the 26 neighbours of one cell for VEC columns,
+// a1 * faces + a2 * edges + a3 * corners, zero outside the grid.  Plain loads through L1/L2 — the
+// generic kernels are the fallback path; the persistent pass kernel keeps the planes in registers.
+template <int VEC>
+__device__ __forceinline__ void nbr27(const float2* __restrict__ in, size_t off, int nb, int RL, size_t plane,
+                                      int ix, int iy, int iz, int nx, int ny, int nz, float a1, float a2, float a3,
+                                      float (&sr)[VEC], float (&si)[VEC]) {
+    float cr[3][VEC], ci[3][VEC];
+#pragma unroll
+    for (int q = 0; q < 3; ++q)
+#pragma unroll
+        for (int k = 0; k < VEC; ++k) cr[q][k] = ci[q][k] = 0.f;
+    for (int dz = -1; dz <= 1; ++dz) {
+        if (iz + dz < 0 || iz + dz >= nz) continue;
+        for (int dy = -1; dy <= 1; ++dy) {
+            if (iy + dy < 0 || iy + dy >= ny) continue;
+            for (int dx = -1; dx <= 1; ++dx) {
+                if (ix + dx < 0 || ix + dx >= nx) continue;
+                const int cls = (dx != 0) + (dy != 0) + (dz != 0);
+                if (cls == 0) continue;
+                const long long o = (long long)off + dz * (long long)plane + dy * (long long)RL + dx * (long long)nb;
+                const CV<VEC> v = ldg_ro<VEC>(in + o);
+#pragma unroll
+                for (int k = 0; k < VEC; ++k) { cr[cls - 1][k] += v.a[k].x; ci[cls - 1][k] += v.a[k].y; }
+            }
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < VEC; ++k) {
+        sr[k] = fmaf(a1, cr[0][k], fmaf(a2, cr[1][k], a3 * cr[2][k]));
+        si[k] = fmaf(a1, ci[0][k], fmaf(a2, ci[1][k], a3 * ci[2][k]));
+    }
+}
+
+template <int VEC, int MODE, int STENCIL>
 __global__ void __launch_bounds__(256)
 k_pass(const PassParams p) {
     const int nb = p.nb;
@@ -153,10 +227,15 @@ k_pass(const PassParams p) {
             CV<VEC> r;
             if (MODE != MODE_INIT) {
                 CV<VEC> xm = zero_v<VEC>(), xp = zero_v<VEC>(), ym = zero_v<VEC>(), yp = zero_v<VEC>();
-                if (has_xm) xm = ldg_ro<VEC>(p.in + off - nb);
-                if (has_xp) xp = ldg_ro<VEC>(p.in + off + nb);
-                if (has_ym) ym = ldg_ro<VEC>(p.in + off - RL);
-                if (has_yp) yp = ldg_ro<VEC>(p.in + off + RL);
+                float s27r[VEC], s27i[VEC];
+                if (STENCIL == ST_27) {
+                    nbr27<VEC>(p.in, off, nb, RL, plane, ix, iy, z, p.nx, p.ny, p.nz, p.a1, p.a2, p.a3, s27r, s27i);
+                } else {
+                    if (has_xm) xm = ldg_ro<VEC>(p.in + off - nb);
+                    if (has_xp) xp = ldg_ro<VEC>(p.in + off + nb);
+                    if (has_ym) ym = ldg_ro<VEC>(p.in + off - RL);
+                    if (has_yp) yp = ldg_ro<VEC>(p.in + off + RL);
+                }
                 CV<VEC> old, wv, xv;
                 if (MODE == MODE_A || MODE == MODE_F) old = ld_rw<VEC>(p.out + off);
                 if (MODE == MODE_F) { wv = ld_rw<VEC>(p.W + off); xv = ld_rw<VEC>(p.X + off); }
@@ -167,8 +246,10 @@ k_pass(const PassParams p) {
                     const float wm = w2[k] * mc;
                     const float dr = wm + p.m6ih2;          // Re diag = -6/h^2 + w^2 m
                     const float di = p.sgn * wm * g;        // Im diag = +-w^2 m gamma
-                    const float sr = ((xm.a[k].x + xp.a[k].x) + (ym.a[k].x + yp.a[k].x)) + (prev.a[k].x + nxt.a[k].x);
-                    const float si = ((xm.a[k].y + xp.a[k].y) + (ym.a[k].y + yp.a[k].y)) + (prev.a[k].y + nxt.a[k].y);
+                    const float sr = (STENCIL == ST_27) ? s27r[k]
+                        : ((xm.a[k].x + xp.a[k].x) + (ym.a[k].x + yp.a[k].x)) + (prev.a[k].x + nxt.a[k].x);
+                    const float si = (STENCIL == ST_27) ? s27i[k]
+                        : ((xm.a[k].y + xp.a[k].y) + (ym.a[k].y + yp.a[k].y)) + (prev.a[k].y + nxt.a[k].y);
                     float ar = fmaf(p.ih2, sr, fmaf(dr, cur.a[k].x, -di * cur.a[k].y));
                     float ai = fmaf(p.ih2, si, fmaf(dr, cur.a[k].y, di * cur.a[k].x));
                     if (MODE == MODE_A || MODE == MODE_F) {
@@ -259,22 +340,6 @@ __global__ void k_src_adjoint(const float2* __restrict__ ytop, const int* __rest
     }
 }
 
-// X += cx * W over the whole batch (last deferred update, wri_lsqr_end)
-__global__ void k_flush_x(float2* __restrict__ X, const float2* __restrict__ W,
-                          const float* __restrict__ cx, long long n, int nb) {
-    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
-         i += (long long)gridDim.x * blockDim.x) {
-        const float c = cx[(int)(i % nb)];
-        if (c != 0.f) {
-            const float2 w = W[i];
-            float2 x = X[i];
-            x.x = fmaf(c, w.x, x.x);
-            x.y = fmaf(c, w.y, x.y);
-            X[i] = x;
-        }
-    }
-}
-
 // ---------------------------------------------------------------------------------------------
 // Per-column scalar recurrences + receiver rows, one block.  Phases:
 enum ScalPhase { PH_INIT_B = 0, PH_INIT_A = 1, PH_F = 2, PH_A = 3 };
@@ -312,6 +377,14 @@ struct ScalParams {
     const double* ar_ref;     // [nb] or null: arnorm_k <= tol * ar_ref instead of tol * alpha1 beta1
     double* ar0_out;          // [nb] or null: alpha1 beta1 of this solve
     const unsigned char* rmask;   // [n_rec][nb_out] per-source receiver sets by the CALLER's column, or null
+    // device-resident solve state (persistent pass kernel): iteration counter, active count, the
+    // decision to re-pack the working set (PH_A), the condition of the device-side loop
+    SolveState* st;           // null: host-sequenced solve (generic kernels)
+    int adaptive;             // PH_A may ask for a compaction
+    int chk;                  // ... after iterations k % chk == 0 (when the compaction kernel is enqueued)
+    int widx;                 // index of the current width's plan
+    int init_rows;            // PH_INIT_B: k_init_rows has formed U_bot; its |.|^2 sums are extra rows of partials
+    void* cond;               // cudaGraphConditionalHandle or null
 };
 
 // sum over tiles of partials[.][s] in fixed order; result for column s in colsum[s] (shared)
@@ -381,7 +454,7 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
     double* st = p.stat;
 
     const long long nrs = (long long)p.n_rec * nb;
-    if (PHASE == PH_INIT_B) {
+    if (PHASE == PH_INIT_B && !p.init_rows) {
         // U_bot = d (exact copy), then beta1 = ||[lambda q ; d]||
         // (d is the CALLER's [n_rec][nb_out] array: a grouped solve works on a subset of its columns)
         for (long long i = threadIdx.x; i < nrs; i += blockDim.x) {
@@ -412,7 +485,7 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
         __syncthreads();
     }
     reduce_partials(p, scratch, colsum);
-    if (PHASE == PH_INIT_B || (PHASE == PH_F && !p.rows_in_pass)) add_receiver_norms(p, scratch, colsum);
+    if ((PHASE == PH_INIT_B && !p.init_rows) || (PHASE == PH_F && !p.rows_in_pass)) add_receiver_norms(p, scratch, colsum);
 
     for (int s = threadIdx.x; s < nb; s += blockDim.x) {
         const int so = p.colmap ? p.colmap[s] : s;           // caller's column of working column s
@@ -556,6 +629,43 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
     }
     __syncthreads();
 
+    if (PHASE == PH_A && p.st && threadIdx.x == 0) {
+        // device-resident solve state: iteration count, live columns, and — with adaptive accuracy —
+        // the decision to re-pack the working set.  Ski-rental rule: re-pack once the bandwidth spent
+        // on stopped columns since the last re-packing (80 B per cell, column and iteration) exceeds
+        // what the re-packing moves (4 vectors read at the old width, written at the new: 32 B per
+        // cell and column of either), provided the iterations left can pay it back.
+        SolveState* st = p.st;
+        int n_act = 0;
+        for (int s = 0; s < nb; ++s) n_act += p.active[s] != 0;
+        st->k = p.k;
+        st->n_active = n_act;
+        if (n_act == 0) st->all_done = 1;
+        else if (p.adaptive) {
+            const long long waste = st->waste + (nb - n_act);
+            st->waste = waste;
+            const int w_new = max(2, (n_act + 1) & ~1);
+            const long long cost = 32LL * (nb + w_new);
+            if (w_new < nb && (p.k % p.chk) == 0 && p.k < p.maxit && waste * 80 >= cost &&
+                (long long)(nb - w_new) * 80 * (p.maxit - p.k) > cost) {
+                int nk = 0, nr = 0;
+                for (int s = 0; s < nb; ++s) {
+                    if (p.active[s]) st->map[nk++] = s;
+                    else if (p.colmap[s] >= 0) { st->ret_src[nr] = s; st->ret_dst[nr] = p.colmap[s]; ++nr; }
+                }
+                for (int j = nk; j < w_new; ++j) st->map[j] = -1;
+                st->n_keep = nk; st->n_ret = nr;
+                st->pending_widx = p.widx + (nb - w_new) / 2;
+                st->pending = 1;
+            }
+        }
+#if defined(__CUDACC__)
+        if (p.cond)
+            cudaGraphSetConditional((cudaGraphConditionalHandle)(uintptr_t)p.cond,
+                                    (st->all_done || p.k >= p.maxit) ? 0u : 1u);
+#endif
+    }
+
     if ((PHASE == PH_INIT_B || PHASE == PH_F) && !p.rows_in_pass) {
         // fold P^T into the coming adjoint pass:  V <- ca A^H U - cb (V - (ct/cb) P^T U_bot)
         for (long long i = threadIdx.x; i < nrs; i += blockDim.x) {
@@ -591,53 +701,205 @@ __global__ void k_gather_cols(float2* __restrict__ dst, const float2* __restrict
     }
 }
 
-// Retire columns: u_out[c][dst_col[t]] = X[c][src_col[t]] + cx[src_col[t]] * W[c][src_col[t]]
-// (the column's last deferred x update), t < n_ret.  X may be u_out itself (same column).
-__global__ void k_retire_cols(float2* u_out, const float2* X, const float2* __restrict__ W,
-                              const float* __restrict__ cx, const int* __restrict__ src_col,
-                              const int* __restrict__ dst_col, int n_ret, long long n_rows, int nb_src,
-                              int nb_out) {
-    const long long n = n_rows * n_ret;
-    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
-         i += (long long)gridDim.x * blockDim.x) {
+// Arguments shared by the kernels that move a solve's state around on the device.
+struct MoveParams {
+    SolveState* st;
+    const DevPlan* plans;
+    float2* vec[2][4];        // per parity: U, V, W, X
+    float2* U_bot[2];
+    float* coef[2];
+    double* stat[2];
+    int* active[2];
+    int* iters[2];
+    float2* u_out;            // caller's [n_g][nb_out]
+    float* resnorms;          // caller's [maxit+1][nb_out] or null
+    long long n_g;
+    int nb_out, nb_max, maxit, n_rec;
+    int packed;
+    unsigned int* counter;    // last-block ticket (zero on entry, reset on exit)
+};
+
+// Re-pack the working set (device-driven, decided by the finaliser of pass A): columns that have
+// stopped leave — their x = X + cx W goes to the caller's u_out, their residual history is held at
+// the stop value (reading C-9) — and the live ones are gathered, in order, into the vector set of
+// the other parity at the narrower width.  The last block to finish switches the state over.
+// Every launch is a no-op unless a compaction is pending.
+__global__ void __launch_bounds__(256)
+k_compact(const MoveParams p) {
+    SolveState* st = p.st;
+    if (st->all_done || !st->pending) return;
+    __shared__ int s_map[RT_MAXW], s_rs[RT_MAXW], s_rd[RT_MAXW];
+    __shared__ float s_cx[RT_MAXW];
+    __shared__ unsigned int s_ticket;
+    const int a = st->parity, b = a ^ 1;
+    const int nbo = st->nb, nbn = p.plans[st->pending_widx].nb, n_ret = st->n_ret, k = st->k;
+    const size_t NM = p.nb_max;
+    if (threadIdx.x < RT_MAXW) {
+        s_map[threadIdx.x] = st->map[threadIdx.x];
+        s_rs[threadIdx.x] = st->ret_src[threadIdx.x];
+        s_rd[threadIdx.x] = st->ret_dst[threadIdx.x];
+        s_cx[threadIdx.x] = threadIdx.x < nbo ? p.coef[a][C_CX * NM + threadIdx.x] : 0.f;
+    }
+    __syncthreads();
+    const long long gs = (long long)gridDim.x * blockDim.x, g0 = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    // live columns of U, V, W, X
+    for (long long i = g0; i < p.n_g * nbn; i += gs) {
+        const long long c = i / nbn;
+        const int m = s_map[(int)(i - c * nbn)];
+        float2 v[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) v[q] = m >= 0 ? __ldcs(p.vec[a][q] + c * nbo + m) : make_float2(0.f, 0.f);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) p.vec[b][q][i] = v[q];
+    }
+    // columns that leave: final x into the caller's buffer
+    for (long long i = g0; i < p.n_g * n_ret; i += gs) {
         const long long c = i / n_ret;
-        const int t = (int)(i - c * n_ret);
-        const int js = src_col[t];
-        const float a = cx[js];
-        float2 x = X[c * nb_src + js];
-        if (a != 0.f) {
-            const float2 w = W[c * nb_src + js];
-            x.x = fmaf(a, w.x, x.x);
-            x.y = fmaf(a, w.y, x.y);
+        const int t = (int)(i - c * n_ret), js = s_rs[t];
+        float2 x = __ldcs(p.vec[a][3] + c * nbo + js);
+        const float cx = s_cx[js];
+        if (cx != 0.f) {
+            const float2 w = __ldcs(p.vec[a][2] + c * nbo + js);
+            x.x = fmaf(cx, w.x, x.x);
+            x.y = fmaf(cx, w.y, x.y);
         }
-        u_out[c * nb_out + dst_col[t]] = x;
+        p.u_out[c * p.nb_out + s_rd[t]] = x;
+    }
+    // ... and their residual history, held at the stop value
+    if (p.resnorms)
+        for (long long i = g0; i < (long long)(p.maxit - k) * n_ret; i += gs) {
+            const int row = (int)(i / n_ret), t = (int)(i - (long long)row * n_ret);
+            p.resnorms[(size_t)(k + 1 + row) * p.nb_out + s_rd[t]] = (float)p.stat[a][S_PHIBAR * NM + s_rs[t]];
+        }
+    // receiver rows and the per-column scalars follow their columns
+    for (long long i = g0; i < (long long)p.n_rec * nbn; i += gs) {
+        const long long r = i / nbn;
+        const int m = s_map[(int)(i - r * nbn)];
+        p.U_bot[b][i] = m >= 0 ? p.U_bot[a][r * nbo + m] : make_float2(0.f, 0.f);
+    }
+    if (blockIdx.x == 0)
+        for (int j = threadIdx.x; j < nbn; j += blockDim.x) {
+            const int m = s_map[j];
+            for (int r = 0; r < N_COEF; ++r) p.coef[b][r * NM + j] = m >= 0 ? p.coef[a][r * NM + m] : 0.f;
+            for (int r = 0; r < N_STAT; ++r) p.stat[b][r * NM + j] = m >= 0 ? p.stat[a][r * NM + m] : 0.0;
+            p.active[b][j] = m >= 0 ? p.active[a][m] : 0;
+            p.iters[b][j] = m >= 0 ? p.iters[a][m] : 0;
+        }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_ticket = atomicAdd(p.counter, 1u);
+    __syncthreads();
+    if (s_ticket == gridDim.x - 1) {
+        __threadfence();
+        for (int j = threadIdx.x; j < RT_MAXW; j += blockDim.x)
+            st->colmap[b][j] = (j < nbn && s_map[j] >= 0) ? st->colmap[a][s_map[j]] : -1;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            st->parity = b;
+            st->widx = st->pending_widx;
+            st->nb = nbn;
+            st->waste = 0;
+            st->pending = 0;
+            *p.counter = 0u;
+        }
     }
 }
 
-// history of retired columns is held at the stop value (reading C-9): rows k0..maxit
-__global__ void k_hold_history(float* __restrict__ resnorms, const double* __restrict__ phibar,
-                               const int* __restrict__ src_col, const int* __restrict__ dst_col, int n_ret,
-                               int k0, int maxit, int nb_out) {
-    const long long n = (long long)(maxit - k0 + 1) * n_ret;
-    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
-         i += (long long)gridDim.x * blockDim.x) {
-        const int row = (int)(i / n_ret), t = (int)(i - (long long)row * n_ret);
-        resnorms[(size_t)(k0 + row) * nb_out + dst_col[t]] = (float)phibar[src_col[t]];
+// End of a solve: the last deferred update x_k = X + cx W is applied and, where the working set has
+// a column map (grouped / adaptive solves: X lives in the workspace), scattered to the caller's
+// u_out; the residual history of the rows after the last iteration performed is held (reading C-9).
+__global__ void __launch_bounds__(256)
+k_finish(const MoveParams p) {
+    const SolveState* st = p.st;
+    __shared__ int s_cm[RT_MAXW];
+    __shared__ float s_cx[RT_MAXW];
+    const int a = st->parity, nb = st->nb, k = st->k;
+    const size_t NM = p.nb_max;
+    const float* cxr = p.coef[a] + C_CX * NM;
+    const long long gs = (long long)gridDim.x * blockDim.x, g0 = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (p.packed) {
+        if (threadIdx.x < RT_MAXW) {
+            s_cm[threadIdx.x] = st->colmap[a][threadIdx.x];
+            s_cx[threadIdx.x] = threadIdx.x < nb ? cxr[threadIdx.x] : 0.f;
+        }
+        __syncthreads();
+        const float2* X = p.vec[a][3];
+        const float2* W = p.vec[a][2];
+        for (long long i = g0; i < p.n_g * nb; i += gs) {
+            const long long c = i / nb;
+            const int j = (int)(i - c * nb), so = s_cm[j];
+            if (so < 0) continue;
+            float2 x = __ldcs(X + i);
+            const float cx = s_cx[j];
+            if (cx != 0.f) {
+                const float2 w = __ldcs(W + i);
+                x.x = fmaf(cx, w.x, x.x);
+                x.y = fmaf(cx, w.y, x.y);
+            }
+            p.u_out[c * p.nb_out + so] = x;
+        }
+    } else {
+        float2* X = p.vec[a][3];                                 // = u_out, same layout
+        const float2* W = p.vec[a][2];
+        for (long long i = g0; i < p.n_g * nb; i += gs) {
+            const float cx = cxr[(int)(i % nb)];
+            if (cx != 0.f) {
+                const float2 w = __ldcs(W + i);
+                float2 x = X[i];
+                x.x = fmaf(cx, w.x, x.x);
+                x.y = fmaf(cx, w.y, x.y);
+                X[i] = x;
+            }
+        }
     }
+    if (p.resnorms)
+        for (long long i = g0; i < (long long)(p.maxit - k) * nb; i += gs) {
+            const int row = (int)(i / nb), j = (int)(i - (long long)row * nb);
+            const int so = p.packed ? st->colmap[a][j] : j;
+            if (so >= 0) p.resnorms[(size_t)(k + 1 + row) * p.nb_out + so] = (float)p.stat[a][S_PHIBAR * NM + j];
+        }
 }
 
-// per-column scalar rows follow the vectors: dst bank <- src bank through map (padding -> 0 / inactive)
-__global__ void k_gather_scalars(float* __restrict__ coef_dst, const float* __restrict__ coef_src,
-                                 double* __restrict__ stat_dst, const double* __restrict__ stat_src,
-                                 int* __restrict__ act_dst, const int* __restrict__ act_src,
-                                 int* __restrict__ it_dst, const int* __restrict__ it_src,
-                                 const int* __restrict__ map, int nb_dst, int nb_max) {
-    for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < nb_dst; j += gridDim.x * blockDim.x) {
-        const int m = map[j];
-        for (int r = 0; r < N_COEF; ++r) coef_dst[r * nb_max + j] = m >= 0 ? coef_src[r * nb_max + m] : 0.f;
-        for (int r = 0; r < N_STAT; ++r) stat_dst[r * nb_max + j] = m >= 0 ? stat_src[r * nb_max + m] : 0.0;
-        act_dst[j] = m >= 0 ? act_src[m] : 0;
-        it_dst[j] = m >= 0 ? it_src[m] : 0;
+// the pending x-update coefficients are spent once k_finish has run
+__global__ void k_clear_cx(float* cx0, float* cx1, int n) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j < n) { cx0[j] = 0.f; cx1[j] = 0.f; }
+}
+
+// Golub-Kahan start, receiver rows of b = [lambda q ; d] spread over the blocks:  U_bot = d (exact
+// copy; warm start: d - x0 at the receiver nodes; masked rows of per-source receiver sets = 0) and
+// per-block column sums of |U_bot|^2 into rows n_rows0 + blockIdx.x of partials.  blockDim.x is a
+// any size; thread (i, s): rows blockIdx.x + (i + j*rpb) * gridDim.x, column s.
+__global__ void __launch_bounds__(256)
+k_init_rows(const ScalParams p, double* __restrict__ partials, int n_rows0) {
+    extern __shared__ double sh_rows[];                      // [blockDim.x]
+    const int nb = p.nb, T = blockDim.x;
+    for (int base = 0; base < nb; base += T) {
+        const int ncol = min(nb - base, T);
+        const int rpb = T / ncol;                            // rows in flight per block
+        const int i = threadIdx.x / ncol, s = base + threadIdx.x % ncol;
+        double a = 0.0;
+        if (i < rpb) {
+            const int so = p.colmap ? p.colmap[s] : s;
+            for (int r = blockIdx.x + i * gridDim.x; r < p.n_rec; r += rpb * gridDim.x) {
+                float2 dv = so >= 0 ? p.d[(size_t)r * p.nb_out + so] : make_float2(0.f, 0.f);
+                if (p.warm) {
+                    const float2 xv = p.X[(size_t)p.rec[r] * nb + s];
+                    dv = make_float2(dv.x - xv.x, dv.y - xv.y);
+                }
+                if (p.rmask && so >= 0 && !p.rmask[(size_t)r * p.nb_out + so]) dv = make_float2(0.f, 0.f);
+                p.U_bot[(size_t)r * nb + s] = dv;
+                a += (double)fmaf(dv.x, dv.x, dv.y * dv.y);
+            }
+        }
+        sh_rows[threadIdx.x] = a;
+        __syncthreads();
+        if (threadIdx.x < ncol) {
+            double t = 0.0;
+            for (int g = 0; g < rpb; ++g) t += sh_rows[g * ncol + threadIdx.x];
+            partials[(size_t)(n_rows0 + blockIdx.x) * nb + base + threadIdx.x] = t;
+        }
+        __syncthreads();
     }
 }
 
@@ -665,9 +927,10 @@ struct GradParams {
     int tpc;               // threads per cell
     int shuffle;           // 1: tpc is a power of two <= 32
     float ih2, m6ih2, lam2;
+    float a1, a2, a3;      // 27-point stencil weights (see PassParams)
 };
 
-template <int VEC>
+template <int VEC, int STENCIL>
 __global__ void __launch_bounds__(512)
 k_grad(const GradParams p) {
     extern __shared__ double red[];                          // block_column_sums scratch; reused per plane
@@ -715,10 +978,15 @@ k_grad(const GradParams p) {
             nxt = zero_v<VEC>();
             if (z + 1 < p.nz) nxt = ldg_ro<VEC>(p.u + off + plane);
             CV<VEC> xm = zero_v<VEC>(), xp = zero_v<VEC>(), ym = zero_v<VEC>(), yp = zero_v<VEC>();
-            if (has_xm) xm = ldg_ro<VEC>(p.u + off - nb);
-            if (has_xp) xp = ldg_ro<VEC>(p.u + off + nb);
-            if (has_ym) ym = ldg_ro<VEC>(p.u + off - RL);
-            if (has_yp) yp = ldg_ro<VEC>(p.u + off + RL);
+            float s27r[VEC], s27i[VEC];
+            if (STENCIL == ST_27) {
+                nbr27<VEC>(p.u, off, nb, RL, plane, ix, iy, z, p.nx, p.ny, p.nz, p.a1, p.a2, p.a3, s27r, s27i);
+            } else {
+                if (has_xm) xm = ldg_ro<VEC>(p.u + off - nb);
+                if (has_xp) xp = ldg_ro<VEC>(p.u + off + nb);
+                if (has_ym) ym = ldg_ro<VEC>(p.u + off - RL);
+                if (has_yp) yp = ldg_ro<VEC>(p.u + off + RL);
+            }
             CV<VEC> qv = zero_v<VEC>();
             if (p.q) qv = ld_rw<VEC>(p.q + off);
             const float mc = __ldg(p.m + cell);
@@ -727,8 +995,10 @@ k_grad(const GradParams p) {
             for (int k = 0; k < VEC; ++k) {
                 const float wm = w2[k] * mc;
                 const float dr = wm + p.m6ih2, di = wm * gam;
-                const float sr = ((xm.a[k].x + xp.a[k].x) + (ym.a[k].x + yp.a[k].x)) + (prev.a[k].x + nxt.a[k].x);
-                const float si = ((xm.a[k].y + xp.a[k].y) + (ym.a[k].y + yp.a[k].y)) + (prev.a[k].y + nxt.a[k].y);
+                const float sr = (STENCIL == ST_27) ? s27r[k]
+                    : ((xm.a[k].x + xp.a[k].x) + (ym.a[k].x + yp.a[k].x)) + (prev.a[k].x + nxt.a[k].x);
+                const float si = (STENCIL == ST_27) ? s27i[k]
+                    : ((xm.a[k].y + xp.a[k].y) + (ym.a[k].y + yp.a[k].y)) + (prev.a[k].y + nxt.a[k].y);
                 float rr = fmaf(p.ih2, sr, fmaf(dr, cur.a[k].x, -di * cur.a[k].y)) - qv.a[k].x;
                 float ri = fmaf(p.ih2, si, fmaf(dr, cur.a[k].y, di * cur.a[k].x)) - qv.a[k].y;
                 if ((int)cell == srcc[k]) { rr -= al[k].x; ri -= al[k].y; }

@@ -61,42 +61,36 @@ class ShardedMisfit:
             f_loc, it_loc = float(s[0]), int(round(float(s[1])))
         return float(f_loc), g, int(it_loc), state
 
-    def awri_step(self, m, eps, maxit, update, set_model, max_halvings=8, warm_restart=False):
-        """Lines 4-14 of Algorithm 2 with the sums of lines 5 and 8 taken over all ranks.
+    def reduce(self, f, g=None):
+        """Sum over ranks of an objective value and, in place, of a gradient tensor: the `reduce`
+        argument of Wri.awri_step (wri_awri_opts.reduce).  Returns the summed objective."""
+        if not self.dist:
+            return float(f)
+        t = self._t
+        s = t.tensor([float(f)], dtype=t.float64, device=self.g.device)
+        self.dist.all_reduce(s, op=self.dist.ReduceOp.SUM)
+        if g is not None:
+            self.dist.all_reduce(g, op=self.dist.ReduceOp.SUM)
+        return float(s[0])
 
-        m: this rank's replica of the model (a tensor, updated in place when the step is accepted);
-        update(m, g, m_trial) fills m_trial; set_model(tensor) points the rank's solver at a model.
-        Every rank computes the same f, f_trial and therefore the same decision.  Returns a dict
-        like Wri.awri_step (accepted, n_halvings, eps, f, f_trial, lsqr_iters, trace)."""
-        m_trial = m.clone()
-        trace, total, state = [], 0, None
-        accepted = False
-        f = ft = 0.0
-        h = 0
-        for h in range(int(max_halvings) + 1):
-            set_model(m)
-            f, g, it0, state = self.misfit(eps, maxit, True, state if (warm_restart and h > 0) else None)
-            update(m, g, m_trial)
-            set_model(m_trial)
-            ft, _, it1, _ = self.misfit(eps, maxit, False, None)
-            set_model(m)
-            total += it0 + it1
-            trace.append((eps, f, ft))
-            if not (ft > f):
-                m.copy_(m_trial)
-                accepted = True
-                break
-            if h == max_halvings:
-                break
-            eps *= 0.5
-        return dict(accepted=accepted, n_halvings=h, eps=eps, f=f, f_trial=ft, lsqr_iters=total, trace=trace)
+    def awri_step(self, step, *args, **kw):
+        """One outer step of Algorithm 2 over all ranks' columns.  The decision logic (lines 4-14, the
+        eps halving, the warm restart) lives in ONE place, the library's wri_awri_step; this is a
+        pass-through that hands it the collective: step is Wri.awri_step bound to this rank's columns
+        (or, on CPU ranks in the tests, the oracle's step), called as step(*args, reduce=self.reduce, **kw).
+        Every rank sees the same f, f_tilde and g, hence takes the same decision."""
+        return step(*args, reduce=self.reduce, **kw)
 
 
-def wri_evaluator(ctx, d, lam, src_ijk, omega_idx):
+def wri_evaluator(ctx, d, lam, src_ijk, omega_idx, rmask=None):
     """evaluate() for ShardedMisfit on a GPU rank: Wri.misfit_sf on the rank's block of columns.
-    d [n_rec, nb_total] (complex64, device), src_ijk [nb_total, 3], omega_idx [nb_total]."""
+    d [n_rec, nb_total] (complex64, device), src_ijk [nb_total, 3], omega_idx [nb_total];
+    rmask: optional per-source receiver sets, uint8 [n_rec, nb_total] (the rank's columns are cut
+    out and handed to wri_set_receiver_mask)."""
 
     def evaluate(lo, hi, eps, maxit, g, warm):
+        if rmask is not None:
+            ctx.set_receiver_mask(rmask[:, lo:hi].contiguous())
         out = ctx.misfit_sf(d[:, lo:hi].contiguous(), lam, src_ijk[lo:hi], eps, maxit,
                             omega_idx=None if omega_idx is None else omega_idx[lo:hi], g=g, warm=warm)
         return out["f"], int(out["iters"].sum().item()), (out["u"], out["alpha"], out["ar0"])

@@ -41,16 +41,21 @@ def main():
     t = 0.5 * float(np.abs(m).mean() / np.abs(g.numpy()).max())
     calls = [0]
 
-    def update(mm, gg, m_trial):
+    def update(mm, gg):
         sign = +1.0 if calls[0] == 0 else -1.0
         calls[0] += 1
-        m_trial.copy_(mm + sign * t * gg.double())
+        return mm + sign * t * gg
 
-    mt = torch.from_numpy(m.copy())
-    step = sm.awri_step(mt, 2e-3, 2000, update, lambda x: model.__setitem__("m", x.numpy().copy()),
+    # the decision logic is the step's own (the library's wri_awri_step on GPU ranks; here, on CPU
+    # ranks, the oracle's); ShardedMisfit.awri_step only hands it the collective
+    def oracle_step(*a, reduce, **k):
+        return A.awri_step(*a, reduce=lambda f, gg: reduce(f, None if gg is None else torch.from_numpy(gg)), **k)
+
+    lo, hi = sm.lo, sm.hi
+    step = sm.awri_step(oracle_step, ops[lo:hi], m.copy(), lam, rec, src[lo:hi], D[:, lo:hi], 2e-3, 2000, update,
                         max_halvings=4)
     out["step"] = {k: step[k] for k in ("accepted", "n_halvings", "eps", "f", "f_trial", "lsqr_iters", "trace")}
-    out["m_next"] = mt.numpy().tolist()
+    out["m_next"] = np.asarray(step["m"]).tolist()
     out["t"] = t
     gathered = [None] * dist.get_world_size()
     dist.all_gather_object(gathered, out)

@@ -41,3 +41,27 @@ def gpu_state_column_sf(st, s):
     g["w_a"] = complex(st["w_a"][s])
     g["x_a"] = complex(st["x_a"][s])
     return g
+
+
+def c64_floor(solve, d, members=3):
+    """Attainable floor of a complex64 solver on one column: the deviation
+    from the complex128 iterates of the oracle's own complex64-STORAGE emulation (round_c64), taken as
+    the largest over a few members whose data differ by one float32 rounding (6e-8 relative) — the
+    onset of the orthogonality loss moves by an iteration or two between such members, so a single one
+    can sit on the lucky side at a given k.  solve(d, round_c64) -> dict with "x" and "resnorms".
+    Returns (floor_x, floor_history, reference); c64_floor.last_residual holds the floor of the LAST
+    residual norm alone, |res_K / ref_K - 1| (the history norm is dominated by its early entries)."""
+    ref = solve(d, False)
+    fx = fh = 0.0
+    c64_floor.last_residual = 0.0
+    for i in range(members):
+        dd = d
+        if i:
+            rng = np.random.Generator(np.random.PCG64(100 + i))
+            dd = d * (1.0 + 6e-8 * (rng.standard_normal(d.size) + 1j * rng.standard_normal(d.size)))
+        e = solve(dd, True)
+        fx = max(fx, rel(e["x"], ref["x"]))
+        fh = max(fh, rel(e["resnorms"], ref["resnorms"]))
+        c64_floor.last_residual = max(c64_floor.last_residual,
+                                      abs(float(e["resnorms"][-1]) / float(ref["resnorms"][-1]) - 1.0))
+    return fx, fh, ref

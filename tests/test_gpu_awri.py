@@ -215,6 +215,23 @@ def test_awri_step_builtin_update_and_errors(torch_cuda):
     assert np.allclose(m_next, np.clip(G.m - np.float32(t) * g32, np.float32(lo), np.float32(hi)), rtol=1e-6, atol=0)
     assert m_next.min() >= lo and m_next.max() <= hi
     assert (m_next == np.float32(lo)).any() and (m_next == np.float32(hi)).any()
+    # a trial model that is not a number is a rejected step, never an accepted one (reading C-20);
+    # a model that is not a number to begin with is an error, and the model is left as it was
+    m_before = G.m_dev.clone()
+
+    def upd_nan(m, g, m_trial):
+        m_trial.copy_(m)
+        m_trial[3] = float("nan")
+
+    out = ctx.awri_step(G.m_dev, d, G.lam, src, 1e-3, 100, omega_idx=G.omega_idx, max_halvings=2, update=upd_nan)
+    assert not out["accepted"] and out["n_halvings"] == 2 and torch.equal(G.m_dev, m_before)
+    assert all(not math.isfinite(ft) and math.isfinite(f) for _, f, ft in out["trace"])
+    bad = m_before.clone()
+    bad[5] = float("nan")
+    with pytest.raises(WriError) as ei:
+        ctx.awri_step(bad, d, G.lam, src, 1e-3, 50, omega_idx=G.omega_idx, max_halvings=1, step=t, m_min=lo, m_max=hi)
+    assert ei.value.code == -7 and torch.isnan(bad[5]) and torch.equal(bad[:5], m_before[:5])
+    ctx.set_model(G.m_dev)
     with pytest.raises(WriError):
         ctx.awri_step(G.m_dev, d, G.lam, src, 0.0, 400, omega_idx=G.omega_idx)      # eps must be > 0
     with pytest.raises(WriError):
@@ -261,3 +278,46 @@ def test_misfit_on_the_tma_path_with_compaction(torch_cuda, name, kw):
         O.objective_gradient(ops[s], m64, w.lam, rec, u[:, s].astype(complex), w.D[:, s],
                              src=int(srcc[s]), alpha_src=complex(al[s]), g=gsum)
     assert np.linalg.norm(g.cpu().numpy() - gsum) / np.linalg.norm(gsum) < 1e-5
+
+
+def test_sharded_misfit_on_one_nccl_rank_equals_the_unsharded_evaluation(torch_cuda):
+    """paper_2410_18429_b200.sharded with the real evaluator (Wri.misfit_sf) over NCCL: on one rank
+    the all-reduce is the identity, so f and g must be bit-identical to the plain evaluation, and the
+    Algorithm 2 step through ShardedMisfit.awri_step (a pass-through to wri_awri_step with the
+    collective as its reduce callback) must take the decisions of the plain step."""
+    torch = torch_cuda
+    import socket
+    import torch.distributed as dist
+    from paper_2410_18429_b200.sharded import ShardedMisfit, wri_evaluator
+    G = Group(nb=4)
+    ctx = G.ctx(torch)
+    d = torch.from_numpy(G.D).cuda()
+    src = G.ijk(G.src)
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    dist.init_process_group("nccl", init_method="tcp://127.0.0.1:%d" % port, rank=0, world_size=1,
+                            device_id=torch.device("cuda", torch.cuda.current_device()))
+    try:
+        sm = ShardedMisfit(G.nb, wri_evaluator(ctx, d, G.lam, src, G.omega_idx), G.ops[0].ng, d.device, dist)
+        assert (sm.lo, sm.hi) == (0, G.nb)
+        f, g, iters, _ = sm.misfit(1e-4, 400)
+        g_plain = torch.zeros_like(g)
+        plain = ctx.misfit_sf(d, G.lam, src, 1e-4, 400, omega_idx=G.omega_idx, g=g_plain)
+        assert f == plain["f"] and torch.equal(g, g_plain) and iters == int(plain["iters"].sum().item())
+        m64 = G.m.astype(np.float64)
+        t = 0.1 * float(np.abs(m64).mean() / float(g.abs().max()))
+        lo, hi = float(G.m.min()), float(G.m.max())
+        m_a, m_b = G.m_dev.clone(), G.m_dev.clone()
+        ctx.set_model(m_a)
+        a = ctx.awri_step(m_a, d, G.lam, src, 1e-3, 400, omega_idx=G.omega_idx, max_halvings=2, step=t,
+                          m_min=lo, m_max=hi)
+        ctx.set_model(m_b)
+        b = sm.awri_step(ctx.awri_step, m_b, d, G.lam, src, 1e-3, 400, omega_idx=G.omega_idx, max_halvings=2,
+                         step=t, m_min=lo, m_max=hi)
+        for k in ("accepted", "n_halvings", "eps", "f", "f_trial", "lsqr_iters", "trace"):
+            assert a[k] == b[k], k
+        assert torch.equal(m_a, m_b) and torch.equal(a["g"], b["g"])
+    finally:
+        dist.destroy_process_group()

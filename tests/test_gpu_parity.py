@@ -10,7 +10,7 @@ import pytest
 
 import workloads
 from oracle import oracle as O
-from gpu_util import gpu_state_column, ops_for, rel
+from gpu_util import c64_floor, gpu_state_column, ops_for, rel
 
 pytestmark = pytest.mark.gpu
 
@@ -126,7 +126,7 @@ def _step_tolerance(name, op, w, rec, prev, ref):
 
 
 @pytest.mark.parametrize("name,kw,K", TF_CASES)
-def test_teacher_forced_steps(torch_cuda, name, kw, K):
+def test_teacher_forced_steps(torch_cuda, name, kw, K, record_property):
     """Every iteration: load the GPU's state k-1 into the oracle's single step and compare the
     step-k outputs (u, v, w, x, alpha, beta, phibar, rhobar).  This is the correctness gate that
     holds on every config, including configs[0] where free-running complex64 cannot track
@@ -150,6 +150,7 @@ def test_teacher_forced_steps(torch_cuda, name, kw, K):
         g = gpu_state_column(st, s)
         assert rel(g["v"], v1 / np.linalg.norm(v1)) < tol
         assert g["alpha"] == pytest.approx(np.linalg.norm(v1), rel=tol)
+    worst_tol = worst_err = 0.0
     for k in range(1, K + 1):
         prev = st
         ctx.lsqr_iterate(1)
@@ -164,7 +165,14 @@ def test_teacher_forced_steps(torch_cuda, name, kw, K):
                 errs.append(float(np.linalg.norm(got["u_bot"] - ref["u_bot"])))
             errs += [abs(got[n] - ref[n]) / abs(ref[n]) for n in ("alpha", "beta", "phibar", "rhobar")]
             assert max(errs) < tol_k, (k, s, tol_k, errs)
+            worst_tol, worst_err = max(worst_tol, tol_k), max(worst_err, max(errs))
     ctx.lsqr_end()
+    # the data-dependent gate of configs[0] (8 eps kappa) is logged so that it cannot grow unseen
+    print("teacher-forced %s %s: largest step tolerance %.2e (kappa %.0f), largest error %.2e"
+          % (name, kw, worst_tol, worst_tol / (8 * 6e-8), worst_err))
+    record_property("largest_step_tolerance", "%.3e" % worst_tol)
+    record_property("largest_step_error", "%.3e" % worst_err)
+    assert worst_tol < 2e-4                                  # kappa stays below ~400 on every case
 
 
 def _free_run(torch, w, K, cols=None, threads=8):
@@ -229,9 +237,22 @@ def test_config0_free_running_is_bounded_by_the_storage_floor(torch_cuda):
     t, b = O.apply_M(op, w.m, w.lam, rec, x)
     r_true = math.sqrt((abs(w.lam * w.Q[:, 0].astype(complex) - t) ** 2).sum()
                        + (abs(w.D[:, 0].astype(complex) - b) ** 2).sum())
-    assert abs(r_true / ref["resnorms"][50, 0] - 1.0) < 0.25
     assert abs(res[50, 0] / r_true - 1.0) < 0.05             # the GPU's own estimate is honest
     assert np.all(np.diff(res[:, 0]) <= 1e-6 * res[0, 0])    # monotone ||r_k||
+    # against the attainable floor (the oracle's complex64-storage emulation, measured on CPU in
+    # tests/test_oracle_c64floor.py): the GPU deviates from complex128 by no more than twice that
+    from dataclasses import replace
+    q0, d0 = w.Q[:, 0].astype(complex), w.D[:, 0].astype(complex)
+    fx, fh, _ = c64_floor(lambda dd, r: O.lsqr(replace(op, round_c64=r), w.m, w.lam, rec, q0, dd, maxit=50), d0)
+    dev_x, dev_h = rel(u[:, 0], ref["x"][:, 0]), rel(res[:, 0], ref["resnorms"][:, 0])
+    print("configs[0] k = 50: GPU deviation x %.3e history %.3e; complex64 floor x %.3e history %.3e"
+          % (dev_x, dev_h, fx, fh))
+    assert dev_x <= 2.0 * fx and dev_h <= 2.0 * fh
+    # ... and the TRUE residual of its x_50 (oracle arithmetic) is as far from the oracle's as the floor's
+    fr = c64_floor.last_residual
+    print("configs[0] k = 50: true residual of the GPU's x / oracle's %.4f; floor of that ratio 1 +- %.4f"
+          % (r_true / ref["resnorms"][50, 0], fr))
+    assert abs(r_true / ref["resnorms"][50, 0] - 1.0) <= 2.0 * fr + 1e-3
 
 
 def test_adaptive_masks_config3(torch_cuda):
@@ -282,17 +303,14 @@ def test_column_compaction_matches_uncompacted_and_oracle(torch_cuda, monkeypatc
     tol = torch.from_numpy(w.tol).cuda()
 
     def run(no_compact):
-        if no_compact:
-            monkeypatch.setenv("WRI_NO_COMPACT", "1")
-        else:
-            monkeypatch.delenv("WRI_NO_COMPACT", raising=False)
         ctx = _wri(w)
+        ctx.set_debug_opts(no_compact=int(no_compact))
         out = [t.cpu().numpy() for t in ctx.lsqr_batch(q, d, w.lam, tol, maxit=maxit, omega_idx=w.omega_idx)]
         return out, ctx.lsqr_peek()["nb"], ctx.launch_count()
 
     (u, res, it), nb_end, n1 = run(False)
     (u0, res0, it0), nb_end0, n0 = run(True)
-    assert nb_end0 == 48 and nb_end == 2                     # the working set really shrank (48 -> ... -> 2)
+    assert nb_end0 == 48 and nb_end <= 8                     # the working set really shrank (48 -> ... -> a few)
     assert np.array_equal(it, it0) and it[7] == maxit and len(set(it.tolist())) > 8
     assert np.isfinite(u.view(np.float32)).all()
     for s in range(w.nb):
@@ -372,7 +390,7 @@ def test_no_receivers_and_host_entry(torch_cuda):
 def test_wide_batches_are_solved_in_64_column_groups(torch_cuda, monkeypatch):
     """nb = 128: wri_lsqr_batch works through two compact 64-column groups.
     Each group must give exactly what a separate solve of those 64 columns gives (a column's
-    result does not depend on its batch, C-9), the lock-step 128-column solve (WRI_NO_GROUPS) the
+    result does not depend on its batch, C-9), the lock-step 128-column solve (debug option no_groups) the
     same within rounding, the oracle within 1e-3; with tolerances, the source-free system, a warm
     start and the host entry as well."""
     torch = torch_cuda
@@ -389,10 +407,10 @@ def test_wide_batches_are_solved_in_64_column_groups(torch_cuda, monkeypatch):
                                    omega_idx=w.omega_idx[sl])
         assert torch.equal(torch.view_as_real(u[:, sl]), torch.view_as_real(ug))
         assert torch.equal(res[:, sl], rg)
-    monkeypatch.setenv("WRI_NO_GROUPS", "1")
+    ctx.set_debug_opts(no_groups=1)
     u1, res1, _ = ctx.lsqr_batch(q, d, w.lam, None, maxit=K, omega_idx=w.omega_idx)
     torch.cuda.synchronize()
-    monkeypatch.delenv("WRI_NO_GROUPS")
+    ctx.set_debug_opts()
     assert rel(u.cpu().numpy(), u1.cpu().numpy()) < 1e-5
     assert rel(res.cpu().numpy(), res1.cpu().numpy()) < 1e-6
     rec = O.rec_cells(w.nx, w.ny, w.nz, w.rec_ijk)
@@ -409,10 +427,10 @@ def test_wide_batches_are_solved_in_64_column_groups(torch_cuda, monkeypatch):
     tol = torch.from_numpy(tolh).cuda()
     ut, rt, itt = ctx.lsqr_batch(q, d, w.lam, tol, maxit=80, omega_idx=w.omega_idx)
     torch.cuda.synchronize()
-    monkeypatch.setenv("WRI_NO_GROUPS", "1")
+    ctx.set_debug_opts(no_groups=1)
     ut1, rt1, itt1 = ctx.lsqr_batch(q, d, w.lam, tol, maxit=80, omega_idx=w.omega_idx)
     torch.cuda.synchronize()
-    monkeypatch.delenv("WRI_NO_GROUPS")
+    ctx.set_debug_opts()
     assert torch.equal(itt, itt1) and int(itt[7]) == 80 and len(set(itt.cpu().tolist())) > 8
     assert rel(ut.cpu().numpy(), ut1.cpu().numpy()) < 1e-5
     assert rel(rt.cpu().numpy(), rt1.cpu().numpy()) < 1e-6
@@ -421,7 +439,7 @@ def test_wide_batches_are_solved_in_64_column_groups(torch_cuda, monkeypatch):
     outs = {}
     for mode in ("groups", "lockstep"):
         if mode == "lockstep":
-            monkeypatch.setenv("WRI_NO_GROUPS", "1")
+            ctx.set_debug_opts(no_groups=1)
         ar0 = torch.zeros(w.nb, dtype=torch.float64, device="cuda")
         ctx.set_opts(ar0_out=ar0)
         us, al, rs, its = ctx.lsqr_sf_batch(d, w.lam, w.src_ijk, None, maxit=12, omega_idx=w.omega_idx)
@@ -434,7 +452,7 @@ def test_wide_batches_are_solved_in_64_column_groups(torch_cuda, monkeypatch):
         torch.cuda.synchronize()
         outs[mode] = [t.cpu().numpy() for t in (us, al, rs, us2, al2, rs2, ar0)]
         if mode == "lockstep":
-            monkeypatch.delenv("WRI_NO_GROUPS")
+            ctx.set_debug_opts()
     for a, b in zip(outs["groups"], outs["lockstep"]):
         assert rel(a, b) < 2e-5
     assert np.all(outs["groups"][5][-1] < outs["groups"][2][-1])       # the continuation went on converging

@@ -9,7 +9,7 @@ import pytest
 
 import workloads
 from oracle import oracle as O
-from gpu_util import gpu_state_column_sf, ops_for, rel
+from gpu_util import c64_floor, gpu_state_column_sf, ops_for, rel
 
 pytestmark = pytest.mark.gpu
 
@@ -195,12 +195,21 @@ def test_sf_free_running_50_iterations(torch_cuda, name, kw, cols):
     u, a, res, it = run(K)
     assert (it == K).all()
     ref = O.lsqr_sf_batch(ops, w.m, w.lam, rec, src, w.D, None, maxit=K, threads=4, columns=cols)
+    from dataclasses import replace
     for j, s in enumerate(cols):
         r_true, _ = _true_residuals(w, ops[s], rec, src[s], s, u[:, s], a[s])
-        assert abs(r_true / ref["resnorms"][K, j] - 1.0) < 0.05, (s, r_true, ref["resnorms"][K, j])
         assert abs(res[K, s] / r_true - 1.0) < 1e-3                 # the GPU's estimate is honest
         assert np.all(np.diff(res[:, s]) <= 1e-6 * res[0, s])       # monotone ||r_k||
-        assert rel(res[:, s], ref["resnorms"][:, j]) < 2e-2
+        # against the attainable floor: the oracle's complex64-storage emulation of the same column
+        # (reading C-16; measured on CPU in tests/test_oracle_c64floor.py)
+        fx, fh, _ = c64_floor(lambda dd, r: O.lsqr_sf(replace(ops[s], round_c64=r), w.m, w.lam, rec, src[s], dd,
+                                                      maxit=K), w.D[:, s].astype(complex))
+        dev_x, dev_h = rel(u[:, s], ref["x"][:, j]), rel(res[:, s], ref["resnorms"][:, j])
+        print("b = [0; d] %s column %d k = %d: GPU deviation x %.3e history %.3e; complex64 floor x %.3e "
+              "history %.3e" % (name, s, K, dev_x, dev_h, fx, fh))
+        assert dev_x <= 2.0 * fx + 1e-3 and dev_h <= 2.0 * fh + 1e-3
+        assert abs(r_true / ref["resnorms"][K, j] - 1.0) <= 2.0 * c64_floor.last_residual + 1e-3, \
+            (s, r_true, ref["resnorms"][K, j])
     u2, a2, res2, _ = run(K)
     assert np.array_equal(u2, u) and np.array_equal(a2, a) and np.array_equal(res2, res)
 
@@ -238,10 +247,10 @@ def test_sf_adaptive_masks_compaction_and_host_entry(torch_cuda, monkeypatch):
         assert np.all(res[k:, s] == res[k, s])
         assert np.all(np.diff(res[:, s]) <= 1e-6 * res[0, s])
     # without compaction: bit-identical per column
-    monkeypatch.setenv("WRI_NO_COMPACT", "1")
+    ctx.set_debug_opts(no_compact=1)
     u2, a2, res2, it2 = ctx.lsqr_sf_batch(d, w.lam, w.src_ijk, told, maxit=maxit, omega_idx=w.omega_idx)
     torch.cuda.synchronize()
-    monkeypatch.delenv("WRI_NO_COMPACT")
+    ctx.set_debug_opts()
     assert np.array_equal(it2.cpu().numpy(), it)
     assert np.array_equal(res2.cpu().numpy(), res)
     assert np.array_equal(a2.cpu().numpy(), a)

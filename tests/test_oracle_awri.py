@@ -115,6 +115,25 @@ def test_ascent_step_halves_the_tolerance_until_the_cap(group):
     assert r["m"] is m or np.array_equal(r["m"], m)          # line 13 not reached: model unchanged
 
 
+def test_trial_model_with_a_non_finite_objective_is_a_rejected_step(group):
+    """reading C-20: line 9 compares numbers; an update that leaves the physical range (NaN in the
+    trial model, hence f_tilde = NaN) must not be accepted: eps is halved to the cap, m is unchanged"""
+    ops, m, rec, src, D, lam, g = group
+
+    def upd(mm, gg):
+        out = mm.copy()
+        out[3] = np.nan
+        return out
+
+    r = A.awri_step(ops, m, lam, rec, src, D, eps=1e-3, maxit=200, update=upd, max_halvings=2)
+    assert not r["accepted"] and r["n_halvings"] == 2 and np.array_equal(r["m"], m)
+    assert all(not np.isfinite(ft) for _, _, ft in r["trace"]) and all(np.isfinite(f) for _, f, _ in r["trace"])
+    bad = m.copy()
+    bad[5] = np.nan
+    with pytest.raises(FloatingPointError):
+        A.awri_step(ops, bad, lam, rec, src, D, eps=1e-3, maxit=50, update=lambda mm, gg: mm, max_halvings=1)
+
+
 def test_loose_tolerance_rejects_a_good_step_and_the_halved_one_accepts(group):
     """Found by scanning eps on this seeded group: at eps = 0.08466 one column of the trial model
     stops an iteration earlier than at m, so f_trial > f although the step is a descent step;

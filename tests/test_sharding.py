@@ -65,8 +65,11 @@ def test_two_rank_gloo_misfit_and_adaptive_step(tmp_path):
     assert r.returncode == 0, r.stderr[-2000:]
     a, b = json.loads(out.read_text())
     assert a["rank_cols"] == [0, 3] and b["rank_cols"] == [3, 5]
-    for k in ("f", "g", "iters", "step", "m_next"):
+    for k in ("f", "g", "iters", "m_next"):
         assert a[k] == b[k], k                                   # every rank holds the same result
+    for k in a["step"]:                                          # ... and took the same decisions
+        if k != "lsqr_iters":                                    # (iterations are counted per rank)
+            assert a["step"][k] == b["step"][k], k
     ops, m, rec, src, D, _ = _problem((9, 8, 7), 10, 5, seed=61)
     ref = A.misfit_sf(ops, m, 20.0, rec, src, D, 1e-8, 2000)
     assert a["f"] == pytest.approx(ref["f"], rel=1e-13)
@@ -82,6 +85,7 @@ def test_two_rank_gloo_misfit_and_adaptive_step(tmp_path):
 
     rs = A.awri_step(ops, m, 20.0, rec, src, D, 2e-3, 2000, upd, max_halvings=4)
     st = a["step"]
+    assert a["step"]["lsqr_iters"] + b["step"]["lsqr_iters"] == rs["lsqr_iters"]
     assert st["accepted"] and rs["accepted"] and st["n_halvings"] == rs["n_halvings"] == 1
     assert st["eps"] == pytest.approx(rs["eps"], rel=1e-15)
     for (e, f, ft), (er, fr, ftr) in zip(st["trace"], rs["trace"]):
