@@ -73,13 +73,15 @@ class ShardedMisfit:
             self.dist.all_reduce(g, op=self.dist.ReduceOp.SUM)
         return float(s[0])
 
-    def awri_step(self, step, *args, **kw):
+    def awri_step(self, awri_step_fn, /, *args, **kw):
         """One outer step of Algorithm 2 over all ranks' columns.  The decision logic (lines 4-14, the
         eps halving, the warm restart) lives in ONE place, the library's wri_awri_step; this is a
-        pass-through that hands it the collective: step is Wri.awri_step bound to this rank's columns
-        (or, on CPU ranks in the tests, the oracle's step), called as step(*args, reduce=self.reduce, **kw).
+        pass-through that hands it the collective: awri_step_fn is Wri.awri_step bound to this rank's
+        columns (or, on CPU ranks in the tests, the oracle's step), called as
+        awri_step_fn(*args, reduce=self.reduce, **kw) — positional-only here, so that the step's own
+        keyword arguments (step=, m_min=, ...) pass through untouched.
         Every rank sees the same f, f_tilde and g, hence takes the same decision."""
-        return step(*args, reduce=self.reduce, **kw)
+        return awri_step_fn(*args, reduce=self.reduce, **kw)
 
 
 def wri_evaluator(ctx, d, lam, src_ijk, omega_idx, rmask=None):
