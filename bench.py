@@ -214,6 +214,54 @@ def run_reference(args, wl_name, w):
     print(json.dumps(line), flush=True)
 
 
+def run_width_sweep(args, wl_name, w):
+    """Per-pass fraction of the copy bandwidth of the persistent pass kernel at each working width
+    a shrinking batch passes through (fixed-K solves of the first nb columns of the workload, per-launch
+    CUDA events of wri_profile_*): one JSON line per width.  The tables under profiles/ come from this."""
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
+    dev = torch.device("cuda", 0)
+    from paper_2410_18429_b200 import Wri
+    ctx = Wri.from_workload(w, device=dev)
+    if args.stencil:
+        ctx.set_stencil(args.stencil)
+    if args.debug_opts:
+        ctx.set_debug_opts(**{k: int(v) for k, v in (kv.split("=") for kv in args.debug_opts.split(","))})
+    peak, _ = measured_hbm_peak()
+    K = args.maxit or 20
+    for nbw in [int(x) for x in args.width_sweep.split(",")]:
+        if nbw > w.nb:
+            continue
+        q = torch.from_numpy(np.ascontiguousarray(w.Q[:, :nbw])).to(dev)
+        d = torch.from_numpy(np.ascontiguousarray(w.D[:, :nbw])).to(dev)
+        oi = w.omega_idx[:nbw]
+        out = ctx._outputs(nbw, K, dev)
+        for _ in range(2):
+            ctx.lsqr_batch(q, d, w.lam, None, maxit=K, omega_idx=oi, out=out)
+        torch.cuda.synchronize()
+        ctx.profile_enable(True)
+        ctx.profile_read()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            ctx.lsqr_batch(q, d, w.lam, None, maxit=K, omega_idx=oi, out=out)
+        e1.record()
+        torch.cuda.synchronize()
+        ms_f, n_f, cols_f, ms_a, n_a, cols_a = ctx.profile_read()
+        ctx.profile_enable(False)
+        bf = (BYTES_PASS_F * nbw + 4) * w.ng
+        ba = (BYTES_PASS_A * nbw + 4) * w.ng
+        ach_f = bf / (ms_f / n_f * 1e-3) / 1e9
+        ach_a = ba / (ms_a / n_a * 1e-3) / 1e9
+        whole = BYTES_ITER * w.ng * nbw * K * args.steps / (e0.elapsed_time(e1) * 1e-3) / 1e9
+        print(json.dumps({"workload": wl_name, "nb": nbw, "maxit": K, "plan": ctx.plan_info(nbw + (nbw & 1)),
+                          "pass_f": {"ms": ms_f / n_f, "GBps": ach_f, "frac": ach_f / peak},
+                          "pass_a": {"ms": ms_a / n_a, "GBps": ach_a, "frac": ach_a / peak},
+                          "whole_solve_frac": whole / peak}), flush=True)
+        del q, d, out
+
+
 def run_ours(args, wl_name, w):
     import torch
     rank, world, local = dist_env()
@@ -480,6 +528,9 @@ def main():
                     help="0: 7-point (north_star), 1: 27-point box discretisation of the Laplacian")
     ap.add_argument("--debug-opts", default=None,
                     help="tuning switches of wri_debug_opts, e.g. txc=4,tyc=4,nstage_a=8 (sweeps under profiles/)")
+    ap.add_argument("--width-sweep", default=None,
+                    help="comma-separated batch widths: per-pass roofline fractions of fixed-K solves at each "
+                         "width, one JSON line per width (instead of the bench line)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true",
                     help="skip the source-free solve and the objective/gradient context lines")
@@ -495,6 +546,8 @@ def main():
         w.maxit = args.maxit
     if args.impl == "reference":
         run_reference(args, args.workload, w)
+    elif args.width_sweep:
+        run_width_sweep(args, args.workload, w)
     else:
         run_ours(args, args.workload, w)
 

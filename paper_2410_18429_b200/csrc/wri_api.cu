@@ -37,7 +37,6 @@ inline int even_up(int n) { return (n + 1) & ~1; }
 inline unsigned blocks_for(long long n) { return (unsigned)std::min<long long>((n + 255) / 256, 148 * 16); }
 constexpr int kMaxCtas = 512;          // upper bound on the persistent grid (>= SM count)
 constexpr int kInitRowBlocks = 64;     // blocks of k_init_rows (extra rows of the generic partials)
-constexpr int kChk = 4;                // the compaction kernel is enqueued every kChk iterations
 
 struct Tiling {
     int vec;            // complex numbers per thread (2 = 128-bit accesses)
@@ -104,7 +103,6 @@ struct wri_ctx {
     // persistent pass kernel: per-width plans, tensor maps and receiver lists (device tables)
     int num_sms = 0;
     unsigned int* counter = nullptr;      // last-CTA ticket of the pass kernels (device)
-    unsigned int* counter2 = nullptr;     // ... of the compaction kernel
     bool rt = false;                      // this solve runs on the persistent pass kernel
     int n_widths = 0;                     // plans of the solve: widths nb, nb-2, ..., (adaptive) or just nb
     int cap_widths = 0, cap_own = 0;
@@ -705,7 +703,8 @@ RtParams rt_solve_params(const wri_ctx* c, int phase) {
     // the first forward pass of a cold batch solve (c->lazy)
     p.has_old = (MODE == MODE_A) ? (phase != PH_INIT_A) : 1;
     p.lazy = c->lazy;
-    p.packed = c->packed; p.adaptive = c->adaptive; p.chk = kChk;
+    p.packed = c->packed; p.adaptive = c->adaptive;
+    p.u_out = c->u_out;
     p.maxit = c->maxit;
     p.n_rec = c->n_rec; p.rec = c->rec;
     p.fin = scal_params(c, c->partials_rt, rt_grid(c), nullptr);
@@ -741,7 +740,6 @@ MoveParams move_params(const wri_ctx* c) {
     p.u_out = c->u_out; p.resnorms = c->resnorms;
     p.n_g = (long long)c->ng; p.nb_out = c->nb0; p.nb_max = c->nb_max; p.maxit = c->maxit; p.n_rec = c->n_rec;
     p.packed = c->packed;
-    p.counter = c->counter2;
     return p;
 }
 
@@ -917,9 +915,8 @@ int wri_create(wri_ctx** out, wri_grid grid, double h, int32_t n_omega, const do
     CKC(cudaMalloc(&c->aw_ar0, NM * sizeof(double)));
     CKC(cudaMalloc(&c->aw_iters, NM * sizeof(int)));
     CKC(cudaMallocHost(&c->h_aw, (size_t)NM * (2 * sizeof(double) + sizeof(int))));
-    CKC(cudaMalloc(&c->counter, 2 * sizeof(unsigned int)));
-    CKC(cudaMemset(c->counter, 0, 2 * sizeof(unsigned int)));
-    c->counter2 = c->counter + 1;
+    CKC(cudaMalloc(&c->counter, sizeof(unsigned int)));
+    CKC(cudaMemset(c->counter, 0, sizeof(unsigned int)));
     CKC(cudaMalloc(&c->d_state, sizeof(SolveState)));
     CKC(cudaMemset(c->d_state, 0, sizeof(SolveState)));
     CKC(cudaMalloc(&c->d_prof, 4 * sizeof(long long)));
@@ -1397,11 +1394,6 @@ int wri_lsqr_iterate(wri_ctx* c, int32_t n_steps) {
             // once when every column has stopped; nothing comes back to the host.
             if ((rc = launch_rt<MODE_F>(c, PH_F))) return rc;
             if ((rc = launch_rt<MODE_A>(c, PH_A))) return rc;
-            if (c->adaptive && c->k % kChk == 0 && c->k < c->maxit) {
-                k_compact<<<c->num_sms * 4, 256, 0, c->stream>>>(move_params(c));
-                c->launches++;
-                CK(cudaGetLastError());
-            }
         } else {
             PassParams p = base_params(c, c->nb, c->tl);
             p.partials = c->partials;

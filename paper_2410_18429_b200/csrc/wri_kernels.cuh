@@ -59,10 +59,12 @@ struct DevPlan {          // tile geometry of one working width
 struct SolveState {       // device-resident state of the solve in flight
     int widx, nb, k, n_active;
     int all_done, parity, pending, pending_widx;
-    int n_keep, n_ret, pad0, pad1;
-    long long waste;                  // stale column-iterations since the last compaction
-    int map[RT_MAXW];                 // pending compaction: new column j <- old column map[j] (-1 = padding)
-    int ret_src[RT_MAXW], ret_dst[RT_MAXW];   // columns leaving: working column -> caller's column
+    // pending re-packing of the working set (decided by the finaliser of pass A, carried out by the
+    // two passes of the next iteration, see k_pass_rt):
+    int map[RT_MAXW];                 // new column j <- old column map[j] (-1 = padding)
+    int dest[RT_MAXW];                // old column c -> new column (>= 0); -1: c leaves; <= -2: c leaves and its
+                                      // threads zero-fill the padding column -2 - dest[c] of the new set
+    int ret_dst[RT_MAXW];             // old column c -> caller's column that receives its final x (-1: none)
     int colmap[2][RT_MAXW];           // per parity: working column -> caller's column (-1 = padding)
 };
 
@@ -380,9 +382,14 @@ struct ScalParams {
     // device-resident solve state (persistent pass kernel): iteration counter, active count, the
     // decision to re-pack the working set (PH_A), the condition of the device-side loop
     SolveState* st;           // null: host-sequenced solve (generic kernels)
-    int adaptive;             // PH_A may ask for a compaction
-    int chk;                  // ... after iterations k % chk == 0 (when the compaction kernel is enqueued)
+    int adaptive;             // PH_A may ask for a re-packing of the working set
     int widx;                 // index of the current width's plan
+    // PH_A of an iteration whose passes re-packed the vectors (trans): the finaliser moves the
+    // per-column state to the other bank and switches the solve state over
+    int trans;
+    int nb_new;               // width of the new working set
+    float* coef2; double* stat2; int* active2; int* iters2;   // the other bank
+    float2* U_bot2;
     int init_rows;            // PH_INIT_B: k_init_rows has formed U_bot; its |.|^2 sums are extra rows of partials
     void* cond;               // cudaGraphConditionalHandle or null
 };
@@ -631,30 +638,27 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
 
     if (PHASE == PH_A && p.st && threadIdx.x == 0) {
         // device-resident solve state: iteration count, live columns, and — with adaptive accuracy —
-        // the decision to re-pack the working set.  Ski-rental rule: re-pack once the bandwidth spent
-        // on stopped columns since the last re-packing (80 B per cell, column and iteration) exceeds
-        // what the re-packing moves (4 vectors read at the old width, written at the new: 32 B per
-        // cell and column of either), provided the iterations left can pay it back.
+        // the decision to re-pack the working set.  Re-packing rides on the two passes of the next
+        // iteration (they write their results at the new width, see k_pass_rt), so it costs one extra
+        // write of U and nothing else: it is asked for as soon as the even width that holds the live
+        // columns is narrower than the working set.
         SolveState* st = p.st;
         int n_act = 0;
         for (int s = 0; s < nb; ++s) n_act += p.active[s] != 0;
         st->k = p.k;
         st->n_active = n_act;
         if (n_act == 0) st->all_done = 1;
-        else if (p.adaptive) {
-            const long long waste = st->waste + (nb - n_act);
-            st->waste = waste;
+        else if (p.adaptive && !p.trans) {
             const int w_new = max(2, (n_act + 1) & ~1);
-            const long long cost = 32LL * (nb + w_new);
-            if (w_new < nb && (p.k % p.chk) == 0 && p.k < p.maxit && waste * 80 >= cost &&
-                (long long)(nb - w_new) * 80 * (p.maxit - p.k) > cost) {
-                int nk = 0, nr = 0;
+            if (w_new < nb && p.k < p.maxit) {
+                int nk = 0;
                 for (int s = 0; s < nb; ++s) {
-                    if (p.active[s]) st->map[nk++] = s;
-                    else if (p.colmap[s] >= 0) { st->ret_src[nr] = s; st->ret_dst[nr] = p.colmap[s]; ++nr; }
+                    if (p.active[s]) { st->map[nk] = s; st->dest[s] = nk; st->ret_dst[s] = -1; ++nk; }
+                    else { st->dest[s] = -1; st->ret_dst[s] = p.colmap[s]; }
                 }
-                for (int j = nk; j < w_new; ++j) st->map[j] = -1;
-                st->n_keep = nk; st->n_ret = nr;
+                // padding columns of the new set (at most one) are zero-filled by the threads of a leaving column
+                for (int s = 0, j = nk; s < nb && j < w_new; ++s)
+                    if (!p.active[s]) { st->dest[s] = -2 - j; st->map[j] = -1; ++j; }
                 st->pending_widx = p.widx + (nb - w_new) / 2;
                 st->pending = 1;
             }
@@ -664,6 +668,43 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
             cudaGraphSetConditional((cudaGraphConditionalHandle)(uintptr_t)p.cond,
                                     (st->all_done || p.k >= p.maxit) ? 0u : 1u);
 #endif
+    }
+
+    if (PHASE == PH_A && p.st && p.trans) {
+        // This iteration's passes wrote U, V, W, X of the live columns into the other vector set at the
+        // new width (and the final x of the leaving columns into the caller's u_out).  The per-column
+        // state follows: scalars, receiver rows, column map; the residual history of the columns that
+        // left is held at the stop value (reading C-9).  Then the solve state switches over.
+        __syncthreads();
+        SolveState* st = p.st;
+        const int a = st->parity, nbn = p.nb_new;
+        for (int j = threadIdx.x; j < nbn; j += blockDim.x) {
+            const int m = st->map[j];
+            for (int r = 0; r < N_COEF; ++r) p.coef2[r * NM + j] = m >= 0 ? cf[r * NM + m] : 0.f;
+            for (int r = 0; r < N_STAT; ++r) p.stat2[r * NM + j] = m >= 0 ? p.stat[r * NM + m] : 0.0;
+            p.active2[j] = m >= 0 ? p.active[m] : 0;
+            p.iters2[j] = m >= 0 ? p.iters[m] : 0;
+            st->colmap[a ^ 1][j] = m >= 0 ? st->colmap[a][m] : -1;
+        }
+        for (int j = nbn + threadIdx.x; j < RT_MAXW; j += blockDim.x) st->colmap[a ^ 1][j] = -1;
+        for (long long i = threadIdx.x; i < (long long)p.n_rec * nbn; i += blockDim.x) {
+            const long long r = i / nbn;
+            const int m = st->map[(int)(i - r * nbn)];
+            p.U_bot2[i] = m >= 0 ? p.U_bot[r * nb + m] : make_float2(0.f, 0.f);
+        }
+        if (p.resnorms)
+            for (long long i = threadIdx.x; i < (long long)(p.maxit - p.k) * nb; i += blockDim.x) {
+                const int row = (int)(i / nb), s = (int)(i - (long long)row * nb);
+                const int so = st->ret_dst[s];
+                if (so >= 0) p.resnorms[(size_t)(p.k + 1 + row) * p.nb_out + so] = (float)p.stat[S_PHIBAR * NM + s];
+            }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            st->parity = a ^ 1;
+            st->widx = st->pending_widx;
+            st->nb = nbn;
+            st->pending = 0;
+        }
     }
 
     if ((PHASE == PH_INIT_B || PHASE == PH_F) && !p.rows_in_pass) {
@@ -685,8 +726,8 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
 }
 
 // ---------------------------------------------------------------------------------------------
-// Column compaction (shrinking active mask): converged columns leave the
-// working set, the remaining ones are re-packed to a narrower source-interleaved layout.
+// Column gather for the start of a grouped solve (the re-packing of a shrinking working set during
+// an adaptive solve rides on the pass kernels themselves, wri_pass.cuh).
 
 // dst[c][j] = src[c][map[j]] (map[j] < 0 -> 0), widths nb_dst <= nb_src; dst and src are distinct buffers
 __global__ void k_gather_cols(float2* __restrict__ dst, const float2* __restrict__ src,
@@ -716,94 +757,7 @@ struct MoveParams {
     long long n_g;
     int nb_out, nb_max, maxit, n_rec;
     int packed;
-    unsigned int* counter;    // last-block ticket (zero on entry, reset on exit)
 };
-
-// Re-pack the working set (device-driven, decided by the finaliser of pass A): columns that have
-// stopped leave — their x = X + cx W goes to the caller's u_out, their residual history is held at
-// the stop value (reading C-9) — and the live ones are gathered, in order, into the vector set of
-// the other parity at the narrower width.  The last block to finish switches the state over.
-// Every launch is a no-op unless a compaction is pending.
-__global__ void __launch_bounds__(256)
-k_compact(const MoveParams p) {
-    SolveState* st = p.st;
-    if (st->all_done || !st->pending) return;
-    __shared__ int s_map[RT_MAXW], s_rs[RT_MAXW], s_rd[RT_MAXW];
-    __shared__ float s_cx[RT_MAXW];
-    __shared__ unsigned int s_ticket;
-    const int a = st->parity, b = a ^ 1;
-    const int nbo = st->nb, nbn = p.plans[st->pending_widx].nb, n_ret = st->n_ret, k = st->k;
-    const size_t NM = p.nb_max;
-    if (threadIdx.x < RT_MAXW) {
-        s_map[threadIdx.x] = st->map[threadIdx.x];
-        s_rs[threadIdx.x] = st->ret_src[threadIdx.x];
-        s_rd[threadIdx.x] = st->ret_dst[threadIdx.x];
-        s_cx[threadIdx.x] = threadIdx.x < nbo ? p.coef[a][C_CX * NM + threadIdx.x] : 0.f;
-    }
-    __syncthreads();
-    const long long gs = (long long)gridDim.x * blockDim.x, g0 = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    // live columns of U, V, W, X
-    for (long long i = g0; i < p.n_g * nbn; i += gs) {
-        const long long c = i / nbn;
-        const int m = s_map[(int)(i - c * nbn)];
-        float2 v[4];
-#pragma unroll
-        for (int q = 0; q < 4; ++q) v[q] = m >= 0 ? __ldcs(p.vec[a][q] + c * nbo + m) : make_float2(0.f, 0.f);
-#pragma unroll
-        for (int q = 0; q < 4; ++q) p.vec[b][q][i] = v[q];
-    }
-    // columns that leave: final x into the caller's buffer
-    for (long long i = g0; i < p.n_g * n_ret; i += gs) {
-        const long long c = i / n_ret;
-        const int t = (int)(i - c * n_ret), js = s_rs[t];
-        float2 x = __ldcs(p.vec[a][3] + c * nbo + js);
-        const float cx = s_cx[js];
-        if (cx != 0.f) {
-            const float2 w = __ldcs(p.vec[a][2] + c * nbo + js);
-            x.x = fmaf(cx, w.x, x.x);
-            x.y = fmaf(cx, w.y, x.y);
-        }
-        p.u_out[c * p.nb_out + s_rd[t]] = x;
-    }
-    // ... and their residual history, held at the stop value
-    if (p.resnorms)
-        for (long long i = g0; i < (long long)(p.maxit - k) * n_ret; i += gs) {
-            const int row = (int)(i / n_ret), t = (int)(i - (long long)row * n_ret);
-            p.resnorms[(size_t)(k + 1 + row) * p.nb_out + s_rd[t]] = (float)p.stat[a][S_PHIBAR * NM + s_rs[t]];
-        }
-    // receiver rows and the per-column scalars follow their columns
-    for (long long i = g0; i < (long long)p.n_rec * nbn; i += gs) {
-        const long long r = i / nbn;
-        const int m = s_map[(int)(i - r * nbn)];
-        p.U_bot[b][i] = m >= 0 ? p.U_bot[a][r * nbo + m] : make_float2(0.f, 0.f);
-    }
-    if (blockIdx.x == 0)
-        for (int j = threadIdx.x; j < nbn; j += blockDim.x) {
-            const int m = s_map[j];
-            for (int r = 0; r < N_COEF; ++r) p.coef[b][r * NM + j] = m >= 0 ? p.coef[a][r * NM + m] : 0.f;
-            for (int r = 0; r < N_STAT; ++r) p.stat[b][r * NM + j] = m >= 0 ? p.stat[a][r * NM + m] : 0.0;
-            p.active[b][j] = m >= 0 ? p.active[a][m] : 0;
-            p.iters[b][j] = m >= 0 ? p.iters[a][m] : 0;
-        }
-    __threadfence();
-    __syncthreads();
-    if (threadIdx.x == 0) s_ticket = atomicAdd(p.counter, 1u);
-    __syncthreads();
-    if (s_ticket == gridDim.x - 1) {
-        __threadfence();
-        for (int j = threadIdx.x; j < RT_MAXW; j += blockDim.x)
-            st->colmap[b][j] = (j < nbn && s_map[j] >= 0) ? st->colmap[a][s_map[j]] : -1;
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            st->parity = b;
-            st->widx = st->pending_widx;
-            st->nb = nbn;
-            st->waste = 0;
-            st->pending = 0;
-            *p.counter = 0u;
-        }
-    }
-}
 
 // End of a solve: the last deferred update x_k = X + cx W is applied and, where the working set has
 // a column map (grouped / adaptive solves: X lives in the workspace), scattered to the caller's

@@ -55,8 +55,8 @@ struct RtParams {
     int has_old;                      // MODE_A / MODE_G: the second stream (old vector / q) is present
     int lazy;                         // MODE_F: W and X are known to be zero before the first iteration
     int packed;                       // the working set has a column map (grouped / adaptive solves)
-    int adaptive;                     // the finaliser may decide compactions (both vector sets exist)
-    int chk;                          // compaction kernels are enqueued after iterations k % chk == 0
+    int adaptive;                     // the finaliser may decide to re-pack the working set (both vector sets exist)
+    float2* u_out;                    // adaptive: caller's [n_g][nb_out] wavefields (final x of the columns that leave)
     int maxit;
     int n_rec;
     const int* rec;                   // [n_rec] cell indices
@@ -170,6 +170,15 @@ __device__ __forceinline__ void stg128_hint(float2* ptr, const float4& v, uint64
     asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1, %2, %3, %4}, %5;" ::"l"(ptr), "f"(v.x), "f"(v.y),
                  "f"(v.z), "f"(v.w), "l"(pol) : "memory");
 }
+__device__ __forceinline__ void stg64_hint(float2* ptr, float a, float b, uint64_t pol) {
+    asm volatile("st.global.L2::cache_hint.v2.f32 [%0], {%1, %2}, %3;" ::"l"(ptr), "f"(a), "f"(b), "l"(pol) : "memory");
+}
+// one column of a result that is being re-packed: d >= 0 its column in the new set, d <= -2 this column
+// leaves and zero-fills the padding column -2 - d instead, -1 nothing to store
+__device__ __forceinline__ void put_col(float2* base, size_t cell_off, int d, float a, float b, uint64_t pol) {
+    if (d >= 0) stg64_hint(base + cell_off + d, a, b, pol);
+    else if (d <= -2) stg64_hint(base + cell_off + (-2 - d), 0.f, 0.f, pol);
+}
 __device__ __forceinline__ void consumer_sync(int nthreads) {
     asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory");
 }
@@ -218,22 +227,35 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
 
     // ---- state of the solve in flight (uniform over the grid; written only by finalisers of
     //      earlier launches and by the compaction kernel)
-    int par = 0, widx = 0, k_done = 0;
+    int par = 0, widx = 0, k_done = 0, nbn = 0;
+    bool trans = false;
     if (p.st) {
         if (p.st->all_done) return;
         k_done = p.st->k;
         if (k_done >= p.maxit && p.phase != PH_INIT_A) return;
         par = p.st->parity;
         widx = p.st->widx;
+        // Re-packing of a shrinking working set (adaptive accuracy): when the finaliser of the last
+        // iteration asked for it, both passes of this iteration run as usual on the old vector set but
+        // store their results column by column into the other set at the new width — pass F the
+        // updated W and X (and the final x of every column that leaves, into the caller's u_out), pass
+        // A the new V and a copy of U.  No separate compaction pass over the vectors.
+        trans = p.adaptive && p.st->pending != 0 && p.phase != PH_INIT_A;
+        if (trans) nbn = p.plans[p.st->pending_widx].nb;
     }
 
     extern __shared__ __align__(128) unsigned char smem[];
     __shared__ DevPlan s_pl;
     __shared__ unsigned int s_ticket;
+    __shared__ int s_dest[RT_MAXW], s_ret[RT_MAXW];
     const int tid = threadIdx.x;
     {
         const int* src = reinterpret_cast<const int*>(p.st ? p.plans + widx : &p.plan0);
         if (tid < (int)(sizeof(DevPlan) / 4)) reinterpret_cast<int*>(&s_pl)[tid] = src[tid];
+        if (tid < RT_MAXW) {
+            s_dest[tid] = trans ? p.st->dest[tid] : -1;
+            s_ret[tid] = trans ? p.st->ret_dst[tid] : -1;
+        }
     }
     __syncthreads();
     const DevPlan& pl = s_pl;
@@ -292,6 +314,11 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
     float2* const vX = p.vec[par][3];
     float2* const out = p.st ? ((MODE == MODE_F) ? vU : vV) : p.out;
     float2* const U_bot = p.U_bot[par];
+    // the other vector set, written at width nbn while the working set is being re-packed
+    float2* const nU = p.vec[par ^ 1][0];
+    float2* const nV = p.vec[par ^ 1][1];
+    float2* const nW = p.vec[par ^ 1][2];
+    float2* const nX = p.vec[par ^ 1][3];
     // pass F's W / X streams are skipped when both are known to be zero (first pass of a cold solve)
     const bool has_old = (MODE == MODE_F) || p.has_old;
     const bool has_wx = (MODE == MODE_F) && !(p.lazy && k_done == 0);
@@ -411,8 +438,9 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
         //   c_prev  centre of plane z,  s_prev  what plane z gives to its z-neighbours (7-point: the
         //   centre itself; 27-point: a1 c + a2 e + a3 d),  lap  in-plane sum of plane z plus the
         //   contribution of plane z-1.  When plane z+1 arrives, plane z is emitted.
-        auto run_tile = [&](auto m_tma_c, auto has_old_c, const int t) {
+        auto run_tile = [&](auto m_tma_c, auto has_old_c, auto trans_c, const int t) {
             constexpr bool M_TMA = decltype(m_tma_c)::value, HAS_OLD = decltype(has_old_c)::value;
+            constexpr bool TR = decltype(trans_c)::value && MODE != MODE_G;   // this iteration re-packs the working set
             int r = t;
             const int chunk = r % pl.nchunk; r /= pl.nchunk;
             const int tx = r % pl.ntx; r /= pl.ntx;
@@ -429,6 +457,8 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
                 cx[e] = tab_c[4 * nb + col + e];
                 cw[e] = tab_c[5 * nb + col + e];
             }
+            const int d0 = TR ? s_dest[col] : -1, d1 = TR ? s_dest[col + 1] : -1;   // columns in the new set
+            const int r0 = TR ? s_ret[col] : -1, r1 = TR ? s_ret[col + 1] : -1;     // caller's columns of leaving ones
             int gsrc0 = -1, gsrc1 = -1;
             float2 gal0 = make_float2(0.f, 0.f), gal1 = gal0;
             if (MODE == MODE_G && p.gsrc) {
@@ -547,7 +577,17 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
                             rr.w = fmaf(ca[1], ai, -cbk[1] * o_old.w);
                         }
                         if (valid) {
-                            stg128_hint(out + off, rr, pol_st);
+                            const size_t offn = (size_t)cell * nbn;
+                            if (!TR || MODE == MODE_F) {
+                                stg128_hint(out + off, rr, pol_st);
+                            } else {
+                                // pass A of a re-packing iteration: the new V and a copy of U (its centre
+                                // value is in registers) go to the new set
+                                put_col(nV, offn, d0, rr.x, rr.y, pol_st);
+                                put_col(nV, offn, d1, rr.z, rr.w, pol_st);
+                                put_col(nU, offn, d0, cc.x, cc.y, pol_st);
+                                put_col(nU, offn, d1, cc.z, cc.w, pol_st);
+                            }
                             acc32[0] += fmaf(rr.x, rr.x, rr.y * rr.y);
                             acc32[1] += fmaf(rr.z, rr.z, rr.w * rr.w);
                             if (MODE == MODE_F) {
@@ -565,8 +605,20 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
                                 wn.y = fmaf(cv[0], cc.y, -cw[0] * o_w.y);
                                 wn.z = fmaf(cv[1], cc.z, -cw[1] * o_w.z);
                                 wn.w = fmaf(cv[1], cc.w, -cw[1] * o_w.w);
-                                stg128_hint(vX + off, xn, pol_st);
-                                stg128_hint(vW + off, wn, pol_st);
+                                if (!TR) {
+                                    stg128_hint(vX + off, xn, pol_st);
+                                    stg128_hint(vW + off, wn, pol_st);
+                                } else {
+                                    // pass F of a re-packing iteration: X and W go to the new set; a column
+                                    // that leaves has just received its last update, x_k = X + cx W
+                                    put_col(nX, offn, d0, xn.x, xn.y, pol_st);
+                                    put_col(nX, offn, d1, xn.z, xn.w, pol_st);
+                                    put_col(nW, offn, d0, wn.x, wn.y, pol_st);
+                                    put_col(nW, offn, d1, wn.z, wn.w, pol_st);
+                                    const size_t offo = (size_t)cell * p.fin.nb_out;
+                                    if (r0 >= 0) stg64_hint(p.u_out + offo + r0, xn.x, xn.y, pol_st);
+                                    if (r1 >= 0) stg64_hint(p.u_out + offo + r1, xn.z, xn.w, pol_st);
+                                }
                             }
                         }
                     }
@@ -600,12 +652,15 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
         for (int t = blockIdx.x; t < geo.n_tiles; t += gridDim.x) {
             int chunk = t % pl.nchunk;
             if (warp_live) {
-                if (pl.m_tma) {
-                    if (has_old) chunk = run_tile(TrueT{}, TrueT{}, t);
-                    else         chunk = run_tile(TrueT{}, FalseT{}, t);
+                if (trans) {                                     // (a re-packing iteration always has its old stream)
+                    if (pl.m_tma) chunk = run_tile(TrueT{}, TrueT{}, TrueT{}, t);
+                    else          chunk = run_tile(FalseT{}, TrueT{}, TrueT{}, t);
+                } else if (pl.m_tma) {
+                    if (has_old) chunk = run_tile(TrueT{}, TrueT{}, FalseT{}, t);
+                    else         chunk = run_tile(TrueT{}, FalseT{}, FalseT{}, t);
                 } else {
-                    if (has_old) chunk = run_tile(FalseT{}, TrueT{}, t);
-                    else         chunk = run_tile(FalseT{}, FalseT{}, t);
+                    if (has_old) chunk = run_tile(FalseT{}, TrueT{}, FalseT{}, t);
+                    else         chunk = run_tile(FalseT{}, FalseT{}, FalseT{}, t);
                 }
             }
             if (pl.nchunk > 1) {
@@ -636,6 +691,10 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
                         const int4 en = (i == 0) ? own_nxt : __ldg(own + own_cur + i);
                         const int c = chunk * cb + s;
                         float2* vp = out + (size_t)en.y * nb + c;
+                        if (trans) {                             // V of this iteration lives in the new set
+                            if (s_dest[c] < 0) return 0.0;       // (a column that leaves is no longer iterated)
+                            vp = nV + (size_t)en.y * nbn + s_dest[c];
+                        }
                         const float2 v = __ldcg(vp);
                         const float2 u = __ldcg(U_bot + (size_t)en.x * nb + c);
                         const float cts = ct[c];
@@ -681,8 +740,11 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
             f.k = k_done + 1;
             f.st = p.st;
             f.adaptive = p.adaptive;
-            f.chk = p.chk;
             f.widx = widx;
+            f.trans = trans;
+            f.nb_new = nbn;
+            f.coef2 = p.coef[par ^ 1]; f.stat2 = p.stat[par ^ 1]; f.active2 = p.active[par ^ 1];
+            f.iters2 = p.iters[par ^ 1]; f.U_bot2 = p.U_bot[par ^ 1];
             f.cond = p.cond_set ? p.cond : nullptr;
             switch (p.phase) {
                 case PH_INIT_A: finalize_phase<PH_INIT_A>(f, sh); break;
