@@ -425,15 +425,16 @@ int rt_chunk_for(const wri_ctx* c, int nb) {
 }
 
 // planes per tile and tile count of one pass.  With plenty of tiles the measured preferences hold
-// (profiles/r01_v6_stages.md: pass F 16 planes at one 64-column chunk per cell, 128 at 32 columns, else
-// 32; pass A 32 — an L2 effect: short tiles keep the halo shared across a wave of tiles resident).  With
+// (profiles/r02_width_sweeps.md; an L2 effect: short tiles keep the halo that neighbouring tiles share
+// resident across a wave of tiles): pass F 16 planes — except 128 at one 32-column chunk per cell on grids
+// of 256 planes and more (profiles/r01_v6_stages.md) —, pass A 16 planes up to 24 columns, 32 beyond.  With
 // few tiles (narrow widths, small grids) the chunk count that minimises rounds x (planes + priming)
 // over the persistent grid is taken instead.
 PassGeo plan_pass(const wri_ctx* c, const DevPlan& P, bool is_f, int zc_forced) {
     PassGeo G{};
     const int nz = c->g.nz, sms = std::max(1, c->num_sms);
     const long long cols = (long long)P.nchunk * P.ntx * P.nty;
-    int zc = (is_f && P.cb == 64 && P.nchunk == 1) ? 16 : (is_f && P.cb == 32) ? 128 : 32;
+    int zc = is_f ? ((P.cb == 32 && nz >= 256) ? 128 : 16) : (P.cb <= 24 ? 16 : 32);
     if (zc_forced > 0) zc = (zc_forced + 7) / 8 * 8;          // multiples of 8 planes (see the |.|^2 sums of the kernel)
     else if (cols * ((nz + zc - 1) / zc) < 6LL * sms) {
         const double prime = is_f ? 0.6 : 1.2;               // two priming planes in units of a full step
@@ -476,6 +477,9 @@ int make_plan(const wri_ctx* c, int nb, DevPlan& P) {
                 double cost = ntx * nty * ((txc + 2.0) * (tyc + 2.0) + 0.75 * maxcells);
                 const int row_bytes = txc * cb * 8;
                 if (row_bytes < 512 && txc < nx) cost *= 1.0 + 0.25 * (512 - row_bytes) / 512.0;
+                // tile rows that do not start on 128-byte lines: measured 6-10 % slower in both passes
+                // (widths 6, 10: profiles/r02_width_sweeps.md)
+                if (row_bytes % 128 != 0 && txc < nx) cost *= 1.12;
                 if (!(m_al && txc % 4 == 0)) cost *= 1.15;   // model tile by plain loads: measured slower
                 if (cost < best) { best = cost; btx = txc; bty = tyc; }
             }
@@ -677,9 +681,10 @@ void rt_common(const wri_ctx* c, RtParams& p) {
     }
 }
 
-template <int MODE>
+template <int MODE, bool TRK = false>
 const void* rt_kernel(const wri_ctx* c) {
-    return c->stencil == WRI_STENCIL_27 ? (const void*)k_pass_rt<MODE, ST_27> : (const void*)k_pass_rt<MODE, ST_7>;
+    return c->stencil == WRI_STENCIL_27 ? (const void*)k_pass_rt<MODE, ST_27, TRK>
+                                        : (const void*)k_pass_rt<MODE, ST_7, TRK>;
 }
 
 // parameters of one pass of the solve in flight (the same for every iteration: what changes lives
@@ -713,17 +718,29 @@ RtParams rt_solve_params(const wri_ctx* c, int phase) {
 
 template <int MODE>
 int launch_rt(wri_ctx* c, int phase) {
-    const size_t smem = (MODE == MODE_F) ? c->smem_f : c->smem_a;
+    // every launch of a solve asks for the same (maximal) amount of dynamic shared memory: kernels that
+    // alternate between different sizes make the SMs re-partition their L1 / shared memory in between
+    if (std::max(c->smem_f, c->smem_a) > (size_t)RT_SMEM_MAX) return WRI_ERR_ARG;
+    const size_t smem = RT_SMEM_MAX;
     const void* fn = rt_kernel<MODE>(c);
     int rc = allow_smem(c, fn, smem);
     if (rc) return rc;
     RtParams p = rt_solve_params<MODE>(c, phase);
+    p.it = c->k;
     CUtensorMap dummy{};
     cudaEvent_t e1 = nullptr;
     if (phase != PH_INIT_A && (rc = profile_event_begin(c, MODE == MODE_F ? 0 : 1, &e1))) return rc;
     void* args[] = {&dummy, &dummy, &dummy, &p};
     CK(cudaLaunchKernel(fn, dim3(rt_grid(c)), dim3(RT_NT + 32), args, smem, c->stream));
     c->launches++;
+    if (c->adaptive && phase != PH_INIT_A) {
+        // the re-packing variant of the same pass: exactly one of the two does the work (decided on the
+        // device from the solve state), the other returns at once
+        const void* fn_t = rt_kernel<MODE, true>(c);
+        if ((rc = allow_smem(c, fn_t, smem))) return rc;
+        CK(cudaLaunchKernel(fn_t, dim3(rt_grid(c)), dim3(RT_NT + 32), args, smem, c->stream));
+        c->launches++;
+    }
     if (e1) CK(cudaEventRecord(e1, c->stream));
     return WRI_OK;
 }

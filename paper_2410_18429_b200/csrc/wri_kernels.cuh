@@ -58,7 +58,7 @@ struct DevPlan {          // tile geometry of one working width
 
 struct SolveState {       // device-resident state of the solve in flight
     int widx, nb, k, n_active;
-    int all_done, parity, pending, pending_widx;
+    int all_done, parity, pending, pending_widx;   // pending: iteration whose passes re-pack the set (0: none)
     // pending re-packing of the working set (decided by the finaliser of pass A, carried out by the
     // two passes of the next iteration, see k_pass_rt):
     int map[RT_MAXW];                 // new column j <- old column map[j] (-1 = padding)
@@ -651,16 +651,26 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
         else if (p.adaptive && !p.trans) {
             const int w_new = max(2, (n_act + 1) & ~1);
             if (w_new < nb && p.k < p.maxit) {
+                // order of the new set: first the old pairs (2i, 2i+1) whose columns both go on — they stay
+                // aligned pairs, so the passes that re-pack store them with one 16-byte store per thread —,
+                // then the columns that lost their partner, then (at most one) padding column, zero-filled
+                // by the threads of a column that leaves
                 int nk = 0;
                 for (int s = 0; s < nb; ++s) {
-                    if (p.active[s]) { st->map[nk] = s; st->dest[s] = nk; st->ret_dst[s] = -1; ++nk; }
-                    else { st->dest[s] = -1; st->ret_dst[s] = p.colmap[s]; }
+                    st->dest[s] = -1;
+                    st->ret_dst[s] = p.active[s] ? -1 : p.colmap[s];
                 }
-                // padding columns of the new set (at most one) are zero-filled by the threads of a leaving column
+                for (int s = 0; s + 1 < nb; s += 2)
+                    if (p.active[s] && p.active[s + 1]) {
+                        st->map[nk] = s; st->dest[s] = nk; ++nk;
+                        st->map[nk] = s + 1; st->dest[s + 1] = nk; ++nk;
+                    }
+                for (int s = 0; s < nb; ++s)
+                    if (p.active[s] && st->dest[s] < 0) { st->map[nk] = s; st->dest[s] = nk; ++nk; }
                 for (int s = 0, j = nk; s < nb && j < w_new; ++s)
                     if (!p.active[s]) { st->dest[s] = -2 - j; st->map[j] = -1; ++j; }
                 st->pending_widx = p.widx + (nb - w_new) / 2;
-                st->pending = 1;
+                st->pending = p.k + 1;          // the passes of the next iteration re-pack
             }
         }
 #if defined(__CUDACC__)

@@ -68,6 +68,7 @@ struct RtParams {
     const float2* galpha;             // [nb] source weights (with gsrc)
     float* g;                         // [n_g] this batch's gradient (overwritten) or null
     float lam2;
+    int it;                           // iteration this launch belongs to (host count, 1-based)
     void* cond;                       // cudaGraphConditionalHandle of the device-side loop (0 = none)
     int cond_set;                     // this launch's finaliser decides whether the loop goes on
 };
@@ -179,6 +180,16 @@ __device__ __forceinline__ void put_col(float2* base, size_t cell_off, int d, fl
     if (d >= 0) stg64_hint(base + cell_off + d, a, b, pol);
     else if (d <= -2) stg64_hint(base + cell_off + (-2 - d), 0.f, 0.f, pol);
 }
+// the two columns of a thread: one 16-byte store when they stay an aligned pair in the new set (the
+// finaliser orders the new set so that this is the rule), else column by column
+__device__ __forceinline__ void put_pair(float2* base, size_t cell_off, int d0, int d1, bool pair16, const float4& v,
+                                         uint64_t pol) {
+    if (pair16) stg128_hint(base + cell_off + d0, v, pol);
+    else {
+        put_col(base, cell_off, d0, v.x, v.y, pol);
+        put_col(base, cell_off, d1, v.z, v.w, pol);
+    }
+}
 __device__ __forceinline__ void consumer_sync(int nthreads) {
     asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory");
 }
@@ -218,7 +229,7 @@ __device__ __forceinline__ void column_sums(const double* mat, int nrows, int nc
     consumer_sync(NT);
 }
 
-template <int MODE, int STENCIL>
+template <int MODE, int STENCIL, bool TRK>
 __global__ void __launch_bounds__(RT_NT + 32, 1)
 k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUtensorMap pm_old,
           const __grid_constant__ CUtensorMap pm_m, const __grid_constant__ RtParams p) {
@@ -240,7 +251,14 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
         // store their results column by column into the other set at the new width — pass F the
         // updated W and X (and the final x of every column that leaves, into the caller's u_out), pass
         // A the new V and a copy of U.  No separate compaction pass over the vectors.
-        trans = p.adaptive && p.st->pending != 0 && p.phase != PH_INIT_A;
+        // The re-packing variant is a kernel of its own (TRK), so that the code of the plain passes is
+        // not touched by it: an adaptive solve enqueues both per pass and the one that does not apply
+        // returns at once.
+        // (pending holds the number of the iteration that re-packs; p.it is this launch's iteration as the
+        // host counts it — the plain pass A that asks for a re-packing is followed, in the same iteration,
+        // by a launch of the re-packing variant, which must not take the request for its own)
+        trans = p.adaptive && p.st->pending == p.it && p.phase != PH_INIT_A;
+        if (trans != TRK) return;
         if (trans) nbn = p.plans[p.st->pending_widx].nb;
     }
 
@@ -252,9 +270,9 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
     {
         const int* src = reinterpret_cast<const int*>(p.st ? p.plans + widx : &p.plan0);
         if (tid < (int)(sizeof(DevPlan) / 4)) reinterpret_cast<int*>(&s_pl)[tid] = src[tid];
-        if (tid < RT_MAXW) {
-            s_dest[tid] = trans ? p.st->dest[tid] : -1;
-            s_ret[tid] = trans ? p.st->ret_dst[tid] : -1;
+        if (TRK && tid < RT_MAXW) {
+            s_dest[tid] = p.st->dest[tid];
+            s_ret[tid] = p.st->ret_dst[tid];
         }
     }
     __syncthreads();
@@ -459,6 +477,7 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
             }
             const int d0 = TR ? s_dest[col] : -1, d1 = TR ? s_dest[col + 1] : -1;   // columns in the new set
             const int r0 = TR ? s_ret[col] : -1, r1 = TR ? s_ret[col + 1] : -1;     // caller's columns of leaving ones
+            const bool pair16 = TR && d0 >= 0 && !(d0 & 1) && d1 == d0 + 1;
             int gsrc0 = -1, gsrc1 = -1;
             float2 gal0 = make_float2(0.f, 0.f), gal1 = gal0;
             if (MODE == MODE_G && p.gsrc) {
@@ -583,10 +602,8 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
                             } else {
                                 // pass A of a re-packing iteration: the new V and a copy of U (its centre
                                 // value is in registers) go to the new set
-                                put_col(nV, offn, d0, rr.x, rr.y, pol_st);
-                                put_col(nV, offn, d1, rr.z, rr.w, pol_st);
-                                put_col(nU, offn, d0, cc.x, cc.y, pol_st);
-                                put_col(nU, offn, d1, cc.z, cc.w, pol_st);
+                                put_pair(nV, offn, d0, d1, pair16, rr, pol_st);
+                                put_pair(nU, offn, d0, d1, pair16, cc, pol_st);
                             }
                             acc32[0] += fmaf(rr.x, rr.x, rr.y * rr.y);
                             acc32[1] += fmaf(rr.z, rr.z, rr.w * rr.w);
@@ -611,10 +628,8 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
                                 } else {
                                     // pass F of a re-packing iteration: X and W go to the new set; a column
                                     // that leaves has just received its last update, x_k = X + cx W
-                                    put_col(nX, offn, d0, xn.x, xn.y, pol_st);
-                                    put_col(nX, offn, d1, xn.z, xn.w, pol_st);
-                                    put_col(nW, offn, d0, wn.x, wn.y, pol_st);
-                                    put_col(nW, offn, d1, wn.z, wn.w, pol_st);
+                                    put_pair(nX, offn, d0, d1, pair16, xn, pol_st);
+                                    put_pair(nW, offn, d0, d1, pair16, wn, pol_st);
                                     const size_t offo = (size_t)cell * p.fin.nb_out;
                                     if (r0 >= 0) stg64_hint(p.u_out + offo + r0, xn.x, xn.y, pol_st);
                                     if (r1 >= 0) stg64_hint(p.u_out + offo + r1, xn.z, xn.w, pol_st);
@@ -652,7 +667,7 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
         for (int t = blockIdx.x; t < geo.n_tiles; t += gridDim.x) {
             int chunk = t % pl.nchunk;
             if (warp_live) {
-                if (trans) {                                     // (a re-packing iteration always has its old stream)
+                if constexpr (TRK) {                             // (a re-packing iteration always has its old stream)
                     if (pl.m_tma) chunk = run_tile(TrueT{}, TrueT{}, TrueT{}, t);
                     else          chunk = run_tile(FalseT{}, TrueT{}, TrueT{}, t);
                 } else if (pl.m_tma) {
@@ -691,7 +706,7 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
                         const int4 en = (i == 0) ? own_nxt : __ldg(own + own_cur + i);
                         const int c = chunk * cb + s;
                         float2* vp = out + (size_t)en.y * nb + c;
-                        if (trans) {                             // V of this iteration lives in the new set
+                        if (TRK) {                               // V of this iteration lives in the new set
                             if (s_dest[c] < 0) return 0.0;       // (a column that leaves is no longer iterated)
                             vp = nV + (size_t)en.y * nbn + s_dest[c];
                         }
