@@ -193,8 +193,16 @@ __device__ __forceinline__ void put_pair(float2* base, size_t cell_off, int d0, 
 __device__ __forceinline__ void consumer_sync(int nthreads) {
     asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory");
 }
-__device__ __forceinline__ float4 lds128(const unsigned char* base, int byte_off) {
-    return *reinterpret_cast<const float4*>(base + byte_off);
+// loads from the ring by 32-bit shared-space address (no generic-to-shared conversion per plane)
+__device__ __forceinline__ float4 lds128(uint32_t addr) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ float lds32(uint32_t addr) {
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+    return v;
 }
 __device__ __forceinline__ float4 f4add(const float4& a, const float4& b) {
     return make_float4(a.x + b.x, a.y + b.y, a.z + b.z, a.w + b.w);
@@ -414,6 +422,8 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
         const uint64_t pol_st = policy_evict_first();
         int stage = 0;
         uint32_t phase = 0;
+        uint32_t sb_cur = smem_u32(stages);                     // shared-space address of the stage in use
+        const uint32_t ring_b = (uint32_t)(nstage * STAGE_BYTES);
 
         // pass A: receivers inside this CTA's tiles (host-built per width, in tile order)
         int own_cur = 0, own_end = 0;
@@ -489,11 +499,11 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
             const int ixc = min(ix, p.nx - 1), iyc = min(iy, p.ny - 1);
             const float gxy = fmaxf(tab_g[ixc], tab_g[p.nx + iyc]);
             int cell = (z0 * p.ny + iyc) * p.nx + ixc;          // cell of the plane being emitted
-            size_t off = (size_t)cell * nb + col;               // its element offset
+            unsigned int off = (unsigned int)cell * nb + col;  // its element offset (< 2^31, checked by the host)
             float m_cur = 0.f, m_nxt = 0.f;
             float4 cA = f4zero(), cB = f4zero(), sA = f4zero(), sB = f4zero(), lap = f4zero();
             float acc32[2] = {0.f, 0.f};
-            const size_t plane_e = (size_t)p.nx * p.ny * nb;
+            const unsigned int plane_e = (unsigned int)(p.nx * p.ny) * nb;
             const int plane_m = p.nx * p.ny;
             const float* gz_tab = tab_g + p.nx + p.ny;
 
@@ -502,16 +512,16 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
             auto plane = [&](const int plz, float4& c_prev, float4& c_new, float4& s_prev, float4& s_new) {
                 if (!M_TMA && plz >= z0 && plz < z1) m_nxt = __ldg(p.m + cell + (plz > z0 ? plane_m : 0));
                 mbar_wait(full0 + 8 * stage, phase);
-                const unsigned char* sb = stages + stage * STAGE_BYTES;
-                c_new = lds128(sb, sm_ctr);
+                const uint32_t sb = sb_cur;                     // this stage's shared-space address
+                c_new = lds128(sb + sm_ctr);
                 float4 t_new;                                   // in-plane part of the stencil on plane plz
                 {
-                    const float4 a = lds128(sb, sm_ctr - CELL_B), b = lds128(sb, sm_ctr + CELL_B);
-                    const float4 c = lds128(sb, sm_ctr - ROW_B), d = lds128(sb, sm_ctr + ROW_B);
+                    const float4 a = lds128(sb + sm_ctr - CELL_B), b = lds128(sb + sm_ctr + CELL_B);
+                    const float4 c = lds128(sb + sm_ctr - ROW_B), d = lds128(sb + sm_ctr + ROW_B);
                     const float4 e4 = f4add(f4add(a, b), f4add(c, d));
                     if (STENCIL == ST_27) {
-                        const float4 a2 = lds128(sb, sm_ctr - ROW_B - CELL_B), b2 = lds128(sb, sm_ctr - ROW_B + CELL_B);
-                        const float4 c2 = lds128(sb, sm_ctr + ROW_B - CELL_B), d2 = lds128(sb, sm_ctr + ROW_B + CELL_B);
+                        const float4 a2 = lds128(sb + sm_ctr - ROW_B - CELL_B), b2 = lds128(sb + sm_ctr - ROW_B + CELL_B);
+                        const float4 c2 = lds128(sb + sm_ctr + ROW_B - CELL_B), d2 = lds128(sb + sm_ctr + ROW_B + CELL_B);
                         const float4 d4 = f4add(f4add(a2, b2), f4add(c2, d2));
                         s_new = make_float4(fmaf(p.a1, c_new.x, fmaf(p.a2, e4.x, p.a3 * d4.x)),
                                             fmaf(p.a1, c_new.y, fmaf(p.a2, e4.y, p.a3 * d4.y)),
@@ -528,15 +538,16 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
                 const bool emit = plz >= z0 + 1;
                 float4 o_old = f4zero();
                 if (emit) {
-                    if (HAS_OLD) o_old = lds128(sb, io);
-                    if (M_TMA) m_cur = *reinterpret_cast<const float*>(sb + mo);
+                    if (HAS_OLD) o_old = lds128(sb + io);
+                    if (M_TMA) m_cur = lds32(sb + mo);
                 }
                 // pass A / G: the stage is free once its loads are done.  Pass F reads W and X from
                 // the stage just before it uses them (fewer live registers) and releases it after.
                 auto release = [&]() {
                     __syncwarp();
                     if ((tid & 31) == 0) mbar_arrive(empty0 + 8 * stage);
-                    if (++stage == nstage) { stage = 0; phase ^= 1; }
+                    sb_cur += STAGE_BYTES;
+                    if (++stage == nstage) { stage = 0; phase ^= 1; sb_cur -= ring_b; }
                 };
                 if (MODE != MODE_F) release();
 
@@ -610,8 +621,8 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
                             if (MODE == MODE_F) {
                                 float4 o_w = f4zero(), o_x = f4zero();
                                 if (has_wx) {
-                                    o_w = lds128(sb, io + CTR_SPAN);
-                                    o_x = lds128(sb, io + 2 * CTR_SPAN);
+                                    o_w = lds128(sb + io + CTR_SPAN);
+                                    o_x = lds128(sb + io + 2 * CTR_SPAN);
                                 }
                                 float4 xn, wn;
                                 xn.x = fmaf(cx[0], o_w.x, o_x.x);
