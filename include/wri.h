@@ -96,13 +96,12 @@ int wri_set_stencil(wri_ctx* ctx, int32_t stencil);
  *   nstage_f / nstage_a   depth of the shared-memory ring of the forward / adjoint pass
  *   zc_f / zc_a           planes per tile
  *   txc / tyc             cells per tile in x / y
- *   no_compact            keep converged columns in the working set (they stay frozen)
+ *   no_compact            keep converged columns in the working set (they stay frozen, no re-packing)
  *   no_groups             run a batch wider than 64 columns in lock-step instead of 64-column groups
- *   generic               use the plain (non-TMA) kernels for every width
- *   no_graph              enqueue the iterations one by one instead of the device-side loop        */
+ *   generic               use the plain (non-TMA) kernels for every width                          */
 typedef struct {
     int32_t nstage_f, nstage_a, zc_f, zc_a, txc, tyc;
-    int32_t no_compact, no_groups, generic, no_graph;
+    int32_t no_compact, no_groups, generic;
 } wri_debug_opts;
 int wri_set_debug_opts(wri_ctx* ctx, const wri_debug_opts* opts);
 
@@ -151,10 +150,12 @@ int wri_apply_MH(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_host, float 
  * Equivalent to wri_lsqr_begin + wri_lsqr_iterate(maxit) + wri_lsqr_end.  Needs a workspace.
  * The call only enqueues work, with or without tolerances: the state of the solve (iteration
  * count, active flags, working width) lives on the device.  With tolerances the finaliser of
- * each iteration counts the live columns; once the bandwidth spent on stopped ones exceeds the
- * price of re-packing, a kernel compacts them out of the working set (adaptive accuracy,
- * PAPER.md:180-211; "the active mask shrinking as sources converge", BASELINE.json configs[3]),
- * and once every column has stopped the remaining launches return at once.                   */
+ * each iteration counts the live columns; as soon as they fit a narrower (even) width, the two
+ * passes of the next iteration store their results into a second vector set at that width, so
+ * stopped columns leave the working set without a separate pass over the vectors (adaptive
+ * accuracy; "the active mask shrinking as sources converge", BASELINE.json
+ * configs[3]); once every column has stopped the remaining launches return at once.  A column's
+ * result does not depend on the batch it runs in (bit-identical with and without re-packing). */
 int wri_lsqr_batch(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_host,
                    const void* q_dev, const void* d_dev, float lambda,
                    const float* tol_dev, int32_t maxit,

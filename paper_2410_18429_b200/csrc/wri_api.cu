@@ -126,9 +126,6 @@ struct wri_ctx {
         wri_debug_opts dbg{};
     } plan_key;
     bool plan_valid = false;
-    // device-side loop (CUDA graph with a conditional WHILE node), rebuilt per solve
-    cudaGraph_t graph = nullptr;
-    cudaGraphExec_t graph_exec = nullptr;
     // optional per-kernel timing (wri_profile_*)
     bool profiling = false;
     std::vector<cudaEvent_t> ev_pool;     // pairs: start, stop
@@ -426,15 +423,15 @@ int rt_chunk_for(const wri_ctx* c, int nb) {
 
 // planes per tile and tile count of one pass.  With plenty of tiles the measured preferences hold
 // (profiles/r02_width_sweeps.md; an L2 effect: short tiles keep the halo that neighbouring tiles share
-// resident across a wave of tiles): pass F 16 planes — except 128 at one 32-column chunk per cell on grids
-// of 256 planes and more (profiles/r01_v6_stages.md) —, pass A 16 planes up to 24 columns, 32 beyond.  With
+// resident across a wave of tiles): pass F 16 planes; pass A 16 planes up to 24 columns and on grids of
+// 256 planes and more (256^3 x 32: 0.93 -> 1.00 of the copy bandwidth), 32 otherwise.  With
 // few tiles (narrow widths, small grids) the chunk count that minimises rounds x (planes + priming)
 // over the persistent grid is taken instead.
 PassGeo plan_pass(const wri_ctx* c, const DevPlan& P, bool is_f, int zc_forced) {
     PassGeo G{};
     const int nz = c->g.nz, sms = std::max(1, c->num_sms);
     const long long cols = (long long)P.nchunk * P.ntx * P.nty;
-    int zc = is_f ? ((P.cb == 32 && nz >= 256) ? 128 : 16) : (P.cb <= 24 ? 16 : 32);
+    int zc = is_f ? 16 : ((P.cb <= 24 || nz >= 256) ? 16 : 32);
     if (zc_forced > 0) zc = (zc_forced + 7) / 8 * 8;          // multiples of 8 planes (see the |.|^2 sums of the kernel)
     else if (cols * ((nz + zc - 1) / zc) < 6LL * sms) {
         const double prime = is_f ? 0.6 : 1.2;               // two priming planes in units of a full step
@@ -474,13 +471,19 @@ int make_plan(const wri_ctx* c, int nb, DevPlan& P) {
                                      3 * align_up((size_t)txc * tyc * cb * 8, 128) + 128;
                 if (2 * stage + 24576 > (size_t)RT_SMEM_MAX) continue;
                 const double ntx = (nx + txc - 1) / txc, nty = (ny + tyc - 1) / tyc;
-                double cost = ntx * nty * ((txc + 2.0) * (tyc + 2.0) + 0.75 * maxcells);
+                // (from 16 columns on idle consumer threads cost little — 384 busy ones keep pass A at its
+                // rate — and contiguous tile rows below 2 KB cost a lot: 48 columns as 8 x 2 cells run 4 %
+                // faster than as 4 x 5, profiles/r02_width_sweeps.md)
+                double cost = ntx * nty * ((txc + 2.0) * (tyc + 2.0) + (cb >= 16 ? 0.25 : 0.75) * maxcells);
                 const int row_bytes = txc * cb * 8;
                 if (row_bytes < 512 && txc < nx) cost *= 1.0 + 0.25 * (512 - row_bytes) / 512.0;
+                if (cb >= 16 && row_bytes < 2048 && txc < nx) cost *= 1.0 + (2048 - row_bytes) / 2048.0;
+                // below 32 columns a box row should carry (column, x) folded into one dimension
+                if (cb < 32 && !(P.nchunk == 1 && cb * (txc + 2) <= 256)) cost *= 1.2;
                 // tile rows that do not start on 128-byte lines: measured 6-10 % slower in both passes
                 // (widths 6, 10: profiles/r02_width_sweeps.md)
                 if (row_bytes % 128 != 0 && txc < nx) cost *= 1.12;
-                if (!(m_al && txc % 4 == 0)) cost *= 1.15;   // model tile by plain loads: measured slower
+                if (!(m_al && txc % 4 == 0)) cost *= 1.3;    // model tile by plain loads: pass A 0.98 -> 0.80 at 48 columns
                 if (cost < best) { best = cost; btx = txc; bty = tyc; }
             }
     P.txc = btx; P.tyc = bty;
@@ -499,18 +502,20 @@ int make_plan(const wri_ctx* c, int nb, DevPlan& P) {
     P.m_span = (int)align_up(P.m_bytes, 128);
     P.f = plan_pass(c, P, true, c->dbg.zc_f);
     P.a = plan_pass(c, P, false, c->dbg.zc_a);
-    // ring depth: near 120 KB (pass F) / 150 KB (pass A) of stages in flight per SM (measured optima,
+    // ring depth of pass A: near 150 KB of stages in flight per SM (measured optimum,
     // profiles/r01_v6_stages.md: a deeper ring costs L2 hits on the stencil halo, a shallower one
     // leaves the copy engine idle), within the shared memory that is left
     const int nxyz = c->g.nx + c->g.ny + c->g.nz;
     auto depth = [&](int nstream, double target, int lo, int hi, int forced) {
         const int stage = rt_stage_bytes(P, nstream);
-        int n = forced > 0 ? forced : (int)std::floor(target / stage + 0.5);
-        n = std::max(lo, std::min(n, hi));
+        int n = forced > 0 ? std::min(forced, RT_MAX_STAGES)
+                           : std::max(lo, std::min((int)std::floor(target / stage + 0.5), hi));
         while (n > 2 && rt_smem_bytes(P, nstream, n, nxyz) > (size_t)RT_SMEM_MAX) --n;
         return n;
     };
-    P.f.nstage = depth(3, 120e3, 2, 4, c->dbg.nstage_f);
+    // pass F: three stages.  A fourth costs 4-8 % wherever the stage is small enough to afford it (widths
+    // 18, 22, 26, 34, 44, 46: profiles/r02_width_sweeps.md) — more loads in flight than the L2 keeps halos for
+    P.f.nstage = depth(3, 120e3, 2, cb < 8 ? 4 : 3, c->dbg.nstage_f);
     P.a.nstage = depth(1, 150e3, 3, 10, c->dbg.nstage_a);
     if (rt_smem_bytes(P, 3, P.f.nstage, nxyz) > (size_t)RT_SMEM_MAX) return WRI_ERR_ARG;
     return WRI_OK;
@@ -957,8 +962,6 @@ int wri_destroy(wri_ctx* c) {
     if (c->h_aw) cudaFreeHost(c->h_aw);
     cudaFree(c->d_plans); cudaFree(c->d_maps); cudaFree(c->d_mmaps); cudaFree(c->d_own_ptr); cudaFree(c->d_own);
     cudaFree(c->d_state); cudaFree(c->d_prof);
-    if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
-    if (c->graph) cudaGraphDestroy(c->graph);
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
     for (auto& sl : c->pipe) {
         if (sl.ev_in) cudaEventDestroy(sl.ev_in);

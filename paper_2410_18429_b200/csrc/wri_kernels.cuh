@@ -380,7 +380,7 @@ struct ScalParams {
     double* ar0_out;          // [nb] or null: alpha1 beta1 of this solve
     const unsigned char* rmask;   // [n_rec][nb_out] per-source receiver sets by the CALLER's column, or null
     // device-resident solve state (persistent pass kernel): iteration counter, active count, the
-    // decision to re-pack the working set (PH_A), the condition of the device-side loop
+    // decision to re-pack the working set (PH_A)
     SolveState* st;           // null: host-sequenced solve (generic kernels)
     int adaptive;             // PH_A may ask for a re-packing of the working set
     int widx;                 // index of the current width's plan
@@ -391,7 +391,6 @@ struct ScalParams {
     float* coef2; double* stat2; int* active2; int* iters2;   // the other bank
     float2* U_bot2;
     int init_rows;            // PH_INIT_B: k_init_rows has formed U_bot; its |.|^2 sums are extra rows of partials
-    void* cond;               // cudaGraphConditionalHandle or null
 };
 
 // sum over tiles of partials[.][s] in fixed order; result for column s in colsum[s] (shared)
@@ -673,11 +672,6 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
                 st->pending = p.k + 1;          // the passes of the next iteration re-pack
             }
         }
-#if defined(__CUDACC__)
-        if (p.cond)
-            cudaGraphSetConditional((cudaGraphConditionalHandle)(uintptr_t)p.cond,
-                                    (st->all_done || p.k >= p.maxit) ? 0u : 1u);
-#endif
     }
 
     if (PHASE == PH_A && p.st && p.trans) {

@@ -69,8 +69,6 @@ struct RtParams {
     float* g;                         // [n_g] this batch's gradient (overwritten) or null
     float lam2;
     int it;                           // iteration this launch belongs to (host count, 1-based)
-    void* cond;                       // cudaGraphConditionalHandle of the device-side loop (0 = none)
-    int cond_set;                     // this launch's finaliser decides whether the loop goes on
 };
 
 template <int MODE> struct RtTraits;
@@ -771,7 +769,6 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
             f.nb_new = nbn;
             f.coef2 = p.coef[par ^ 1]; f.stat2 = p.stat[par ^ 1]; f.active2 = p.active[par ^ 1];
             f.iters2 = p.iters[par ^ 1]; f.U_bot2 = p.U_bot[par ^ 1];
-            f.cond = p.cond_set ? p.cond : nullptr;
             switch (p.phase) {
                 case PH_INIT_A: finalize_phase<PH_INIT_A>(f, sh); break;
                 case PH_F:      finalize_phase<PH_F>(f, sh); break;
