@@ -90,6 +90,9 @@ struct wri_ctx {
     bool packed = false;            // the working set has a column map; X lives in the workspace
     bool adaptive = false;          // converged columns are compacted away on the device
     float2* u_out = nullptr;
+    float2* retire_buf = nullptr;   // adaptive: workspace region [caller's column][cell] for the x of retired columns
+    int* retired = nullptr;         // [nb_max] device flags by the caller's column
+    int col0 = 0, ncols = 0;        // this group's columns of the caller's batch
     float lambda = 0;
     float2* vec[2][4] = {};         // per parity: U, V, W, X
     float2* U_bot[2] = {nullptr, nullptr};
@@ -200,7 +203,7 @@ GradTiling make_grad_tiling(const wri_ctx* c, int nb) {
 // WS_COMPACTION five more (the working set of an adaptive solve keeps X in the workspace and has a
 // second vector set to re-pack into), with WS_HOST_STAGING the device copy of x for the host entry.
 struct WsLayout {
-    size_t vecs[8], U_bot, partials, partials_rt, gscratch, Xs, Ds, tols, res, its, alphas, U_bot2, total;
+    size_t vecs[9], U_bot, partials, partials_rt, gscratch, Xs, Ds, tols, res, its, alphas, U_bot2, total;
     int n_vecs;
 };
 enum { WS_HOST_STAGING = 1, WS_COMPACTION = 2 };
@@ -228,8 +231,8 @@ WsLayout ws_layout(const wri_ctx* c, int nb, int flags, int maxit_cap) {
         L.alphas = o; o += align_up((size_t)nbe * sizeof(float2), 256);
     }
     if (flags & WS_COMPACTION) {
-        for (int i = 3; i < 8; ++i) { L.vecs[i] = o; o += vec; }
-        L.n_vecs = 8;
+        for (int i = 3; i < 9; ++i) { L.vecs[i] = o; o += vec; }   // [8]: final x of retired columns
+        L.n_vecs = 9;
         L.U_bot2 = o; o += bot;
     }
     L.total = o;
@@ -714,7 +717,7 @@ RtParams rt_solve_params(const wri_ctx* c, int phase) {
     p.has_old = (MODE == MODE_A) ? (phase != PH_INIT_A) : 1;
     p.lazy = c->lazy;
     p.packed = c->packed; p.adaptive = c->adaptive;
-    p.u_out = c->u_out;
+    p.retire_buf = c->retire_buf; p.retired = c->retired;
     p.maxit = c->maxit;
     p.n_rec = c->n_rec; p.rec = c->rec;
     p.fin = scal_params(c, c->partials_rt, rt_grid(c), nullptr);
@@ -762,6 +765,9 @@ MoveParams move_params(const wri_ctx* c) {
     p.u_out = c->u_out; p.resnorms = c->resnorms;
     p.n_g = (long long)c->ng; p.nb_out = c->nb0; p.nb_max = c->nb_max; p.maxit = c->maxit; p.n_rec = c->n_rec;
     p.packed = c->packed;
+    p.R = c->adaptive ? c->retire_buf : nullptr;
+    p.retired = c->retired;
+    p.col0 = c->col0; p.ncols = c->ncols;
     return p;
 }
 
@@ -931,6 +937,7 @@ int wri_create(wri_ctx** out, wri_grid grid, double h, int32_t n_omega, const do
         CKC(cudaMemset(c->iters[b], 0, NM * sizeof(int)));
     }
     CKC(cudaMalloc(&c->colmap, NM * sizeof(int)));
+    CKC(cudaMalloc(&c->retired, NM * sizeof(int)));
     CKC(cudaMalloc(&c->src, NM * sizeof(int)));
     CKC(cudaMalloc(&c->aw_tol, NM * sizeof(float)));
     CKC(cudaMalloc(&c->aw_f, (size_t)2 * NM * sizeof(double)));
@@ -957,7 +964,7 @@ int wri_destroy(wri_ctx* c) {
     if (!c) return WRI_OK;
     cudaFree(c->gtab); cudaFree(c->rec); cudaFree(c->counter);
     for (int b = 0; b < 2; ++b) { cudaFree(c->coef[b]); cudaFree(c->stat[b]); cudaFree(c->active[b]); cudaFree(c->iters[b]); }
-    cudaFree(c->colmap); cudaFree(c->src);
+    cudaFree(c->colmap); cudaFree(c->src); cudaFree(c->retired);
     cudaFree(c->aw_tol); cudaFree(c->aw_f); cudaFree(c->aw_ar0); cudaFree(c->aw_iters);
     if (c->h_aw) cudaFreeHost(c->h_aw);
     cudaFree(c->d_plans); cudaFree(c->d_maps); cudaFree(c->d_mmaps); cudaFree(c->d_own_ptr); cudaFree(c->d_own);
@@ -1260,6 +1267,9 @@ int lsqr_begin_impl(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const
     c->partials = (double*)(c->ws + L.partials);
     c->partials_rt = (double*)(c->ws + L.partials_rt);
     c->u_out = (float2*)u_out_dev;
+    c->col0 = col0; c->ncols = ncols;
+    c->retire_buf = ws_big ? (float2*)(c->ws + L.vecs[8]) : nullptr;
+    if (adaptive) CK(cudaMemsetAsync(c->retired, 0, c->nb_max * sizeof(int), c->stream));
     std::memset(c->vec, 0, sizeof c->vec);
     for (int q = 0; q < 3; ++q) c->vec[0][q] = slots[q];
     c->vec[0][3] = packed ? slots[3] : (float2*)u_out_dev;

@@ -390,6 +390,7 @@ struct ScalParams {
     int nb_new;               // width of the new working set
     float* coef2; double* stat2; int* active2; int* iters2;   // the other bank
     float2* U_bot2;
+    int* retired;             // [nb_out] by the CALLER's column: its final x sits in the side buffer (adaptive solves)
     int init_rows;            // PH_INIT_B: k_init_rows has formed U_bot; its |.|^2 sums are extra rows of partials
 };
 
@@ -696,6 +697,8 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
             const int m = st->map[(int)(i - r * nbn)];
             p.U_bot2[i] = m >= 0 ? p.U_bot[r * nb + m] : make_float2(0.f, 0.f);
         }
+        for (int s = threadIdx.x; s < nb; s += blockDim.x)
+            if (st->ret_dst[s] >= 0) p.retired[st->ret_dst[s]] = 1;
         if (p.resnorms)
             for (long long i = threadIdx.x; i < (long long)(p.maxit - p.k) * nb; i += blockDim.x) {
                 const int row = (int)(i / nb), s = (int)(i - (long long)row * nb);
@@ -761,6 +764,11 @@ struct MoveParams {
     long long n_g;
     int nb_out, nb_max, maxit, n_rec;
     int packed;
+    // adaptive solves: the final x of the columns that left the working set, column by column
+    // ([caller's column][cell]), and which columns those are; this group's columns of the caller's batch
+    const float2* R;
+    const int* retired;
+    int col0, ncols;
 };
 
 // End of a solve: the last deferred update x_k = X + cx W is applied and, where the working set has
@@ -783,6 +791,45 @@ k_finish(const MoveParams p) {
         __syncthreads();
         const float2* X = p.vec[a][3];
         const float2* W = p.vec[a][2];
+        if (p.R) {
+            // adaptive solve: the caller's rows are put together in shared memory, 32 cells at a time —
+            // the columns still in the working set from X (+ cx W), the ones that left from the side
+            // buffer (read along the cells) — and written as whole rows: full sectors both ways
+            constexpr int CH = 32;
+            __shared__ float2 tile[CH][RT_MAXW + 1];
+            __shared__ int s_ok[RT_MAXW];
+            const int ncols = p.ncols, col0 = p.col0;
+            if (threadIdx.x < RT_MAXW) s_ok[threadIdx.x] = threadIdx.x < ncols && p.retired[col0 + threadIdx.x] ? 2 : 0;
+            __syncthreads();
+            if (threadIdx.x < nb && s_cm[threadIdx.x] >= 0) s_ok[s_cm[threadIdx.x] - col0] = 1;
+            __syncthreads();
+            for (long long c0 = (long long)blockIdx.x * CH; c0 < p.n_g; c0 += (long long)gridDim.x * CH) {
+                const int nc = (int)min((long long)CH, p.n_g - c0);
+                for (int idx = threadIdx.x; idx < nc * nb; idx += blockDim.x) {
+                    const int c = idx / nb, j = idx - c * nb, so = s_cm[j];
+                    if (so < 0) continue;
+                    const long long i = (c0 + c) * nb + j;
+                    float2 x = __ldcs(X + i);
+                    const float cx = s_cx[j];
+                    if (cx != 0.f) {
+                        const float2 w = __ldcs(W + i);
+                        x.x = fmaf(cx, w.x, x.x);
+                        x.y = fmaf(cx, w.y, x.y);
+                    }
+                    tile[c][so - col0] = x;
+                }
+                for (int idx = threadIdx.x; idx < ncols * CH; idx += blockDim.x) {
+                    const int jj = idx / CH, t = idx - jj * CH;
+                    if (s_ok[jj] == 2 && t < nc) tile[t][jj] = __ldcs(p.R + (size_t)(col0 + jj) * p.n_g + c0 + t);
+                }
+                __syncthreads();
+                for (int idx = threadIdx.x; idx < nc * ncols; idx += blockDim.x) {
+                    const int c = idx / ncols, jj = idx - c * ncols;
+                    if (s_ok[jj]) p.u_out[(c0 + c) * p.nb_out + col0 + jj] = tile[c][jj];
+                }
+                __syncthreads();
+            }
+        } else
         for (long long i = g0; i < p.n_g * nb; i += gs) {
             const long long c = i / nb;
             const int j = (int)(i - c * nb), so = s_cm[j];

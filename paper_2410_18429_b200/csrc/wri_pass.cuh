@@ -56,7 +56,9 @@ struct RtParams {
     int lazy;                         // MODE_F: W and X are known to be zero before the first iteration
     int packed;                       // the working set has a column map (grouped / adaptive solves)
     int adaptive;                     // the finaliser may decide to re-pack the working set (both vector sets exist)
-    float2* u_out;                    // adaptive: caller's [n_g][nb_out] wavefields (final x of the columns that leave)
+    int* retired;                     // adaptive: [nb_out] flags by the caller's column, set when a column leaves
+    float2* retire_buf;               // adaptive: [caller's column][cell] final x of the columns that leave (k_finish
+                                      // moves them to the caller's u_out as whole rows)
     int maxit;
     int n_rec;
     const int* rec;                   // [n_rec] cell indices
@@ -486,6 +488,7 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
             const int d0 = TR ? s_dest[col] : -1, d1 = TR ? s_dest[col + 1] : -1;   // columns in the new set
             const int r0 = TR ? s_ret[col] : -1, r1 = TR ? s_ret[col + 1] : -1;     // caller's columns of leaving ones
             const bool pair16 = TR && d0 >= 0 && !(d0 & 1) && d1 == d0 + 1;
+            const size_t n_g = (size_t)p.nx * p.ny * p.nz;
             int gsrc0 = -1, gsrc1 = -1;
             float2 gal0 = make_float2(0.f, 0.f), gal1 = gal0;
             if (MODE == MODE_G && p.gsrc) {
@@ -639,9 +642,11 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
                                     // that leaves has just received its last update, x_k = X + cx W
                                     put_pair(nX, offn, d0, d1, pair16, xn, pol_st);
                                     put_pair(nW, offn, d0, d1, pair16, wn, pol_st);
-                                    const size_t offo = (size_t)cell * p.fin.nb_out;
-                                    if (r0 >= 0) stg64_hint(p.u_out + offo + r0, xn.x, xn.y, pol_st);
-                                    if (r1 >= 0) stg64_hint(p.u_out + offo + r1, xn.z, xn.w, pol_st);
+                                    // (column by column in a side buffer: the threads of neighbouring cells
+                                    // fill its sectors; straight into u_out these would be 8-byte pieces
+                                    // of 32-byte sectors, read-modify-write in DRAM)
+                                    if (r0 >= 0) stg64_hint(p.retire_buf + (size_t)r0 * n_g + cell, xn.x, xn.y, pol_st);
+                                    if (r1 >= 0) stg64_hint(p.retire_buf + (size_t)r1 * n_g + cell, xn.z, xn.w, pol_st);
                                 }
                             }
                         }
@@ -769,6 +774,7 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
             f.nb_new = nbn;
             f.coef2 = p.coef[par ^ 1]; f.stat2 = p.stat[par ^ 1]; f.active2 = p.active[par ^ 1];
             f.iters2 = p.iters[par ^ 1]; f.U_bot2 = p.U_bot[par ^ 1];
+            f.retired = p.retired;
             switch (p.phase) {
                 case PH_INIT_A: finalize_phase<PH_INIT_A>(f, sh); break;
                 case PH_F:      finalize_phase<PH_F>(f, sh); break;
