@@ -739,14 +739,23 @@ int launch_rt(wri_ctx* c, int phase) {
     cudaEvent_t e1 = nullptr;
     if (phase != PH_INIT_A && (rc = profile_event_begin(c, MODE == MODE_F ? 0 : 1, &e1))) return rc;
     void* args[] = {&dummy, &dummy, &dummy, &p};
-    CK(cudaLaunchKernel(fn, dim3(rt_grid(c)), dim3(RT_NT + 32), args, smem, c->stream));
+    // programmatic dependent launch: the next pass's CTAs move in while this one's last CTA still runs
+    // its finaliser, and wait (griddepcontrol.wait at the top of the kernel) for the launch to complete
+    cudaLaunchAttribute attr{};
+    attr.id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr.val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(rt_grid(c)); cfg.blockDim = dim3(RT_NT + 32);
+    cfg.dynamicSmemBytes = smem; cfg.stream = c->stream;
+    cfg.attrs = &attr; cfg.numAttrs = 1;
+    CK(cudaLaunchKernelExC(&cfg, fn, args));
     c->launches++;
     if (c->adaptive && phase != PH_INIT_A) {
         // the re-packing variant of the same pass: exactly one of the two does the work (decided on the
         // device from the solve state), the other returns at once
         const void* fn_t = rt_kernel<MODE, true>(c);
         if ((rc = allow_smem(c, fn_t, smem))) return rc;
-        CK(cudaLaunchKernel(fn_t, dim3(rt_grid(c)), dim3(RT_NT + 32), args, smem, c->stream));
+        CK(cudaLaunchKernelExC(&cfg, fn_t, args));
         c->launches++;
     }
     if (e1) CK(cudaEventRecord(e1, c->stream));

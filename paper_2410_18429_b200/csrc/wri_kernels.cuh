@@ -394,13 +394,15 @@ struct ScalParams {
     int init_rows;            // PH_INIT_B: k_init_rows has formed U_bot; its |.|^2 sums are extra rows of partials
 };
 
-// sum over tiles of partials[.][s] in fixed order; result for column s in colsum[s] (shared)
+// sum over tiles of partials[.][s] in fixed order; result for column s in colsum[s] (shared).
+// Runs while every other SM waits (last CTA of a pass), so the loads are issued four at a time and the
+// groups are folded in two levels (groups of 8, then those): the longest dependent chain is
+// n_tiles / Gc / 4 load rounds + Gc / 8 + 8 additions instead of n_tiles / Gc + Gc.
 __device__ __forceinline__ void reduce_partials(const ScalParams& p, double* scratch, double* colsum) {
     const int nb = p.nb, T = blockDim.x;
-    const int G = max(1, T / nb);
     for (int base = 0; base < nb; base += T) {           // nb > T handled in column chunks
         const int ncol = min(nb - base, T);
-        const int g = threadIdx.x / ncol, s = base + threadIdx.x % ncol;
+        const int g = threadIdx.x / ncol, cl = threadIdx.x % ncol, s = base + cl;
         const int Gc = max(1, T / ncol);
         double a = 0.0;
         if (g < Gc) {
@@ -412,18 +414,35 @@ __device__ __forceinline__ void reduce_partials(const ScalParams& p, double* scr
 #pragma unroll
                 for (int j = 0; j < 8; ++j) a += t[j];
             }
-            for (; b < p.n_tiles; b += Gc) a += __ldcg(p.partials + (size_t)b * nb + s);
+            for (; b < p.n_tiles; b += 4 * Gc) {                     // the rest, still four at a time
+                double t[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+                    t[j] = (b + j * Gc < p.n_tiles) ? __ldcg(p.partials + (size_t)(b + j * Gc) * nb + s) : 0.0;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) a += t[j];
+            }
         }
         scratch[threadIdx.x] = a;
         __syncthreads();
+        int ng = Gc;                                                 // groups left to fold
+        if (Gc > 8) {
+            const int h = threadIdx.x / ncol;                        // thread (h, cl), h < 8: groups h, h + 8, ...
+            double t = 0.0;
+            if (h < 8)
+                for (int gg = h; gg < Gc; gg += 8) t += scratch[gg * ncol + cl];
+            __syncthreads();
+            if (h < 8) scratch[h * ncol + cl] = t;
+            __syncthreads();
+            ng = 8;
+        }
         if (threadIdx.x < ncol) {
             double t = 0.0;
-            for (int gg = 0; gg < Gc; ++gg) t += scratch[gg * ncol + threadIdx.x];
+            for (int gg = 0; gg < ng; ++gg) t += scratch[gg * ncol + threadIdx.x];
             colsum[base + threadIdx.x] = t;
         }
         __syncthreads();
     }
-    (void)G;
 }
 
 // fixed-order sum over receivers of |U_bot[r][s]|^2, added to colsum[s]
@@ -459,6 +478,20 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
     const int nb = p.nb, NM = p.nb_max;
     float* cf = p.coef;
     double* st = p.stat;
+
+    // The per-column state is needed after the partial sums have been folded; asking for it now lets
+    // those trips to L2 overlap (this code runs in one CTA while the rest of the grid has finished).
+    if ((PHASE == PH_F || PHASE == PH_A) && threadIdx.x < nb) {
+        const int s = threadIdx.x;
+        auto pf = [](const void* a) { asm volatile("prefetch.global.L1 [%0];" ::"l"(a)); };
+        pf(p.active + s);
+        if (p.colmap) pf(p.colmap + s);
+        if (p.tol) pf(p.tol + s);
+#pragma unroll
+        for (int r = S_ALPHA; r <= S_AR0; ++r) pf(st + r * NM + s);
+        if (p.src) pf(st + S_VA_RE * NM + s);
+        pf(cf + (PHASE == PH_F ? C_CA_F : C_CA_A) * NM + s);
+    }
 
     const long long nrs = (long long)p.n_rec * nb;
     if (PHASE == PH_INIT_B && !p.init_rows) {

@@ -246,6 +246,11 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
 
     // ---- state of the solve in flight (uniform over the grid; written only by finalisers of
     //      earlier launches and by the compaction kernel)
+    // Programmatic dependent launch: the passes of a solve are enqueued with the stream-serialisation
+    // attribute, so a CTA of the next launch may take an SM as soon as this launch's CTA there has left;
+    // it waits here until the whole launch before it has completed and its writes are visible.  (Without
+    // the attribute both instructions do nothing.)
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     int par = 0, widx = 0, k_done = 0, nbn = 0;
     bool trans = false;
     if (p.st) {
@@ -749,6 +754,7 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
     }
 
     // ---------------------------------------------------------------------- CTA epilogue
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     __syncthreads();
     if (p.partials)
         for (int j = tid; j < nb; j += blockDim.x) p.partials[(size_t)blockIdx.x * nb + j] = colacc[j];
