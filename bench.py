@@ -339,6 +339,7 @@ def run_ours(args, wl_name, w):
     ms_f, n_f, cols_f, ms_a, n_a, cols_a = ctx.profile_read()
     ctx.profile_enable(False)
     clocks = sampler.stop() if rank == 0 else None
+    time.sleep(0.3)          # let nvidia-smi go: its start-up and exit stall launches for tens of ms on a short run
 
     # ---- end-to-end timing through the host-buffer entry
     qh = torch.from_numpy(w.Q).pin_memory()
@@ -418,7 +419,7 @@ def run_ours(args, wl_name, w):
         yt = torch.empty_like(u_sf)
         ctx.apply_M(u_sf, w.lam, w.omega_idx, out=(yt, yb)); ctx.apply_MH(u_sf, yb, w.lam, w.omega_idx, out=yt)
         torch.cuda.synchronize()
-        n_ap = 5
+        n_ap = 20
         ev2[0].record()
         for _ in range(n_ap):
             ctx.apply_M(u_sf, w.lam, w.omega_idx, out=(yt, yb))

@@ -114,11 +114,12 @@ int wri_plan_info(wri_ctx* ctx, int32_t nb, int32_t* out16);
 
 /* Workspace for wri_lsqr_* at batch width nb (u, v, w vectors, receiver rows, reduction
  * partials).  flags: WRI_WS_HOST_STAGING adds room for the device copies wri_lsqr_batch_host
- * needs; WRI_WS_COMPACTION adds five more vectors: with per-column tolerances the working set then
- * lives entirely in the workspace and has a second vector set, so that converged columns can be
+ * needs; WRI_WS_COMPACTION adds six more vectors: with per-column tolerances the working set then
+ * lives entirely in the workspace, has a second vector set and a side buffer, so that converged columns can be
  * compacted out of it on the device (without it such a solve still stops early once every column
- * has converged, but converged columns keep costing bandwidth); an odd batch width uses one of them
- * to run in an even-width working set on the fast kernel.
+ * has converged, but converged columns keep costing bandwidth).  An odd batch width is given one
+ * spare vector (two with host staging) whatever the flags: wri_lsqr_batch runs it in an even-width
+ * working set on the fast kernel.
  * The caller allocates (e.g. a torch uint8 tensor) and hands it over; it must stay alive and
  * untouched while a solve is in flight.                                                      */
 #define WRI_WS_HOST_STAGING 1

@@ -199,8 +199,8 @@ GradTiling make_grad_tiling(const wri_ctx* c, int nb) {
     return G;
 }
 
-// Caller's workspace.  Vector regions hold n_g x even(nb) complex64 each: U, V, W always; with
-// WS_COMPACTION five more (the working set of an adaptive solve keeps X in the workspace and has a
+// Caller's workspace.  Vector regions hold n_g x even(nb) complex64 each: U, V, W always (an odd nb: one
+// or two more); with WS_COMPACTION up to nine (the working set of an adaptive solve keeps X in the workspace and has a
 // second vector set to re-pack into), with WS_HOST_STAGING the device copy of x for the host entry.
 struct WsLayout {
     size_t vecs[9], U_bot, partials, partials_rt, gscratch, Xs, Ds, tols, res, its, alphas, U_bot2, total;
@@ -230,9 +230,12 @@ WsLayout ws_layout(const wri_ctx* c, int nb, int flags, int maxit_cap) {
         L.its = o; o += align_up((size_t)nbe * sizeof(int), 256);
         L.alphas = o; o += align_up((size_t)nbe * sizeof(float2), 256);
     }
+    // an odd batch runs on the pass kernel in an even-width working set of its own (X too lives in the
+    // workspace then; the host entry keeps its staged q in the V region meanwhile): one or two more regions
+    if (nb & 1)
+        for (int i = 0; i < ((flags & WS_HOST_STAGING) ? 2 : 1); ++i) { L.vecs[L.n_vecs++] = o; o += vec; }
     if (flags & WS_COMPACTION) {
-        for (int i = 3; i < 9; ++i) { L.vecs[i] = o; o += vec; }   // [8]: final x of retired columns
-        L.n_vecs = 9;
+        while (L.n_vecs < 9) { L.vecs[L.n_vecs++] = o; o += vec; }   // [8]: final x of retired columns
         L.U_bot2 = o; o += bot;
     }
     L.total = o;
@@ -792,7 +795,13 @@ int static_plan(wri_ctx* c, int nb, const void* in, const void* old, StaticLaunc
     int rc = make_plan(c, nb, S.P);
     if (rc) return rc;
     DevPlan& P = S.P;
-    // one light stream: the deepest ring that fits (measured for the operator entries: deeper is better)
+    // one light stream: long tiles (128 planes: 0.88 -> 0.90 of the copy bandwidth at 128^3 x 64) and the
+    // deepest ring that fits (measured for the operator entries: deeper is better)
+    if (!c->dbg.zc_a && P.a.zc < 128 && (long long)P.nchunk * P.ntx * P.nty >= 6LL * rt_grid(c)) {
+        P.a.zc = 128;
+        P.a.ntz = (c->g.nz + 127) / 128;
+        P.a.n_tiles = P.nchunk * P.ntx * P.nty * P.a.ntz;
+    }
     const int nxyz = c->g.nx + c->g.ny + c->g.nz;
     int n = c->dbg.nstage_a > 0 ? c->dbg.nstage_a : RT_MAX_STAGES;
     n = std::min(n, RT_MAX_STAGES);
@@ -1243,13 +1252,14 @@ int lsqr_begin_impl(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const
     const int base_flags = host_staged ? WS_HOST_STAGING : 0;
     if (c->ws_bytes < ws_layout(c, nb, base_flags, kHostMaxitCap).total) return WRI_ERR_WORKSPACE;
     const WsLayout L = ws_layout(c, nb, base_flags | WS_COMPACTION, kHostMaxitCap);
-    const bool ws_big = c->ws_bytes >= L.total;               // the five spare vector regions are there
+    const bool ws_big = c->ws_bytes >= L.total;               // the spare vector regions of WS_COMPACTION are there
+    const int n_rgn = ws_big ? 8 : ws_layout(c, nb, base_flags, kHostMaxitCap).n_vecs;
     bool grouped = ncols > 0;
     if (!grouped) { col0 = 0; ncols = nb; }
     int nbw = grouped ? even_up(ncols) : nb;
     // the pass kernel serves even widths; an odd batch runs padded when the workspace has a spare region
     bool rt = rt_chunk_for(c, nbw) != 0;
-    if (!grouped && (nb % 2) && batch && ws_big && rt_chunk_for(c, nb + 1)) { grouped = true; nbw = nb + 1; rt = true; }
+    if (!grouped && (nb % 2) && batch && n_rgn >= 4 && rt_chunk_for(c, nb + 1)) { grouped = true; nbw = nb + 1; rt = true; }
     // adaptive accuracy: with tolerances, converged columns are compacted out of the working set on the device
     const bool adaptive = rt && batch && tol_dev && ws_big && nbw <= RT_MAXW && nbw >= 4 && !c->dbg.no_compact;
     const bool packed = grouped || adaptive;
@@ -1260,7 +1270,7 @@ int lsqr_begin_impl(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const
     {
         const size_t slot = align_up(c->ng * (size_t)nbw * sizeof(float2), 256);
         const size_t region = align_up(c->ng * (size_t)even_up(nb) * sizeof(float2), 256);
-        for (int rgn = 0; rgn < (ws_big ? 8 : 3); ++rgn) {
+        for (int rgn = 0; rgn < n_rgn; ++rgn) {
             if (rgn == 1 && host_staged && q_dev && grouped) continue;
             for (size_t o = 0; o + slot <= region; o += slot) slots.push_back((float2*)(c->ws + L.vecs[rgn] + o));
         }
