@@ -98,10 +98,11 @@ int wri_set_stencil(wri_ctx* ctx, int32_t stencil);
  *   txc / tyc             cells per tile in x / y
  *   no_compact            keep converged columns in the working set (they stay frozen, no re-packing)
  *   no_groups             run a batch wider than 64 columns in lock-step instead of 64-column groups
- *   generic               use the plain (non-TMA) kernels for every width                          */
+ *   generic               use the plain (non-TMA) kernels for every width
+ *   m_ldg_f               pass F reads the model by plain loads (1) / through its TMA stage (2)     */
 typedef struct {
     int32_t nstage_f, nstage_a, zc_f, zc_a, txc, tyc;
-    int32_t no_compact, no_groups, generic;
+    int32_t no_compact, no_groups, generic, m_ldg_f;
 } wri_debug_opts;
 int wri_set_debug_opts(wri_ctx* ctx, const wri_debug_opts* opts);
 

@@ -51,7 +51,7 @@ class wri_awri_opts(C.Structure):
 
 class wri_debug_opts(C.Structure):
     _fields_ = [(n, C.c_int32) for n in ("nstage_f", "nstage_a", "zc_f", "zc_a", "txc", "tyc",
-                                         "no_compact", "no_groups", "generic")]
+                                         "no_compact", "no_groups", "generic", "m_ldg_f")]
 
 
 class wri_awri_report(C.Structure):

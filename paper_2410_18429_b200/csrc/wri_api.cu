@@ -480,15 +480,16 @@ int make_plan(const wri_ctx* c, int nb, DevPlan& P) {
                 // (from 16 columns on idle consumer threads cost little — 384 busy ones keep pass A at its
                 // rate — and contiguous tile rows below 2 KB cost a lot: 48 columns as 8 x 2 cells run 4 %
                 // faster than as 4 x 5, profiles/r02_width_sweeps.md)
-                double cost = ntx * nty * ((txc + 2.0) * (tyc + 2.0) + (cb >= 16 ? 0.25 : 0.75) * maxcells);
+                const bool long_rows = cb >= 10 || cb == 6;      // (2, 4 and 8 columns: measured no gain)
+                double cost = ntx * nty * ((txc + 2.0) * (tyc + 2.0) + (long_rows ? 0.25 : 0.75) * maxcells);
                 const int row_bytes = txc * cb * 8;
                 if (row_bytes < 512 && txc < nx) cost *= 1.0 + 0.25 * (512 - row_bytes) / 512.0;
-                if (cb >= 16 && row_bytes < 2048 && txc < nx) cost *= 1.0 + (2048 - row_bytes) / 2048.0;
+                if (long_rows && row_bytes < 2048 && txc < nx) cost *= 1.0 + (2048 - row_bytes) / 2048.0;
                 // below 32 columns a box row should carry (column, x) folded into one dimension
                 if (cb < 32 && !(P.nchunk == 1 && cb * (txc + 2) <= 256)) cost *= 1.2;
                 // tile rows that do not start on 128-byte lines: measured 6-10 % slower in both passes
                 // (widths 6, 10: profiles/r02_width_sweeps.md)
-                if (row_bytes % 128 != 0 && txc < nx) cost *= 1.12;
+                if (row_bytes % 128 != 0 && txc < nx) cost *= 1.2;
                 if (!(m_al && txc % 4 == 0)) cost *= 1.3;    // model tile by plain loads: pass A 0.98 -> 0.80 at 48 columns
                 if (cost < best) { best = cost; btx = txc; bty = tyc; }
             }
@@ -498,6 +499,8 @@ int make_plan(const wri_ctx* c, int nb, DevPlan& P) {
     P.nty = (ny + bty - 1) / bty;
     P.merged = (P.nchunk == 1 && cb * (btx + 2) <= 256) ? 1 : 0;
     P.m_tma = (m_al && btx % 4 == 0) ? 1 : 0;
+    // pass F reads the model by plain loads: +1 to +4 % at every width (profiles/r02_width_sweeps.md)
+    P.f_m_ldg = c->dbg.m_ldg_f == 2 ? 0 : 1;
     P.row_b = (btx + 2) * cb * 8;
     P.cell_b = cb * 8;
     P.in_bytes = (btx + 2) * (bty + 2) * cb * 8;
@@ -588,7 +591,7 @@ int rt_setup(wri_ctx* c) {
                 if (a.v[p][q] != b.v[p][q]) return false;
         const wri_debug_opts &x = a.dbg, &y = b.dbg;
         return x.nstage_f == y.nstage_f && x.nstage_a == y.nstage_a && x.zc_f == y.zc_f && x.zc_a == y.zc_a &&
-               x.txc == y.txc && x.tyc == y.tyc && x.generic == y.generic;
+               x.txc == y.txc && x.tyc == y.tyc && x.generic == y.generic && x.m_ldg_f == y.m_ldg_f;
     };
     if (c->plan_valid && same(key, c->plan_key)) return WRI_OK;
     c->plan_valid = false;

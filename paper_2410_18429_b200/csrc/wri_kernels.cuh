@@ -49,6 +49,7 @@ struct DevPlan {          // tile geometry of one working width
     int txc, tyc, items;              // cells per tile (x, y); consumer threads with work = txc*tyc*hp
     int ntx, nty;
     int merged, m_tma;                // tensor maps fold (column, x); the model tile rides in the stage
+    int f_m_ldg, pad0;                // ... except in pass F (plain loads there)
     int row_b, cell_b;                // bytes per row / per cell of the halo box in shared memory
     int in_bytes, in_span;            // halo box: bytes delivered, room taken (128 B granules)
     int ctr_bytes, ctr_span;          // centre box

@@ -291,6 +291,9 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
     __syncthreads();
     const DevPlan& pl = s_pl;
     const PassGeo geo = (MODE == MODE_F) ? pl.f : pl.a;
+    // the model tile rides in the TMA stage, except in pass F where the plan may ask for plain loads (its
+    // stage already takes four tensor loads per plane; a fifth, tiny one costs 2-3 % from 24 columns on)
+    const bool m_tma = pl.m_tma && !(MODE == MODE_F && pl.f_m_ldg);
     const int nb = pl.nb, cb = pl.cb, hp = pl.hp;
     const int nstage = geo.nstage;
     const int STAGE_BYTES = rt_stage_bytes(pl, NSTREAM);
@@ -370,7 +373,7 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
             if (issuer) {
                 tmap_acquire(tm_in); tmap_acquire(tm_old);
                 if (MODE == MODE_F) { tmap_acquire(tm_w); tmap_acquire(tm_x); }
-                if (pl.m_tma) tmap_acquire(tm_m);
+                if (m_tma) tmap_acquire(tm_m);
             }
         } else {
             tm_in = &pm_in; tm_old = &pm_old; tm_m = &pm_m;
@@ -379,7 +382,7 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
         const uint64_t pol_in = policy_evict_last();
         const uint32_t tx_first = pl.in_bytes;
         const uint32_t tx_full = pl.in_bytes + (has_old ? (has_wx ? 3 : 1) * pl.ctr_bytes : 0) +
-                                 (pl.m_tma ? pl.m_bytes : 0);
+                                 (m_tma ? pl.m_bytes : 0);
         int stage = 0;
         uint32_t phase = 0;
         for (int t = blockIdx.x; t < geo.n_tiles; t += gridDim.x) {
@@ -407,7 +410,7 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
                             tma_load_4d_hint(dst + IN_SPAN + CTR_SPAN, tm_w, fb, a0, a1, a2, a3, pol_stream);
                             tma_load_4d_hint(dst + IN_SPAN + 2 * CTR_SPAN, tm_x, fb, a0, a1, a2, a3, pol_stream);
                         }
-                        if (pl.m_tma) tma_load_3d(dst + M_OFF, tm_m, fb, x0, y0, plz - 1);
+                        if (m_tma) tma_load_3d(dst + M_OFF, tm_m, fb, x0, y0, plz - 1);
                     }
                 }
                 __syncwarp();
@@ -687,9 +690,9 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
             int chunk = t % pl.nchunk;
             if (warp_live) {
                 if constexpr (TRK) {                             // (a re-packing iteration always has its old stream)
-                    if (pl.m_tma) chunk = run_tile(TrueT{}, TrueT{}, TrueT{}, t);
+                    if (m_tma) chunk = run_tile(TrueT{}, TrueT{}, TrueT{}, t);
                     else          chunk = run_tile(FalseT{}, TrueT{}, TrueT{}, t);
-                } else if (pl.m_tma) {
+                } else if (m_tma) {
                     if (has_old) chunk = run_tile(TrueT{}, TrueT{}, FalseT{}, t);
                     else         chunk = run_tile(TrueT{}, FalseT{}, FalseT{}, t);
                 } else {
