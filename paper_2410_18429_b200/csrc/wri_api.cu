@@ -800,7 +800,9 @@ int static_plan(wri_ctx* c, int nb, const void* in, const void* old, StaticLaunc
     DevPlan& P = S.P;
     // one light stream: long tiles (128 planes: 0.88 -> 0.90 of the copy bandwidth at 128^3 x 64) and the
     // deepest ring that fits (measured for the operator entries: deeper is better)
-    if (!c->dbg.zc_a && P.a.zc < 128 && (long long)P.nchunk * P.ntx * P.nty >= 6LL * rt_grid(c)) {
+    // (one chunk per cell, grids below 256 planes: at 256^3 x 32 and at 128^3 x 192 it costs 10 %)
+    if (!c->dbg.zc_a && P.a.zc < 128 && P.nchunk == 1 && c->g.nz < 256 &&
+        (long long)P.ntx * P.nty >= 6LL * rt_grid(c)) {
         P.a.zc = 128;
         P.a.ntz = (c->g.nz + 127) / 128;
         P.a.n_tiles = P.nchunk * P.ntx * P.nty * P.a.ntz;
