@@ -366,7 +366,7 @@ struct ScalParams {
     int k;                    // iteration number (PH_A), for resnorms / iters
     int maxit;
     float lambda;
-    int rows_in_pass;         // 1: the pass kernels own the receiver rows (wri_tma.cuh); the
+    int rows_in_pass;         // 1: the pass kernels own the receiver rows (wri_pass.cuh); the
                               //    finaliser only reduces partials and runs the recurrences
     const int* colmap;        // [nb] working column -> caller's column (-1 = padding); null = identity
     int nb_out;               // caller's batch width: row stride of resnorms

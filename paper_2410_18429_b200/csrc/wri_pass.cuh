@@ -14,9 +14,11 @@
 // running in-plane sum) and write results straight to HBM with 128-bit stores.
 //
 // Solve state on the device (SolveState): working width, iteration count, parity of the vector
-// set in use, the compaction that the last finaliser decided.  Every launch of a solve reads it
+// set in use, the re-packing that the last finaliser asked for.  Every launch of a solve reads it
 // first; once every column has stopped the launches return at once.  No host round trip anywhere
-// in an LSQR solve, with or without tolerances.
+// in an LSQR solve, with or without tolerances.  Re-packing a shrinking working set is done by
+// the passes themselves (TRK instances: results stored into the other vector set at the new
+// width); the launches of a solve are chained by programmatic dependent launch.
 //
 // The squared-norm partials are accumulated per column in a fixed order (thread -> CTA row of
 // partials[] -> last CTA); the last CTA to finish reduces the rows and runs the per-column scalar
@@ -245,7 +247,7 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
     constexpr int NSTREAM = RtTraits<MODE>::NSTREAM;
 
     // ---- state of the solve in flight (uniform over the grid; written only by finalisers of
-    //      earlier launches and by the compaction kernel)
+    //      earlier launches)
     // Programmatic dependent launch: the passes of a solve are enqueued with the stream-serialisation
     // attribute, so a CTA of the next launch may take an SM as soon as this launch's CTA there has left;
     // it waits here until the whole launch before it has completed and its writes are visible.  (Without
