@@ -794,7 +794,7 @@ struct StaticLaunch {
     size_t smem;
     int grid;
 };
-int static_plan(wri_ctx* c, int nb, const void* in, const void* old, StaticLaunch& S) {
+int static_plan(wri_ctx* c, int nb, const void* in, const void* old, StaticLaunch& S, size_t reserve = 0) {
     int rc = make_plan(c, nb, S.P);
     if (rc) return rc;
     DevPlan& P = S.P;
@@ -810,9 +810,9 @@ int static_plan(wri_ctx* c, int nb, const void* in, const void* old, StaticLaunc
     const int nxyz = c->g.nx + c->g.ny + c->g.nz;
     int n = c->dbg.nstage_a > 0 ? c->dbg.nstage_a : RT_MAX_STAGES;
     n = std::min(n, RT_MAX_STAGES);
-    while (n > 2 && rt_smem_bytes(P, 1, n, nxyz) > (size_t)RT_SMEM_MAX) --n;
+    while (n > 2 && rt_smem_bytes(P, 1, n, nxyz) + reserve > (size_t)RT_SMEM_MAX) --n;
     P.a.nstage = n;
-    S.smem = rt_smem_bytes(P, 1, n, nxyz);
+    S.smem = rt_smem_bytes(P, 1, n, nxyz) + reserve;
     S.grid = std::min(P.a.n_tiles, rt_grid(c));
     const bool mg = P.merged != 0;
     if ((rc = make_tmap(&S.in, in, c, nb, P.cb, P.txc + 2, P.tyc + 2, mg))) return rc;
@@ -1181,7 +1181,7 @@ int wri_objective_gradient(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host
     const int cb = rt_chunk_for(c, nb);
     if (cb == nb && nb >= 4 && (nb & (nb - 1)) == 0) {
         StaticLaunch S;
-        if ((rc = static_plan(c, nb, u_dev, q_dev, S))) return rc;
+        if ((rc = static_plan(c, nb, u_dev, q_dev, S, RT_G_SCRATCH))) return rc;
         float* g_scr = g_dev ? (float*)(c->ws + L.gscratch) : nullptr;
         RtParams p{};
         p.sgn = 1.f; p.phase = -1;

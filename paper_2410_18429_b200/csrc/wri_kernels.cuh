@@ -36,6 +36,7 @@ constexpr int RT_MAXW = 64;           // widest column chunk (and widest working
 constexpr int RT_MAX_STAGES = 12;
 constexpr int RT_SMEM_MAX = 232448 - 1024;  // 227 KB of shared memory per CTA, less the static part
 constexpr int RT_MIN_STAGE_AREA = 20480;   // the CTA epilogue re-uses the (idle) stages as scratch
+constexpr int RT_G_SCRATCH = (RT_NT / 32) * 4 * 32 * 4 + 16;   // gradient pass: four planes of terms per consumer warp
 
 enum StencilKind { ST_7 = 0, ST_27 = 1 };
 enum MapSlot { MP_V_HALO = 0, MP_U_CTR, MP_W_CTR, MP_X_CTR, MP_U_HALO, MP_V_CTR, N_MAPS };

@@ -310,6 +310,8 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
     double* red = colacc + nb;                                                    // [NT]
     float* tab_g = reinterpret_cast<float*>(red + NT);                            // gx | gy | gz
     float* tab_c = tab_g + (p.nx + p.ny + p.nz);                                  // w2|ca|cb|cv|cx|cw, [6][nb]
+    // MODE_G: per consumer warp, the gradient terms of four planes (RT_G_SCRATCH bytes behind the tables)
+    float* gbuf_all = reinterpret_cast<float*>((reinterpret_cast<uintptr_t>(tab_c + 6 * nb) + 15) & ~(uintptr_t)15);
 
     const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + RT_MAX_STAGES);
     const size_t NM = p.nb_max;
@@ -590,13 +592,35 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
                             const float tr = fmaf(cc.z, r_re, cc.w * r_im), ti = fmaf(cc.z, r_im, -cc.w * r_re);
                             gterm = fmaf(w2[1], fmaf(g, ti, tr), gterm);
                         }
-                        if (p.g) {
-                            // the hp threads of one cell are consecutive lanes (the host sends only
-                            // power-of-two hp <= 32 down this path)
+                        if (p.g && hp >= 4) {
+                            // Sum over the batch columns of a cell: the hp threads of a cell are consecutive
+                            // lanes (the host sends only power-of-two hp <= 32 down this path).  The terms of
+                            // FOUR planes are parked in the warp's scratch and folded together — a lane takes
+                            // four neighbouring terms (one plane, one cell), then hp/4 lanes are folded by
+                            // shuffles: 1 + log2(hp/4) dependent steps per four planes instead of log2(hp)
+                            // per plane (the chain of shuffles was the longest stall of this pass).  Fixed
+                            // order; planes are emitted in aligned blocks of four (tiles start at multiples
+                            // of 8 planes).  Pure stores (no load in the pipeline's critical path): this
+                            // batch's gradient goes to a scratch array, k_add_f32 accumulates it afterwards.
+                            const int lane = tid & 31, slot = (plz - 1) & 3;
+                            float* gbuf = gbuf_all + (tid >> 5) * 128;
+                            gbuf[slot * 32 + lane] = gterm;
+                            if (slot == 3 || plz == z1) {
+                                __syncwarp();
+                                const float4 v4 = *reinterpret_cast<const float4*>(gbuf + 4 * lane);
+                                float sum = (v4.x + v4.y) + (v4.z + v4.w);
+                                const int qpc = hp >> 2;                       // lanes per (plane, cell) now
+                                for (int dlt = qpc >> 1; dlt > 0; dlt >>= 1)
+                                    sum += __shfl_down_sync(0xffffffffu, sum, dlt, qpc);
+                                const int pl = lane >> 3, cw = ((lane & 7) << 2) / hp;
+                                // cell of (first plane of the block, cell cw of this warp) from a lane that owns it
+                                const int c0 = __shfl_sync(0xffffffffu, valid ? cell - slot * plane_m : -1, cw * hp);
+                                if ((lane % qpc) == 0 && pl <= slot && c0 >= 0) p.g[c0 + pl * plane_m] = p.lam2 * sum;
+                                __syncwarp();
+                            }
+                        } else if (p.g) {
                             for (int dlt = hp >> 1; dlt > 0; dlt >>= 1)
                                 gterm += __shfl_down_sync(0xffffffffu, gterm, dlt, hp);
-                            // pure store (no load in the pipeline's critical path): this batch's
-                            // gradient goes to a scratch array, k_add_f32 accumulates it afterwards
                             if (cp == 0 && valid) p.g[cell] = p.lam2 * gterm;
                         }
                     } else {
