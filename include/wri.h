@@ -47,6 +47,7 @@ extern "C" {
 #define WRI_ERR_CUDA             -5   /* CUDA runtime error; text via wri_strerror                 */
 #define WRI_ERR_STATE            -6   /* call out of order (e.g. iterate before begin)             */
 #define WRI_ERR_NUMERIC          -7   /* wri_awri_step: the objective at the current model is not finite */
+#define WRI_ERR_SCRATCH_LIMIT    -8   /* wri_objective_gradient_static: needs more than WRI_STATIC_SCRATCH_BYTES */
 
 typedef struct wri_ctx wri_ctx;                 /* opaque, library-owned */
 
@@ -212,6 +213,29 @@ int wri_objective_gradient(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_ho
                            const int32_t* src_ijk_host, const void* alpha_dev, const void* q_dev,
                            const void* u_dev, const void* d_dev, float lambda,
                            double* f_pde_dev, double* f_data_dev, float* g_dev);
+
+/* wri_objective_gradient without a workspace and without any device allocation, for callers that may
+ * not call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it).
+ * Same operation, arguments, outputs and accumulation rule as wri_objective_gradient (eq. 4, eq. 8-9,
+ * PAPER.md:71-76, 98-110); every width runs the generic gradient kernel, whose per-tile column sums of
+ * |r|^2 go to a scratch array that is part of the library image: WRI_STATIC_SCRATCH_BYTES of device
+ * memory on every GPU that loads the library, held until the process exits.  The scratch need is
+ * (number of thread-block tiles) x nb doubles; the tiles are made taller until that fits, and a case
+ * that does not fit even with tiles as tall as the grid (128^3 x 64, 256^3 x 64 and 200 x 200 x 160 x 48
+ * fit; 128^3 x 192 and wider do not) is refused with WRI_ERR_SCRATCH_LIMIT before anything is
+ * launched or written.  The call does no cudaMalloc / cudaFree and calls no
+ * allocating library routine; it needs no wri_set_workspace.  Nothing in the scratch has to start at
+ * zero (every entry that is read is written first by the same call).  ALL calls on one GPU share the
+ * array, whatever their context or stream: calls that can overlap on the GPU (different streams,
+ * different contexts, different host threads without ordering) race on it and return garbage sums —
+ * order them on one stream or with events.  f_pde / f_data agree with wri_objective_gradient to
+ * double rounding of a differently grouped sum, g to float rounding (the power-of-two widths use
+ * another kernel there).                                                                          */
+#define WRI_STATIC_SCRATCH_BYTES (4u << 20)
+int wri_objective_gradient_static(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_host,
+                                  const int32_t* src_ijk_host, const void* alpha_dev, const void* q_dev,
+                                  const void* u_dev, const void* d_dev, float lambda,
+                                  double* f_pde_dev, double* f_data_dev, float* g_dev);
 
 /* Per-source receiver sets P_i ("P_i is the restriction operator for source i").
  * mask_dev: uint8 [n_rec][nb], 1 = receiver r records batch column s, 0 = that row is absent from

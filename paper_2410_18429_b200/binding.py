@@ -69,6 +69,8 @@ WRI_ERR_WORKSPACE = -4
 WRI_ERR_CUDA = -5
 WRI_ERR_STATE = -6
 WRI_ERR_NUMERIC = -7
+WRI_ERR_SCRATCH_LIMIT = -8
+WRI_STATIC_SCRATCH_BYTES = 4 << 20
 WRI_STENCIL_7 = 0
 WRI_STENCIL_27 = 1
 WRI_WS_HOST_STAGING = 1
@@ -129,6 +131,7 @@ def load_library():
     lib.wri_lsqr_sf_batch_host.argtypes = solve_sf
     lib.wri_lsqr_sf_batch_host_async.argtypes = solve_sf
     lib.wri_objective_gradient.argtypes = [P, I32, P, P, P, P, P, P, F32, P, P, P]
+    lib.wri_objective_gradient_static.argtypes = [P, I32, P, P, P, P, P, P, F32, P, P, P]
     lib.wri_lsqr_set_opts.argtypes = [P, C.POINTER(wri_lsqr_opts)]
     lib.wri_set_receiver_mask.argtypes = [P, I32, P]
     lib.wri_misfit_sf.argtypes = [P, I32, P, P, P, F32, F32, I32, I32, P, P, P, P, P, P, P, P]
@@ -468,6 +471,23 @@ class Wri:
         _ck(self._lib.wri_objective_gradient(self._h, nb, oi, si, _dptr(alpha), _dptr(q), _dptr(u), _dptr(d),
                                              float(lam), _dptr(fp), _dptr(fd), _dptr(g)))
         return fp, fd
+
+    def objective_gradient_static(self, u, d, lam, f_pde, f_data, omega_idx=None, q=None, src_ijk=None,
+                                  alpha=None, g=None):
+        """wri_objective_gradient_static: the same operation with the scratch in the library image — no
+        workspace, no device allocation here or in the library.  The caller passes the outputs f_pde,
+        f_data (float64 [nb], device); g (float32 [n_g]) is accumulated in place.  Raises WriError
+        (WRI_ERR_SCRATCH_LIMIT) when grid x width needs more than WRI_STATIC_SCRATCH_BYTES."""
+        t = self._torch
+        nb = u.shape[1]
+        for f in (f_pde, f_data):
+            if f.dtype != t.float64 or f.numel() != nb or not f.is_contiguous() or f.device != u.device:
+                raise ValueError("f_pde / f_data: contiguous float64 [nb] on the device of u")
+        keep, oi = _i32(omega_idx)
+        keep2, si = _i32(src_ijk)
+        _ck(self._lib.wri_objective_gradient_static(self._h, nb, oi, si, _dptr(alpha), _dptr(q), _dptr(u),
+                                                    _dptr(d), float(lam), _dptr(f_pde), _dptr(f_data),
+                                                    _dptr(g)))
 
     def misfit_sf(self, d, lam, src_ijk, eps, maxit, omega_idx=None, g=None, warm=None, want_f=True):
         """One misfit evaluation (wri_misfit_sf).  warm = (u, alpha, ar0) from an earlier evaluation

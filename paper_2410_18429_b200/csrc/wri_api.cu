@@ -10,6 +10,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <type_traits>
 #include <utility>
 #include <vector>
@@ -879,6 +880,9 @@ const char* wri_strerror(int code) {
         case WRI_ERR_CUDA: return g_cuda_msg;
         case WRI_ERR_STATE: return "call out of order";
         case WRI_ERR_NUMERIC: return "objective is not finite";
+        case WRI_ERR_SCRATCH_LIMIT:
+            return "wri_objective_gradient_static: grid x batch width needs more than the "
+                   "WRI_STATIC_SCRATCH_BYTES (4 MiB) of built-in scratch; use wri_objective_gradient with a workspace";
         default: return "unknown error code";
     }
 }
@@ -1234,8 +1238,100 @@ int wri_objective_gradient(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host
     return WRI_OK;
 }
 
-// ---- solver entries ----------------------------------------------------------------------------
 }  // extern "C"
+
+// ---- objective / gradient without device allocation ----------------------------------------------
+// Scratch of wri_objective_gradient_static (include/wri.h): the [n_tiles][nb] column sums of |r|^2 that
+// k_grad writes and k_objective folds.  Part of the library image: every GPU that loads libwri holds
+// these WRI_STATIC_SCRATCH_BYTES until the process exits.  In host code the name below is only a
+// stand-in for the symbol — the kernels get the address cudaGetSymbolAddress returns for the current
+// device, looked up once per device.
+constexpr size_t kStaticScratchDoubles = WRI_STATIC_SCRATCH_BYTES / sizeof(double);
+static __device__ __align__(256) double g_static_partials[kStaticScratchDoubles];
+
+namespace {
+
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mu;
+double* g_static_ptr[kStaticMaxDevices] = {};
+
+// device address of g_static_partials on the current device (the one the context's buffers live on)
+int static_scratch_ptr(double** out) {
+    int dev = -1;
+    CK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticMaxDevices) return WRI_ERR_ARG;
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_ptr[dev]) {
+        void* ptr = nullptr;
+        CK(cudaGetSymbolAddress(&ptr, g_static_partials));
+        if (!ptr) return WRI_ERR_CUDA;
+        g_static_ptr[dev] = static_cast<double*>(ptr);
+    }
+    *out = g_static_ptr[dev];
+    return WRI_OK;
+}
+
+}  // namespace
+
+extern "C" int wri_objective_gradient_static(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host,
+                                             const int32_t* src_ijk_host, const void* alpha_dev,
+                                             const void* q_dev, const void* u_dev, const void* d_dev,
+                                             float lambda, double* f_pde_dev, double* f_data_dev,
+                                             float* g_dev) {
+    int rc = check_batch_args(c, nb);
+    if (rc) return rc;
+    if (!u_dev || !aligned16(u_dev) || (q_dev && !aligned16(q_dev)) || (c->n_rec && !d_dev) || !f_pde_dev ||
+        !f_data_dev || (src_ijk_host && !alpha_dev))
+        return WRI_ERR_ARG;
+    if (c->solving) return WRI_ERR_STATE;
+    GradTiling G = make_grad_tiling(c, nb);
+    if (!G.ok) return WRI_ERR_ARG;
+    // taller tiles until the per-tile sums fit the static array; refused when even whole columns do not
+    while (G.t.n_tiles * (size_t)nb > kStaticScratchDoubles && G.t.zc < c->g.nz) {
+        G.t.zc = std::min(c->g.nz, G.t.zc * 2);
+        G.t.grid.z = (unsigned)((c->g.nz + G.t.zc - 1) / G.t.zc);
+        G.t.n_tiles = (size_t)G.t.grid.x * G.t.grid.y * G.t.grid.z;
+    }
+    if (G.t.n_tiles * (size_t)nb > kStaticScratchDoubles) return WRI_ERR_SCRATCH_LIMIT;
+    double* partials = nullptr;
+    if ((rc = static_scratch_ptr(&partials))) return rc;
+    if ((rc = upload_columns(c, nb, omega_idx_host, lambda))) return rc;
+    if (src_ijk_host && (rc = upload_sources(c, nb, src_ijk_host))) return rc;
+    const StencilW sw = stencil_weights(c->stencil);
+    GradParams p{};
+    p.u = (const float2*)u_dev; p.q = (const float2*)q_dev;
+    p.src = src_ijk_host ? c->src : nullptr; p.alpha = (const float2*)alpha_dev;
+    p.m = c->m;
+    p.gx = c->gtab; p.gy = c->gtab + c->g.nx; p.gz = c->gtab + c->g.nx + c->g.ny;
+    p.w2 = c->coef[0] + C_W2 * (size_t)c->nb_max;
+    p.g = g_dev;
+    p.partials = partials;
+    p.nx = c->g.nx; p.ny = c->g.ny; p.nz = c->g.nz; p.nb = nb; p.zc = G.t.zc;
+    p.tpc = G.tpc; p.shuffle = G.shuffle;
+    p.ih2 = (float)(1.0 / (c->h * c->h));
+    p.m6ih2 = (float)(sw.a0 / (c->h * c->h));
+    p.a1 = (float)sw.a1; p.a2 = (float)sw.a2; p.a3 = (float)sw.a3;
+    p.lam2 = lambda * lambda;
+    const size_t smem = (size_t)G.t.block.x * G.t.block.y * G.t.vec * sizeof(double);
+    const bool s27 = c->stencil == WRI_STENCIL_27;
+    if (G.t.vec == 2) {
+        if (s27) k_grad<2, ST_27><<<G.t.grid, G.t.block, smem, c->stream>>>(p);
+        else     k_grad<2, ST_7><<<G.t.grid, G.t.block, smem, c->stream>>>(p);
+    } else {
+        if (s27) k_grad<1, ST_27><<<G.t.grid, G.t.block, smem, c->stream>>>(p);
+        else     k_grad<1, ST_7><<<G.t.grid, G.t.block, smem, c->stream>>>(p);
+    }
+    c->launches++;
+    CK(cudaGetLastError());
+    k_objective<<<(nb + OBJ_CPB - 1) / OBJ_CPB, 1024, 1024 * sizeof(double), c->stream>>>(
+        partials, (int)G.t.n_tiles, nb, (const float2*)u_dev, (const float2*)d_dev, c->rec, c->n_rec,
+        (double)lambda * (double)lambda, f_pde_dev, f_data_dev, c->rmask);
+    c->launches++;
+    CK(cudaGetLastError());
+    return WRI_OK;
+}
+
+// ---- solver entries ----------------------------------------------------------------------------
 
 namespace {
 

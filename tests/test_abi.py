@@ -33,7 +33,7 @@ def test_every_declared_symbol_is_exported(lib):
             "wri_misfit_sf", "wri_awri_step", "wri_set_receiver_mask",
             "wri_host_pipeline_bytes", "wri_set_host_pipeline", "wri_lsqr_batch_host_async",
             "wri_lsqr_sf_batch_host_async", "wri_host_wait", "wri_set_stencil",
-            "wri_set_debug_opts", "wri_plan_info"} <= set(names)
+            "wri_set_debug_opts", "wri_plan_info", "wri_objective_gradient_static"} <= set(names)
     for n in names:
         assert hasattr(lib, n), n
 
