@@ -404,15 +404,17 @@ def run_ours(args, wl_name, w):
         ms_g = ev[2].elapsed_time(ev[3]) / n_g
         bytes_g = (8 * nb + 4 + 8) * w.ng          # u read once, m read, g read + written
         peak_g, _ = measured_hbm_peak()
-        # this pass is bound by its instruction stream: 2.27 warp-instructions per
-        # cell-column against 148 SMs x 4 schedulers x the maximum SM clock
+        # this pass is bound by its instruction stream: 2.22 executed warp-instructions per
+        # cell-column (ncu, profiles/r02_gradient.md) against 148 SMs x 4 schedulers x the maximum SM clock
         alu_peak = 148 * 4 * 1.965e9
         extras["objective_gradient"] = {"ms": ms_g, "algorithmic_bytes": bytes_g,
                                         "achieved": bytes_g / (ms_g * 1e-3) / 1e9, "unit": "GB/s",
                                         "frac": bytes_g / (ms_g * 1e-3) / 1e9 / peak_g,
-                                        "bound": "alu", "warp_instructions_per_cell_column": 2.27,
-                                        "frac_alu": 2.27 * w.ng * nb / (ms_g * 1e-3) / alu_peak,
-                                        "kernel": "k_grad + k_objective (eq. 9 fused with the stencil residual)"}
+                                        "bound": "alu", "warp_instructions_per_cell_column": 2.22,
+                                        "frac_alu": 2.22 * w.ng * nb / (ms_g * 1e-3) / alu_peak,
+                                        "kernel": "k_pass_rt<MODE_G> + k_add_f32 + k_objective (eq. 9 fused with "
+                                                  "the stencil residual); k_grad at widths the pass kernel "
+                                                  "does not take"}
         # the operator entries on their own (wri_apply_M / wri_apply_MH): read x, write y = 16 B per cell-column
         ev2 = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
         yb = torch.empty((w.n_rec, nb), dtype=torch.complex64, device=dev)

@@ -206,6 +206,9 @@ __device__ __forceinline__ float lds32(uint32_t addr) {
     asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
     return v;
 }
+__device__ __forceinline__ void sts32(uint32_t addr, float v) {
+    asm volatile("st.shared.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory");
+}
 __device__ __forceinline__ float4 f4add(const float4& a, const float4& b) {
     return make_float4(a.x + b.x, a.y + b.y, a.z + b.z, a.w + b.w);
 }
@@ -312,6 +315,8 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
     float* tab_c = tab_g + (p.nx + p.ny + p.nz);                                  // w2|ca|cb|cv|cx|cw, [6][nb]
     // MODE_G: per consumer warp, the gradient terms of four planes (RT_G_SCRATCH bytes behind the tables)
     float* gbuf_all = reinterpret_cast<float*>((reinterpret_cast<uintptr_t>(tab_c + 6 * nb) + 15) & ~(uintptr_t)15);
+    const uint32_t gbuf_w = smem_u32(gbuf_all) + (uint32_t)(threadIdx.x >> 5) * 512u;   // this warp's 4 x 32 terms
+    const int lhp = 31 - __clz(max(hp, 1));                                            // log2(hp) where hp is a power of two
 
     const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + RT_MAX_STAGES);
     const size_t NM = p.nb_max;
@@ -524,6 +529,9 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
             // plus the contribution of plane plz-1
             auto plane = [&](const int plz, float4& c_prev, float4& c_new, float4& s_prev, float4& s_new) {
                 if (!M_TMA && plz >= z0 && plz < z1) m_nxt = __ldg(p.m + cell + (plz > z0 ? plane_m : 0));
+                const bool emit = plz >= z0 + 1;
+                float gzv = 0.f;                                // sponge profile of the plane being emitted, read
+                if (emit) gzv = gz_tab[plz - 1];                // before the wait so that its latency hides behind it
                 mbar_wait(full0 + 8 * stage, phase);
                 const uint32_t sb = sb_cur;                     // this stage's shared-space address
                 c_new = lds128(sb + sm_ctr);
@@ -548,7 +556,6 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
                 }
                 const float4& zn = (STENCIL == ST_27) ? s_new : c_new;   // what plane plz gives plane plz-1
                 const float4& zp = (STENCIL == ST_27) ? s_prev : c_prev; // what plane plz-1 gives plane plz
-                const bool emit = plz >= z0 + 1;
                 float4 o_old = f4zero();
                 if (emit) {
                     if (HAS_OLD) o_old = lds128(sb + io);
@@ -565,7 +572,7 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
                 if (MODE != MODE_F) release();
 
                 if (emit) {
-                    const float g = fmaxf(gxy, gz_tab[plz - 1]);
+                    const float g = fmaxf(gxy, gzv);
                     const float4 cc = c_prev;
                     const float s0 = lap.x + zn.x, s1 = lap.y + zn.y, s2 = lap.z + zn.z, s3 = lap.w + zn.w;
                     if (MODE == MODE_G) {
@@ -602,20 +609,21 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
                             // order; planes are emitted in aligned blocks of four (tiles start at multiples
                             // of 8 planes).  Pure stores (no load in the pipeline's critical path): this
                             // batch's gradient goes to a scratch array, k_add_f32 accumulates it afterwards.
+                            // (hp is a power of two here: shifts and masks, no division in the loop)
                             const int lane = tid & 31, slot = (plz - 1) & 3;
-                            float* gbuf = gbuf_all + (tid >> 5) * 128;
-                            gbuf[slot * 32 + lane] = gterm;
+                            sts32(gbuf_w + 128 * slot + 4 * lane, gterm);
                             if (slot == 3 || plz == z1) {
                                 __syncwarp();
-                                const float4 v4 = *reinterpret_cast<const float4*>(gbuf + 4 * lane);
+                                const float4 v4 = lds128(gbuf_w + 16 * lane);
                                 float sum = (v4.x + v4.y) + (v4.z + v4.w);
                                 const int qpc = hp >> 2;                       // lanes per (plane, cell) now
-                                for (int dlt = qpc >> 1; dlt > 0; dlt >>= 1)
-                                    sum += __shfl_down_sync(0xffffffffu, sum, dlt, qpc);
-                                const int pl = lane >> 3, cw = ((lane & 7) << 2) / hp;
+                                if (qpc > 4) sum += __shfl_down_sync(0xffffffffu, sum, 4, qpc);
+                                if (qpc > 2) sum += __shfl_down_sync(0xffffffffu, sum, 2, qpc);
+                                if (qpc > 1) sum += __shfl_down_sync(0xffffffffu, sum, 1, qpc);
+                                const int pl = lane >> 3, cw = ((lane & 7) << 2) >> lhp;
                                 // cell of (first plane of the block, cell cw of this warp) from a lane that owns it
-                                const int c0 = __shfl_sync(0xffffffffu, valid ? cell - slot * plane_m : -1, cw * hp);
-                                if ((lane % qpc) == 0 && pl <= slot && c0 >= 0) p.g[c0 + pl * plane_m] = p.lam2 * sum;
+                                const int c0 = __shfl_sync(0xffffffffu, valid ? cell - slot * plane_m : -1, cw << lhp);
+                                if ((lane & (qpc - 1)) == 0 && pl <= slot && c0 >= 0) p.g[c0 + pl * plane_m] = p.lam2 * sum;
                                 __syncwarp();
                             }
                         } else if (p.g) {
