@@ -224,7 +224,11 @@ int wri_objective_gradient(wri_ctx* ctx, int32_t nb, const int32_t* omega_idx_ho
  * that does not fit even with tiles as tall as the grid (128^3 x 64, 256^3 x 64 and 200 x 200 x 160 x 48
  * fit; 128^3 x 192 and wider do not) is refused with WRI_ERR_SCRATCH_LIMIT before anything is
  * launched or written.  The call does no cudaMalloc / cudaFree and calls no
- * allocating library routine; it needs no wri_set_workspace.  Nothing in the scratch has to start at
+ * allocating library routine; it needs no wri_set_workspace.  Like every entry it must be called with
+ * the context's GPU current: the array's device address is looked up for the current device
+ * (cudaGetSymbolAddress, once per device).  As in wri_objective_gradient, the per-column tables (omega^2,
+ * lambda, source cells; a few KB) go host -> device by cudaMemcpyAsync into buffers the context already
+ * owns, so the call itself is not capturable into a CUDA graph as it stands.  Nothing in the scratch has to start at
  * zero (every entry that is read is written first by the same call).  ALL calls on one GPU share the
  * array, whatever their context or stream: calls that can overlap on the GPU (different streams,
  * different contexts, different host threads without ordering) race on it and return garbage sums —
