@@ -209,6 +209,8 @@ GradTiling make_grad_tiling(const wri_ctx* c, int nb) {
 // Caller's workspace.  Vector regions hold n_g x even(nb) complex64 each: U, V, W always (an odd nb: one
 // or two more); with WS_COMPACTION up to nine (the working set of an adaptive solve keeps X in the workspace and has a
 // second vector set to re-pack into), with WS_HOST_STAGING the device copy of x for the host entry.
+int grad_chunk_for(const wri_ctx* c, int nb);   // column chunk of the gradient pass (below)
+
 struct WsLayout {
     size_t vecs[9], U_bot, partials, partials_rt, gscratch, Xs, Ds, tols, res, its, alphas, U_bot2, total;
     int n_vecs;
@@ -228,7 +230,9 @@ WsLayout ws_layout(const wri_ctx* c, int nb, int flags, int maxit_cap) {
     L.partials = o;
     o += align_up((std::max(t.n_tiles, gt.ok ? gt.t.n_tiles : 0) + kInitRowBlocks) * nbe * sizeof(double), 256);
     L.partials_rt = o; o += align_up((size_t)kMaxCtas * nbe * sizeof(double), 256);
-    L.gscratch = o; o += align_up(c->ng * sizeof(float), 256);       // one batch's gradient (pass kernel)
+    // one batch's gradient from the pass kernel, one array per column chunk
+    const int gcb = grad_chunk_for(c, nb);
+    L.gscratch = o; o += align_up(c->ng * sizeof(float), 256) * (size_t)(gcb ? nb / gcb : 1);
     if (flags & WS_HOST_STAGING) {
         L.Xs = o; o += vec;
         L.Ds = o; o += bot;
@@ -444,6 +448,18 @@ int rt_chunk_for(const wri_ctx* c, int nb) {
     return 0;
 }
 
+// Column chunk of the gradient pass (MODE_G): its per-cell sum over the columns runs on warp shuffles and
+// wants a power-of-two chunk.  The width itself when it is one (4 ... 64 columns), else the largest power of
+// two that divides it (48 -> 3 x 16, 192 -> 3 x 64, 24 -> 3 x 8), each chunk with a gradient scratch of its
+// own; 0 = generic kernel (odd widths, chunks below 8 columns: the scratch would pass 1/16 of a vector).
+int grad_chunk_for(const wri_ctx* c, int nb) {
+    if (!rt_chunk_for(c, nb)) return 0;
+    int cb = 1;
+    while (cb < RT_MAXW && nb % (2 * cb) == 0) cb *= 2;
+    if (cb == nb) return nb >= 4 ? cb : 0;
+    return cb >= 8 ? cb : 0;
+}
+
 // planes per tile and tile count of one pass.  With plenty of tiles the measured preferences hold
 // (profiles/r02_width_sweeps.md; an L2 effect: short tiles keep the halo that neighbouring tiles share
 // resident across a wave of tiles): pass F 16 planes; pass A 16 planes up to 24 columns and on grids of
@@ -475,10 +491,10 @@ PassGeo plan_pass(const wri_ctx* c, const DevPlan& P, bool is_f, int zc_forced) 
 // the stencil input the tiles pull through L2 (halo included) plus the issue slots of the 512
 // consumer threads (idle ones included), with a penalty for tile rows below 512 contiguous bytes
 // and a small one for shapes whose model tile cannot ride in the TMA stage.
-int make_plan(const wri_ctx* c, int nb, DevPlan& P) {
+int make_plan(const wri_ctx* c, int nb, DevPlan& P, int cb_forced = 0) {
     std::memset(&P, 0, sizeof P);
-    const int cb = rt_chunk_for(c, nb);
-    if (!cb) return WRI_ERR_ARG;
+    const int cb = cb_forced > 0 ? cb_forced : rt_chunk_for(c, nb);
+    if (!cb || nb % cb) return WRI_ERR_ARG;
     P.nb = nb; P.cb = cb; P.hp = cb / 2; P.nchunk = nb / cb;
     const int maxcells = RT_NT / P.hp;
     const int nx = c->g.nx, ny = c->g.ny;
@@ -811,8 +827,9 @@ struct StaticLaunch {
     size_t smem;
     int grid;
 };
-int static_plan(wri_ctx* c, int nb, const void* in, const void* old, StaticLaunch& S, size_t reserve = 0) {
-    int rc = make_plan(c, nb, S.P);
+int static_plan(wri_ctx* c, int nb, const void* in, const void* old, StaticLaunch& S, size_t reserve = 0,
+                int cb_forced = 0) {
+    int rc = make_plan(c, nb, S.P, cb_forced);
     if (rc) return rc;
     DevPlan& P = S.P;
     // one light stream: long tiles (128 planes: 0.88 -> 0.90 of the copy bandwidth at 128^3 x 64) and the
@@ -1198,10 +1215,10 @@ int wri_objective_gradient(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host
     int n_rows = (int)G.t.n_tiles;
     // pass kernel when the batch is one power-of-two chunk per cell (64 / 32 / 16 / 8 / 4 columns): the
     // per-cell sum over the columns runs on warp shuffles; the generic kernel otherwise
-    const int cb = rt_chunk_for(c, nb);
-    if (cb == nb && nb >= 4 && (nb & (nb - 1)) == 0) {
+    const int cb = grad_chunk_for(c, nb);
+    if (cb) {
         StaticLaunch S;
-        if ((rc = static_plan(c, nb, u_dev, q_dev, S, RT_G_SCRATCH))) return rc;
+        if ((rc = static_plan(c, nb, u_dev, q_dev, S, RT_G_SCRATCH, cb))) return rc;
         float* g_scr = g_dev ? (float*)(c->ws + L.gscratch) : nullptr;
         RtParams p{};
         p.sgn = 1.f; p.phase = -1;
@@ -1213,7 +1230,7 @@ int wri_objective_gradient(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host
         p.lam2 = lambda * lambda;
         if ((rc = launch_static<MODE_G>(c, S, p))) return rc;
         if (g_dev) {
-            k_add_f32<<<blocks_for((long long)c->ng), 256, 0, c->stream>>>(g_dev, g_scr, (long long)c->ng);
+            k_add_f32<<<blocks_for((long long)c->ng), 256, 0, c->stream>>>(g_dev, g_scr, (long long)c->ng, nb / cb);
             c->launches++;
             CK(cudaGetLastError());
         }

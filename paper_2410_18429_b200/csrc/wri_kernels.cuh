@@ -1083,11 +1083,15 @@ __global__ void k_model_step(float* __restrict__ m_trial, const float* __restric
         m_trial[i] = fminf(fmaxf(fmaf(-step, g[i], m[i]), m_min), m_max);
 }
 
-// g += t  (the batch's gradient from the TMA pass into the caller's accumulated gradient)
-__global__ void k_add_f32(float* __restrict__ g, const float* __restrict__ t, long long n) {
+// g += t[0] + t[1] + ...  (the batch's gradient from the pass kernel, one array per column chunk, added
+// in chunk order into the caller's accumulated gradient)
+__global__ void k_add_f32(float* __restrict__ g, const float* __restrict__ t, long long n, int nchunk) {
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
-         i += (long long)gridDim.x * blockDim.x)
-        g[i] += t[i];
+         i += (long long)gridDim.x * blockDim.x) {
+        float a = t[i];
+        for (int k = 1; k < nchunk; ++k) a += t[(size_t)k * n + i];
+        g[i] += a;
+    }
 }
 
 // f_pde[s] = 1/2 lambda^2 sum_tiles partials[.][s];  f_data[s] = 1/2 sum_r |u[rec_r][s] - d[r][s]|^2

@@ -508,6 +508,8 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
             const size_t n_g = (size_t)p.nx * p.ny * p.nz;
             int gsrc0 = -1, gsrc1 = -1;
             float2 gal0 = make_float2(0.f, 0.f), gal1 = gal0;
+            // MODE_G: each column chunk has a gradient scratch of its own (the host adds them in chunk order)
+            float* const gq = (MODE == MODE_G && p.g) ? p.g + (size_t)chunk * n_g : nullptr;
             if (MODE == MODE_G && p.gsrc) {
                 gsrc0 = p.gsrc[col]; gsrc1 = p.gsrc[col + 1];
                 gal0 = p.galpha[col]; gal1 = p.galpha[col + 1];
@@ -623,13 +625,13 @@ k_pass_rt(const __grid_constant__ CUtensorMap pm_in, const __grid_constant__ CUt
                                 const int pl = lane >> 3, cw = ((lane & 7) << 2) >> lhp;
                                 // cell of (first plane of the block, cell cw of this warp) from a lane that owns it
                                 const int c0 = __shfl_sync(0xffffffffu, valid ? cell - slot * plane_m : -1, cw << lhp);
-                                if ((lane & (qpc - 1)) == 0 && pl <= slot && c0 >= 0) p.g[c0 + pl * plane_m] = p.lam2 * sum;
+                                if ((lane & (qpc - 1)) == 0 && pl <= slot && c0 >= 0) gq[c0 + pl * plane_m] = p.lam2 * sum;
                                 __syncwarp();
                             }
                         } else if (p.g) {
                             for (int dlt = hp >> 1; dlt > 0; dlt >>= 1)
                                 gterm += __shfl_down_sync(0xffffffffu, gterm, dlt, hp);
-                            if (cp == 0 && valid) p.g[cell] = p.lam2 * gterm;
+                            if (cp == 0 && valid) gq[cell] = p.lam2 * gterm;
                         }
                     } else {
                         float4 rr;

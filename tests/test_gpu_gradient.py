@@ -47,10 +47,15 @@ CASES = [
     ("config2", dict(grid=(20, 33, 18), nb=3), "sf"),        # 3 threads per cell: shared-memory reduction
     ("config2", dict(grid=(24, 17, 40), nb=5), "q"),
     ("config1", dict(grid=(32, 32, 32), nb=16), "sf"),       # shuffle reduction, width 8
-    ("config3", dict(grid=(27, 25, 20), nb=48), "both"),     # 24 threads per cell
+    ("config3", dict(grid=(27, 25, 20), nb=48), "both"),     # pass kernel, 3 chunks of 16 columns
     ("config2", dict(grid=(21, 18, 37), nb=64), "sf"),       # one warp per cell, three frequencies
     ("config4", dict(grid=(19, 22, 35), nb=32), "q"),
-    ("config2", dict(grid=(12, 14, 10), nb=192), "sf"),      # 96 threads per cell
+    ("config2", dict(grid=(12, 14, 10), nb=192), "sf"),      # pass kernel, 3 chunks of 64 columns
+    ("config3", dict(grid=(30, 26, 22), nb=24), "sf"),       # 3 chunks of 8 (four lanes per cell, no shuffle step)
+    ("config3", dict(grid=(22, 19, 24), nb=40), "both"),     # 5 chunks of 8
+    ("config2", dict(grid=(16, 12, 18), nb=128), "q"),       # 2 chunks of 64
+    ("config3", dict(grid=(20, 23, 17), nb=12), "sf"),       # chunk of 4 would be too narrow: generic, 6 threads per cell
+    ("config3", dict(grid=(18, 20, 16), nb=44), "both"),     # likewise (4 x 11): generic, 22 threads per cell
 ]
 
 
@@ -90,6 +95,32 @@ def test_objective_and_gradient_match_oracle(torch_cuda, name, kw, mode):
     kwargs["g"] = None
     fp3, _ = ctx.objective_gradient(ud, dd, w.lam, **kwargs)
     assert np.array_equal(fp3.cpu().numpy(), fp.cpu().numpy())
+
+
+@pytest.mark.parametrize("nb", [16, 48, 192])
+def test_pass_kernel_and_generic_kernel_agree(torch_cuda, nb):
+    """The same evaluation through the pass kernel (one chunk, 3 x 16, 3 x 64) and through the generic
+    kernel (debug option): objective to fp64 rounding of a differently grouped sum, gradient to 1e-5."""
+    torch = torch_cuda
+    w = workloads.make("config2", grid=(20, 18, 24), nb=nb)
+    ctx = _wri(w)
+    rng = np.random.Generator(np.random.PCG64(31))
+    u = torch.from_numpy(_cn(rng, (w.ng, w.nb))).cuda()
+    al = torch.from_numpy(_cn(rng, (w.nb,))).cuda()
+    d = torch.from_numpy(w.D).cuda()
+    out = []
+    for generic in (0, 1):
+        ctx.set_debug_opts(generic=generic)
+        g = torch.zeros(w.ng, dtype=torch.float32, device="cuda")
+        n0 = ctx.launch_count()
+        fp, fd = ctx.objective_gradient(u, d, w.lam, omega_idx=w.omega_idx, src_ijk=w.src_ijk, alpha=al, g=g)
+        torch.cuda.synchronize()
+        out.append((fp.cpu().numpy(), fd.cpu().numpy(), g.cpu().numpy(), ctx.launch_count() - n0))
+    (fp0, fd0, g0, l0), (fp1, fd1, g1, l1) = out
+    assert (l0, l1) == (3, 2)                        # pass kernel + k_add_f32 + k_objective | k_grad + k_objective
+    assert np.allclose(fp0, fp1, rtol=1e-6) and np.array_equal(fd0, fd1)
+    assert rel(g0, g1) < 1e-5
+    ctx.close()
 
 
 def test_objective_equals_half_squared_residual_of_the_solve(torch_cuda):
