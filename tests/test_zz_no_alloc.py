@@ -135,6 +135,42 @@ def test_static_scratch_entry_with_the_27_point_stencil_and_a_receiver_mask(torc
         c.close()
 
 
+@pytest.mark.parametrize("grid,nb", [((128, 128, 128), 64),      # the headline size: 4096 tiles x 64 columns, half the array
+                                     ((24, 24, 256), 512)])      # 4608 tiles x 512 columns at the usual tile height:
+def test_static_scratch_entry_at_sizes_near_its_limit(torch_cuda, grid, nb):   # fits only with tiles as tall as the grid
+    """Sizes the header names as fitting: the result equals the workspace path's (1e-5) and, for the tall
+    grid, the entry gets there by making its tiles taller (the default tiling would need 18.9 MB of sums)."""
+    torch = torch_cuda
+    from paper_2410_18429_b200 import Wri
+    w = workloads.make("config2", grid=grid, nb=4)
+    rng = np.random.Generator(np.random.PCG64(17))
+    gen = torch.Generator(device="cuda").manual_seed(5)
+    u = torch.view_as_complex(torch.randn((w.ng, nb, 2), dtype=torch.float32, device="cuda", generator=gen))
+    d = torch.view_as_complex(torch.randn((w.n_rec, nb, 2), dtype=torch.float32, device="cuda", generator=gen))
+    al = torch.view_as_complex(torch.randn((nb, 2), dtype=torch.float32, device="cuda", generator=gen))
+    idx = rng.integers(0, len(w.omegas), nb).astype(np.int32)
+    src = np.stack([rng.integers(2, w.nx - 2, nb), rng.integers(2, w.ny - 2, nb), rng.integers(2, w.nz - 2, nb)],
+                   axis=1).astype(np.int32)
+    ref_ctx = Wri.from_workload(w, nb_max=nb)
+    g_ref = torch.zeros(w.ng, dtype=torch.float32, device="cuda")
+    fp, fd = ref_ctx.objective_gradient(u, d, w.lam, omega_idx=idx, src_ijk=src, alpha=al, g=g_ref)
+    ctx = Wri.from_workload(w, nb_max=nb)
+    f_pde = torch.empty(nb, dtype=torch.float64, device="cuda")
+    f_data = torch.empty(nb, dtype=torch.float64, device="cuda")
+    g = torch.zeros(w.ng, dtype=torch.float32, device="cuda")
+    try:
+        for _ in range(2):                   # two calls in a row on the shared array
+            g.zero_()
+            ctx.objective_gradient_static(u, d, w.lam, f_pde, f_data, omega_idx=idx, src_ijk=src, alpha=al, g=g)
+            torch.cuda.synchronize()
+            assert float(((f_pde - fp).abs() / fp.abs()).max()) < TOL
+            assert float(((f_data - fd).abs() / fd.abs()).max()) < TOL
+            assert float((g - g_ref).norm() / g_ref.norm()) < TOL
+    finally:
+        ref_ctx.close()
+        ctx.close()
+
+
 def test_static_scratch_entry_refuses_sizes_beyond_its_array(torch_cuda):
     """48 x 48 x 16 x 300 columns: one cell per thread-block row, so 48 x 48 tiles x 300 doubles = 5.5 MB
     of sums even with tiles as tall as the grid -> WRI_ERR_SCRATCH_LIMIT with a message that names the
