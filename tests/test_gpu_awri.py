@@ -241,6 +241,7 @@ def test_awri_step_builtin_update_and_errors(torch_cuda):
 @pytest.mark.parametrize("name,kw", [
     ("config2", dict(grid=(32, 28, 24), nb=64)),       # TMA path, compaction of the shrinking batch
     ("config3", dict(grid=(40, 40, 32), nb=16)),
+    ("config3", dict(grid=(36, 32, 28), nb=48)),       # configs[3]'s width: the gradient pass runs as 3 chunks of 16
 ])
 def test_misfit_on_the_tma_path_with_compaction(torch_cuda, name, kw):
     """Workload-shaped groups at TMA widths: the columns stop at different iterations, the batch is

@@ -183,6 +183,7 @@ def test_adaptive_solve_27_does_not_depend_on_the_repacking(torch_cuda):
 
 
 @pytest.mark.parametrize("name,kw", [("config1", dict(grid=(24, 20, 28), nb=16)),     # pass kernel (MODE_G)
+                                      ("config3", dict(grid=(27, 25, 20), nb=48)),     # pass kernel, 3 chunks of 16
                                       ("config2", dict(grid=(20, 33, 18), nb=5))])     # generic k_grad
 def test_objective_and_gradient_27(torch_cuda, name, kw):
     """eq. 4 and eq. 9 with the 27-point A: f_pde, f_data per column and the group gradient, 1e-5."""
