@@ -1,11 +1,13 @@
 /* abi_demo.c — libwri through its C ABI alone (include/wri.h): plain C99, the CUDA runtime for device
- * memory, no Python and no torch.  Reads one problem from a binary file, runs wri_apply_M and
- * wri_lsqr_batch, writes the results to another file; tests/test_gpu_c_abi.py generates the inputs,
- * builds and runs this program and compares the results with the CPU oracle.
+ * memory, no Python and no torch.  Reads one problem from a binary file, runs wri_apply_M,
+ * wri_lsqr_batch and wri_objective_gradient_static, writes the results to another file;
+ * tests/test_gpu_c_abi.py generates the inputs, builds and runs this program and compares the results
+ * with the CPU oracle.
  *
  * input  : int32 nx ny nz nb n_rec L maxit n_omega | double h lambda | double omega[n_omega]
  *          | int32 omega_idx[nb] | int32 rec_ijk[n_rec][3] | float m[n_g] | c64 q[n_g][nb] | c64 d[n_rec][nb]
  * output : c64 ytop[n_g][nb] | c64 ybot[n_rec][nb] | c64 u[n_g][nb] | float resnorms[maxit+1][nb] | int32 iters[nb]
+ *          | double f_pde[nb] | double f_data[nb] | float g[n_g]
  */
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -80,6 +82,21 @@ int main(int argc, char** argv) {
     if (wri_lsqr_batch(ctx, nb, oi, q_dev, d_dev, (float)hl[1], NULL, maxit, u_dev, res_dev, it_dev) != WRI_ERR_WORKSPACE)
         return 4;
 
+    /* objective and gradient at the solve's u through the entry that needs neither a workspace (the
+     * 16-byte one is still set) nor any device allocation of its own: outputs allocated here, before */
+    double *fp_dev = NULL, *fd_dev = NULL;
+    float* g_dev = NULL;
+    CU(cudaMalloc((void**)&fp_dev, nb * sizeof(double))); CU(cudaMalloc((void**)&fd_dev, nb * sizeof(double)));
+    CU(cudaMalloc((void**)&g_dev, ng * sizeof(float)));
+    CU(cudaMemset(g_dev, 0, ng * sizeof(float)));
+    CHECK(wri_objective_gradient_static(ctx, nb, oi, NULL, NULL, q_dev, u_dev, d_dev, (float)hl[1], fp_dev, fd_dev, g_dev));
+    CU(cudaDeviceSynchronize());
+    double *fp = malloc(nb * sizeof(double)), *fd = malloc(nb * sizeof(double));
+    float* g = malloc(ng * sizeof(float));
+    CU(cudaMemcpy(fp, fp_dev, nb * sizeof(double), cudaMemcpyDeviceToHost));
+    CU(cudaMemcpy(fd, fd_dev, nb * sizeof(double), cudaMemcpyDeviceToHost));
+    CU(cudaMemcpy(g, g_dev, ng * sizeof(float), cudaMemcpyDeviceToHost));
+
     void *ytop = malloc(vb), *ybot = malloc(db), *u = malloc(vb);
     float* res = malloc((size_t)(maxit + 1) * nb * sizeof(float));
     int32_t* it = malloc(nb * sizeof(int32_t));
@@ -92,6 +109,7 @@ int main(int argc, char** argv) {
     if (!f) return 1;
     fwrite(ytop, 1, vb, f); fwrite(ybot, 1, db, f); fwrite(u, 1, vb, f);
     fwrite(res, sizeof(float), (size_t)(maxit + 1) * nb, f); fwrite(it, sizeof(int32_t), nb, f);
+    fwrite(fp, sizeof(double), nb, f); fwrite(fd, sizeof(double), nb, f); fwrite(g, sizeof(float), ng, f);
     fclose(f);
     printf("launches %lld\n", (long long)wri_launch_count(ctx));
     CHECK(wri_destroy(ctx));

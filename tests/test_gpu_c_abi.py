@@ -49,7 +49,11 @@ def test_c_program_through_the_abi(tmp_path):
     ybot = raw[o:o + nd * 8].view(np.complex64).reshape(w.n_rec, w.nb); o += nd * 8
     u = raw[o:o + nv * 8].view(np.complex64).reshape(w.ng, w.nb); o += nv * 8
     res = raw[o:o + (K + 1) * w.nb * 4].view(np.float32).reshape(K + 1, w.nb); o += (K + 1) * w.nb * 4
-    it = raw[o:o + w.nb * 4].view(np.int32)
+    it = raw[o:o + w.nb * 4].view(np.int32); o += w.nb * 4
+    f_pde = raw[o:o + w.nb * 8].view(np.float64); o += w.nb * 8
+    f_data = raw[o:o + w.nb * 8].view(np.float64); o += w.nb * 8
+    g = raw[o:o + w.ng * 4].view(np.float32); o += w.ng * 4
+    assert o == raw.size
     rec = O.rec_cells(w.nx, w.ny, w.nz, w.rec_ijk)
     ops = ops_for(w)
     assert np.array_equal(ybot, w.Q[rec, :])
@@ -59,3 +63,10 @@ def test_c_program_through_the_abi(tmp_path):
         assert rel(ytop[:, s], rt) < 1e-5
         ref = O.lsqr(ops[s], w.m, w.lam, rec, w.Q[:, s], w.D[:, s], tol=0.0, maxit=K)
         assert rel(res[:, s], ref["resnorms"]) < 1e-3 and rel(u[:, s], ref["x"]) < 1e-3
+    # eq. 4 / eq. 9 at the program's own u, from the entry that allocates nothing (scratch in the library image)
+    gsum = np.zeros(w.ng)
+    for s in range(w.nb):
+        fp, fd = O.objective_gradient(ops[s], w.m.astype(np.float64), w.lam, rec, u[:, s].astype(complex), w.D[:, s],
+                                      q=w.Q[:, s].astype(complex), g=gsum)
+        assert f_pde[s] == pytest.approx(fp, rel=1e-5) and f_data[s] == pytest.approx(fd, rel=1e-5), s
+    assert rel(g, gsum) < 1e-5
