@@ -114,8 +114,9 @@ int wri_set_debug_opts(wri_ctx* ctx, const wri_debug_opts* opts);
  * WRI_ERR_ARG when the width is served by the generic kernels (odd widths).                        */
 int wri_plan_info(wri_ctx* ctx, int32_t nb, int32_t* out16);
 
-/* Workspace for wri_lsqr_* at batch width nb (u, v, w vectors, receiver rows, reduction
- * partials).  flags: WRI_WS_HOST_STAGING adds room for the device copies wri_lsqr_batch_host
+/* Workspace for wri_lsqr_* and wri_objective_gradient at batch width nb (u, v, w vectors, receiver
+ * rows, reduction partials, one float32 [n_g] gradient scratch per power-of-two column chunk of the
+ * gradient pass: 1 for 64 columns, 3 for 48 or 192).  flags: WRI_WS_HOST_STAGING adds room for the device copies wri_lsqr_batch_host
  * needs; WRI_WS_COMPACTION adds six more vectors: with per-column tolerances the working set then
  * lives entirely in the workspace, has a second vector set and a side buffer, so that converged columns can be
  * compacted out of it on the device (without it such a solve still stops early once every column
