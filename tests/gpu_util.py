@@ -5,9 +5,10 @@ import numpy as np
 from oracle import oracle as O
 
 
-def ops_for(w):
-    """One oracle Operator per batch column of a workload."""
-    return [O.Operator(w.nx, w.ny, w.nz, w.h, w.omegas[j], w.sponge_width, w.gamma_max, w.power, w.faces)
+def ops_for(w, stencil=0):
+    """One oracle Operator per batch column of a workload (stencil: 0 = 7-point, 1 = 27-point)."""
+    return [O.Operator(w.nx, w.ny, w.nz, w.h, w.omegas[j], w.sponge_width, w.gamma_max, w.power, w.faces,
+                       stencil=stencil)
             for j in w.omega_idx]
 
 

@@ -40,18 +40,19 @@ def _true_residual_norms(torch, ctx, w, q, d, u):
     return n2.sqrt().cpu().numpy()
 
 
-def _check_operator_columns(torch, ctx, w, x, cols, rec):
+def _check_operator_columns(torch, ctx, w, x, cols, rec, stencil=0):
     top, bot = ctx.apply_M(x, w.lam, w.omega_idx)
     xh = x.cpu().numpy()
     assert np.array_equal(bot.cpu().numpy(), xh[rec, :])          # P: bit-exact indexing
-    ops = ops_for(w)
+    ops = ops_for(w, stencil)
     for s in cols:
         rt, _ = O.apply_M(ops[s], w.m, w.lam, rec, xh[:, s])
         assert rel(top[:, s].cpu().numpy(), rt) < 1e-5, s
 
 
-def _fixed_k_case(torch, w, K, cols, threads):
+def _fixed_k_case(torch, w, K, cols, threads, stencil=0):
     ctx = _wri(w)
+    ctx.set_stencil(stencil)
     rec = O.rec_cells(w.nx, w.ny, w.nz, w.rec_ijk)
     q, d = torch.from_numpy(w.Q).cuda(), torch.from_numpy(w.D).cuda()
     u, res, it = ctx.lsqr_batch(q, d, w.lam, None, maxit=K, omega_idx=w.omega_idx)
@@ -64,8 +65,8 @@ def _fixed_k_case(torch, w, K, cols, threads):
     r_true = _true_residual_norms(torch, ctx, w, q, d, u)
     assert np.max(np.abs(resh[K] / r_true - 1.0)) < 1e-3
     # the operator entry used above, and the solve itself, against the oracle on sampled columns
-    _check_operator_columns(torch, ctx, w, u, cols[:2], rec)
-    ref = O.lsqr_batch(ops_for(w), w.m, w.lam, rec, w.Q, w.D, None, maxit=K, threads=threads, columns=cols)
+    _check_operator_columns(torch, ctx, w, u, cols[:2], rec, stencil)
+    ref = O.lsqr_batch(ops_for(w, stencil), w.m, w.lam, rec, w.Q, w.D, None, maxit=K, threads=threads, columns=cols)
     for j, s in enumerate(cols):
         assert rel(resh[:, s], ref["resnorms"][:, j]) < 1e-3, s
         assert rel(u[:, s].cpu().numpy(), ref["x"][:, j]) < 1e-3, s
@@ -83,6 +84,13 @@ def test_config2_128cubed_x64src_50_iterations(torch_cuda):
     w = workloads.make("config2", freqs=(6.0,))
     assert (w.nx, w.ny, w.nz, w.nb, w.n_rec) == (128, 128, 128, 64, 1024)
     _fixed_k_case(torch_cuda, w, 50, [0, 31, 63], threads=3)
+
+
+def test_config2_128cubed_x64src_27_point_stencil(torch_cuda):
+    """The headline workload with the 27-point discretisation (reading C-23), the configuration
+    `bench.py --stencil 27` times: 50 iterations, columns 0 and 63 against the oracle's 27-point operator."""
+    w = workloads.make("config2", freqs=(6.0,))
+    _fixed_k_case(torch_cuda, w, 50, [0, 63], threads=2, stencil=1)
 
 
 def test_config2_128cubed_x192col_three_frequencies(torch_cuda):
