@@ -252,3 +252,40 @@ def test_config2_128cubed_x64src_source_free_and_misfit(torch_cuda):
         assert f_cols[s] == pytest.approx(0.5 * r["resnorms"][r["iters"]] ** 2, rel=5e-3), s
         assert ar0[s] == pytest.approx(r["arnorms"][0], rel=1e-5), s
     ctx.close()
+
+
+def test_config3_vsp_objective_and_gradient_full_size(torch_cuda):
+    """configs[3]'s grid and width (200 x 200 x 160, 48 columns: the gradient pass runs as three chunks of
+    16 columns) through eq. 4 / eq. 9 at a random wavefield with a known source q and a source weight on
+    top: f_pde, f_data of every column and the group gradient against the oracle, 1e-5."""
+    torch = torch_cuda
+    from concurrent.futures import ThreadPoolExecutor
+    w = workloads.make("config3")
+    assert (w.nx, w.ny, w.nz, w.nb) == (200, 200, 160, 48)
+    ctx = _wri(w)
+    rec = O.rec_cells(w.nx, w.ny, w.nz, w.rec_ijk)
+    srcc = O.rec_cells(w.nx, w.ny, w.nz, w.src_ijk)
+    ops = ops_for(w)
+    gen = torch.Generator(device="cuda").manual_seed(11)
+    u = torch.view_as_complex(torch.randn((w.ng, w.nb, 2), dtype=torch.float32, device="cuda", generator=gen))
+    al = torch.view_as_complex(torch.randn((w.nb, 2), dtype=torch.float32, device="cuda", generator=gen))
+    q, d = torch.from_numpy(w.Q).cuda(), torch.from_numpy(w.D).cuda()
+    g = torch.zeros(w.ng, dtype=torch.float32, device="cuda")
+    fp, fd = ctx.objective_gradient(u, d, w.lam, omega_idx=w.omega_idx, q=q, src_ijk=w.src_ijk, alpha=al, g=g)
+    torch.cuda.synchronize()
+    fp, fd, uh, alh = fp.cpu().numpy(), fd.cpu().numpy(), u.cpu().numpy(), al.cpu().numpy()
+    m64 = w.m.astype(np.float64)
+
+    def one(s):
+        gs = np.zeros(w.ng)
+        a, b = O.objective_gradient(ops[s], m64, w.lam, rec, uh[:, s].astype(complex), w.D[:, s],
+                                    q=w.Q[:, s].astype(complex), src=int(srcc[s]), alpha_src=complex(alh[s]), g=gs)
+        return s, a, b, gs
+
+    gsum = np.zeros(w.ng)
+    with ThreadPoolExecutor(8) as ex:
+        for s, a, b, gs in ex.map(one, range(w.nb)):
+            assert fp[s] == pytest.approx(a, rel=1e-5) and fd[s] == pytest.approx(b, rel=1e-5), s
+            gsum += gs
+    assert rel(g.cpu().numpy(), gsum) < 1e-5
+    ctx.close()
