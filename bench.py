@@ -412,6 +412,8 @@ def run_ours(args, wl_name, w):
                                         "frac": bytes_g / (ms_g * 1e-3) / 1e9 / peak_g,
                                         "bound": "alu", "warp_instructions_per_cell_column": 2.22,
                                         "frac_alu": 2.22 * w.ng * nb / (ms_g * 1e-3) / alu_peak,
+                                        "clock_state": "timed right after the K steps, at the sustained "
+                                                       "(power-capped) SM clock of `clocks`, not at the burst clock",
                                         "kernel": "k_pass_rt<MODE_G> + k_add_f32 + k_objective (eq. 9 fused with "
                                                   "the stencil residual); k_grad at widths the pass kernel "
                                                   "does not take"}
