@@ -284,7 +284,13 @@ int wri_lsqr_set_opts(wri_ctx* ctx, const wri_lsqr_opts* opts);
  *   g_dev      float [n_g], ACCUMULATED (clear it first), or NULL for the objective alone
  *   iters_dev  int32 [nb] or NULL
  *   f_host     HOST double or NULL: sum_s (f_pde + f_data), summed in column order; asking for it
- *              synchronises the stream
+ *              synchronises the stream.  The call then blocks until the result is there anyway, so
+ *              with eps > 0 it enqueues its solve only 16 iterations ahead of the device (which
+ *              reports its progress in a word of mapped host memory) and stops once every column
+ *              has stopped, instead of enqueuing all maxit iterations; same results, and the
+ *              1-3 ms of launches that would each return at once are not paid.  wri_awri_step and
+ *              the host-buffer solves with tolerances (wri_lsqr_batch_host, wri_lsqr_sf_batch_host)
+ *              do the same.  The device-buffer solves enqueue everything and return.
  * Needs a workspace (with WRI_WS_COMPACTION room converged columns are compacted away).
  *
  * wri_awri_step — lines 4-14 of Algorithm 2 for one group of columns and the model in m_dev:

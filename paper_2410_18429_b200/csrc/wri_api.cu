@@ -11,6 +11,8 @@
 #include <cstdlib>
 #include <cstring>
 #include <mutex>
+#include <thread>
+#include <chrono>
 #include <type_traits>
 #include <utility>
 #include <vector>
@@ -86,6 +88,15 @@ struct wri_ctx {
     double* aw_ar0 = nullptr;    // [nb_max] alpha1*beta1 of the cold solve at the current model
     int* aw_iters = nullptr;     // [nb_max]
     double* h_aw = nullptr;      // pinned: [2][nb_max] doubles followed by [nb_max] ints
+    // paced enqueue: an entry that ends with a stream synchronisation anyway (misfit evaluation, Algorithm 2
+    // step, host-buffer solve) enqueues a solve with tolerances a few iterations ahead of the device and
+    // stops once the device reports that every column has stopped — instead of enqueuing all maxit
+    // iterations, whose launches would each return at once but cost about 2 us apiece (1-3 ms per solve).
+    unsigned long long* h_prog = nullptr;   // mapped pinned word written by the finaliser of pass A
+    unsigned long long* d_prog = nullptr;   // its device address
+    unsigned int solve_id = 0;              // tags the word: a late write of an earlier solve is ignored
+    bool pace = false;                      // set by the entries that synchronise at their end
+    bool pacing = false;                    // the solve in flight reports its progress
     // caller's workspace
     char* ws = nullptr;
     size_t ws_bytes = 0;
@@ -697,6 +708,8 @@ ScalParams scal_params(const wri_ctx* c, const double* partials, int n_rows, con
     s.V = c->V; s.U_bot = c->U_bot[0]; s.d = d;
     s.coef = c->coef[0]; s.stat = c->stat[0]; s.active = c->active[0]; s.iters = c->iters[0];
     s.tol = c->tol; s.resnorms = c->resnorms; s.iters_out = c->iters_out;
+    s.progress = c->pacing ? c->d_prog : nullptr;
+    s.solve_id = c->solve_id;
     s.k = c->k; s.maxit = c->maxit; s.lambda = c->lambda;
     s.rows_in_pass = 1;
     s.colmap = c->packed ? c->colmap : nullptr;
@@ -1004,6 +1017,9 @@ int wri_create(wri_ctx** out, wri_grid grid, double h, int32_t n_omega, const do
     CKC(cudaMalloc(&c->aw_ar0, NM * sizeof(double)));
     CKC(cudaMalloc(&c->aw_iters, NM * sizeof(int)));
     CKC(cudaMallocHost(&c->h_aw, (size_t)NM * (2 * sizeof(double) + sizeof(int))));
+    CKC(cudaHostAlloc((void**)&c->h_prog, 64, cudaHostAllocMapped));
+    *c->h_prog = 0;
+    CKC(cudaHostGetDevicePointer((void**)&c->d_prog, c->h_prog, 0));
     CKC(cudaMalloc(&c->counter, sizeof(unsigned int)));
     CKC(cudaMemset(c->counter, 0, sizeof(unsigned int)));
     CKC(cudaMalloc(&c->d_state, sizeof(SolveState)));
@@ -1027,6 +1043,7 @@ int wri_destroy(wri_ctx* c) {
     cudaFree(c->colmap); cudaFree(c->src); cudaFree(c->retired);
     cudaFree(c->aw_tol); cudaFree(c->aw_f); cudaFree(c->aw_ar0); cudaFree(c->aw_iters);
     if (c->h_aw) cudaFreeHost(c->h_aw);
+    if (c->h_prog) cudaFreeHost(c->h_prog);
     cudaFree(c->d_plans); cudaFree(c->d_maps); cudaFree(c->d_mmaps); cudaFree(c->d_own_ptr); cudaFree(c->d_own);
     cudaFree(c->d_state); cudaFree(c->d_prof);
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
@@ -1509,6 +1526,40 @@ int lsqr_begin_impl(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const
     return WRI_OK;
 }
 
+// Enqueue of a solve with tolerances from an entry that synchronises at its end: at most kAhead
+// iterations ahead of the device, and no further once every column has stopped.
+int iterate_paced(wri_ctx* c, int n_steps) {
+    constexpr int kAhead = 16;
+    volatile unsigned long long* prog = c->h_prog;
+    using clock = std::chrono::steady_clock;
+    unsigned long long seen = ~0ull;
+    clock::time_point since = clock::now();
+    for (int i = 0; i < n_steps; ++i) {
+        for (;;) {
+            const unsigned long long w = *prog;
+            const bool mine = (unsigned int)(w >> 32) == c->solve_id;
+            if (mine && (w & 1ull)) return WRI_OK;                    // every column has stopped
+            const int k_dev = mine ? (int)((w & 0xffffffffull) >> 1) : 0;
+            if (c->k - k_dev < kAhead) break;
+            // the word has not moved for a long time: ask the stream whether anything is still in flight
+            // (an error, or a device that cannot reach the word) rather than wait for ever.  Rare on
+            // purpose: a stream query in a tight loop slows the kernels in flight.
+            const clock::time_point now = clock::now();
+            if (w != seen) { seen = w; since = now; }
+            else if (now - since > std::chrono::milliseconds(200)) {
+                const cudaError_t e = cudaStreamQuery(c->stream);
+                if (e == cudaSuccess) break;
+                if (e != cudaErrorNotReady) return cuda_fail(e, "paced enqueue");
+                since = now;
+            }
+            std::this_thread::sleep_for(std::chrono::microseconds(20));
+        }
+        const int rc = wri_lsqr_iterate(c, 1);
+        if (rc) return rc;
+    }
+    return WRI_OK;
+}
+
 // A batch is worked through in groups of at most 64 columns, each in a compact even-width working set
 // of its own inside the workspace; a group that is the whole (even, <= 64 wide) batch works in the
 // caller's own layout.  With several chunks per cell a tile row is a 512-byte piece of a wider cell
@@ -1533,11 +1584,19 @@ int solve_groups(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const vo
     const int gw = split ? RT_MAXW : nb;
     for (int col0 = 0; col0 < nb; col0 += gw) {
         const int ncols = std::min(gw, nb - col0);
+        // (the generic kernels' host-sequenced solve has no device-side stop to report)
+        c->pacing = c->pace && tol_dev && maxit > 0 && rt_chunk_for(c, even_up(split ? ncols : nb)) != 0;
+        if (c->pacing) ++c->solve_id;
         if ((rc = lsqr_begin_impl(c, nb, omega_idx_host, q_dev, d_dev, lambda, tol_dev, maxit, u_out_dev,
                                   resnorms_dev, iters_dev, host_staged, src_ijk_host, alpha_out_dev, col0,
-                                  split ? ncols : 0, true)))
+                                  split ? ncols : 0, true))) {
+            c->pacing = false;
             return rc;
-        if ((rc = wri_lsqr_iterate(c, maxit))) { c->solving = false; return rc; }
+        }
+        if (!c->rt) c->pacing = false;
+        rc = c->pacing ? iterate_paced(c, maxit) : wri_lsqr_iterate(c, maxit);
+        c->pacing = false;
+        if (rc) { c->solving = false; return rc; }
         if ((rc = wri_lsqr_end(c))) return rc;
     }
     return WRI_OK;
@@ -1670,9 +1729,11 @@ int lsqr_batch_host_impl(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, 
     if (Qs) CK(cudaMemcpyAsync(Qs, q_host, vbytes, cudaMemcpyHostToDevice, c->stream));
     if (dbytes) CK(cudaMemcpyAsync(Ds, d_host, dbytes, cudaMemcpyHostToDevice, c->stream));
     if (tol_host) CK(cudaMemcpyAsync(tols, tol_host, nb * sizeof(float), cudaMemcpyHostToDevice, c->stream));
-    if ((rc = solve_groups(c, nb, omega_idx_host, Qs, Ds, lambda, tol_host ? tols : nullptr, maxit, Xs, res, its,
-                           true, src_ijk_host, sf ? As : nullptr)))
-        return rc;
+    c->pace = true;                          // this entry synchronises at its end
+    rc = solve_groups(c, nb, omega_idx_host, Qs, Ds, lambda, tol_host ? tols : nullptr, maxit, Xs, res, its,
+                      true, src_ijk_host, sf ? As : nullptr);
+    c->pace = false;
+    if (rc) return rc;
     CK(cudaMemcpyAsync(u_out_host, Xs, vbytes, cudaMemcpyDeviceToHost, c->stream));
     CK(cudaMemcpyAsync(resnorms_host, res, (size_t)(maxit + 1) * nb * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
     if (iters_host) CK(cudaMemcpyAsync(iters_host, its, nb * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
@@ -1884,8 +1945,10 @@ int misfit_impl(wri_ctx* c, int32_t nb, const int32_t* omega_idx_host, const int
     c->opts = wri_lsqr_opts{};
     if (warm) { c->opts.warm_start = 1; c->opts.ar_ref_dev = ar0_dev; }
     else c->opts.ar0_out_dev = ar0_dev;
+    c->pace = f_host || iters_host;         // the call synchronises at its end: enqueue a little ahead only
     rc = wri_lsqr_sf_batch(c, nb, omega_idx_host, src_ijk_host, nullptr, d_dev, lambda,
                            eps > 0.f ? c->aw_tol : nullptr, maxit, u_dev, alpha_dev, nullptr, its);
+    c->pace = false;
     c->opts = saved;
     if (rc) return rc;
     if ((rc = wri_objective_gradient(c, nb, omega_idx_host, src_ijk_host, alpha_dev, nullptr, u_dev, d_dev,

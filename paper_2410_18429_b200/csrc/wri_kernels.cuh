@@ -364,6 +364,10 @@ struct ScalParams {
     const float* tol;         // [nb] or null
     float* resnorms;          // [maxit+1][nb]
     int* iters_out;           // [nb] or null
+    // paced enqueue (entries that end with a stream synchronisation): the finaliser of pass A reports
+    // (solve id, iteration, every column stopped) in one 8-byte word of mapped host memory; null otherwise
+    unsigned long long* progress;
+    unsigned int solve_id;
     int k;                    // iteration number (PH_A), for resnorms / iters
     int maxit;
     float lambda;
@@ -682,6 +686,11 @@ __device__ __forceinline__ void finalize_phase(const ScalParams& p, double* sh) 
         for (int s = 0; s < nb; ++s) n_act += p.active[s] != 0;
         st->k = p.k;
         st->n_active = n_act;
+        if (p.progress) {
+            *p.progress = ((unsigned long long)p.solve_id << 32) | ((unsigned long long)(unsigned)p.k << 1) |
+                          (n_act == 0 ? 1ull : 0ull);
+            __threadfence_system();
+        }
         if (n_act == 0) st->all_done = 1;
         else if (p.adaptive && !p.trans) {
             const int w_new = max(2, (n_act + 1) & ~1);

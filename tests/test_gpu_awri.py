@@ -366,3 +366,48 @@ def test_sharded_evaluator_cuts_the_receiver_mask_per_rank(torch_cuda):
         f_ref += 0.5 * r["resnorms"][r["iters"]] ** 2
     assert f_blocks == pytest.approx(f_ref, rel=1e-4)
     assert float(g_sum.abs().max()) > 0
+
+
+def test_paced_enqueue_of_a_synchronising_evaluation(torch_cuda):
+    """wri_misfit_sf with a host result synchronises at its end, so it enqueues its solve a few iterations
+    ahead of the device and stops once the device reports that every column has stopped (instead of all
+    maxit iterations, whose launches would each return at once).  Same results, bit for bit, as the
+    evaluation that enqueues everything (want_f=False: nothing synchronises); far fewer launches; and the
+    working set still shrinks on the way (the re-packing decision is taken on the device either way)."""
+    torch = torch_cuda
+    import workloads
+    from paper_2410_18429_b200 import Wri
+    w = workloads.make("config3", grid=(40, 40, 32), nb=16)
+    ctx = Wri.from_workload(w)
+    d = torch.from_numpy(w.D).cuda()
+    eps, maxit = 5e-3, 400
+    outs, launches, cols = [], [], []
+    ctx.profile_enable(True)
+    for want_f in (False, True):
+        g = torch.zeros(ctx.ng, dtype=torch.float32, device="cuda")
+        ctx.profile_read()
+        n0 = ctx.launch_count()
+        out = ctx.misfit_sf(d, w.lam, w.src_ijk, eps, maxit, omega_idx=w.omega_idx, g=g, want_f=want_f)
+        torch.cuda.synchronize()
+        launches.append(ctx.launch_count() - n0)
+        _, n_f, cols_f, _, n_a, cols_a = ctx.profile_read()
+        cols.append((n_f, cols_f, n_a, cols_a))
+        outs.append((out, g))
+    ctx.profile_enable(False)
+    (a, ga), (b, gb) = outs
+    it = a["iters"].cpu().numpy()
+    assert it.max() < maxit // 2 and len(set(it.tolist())) > 2          # early, spread stops
+    for key in ("u", "alpha"):
+        assert torch.equal(torch.view_as_real(a[key]), torch.view_as_real(b[key])), key
+    for key in ("f_pde", "f_data", "iters", "ar0"):
+        assert torch.equal(a[key], b[key]), key
+    assert torch.equal(ga, gb)
+    # everything enqueued: at least 2 launches per iteration; paced: about 16 iterations past the last stop
+    assert launches[0] >= 2 * maxit
+    assert launches[1] <= 4 * (int(it.max()) + 16) + 16, launches
+    # the launches that did work are the same in both, and the working set shrank (fewer column-launches
+    # than launches x 16 columns)
+    assert cols[0] == cols[1]
+    n_f, cols_f, _, _ = cols[1]
+    assert cols_f < n_f * w.nb
+    ctx.close()
